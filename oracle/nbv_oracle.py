@@ -1,0 +1,323 @@
+"""CPU oracle, Python side.  TEST INFRASTRUCTURE -- see the header of nbv_oracle.cpp.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl
+reference` legs may import this.  It imports nothing from
+paper_2602_08266_b200: inputs arrive as plain numpy arrays.
+
+C++ part (nbv_oracle.cpp, via ctypes): activation, projection, depth order, tile
+lists, per-pixel compositing, analytic Jacobian rows and J^T J blocks.
+numpy part (this file): confidence (Eq. 7, 8, 12), confidence-weighted
+block-diagonal log-det information gain (Eq. 5, 6, 9) with numpy.linalg.slogdet
+as the library primitive, and the arg-max over candidates (Eq. 5).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "nbv_oracle.cpp"
+_LIB = _HERE / "libnbv_oracle.so"
+
+P = 14
+NB = 105
+
+CAMERA_DTYPE = np.dtype([("width", "<i4"), ("height", "<i4"), ("fx", "<f4"), ("fy", "<f4"), ("cx", "<f4"),
+                         ("cy", "<f4"), ("R", "<f4", (9,)), ("t", "<f4", (3,))])
+
+
+class Config(C.Structure):
+    _fields_ = [
+        ("near_plane", C.c_float), ("blur", C.c_float), ("alpha_min", C.c_float), ("alpha_max", C.c_float),
+        ("t_stop", C.c_float), ("power_min", C.c_float), ("bg", C.c_float * 3), ("channel_mask", C.c_int32),
+        ("channel_weight", C.c_float * 4), ("opacity_coord", C.c_int32),
+    ]
+
+
+def default_config(channel_mask: int = 7, bg=(0.0, 0.0, 0.0), opacity_coord: int = 0,
+                   channel_weight=(1.0, 1.0, 1.0, 1.0)) -> Config:
+    cfg = Config()
+    cfg.near_plane = 0.01
+    cfg.blur = 0.3
+    cfg.alpha_min = np.float32(1.0 / 255.0)
+    cfg.alpha_max = 0.99
+    cfg.t_stop = 1e-4
+    cfg.power_min = -6.0
+    cfg.bg = (C.c_float * 3)(*bg)
+    cfg.channel_mask = channel_mask
+    cfg.channel_weight = (C.c_float * 4)(*channel_weight)
+    cfg.opacity_coord = opacity_coord
+    return cfg
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle shared library (g++, OpenMP, no FP contraction)."""
+    if _LIB.exists() and not force and _LIB.stat().st_mtime >= _SRC.stat().st_mtime:
+        return _LIB
+    flags = ["-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
+    try:
+        if " fma " in open("/proc/cpuinfo").read():
+            flags.append("-mfma")  # std::fmaf inlined; without it libm's (correctly rounded) fmaf is called
+    except OSError:
+        pass
+    tmp = _LIB.with_suffix(".so.tmp%d" % os.getpid())
+    subprocess.check_call(["g++", *flags, str(_SRC), "-o", str(tmp)])
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(str(build()))
+        _lib.orc_create.restype = C.c_void_p
+        _lib.orc_exp_spec.restype = C.c_float
+        _lib.orc_exp_spec.argtypes = [C.c_float]
+        _lib.orc_log_bound.restype = C.c_float
+        _lib.orc_log_bound.argtypes = [C.c_float]
+        _lib.orc_tile_lists.restype = C.c_int64
+        _lib.orc_trace.restype = C.c_int64
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+def _cam(cam) -> np.ndarray:
+    """one camera record as a contiguous (1,) CAMERA_DTYPE array"""
+    return np.ascontiguousarray(np.asarray(cam, dtype=CAMERA_DTYPE).reshape(-1)[:1])
+
+
+def _wh(cam):
+    return int(cam["width"][0]), int(cam["height"][0])
+
+
+def exp_spec(x) -> np.ndarray:
+    x = np.atleast_1d(np.asarray(x, dtype=np.float32))
+    return np.array([lib().orc_exp_spec(C.c_float(float(v))) for v in x], dtype=np.float32)
+
+
+def log_bound(s) -> np.ndarray:
+    s = np.atleast_1d(np.asarray(s, dtype=np.float32))
+    return np.array([lib().orc_log_bound(C.c_float(float(v))) for v in s], dtype=np.float32)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+class OracleScene:
+    """Gaussian map G held by the C++ oracle."""
+
+    def __init__(self, mean, logscale, quat, opacity, rgb, obj_logits, cfg: Config | None = None):
+        f = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+        self.mean, self.logscale, self.quat = f(mean), f(logscale), f(quat)
+        self.opacity, self.rgb, self.obj_logits = f(opacity), f(rgb), f(obj_logits)
+        self.N = int(self.mean.shape[0])
+        self.K = int(self.obj_logits.shape[1]) if self.obj_logits.ndim == 2 else 0
+        self.cfg = cfg if cfg is not None else default_config()
+        self._h = C.c_void_p(lib().orc_create(self.N, self.K, _p(self.mean), _p(self.logscale), _p(self.quat),
+                                              _p(self.opacity), _p(self.rgb), C.byref(self.cfg)))
+
+    def __del__(self):
+        try:
+            if self._h:
+                lib().orc_destroy(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    @property
+    def bad_data(self) -> bool:
+        return bool(lib().orc_bad_data(self._h))
+
+    def activation(self) -> np.ndarray:
+        M = np.zeros((self.N, 9), dtype=np.float32)
+        lib().orc_activation(self._h, _p(M))
+        return M
+
+    def project(self, cam):
+        """decision-path splats: visible (N,), rec (N,9) = mx,my,qa,qb,qc,z,a,b,c ; rect (N,4) tx0,ty0,tx1,ty1"""
+        cam = _cam(cam)
+        vis = np.zeros(self.N, dtype=np.int32)
+        rec = np.zeros((self.N, 9), dtype=np.float32)
+        rect = np.zeros((self.N, 4), dtype=np.int32)
+        lib().orc_project(self._h, _p(cam), _p(vis), _p(rec), _p(rect))
+        return vis, rec, rect
+
+    def depth_order(self, cam) -> np.ndarray:
+        cam = _cam(cam)
+        order = np.zeros(self.N, dtype=np.int32)
+        n = lib().orc_depth_order(self._h, _p(cam), _p(order))
+        return order[:n].copy()
+
+    def tile_lists(self, cam):
+        cam = _cam(cam)
+        W, H = _wh(cam)
+        tx, ty = (W + 15) // 16, (H + 15) // 16
+        offsets = np.zeros(tx * ty + 1, dtype=np.int64)
+        total = lib().orc_tile_lists(self._h, _p(cam), _p(offsets), None, C.c_int64(0))
+        ids = np.zeros(max(int(total), 1), dtype=np.int32)
+        total2 = lib().orc_tile_lists(self._h, _p(cam), _p(offsets), _p(ids), C.c_int64(ids.size))
+        assert total2 == total
+        return offsets, ids[:total]
+
+    def render(self, cam, pixel_mask=None):
+        """dict(rgb (H,W,3), depth, T (binary64 value path), T32 (decision path), ncontrib)"""
+        cam = _cam(cam)
+        W, H = _wh(cam)
+        rgb = np.zeros((H, W, 3))
+        depth = np.zeros((H, W))
+        T = np.ones((H, W))
+        T32 = np.ones((H, W), dtype=np.float32)
+        nc = np.zeros((H, W), dtype=np.int32)
+        pm = None if pixel_mask is None else np.ascontiguousarray(pixel_mask, dtype=np.uint8)
+        lib().orc_render(self._h, _p(cam), _p(pm), _p(rgb), _p(depth), _p(T), _p(T32), _p(nc))
+        return dict(rgb=rgb, depth=depth, T=T, T32=T32, ncontrib=nc)
+
+    def trace(self, cam):
+        """per-pixel contributor lists, CSR: offsets (H*W+1,), ids, clamped"""
+        cam = _cam(cam)
+        W, H = _wh(cam)
+        offsets = np.zeros(H * W + 1, dtype=np.int64)
+        total = lib().orc_trace(self._h, _p(cam), _p(offsets), None, None, C.c_int64(0))
+        ids = np.zeros(max(int(total), 1), dtype=np.int32)
+        cl = np.zeros(max(int(total), 1), dtype=np.uint8)
+        lib().orc_trace(self._h, _p(cam), _p(offsets), _p(ids), _p(cl), C.c_int64(ids.size))
+        return offsets, ids[:total], cl[:total]
+
+    def view_hessian(self, cam, pixel_mask=None, out=None) -> np.ndarray:
+        """(N,105) packed upper triangles of sum_pixels sum_channels omega J^T J; accumulates into `out`."""
+        cam = _cam(cam)
+        if out is None:
+            out = np.zeros((self.N, NB))
+        pm = None if pixel_mask is None else np.ascontiguousarray(pixel_mask, dtype=np.uint8)
+        lib().orc_view_hessian(self._h, _p(cam), _p(pm), _p(out))
+        return out
+
+    def theta(self) -> np.ndarray:
+        """(N,14) binary64 parameter vectors [mu | logscale | quat | opacity logit | rgb]"""
+        th = np.zeros((self.N, P))
+        th[:, 0:3] = self.mean
+        th[:, 3:6] = self.logscale
+        th[:, 6:10] = self.quat
+        s = self.opacity.astype(np.float64)
+        th[:, 10] = np.log(s) - np.log1p(-s)
+        th[:, 11:14] = self.rgb
+        return th
+
+
+def render_smooth(theta, cam, cfg, offsets, ids, clamped) -> np.ndarray:
+    cam = _cam(cam)
+    theta = np.ascontiguousarray(theta, dtype=np.float64)
+    W, H = _wh(cam)
+    out = np.zeros((H, W, 4))
+    lib().orc_render_smooth(theta.shape[0], _p(theta), _p(cam), C.byref(cfg), _p(offsets), _p(ids), _p(clamped), _p(out))
+    return out
+
+
+def view_hessian_smooth(theta, cam, cfg, offsets, ids, clamped) -> np.ndarray:
+    cam = _cam(cam)
+    theta = np.ascontiguousarray(theta, dtype=np.float64)
+    out = np.zeros((theta.shape[0], NB))
+    lib().orc_view_hessian_smooth(theta.shape[0], _p(theta), _p(cam), C.byref(cfg), _p(offsets), _p(ids), _p(clamped), _p(out))
+    return out
+
+
+def chain(theta14, cam, cfg):
+    """binary64 projection of one Gaussian and its derivatives: (mx,my,a,b,c,z), G (5,10), dz (3,)"""
+    cam = _cam(cam)
+    th = np.ascontiguousarray(theta14, dtype=np.float64)
+    out6 = np.zeros(6)
+    G = np.zeros((5, 10))
+    dz = np.zeros(3)
+    lib().orc_chain(_p(cam), C.byref(cfg), _p(th), _p(out6), _p(G), _p(dz))
+    return out6, G, dz
+
+
+# ---------------------------------------------------------------------------
+# numpy part: blocks, confidence, gain, arg-max
+# ---------------------------------------------------------------------------
+_IU = np.triu_indices(P)
+
+
+def unpack_blocks(packed: np.ndarray) -> np.ndarray:
+    """(N,105) -> (N,14,14) symmetric."""
+    packed = np.asarray(packed, dtype=np.float64)
+    full = np.zeros(packed.shape[:-1] + (P, P))
+    full[..., _IU[0], _IU[1]] = packed
+    full[..., _IU[1], _IU[0]] = packed
+    return full
+
+
+def pack_blocks(full: np.ndarray) -> np.ndarray:
+    return np.asarray(full)[..., _IU[0], _IU[1]]
+
+
+def softmax(logits: np.ndarray) -> np.ndarray:
+    z = np.asarray(logits, dtype=np.float64)
+    z = z - z.max(axis=1, keepdims=True)
+    e = np.exp(z)
+    return e / e.sum(axis=1, keepdims=True)
+
+
+def confidence(obj_logits, opacity, alpha_obj=0.3, alpha_opa=0.3, target=-1, p_floor=1e-4, s_floor=1e-4) -> np.ndarray:
+    """PAPER.md Eq. 7 (L229-232): c_g = max_k(p_gk)^-alpha_obj * sigma_g^-alpha_opa, p_g = softmax(o_g) (L146).
+    Eq. 12 (L698-704) with a target object: p_{g,obj} replaces the max, and c_g = 0 unless argmax_k p_gk = obj.
+    Floors on p and sigma: reading R-14."""
+    p = softmax(obj_logits)
+    s = np.maximum(np.asarray(opacity, dtype=np.float64), s_floor)
+    if target < 0:
+        pm = np.maximum(p.max(axis=1), p_floor)
+        return pm ** (-alpha_obj) * s ** (-alpha_opa)
+    am = p.argmax(axis=1)  # lowest index on ties
+    pt = np.maximum(p[:, target], p_floor)
+    c = pt ** (-alpha_obj) * s ** (-alpha_opa)
+    return np.where(am == target, c, 0.0)
+
+
+def gaussian_gains(H_T, H_c, c, prior) -> np.ndarray:
+    """Per-Gaussian information gain (Eq. 5, 6, 9; block-diagonal, L210):
+        IG_g = log det(c_g (H_T,g + H_c,g) + Lambda) - log det(c_g H_T,g + Lambda)
+    H_T, H_c: (N,105) packed; c: (N,); prior: (14,) diagonal of Lambda (reading R-13)."""
+    Lam = np.diag(np.asarray(prior, dtype=np.float64))
+    A = unpack_blocks(H_T)
+    B = unpack_blocks(H_c)
+    c = np.asarray(c, dtype=np.float64)[:, None, None]
+    s1, l1 = np.linalg.slogdet(c * (A + B) + Lam)
+    s0, l0 = np.linalg.slogdet(c * A + Lam)
+    assert np.all(s1 > 0) and np.all(s0 > 0)
+    return l1 - l0
+
+
+def argmax_lowest(scores) -> int:
+    """PAPER.md Eq. 5: c* = argmax_c IG(T,c); ties -> lowest index (R-15)."""
+    scores = np.asarray(scores)
+    return int(np.flatnonzero(scores == scores.max())[0])
+
+
+def score_candidates(scene: OracleScene, train_cams, cand_cams, target=-1, alpha_obj=0.3, alpha_opa=0.3,
+                     prior=None, H_T=None):
+    """The whole hot path on the CPU.  Returns dict(H_T, scores, best, conf, gains (C,N))."""
+    prior = np.ones(P) if prior is None else np.asarray(prior, dtype=np.float64)
+    if H_T is None:
+        H_T = np.zeros((scene.N, NB))
+        for cam in np.atleast_1d(train_cams):
+            scene.view_hessian(cam, out=H_T)
+    conf = confidence(scene.obj_logits, scene.opacity, alpha_obj, alpha_opa, target)
+    scores, gains = [], []
+    for cam in np.atleast_1d(cand_cams):
+        H_c = scene.view_hessian(cam)
+        g = gaussian_gains(H_T, H_c, conf, prior)
+        gains.append(g)
+        scores.append(g.sum())
+    scores = np.array(scores)
+    return dict(H_T=H_T, scores=scores, best=argmax_lowest(scores), conf=conf, gains=np.array(gains))
