@@ -1,0 +1,172 @@
+/* nbv.h -- C ABI of libnbv: candidate-view scoring for object-aware 3D Gaussian Splatting
+ * next-best-view (arxiv/paper_2602_08266), hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations: P:Lnnn = PAPER.md line nnn; R-n = reading n in DESIGN.md section 2.
+ *
+ * The library scores candidate camera poses by the confidence-weighted, block-diagonal
+ * log-det information gain of the paper:
+ *     IG(T,c) = f(T u c) - f(T),   f(V) = log det sum_{v in V} J_v^T J_v      (Eq. 5-6)
+ *     only each Gaussian's own P x P block is kept
+ *     H := J^T C J,  C_g = c_g I,  c_g = max_k(p_gk)^-a_obj sigma_g^-a_opa    (Eq. 7-9)
+ *     object-centric: c_g = p_{g,obj}^-a_obj sigma_g^-a_opa if argmax_k p_gk = obj else 0 (Eq. 12)
+ * J is the Jacobian of the rendered colour and depth w.r.t. the P = 14 parameters of a Gaussian
+ * at SH degree 0, in this order (R-10):
+ *     theta = [mu_x mu_y mu_z | logscale_x y z | quat_w x y z (raw, through q/|q|) | opacity logit | r g b]
+ * A packed block holds the upper triangle row-major: entry (r,c), r <= c, at r*14 - r*(r-1)/2 + (c-r)
+ * (105 floats).
+ *
+ * Conventions
+ *  - Every function returns NBV_OK (0) or a negative nbv_status; nothing throws or aborts.
+ *    nbv_last_error() gives a text for the last failure on that context.
+ *  - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch tensors); the library reads or
+ *    writes them during the call, on `stream`, and never frees them.  Pointers named h_* are HOST pointers.
+ *    Cameras are host structs.  Everything the library allocates belongs to the context and is released
+ *    by nbv_destroy().
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls enqueue work on it; calls
+ *    that size device buffers from device-side counts synchronise the stream internally (stated per call).
+ *  - One context serves one GPU (the current device at nbv_create) and is not thread-safe.
+ *  - There is no CPU fallback: without a CUDA device every call fails with NBV_ERR_CUDA.
+ */
+#ifndef NBV_H_
+#define NBV_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NBV_P 14          /* parameters per Gaussian block */
+#define NBV_BLOCK 105     /* packed upper triangle of a 14 x 14 block */
+#define NBV_TILE 16       /* tile edge in pixels (B: north_star "16x16 tile") */
+
+#define NBV_CH_RGB 7      /* channel_mask bits: 1 = r, 2 = g, 4 = b, 8 = depth */
+#define NBV_CH_DEPTH 8
+#define NBV_CH_RGBD 15
+
+typedef enum nbv_status {
+  NBV_OK = 0,
+  NBV_ERR_INVALID_ARG = -1,      /* null pointer, non-positive size, bad camera (R not orthonormal within 1e-4, fx<=0 ...) */
+  NBV_ERR_BAD_DATA = -2,         /* zero / non-finite quaternion, opacity outside (0,1), non-finite parameter */
+  NBV_ERR_NOT_LOADED = -3,       /* a call that needs Gaussians before nbv_load_gaussians */
+  NBV_ERR_EMPTY_CANDIDATES = -4, /* nbv_score_candidates with n == 0 */
+  NBV_ERR_UNKNOWN_TARGET = -5,   /* target_obj >= K or < -1 */
+  NBV_ERR_OOM = -6,              /* device allocation failed */
+  NBV_ERR_CUDA = -7,             /* any other CUDA runtime error (text in nbv_last_error) */
+  NBV_ERR_CAPACITY = -8          /* a caller-provided output buffer is too small (nbv_tile_lists) */
+} nbv_status;
+
+/* Pinhole camera, OpenCV axes (+x right, +y down, +z forward); pixel (i,j) is sampled at (i+0.5, j+0.5),
+ * origin top-left (R-1).  R_cw is row-major world->camera, p_cam = R_cw p_world + t_cw. */
+typedef struct nbv_camera {
+  int32_t width, height;
+  float fx, fy, cx, cy;
+  float R_cw[9];
+  float t_cw[3];
+} nbv_camera;
+
+/* Context configuration.  nbv_default_config() fills the values the oracle and DESIGN.md use. */
+typedef struct nbv_config {
+  float near_plane;          /* 0.01   cull z <= near (R-2) */
+  float blur;                /* 0.3    px^2 added to the diagonal of Sigma2D (R-3) */
+  float alpha_min;           /* 1/255  skip threshold (R-4) */
+  float alpha_max;           /* 0.99   alpha cap (R-4) */
+  float t_stop;              /* 1e-4   stop before T would fall below (R-4) */
+  float bg[3];               /* background colour, default 0 (R-8); depth background is 0 (R-6) */
+  int32_t channel_mask;      /* NBV_CH_RGB or NBV_CH_RGBD or NBV_CH_DEPTH: outputs whose Jacobians enter H (R-12) */
+  float channel_weight[4];   /* omega_ch, inverse noise variance per channel, default 1 (R-12) */
+  int32_t opacity_coord;     /* 0 = logit (default), 1 = sigma (R-10) */
+  float alpha_obj, alpha_opa;/* 0.3, 0.3 exponents of Eq. 7 / Eq. 12 */
+  float p_floor, sigma_floor;/* 1e-4 floors inside Eq. 7 (R-14) */
+  float prior_precision[14]; /* diagonal of Lambda (R-13), default 1.0 each */
+} nbv_config;
+
+typedef struct nbv_ctx nbv_ctx;
+
+/* Per-view counters of the last view processed (diagnostics and roofline accounting; host readable). */
+typedef struct nbv_view_stats {
+  int64_t n_visible;      /* Gaussians surviving the culls */
+  int64_t n_keys;         /* (tile, Gaussian) keys emitted = sum of rect areas */
+  int64_t n_entries;      /* (tile, Gaussian) list entries walked by the forward pass before the tile terminated */
+  int64_t n_pairs;        /* (pixel, Gaussian) pairs composited = sum of per-pixel contributor counts */
+  int64_t n_touched;      /* Gaussians with a non-zero block in this view */
+} nbv_view_stats;
+
+void nbv_default_config(nbv_config* cfg);
+
+/* Create / destroy a context on the current CUDA device.  cfg == NULL -> defaults.
+ * Errors: INVALID_ARG (out == NULL, non-positive thresholds, prior_precision <= 0, empty channel_mask), CUDA. */
+int nbv_create(nbv_ctx** out, const nbv_config* cfg);
+void nbv_destroy(nbv_ctx* ctx);
+const char* nbv_last_error(const nbv_ctx* ctx);
+
+/* S0 -- load the Gaussian map G with object vectors: device arrays, row-major, float32.
+ *   d_mean N x 3, d_logscale N x 3, d_quat N x 4 (w,x,y,z; any non-zero norm), d_opacity N (sigma in (0,1)),
+ *   d_rgb N x 3, d_obj_logits N x K.
+ * Runs the activation kernel (s = exp l, q/|q|, M = R diag s; softmax statistics of the object logits), copies
+ * what later calls need, and resets the training Hessian to zero.  Synchronises `stream` (it reads back the
+ * bad-data flag).  Errors: INVALID_ARG (N <= 0, K <= 0, null), BAD_DATA, OOM, CUDA. */
+int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, const float* d_logscale,
+                       const float* d_quat, const float* d_opacity, const float* d_rgb,
+                       const float* d_obj_logits, void* stream);
+
+/* H_T <- 0, |T| <- 0. */
+int nbv_reset_training(nbv_ctx* ctx, void* stream);
+
+/* H_T += sum over the n cameras of the per-Gaussian J^T J blocks of that view (Eq. 6),
+ * unweighted: confidence enters at scoring time, which is Eq. 9 because C_g = c_g I (R-14).
+ * Gaussians behind a camera contribute zero.  h_cams: HOST array of n cameras.
+ * Errors: NOT_LOADED, INVALID_ARG (n < 0, bad camera), OOM, CUDA. */
+int nbv_accumulate_training(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, void* stream);
+
+/* Score n candidate cameras (S0', S1-S7):
+ *   d_scores[i] = sum_g [ log det(c_g (H_T,g + H_i,g) + Lambda) - log det(c_g H_T,g + Lambda) ]   (Eq. 5, 6, 9)
+ *   *d_best     = arg max_i d_scores[i], lowest index on ties (R-15)
+ * target_obj = -1 scores the whole scene with Eq. 7; 0 <= target_obj < K restricts the gain to that object's
+ * Gaussians with Eq. 12.  Scoring with no training view is allowed (H_T = 0).  d_scores: n floats, d_best: one
+ * int32, both DEVICE.  Errors: NOT_LOADED, EMPTY_CANDIDATES (n == 0), UNKNOWN_TARGET, INVALID_ARG, OOM, CUDA. */
+int nbv_score_candidates(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t target_obj,
+                         float* d_scores, int32_t* d_best, void* stream);
+
+/* Same as nbv_score_candidates but with HOST outputs (copies back and synchronises `stream`). */
+int nbv_score_candidates_host(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t target_obj,
+                              float* h_scores, int32_t* h_best, void* stream);
+
+/* Counters of the last view processed by any call (synchronises `stream`). */
+int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream);
+
+/* ---- parity / debug exports (not on the timed path) ------------------------------------------------ */
+
+/* S1 outputs of one view, indexed by Gaussian: d_visible N int32; d_rec N x 9 floats
+ * (mx, my, qa, qb, qc, z, a, b, c) with power(d) = qa dx^2 + qb dx dy + qc dy^2 and Sigma2D = [[a,b],[b,c]];
+ * d_rect N x 4 int32 (tx0, ty0, tx1, ty1) half-open tile rectangle.  Any output may be NULL. */
+int nbv_projected(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t* d_visible, float* d_rec, int32_t* d_rect,
+                  void* stream);
+
+/* S2 output of one view: d_offsets (tiles+1 int64, tile t = ty*ceil(W/16)+tx lists [offsets[t], offsets[t+1]))
+ * and d_ids (Gaussian indices in depth order per tile, capacity `cap` entries).  *h_total receives the number
+ * of entries; if it exceeds cap, d_ids is not written and NBV_ERR_CAPACITY is returned.  Synchronises. */
+int nbv_tile_lists(nbv_ctx* ctx, const nbv_camera* h_cam, int64_t* d_offsets, int32_t* d_ids, int64_t cap,
+                   int64_t* h_total, void* stream);
+
+/* S3 output of one view: d_rgb H x W x 3, d_depth H x W, d_T H x W (final transmittance), d_ncontrib H x W int32
+ * (number of composited Gaussians per pixel).  Any output may be NULL. */
+int nbv_render(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_rgb, float* d_depth, float* d_T,
+               int32_t* d_ncontrib, void* stream);
+
+/* S4+S5 output of one view: d_blocks N x 105, overwritten with that view's unweighted blocks. */
+int nbv_view_hessian(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_blocks, void* stream);
+
+/* Copy of the accumulated training Hessian H_T (N x 105). */
+int nbv_training_hessian(nbv_ctx* ctx, float* d_blocks, void* stream);
+
+/* S0' output: confidence c_g (N floats) for the given mode (Eq. 7 or Eq. 12). */
+int nbv_confidence(nbv_ctx* ctx, int32_t target_obj, float* d_conf, void* stream);
+
+/* S6 per-Gaussian terms of one candidate: d_gains N floats (zero for Gaussians the view does not touch). */
+int nbv_gaussian_gains(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t target_obj, float* d_gains, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBV_H_ */

@@ -1,0 +1,268 @@
+"""Thin Python binding of libnbv (include/nbv.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/.  PyTorch supplies device memory (tensors whose
+data_ptr() is passed through) and the current CUDA stream; nothing is computed here.  There is no CPU
+fallback: without the built library and a CUDA device every call raises.
+
+Names mirror the C ABI: NBV.load_gaussians -> nbv_load_gaussians, NBV.accumulate_training ->
+nbv_accumulate_training, NBV.score_candidates -> nbv_score_candidates, ...
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+from .synth import CAMERA_DTYPE
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libnbv.so"
+
+P = 14
+NBLK = 105
+CH_RGB, CH_DEPTH, CH_RGBD = 7, 8, 15
+
+STATUS = {
+    0: "NBV_OK", -1: "NBV_ERR_INVALID_ARG", -2: "NBV_ERR_BAD_DATA", -3: "NBV_ERR_NOT_LOADED",
+    -4: "NBV_ERR_EMPTY_CANDIDATES", -5: "NBV_ERR_UNKNOWN_TARGET", -6: "NBV_ERR_OOM", -7: "NBV_ERR_CUDA",
+    -8: "NBV_ERR_CAPACITY",
+}
+
+# every symbol include/nbv.h declares (tests check that the library exports all of them)
+EXPORTS = [
+    "nbv_default_config", "nbv_create", "nbv_destroy", "nbv_last_error", "nbv_load_gaussians", "nbv_reset_training",
+    "nbv_accumulate_training", "nbv_score_candidates", "nbv_score_candidates_host", "nbv_last_view_stats",
+    "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
+    "nbv_gaussian_gains",
+]
+
+
+class NBVError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__("%s (%d): %s" % (STATUS.get(code, "?"), code, msg))
+        self.code = code
+        self.status = STATUS.get(code, "?")
+
+
+class Config(C.Structure):
+    """nbv_config"""
+    _fields_ = [
+        ("near_plane", C.c_float), ("blur", C.c_float), ("alpha_min", C.c_float), ("alpha_max", C.c_float),
+        ("t_stop", C.c_float), ("bg", C.c_float * 3), ("channel_mask", C.c_int32), ("channel_weight", C.c_float * 4),
+        ("opacity_coord", C.c_int32), ("alpha_obj", C.c_float), ("alpha_opa", C.c_float), ("p_floor", C.c_float),
+        ("sigma_floor", C.c_float), ("prior_precision", C.c_float * 14),
+    ]
+
+
+class ViewStats(C.Structure):
+    """nbv_view_stats"""
+    _fields_ = [("n_visible", C.c_int64), ("n_keys", C.c_int64), ("n_entries", C.c_int64), ("n_pairs", C.c_int64),
+                ("n_touched", C.c_int64)]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def load_library(path: Path | None = None):
+    """dlopen libnbv.so (built in-tree by paper_2602_08266_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = Path(path) if path else LIB_PATH
+    if not p.exists():
+        raise FileNotFoundError("%s not built: run `python -m paper_2602_08266_b200.build` (nvcc, sm_100a)" % p)
+    lib = C.CDLL(str(p))
+    lib.nbv_last_error.restype = C.c_char_p
+    lib.nbv_last_error.argtypes = [C.c_void_p]
+    lib.nbv_destroy.restype = None
+    lib.nbv_destroy.argtypes = [C.c_void_p]
+    lib.nbv_default_config.restype = None
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def default_config(**overrides) -> Config:
+    cfg = Config()
+    load_library().nbv_default_config(C.byref(cfg))
+    for k, v in overrides.items():
+        if k in ("bg", "channel_weight", "prior_precision"):
+            arr = getattr(cfg, k)
+            vals = list(v) if np.ndim(v) else [v] * len(arr)
+            for i, x in enumerate(vals):
+                arr[i] = float(x)
+        else:
+            setattr(cfg, k, v)
+    return cfg
+
+
+def _cams(cams) -> np.ndarray:
+    a = np.ascontiguousarray(np.asarray(cams, dtype=CAMERA_DTYPE).reshape(-1))
+    return a
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+class NBV:
+    """One libnbv context (one GPU)."""
+
+    def __init__(self, cfg: Config | None = None, **overrides):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libnbv needs a CUDA device (sm_100a); there is no CPU fallback")
+        self._torch = torch
+        self.lib = load_library()
+        self.cfg = cfg if cfg is not None else default_config(**overrides)
+        self._h = C.c_void_p()
+        rc = self.lib.nbv_create(C.byref(self._h), C.byref(self.cfg))
+        if rc != 0:
+            raise NBVError(rc, "nbv_create failed")
+        self.N = 0
+        self.K = 0
+        self.device = torch.device("cuda", torch.cuda.current_device())
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            self.lib.nbv_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int):
+        if rc != 0:
+            msg = self.lib.nbv_last_error(self._h)
+            raise NBVError(rc, msg.decode() if msg else "")
+
+    def _dev(self, a, dtype=None):
+        torch = self._torch
+        if isinstance(a, torch.Tensor):
+            t = a.to(device=self.device, dtype=dtype or torch.float32)
+        else:
+            t = torch.as_tensor(np.ascontiguousarray(a), device=self.device).to(dtype or torch.float32)
+        return t.contiguous()
+
+    # ---- hot path -----------------------------------------------------------------------------
+    def load_gaussians(self, mean, logscale, quat, opacity, rgb, obj_logits):
+        """nbv_load_gaussians.  Arguments: torch CUDA tensors (used in place) or numpy arrays (copied to the GPU)."""
+        m, ls, q = self._dev(mean), self._dev(logscale), self._dev(quat)
+        o, c, lg = self._dev(opacity), self._dev(rgb), self._dev(obj_logits)
+        N = int(m.shape[0])
+        if N == 0 or lg.ndim != 2:
+            raise NBVError(-1, "empty Gaussian set or malformed object logits")
+        K = int(lg.shape[1])
+        self._check(self.lib.nbv_load_gaussians(self._h, N, K, _ptr(m), _ptr(ls), _ptr(q), _ptr(o), _ptr(c), _ptr(lg), _stream()))
+        self.N, self.K = N, K
+
+    def load_scene(self, scene):
+        self.load_gaussians(scene.mean, scene.logscale, scene.quat, scene.opacity, scene.rgb, scene.obj_logits)
+
+    def reset_training(self):
+        self._check(self.lib.nbv_reset_training(self._h, _stream()))
+
+    def accumulate_training(self, cams):
+        cams = _cams(cams)
+        self._check(self.lib.nbv_accumulate_training(self._h, C.c_void_p(cams.ctypes.data), int(cams.shape[0]), _stream()))
+
+    def score_candidates(self, cams, target_obj: int = -1, scores=None, best=None):
+        """nbv_score_candidates: returns (scores, best) as CUDA tensors (no host synchronisation)."""
+        torch = self._torch
+        cams = _cams(cams)
+        n = int(cams.shape[0])
+        if scores is None:
+            scores = torch.empty(max(n, 1), dtype=torch.float32, device=self.device)
+        if best is None:
+            best = torch.empty(1, dtype=torch.int32, device=self.device)
+        self._check(self.lib.nbv_score_candidates(self._h, C.c_void_p(cams.ctypes.data), n, int(target_obj), _ptr(scores), _ptr(best), _stream()))
+        return scores[:n], best
+
+    def score_candidates_host(self, cams, target_obj: int = -1):
+        """nbv_score_candidates_host: HOST outputs (numpy scores, int best); synchronises."""
+        cams = _cams(cams)
+        n = int(cams.shape[0])
+        scores = np.zeros(max(n, 1), dtype=np.float32)
+        best = C.c_int32(-1)
+        self._check(self.lib.nbv_score_candidates_host(self._h, C.c_void_p(cams.ctypes.data), n, int(target_obj),
+                                                       C.c_void_p(scores.ctypes.data), C.byref(best), _stream()))
+        return scores[:n], int(best.value)
+
+    def last_view_stats(self) -> dict:
+        st = ViewStats()
+        self._check(self.lib.nbv_last_view_stats(self._h, C.byref(st), _stream()))
+        return st.as_dict()
+
+    # ---- parity / debug exports ------------------------------------------------------------------
+    def projected(self, cam):
+        torch = self._torch
+        cam = _cams(cam)
+        vis = torch.empty(self.N, dtype=torch.int32, device=self.device)
+        rec = torch.empty((self.N, 9), dtype=torch.float32, device=self.device)
+        rect = torch.empty((self.N, 4), dtype=torch.int32, device=self.device)
+        self._check(self.lib.nbv_projected(self._h, C.c_void_p(cam.ctypes.data), _ptr(vis), _ptr(rec), _ptr(rect), _stream()))
+        return vis, rec, rect
+
+    def tile_lists(self, cam):
+        torch = self._torch
+        cam = _cams(cam)
+        W, H = int(cam["width"][0]), int(cam["height"][0])
+        nt = ((W + 15) // 16) * ((H + 15) // 16)
+        offsets = torch.empty(nt + 1, dtype=torch.int64, device=self.device)
+        total = C.c_int64(0)
+        rc = self.lib.nbv_tile_lists(self._h, C.c_void_p(cam.ctypes.data), _ptr(offsets), None, C.c_int64(0), C.byref(total), _stream())
+        if rc not in (0, -8):
+            self._check(rc)
+        ids = torch.empty(max(int(total.value), 1), dtype=torch.int32, device=self.device)
+        self._check(self.lib.nbv_tile_lists(self._h, C.c_void_p(cam.ctypes.data), _ptr(offsets), _ptr(ids), C.c_int64(ids.numel()),
+                                            C.byref(total), _stream()))
+        return offsets, ids[: int(total.value)]
+
+    def render(self, cam):
+        torch = self._torch
+        cam = _cams(cam)
+        W, H = int(cam["width"][0]), int(cam["height"][0])
+        rgb = torch.empty((H, W, 3), dtype=torch.float32, device=self.device)
+        depth = torch.empty((H, W), dtype=torch.float32, device=self.device)
+        T = torch.empty((H, W), dtype=torch.float32, device=self.device)
+        nc = torch.empty((H, W), dtype=torch.int32, device=self.device)
+        self._check(self.lib.nbv_render(self._h, C.c_void_p(cam.ctypes.data), _ptr(rgb), _ptr(depth), _ptr(T), _ptr(nc), _stream()))
+        return dict(rgb=rgb, depth=depth, T=T, ncontrib=nc)
+
+    def view_hessian(self, cam):
+        torch = self._torch
+        cam = _cams(cam)
+        blocks = torch.empty((self.N, NBLK), dtype=torch.float32, device=self.device)
+        self._check(self.lib.nbv_view_hessian(self._h, C.c_void_p(cam.ctypes.data), _ptr(blocks), _stream()))
+        return blocks
+
+    def training_hessian(self):
+        torch = self._torch
+        blocks = torch.empty((self.N, NBLK), dtype=torch.float32, device=self.device)
+        self._check(self.lib.nbv_training_hessian(self._h, _ptr(blocks), _stream()))
+        return blocks
+
+    def confidence(self, target_obj: int = -1):
+        torch = self._torch
+        conf = torch.empty(self.N, dtype=torch.float32, device=self.device)
+        self._check(self.lib.nbv_confidence(self._h, int(target_obj), _ptr(conf), _stream()))
+        return conf
+
+    def gaussian_gains(self, cam, target_obj: int = -1):
+        torch = self._torch
+        cam = _cams(cam)
+        gains = torch.empty(self.N, dtype=torch.float32, device=self.device)
+        self._check(self.lib.nbv_gaussian_gains(self._h, C.c_void_p(cam.ctypes.data), int(target_obj), _ptr(gains), _stream()))
+        return gains

@@ -1,0 +1,78 @@
+// common.cuh -- shared definitions of the CUDA path (sm_100a).  Not used by, and shares nothing with, oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/nbv.h"
+
+namespace nbv {
+
+constexpr int P = NBV_P;
+constexpr int NBLK = NBV_BLOCK;
+constexpr int TILE = NBV_TILE;
+constexpr int NMOM = 40;        // screen-space moments per (view, Gaussian): 15 + 4*6 + 1
+constexpr int MOM_X = 15;       // first cross moment
+constexpr int MOM_W2 = 39;      // sum of w^2
+constexpr float POWER_MIN = -6.0f;
+
+// Projected splat, 48 bytes, stored in depth-rank order for the rasteriser.
+struct __align__(16) Splat {
+  float mx, my, qa, qb;      // centre (px); power(d) = qa dx^2 + qb dx dy + qc dy^2
+  float qc, sigma, z, tau;   // tau: conservative lower bound of ln(alpha_min / sigma) (pre-test only, never decides)
+  float r, g, b, pad;
+};
+
+struct ViewCounters {          // device-side counters of one view
+  unsigned long long n_keys;   // sum of rect areas
+  unsigned long long n_entries;
+  unsigned long long n_pairs;
+  unsigned int n_visible;
+  unsigned int n_touched;
+  unsigned int bad_data;
+  unsigned int pad;
+};
+
+// ---------------------------------------------------------------------------------------------
+// Decision-path arithmetic (R-9).  Every operation individually rounded with
+// the _rn intrinsics (never contracted by the compiler); fused multiply-adds only where __fmaf_rn
+// is written.  Must reproduce the binary32 results of the specification bit for bit.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float div_rn(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ float sqrt_rn(float a) { return __fsqrt_rn(a); }
+
+__device__ __forceinline__ float exp_spec(float x) {
+  const float MAGIC = 12582912.0f;
+  float t = __fmaf_rn(x, 0x1.715476p+0f, MAGIC);
+  float kf = __fsub_rn(t, MAGIC);
+  float r = __fmaf_rn(kf, -0x1.62e4p-1f, x);
+  r = __fmaf_rn(kf, -0x1.7f7d1cp-20f, r);
+  float p = 0x1.6c16c2p-10f;
+  p = __fmaf_rn(p, r, 0x1.111112p-7f);
+  p = __fmaf_rn(p, r, 0x1.555556p-5f);
+  p = __fmaf_rn(p, r, 0x1.555556p-3f);
+  p = __fmaf_rn(p, r, 0.5f);
+  p = __fmaf_rn(p, r, 1.0f);
+  p = __fmaf_rn(p, r, 1.0f);
+  int k = __float_as_int(t) - __float_as_int(MAGIC);
+  return __int_as_float(__float_as_int(p) + (k << 23));
+}
+
+// power of the Gaussian exponent at offset (dx,dy)
+__device__ __forceinline__ float splat_power(float qa, float qb, float qc, float dx, float dy) {
+  return __fmaf_rn(dx, __fmaf_rn(qa, dx, __fmul_rn(qb, dy)), __fmul_rn(__fmul_rn(qc, dy), dy));
+}
+
+// packed upper-triangle index, r <= c
+__host__ __device__ __forceinline__ constexpr int tri(int r, int c) { return r * P - r * (r - 1) / 2 + (c - r); }
+
+// monomial sums sum B alpha^2 ux^i uy^j, i+j <= 4, stored at mono_index(i,j)
+__host__ __device__ __forceinline__ constexpr int mono_index(int i, int j) {
+  // order: (0,0) | (1,0),(0,1) | (2,0),(1,1),(0,2) | (3,0),(2,1),(1,2),(0,3) | (4,0),(3,1),(2,2),(1,3),(0,4)
+  return (i + j) * (i + j + 1) / 2 + j;
+}
+
+}  // namespace nbv

@@ -1,0 +1,343 @@
+// hessian.cu -- S5 (moments -> 14x14 block), S0' (confidence), S6 (log-det gain), S7 (arg-max).
+//
+// S5: for a Gaussian touched by the view, the 40 screen-space moments of S4 become
+//       H_g = A Q A^T + sum_ch omega_ch [ (A x_ch) e_ch^T + e_ch (A x_ch)^T + W2 e_ch e_ch^T ]
+//     with Q (6x6) the monomial sums arranged by m6 = (ux,uy,ux^2,ux uy,uy^2,1), x_ch the cross moments, W2 = sum w^2,
+//     e_ch = d v_ch / d theta (unit vector on the colour parameter, or (dz/dmu, 0..) for depth), and
+//     A (14 x 6): rows of the chain d(mx,my,a,b,c)/d(mu,logscale,quat) (first-order EWA, through q/|q|), the
+//     opacity row kappa, zero colour rows.   PAPER.md L189-191 (H ~= J^T J), L210 (per-Gaussian blocks), L248.
+// S6: IG_g = log det(c_g (H_T,g + H_c,g) + Lambda) - log det(c_g H_T,g + Lambda)   (Eq. 5, 6, 9; R-13, R-14)
+//     by a packed Cholesky per Gaussian, one thread each; the second term is precomputed once per scoring call.
+#include "kernels.h"
+
+namespace nbv {
+
+struct ChainF {
+  float G[5][10];   // d(mx,my,a,b,c) / d(mu(3), logscale(3), quat(4))
+  float dz[3];      // dz/dmu
+};
+
+__device__ void sandwich_f(const float* Tm, const float* S3, float& a, float& b, float& c) {
+  float TS[6];
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) TS[3 * i + k] = Tm[3 * i] * S3[k] + Tm[3 * i + 1] * S3[3 + k] + Tm[3 * i + 2] * S3[6 + k];
+  a = TS[0] * Tm[0] + TS[1] * Tm[1] + TS[2] * Tm[2];
+  b = TS[0] * Tm[3] + TS[1] * Tm[4] + TS[2] * Tm[5];
+  c = TS[3] * Tm[3] + TS[4] * Tm[4] + TS[5] * Tm[5];
+}
+
+// Value-path chain rule of the projection (binary32).
+__device__ void chain_f(const nbv_camera& cam, const float* mu, const float* ls, const float* q, ChainF& ch) {
+  const float* W = cam.R_cw;
+  const float fx = cam.fx, fy = cam.fy;
+  const float x = W[0] * mu[0] + W[1] * mu[1] + W[2] * mu[2] + cam.t_cw[0];
+  const float y = W[3] * mu[0] + W[4] * mu[1] + W[5] * mu[2] + cam.t_cw[1];
+  const float z = W[6] * mu[0] + W[7] * mu[1] + W[8] * mu[2] + cam.t_cw[2];
+  const float iz = 1.0f / z, iz2 = iz * iz;
+  const float J[6] = {fx * iz, 0.f, -fx * x * iz2, 0.f, fy * iz, -fy * y * iz2};
+  float Tm[6];
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) Tm[3 * i + k] = J[3 * i] * W[k] + J[3 * i + 1] * W[3 + k] + J[3 * i + 2] * W[6 + k];
+  const float qn = sqrtf(q[0] * q[0] + q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+  const float iqn = 1.0f / qn;
+  const float qw = q[0] * iqn, qx = q[1] * iqn, qy = q[2] * iqn, qz = q[3] * iqn;
+  float R[9];
+  R[0] = 1.f - 2.f * (qy * qy + qz * qz); R[1] = 2.f * (qx * qy - qw * qz);       R[2] = 2.f * (qx * qz + qw * qy);
+  R[3] = 2.f * (qx * qy + qw * qz);       R[4] = 1.f - 2.f * (qx * qx + qz * qz); R[5] = 2.f * (qy * qz - qw * qx);
+  R[6] = 2.f * (qx * qz - qw * qy);       R[7] = 2.f * (qy * qz + qw * qx);       R[8] = 1.f - 2.f * (qx * qx + qy * qy);
+  const float s2[3] = {expf(2.f * ls[0]), expf(2.f * ls[1]), expf(2.f * ls[2])};
+  float S3[9];
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j)
+      S3[3 * i + j] = R[3 * i] * s2[0] * R[3 * j] + R[3 * i + 1] * s2[1] * R[3 * j + 1] + R[3 * i + 2] * s2[2] * R[3 * j + 2];
+  // d/dmu
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    ch.G[0][k] = Tm[k];
+    ch.G[1][k] = Tm[3 + k];
+    ch.dz[k] = W[6 + k];
+  }
+  const float iz3 = iz2 * iz;
+  const float dJ[3][6] = {{0.f, 0.f, -fx * iz2, 0.f, 0.f, 0.f},
+                          {0.f, 0.f, 0.f, 0.f, 0.f, -fy * iz2},
+                          {-fx * iz2, 0.f, 2.f * fx * x * iz3, 0.f, -fy * iz2, 2.f * fy * y * iz3}};
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    float dJk[6], dT[6], dTS[6];
+#pragma unroll
+    for (int e = 0; e < 6; ++e) dJk[e] = dJ[0][e] * W[k] + dJ[1][e] * W[3 + k] + dJ[2][e] * W[6 + k];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) dT[3 * i + c] = dJk[3 * i] * W[c] + dJk[3 * i + 1] * W[3 + c] + dJk[3 * i + 2] * W[6 + c];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) dTS[3 * i + c] = dT[3 * i] * S3[c] + dT[3 * i + 1] * S3[3 + c] + dT[3 * i + 2] * S3[6 + c];
+    const float E00 = dTS[0] * Tm[0] + dTS[1] * Tm[1] + dTS[2] * Tm[2];
+    const float E01 = dTS[0] * Tm[3] + dTS[1] * Tm[4] + dTS[2] * Tm[5];
+    const float E10 = dTS[3] * Tm[0] + dTS[4] * Tm[1] + dTS[5] * Tm[2];
+    const float E11 = dTS[3] * Tm[3] + dTS[4] * Tm[4] + dTS[5] * Tm[5];
+    ch.G[2][k] = 2.f * E00;
+    ch.G[3][k] = E01 + E10;
+    ch.G[4][k] = 2.f * E11;
+  }
+  // d/dlogscale_k : dSigma3D = 2 s_k^2 r_k r_k^T
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const float v0 = Tm[0] * R[k] + Tm[1] * R[3 + k] + Tm[2] * R[6 + k];
+    const float v1 = Tm[3] * R[k] + Tm[4] * R[3 + k] + Tm[5] * R[6 + k];
+    ch.G[0][3 + k] = 0.f; ch.G[1][3 + k] = 0.f;
+    ch.G[2][3 + k] = 2.f * s2[k] * v0 * v0;
+    ch.G[3][3 + k] = 2.f * s2[k] * v0 * v1;
+    ch.G[4][3 + k] = 2.f * s2[k] * v1 * v1;
+  }
+  // d/dquat through q_hat = q/|q|
+  const float qh[4] = {qw, qx, qy, qz};
+  float dh[4][3];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    float Dm[9];
+    if (i == 0) { const float d[9] = {0.f, -2.f * qz, 2.f * qy, 2.f * qz, 0.f, -2.f * qx, -2.f * qy, 2.f * qx, 0.f}; for (int e = 0; e < 9; ++e) Dm[e] = d[e]; }
+    else if (i == 1) { const float d[9] = {0.f, 2.f * qy, 2.f * qz, 2.f * qy, -4.f * qx, -2.f * qw, 2.f * qz, 2.f * qw, -4.f * qx}; for (int e = 0; e < 9; ++e) Dm[e] = d[e]; }
+    else if (i == 2) { const float d[9] = {-4.f * qy, 2.f * qx, 2.f * qw, 2.f * qx, 0.f, 2.f * qz, -2.f * qw, 2.f * qz, -4.f * qy}; for (int e = 0; e < 9; ++e) Dm[e] = d[e]; }
+    else { const float d[9] = {-4.f * qz, -2.f * qw, 2.f * qx, 2.f * qw, -4.f * qz, 2.f * qy, 2.f * qx, 2.f * qy, 0.f}; for (int e = 0; e < 9; ++e) Dm[e] = d[e]; }
+    float dS3[9];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        float v = 0.f;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) v += Dm[3 * r + k] * s2[k] * R[3 * c + k] + R[3 * r + k] * s2[k] * Dm[3 * c + k];
+        dS3[3 * r + c] = v;
+      }
+    sandwich_f(Tm, dS3, dh[i][0], dh[i][1], dh[i][2]);
+  }
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    ch.G[0][6 + j] = 0.f; ch.G[1][6 + j] = 0.f;
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+      float v = 0.f;
+#pragma unroll
+      for (int i = 0; i < 4; ++i) v += dh[i][e] * ((i == j ? 1.f : 0.f) - qh[i] * qh[j]) * iqn;
+      ch.G[2 + e][6 + j] = v;
+    }
+  }
+}
+
+// moments (40) + chain -> packed block H[105]
+__device__ void build_block(const float* mom, const ChainF& ch, float kappa, const float* omega, float* H) {
+  // A: 11 nonzero rows x 6
+  float A[11][6];
+#pragma unroll
+  for (int k = 0; k < 10; ++k) {
+    A[k][0] = ch.G[0][k]; A[k][1] = ch.G[1][k]; A[k][2] = 0.5f * ch.G[2][k]; A[k][3] = ch.G[3][k]; A[k][4] = 0.5f * ch.G[4][k]; A[k][5] = 0.f;
+  }
+#pragma unroll
+  for (int e = 0; e < 5; ++e) A[10][e] = 0.f;
+  A[10][5] = kappa;
+  const int ex[6] = {1, 0, 2, 1, 0, 0}, ey[6] = {0, 1, 0, 1, 2, 0};
+  float Q[6][6];
+#pragma unroll
+  for (int i = 0; i < 6; ++i)
+#pragma unroll
+    for (int j = 0; j < 6; ++j) Q[i][j] = mom[mono_index(ex[i] + ex[j], ey[i] + ey[j])];
+  float AQ[11][6];
+  for (int k = 0; k < 11; ++k)
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+      float v = 0.f;
+#pragma unroll
+      for (int i = 0; i < 6; ++i) v += A[k][i] * Q[i][j];
+      AQ[k][j] = v;
+    }
+  for (int i = 0; i < NBLK; ++i) H[i] = 0.f;
+  for (int k = 0; k < 11; ++k)
+    for (int l = k; l < 11; ++l) {
+      float v = 0.f;
+#pragma unroll
+      for (int j = 0; j < 6; ++j) v += AQ[k][j] * A[l][j];
+      H[tri(k, l)] = v;
+    }
+  const float W2 = mom[MOM_W2];
+  for (int c = 0; c < 4; ++c) {
+    const float om = omega[c];
+    if (om == 0.f) continue;
+    float yv[11];
+    for (int k = 0; k < 11; ++k) {
+      float v = 0.f;
+#pragma unroll
+      for (int i = 0; i < 6; ++i) v += A[k][i] * mom[MOM_X + 6 * c + i];
+      yv[k] = om * v;
+    }
+    if (c < 3) {
+      for (int k = 0; k < 11; ++k) H[tri(k, 11 + c)] += yv[k];
+      H[tri(11 + c, 11 + c)] += om * W2;
+    } else {
+      for (int k = 0; k < 11; ++k)
+        for (int l = k; l < 11; ++l) {
+          const float ek = k < 3 ? ch.dz[k] : 0.f, el = l < 3 ? ch.dz[l] : 0.f;
+          H[tri(k, l)] += yv[k] * el + ek * yv[l] + om * W2 * ek * el;
+        }
+    }
+  }
+}
+
+// log det of a packed SPD 14x14 (upper Cholesky, in place).  Pivots are floored at a tiny positive number.
+__device__ float logdet_packed(float* Mx) {
+  float ld = 0.f;
+  for (int j = 0; j < P; ++j) {
+    float d = Mx[tri(j, j)];
+    for (int k = 0; k < j; ++k) d -= Mx[tri(k, j)] * Mx[tri(k, j)];
+    d = fmaxf(d, 1e-30f);
+    ld += logf(d);
+    const float inv = rsqrtf(d);
+    Mx[tri(j, j)] = d * inv;
+    for (int i = j + 1; i < P; ++i) {
+      float v = Mx[tri(j, i)];
+      for (int k = 0; k < j; ++k) v -= Mx[tri(k, j)] * Mx[tri(k, i)];
+      Mx[tri(j, i)] = v * inv;
+    }
+  }
+  return ld;
+}
+
+__global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam, nbv_config cfg, const uint32_t* __restrict__ ids_sorted,
+                                                     const float* __restrict__ moments, int mode, float* __restrict__ H_T,
+                                                     float* __restrict__ out_blocks, const float* __restrict__ conf,
+                                                     const float* __restrict__ ldT, float* __restrict__ score,
+                                                     float* __restrict__ gains, ViewCounters* counters) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  float gain = 0.f;
+  bool touched = false;
+  if (r < sc.N) {
+    const float* mom = moments + (size_t)r * NMOM;
+    touched = mom[MOM_W2] > 0.f;
+    if (touched) {
+      const uint32_t g = ids_sorted[r];
+      float m[NMOM];
+#pragma unroll
+      for (int i = 0; i < NMOM / 4; ++i) {
+        const float4 v = reinterpret_cast<const float4*>(mom)[i];
+        m[4 * i] = v.x; m[4 * i + 1] = v.y; m[4 * i + 2] = v.z; m[4 * i + 3] = v.w;
+      }
+      ChainF ch;
+      chain_f(cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
+      const float sg = sc.sigma[g];
+      const float kappa = cfg.opacity_coord == 0 ? (1.f - sg) : 1.f / sg;       // R-10
+      float omega[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) omega[c] = ((cfg.channel_mask >> c) & 1) ? cfg.channel_weight[c] : 0.f;
+      float H[NBLK];
+      build_block(m, ch, kappa, omega, H);
+      if (mode == EXPAND_TRAIN) {
+        float* dst = H_T + (size_t)g * NBLK;
+        for (int i = 0; i < NBLK; ++i) dst[i] += H[i];
+      } else if (mode == EXPAND_VIEW) {
+        float* dst = out_blocks + (size_t)g * NBLK;
+        for (int i = 0; i < NBLK; ++i) dst[i] = H[i];
+      } else {
+        const float c = conf[g];
+        if (c > 0.f) {
+          const float* ht = H_T + (size_t)g * NBLK;
+          for (int i = 0; i < NBLK; ++i) H[i] = c * (ht[i] + H[i]);
+          for (int k = 0; k < P; ++k) H[tri(k, k)] += cfg.prior_precision[k];
+          gain = logdet_packed(H) - ldT[g];
+        }
+        if (gains) gains[g] = gain;
+      }
+    }
+  }
+  if (mode == EXPAND_GAIN) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) gain += __shfl_xor_sync(0xffffffffu, gain, o);
+    __shared__ float ws[2];
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = gain;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const float t = ws[0] + ws[1];
+      if (t != 0.f) atomicAdd(score, t);
+    }
+  }
+  const unsigned tm = __ballot_sync(0xffffffffu, touched);
+  if ((threadIdx.x & 31) == 0 && tm) atomicAdd(&counters->n_touched, (unsigned)__popc(tm));
+}
+
+void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
+                   const float* moments, int mode, float* H_T, float* out_blocks, const float* conf, const float* ldT,
+                   float* score, float* gains, ViewCounters* counters, cudaStream_t st) {
+  expand_kernel<<<(sc.N + 63) / 64, 64, 0, st>>>(sc, cam, cfg, ids_sorted, moments, mode, H_T, out_blocks, conf, ldT, score,
+                                                 gains, counters);
+}
+
+// S0': confidence (Eq. 7; Eq. 12)
+__global__ void __launch_bounds__(256) confidence_kernel(SceneDev sc, nbv_config cfg, int target, float* __restrict__ conf) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= sc.N) return;
+  const float s = fmaxf(sc.sigma[g], cfg.sigma_floor);
+  float p, c;
+  if (target < 0) {
+    p = sc.pmax[g];
+  } else {
+    p = expf(sc.logits[(size_t)g * sc.K + target] - sc.lse[g]);
+  }
+  p = fmaxf(p, cfg.p_floor);
+  c = powf(p, -cfg.alpha_obj) * powf(s, -cfg.alpha_opa);
+  if (target >= 0 && sc.amax[g] != target) c = 0.f;
+  conf[g] = c;
+}
+
+void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st) {
+  confidence_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(sc, cfg, target, conf);
+}
+
+// once per scoring call: ldT_g = log det(c_g H_T,g + Lambda)
+__global__ void __launch_bounds__(64) prepare_kernel(int N, nbv_config cfg, const float* __restrict__ H_T, const float* __restrict__ conf,
+                                                      float* __restrict__ ldT) {
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= N) return;
+  const float c = conf[g];
+  float prior_ld = 0.f;
+  for (int k = 0; k < P; ++k) prior_ld += logf(cfg.prior_precision[k]);
+  const float* ht = H_T + (size_t)g * NBLK;
+  float H[NBLK];
+  bool zero = true;
+  for (int i = 0; i < NBLK; ++i) { H[i] = c * ht[i]; zero &= H[i] == 0.f; }
+  if (zero) { ldT[g] = prior_ld; return; }   // never observed in training (or c_g = 0): log det Lambda
+  for (int k = 0; k < P; ++k) H[tri(k, k)] += cfg.prior_precision[k];
+  ldT[g] = logdet_packed(H);
+}
+
+void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* ldT, cudaStream_t st) {
+  prepare_kernel<<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, cfg, H_T, conf, ldT);
+}
+
+// S7: arg-max, lowest index on ties (R-15)
+__global__ void argmax_kernel(const float* __restrict__ scores, int n, int32_t* __restrict__ best) {
+  const int lane = threadIdx.x;
+  float bv = -INFINITY;
+  int bi = 0x7fffffff;
+  for (int i = lane; i < n; i += 32) {
+    const float v = scores[i];
+    if (v > bv || (v == bv && i < bi)) { bv = v; bi = i; }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+    const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+  }
+  if (lane == 0) *best = bi == 0x7fffffff ? 0 : bi;
+}
+
+void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st) { argmax_kernel<<<1, 32, 0, st>>>(scores, n, best); }
+
+}  // namespace nbv

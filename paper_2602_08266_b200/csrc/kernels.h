@@ -1,0 +1,65 @@
+// kernels.h -- host-side launchers of the CUDA kernels (internal to libnbv).
+#pragma once
+#include "common.cuh"
+
+namespace nbv {
+
+// ---- sort.cu
+size_t scan_temp_words(size_t n);
+void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* tmp, uint32_t* total_out, cudaStream_t st);
+size_t radix_temp_words(size_t n);
+// one stable pass over `bits` (<= 8) bits at `shift`; vals_in == nullptr -> keys only
+void radix_pass(const uint32_t* keys_in, uint32_t* keys_out, const uint32_t* vals_in, uint32_t* vals_out, size_t n,
+                int shift, int bits, uint32_t* tmp, cudaStream_t st);
+
+// ---- project.cu
+struct SceneDev {            // device arrays of the loaded map
+  int N, K;
+  const float* mean;         // N x 3
+  const float* logscale;     // N x 3
+  const float* quat;         // N x 4
+  const float* sigma;        // N
+  const float* rgb;          // N x 3
+  const float* logits;       // N x K
+  float* M;                  // N x 9   R(q_hat) diag(s)            (activation output)
+  float* pmax;               // N       max_k softmax
+  int* amax;                 // N       argmax_k (lowest index on ties)
+  float* lse;                // N       log sum exp of the logits
+};
+void launch_activate(const SceneDev& sc, ViewCounters* counters, cudaStream_t st);
+void launch_project(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, Splat* splat, uint32_t* zkey,
+                    uint32_t* ids, ushort4* rect, float* abc, ViewCounters* counters, cudaStream_t st);
+
+// ---- binning.cu
+void launch_gather(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, Splat* splat_sorted,
+                   ushort4* rect_sorted, uint32_t* ntiles_sorted, cudaStream_t st);
+void launch_emit_keys(const ushort4* rect_sorted, const uint32_t* offsets, int N, int tiles_x, int rank_bits,
+                      uint32_t* keys, cudaStream_t st);
+void launch_tile_ranges(const uint32_t* keys, size_t n_keys, int rank_bits, uint2* ranges, int n_tiles, cudaStream_t st);
+void launch_export_lists(const uint32_t* keys, size_t n_keys, int rank_bits, const uint32_t* ids_sorted, const uint2* ranges,
+                         int n_tiles, int64_t* offsets, int32_t* ids_out, uint32_t* tmp_counts, uint32_t* scan_tmp, cudaStream_t st);
+
+// ---- raster.cu
+struct PixelBuf {            // per-pixel outputs of the forward pass (H x W each)
+  float* rgb;                // x3
+  float* depth;
+  float* T;
+  int32_t* ncontrib;
+  int32_t* last;             // list position (relative to the tile's range) after the last composited entry
+};
+void launch_forward(const Splat* splat_sorted, const uint32_t* keys, const uint2* ranges, int rank_bits, int W, int H,
+                    const nbv_config& cfg, PixelBuf px, ViewCounters* counters, cudaStream_t st);
+void launch_backward(const Splat* splat_sorted, const uint32_t* keys, const uint2* ranges, int rank_bits, int W, int H,
+                     const nbv_config& cfg, PixelBuf px, float* moments, cudaStream_t st);
+
+// ---- hessian.cu
+enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2 };
+// EXPAND_TRAIN: H_T[id] += H ; EXPAND_VIEW: out_blocks[id] = H ; EXPAND_GAIN: gain vs H_T, sum into *score (and gains[id] if not null)
+void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
+                   const float* moments, int mode, float* H_T, float* out_blocks, const float* conf, const float* ldT,
+                   float* score, float* gains, ViewCounters* counters, cudaStream_t st);
+void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);
+void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* ldT, cudaStream_t st);
+void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);
+
+}  // namespace nbv

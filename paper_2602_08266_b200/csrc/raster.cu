@@ -1,0 +1,303 @@
+// raster.cu -- S3 front-to-back compositing and S4 back-to-front Jacobian sweep, per 16x16 tile.
+//
+// Mapping: ONE WARP PER TILE, each lane owns a column of 8 pixels
+// (x = lane & 15, rows (lane >> 4) * 8 .. +7).  The tile's depth-sorted splats are staged 32 at a time in
+// shared memory; every lane evaluates each splat at its 8 pixels, so the 40 moment sums of S4 are reduced
+// over 8 pixels in registers before the cross-lane butterfly, and no block-level barrier exists at all.
+//
+// S3 is on the decision path (bit-exact power / alpha / transmittance chain).
+// S4 ("computes the Jacobian of the rendering with respect to Gaussian parameters", L189-191
+// H ~= J^T J, L210 per-Gaussian blocks) does NOT form 14-wide rows per pixel.  With d = p - m, u = Sigma2D^-1 d,
+//   dalpha/d(mx,my,a,b,c,o) = alpha (ux, uy, ux^2/2, ux uy, uy^2/2, kappa),   dy_ch/dalpha_i = beta_ch,
+// the per-pixel row of channel ch is  J_ch = beta_ch * alpha * A m6 + w e_ch  with the monomial vector
+// m6 = (ux, uy, ux^2, ux uy, uy^2, 1), a per-(view, Gaussian) matrix A (14 x 6, applied later in S5) and
+// w = alpha T.  Hence  sum_px sum_ch omega_ch J_ch J_ch^T  needs only
+//   15 sums  sum_px (sum_ch omega_ch beta_ch^2) alpha^2 ux^i uy^j, i + j <= 4
+//    6 sums per channel  sum_px beta_ch w alpha m6
+//    1 sum   sum_px w^2
+// = 40 numbers per (tile, Gaussian) for RGB + depth.  The oracle forms explicit rows instead, so parity
+// checks this algebra.
+#include "kernels.h"
+
+namespace nbv {
+
+constexpr int PPL = 8;                 // pixels per lane
+constexpr unsigned FULL = 0xffffffffu;
+
+struct RasterParams {
+  int W, H, tiles_x, rank_bits;
+  float alpha_min, alpha_max, t_stop;
+  float bg[3];
+  float omega[4];                      // channel weights, 0 for disabled channels
+};
+
+__device__ __forceinline__ void stage_batch(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ keys,
+                                            uint32_t first, uint32_t count, uint32_t rmask, float4* sm, uint32_t* sm_rank) {
+  const int lane = threadIdx.x;
+  if ((uint32_t)lane < count) {
+    const uint32_t r = keys[first + lane] & rmask;
+    const float4* s = reinterpret_cast<const float4*>(splat_sorted + r);
+    sm[lane * 3 + 0] = s[0];
+    sm[lane * 3 + 1] = s[1];
+    sm[lane * 3 + 2] = s[2];
+    if (sm_rank) sm_rank[lane] = r;
+  }
+  __syncwarp();
+}
+
+__global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ keys,
+                                                      const uint2* __restrict__ ranges, RasterParams prm, PixelBuf out,
+                                                      ViewCounters* counters) {
+  __shared__ float4 sm[32 * 3];
+  const int tile = blockIdx.x, lane = threadIdx.x;
+  const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
+  const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
+  const float px = (float)x + 0.5f;
+  const uint2 range = ranges[tile];
+  const uint32_t rmask = (1u << prm.rank_bits) - 1u;
+
+  float T[PPL], C0[PPL], C1[PPL], C2[PPL], D[PPL];
+  int n[PPL], last[PPL];
+  unsigned done = 0;
+#pragma unroll
+  for (int k = 0; k < PPL; ++k) {
+    T[k] = 1.0f; C0[k] = C1[k] = C2[k] = D[k] = 0.0f; n[k] = 0; last[k] = 0;
+    if (x >= prm.W || y0 + k >= prm.H) done |= 1u << k;
+  }
+  uint32_t walked = 0;
+  bool finished = __all_sync(FULL, done == 0xffu);
+  for (uint32_t base = range.x; base < range.y && !finished; base += 32) {
+    const uint32_t cnt = min(32u, range.y - base);
+    stage_batch(splat_sorted, keys, base, cnt, rmask, sm, nullptr);
+    for (uint32_t j = 0; j < cnt; ++j) {
+      const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
+      const int e1 = (int)(base - range.x + j) + 1;
+      ++walked;
+#pragma unroll
+      for (int k = 0; k < PPL; ++k) {
+        if (!((done >> k) & 1u)) {
+          const float dx = sub_rn(px, s0.x), dy = sub_rn((float)(y0 + k) + 0.5f, s0.y);
+          const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
+          if (power <= 0.0f && power >= s1.w) {          // s1.w = tau >= -6: pre-test, never decides (see project.cu)
+            const float a = mul_rn(s1.y, exp_spec(power));
+            if (a >= prm.alpha_min) {
+              const float alpha = fminf(a, prm.alpha_max);
+              const float Tn = mul_rn(T[k], sub_rn(1.0f, alpha));
+              if (Tn < prm.t_stop) {
+                done |= 1u << k;                          // stop BEFORE compositing (R-4)
+              } else {
+                const float w = alpha * T[k];
+                C0[k] = fmaf(s2.x, w, C0[k]); C1[k] = fmaf(s2.y, w, C1[k]); C2[k] = fmaf(s2.z, w, C2[k]);
+                D[k] = fmaf(s1.z, w, D[k]);
+                T[k] = Tn;
+                ++n[k];
+                last[k] = e1;
+              }
+            }
+          }
+        }
+      }
+      if (__all_sync(FULL, done == 0xffu)) { finished = true; break; }
+    }
+    __syncwarp();
+  }
+  unsigned pairs = 0;
+#pragma unroll
+  for (int k = 0; k < PPL; ++k) {
+    pairs += n[k];
+    if (x < prm.W && y0 + k < prm.H) {
+      const size_t p = (size_t)(y0 + k) * prm.W + x;
+      if (out.rgb) {
+        out.rgb[3 * p + 0] = fmaf(prm.bg[0], T[k], C0[k]);
+        out.rgb[3 * p + 1] = fmaf(prm.bg[1], T[k], C1[k]);
+        out.rgb[3 * p + 2] = fmaf(prm.bg[2], T[k], C2[k]);
+      }
+      if (out.depth) out.depth[p] = D[k];
+      out.T[p] = T[k];
+      if (out.ncontrib) out.ncontrib[p] = n[k];
+      out.last[p] = last[k];
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) pairs += __shfl_xor_sync(FULL, pairs, o);
+  if (lane == 0) {
+    atomicAdd(&counters->n_entries, (unsigned long long)walked);
+    atomicAdd(&counters->n_pairs, (unsigned long long)pairs);
+  }
+}
+
+// Sum v[0..39] over the 32 lanes.  On return lane l holds the totals of moments idx0 and idx1 (or -1).
+// 40 shuffles instead of 200: at every level a lane keeps one half of its values and sends the other half.
+__device__ __forceinline__ void butterfly40(const float (&v)[NMOM], int lane, float& o0, float& o1, int& idx0, int& idx1) {
+  float a20[20], a10[10], a5[5], a3[3];
+  bool up = (lane & 16) != 0;
+#pragma unroll
+  for (int i = 0; i < 20; ++i) {
+    const float keep = up ? v[20 + i] : v[i], send = up ? v[i] : v[20 + i];
+    a20[i] = keep + __shfl_xor_sync(FULL, send, 16);
+  }
+  up = (lane & 8) != 0;
+#pragma unroll
+  for (int i = 0; i < 10; ++i) {
+    const float keep = up ? a20[10 + i] : a20[i], send = up ? a20[i] : a20[10 + i];
+    a10[i] = keep + __shfl_xor_sync(FULL, send, 8);
+  }
+  up = (lane & 4) != 0;
+#pragma unroll
+  for (int i = 0; i < 5; ++i) {
+    const float keep = up ? a10[5 + i] : a10[i], send = up ? a10[i] : a10[5 + i];
+    a5[i] = keep + __shfl_xor_sync(FULL, send, 4);
+  }
+  up = (lane & 2) != 0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    const float hi = (i < 2) ? a5[3 + i] : 0.0f;     // 5 -> 3 + 3 (one pad)
+    const float keep = up ? hi : a5[i], send = up ? a5[i] : hi;
+    a3[i] = keep + __shfl_xor_sync(FULL, send, 2);
+  }
+  up = (lane & 1) != 0;
+  {
+    const float keep0 = up ? a3[2] : a3[0], send0 = up ? a3[0] : a3[2];
+    const float keep1 = up ? 0.0f : a3[1], send1 = up ? a3[1] : 0.0f;   // 3 -> 2 + 2 (one pad)
+    o0 = keep0 + __shfl_xor_sync(FULL, send0, 1);
+    o1 = keep1 + __shfl_xor_sync(FULL, send1, 1);
+  }
+  const int b16 = (lane >> 4) & 1, b8 = (lane >> 3) & 1, b4 = (lane >> 2) & 1, b2 = (lane >> 1) & 1, b1 = lane & 1;
+  const int basei = 20 * b16 + 10 * b8 + 5 * b4 + 3 * b2;
+  const int s0 = 2 * b1, s1 = 2 * b1 + 1;
+  idx0 = (s0 < 3 && 3 * b2 + s0 < 5) ? basei + s0 : -1;
+  idx1 = (s1 < 3 && 3 * b2 + s1 < 5) ? basei + s1 : -1;
+}
+
+template <int NCH>
+__global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ keys,
+                                                       const uint2* __restrict__ ranges, RasterParams prm, PixelBuf pix,
+                                                       float* __restrict__ moments) {
+  __shared__ float4 sm[32 * 3];
+  __shared__ uint32_t sm_rank[32];
+  const int tile = blockIdx.x, lane = threadIdx.x;
+  const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
+  const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
+  const float px = (float)x + 0.5f;
+  const uint2 range = ranges[tile];
+  const uint32_t rmask = (1u << prm.rank_bits) - 1u;
+
+  float Tc[PPL], S0[PPL], S1[PPL], S2[PPL], S3[PPL];
+  int last[PPL];
+  int maxlast = 0;
+#pragma unroll
+  for (int k = 0; k < PPL; ++k) {
+    last[k] = 0; Tc[k] = 1.0f;
+    if (x < prm.W && y0 + k < prm.H) {
+      const size_t p = (size_t)(y0 + k) * prm.W + x;
+      last[k] = pix.last[p];
+      Tc[k] = pix.T[p];
+    }
+    S0[k] = prm.bg[0] * Tc[k]; S1[k] = prm.bg[1] * Tc[k]; S2[k] = prm.bg[2] * Tc[k]; S3[k] = 0.0f;
+    maxlast = max(maxlast, last[k]);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) maxlast = max(maxlast, __shfl_xor_sync(FULL, maxlast, o));
+  if (maxlast == 0) return;
+
+  for (int bb = (maxlast - 1) / 32; bb >= 0; --bb) {
+    const int base_e = bb * 32;
+    const int cnt = min(32, maxlast - base_e);
+    stage_batch(splat_sorted, keys, range.x + (uint32_t)base_e, (uint32_t)cnt, rmask, sm, sm_rank);
+    for (int j = cnt - 1; j >= 0; --j) {
+      const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
+      const int e = base_e + j;
+      const float cA = -2.0f * s0.z, cB = -s0.w, cC = -2.0f * s1.x;    // conic = Sigma2D^-1
+      float acc[NMOM];
+#pragma unroll
+      for (int m = 0; m < NMOM; ++m) acc[m] = 0.0f;
+      bool any = false;
+#pragma unroll
+      for (int k = 0; k < PPL; ++k) {
+        if (e < last[k]) {
+          const float dx = sub_rn(px, s0.x), dy = sub_rn((float)(y0 + k) + 0.5f, s0.y);
+          const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
+          if (power <= 0.0f && power >= s1.w) {
+            const float a = mul_rn(s1.y, exp_spec(power));
+            if (a >= prm.alpha_min) {                      // same tests as S3 -> same contributor set
+              any = true;
+              const bool clamped = a > prm.alpha_max;
+              const float alpha = fminf(a, prm.alpha_max);
+              const float rc = __fdividef(1.0f, 1.0f - alpha);
+              const float Ti = Tc[k] * rc;                 // T_i = T_{i+1} / (1 - alpha_i)
+              const float w = alpha * Ti;
+              // beta_ch = dy_ch/dalpha_i = T_i v_i - Splus_i / (1 - alpha_i)
+              const float b0 = Ti * s2.x - S0[k] * rc, b1 = Ti * s2.y - S1[k] * rc, b2 = Ti * s2.z - S2[k] * rc;
+              S0[k] = fmaf(s2.x, w, S0[k]); S1[k] = fmaf(s2.y, w, S1[k]); S2[k] = fmaf(s2.z, w, S2[k]);
+              float b3 = 0.0f;
+              if (NCH == 4) { b3 = Ti * s1.z - S3[k] * rc; S3[k] = fmaf(s1.z, w, S3[k]); }
+              Tc[k] = Ti;
+              acc[MOM_W2] = fmaf(w, w, acc[MOM_W2]);
+              if (!clamped) {                              // R-11: zero derivative at the 0.99 cap
+                const float ux = cA * dx + cB * dy, uy = cB * dx + cC * dy;
+                float B = prm.omega[0] * b0 * b0 + prm.omega[1] * b1 * b1 + prm.omega[2] * b2 * b2;
+                if (NCH == 4) B = fmaf(prm.omega[3] * b3, b3, B);
+                const float f = B * alpha * alpha;
+                const float ux2 = ux * ux, uxy = ux * uy, uy2 = uy * uy;
+                const float f10 = f * ux, f01 = f * uy, f20 = f * ux2, f11 = f * uxy, f02 = f * uy2;
+                acc[0] += f; acc[1] += f10; acc[2] += f01; acc[3] += f20; acc[4] += f11; acc[5] += f02;
+                acc[6] = fmaf(f20, ux, acc[6]); acc[7] = fmaf(f20, uy, acc[7]); acc[8] = fmaf(f02, ux, acc[8]); acc[9] = fmaf(f02, uy, acc[9]);
+                acc[10] = fmaf(f20, ux2, acc[10]); acc[11] = fmaf(f20, uxy, acc[11]); acc[12] = fmaf(f20, uy2, acc[12]);
+                acc[13] = fmaf(f02, uxy, acc[13]); acc[14] = fmaf(f02, uy2, acc[14]);
+                const float wa = w * alpha;
+                const float bch[4] = {b0, b1, b2, b3};
+#pragma unroll
+                for (int c = 0; c < NCH; ++c) {
+                  const float g = bch[c] * wa;
+                  acc[MOM_X + 6 * c + 0] = fmaf(g, ux, acc[MOM_X + 6 * c + 0]);
+                  acc[MOM_X + 6 * c + 1] = fmaf(g, uy, acc[MOM_X + 6 * c + 1]);
+                  acc[MOM_X + 6 * c + 2] = fmaf(g, ux2, acc[MOM_X + 6 * c + 2]);
+                  acc[MOM_X + 6 * c + 3] = fmaf(g, uxy, acc[MOM_X + 6 * c + 3]);
+                  acc[MOM_X + 6 * c + 4] = fmaf(g, uy2, acc[MOM_X + 6 * c + 4]);
+                  acc[MOM_X + 6 * c + 5] += g;
+                }
+              }
+            }
+          }
+        }
+      }
+      if (__any_sync(FULL, any)) {
+        float o0, o1;
+        int i0, i1;
+        butterfly40(acc, lane, o0, o1, i0, i1);
+        float* dst = moments + (size_t)sm_rank[j] * NMOM;
+        if (i0 >= 0) atomicAdd(dst + i0, o0);
+        if (i1 >= 0) atomicAdd(dst + i1, o1);
+      }
+    }
+    __syncwarp();
+  }
+}
+
+static RasterParams make_params(int rank_bits, int W, int H, const nbv_config& cfg) {
+  RasterParams p;
+  p.W = W; p.H = H; p.tiles_x = (W + TILE - 1) / TILE; p.rank_bits = rank_bits;
+  p.alpha_min = cfg.alpha_min; p.alpha_max = cfg.alpha_max; p.t_stop = cfg.t_stop;
+  for (int c = 0; c < 3; ++c) p.bg[c] = cfg.bg[c];
+  for (int c = 0; c < 4; ++c) p.omega[c] = ((cfg.channel_mask >> c) & 1) ? cfg.channel_weight[c] : 0.0f;
+  return p;
+}
+
+void launch_forward(const Splat* splat_sorted, const uint32_t* keys, const uint2* ranges, int rank_bits, int W, int H,
+                    const nbv_config& cfg, PixelBuf px, ViewCounters* counters, cudaStream_t st) {
+  const RasterParams p = make_params(rank_bits, W, H, cfg);
+  const int tiles = p.tiles_x * ((H + TILE - 1) / TILE);
+  forward_kernel<<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, counters);
+}
+
+void launch_backward(const Splat* splat_sorted, const uint32_t* keys, const uint2* ranges, int rank_bits, int W, int H,
+                     const nbv_config& cfg, PixelBuf px, float* moments, cudaStream_t st) {
+  const RasterParams p = make_params(rank_bits, W, H, cfg);
+  const int tiles = p.tiles_x * ((H + TILE - 1) / TILE);
+  if (cfg.channel_mask & NBV_CH_DEPTH)
+    backward_kernel<4><<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, moments);
+  else
+    backward_kernel<3><<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, moments);
+}
+
+}  // namespace nbv

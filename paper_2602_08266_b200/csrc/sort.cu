@@ -1,0 +1,230 @@
+// sort.cu -- S2 primitives: device exclusive scan and a stable LSD radix sort pass (hand-written, sm_100a).
+//
+// The (tile, depth) sort of B: north_star is done as an LSD radix sort whose least significant digits (the
+// depth key) are sorted BEFORE the Gaussians are duplicated into tiles: N 32-bit depth keys with their
+// Gaussian index (4 passes of 8 bits), then keys (tile << rank_bits | depth_rank) are emitted in depth-rank
+// order and only the tile digit is sorted, by stable passes.  Stability makes the result identical to a full
+// sort on (tile, z bits, index) -- the definition of the tile lists (R-5, R-7).
+#include "kernels.h"
+
+namespace nbv {
+
+// ------------------------------------------------------------------------------------------------
+// exclusive scan (uint32), any length < 2^32: reduce -> (recursive) scan of block sums -> downsweep
+// ------------------------------------------------------------------------------------------------
+constexpr int SCAN_T = 256;
+constexpr int SCAN_I = 8;
+constexpr int SCAN_TILE = SCAN_T * SCAN_I;
+
+// exclusive prefix of v over the block; total = block sum.  sm must hold 32 words.
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* sm, uint32_t& total) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  uint32_t x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += y;
+  }
+  if (lane == 31) sm[wid] = x;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t w = lane < nw ? sm[lane] : 0u;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      uint32_t y = __shfl_up_sync(0xffffffffu, w, o);
+      if (lane >= o) w += y;
+    }
+    sm[lane] = w;
+  }
+  __syncthreads();
+  uint32_t woff = wid > 0 ? sm[wid - 1] : 0u;
+  total = sm[nw - 1];
+  __syncthreads();
+  return woff + x - v;
+}
+
+__global__ void __launch_bounds__(SCAN_T) scan_reduce_kernel(const uint32_t* __restrict__ in, uint32_t n,
+                                                              uint32_t* __restrict__ sums) {
+  __shared__ uint32_t sm[32];
+  const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_I;
+  uint32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_I; ++i) {
+    uint32_t idx = base + i;
+    s += idx < n ? in[idx] : 0u;
+  }
+  uint32_t total;
+  block_exclusive_scan(s, sm, total);
+  if (threadIdx.x == 0) sums[blockIdx.x] = total;
+}
+
+// out[i] = offsets[block] + exclusive prefix within the block.  offsets == nullptr -> 0.
+// If total_out != nullptr the last block also writes the grand total there (as uint32).
+__global__ void __launch_bounds__(SCAN_T) scan_downsweep_kernel(const uint32_t* in, uint32_t* out,
+                                                                 uint32_t n, const uint32_t* __restrict__ offsets,
+                                                                 uint32_t* __restrict__ total_out) {
+  __shared__ uint32_t sm[32];
+  const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_I;
+  uint32_t v[SCAN_I];
+  uint32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_I; ++i) {
+    uint32_t idx = base + i;
+    v[i] = idx < n ? in[idx] : 0u;
+    s += v[i];
+  }
+  uint32_t total;
+  uint32_t ex = block_exclusive_scan(s, sm, total);
+  uint32_t off = (offsets ? offsets[blockIdx.x] : 0u) + ex;
+#pragma unroll
+  for (int i = 0; i < SCAN_I; ++i) {
+    uint32_t idx = base + i;
+    if (idx < n) out[idx] = off;
+    off += v[i];
+  }
+  if (total_out && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *total_out = (offsets ? offsets[blockIdx.x] : 0u) + total;
+}
+
+size_t scan_temp_words(size_t n) {
+  size_t words = 0;
+  while (n > (size_t)SCAN_TILE) {
+    n = (n + SCAN_TILE - 1) / SCAN_TILE;
+    words += n;
+  }
+  return words + 1;
+}
+
+void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* tmp, uint32_t* total_out, cudaStream_t st) {
+  if (n == 0) {
+    if (total_out) cudaMemsetAsync(total_out, 0, 4, st);
+    return;
+  }
+  const uint32_t nb = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
+  if (nb == 1) {
+    scan_downsweep_kernel<<<1, SCAN_T, 0, st>>>(in, out, (uint32_t)n, nullptr, total_out);
+    return;
+  }
+  uint32_t* sums = tmp;
+  scan_reduce_kernel<<<nb, SCAN_T, 0, st>>>(in, (uint32_t)n, sums);
+  exclusive_scan_u32(sums, sums, nb, tmp + nb, nullptr, st);
+  scan_downsweep_kernel<<<nb, SCAN_T, 0, st>>>(in, out, (uint32_t)n, sums, total_out);
+}
+
+// ------------------------------------------------------------------------------------------------
+// one stable radix pass on `bits` (<= 8) bits at `shift`
+// ------------------------------------------------------------------------------------------------
+constexpr int RS_T = 256;
+constexpr int RS_I = 16;
+constexpr int RS_TILE = RS_T * RS_I;   // 4096 keys per block
+constexpr int RS_W = RS_T / 32;        // 8 warps, 512 consecutive keys each
+
+__global__ void __launch_bounds__(RS_T) radix_hist_kernel(const uint32_t* __restrict__ keys, uint32_t n, int shift,
+                                                           uint32_t mask, uint32_t* __restrict__ hist, uint32_t nblocks) {
+  __shared__ uint32_t h[256];
+  h[threadIdx.x] = 0;
+  __syncthreads();
+  const uint32_t base = blockIdx.x * RS_TILE;
+#pragma unroll
+  for (int i = 0; i < RS_I; ++i) {
+    uint32_t idx = base + i * RS_T + threadIdx.x;
+    if (idx < n) atomicAdd(&h[(keys[idx] >> shift) & mask], 1u);
+  }
+  __syncthreads();
+  if (threadIdx.x <= mask) hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
+}
+
+template <bool HAS_VALS>
+__global__ void __launch_bounds__(RS_T) radix_scatter_kernel(const uint32_t* __restrict__ keys_in, uint32_t* __restrict__ keys_out,
+                                                              const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ vals_out,
+                                                              uint32_t n, int shift, uint32_t mask,
+                                                              const uint32_t* __restrict__ hist_scanned, uint32_t nblocks) {
+  __shared__ uint32_t wh[RS_W][256];     // per-warp digit counts, then per-warp digit bases
+  __shared__ uint32_t dstart[256];       // block-local start of each digit's run
+  __shared__ uint32_t gofs[256];         // global position of local slot i with digit d = gofs[d] + i
+  __shared__ uint32_t sm_scan[32];
+  __shared__ uint32_t skeys[RS_TILE];
+  __shared__ uint32_t svals[HAS_VALS ? RS_TILE : 1];
+
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const uint32_t lt = (1u << lane) - 1u;
+  for (int i = tid; i < RS_W * 256; i += RS_T) (&wh[0][0])[i] = 0;
+  __syncthreads();
+
+  const uint32_t base = blockIdx.x * RS_TILE + w * (RS_TILE / RS_W);
+  uint32_t k[RS_I];
+  uint32_t rk[RS_I];
+  // phase 1: rank every key among the keys of its warp with the same digit, in memory order
+#pragma unroll
+  for (int r = 0; r < RS_I; ++r) {
+    const uint32_t idx = base + r * 32 + lane;
+    const bool valid = idx < n;
+    k[r] = valid ? keys_in[idx] : 0xffffffffu;
+    const uint32_t d = valid ? ((k[r] >> shift) & mask) : 0x100u;
+    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    const uint32_t pre = valid ? wh[w][d] : 0u;
+    __syncwarp();
+    rk[r] = pre + __popc(peers & lt);
+    if (valid && lane == __ffs(peers) - 1) wh[w][d] = pre + __popc(peers);
+    __syncwarp();
+  }
+  __syncthreads();
+  // phase 2: per digit, prefix over warps; then prefix over digits
+  uint32_t bt = 0;
+  if ((uint32_t)tid <= mask) {
+#pragma unroll
+    for (int w2 = 0; w2 < RS_W; ++w2) {
+      uint32_t t = wh[w2][tid];
+      wh[w2][tid] = bt;
+      bt += t;
+    }
+  }
+  uint32_t total;
+  uint32_t ds = block_exclusive_scan(bt, sm_scan, total);
+  if ((uint32_t)tid <= mask) {
+    dstart[tid] = ds;
+    gofs[tid] = hist_scanned[(size_t)tid * nblocks + blockIdx.x] - ds;
+  }
+  __syncthreads();
+  // phase 3: stage in shared memory in sorted order
+#pragma unroll
+  for (int r = 0; r < RS_I; ++r) {
+    const uint32_t idx = base + r * 32 + lane;
+    if (idx < n) {
+      const uint32_t d = (k[r] >> shift) & mask;
+      const uint32_t lpos = dstart[d] + wh[w][d] + rk[r];
+      skeys[lpos] = k[r];
+      if (HAS_VALS) svals[lpos] = vals_in[idx];
+    }
+  }
+  __syncthreads();
+  // phase 4: coalesced runs to global
+  for (uint32_t i = tid; i < total; i += RS_T) {
+    const uint32_t key = skeys[i];
+    const uint32_t pos = gofs[(key >> shift) & mask] + i;
+    keys_out[pos] = key;
+    if (HAS_VALS) vals_out[pos] = svals[i];
+  }
+}
+
+size_t radix_temp_words(size_t n) {
+  size_t nb = (n + RS_TILE - 1) / RS_TILE;
+  size_t hist = 256 * nb;
+  return hist + scan_temp_words(hist);
+}
+
+void radix_pass(const uint32_t* keys_in, uint32_t* keys_out, const uint32_t* vals_in, uint32_t* vals_out, size_t n,
+                int shift, int bits, uint32_t* tmp, cudaStream_t st) {
+  if (n == 0) return;
+  const uint32_t nb = (uint32_t)((n + RS_TILE - 1) / RS_TILE);
+  const uint32_t mask = (1u << bits) - 1u;
+  const size_t hist_n = (size_t)(mask + 1) * nb;
+  uint32_t* hist = tmp;
+  radix_hist_kernel<<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, shift, mask, hist, nb);
+  exclusive_scan_u32(hist, hist, hist_n, tmp + 256 * (size_t)nb, nullptr, st);
+  if (vals_in)
+    radix_scatter_kernel<true><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, shift, mask, hist, nb);
+  else
+    radix_scatter_kernel<false><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, shift, mask, hist, nb);
+}
+
+}  // namespace nbv

@@ -1,0 +1,245 @@
+"""GPU-vs-oracle parity through the C ABI (B: north_star tolerances).
+
+  tile lists, depth order, per-pixel contributor counts, projected splats : bit-exact
+  rendered colour / depth / transmittance                                  : 1e-5 abs
+  Hessian blocks                                                           : 1e-3 relative (1e-6 abs floor)
+  information gains                                                        : 1e-3 relative (1e-6 abs floor)
+  chosen next-best-view index                                              : identical
+
+"Relative" for a block entry (k,l) is taken against sqrt(H_kk H_ll), the Cauchy-Schwarz scale of that entry
+(off-diagonal entries are sums with cancellation; their own magnitude is not a scale).
+"""
+import numpy as np
+import pytest
+
+from oracle import nbv_oracle as orc
+from paper_2602_08266_b200 import synth
+from conftest import make_oracle_scene, scene_from_arrays
+
+pytestmark = pytest.mark.gpu
+
+P, NB = 14, 105
+
+
+def _nbv(scene, channel_mask=7, **kw):
+    from paper_2602_08266_b200 import api
+    n = api.NBV(channel_mask=channel_mask, **kw)
+    n.load_scene(scene)
+    return n
+
+
+def block_rel_err(Hg, Ho):
+    """max over entries of |Hg - Ho| / (sqrt(Ho_kk Ho_ll) + floor), per Gaussian"""
+    Fo = orc.unpack_blocks(Ho)
+    d = np.sqrt(np.maximum(np.einsum("nii->ni", Fo), 0))
+    scale = orc.pack_blocks(d[:, :, None] * d[:, None, :])
+    return np.abs(Hg - Ho) / (scale + 1e-6 / 1e-3)
+
+
+CASES = [
+    # (scene builder, camera builder, channel mask)
+    ("cfg0_train", lambda: synth.make_workload(0), 7),
+    ("cfg0_rgbd", lambda: synth.make_workload(0), 15),
+]
+
+
+def _ragged_camera():
+    # 70 x 50: ragged right / bottom tiles (5 x 4 tiles, the last ones partly outside the image)
+    return synth.hemisphere_cameras(1, (0.6, 0.6), 70, 50, 60.0, 60.0, np.random.default_rng(5))[0]
+
+
+@pytest.fixture(scope="module")
+def wl():
+    return synth.make_workload(0)
+
+
+@pytest.mark.parametrize("which", ["train0", "cand2", "ragged"])
+def test_projection_order_and_tile_lists_bit_exact(wl, which):
+    cam = {"train0": wl.train_cams[0], "cand2": wl.cand_cams[2], "ragged": _ragged_camera()}[which]
+    scn = make_oracle_scene(wl.scene)
+    nbv = _nbv(wl.scene)
+    vis_o, rec_o, rect_o = scn.project(cam)
+    vis_g, rec_g, rect_g = [t.cpu().numpy() for t in nbv.projected(cam)]
+    np.testing.assert_array_equal(vis_g, vis_o)
+    v = vis_o > 0
+    np.testing.assert_array_equal(rec_g[v].view(np.uint32), rec_o[v].view(np.uint32))  # bit-exact floats
+    np.testing.assert_array_equal(rect_g[v], rect_o[v])
+    off_o, ids_o = scn.tile_lists(cam)
+    off_g, ids_g = [t.cpu().numpy() for t in nbv.tile_lists(cam)]
+    np.testing.assert_array_equal(off_g, off_o)
+    np.testing.assert_array_equal(ids_g, ids_o)
+    st = nbv.last_view_stats()
+    assert st["n_visible"] == int(v.sum()) and st["n_keys"] == len(ids_o)
+
+
+@pytest.mark.parametrize("which,mask", [("train0", 7), ("cand1", 15), ("ragged", 15)])
+def test_render_and_contributor_counts(wl, which, mask):
+    cam = {"train0": wl.train_cams[0], "cand1": wl.cand_cams[1], "ragged": _ragged_camera()}[which]
+    bg = (0.2, 0.4, 0.6)
+    scn = make_oracle_scene(wl.scene, channel_mask=mask, bg=bg)
+    nbv = _nbv(wl.scene, channel_mask=mask, bg=bg)
+    ro = scn.render(cam)
+    rg = {k: v.cpu().numpy() for k, v in nbv.render(cam).items()}
+    np.testing.assert_array_equal(rg["ncontrib"], ro["ncontrib"])                       # bit-exact
+    np.testing.assert_array_equal(rg["T"].view(np.uint32), ro["T32"].view(np.uint32))   # decision-path transmittance
+    np.testing.assert_allclose(rg["rgb"], ro["rgb"], rtol=0, atol=1e-5)
+    np.testing.assert_allclose(rg["depth"], ro["depth"], rtol=0, atol=1e-5)
+    assert nbv.last_view_stats()["n_pairs"] == int(ro["ncontrib"].sum())
+
+
+@pytest.mark.parametrize("which,mask,coord", [("train0", 7, 0), ("cand3", 15, 0), ("ragged", 15, 1), ("cand0", 8, 0)])
+def test_view_hessian_blocks(wl, which, mask, coord):
+    cam = {"train0": wl.train_cams[0], "cand3": wl.cand_cams[3], "cand0": wl.cand_cams[0], "ragged": _ragged_camera()}[which]
+    kw = dict(bg=(0.1, 0.2, 0.3), opacity_coord=coord, channel_weight=(1.0, 0.5, 2.0, 3.0))
+    scn = make_oracle_scene(wl.scene, channel_mask=mask, **kw)
+    nbv = _nbv(wl.scene, channel_mask=mask, **kw)
+    Ho = scn.view_hessian(cam)
+    Hg = nbv.view_hessian(cam).cpu().numpy().astype(np.float64)
+    touched_o = np.abs(Ho).sum(axis=1) > 0
+    touched_g = np.abs(Hg).sum(axis=1) > 0
+    np.testing.assert_array_equal(touched_g, touched_o)
+    err = block_rel_err(Hg, Ho)
+    assert err.max() < 1e-3, (err.max(), np.unravel_index(err.argmax(), err.shape))
+    assert nbv.last_view_stats()["n_touched"] == int(touched_o.sum())
+
+
+def test_training_accumulation_and_gains_and_argmax(wl):
+    scn = make_oracle_scene(wl.scene)
+    nbv = _nbv(wl.scene)
+    # two training views (the config's one + a candidate) so that H_T is a sum
+    train = np.concatenate([wl.train_cams, wl.cand_cams[3:4]])
+    nbv.accumulate_training(train)
+    res = orc.score_candidates(scn, train, wl.cand_cams)
+    HT = nbv.training_hessian().cpu().numpy().astype(np.float64)
+    assert block_rel_err(HT, res["H_T"]).max() < 1e-3
+    conf = nbv.confidence(-1).cpu().numpy()
+    np.testing.assert_allclose(conf, res["conf"], rtol=2e-6)
+    scores, best = nbv.score_candidates(wl.cand_cams)
+    scores = scores.cpu().numpy()
+    np.testing.assert_allclose(scores, res["scores"], rtol=1e-3, atol=1e-6)
+    assert int(best.item()) == res["best"]
+    hs, hb = nbv.score_candidates_host(wl.cand_cams)
+    np.testing.assert_allclose(hs, scores, rtol=1e-5)
+    assert hb == res["best"]
+    # per-Gaussian terms of one candidate
+    g = nbv.gaussian_gains(wl.cand_cams[1]).cpu().numpy()
+    go = res["gains"][1]
+    np.testing.assert_array_equal(g != 0, go != 0)
+    np.testing.assert_allclose(g, go, rtol=1e-3, atol=1e-3 * np.abs(go).max() * 1e-2 + 1e-6)
+
+
+def test_object_centric_scoring(wl):
+    scn = make_oracle_scene(wl.scene)
+    nbv = _nbv(wl.scene)
+    nbv.accumulate_training(wl.train_cams)
+    for tgt in (0, 2):
+        res = orc.score_candidates(scn, wl.train_cams, wl.cand_cams, target=tgt)
+        conf = nbv.confidence(tgt).cpu().numpy()
+        np.testing.assert_array_equal(conf == 0, res["conf"] == 0)
+        np.testing.assert_allclose(conf, res["conf"], rtol=5e-6)
+        scores, best = nbv.score_candidates(wl.cand_cams, target_obj=tgt)
+        np.testing.assert_allclose(scores.cpu().numpy(), res["scores"], rtol=1e-3, atol=1e-6)
+        assert int(best.item()) == res["best"]
+        g = nbv.gaussian_gains(wl.cand_cams[0], target_obj=tgt).cpu().numpy()
+        assert np.all(g[res["conf"] == 0] == 0)  # Eq. 12: non-target Gaussians contribute exactly 0
+
+
+def test_scoring_without_training_views_uses_the_prior_only(wl):
+    scn = make_oracle_scene(wl.scene)
+    nbv = _nbv(wl.scene)
+    res = orc.score_candidates(scn, wl.train_cams[:0], wl.cand_cams[:2])
+    scores, best = nbv.score_candidates(wl.cand_cams[:2])
+    np.testing.assert_allclose(scores.cpu().numpy(), res["scores"], rtol=1e-3, atol=1e-6)
+    assert int(best.item()) == res["best"]
+
+
+def test_reset_training_and_repeatability(wl):
+    nbv = _nbv(wl.scene)
+    nbv.accumulate_training(wl.train_cams)
+    s1, b1 = nbv.score_candidates(wl.cand_cams)
+    s1 = s1.cpu().numpy().copy()
+    nbv.reset_training()
+    assert float(nbv.training_hessian().abs().sum()) == 0.0
+    nbv.accumulate_training(wl.train_cams)
+    s2, b2 = nbv.score_candidates(wl.cand_cams)
+    np.testing.assert_allclose(s2.cpu().numpy(), s1, rtol=1e-5)  # float atomics: order varies, values agree
+    assert int(b1.item()) == int(b2.item())
+
+
+# ------------------------------------------------------------------ micro scenes and edge cases
+def test_micro_scenes_match_the_oracle():
+    for n, seed, size in ((1, 0, 12), (2, 1, 8), (5, 3, 33)):
+        sc = synth.micro_scene(n, seed)
+        cam = synth.simple_camera(size, size, 40.0, dist=0.5)
+        scn = make_oracle_scene(sc, channel_mask=15)
+        nbv = _nbv(sc, channel_mask=15)
+        ro = scn.render(cam)
+        rg = {k: v.cpu().numpy() for k, v in nbv.render(cam).items()}
+        np.testing.assert_array_equal(rg["ncontrib"], ro["ncontrib"])
+        np.testing.assert_allclose(rg["rgb"], ro["rgb"], atol=1e-5, rtol=0)
+        Ho = scn.view_hessian(cam)
+        Hg = nbv.view_hessian(cam).cpu().numpy().astype(np.float64)
+        assert block_rel_err(Hg, Ho).max() < 1e-3
+
+
+def test_empty_view_and_all_culled():
+    cam = synth.simple_camera(40, 24, 50.0, dist=0.0)
+    sc = scene_from_arrays([[0, 0, -1.0], [0, 0, 0.005]], [[-3] * 3] * 2, [[1, 0, 0, 0]] * 2, [0.5, 0.5], [[1, 1, 1]] * 2)
+    nbv = _nbv(sc, bg=(0.1, 0.2, 0.3))
+    r = {k: v.cpu().numpy() for k, v in nbv.render(cam).items()}
+    assert np.all(r["ncontrib"] == 0) and np.all(r["T"] == 1.0) and np.all(r["depth"] == 0)
+    np.testing.assert_allclose(r["rgb"], np.broadcast_to(np.float32([0.1, 0.2, 0.3]), r["rgb"].shape))
+    off, ids = nbv.tile_lists(cam)
+    assert int(off[-1]) == 0 and ids.numel() == 0
+    assert float(nbv.view_hessian(cam).abs().sum()) == 0.0
+    scores, best = nbv.score_candidates([cam, cam])
+    assert np.all(scores.cpu().numpy() == 0) and int(best.item()) == 0  # tie -> lowest index
+
+
+def test_clamped_opaque_gaussian_and_stacked_half_alphas():
+    cam = synth.simple_camera(32, 32, 100.0, dist=0.0)
+    f = 100.0
+    on = lambda ix, iy, z: [((ix + 0.5) - 16) * z / f, ((iy + 0.5) - 16) * z / f, z]
+    sc = scene_from_arrays([on(16, 16, 1.0), on(16, 16, 2.0), on(5, 7, 1.5)], [[-3] * 3] * 3, [[1, 0, 0, 0]] * 3,
+                           [0.5, 0.5, 0.999999], [[1, 0, 0], [0, 1, 0], [1, 1, 1]])
+    scn = make_oracle_scene(sc, channel_mask=15)
+    nbv = _nbv(sc, channel_mask=15)
+    r = {k: v.cpu().numpy() for k, v in nbv.render(cam).items()}
+    assert 1.0 - r["T"][16, 16] == pytest.approx(0.75, abs=2e-6)
+    assert 1.0 - r["T"][7, 5] == pytest.approx(0.99, abs=1e-6)
+    Ho = scn.view_hessian(cam)
+    Hg = nbv.view_hessian(cam).cpu().numpy().astype(np.float64)
+    assert block_rel_err(Hg, Ho).max() < 1e-3
+
+
+def test_error_codes():
+    from paper_2602_08266_b200 import api
+    wl = synth.make_workload(0)
+    n = api.NBV()
+    with pytest.raises(api.NBVError) as e:
+        n.accumulate_training(wl.train_cams)
+    assert e.value.status == "NBV_ERR_NOT_LOADED"
+    bad = wl.scene.subset(np.arange(10))
+    bad.quat[3] = 0
+    with pytest.raises(api.NBVError) as e:
+        n.load_scene(bad)
+    assert e.value.status == "NBV_ERR_BAD_DATA"
+    bad = wl.scene.subset(np.arange(10))
+    bad.opacity[2] = 1.0
+    with pytest.raises(api.NBVError) as e:
+        n.load_scene(bad)
+    assert e.value.status == "NBV_ERR_BAD_DATA"
+    n.load_scene(wl.scene)
+    with pytest.raises(api.NBVError) as e:
+        n.score_candidates(wl.cand_cams[:0])
+    assert e.value.status == "NBV_ERR_EMPTY_CANDIDATES"
+    with pytest.raises(api.NBVError) as e:
+        n.score_candidates(wl.cand_cams, target_obj=3)
+    assert e.value.status == "NBV_ERR_UNKNOWN_TARGET"
+    cam = wl.cand_cams[:1].copy()
+    cam["R"][0][0] = 2.0
+    with pytest.raises(api.NBVError) as e:
+        n.score_candidates(cam)
+    assert e.value.status == "NBV_ERR_INVALID_ARG"
+    with pytest.raises(api.NBVError):
+        api.NBV(alpha_min=0.001)  # below 1/255: the support bound is built for 1/255
