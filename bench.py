@@ -1,0 +1,346 @@
+#!/usr/bin/env python
+"""bench.py -- candidate views scored per second (Hessian + information gain) on synthetic clutter scenes.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
+
+A STEP is one pass of the whole hot path over one batch: nbv_score_candidates() on the C candidate cameras of
+the workload (S0' confidence + factorisation, then S1..S6 per view, S7 arg-max), against the training Hessian
+accumulated (untimed set-up) from the workload's training cameras.  The default workload is BASELINE.json
+configs[2] (200,000 Gaussians, 20 objects, 1280x720, 20 training + 64 candidate cameras, RGB + depth): the
+configuration north_star quotes its roofline target on.  Inputs are seeded and synthetic (paper_2602_08266_b200.synth).
+
+`value`   : views/s with the Gaussians, H_T and all work buffers resident in HBM, device-timed per step.
+`e2e`     : the same through nbv_score_candidates_host: host camera structs in, host scores + best index out,
+            host<->device copies and the final synchronisation inside the timed region.
+`roofline`: the dominant stage, its algorithmic work over its CUDA-event time.
+`cpu_baseline`: the oracle (oracle/, as it stands) on the host cores, on a bounded sample of the same workload.
+`--impl reference` times the oracle alone (this tier has no reference implementation).
+N > 1 (torchrun): every rank holds a replica of the scene and scores its own C candidates (no collective on
+the data path; weak scaling).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "candidate views scored/sec (Hessian + info gain)"
+UNIT = "views/s"
+SM_COUNT_B200 = 148
+FP32_LANES_PER_SM = 128
+
+# Algorithmic work per unit (FMA = 2 flop).
+FLOP_TEST = 11            # (pixel, list entry) evaluated: dx, dy, power, two range tests
+FLOP_FWD_PAIR = 31        # composited pair, S3: exp, alpha, T update, 4 blended channels
+FLOP_BWD_PAIR = {3: 134, 4: 154}   # composited pair, S4: exp, beta, 34 / 40 moment updates
+BYTES_PER_KEY = 8         # S2: a (tile, depth) key must be written once and read once (4 + 4 B)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-sample-views", type=int, default=0, help="oracle sample size (0 = automatic)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+# --------------------------------------------------------------------------------------------------
+# clocks: nvidia-smi sampled DURING the timed region
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name).read().strip().splitlines() if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            if len(r) < 6:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[2:6]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference)
+# --------------------------------------------------------------------------------------------------
+def oracle_setup(wl):
+    from oracle import nbv_oracle as orc
+    s = wl.scene
+    scn = orc.OracleScene(s.mean, s.logscale, s.quat, s.opacity, s.rgb, s.obj_logits, orc.default_config(wl.channel_mask))
+    return orc, scn
+
+
+def oracle_score_views(orc, scn, wl, H_T, cams):
+    """S0' + (S1..S6 per view) + S7 with the oracle; returns seconds."""
+    t0 = time.perf_counter()
+    orc.score_candidates(scn, wl.train_cams[:0], cams, wl.target_obj, H_T=H_T)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(wl, n_views: int):
+    orc, scn = oracle_setup(wl)
+    # H_T of ONE training view (untimed): scoring cost does not depend on how many views H_T sums
+    H_T = np.zeros((scn.N, orc.NB))
+    scn.view_hessian(wl.train_cams[0], out=H_T)
+    dt = oracle_score_views(orc, scn, wl, H_T, wl.cand_cams[:n_views])
+    return {"value": n_views / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "sample": "first %d candidate view(s) of the workload scored against H_T of its first training view "
+                      "(%.1f s wall, OpenMP over pixels)" % (n_views, dt)}
+
+
+def auto_sample_views(cfg_index: int) -> int:
+    return {0: 4, 1: 2, 2: 1, 3: 1, 4: 1}[cfg_index]
+
+
+def run_reference(args, wl, rank: int):
+    """--impl reference: the oracle, each step a bounded sample (n candidate views) of the workload."""
+    if rank != 0:
+        return
+    n = args.cpu_sample_views or auto_sample_views(args.config)
+    orc, scn = oracle_setup(wl)
+    H_T = np.zeros((scn.N, orc.NB))
+    scn.view_hessian(wl.train_cams[0], out=H_T)
+    C = len(wl.cand_cams)
+    pick = lambda i: wl.cand_cams[[(i * n + j) % C for j in range(n)]]
+    for i in range(args.warmup):
+        oracle_score_views(orc, scn, wl, H_T, pick(i))
+    total = 0.0
+    for i in range(args.steps):
+        total += oracle_score_views(orc, scn, wl, H_T, pick(args.warmup + i))
+    v = n * args.steps / total
+    sample = "each step = %d candidate view(s) of the workload scored by the oracle against H_T of one training view" % n
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(args, wl, "host"),
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def workload_config(args, wl, where: str):
+    s = wl.scene
+    return {"workload": "BASELINE.json configs[%d] (%s)" % (args.config, wl.name), "gaussians": s.N, "objects": s.K,
+            "image": "%dx%d" % (int(wl.cand_cams[0]["width"]), int(wl.cand_cams[0]["height"])),
+            "training_views": int(len(wl.train_cams)), "candidates_per_step": int(len(wl.cand_cams)),
+            "channels": "rgb+depth" if wl.channel_mask == 15 else "rgb", "target_obj": int(wl.target_obj), "P": 14,
+            "seed": int(wl.seed), "parallelism": "replicas x%d" % args.gpus,
+            "l2": "flushed between steps (512 MiB write); per-view working set (keys, H_T, factors) exceeds the 126 MB L2"
+                  if where == "device" else "n/a"}
+
+
+# --------------------------------------------------------------------------------------------------
+def aggregate(step_ms_per_rank, views_per_rank_step):
+    """Whole-job throughput: units of all ranks / slowest rank's time.  step_ms_per_rank: (ranks, steps)."""
+    t = np.asarray(step_ms_per_rank, dtype=np.float64)
+    total_ms = t.sum(axis=1).max()
+    steps = t.shape[1]
+    return dict(value=t.shape[0] * views_per_rank_step * steps / (total_ms * 1e-3), ms_per_step=total_ms / steps)
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from paper_2602_08266_b200 import synth
+    wl = synth.make_workload(args.config)
+    if args.impl == "reference":
+        run_reference(args, wl, rank)
+        return
+
+    import torch
+    from paper_2602_08266_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (B200); the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank > 0:   # replicas score their own candidate sets (same scene): rank-seeded cameras
+        c = synth.CONFIGS[args.config]
+        f = synth._intrinsics(c)
+        wl.cand_cams = synth.hemisphere_cameras(c["C"], c["radius"], c["W"], c["H"], f, f, np.random.default_rng(10_000 + rank))
+
+    nbv = api.NBV(channel_mask=wl.channel_mask)
+    t0 = time.perf_counter()
+    nbv.load_scene(wl.scene)
+    torch.cuda.synchronize()
+    load_s = time.perf_counter() - t0
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    e0, e1 = ev(), ev()
+    e0.record()
+    nbv.accumulate_training(wl.train_cams)
+    e1.record()
+    torch.cuda.synchronize()
+    train_ms = e0.elapsed_time(e1)
+
+    C = len(wl.cand_cams)
+    scores = torch.empty(C, dtype=torch.float32, device="cuda")
+    best = torch.empty(1, dtype=torch.int32, device="cuda")
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        nbv.score_candidates(wl.cand_cams, wl.target_obj, scores, best)
+    # ---- timed region: K steps, device-timed per step, L2 flushed between steps, stage events on ----
+    nbv.set_stage_timing(True)
+    launches0 = nbv.kernel_launches()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    barrier()
+    step_ms = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        a, b = ev(), ev()
+        a.record()
+        nbv.score_candidates(wl.cand_cams, wl.target_obj, scores, best)
+        b.record()
+        b.synchronize()
+        step_ms.append(a.elapsed_time(b))
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    launches = (nbv.kernel_launches() - launches0) // max(args.steps, 1)
+    stage_ms, n_timed_views = nbv.stage_times()
+    nbv.set_stage_timing(False)
+
+    # ---- e2e: host cameras in, host scores out, through nbv_score_candidates_host ----
+    for _ in range(min(args.warmup, 2)):
+        nbv.score_candidates_host(wl.cand_cams, wl.target_obj)
+    barrier()
+    e2e_s = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h_scores, h_best = nbv.score_candidates_host(wl.cand_cams, wl.target_obj)
+        e2e_s.append(time.perf_counter() - t0)
+    barrier()
+
+    # ---- counts of the same views (untimed pass) for the algorithmic work ----
+    tot = dict(n_visible=0, n_keys=0, n_entries=0, n_pairs=0, n_touched=0)
+    for cam in wl.cand_cams:
+        nbv.gaussian_gains(cam, wl.target_obj)
+        st = nbv.last_view_stats()
+        for k in tot:
+            tot[k] += st[k]
+
+    # ---- gather over ranks ----
+    t_all = torch.tensor([step_ms], dtype=torch.float64, device="cuda")
+    e_all = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        tl = [torch.zeros_like(t_all) for _ in range(world)]
+        el = [torch.zeros_like(e_all) for _ in range(world)]
+        dist.all_gather(tl, t_all)
+        dist.all_gather(el, e_all)
+        t_all, e_all = torch.cat(tl), torch.cat(el)
+    agg = aggregate(t_all.cpu().numpy(), C)
+    agg_e2e = aggregate(e_all.cpu().numpy() * 1e3, C)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peaks = load_peaks()
+    nch = 4 if wl.channel_mask & 8 else 3
+    views = max(n_timed_views, 1)
+    per_view_ms = {k: v / views for k, v in stage_ms.items()}
+    avg = {k: v / C for k, v in tot.items()}            # per view
+    tests = avg["n_entries"] * 256.0
+    alu_peak = SM_COUNT_B200 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12    # TFLOP/s
+    work = {
+        "backward": ("alu", (tests * FLOP_TEST + avg["n_pairs"] * FLOP_BWD_PAIR[nch]) / 1e12, alu_peak, "TFLOP/s"),
+        "forward": ("alu", (tests * FLOP_TEST + avg["n_pairs"] * FLOP_FWD_PAIR) / 1e12, alu_peak, "TFLOP/s"),
+        "tile_sort": ("hbm", avg["n_keys"] * BYTES_PER_KEY / 1e9, peaks["hbm_gbs"], "GB/s"),
+    }
+    rl = {}
+    for k, (bound, amount, peak, unit) in work.items():
+        sec = per_view_ms[k] * 1e-3
+        ach = amount / sec if sec > 0 else 0.0
+        rl[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak, "traffic": None,
+                 "ms_per_launch": per_view_ms[k], "peak_source": peaks["source"] if bound == "hbm" else
+                 "148 SM x 128 lanes x 2 x %.0f MHz (DESIGN.md section 8)" % peaks["sm_max_mhz"]}
+    dominant = max(work, key=lambda k: per_view_ms[k])
+    roofline = dict(rl[dominant], kernel=dominant)
+    # whole-view bound: sum over stages of the stage's own lower bound
+    t_min_ms = sum(1e3 * work[k][1] / work[k][2] for k in work)
+    view_ms = sum(per_view_ms.values())
+
+    out = {
+        "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": agg["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic", "config": workload_config(args, wl, "device"),
+        "clocks": clocks,
+        "e2e": {"value": agg_e2e["value"], "unit": UNIT, "h2d_bytes_per_step": int(72 * C), "d2h_bytes_per_step": int(4 * C + 4),
+                "call": "nbv_score_candidates_host (host camera structs in, host scores + best out, stream synchronised)"},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "stage_ms_per_view": per_view_ms,
+        "stage_rooflines": rl,
+        "view_roofline": {"t_min_ms": t_min_ms, "t_measured_ms": view_ms, "frac": t_min_ms / view_ms if view_ms else None},
+        "counts_per_view": avg,
+        "setup": {"load_s": load_s, "training_views_per_s": len(wl.train_cams) / (train_ms * 1e-3) if train_ms else None},
+        "best": int(h_best),
+    }
+    if not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(wl, args.cpu_sample_views or auto_sample_views(args.config))
+    print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -135,6 +135,30 @@ int nbv_score_candidates_host(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n,
 /* Counters of the last view processed by any call (synchronises `stream`). */
 int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream);
 
+/* ---- measurement ------------------------------------------------------------------------------------ */
+
+/* Stages of one view, in stream order: S1 | depth radix sort | gather + scan + key
+ * emission | tile-digit radix passes + tile ranges | S3 | S4 | S5 + S6. */
+#define NBV_STAGE_PROJECT 0
+#define NBV_STAGE_DEPTH_SORT 1
+#define NBV_STAGE_BIN 2
+#define NBV_STAGE_TILE_SORT 3
+#define NBV_STAGE_FORWARD 4
+#define NBV_STAGE_BACKWARD 5
+#define NBV_STAGE_EXPAND 6
+#define NBV_N_STAGES 7
+
+/* enable != 0: record CUDA events on `stream` at every stage boundary of every view processed from now on
+ * (a few microseconds per view); clears the accumulated times.  Synchronises `stream`. */
+int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream);
+
+/* h_ms[NBV_N_STAGES] <- milliseconds spent per stage, summed over the *h_views views processed since timing was
+ * enabled (h_views may be NULL).  Synchronises `stream`. */
+int nbv_stage_times(nbv_ctx* ctx, double* h_ms, int64_t* h_views, void* stream);
+
+/* Number of CUDA kernels this library has launched in this process so far (all contexts). */
+int64_t nbv_kernel_launches(void);
+
 /* ---- parity / debug exports (not on the timed path) ------------------------------------------------ */
 
 /* S1 outputs of one view, indexed by Gaussian: d_visible N int32; d_rec N x 9 floats

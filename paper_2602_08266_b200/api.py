@@ -34,8 +34,10 @@ EXPORTS = [
     "nbv_default_config", "nbv_create", "nbv_destroy", "nbv_last_error", "nbv_load_gaussians", "nbv_reset_training",
     "nbv_accumulate_training", "nbv_score_candidates", "nbv_score_candidates_host", "nbv_last_view_stats",
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
-    "nbv_gaussian_gains",
+    "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches",
 ]
+
+STAGES = ["project", "depth_sort", "bin", "tile_sort", "forward", "backward", "expand_gain"]
 
 
 class NBVError(RuntimeError):
@@ -81,6 +83,7 @@ def load_library(path: Path | None = None):
     lib.nbv_destroy.restype = None
     lib.nbv_destroy.argtypes = [C.c_void_p]
     lib.nbv_default_config.restype = None
+    lib.nbv_kernel_launches.restype = C.c_int64
     if path is None:
         _lib = lib
     return lib
@@ -204,6 +207,20 @@ class NBV:
         st = ViewStats()
         self._check(self.lib.nbv_last_view_stats(self._h, C.byref(st), _stream()))
         return st.as_dict()
+
+    # ---- measurement ----------------------------------------------------------------------------
+    def set_stage_timing(self, enable: bool = True):
+        self._check(self.lib.nbv_set_stage_timing(self._h, int(bool(enable)), _stream()))
+
+    def stage_times(self) -> tuple[dict, int]:
+        """({stage: milliseconds summed over the timed views}, number of views)"""
+        ms = (C.c_double * len(STAGES))()
+        views = C.c_int64(0)
+        self._check(self.lib.nbv_stage_times(self._h, ms, C.byref(views), _stream()))
+        return {k: float(ms[i]) for i, k in enumerate(STAGES)}, int(views.value)
+
+    def kernel_launches(self) -> int:
+        return int(self.lib.nbv_kernel_launches())
 
     # ---- parity / debug exports ------------------------------------------------------------------
     def projected(self, cam):

@@ -25,6 +25,7 @@ __global__ void __launch_bounds__(256) gather_kernel(const uint32_t* __restrict_
 
 void launch_gather(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, Splat* splat_sorted,
                    ushort4* rect_sorted, uint32_t* ntiles_sorted, cudaStream_t st) {
+  ++g_kernel_launches;
   gather_kernel<<<(N + 255) / 256, 256, 0, st>>>(ids_sorted, splat, rect, N, splat_sorted, rect_sorted, ntiles_sorted);
 }
 
@@ -48,6 +49,7 @@ __global__ void __launch_bounds__(256) emit_keys_kernel(const ushort4* __restric
 void launch_emit_keys(const ushort4* rect_sorted, const uint32_t* offsets, int N, int tiles_x, int rank_bits,
                       uint32_t* keys, cudaStream_t st) {
   const long long threads = (long long)N * 32;
+  ++g_kernel_launches;
   emit_keys_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(rect_sorted, offsets, N, tiles_x, rank_bits, keys);
 }
 
@@ -63,6 +65,7 @@ __global__ void __launch_bounds__(256) tile_ranges_kernel(const uint32_t* __rest
 void launch_tile_ranges(const uint32_t* keys, size_t n_keys, int rank_bits, uint2* ranges, int n_tiles, cudaStream_t st) {
   cudaMemsetAsync(ranges, 0, sizeof(uint2) * (size_t)n_tiles, st);
   if (n_keys == 0) return;
+  ++g_kernel_launches;
   tile_ranges_kernel<<<(unsigned)((n_keys + 255) / 256), 256, 0, st>>>(keys, (uint32_t)n_keys, rank_bits, ranges);
 }
 
@@ -87,11 +90,15 @@ __global__ void export_ids_kernel(const uint32_t* __restrict__ keys, uint32_t n,
 void launch_export_lists(const uint32_t* keys, size_t n_keys, int rank_bits, const uint32_t* ids_sorted, const uint2* ranges,
                          int n_tiles, int64_t* offsets, int32_t* ids_out, uint32_t* tmp_counts, uint32_t* scan_tmp, cudaStream_t st) {
   // the sorted keys are already grouped by ascending tile, so offsets are the scanned counts
+  ++g_kernel_launches;
   range_counts_kernel<<<(n_tiles + 255) / 256, 256, 0, st>>>(ranges, n_tiles, tmp_counts);
   exclusive_scan_u32(tmp_counts, tmp_counts, (size_t)n_tiles, scan_tmp, nullptr, st);
+  ++g_kernel_launches;
   export_offsets_kernel<<<(n_tiles + 1 + 255) / 256, 256, 0, st>>>(tmp_counts, n_tiles, (uint32_t)n_keys, offsets);
-  if (ids_out && n_keys)
+  if (ids_out && n_keys) {
+    ++g_kernel_launches;
     export_ids_kernel<<<(unsigned)((n_keys + 255) / 256), 256, 0, st>>>(keys, (uint32_t)n_keys, rank_bits, ids_sorted, ids_out);
+  }
 }
 
 }  // namespace nbv

@@ -7,7 +7,10 @@
 //     A (14 x 6): rows of the chain d(mx,my,a,b,c)/d(mu,logscale,quat) (first-order EWA, through q/|q|), the
 //     opacity row kappa, zero colour rows.   PAPER.md L189-191 (H ~= J^T J), L210 (per-Gaussian blocks), L248.
 // S6: IG_g = log det(c_g (H_T,g + H_c,g) + Lambda) - log det(c_g H_T,g + Lambda)   (Eq. 5, 6, 9; R-13, R-14)
-//     by a packed Cholesky per Gaussian, one thread each; the second term is precomputed once per scoring call.
+//     evaluated in the SOLVE FORM  log det(I + U^-T (c_g H_c,g) U^-1),  U^T U = c_g H_T,g + Lambda,
+//     which is the same number without the binary32 cancellation of two log-dets of size ~100.
+//     U is factored once per scoring call (prepare_kernel); per candidate one thread per touched Gaussian does the
+//     two-sided triangular solve and a Cholesky of I + W whose pivots 1 + e_j enter as log1p(e_j).
 #include "kernels.h"
 
 namespace nbv {
@@ -191,14 +194,13 @@ __device__ void build_block(const float* mom, const ChainF& ch, float kappa, con
   }
 }
 
-// log det of a packed SPD 14x14 (upper Cholesky, in place).  Pivots are floored at a tiny positive number.
-__device__ float logdet_packed(float* Mx) {
-  float ld = 0.f;
+// Upper Cholesky factor of a packed SPD 14x14, in place (row j holds U[j][j..13]).  Pivots are floored at a tiny
+// positive number: with Lambda > 0 the matrix is positive definite and the floor never acts in exact arithmetic.
+__device__ void cholesky_packed(float* Mx) {
   for (int j = 0; j < P; ++j) {
     float d = Mx[tri(j, j)];
     for (int k = 0; k < j; ++k) d -= Mx[tri(k, j)] * Mx[tri(k, j)];
     d = fmaxf(d, 1e-30f);
-    ld += logf(d);
     const float inv = rsqrtf(d);
     Mx[tri(j, j)] = d * inv;
     for (int i = j + 1; i < P; ++i) {
@@ -207,13 +209,52 @@ __device__ float logdet_packed(float* Mx) {
       Mx[tri(j, i)] = v * inv;
     }
   }
+}
+
+// log det(I + U^-T B U^-1) for packed symmetric PSD B (destroyed) and packed upper-triangular U.
+// Step 1 is the unblocked two-sided solve (the algorithm of LAPACK's xSYGS2, itype 1, upper); step 2 a Cholesky
+// of I + W that never forms 1 + e: the pivot excess e_j goes through log1p.
+__device__ float gain_solve(float* B, const float* U) {
+  for (int k = 0; k < P; ++k) {
+    const float inv = 1.0f / U[tri(k, k)];
+    const float bkk = B[tri(k, k)] * inv * inv;
+    B[tri(k, k)] = bkk;
+    if (k < P - 1) {
+      const float ct = -0.5f * bkk;
+      for (int j = k + 1; j < P; ++j) B[tri(k, j)] = fmaf(ct, U[tri(k, j)], B[tri(k, j)] * inv);
+      for (int i = k + 1; i < P; ++i) {
+        const float bki = B[tri(k, i)], uki = U[tri(k, i)];
+        for (int j = i; j < P; ++j) B[tri(i, j)] -= bki * U[tri(k, j)] + uki * B[tri(k, j)];
+      }
+      for (int j = k + 1; j < P; ++j) B[tri(k, j)] = fmaf(ct, U[tri(k, j)], B[tri(k, j)]);
+      // row k, columns k+1.. :  x^T <- x^T U22^-1   (forward substitution with U22^T)
+      for (int j = k + 1; j < P; ++j) {
+        float v = B[tri(k, j)];
+        for (int i = k + 1; i < j; ++i) v -= U[tri(i, j)] * B[tri(k, i)];
+        B[tri(k, j)] = v / U[tri(j, j)];
+      }
+    }
+  }
+  float ld = 0.f;
+  for (int j = 0; j < P; ++j) {
+    float e = B[tri(j, j)];
+    for (int k = 0; k < j; ++k) e -= B[tri(k, j)] * B[tri(k, j)];
+    e = fmaxf(e, 0.f);                       // W is PSD: the excess is >= 0 up to rounding
+    ld += log1pf(e);
+    const float inv = rsqrtf(1.0f + e);
+    for (int i = j + 1; i < P; ++i) {
+      float v = B[tri(j, i)];
+      for (int k = 0; k < j; ++k) v -= B[tri(k, j)] * B[tri(k, i)];
+      B[tri(j, i)] = v * inv;
+    }
+  }
   return ld;
 }
 
 __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam, nbv_config cfg, const uint32_t* __restrict__ ids_sorted,
                                                      const float* __restrict__ moments, int mode, float* __restrict__ H_T,
                                                      float* __restrict__ out_blocks, const float* __restrict__ conf,
-                                                     const float* __restrict__ ldT, float* __restrict__ score,
+                                                     const float* __restrict__ cholT, float* __restrict__ score,
                                                      float* __restrict__ gains, ViewCounters* counters) {
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
   float gain = 0.f;
@@ -246,11 +287,11 @@ __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam,
         for (int i = 0; i < NBLK; ++i) dst[i] = H[i];
       } else {
         const float c = conf[g];
-        if (c > 0.f) {
-          const float* ht = H_T + (size_t)g * NBLK;
-          for (int i = 0; i < NBLK; ++i) H[i] = c * (ht[i] + H[i]);
-          for (int k = 0; k < P; ++k) H[tri(k, k)] += cfg.prior_precision[k];
-          gain = logdet_packed(H) - ldT[g];
+        if (c > 0.f) {                       // c_g = 0 (Eq. 12, non-target): exactly zero gain
+          float U[NBLK];
+          const float* ut = cholT + (size_t)g * NBLK;
+          for (int i = 0; i < NBLK; ++i) { U[i] = ut[i]; H[i] *= c; }
+          gain = gain_solve(H, U);
         }
         if (gains) gains[g] = gain;
       }
@@ -272,9 +313,10 @@ __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam,
 }
 
 void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
-                   const float* moments, int mode, float* H_T, float* out_blocks, const float* conf, const float* ldT,
+                   const float* moments, int mode, float* H_T, float* out_blocks, const float* conf, const float* cholT,
                    float* score, float* gains, ViewCounters* counters, cudaStream_t st) {
-  expand_kernel<<<(sc.N + 63) / 64, 64, 0, st>>>(sc, cam, cfg, ids_sorted, moments, mode, H_T, out_blocks, conf, ldT, score,
+  ++g_kernel_launches;
+  expand_kernel<<<(sc.N + 63) / 64, 64, 0, st>>>(sc, cam, cfg, ids_sorted, moments, mode, H_T, out_blocks, conf, cholT, score,
                                                  gains, counters);
 }
 
@@ -296,28 +338,29 @@ __global__ void __launch_bounds__(256) confidence_kernel(SceneDev sc, nbv_config
 }
 
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st) {
+  ++g_kernel_launches;
   confidence_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(sc, cfg, target, conf);
 }
 
-// once per scoring call: ldT_g = log det(c_g H_T,g + Lambda)
+// once per scoring call: U_g = upper Cholesky factor of c_g H_T,g + Lambda (skipped for c_g = 0: never read)
 __global__ void __launch_bounds__(64) prepare_kernel(int N, nbv_config cfg, const float* __restrict__ H_T, const float* __restrict__ conf,
-                                                      float* __restrict__ ldT) {
+                                                      float* __restrict__ cholT) {
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= N) return;
   const float c = conf[g];
-  float prior_ld = 0.f;
-  for (int k = 0; k < P; ++k) prior_ld += logf(cfg.prior_precision[k]);
+  if (!(c > 0.f)) return;
   const float* ht = H_T + (size_t)g * NBLK;
   float H[NBLK];
-  bool zero = true;
-  for (int i = 0; i < NBLK; ++i) { H[i] = c * ht[i]; zero &= H[i] == 0.f; }
-  if (zero) { ldT[g] = prior_ld; return; }   // never observed in training (or c_g = 0): log det Lambda
+  for (int i = 0; i < NBLK; ++i) H[i] = c * ht[i];
   for (int k = 0; k < P; ++k) H[tri(k, k)] += cfg.prior_precision[k];
-  ldT[g] = logdet_packed(H);
+  cholesky_packed(H);
+  float* dst = cholT + (size_t)g * NBLK;
+  for (int i = 0; i < NBLK; ++i) dst[i] = H[i];
 }
 
-void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* ldT, cudaStream_t st) {
-  prepare_kernel<<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, cfg, H_T, conf, ldT);
+void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st) {
+  ++g_kernel_launches;
+  prepare_kernel<<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, cfg, H_T, conf, cholT);
 }
 
 // S7: arg-max, lowest index on ties (R-15)
@@ -338,6 +381,6 @@ __global__ void argmax_kernel(const float* __restrict__ scores, int n, int32_t* 
   if (lane == 0) *best = bi == 0x7fffffff ? 0 : bi;
 }
 
-void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st) { argmax_kernel<<<1, 32, 0, st>>>(scores, n, best); }
+void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st) { { ++g_kernel_launches; argmax_kernel<<<1, 32, 0, st>>>(scores, n, best); } }
 
 }  // namespace nbv

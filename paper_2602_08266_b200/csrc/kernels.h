@@ -4,6 +4,8 @@
 
 namespace nbv {
 
+extern unsigned long long g_kernel_launches;   // host-side count of kernel launches (nbv_kernel_launches)
+
 // ---- sort.cu
 size_t scan_temp_words(size_t n);
 void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* tmp, uint32_t* total_out, cudaStream_t st);
@@ -56,10 +58,10 @@ void launch_backward(const Splat* splat_sorted, const uint32_t* keys, const uint
 enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2 };
 // EXPAND_TRAIN: H_T[id] += H ; EXPAND_VIEW: out_blocks[id] = H ; EXPAND_GAIN: gain vs H_T, sum into *score (and gains[id] if not null)
 void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
-                   const float* moments, int mode, float* H_T, float* out_blocks, const float* conf, const float* ldT,
+                   const float* moments, int mode, float* H_T, float* out_blocks, const float* conf, const float* cholT,
                    float* score, float* gains, ViewCounters* counters, cudaStream_t st);
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);
-void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* ldT, cudaStream_t st);
+void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);
 
 }  // namespace nbv

@@ -5,10 +5,15 @@
 #include <cstring>
 #include <string>
 #include <utility>
+#include <vector>
 
 #include "kernels.h"
 
 using namespace nbv;
+
+namespace nbv {
+unsigned long long g_kernel_launches = 0;
+}
 
 namespace {
 
@@ -28,7 +33,7 @@ struct nbv_ctx {
   bool loaded = false;
   int n_train = 0;
   // scene
-  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, ldT;
+  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT;
   // per-view work buffers
   DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, ntiles, offsets;
   DevBuf keys, keys_alt, ranges, sort_tmp, scan_tmp, tile_counts;
@@ -40,7 +45,14 @@ struct nbv_ctx {
   size_t n_keys = 0;
   uint32_t* keys_sorted = nullptr;
   int cur_W = 0, cur_H = 0;
-  int conf_target = -2;                 // target the conf / ldT buffers were prepared for (-2 = stale)
+  int conf_target = -2;                 // target the conf / cholT buffers were prepared for (-2 = stale)
+  // optional per-stage timing (nbv_set_stage_timing): one event row per view, folded on read-out
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;          // ev[view * (NBV_N_STAGES + 1) + boundary]
+  std::vector<unsigned> ev_mask;        // per view: bit b set when boundary b was recorded
+  size_t ev_views = 0;
+  double stage_ms[NBV_N_STAGES] = {0};
+  long long timed_views = 0;
 };
 
 namespace {
@@ -133,6 +145,47 @@ PixelBuf pixel_buf(const nbv_ctx* c) {
   return p;
 }
 
+constexpr int EV_ROW = NBV_N_STAGES + 1;
+constexpr size_t EV_MAX_VIEWS = 1024;
+
+// fold the recorded event rows into ctx->stage_ms (the stream must be idle)
+void fold_timing(nbv_ctx* ctx) {
+  for (size_t v = 0; v < ctx->ev_views; ++v) {
+    const unsigned m = ctx->ev_mask[v];
+    for (int s = 0; s < NBV_N_STAGES; ++s)
+      if (((m >> s) & 1u) && ((m >> (s + 1)) & 1u)) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, ctx->ev[v * EV_ROW + s], ctx->ev[v * EV_ROW + s + 1]) == cudaSuccess) ctx->stage_ms[s] += ms;
+      }
+    if (m) ctx->timed_views++;
+    ctx->ev_mask[v] = 0;
+  }
+  cudaGetLastError();
+  ctx->ev_views = 0;
+}
+
+// start a new event row for the next view
+void timing_begin_view(nbv_ctx* ctx, cudaStream_t st) {
+  if (!ctx->timing) return;
+  if (ctx->ev_views >= EV_MAX_VIEWS) { cudaStreamSynchronize(st); fold_timing(ctx); }
+  const size_t v = ctx->ev_views++;
+  if (ctx->ev.size() < (v + 1) * EV_ROW) {
+    const size_t old = ctx->ev.size();
+    ctx->ev.resize((v + 1) * EV_ROW);
+    for (size_t i = old; i < ctx->ev.size(); ++i) cudaEventCreate(&ctx->ev[i]);
+    ctx->ev_mask.resize(v + 1, 0u);
+  }
+  ctx->ev_mask[v] = 0;
+}
+
+// record boundary b (= start of stage b, end of stage b-1) of the current view
+void mark(nbv_ctx* ctx, int b, cudaStream_t st) {
+  if (!ctx->timing || ctx->ev_views == 0) return;
+  const size_t v = ctx->ev_views - 1;
+  cudaEventRecord(ctx->ev[v * EV_ROW + b], st);
+  ctx->ev_mask[v] |= 1u << b;
+}
+
 enum Stage { STAGE_PROJECT = 0, STAGE_BIN = 1, STAGE_FORWARD = 2, STAGE_BACKWARD = 3 };
 
 // S1..S4 for one camera.  Leaves the depth order in ctx->ids, rank-ordered splats, sorted keys, tile ranges,
@@ -158,12 +211,15 @@ int process_view(nbv_ctx* ctx, const nbv_camera& cam, int upto, bool want_abc, c
   CKRET(ensure(ctx, ctx->scan_tmp, 4 * scan_temp_words((size_t)N + 1)));
 
   CK(cudaMemsetAsync(ctx->d_counters, 0, sizeof(ViewCounters), st));
+  timing_begin_view(ctx, st);
+  mark(ctx, NBV_STAGE_PROJECT, st);
   launch_project(sc, cam, ctx->cfg, ctx->splat.as<Splat>(), ctx->zkey.as<uint32_t>(), ctx->ids.as<uint32_t>(),
                  ctx->rect.as<ushort4>(), want_abc ? ctx->abc.as<float>() : nullptr, ctx->d_counters, st);
   CK(cudaGetLastError());
   if (upto == STAGE_PROJECT) return NBV_OK;
 
   // depth sort: 4 stable passes of 8 bits on the z bits, Gaussian index as value (ties keep index order: R-7)
+  mark(ctx, NBV_STAGE_DEPTH_SORT, st);
   {
     uint32_t *k0 = ctx->zkey.as<uint32_t>(), *k1 = ctx->zkey_alt.as<uint32_t>();
     uint32_t *v0 = ctx->ids.as<uint32_t>(), *v1 = ctx->ids_alt.as<uint32_t>();
@@ -174,6 +230,7 @@ int process_view(nbv_ctx* ctx, const nbv_camera& cam, int upto, bool want_abc, c
     }
     CK(cudaGetLastError());
   }
+  mark(ctx, NBV_STAGE_BIN, st);
   CKRET(ensure(ctx, ctx->splat_sorted, sizeof(Splat) * (size_t)N));
   CKRET(ensure(ctx, ctx->rect_sorted, sizeof(ushort4) * (size_t)N));
   CKRET(ensure(ctx, ctx->ntiles, 4 * (size_t)N));
@@ -193,6 +250,7 @@ int process_view(nbv_ctx* ctx, const nbv_camera& cam, int upto, bool want_abc, c
   CKRET(ensure(ctx, ctx->sort_tmp, 4 * radix_temp_words(std::max((size_t)n_keys, (size_t)N)), true));
   CKRET(ensure(ctx, ctx->ranges, sizeof(uint2) * (size_t)n_tiles));
   launch_emit_keys(ctx->rect_sorted.as<ushort4>(), ctx->offsets.as<uint32_t>(), N, TX, rank_bits, ctx->keys.as<uint32_t>(), st);
+  mark(ctx, NBV_STAGE_TILE_SORT, st);
   {
     uint32_t *k0 = ctx->keys.as<uint32_t>(), *k1 = ctx->keys_alt.as<uint32_t>();
     const int npass = (tile_bits + 7) / 8;
@@ -205,6 +263,7 @@ int process_view(nbv_ctx* ctx, const nbv_camera& cam, int upto, bool want_abc, c
   }
   launch_tile_ranges(ctx->keys_sorted, (size_t)n_keys, rank_bits, ctx->ranges.as<uint2>(), n_tiles, st);
   CK(cudaGetLastError());
+  mark(ctx, NBV_STAGE_FORWARD, st);
   if (upto == STAGE_BIN) return NBV_OK;
 
   const size_t npx = (size_t)cam.width * cam.height;
@@ -213,6 +272,7 @@ int process_view(nbv_ctx* ctx, const nbv_camera& cam, int upto, bool want_abc, c
   launch_forward(ctx->splat_sorted.as<Splat>(), ctx->keys_sorted, ctx->ranges.as<uint2>(), rank_bits, cam.width, cam.height,
                  ctx->cfg, pixel_buf(ctx), ctx->d_counters, st);
   CK(cudaGetLastError());
+  mark(ctx, NBV_STAGE_BACKWARD, st);
   if (upto == STAGE_FORWARD) return NBV_OK;
 
   CKRET(ensure(ctx, ctx->moments, 4 * (size_t)NMOM * N));
@@ -220,6 +280,7 @@ int process_view(nbv_ctx* ctx, const nbv_camera& cam, int upto, bool want_abc, c
   launch_backward(ctx->splat_sorted.as<Splat>(), ctx->keys_sorted, ctx->ranges.as<uint2>(), rank_bits, cam.width, cam.height,
                   ctx->cfg, pixel_buf(ctx), ctx->moments.as<float>(), st);
   CK(cudaGetLastError());
+  mark(ctx, NBV_STAGE_EXPAND, st);
   return NBV_OK;
 }
 
@@ -228,7 +289,7 @@ int prepare_scoring(nbv_ctx* ctx, int target, cudaStream_t st) {
   if (ctx->conf_target == target) return NBV_OK;
   const SceneDev sc = scene_dev(ctx);
   launch_confidence(sc, ctx->cfg, target, ctx->conf.as<float>(), st);
-  launch_prepare(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->ldT.as<float>(), st);
+  launch_prepare(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
   CK(cudaGetLastError());
   ctx->conf_target = target;
   return NBV_OK;
@@ -309,13 +370,14 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
 void nbv_destroy(nbv_ctx* ctx) {
   if (!ctx) return;
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
-                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->ldT, &ctx->splat, &ctx->zkey, &ctx->zkey_alt, &ctx->ids, &ctx->ids_alt,
+                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->splat, &ctx->zkey, &ctx->zkey_alt, &ctx->ids, &ctx->ids_alt,
                    &ctx->rect, &ctx->abc, &ctx->splat_sorted, &ctx->rect_sorted, &ctx->ntiles, &ctx->offsets, &ctx->keys,
                    &ctx->keys_alt, &ctx->ranges, &ctx->sort_tmp, &ctx->scan_tmp, &ctx->tile_counts, &ctx->pix_rgb, &ctx->pix_depth,
                    &ctx->pix_T, &ctx->pix_nc, &ctx->pix_last, &ctx->moments, &ctx->score_tmp};
   for (DevBuf* b : all) release(*b);
   if (ctx->d_counters) cudaFree(ctx->d_counters);
   if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
+  for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
   delete ctx;
 }
 
@@ -334,7 +396,7 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
   CKRET(ensure(ctx, ctx->sigma, 4 * n)); CKRET(ensure(ctx, ctx->rgb, 12 * n)); CKRET(ensure(ctx, ctx->logits, 4 * n * K));
   CKRET(ensure(ctx, ctx->M, 36 * n)); CKRET(ensure(ctx, ctx->pmax, 4 * n)); CKRET(ensure(ctx, ctx->amax, 4 * n));
   CKRET(ensure(ctx, ctx->lse, 4 * n)); CKRET(ensure(ctx, ctx->H_T, 4 * (size_t)NBLK * n)); CKRET(ensure(ctx, ctx->conf, 4 * n));
-  CKRET(ensure(ctx, ctx->ldT, 4 * n));
+  CKRET(ensure(ctx, ctx->cholT, 4 * (size_t)NBLK * n));
   CK(cudaMemcpyAsync(ctx->mean.p, d_mean, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->logscale.p, d_logscale, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->quat.p, d_quat, 16 * n, cudaMemcpyDeviceToDevice, st));
@@ -376,6 +438,7 @@ int nbv_accumulate_training(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, v
     launch_expand(scene_dev(ctx), h_cams[i], ctx->cfg, ctx->ids.as<uint32_t>(), ctx->moments.as<float>(), EXPAND_TRAIN,
                   ctx->H_T.as<float>(), nullptr, nullptr, nullptr, nullptr, nullptr, ctx->d_counters, st);
     CK(cudaGetLastError());
+    mark(ctx, NBV_N_STAGES, st);
     ctx->n_train++;
     ctx->conf_target = -2;
   }
@@ -397,9 +460,10 @@ int nbv_score_candidates(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int3
   for (int i = 0; i < n; ++i) {
     CKRET(process_view(ctx, h_cams[i], STAGE_BACKWARD, false, st));
     launch_expand(scene_dev(ctx), h_cams[i], ctx->cfg, ctx->ids.as<uint32_t>(), ctx->moments.as<float>(), EXPAND_GAIN,
-                  ctx->H_T.as<float>(), nullptr, ctx->conf.as<float>(), ctx->ldT.as<float>(), d_scores + i, nullptr,
+                  ctx->H_T.as<float>(), nullptr, ctx->conf.as<float>(), ctx->cholT.as<float>(), d_scores + i, nullptr,
                   ctx->d_counters, st);
     CK(cudaGetLastError());
+    mark(ctx, NBV_N_STAGES, st);
   }
   launch_argmax(d_scores, n, d_best, st);
   CK(cudaGetLastError());
@@ -435,11 +499,34 @@ int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream) {
   return NBV_OK;
 }
 
+int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream) {
+  if (!ctx) return NBV_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize((cudaStream_t)stream));
+  ctx->ev_views = 0;
+  for (auto& m : ctx->ev_mask) m = 0;
+  for (int s = 0; s < NBV_N_STAGES; ++s) ctx->stage_ms[s] = 0.0;
+  ctx->timed_views = 0;
+  ctx->timing = enable != 0;
+  return NBV_OK;
+}
+
+int nbv_stage_times(nbv_ctx* ctx, double* h_ms, int64_t* h_views, void* stream) {
+  if (!ctx || !h_ms) return NBV_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize((cudaStream_t)stream));
+  fold_timing(ctx);
+  for (int s = 0; s < NBV_N_STAGES; ++s) h_ms[s] = ctx->stage_ms[s];
+  if (h_views) *h_views = ctx->timed_views;
+  return NBV_OK;
+}
+
+int64_t nbv_kernel_launches(void) { return (int64_t)nbv::g_kernel_launches; }
+
 int nbv_projected(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t* d_visible, float* d_rec, int32_t* d_rect, void* stream) {
   if (!ctx || !h_cam) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   cudaStream_t st = (cudaStream_t)stream;
   CKRET(process_view(ctx, *h_cam, STAGE_PROJECT, true, st));
+  ++g_kernel_launches;
   export_projected_kernel<<<(ctx->N + 255) / 256, 256, 0, st>>>(ctx->N, ctx->splat.as<Splat>(), ctx->zkey.as<uint32_t>(),
                                                                 ctx->rect.as<ushort4>(), ctx->abc.as<float>(), d_visible, d_rec, d_rect);
   CK(cudaGetLastError());
@@ -516,7 +603,7 @@ int nbv_gaussian_gains(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t target_obj
   CK(cudaMemsetAsync(d_gains, 0, 4 * (size_t)ctx->N, st));
   CKRET(process_view(ctx, *h_cam, STAGE_BACKWARD, false, st));
   launch_expand(scene_dev(ctx), *h_cam, ctx->cfg, ctx->ids.as<uint32_t>(), ctx->moments.as<float>(), EXPAND_GAIN, ctx->H_T.as<float>(),
-                nullptr, ctx->conf.as<float>(), ctx->ldT.as<float>(), ctx->score_tmp.as<float>(), d_gains, ctx->d_counters, st);
+                nullptr, ctx->conf.as<float>(), ctx->cholT.as<float>(), ctx->score_tmp.as<float>(), d_gains, ctx->d_counters, st);
   CK(cudaGetLastError());
   return NBV_OK;
 }

@@ -59,6 +59,7 @@ __global__ void __launch_bounds__(256) activate_kernel(SceneDev sc, ViewCounters
 }
 
 void launch_activate(const SceneDev& sc, ViewCounters* counters, cudaStream_t st) {
+  ++g_kernel_launches;
   activate_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(sc, counters);
 }
 
@@ -165,6 +166,7 @@ __global__ void __launch_bounds__(256) project_kernel(SceneDev sc, nbv_camera ca
 
 void launch_project(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, Splat* splat, uint32_t* zkey,
                     uint32_t* ids, ushort4* rect, float* abc, ViewCounters* counters, cudaStream_t st) {
+  ++g_kernel_launches;
   project_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(sc, cam, cfg, splat, zkey, ids, rect, abc, counters);
 }
 

@@ -287,6 +287,7 @@ void launch_forward(const Splat* splat_sorted, const uint32_t* keys, const uint2
                     const nbv_config& cfg, PixelBuf px, ViewCounters* counters, cudaStream_t st) {
   const RasterParams p = make_params(rank_bits, W, H, cfg);
   const int tiles = p.tiles_x * ((H + TILE - 1) / TILE);
+  ++g_kernel_launches;
   forward_kernel<<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, counters);
 }
 
@@ -294,10 +295,14 @@ void launch_backward(const Splat* splat_sorted, const uint32_t* keys, const uint
                      const nbv_config& cfg, PixelBuf px, float* moments, cudaStream_t st) {
   const RasterParams p = make_params(rank_bits, W, H, cfg);
   const int tiles = p.tiles_x * ((H + TILE - 1) / TILE);
-  if (cfg.channel_mask & NBV_CH_DEPTH)
+  if (cfg.channel_mask & NBV_CH_DEPTH) {
+    ++g_kernel_launches;
     backward_kernel<4><<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, moments);
-  else
+  }
+  else {
+    ++g_kernel_launches;
     backward_kernel<3><<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, moments);
+  }
 }
 
 }  // namespace nbv

@@ -101,12 +101,15 @@ void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* t
   }
   const uint32_t nb = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
   if (nb == 1) {
+    ++g_kernel_launches;
     scan_downsweep_kernel<<<1, SCAN_T, 0, st>>>(in, out, (uint32_t)n, nullptr, total_out);
     return;
   }
   uint32_t* sums = tmp;
+  ++g_kernel_launches;
   scan_reduce_kernel<<<nb, SCAN_T, 0, st>>>(in, (uint32_t)n, sums);
   exclusive_scan_u32(sums, sums, nb, tmp + nb, nullptr, st);
+  ++g_kernel_launches;
   scan_downsweep_kernel<<<nb, SCAN_T, 0, st>>>(in, out, (uint32_t)n, sums, total_out);
 }
 
@@ -219,12 +222,17 @@ void radix_pass(const uint32_t* keys_in, uint32_t* keys_out, const uint32_t* val
   const uint32_t mask = (1u << bits) - 1u;
   const size_t hist_n = (size_t)(mask + 1) * nb;
   uint32_t* hist = tmp;
+  ++g_kernel_launches;
   radix_hist_kernel<<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, shift, mask, hist, nb);
   exclusive_scan_u32(hist, hist, hist_n, tmp + 256 * (size_t)nb, nullptr, st);
-  if (vals_in)
+  if (vals_in) {
+    ++g_kernel_launches;
     radix_scatter_kernel<true><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, shift, mask, hist, nb);
-  else
+  }
+  else {
+    ++g_kernel_launches;
     radix_scatter_kernel<false><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, shift, mask, hist, nb);
+  }
 }
 
 }  // namespace nbv

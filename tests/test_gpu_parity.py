@@ -124,8 +124,9 @@ def test_training_accumulation_and_gains_and_argmax(wl):
     # per-Gaussian terms of one candidate
     g = nbv.gaussian_gains(wl.cand_cams[1]).cpu().numpy()
     go = res["gains"][1]
-    np.testing.assert_array_equal(g != 0, go != 0)
-    np.testing.assert_allclose(g, go, rtol=1e-3, atol=1e-3 * np.abs(go).max() * 1e-2 + 1e-6)
+    assert np.all(g[go == 0] == 0)          # Gaussians the view does not touch: exactly zero
+    assert np.all(g[go > 1e-6] > 0)
+    np.testing.assert_allclose(g, go, rtol=1e-3, atol=1e-6)
 
 
 def test_object_centric_scoring(wl):
@@ -200,13 +201,17 @@ def test_clamped_opaque_gaussian_and_stacked_half_alphas():
     cam = synth.simple_camera(32, 32, 100.0, dist=0.0)
     f = 100.0
     on = lambda ix, iy, z: [((ix + 0.5) - 16) * z / f, ((iy + 0.5) - 16) * z / f, z]
-    sc = scene_from_arrays([on(16, 16, 1.0), on(16, 16, 2.0), on(5, 7, 1.5)], [[-3] * 3] * 3, [[1, 0, 0, 0]] * 3,
+    # third Gaussian far enough from the stacked pair (power < -6 there) that it is alone at its centre pixel
+    sc = scene_from_arrays([on(16, 16, 1.0), on(16, 16, 2.0), on(2, 2, 1.5)], [[-3] * 3] * 3, [[1, 0, 0, 0]] * 3,
                            [0.5, 0.5, 0.999999], [[1, 0, 0], [0, 1, 0], [1, 1, 1]])
     scn = make_oracle_scene(sc, channel_mask=15)
     nbv = _nbv(sc, channel_mask=15)
     r = {k: v.cpu().numpy() for k, v in nbv.render(cam).items()}
     assert 1.0 - r["T"][16, 16] == pytest.approx(0.75, abs=2e-6)
-    assert 1.0 - r["T"][7, 5] == pytest.approx(0.99, abs=1e-6)
+    assert 1.0 - r["T"][2, 2] == pytest.approx(0.99, abs=1e-6)
+    ro = scn.render(cam)
+    np.testing.assert_array_equal(r["ncontrib"], ro["ncontrib"])
+    np.testing.assert_allclose(r["rgb"], ro["rgb"], atol=1e-5, rtol=0)
     Ho = scn.view_hessian(cam)
     Hg = nbv.view_hessian(cam).cpu().numpy().astype(np.float64)
     assert block_rel_err(Hg, Ho).max() < 1e-3
