@@ -43,7 +43,7 @@ FP32_LANES_PER_SM = 128
 FLOP_TEST = 11            # (pixel, list entry) evaluated: dx, dy, power, two range tests
 FLOP_FWD_PAIR = 31        # composited pair, S3: exp, alpha, T update, 4 blended channels
 FLOP_BWD_PAIR = {3: 134, 4: 154}   # composited pair, S4: exp, beta, 34 / 40 moment updates
-BYTES_PER_KEY = 8         # S2: a (tile, depth) key must be written once and read once (4 + 4 B)
+BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
 
 
 def parse_args():
@@ -55,6 +55,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-sample-views", type=int, default=0, help="oracle sample size (0 = automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--concurrency", type=int, default=0, help="views in flight (0 = library default)")
     return ap.parse_args()
 
 
@@ -213,6 +214,8 @@ def main():
         wl.cand_cams = synth.hemisphere_cameras(c["C"], c["radius"], c["W"], c["H"], f, f, np.random.default_rng(10_000 + rank))
 
     nbv = api.NBV(channel_mask=wl.channel_mask)
+    if args.concurrency:
+        nbv.set_concurrency(args.concurrency)
     t0 = time.perf_counter()
     nbv.load_scene(wl.scene)
     torch.cuda.synchronize()
@@ -271,7 +274,7 @@ def main():
     barrier()
 
     # ---- counts of the same views (untimed pass) for the algorithmic work ----
-    tot = dict(n_visible=0, n_keys=0, n_entries=0, n_pairs=0, n_touched=0)
+    tot = dict(n_visible=0, n_keys=0, n_entries=0, n_pairs=0, n_touched=0, n_coarse=0)
     for cam in wl.cand_cams:
         nbv.gaussian_gains(cam, wl.target_obj)
         st = nbv.last_view_stats()
@@ -304,7 +307,7 @@ def main():
     work = {
         "backward": ("alu", (tests * FLOP_TEST + avg["n_pairs"] * FLOP_BWD_PAIR[nch]) / 1e12, alu_peak, "TFLOP/s"),
         "forward": ("alu", (tests * FLOP_TEST + avg["n_pairs"] * FLOP_FWD_PAIR) / 1e12, alu_peak, "TFLOP/s"),
-        "tile_sort": ("hbm", avg["n_keys"] * BYTES_PER_KEY / 1e9, peaks["hbm_gbs"], "GB/s"),
+        "coarse_sort": ("hbm", avg["n_coarse"] * BYTES_PER_KEY / 1e9, peaks["hbm_gbs"], "GB/s"),
     }
     rl = {}
     for k, (bound, amount, peak, unit) in work.items():

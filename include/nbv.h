@@ -86,10 +86,11 @@ typedef struct nbv_ctx nbv_ctx;
 /* Per-view counters of the last view processed (diagnostics and roofline accounting; host readable). */
 typedef struct nbv_view_stats {
   int64_t n_visible;      /* Gaussians surviving the culls */
-  int64_t n_keys;         /* (tile, Gaussian) keys emitted = sum of rect areas */
+  int64_t n_keys;         /* total length of the tile lists (R-5) = sum of rect areas; the hot path never materialises them */
   int64_t n_entries;      /* (tile, Gaussian) list entries walked by the forward pass before the tile terminated */
   int64_t n_pairs;        /* (pixel, Gaussian) pairs composited = sum of per-pixel contributor counts */
   int64_t n_touched;      /* Gaussians with a non-zero block in this view */
+  int64_t n_coarse;       /* (supertile, Gaussian) keys of the coarse binning pass */
 } nbv_view_stats;
 
 void nbv_default_config(nbv_config* cfg);
@@ -99,6 +100,12 @@ void nbv_default_config(nbv_config* cfg);
 int nbv_create(nbv_ctx** out, const nbv_config* cfg);
 void nbv_destroy(nbv_ctx* ctx);
 const char* nbv_last_error(const nbv_ctx* ctx);
+
+/* Number of views processed concurrently (each on its own internal stream, forked from and joined back into the
+ * caller's stream with events; 1 = everything on the caller's stream).  Default 4; the NBV_CONCURRENCY environment
+ * variable overrides the default at nbv_create.  Views are independent (the arg max is over per-view gains),
+ * so this changes no result beyond the order of floating-point atomics.  Errors: INVALID_ARG outside [1, 16]. */
+int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight);
 
 /* S0 -- load the Gaussian map G with object vectors: device arrays, row-major, float32.
  *   d_mean N x 3, d_logscale N x 3, d_quat N x 4 (w,x,y,z; any non-zero norm), d_opacity N (sigma in (0,1)),
@@ -137,12 +144,12 @@ int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream);
 
 /* ---- measurement ------------------------------------------------------------------------------------ */
 
-/* Stages of one view, in stream order: S1 | depth radix sort | gather + scan + key
- * emission | tile-digit radix passes + tile ranges | S3 | S4 | S5 + S6. */
+/* Stages of one view, in stream order: S1 | depth radix sort | gather + scan + coarse key
+ * emission | supertile-digit radix pass + ranges + rect gather | S3 (with the lazy tile-list filter) | S4 | S5 + S6. */
 #define NBV_STAGE_PROJECT 0
 #define NBV_STAGE_DEPTH_SORT 1
 #define NBV_STAGE_BIN 2
-#define NBV_STAGE_TILE_SORT 3
+#define NBV_STAGE_COARSE_SORT 3
 #define NBV_STAGE_FORWARD 4
 #define NBV_STAGE_BACKWARD 5
 #define NBV_STAGE_EXPAND 6
@@ -167,11 +174,19 @@ int64_t nbv_kernel_launches(void);
 int nbv_projected(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t* d_visible, float* d_rec, int32_t* d_rect,
                   void* stream);
 
-/* S2 output of one view: d_offsets (tiles+1 int64, tile t = ty*ceil(W/16)+tx lists [offsets[t], offsets[t+1]))
+/* S2 output of one view, materialised in full (the timed path produces each list lazily inside S3 and only as far as
+ * its tile needs; this export applies the same test to the same coarse lists without stopping):
+ * d_offsets (tiles+1 int64, tile t = ty*ceil(W/16)+tx lists [offsets[t], offsets[t+1]))
  * and d_ids (Gaussian indices in depth order per tile, capacity `cap` entries).  *h_total receives the number
  * of entries; if it exceeds cap, d_ids is not written and NBV_ERR_CAPACITY is returned.  Synchronises. */
 int nbv_tile_lists(nbv_ctx* ctx, const nbv_camera* h_cam, int64_t* d_offsets, int32_t* d_ids, int64_t cap,
                    int64_t* h_total, void* stream);
+
+/* What the hot path actually walked in one view: d_walked (tiles int32) = number of leading entries of each tile's
+ * list that S3 consumed before all 256 pixels had terminated (a prefix of the list nbv_tile_lists returns);
+ * d_last (H x W int32, may be NULL) = per pixel, 1 + the position in its tile's list of the last Gaussian composited
+ * (0 if none).  Invariant: max of d_last over a tile's pixels <= d_walked[tile] <= length of the tile's list. */
+int nbv_tile_walk(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t* d_walked, int32_t* d_last, void* stream);
 
 /* S3 output of one view: d_rgb H x W x 3, d_depth H x W, d_T H x W (final transmittance), d_ncontrib H x W int32
  * (number of composited Gaussians per pixel).  Any output may be NULL. */

@@ -34,10 +34,11 @@ EXPORTS = [
     "nbv_default_config", "nbv_create", "nbv_destroy", "nbv_last_error", "nbv_load_gaussians", "nbv_reset_training",
     "nbv_accumulate_training", "nbv_score_candidates", "nbv_score_candidates_host", "nbv_last_view_stats",
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
-    "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches",
+    "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
+    "nbv_tile_walk",
 ]
 
-STAGES = ["project", "depth_sort", "bin", "tile_sort", "forward", "backward", "expand_gain"]
+STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
 
 
 class NBVError(RuntimeError):
@@ -60,7 +61,7 @@ class Config(C.Structure):
 class ViewStats(C.Structure):
     """nbv_view_stats"""
     _fields_ = [("n_visible", C.c_int64), ("n_keys", C.c_int64), ("n_entries", C.c_int64), ("n_pairs", C.c_int64),
-                ("n_touched", C.c_int64)]
+                ("n_touched", C.c_int64), ("n_coarse", C.c_int64)]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
@@ -203,6 +204,9 @@ class NBV:
                                                        C.c_void_p(scores.ctypes.data), C.byref(best), _stream()))
         return scores[:n], int(best.value)
 
+    def set_concurrency(self, views_in_flight: int):
+        self._check(self.lib.nbv_set_concurrency(self._h, int(views_in_flight)))
+
     def last_view_stats(self) -> dict:
         st = ViewStats()
         self._check(self.lib.nbv_last_view_stats(self._h, C.byref(st), _stream()))
@@ -246,6 +250,17 @@ class NBV:
         self._check(self.lib.nbv_tile_lists(self._h, C.c_void_p(cam.ctypes.data), _ptr(offsets), _ptr(ids), C.c_int64(ids.numel()),
                                             C.byref(total), _stream()))
         return offsets, ids[: int(total.value)]
+
+    def tile_walk(self, cam):
+        """nbv_tile_walk: (walked per tile, last per pixel)"""
+        torch = self._torch
+        cam = _cams(cam)
+        W, H = int(cam["width"][0]), int(cam["height"][0])
+        nt = ((W + 15) // 16) * ((H + 15) // 16)
+        walked = torch.empty(nt, dtype=torch.int32, device=self.device)
+        last = torch.empty((H, W), dtype=torch.int32, device=self.device)
+        self._check(self.lib.nbv_tile_walk(self._h, C.c_void_p(cam.ctypes.data), _ptr(walked), _ptr(last), _stream()))
+        return walked, last
 
     def render(self, cam):
         torch = self._torch

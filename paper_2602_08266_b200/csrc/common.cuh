@@ -24,13 +24,22 @@ struct __align__(16) Splat {
 };
 
 struct ViewCounters {          // device-side counters of one view
-  unsigned long long n_keys;   // sum of rect areas
-  unsigned long long n_entries;
-  unsigned long long n_pairs;
+  unsigned long long n_keys;   // sum of rect areas = length of all tile lists (R-5); not materialised on the hot path
+  unsigned long long n_entries;// tile-list entries the forward pass walked before its tile terminated
+  unsigned long long n_pairs;  // (pixel, Gaussian) pairs composited
   unsigned int n_visible;
-  unsigned int n_touched;
+  unsigned int n_touched;      // Gaussians with a non-zero block in this view (= length of the touched list)
   unsigned int bad_data;
-  unsigned int pad;
+  unsigned int n_coarse;       // (supertile, Gaussian) keys of the coarse binning
+  unsigned int n_expanded;     // touched Gaussians consumed by the expand kernel (work-queue cursor)
+  unsigned int pad[3];
+};
+
+// Tile grid of one view and its supertiles (S x S tiles, S = 1 << sshift).
+struct TileGrid {
+  int tiles_x, tiles_y;
+  int sshift;
+  int super_x, super_y;
 };
 
 // ---------------------------------------------------------------------------------------------

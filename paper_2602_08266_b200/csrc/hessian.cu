@@ -252,49 +252,49 @@ __device__ float gain_solve(float* B, const float* U) {
 }
 
 __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam, nbv_config cfg, const uint32_t* __restrict__ ids_sorted,
-                                                     const float* __restrict__ moments, int mode, float* __restrict__ H_T,
-                                                     float* __restrict__ out_blocks, const float* __restrict__ conf,
-                                                     const float* __restrict__ cholT, float* __restrict__ score,
-                                                     float* __restrict__ gains, ViewCounters* counters) {
-  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+                                                     const uint32_t* __restrict__ touched, float* __restrict__ moments, int mode,
+                                                     float* __restrict__ H_T, float* __restrict__ out_blocks,
+                                                     const float* __restrict__ conf, const float* __restrict__ cholT,
+                                                     float* __restrict__ score, float* __restrict__ gains, ViewCounters* counters) {
+  const uint32_t n_touched = counters->n_touched;
   float gain = 0.f;
-  bool touched = false;
-  if (r < sc.N) {
-    const float* mom = moments + (size_t)r * NMOM;
-    touched = mom[MOM_W2] > 0.f;
-    if (touched) {
-      const uint32_t g = ids_sorted[r];
-      float m[NMOM];
+  float omega[4];
 #pragma unroll
-      for (int i = 0; i < NMOM / 4; ++i) {
-        const float4 v = reinterpret_cast<const float4*>(mom)[i];
-        m[4 * i] = v.x; m[4 * i + 1] = v.y; m[4 * i + 2] = v.z; m[4 * i + 3] = v.w;
-      }
-      ChainF ch;
-      chain_f(cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
-      const float sg = sc.sigma[g];
-      const float kappa = cfg.opacity_coord == 0 ? (1.f - sg) : 1.f / sg;       // R-10
-      float omega[4];
+  for (int c = 0; c < 4; ++c) omega[c] = ((cfg.channel_mask >> c) & 1) ? cfg.channel_weight[c] : 0.f;
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < n_touched; t += gridDim.x * blockDim.x) {
+    const uint32_t r = touched[t];
+    const uint32_t g = ids_sorted[r];
+    float4* mom4 = reinterpret_cast<float4*>(moments + (size_t)r * NMOM);
+    float m[NMOM];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) omega[c] = ((cfg.channel_mask >> c) & 1) ? cfg.channel_weight[c] : 0.f;
-      float H[NBLK];
-      build_block(m, ch, kappa, omega, H);
-      if (mode == EXPAND_TRAIN) {
-        float* dst = H_T + (size_t)g * NBLK;
-        for (int i = 0; i < NBLK; ++i) dst[i] += H[i];
-      } else if (mode == EXPAND_VIEW) {
-        float* dst = out_blocks + (size_t)g * NBLK;
-        for (int i = 0; i < NBLK; ++i) dst[i] = H[i];
-      } else {
-        const float c = conf[g];
-        if (c > 0.f) {                       // c_g = 0 (Eq. 12, non-target): exactly zero gain
-          float U[NBLK];
-          const float* ut = cholT + (size_t)g * NBLK;
-          for (int i = 0; i < NBLK; ++i) { U[i] = ut[i]; H[i] *= c; }
-          gain = gain_solve(H, U);
-        }
-        if (gains) gains[g] = gain;
+    for (int i = 0; i < NMOM / 4; ++i) {
+      const float4 v = mom4[i];
+      m[4 * i] = v.x; m[4 * i + 1] = v.y; m[4 * i + 2] = v.z; m[4 * i + 3] = v.w;
+      mom4[i] = make_float4(0.f, 0.f, 0.f, 0.f);     // leave the buffer zeroed for the next view
+    }
+    ChainF ch;
+    chain_f(cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
+    const float sg = sc.sigma[g];
+    const float kappa = cfg.opacity_coord == 0 ? (1.f - sg) : 1.f / sg;       // R-10
+    float H[NBLK];
+    build_block(m, ch, kappa, omega, H);
+    if (mode == EXPAND_TRAIN) {
+      float* dst = H_T + (size_t)g * NBLK;             // views run concurrently on several streams: atomic accumulation
+      for (int i = 0; i < NBLK; ++i) atomicAdd(dst + i, H[i]);
+    } else if (mode == EXPAND_VIEW) {
+      float* dst = out_blocks + (size_t)g * NBLK;
+      for (int i = 0; i < NBLK; ++i) dst[i] = H[i];
+    } else {
+      const float c = conf[g];
+      float gn = 0.f;
+      if (c > 0.f) {                       // c_g = 0 (Eq. 12, non-target): exactly zero gain
+        float U[NBLK];
+        const float* ut = cholT + (size_t)g * NBLK;
+        for (int i = 0; i < NBLK; ++i) { U[i] = ut[i]; H[i] *= c; }
+        gn = gain_solve(H, U);
       }
+      if (gains) gains[g] = gn;
+      gain += gn;
     }
   }
   if (mode == EXPAND_GAIN) {
@@ -308,16 +308,16 @@ __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam,
       if (t != 0.f) atomicAdd(score, t);
     }
   }
-  const unsigned tm = __ballot_sync(0xffffffffu, touched);
-  if ((threadIdx.x & 31) == 0 && tm) atomicAdd(&counters->n_touched, (unsigned)__popc(tm));
 }
 
 void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
-                   const float* moments, int mode, float* H_T, float* out_blocks, const float* conf, const float* cholT,
-                   float* score, float* gains, ViewCounters* counters, cudaStream_t st) {
+                   const uint32_t* touched, float* moments, int mode, float* H_T, float* out_blocks, const float* conf,
+                   const float* cholT, float* score, float* gains, ViewCounters* counters, cudaStream_t st) {
+  int blocks = (sc.N + 63) / 64;
+  if (blocks > 148 * 8) blocks = 148 * 8;
   ++g_kernel_launches;
-  expand_kernel<<<(sc.N + 63) / 64, 64, 0, st>>>(sc, cam, cfg, ids_sorted, moments, mode, H_T, out_blocks, conf, cholT, score,
-                                                 gains, counters);
+  expand_kernel<<<blocks, 64, 0, st>>>(sc, cam, cfg, ids_sorted, touched, moments, mode, H_T, out_blocks, conf, cholT, score, gains,
+                                       counters);
 }
 
 // S0': confidence (Eq. 7; Eq. 12)

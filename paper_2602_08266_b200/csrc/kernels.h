@@ -11,8 +11,11 @@ size_t scan_temp_words(size_t n);
 void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* tmp, uint32_t* total_out, cudaStream_t st);
 size_t radix_temp_words(size_t n);
 // one stable pass over `bits` (<= 8) bits at `shift`; vals_in == nullptr -> keys only
+// n: number of keys, or (d_n != nullptr) the capacity the grids are sized for with the length read from *d_n.
+// On return tmp[digit * radix_blocks(n)] holds the start of every digit in the output.
 void radix_pass(const uint32_t* keys_in, uint32_t* keys_out, const uint32_t* vals_in, uint32_t* vals_out, size_t n,
-                int shift, int bits, uint32_t* tmp, cudaStream_t st);
+                const uint32_t* d_n, int shift, int bits, uint32_t* tmp, cudaStream_t st);
+uint32_t radix_blocks(size_t n);
 
 // ---- project.cu
 struct SceneDev {            // device arrays of the loaded map
@@ -33,13 +36,19 @@ void launch_project(const SceneDev& sc, const nbv_camera& cam, const nbv_config&
                     uint32_t* ids, ushort4* rect, float* abc, ViewCounters* counters, cudaStream_t st);
 
 // ---- binning.cu
-void launch_gather(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, Splat* splat_sorted,
-                   ushort4* rect_sorted, uint32_t* ntiles_sorted, cudaStream_t st);
-void launch_emit_keys(const ushort4* rect_sorted, const uint32_t* offsets, int N, int tiles_x, int rank_bits,
-                      uint32_t* keys, cudaStream_t st);
-void launch_tile_ranges(const uint32_t* keys, size_t n_keys, int rank_bits, uint2* ranges, int n_tiles, cudaStream_t st);
-void launch_export_lists(const uint32_t* keys, size_t n_keys, int rank_bits, const uint32_t* ids_sorted, const uint2* ranges,
-                         int n_tiles, int64_t* offsets, int32_t* ids_out, uint32_t* tmp_counts, uint32_t* scan_tmp, cudaStream_t st);
+void launch_gather(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, int sshift, Splat* splat_sorted,
+                   ushort4* rect_sorted, uint32_t* ncoarse_sorted, cudaStream_t st);
+void launch_emit_coarse(const ushort4* rect_sorted, const uint32_t* offsets, int N, int sshift, int super_x, int rank_bits,
+                        uint32_t cap, uint32_t* keys, cudaStream_t st);
+void launch_coarse_ranges(const uint32_t* hist_scanned, uint32_t nb, int n_super, int n_digits, const uint32_t* d_n, uint32_t cap,
+                          uint2* ranges, cudaStream_t st);
+void launch_coarse_rect(const uint32_t* keys, const uint32_t* d_n, uint32_t cap, int rank_bits, const ushort4* rect_sorted,
+                        ushort4* crect, cudaStream_t st);
+// parity export of the full tile lists: counts -> scanned offsets (+ total) -> ids
+void launch_tile_counts(const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg, int rank_bits,
+                        uint32_t* counts, uint32_t* scanned, uint32_t* total, uint32_t* scan_tmp, int64_t* offsets_out, cudaStream_t st);
+void launch_tile_ids(const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg, int rank_bits,
+                     const uint32_t* ids_sorted, const uint32_t* scanned, int32_t* ids_out, cudaStream_t st);
 
 // ---- raster.cu
 struct PixelBuf {            // per-pixel outputs of the forward pass (H x W each)
@@ -49,17 +58,23 @@ struct PixelBuf {            // per-pixel outputs of the forward pass (H x W eac
   int32_t* ncontrib;
   int32_t* last;             // list position (relative to the tile's range) after the last composited entry
 };
-void launch_forward(const Splat* splat_sorted, const uint32_t* keys, const uint2* ranges, int rank_bits, int W, int H,
-                    const nbv_config& cfg, PixelBuf px, ViewCounters* counters, cudaStream_t st);
-void launch_backward(const Splat* splat_sorted, const uint32_t* keys, const uint2* ranges, int rank_bits, int W, int H,
-                     const nbv_config& cfg, PixelBuf px, float* moments, cudaStream_t st);
+void launch_forward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
+                    int rank_bits, int W, int H, const nbv_config& cfg, PixelBuf px, uint32_t* tile_cend, uint32_t* tile_walk,
+                    ViewCounters* counters, cudaStream_t st);
+// moments must be zero on entry for every Gaussian; `touched` receives the ranks with a non-zero block
+// (counters->n_touched of them, in no particular order)
+void launch_backward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
+                     int rank_bits, int W, int H, const nbv_config& cfg, PixelBuf px, const uint32_t* tile_cend, float* moments,
+                     uint32_t* touched, ViewCounters* counters, cudaStream_t st);
 
 // ---- hessian.cu
 enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2 };
 // EXPAND_TRAIN: H_T[id] += H ; EXPAND_VIEW: out_blocks[id] = H ; EXPAND_GAIN: gain vs H_T, sum into *score (and gains[id] if not null)
+// Consumes the touched list: reads the moments of every touched rank and writes zeros back (the moment buffer is
+// all-zero again afterwards).
 void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
-                   const float* moments, int mode, float* H_T, float* out_blocks, const float* conf, const float* cholT,
-                   float* score, float* gains, ViewCounters* counters, cudaStream_t st);
+                   const uint32_t* touched, float* moments, int mode, float* H_T, float* out_blocks, const float* conf,
+                   const float* cholT, float* score, float* gains, ViewCounters* counters, cudaStream_t st);
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);
 void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);

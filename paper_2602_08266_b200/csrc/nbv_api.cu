@@ -2,6 +2,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <utility>
@@ -25,6 +26,28 @@ struct DevBuf {
 
 }  // namespace
 
+// Work buffers of one view in flight.  Views are independent, so several slots run concurrently on their own streams
+// (DESIGN.md section 5); the parity exports use slot 0 on the caller's stream.
+struct ViewSlot {
+  cudaStream_t st = nullptr;
+  cudaEvent_t done = nullptr;
+  DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, ncoarse, offsets;
+  DevBuf ckeys, ckeys_alt, crect, cranges, sort_tmp, scan_tmp, tile_counts;
+  DevBuf pix_rgb, pix_depth, pix_T, pix_nc, pix_last, tile_cend, tile_walk, moments, touched;
+  ViewCounters* d_counters = nullptr;
+  ViewCounters* h_counters = nullptr;   // pinned
+  // products of the last process_view()
+  TileGrid tg = {0, 0, 0, 0, 0};
+  int rank_bits = 1;
+  uint32_t ccap = 0;                    // capacity of the coarse key buffers
+  uint32_t* ckeys_sorted = nullptr;
+  bool moments_clean = false;           // the moment buffer is known to be all zero
+  // per-stage timing: one event row per view, folded on read-out
+  std::vector<cudaEvent_t> ev;          // ev[view * (NBV_N_STAGES + 1) + boundary]
+  std::vector<unsigned> ev_mask;        // per view: bit b set when boundary b was recorded
+  size_t ev_views = 0;
+};
+
 struct nbv_ctx {
   nbv_config cfg;
   std::string err;
@@ -33,24 +56,15 @@ struct nbv_ctx {
   bool loaded = false;
   int n_train = 0;
   // scene
-  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT;
-  // per-view work buffers
-  DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, ntiles, offsets;
-  DevBuf keys, keys_alt, ranges, sort_tmp, scan_tmp, tile_counts;
-  DevBuf pix_rgb, pix_depth, pix_T, pix_nc, pix_last, moments, score_tmp;
-  ViewCounters* d_counters = nullptr;
-  ViewCounters* h_counters = nullptr;   // pinned
-  // products of the last process_view()
-  int rank_bits = 1;
-  size_t n_keys = 0;
-  uint32_t* keys_sorted = nullptr;
-  int cur_W = 0, cur_H = 0;
+  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp;
   int conf_target = -2;                 // target the conf / cholT buffers were prepared for (-2 = stale)
-  // optional per-stage timing (nbv_set_stage_timing): one event row per view, folded on read-out
+  // views in flight
+  std::vector<ViewSlot*> slots;
+  int concurrency = 4;
+  cudaEvent_t ev_fork = nullptr;
+  ViewSlot* last_slot = nullptr;        // slot of the last view processed (nbv_last_view_stats)
+  // optional per-stage timing (nbv_set_stage_timing)
   bool timing = false;
-  std::vector<cudaEvent_t> ev;          // ev[view * (NBV_N_STAGES + 1) + boundary]
-  std::vector<unsigned> ev_mask;        // per view: bit b set when boundary b was recorded
-  size_t ev_views = 0;
   double stage_ms[NBV_N_STAGES] = {0};
   long long timed_views = 0;
 };
@@ -138,150 +152,239 @@ SceneDev scene_dev(const nbv_ctx* c) {
   return s;
 }
 
-PixelBuf pixel_buf(const nbv_ctx* c) {
-  PixelBuf p;
-  p.rgb = c->pix_rgb.as<float>(); p.depth = c->pix_depth.as<float>(); p.T = c->pix_T.as<float>();
-  p.ncontrib = c->pix_nc.as<int32_t>(); p.last = c->pix_last.as<int32_t>();
-  return p;
-}
-
 constexpr int EV_ROW = NBV_N_STAGES + 1;
 constexpr size_t EV_MAX_VIEWS = 1024;
 
-// fold the recorded event rows into ctx->stage_ms (the stream must be idle)
-void fold_timing(nbv_ctx* ctx) {
-  for (size_t v = 0; v < ctx->ev_views; ++v) {
-    const unsigned m = ctx->ev_mask[v];
+// fold the recorded event rows of a slot into ctx->stage_ms (its stream must be idle)
+void fold_timing(nbv_ctx* ctx, ViewSlot* sl) {
+  for (size_t v = 0; v < sl->ev_views; ++v) {
+    const unsigned m = sl->ev_mask[v];
     for (int s = 0; s < NBV_N_STAGES; ++s)
       if (((m >> s) & 1u) && ((m >> (s + 1)) & 1u)) {
         float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, ctx->ev[v * EV_ROW + s], ctx->ev[v * EV_ROW + s + 1]) == cudaSuccess) ctx->stage_ms[s] += ms;
+        if (cudaEventElapsedTime(&ms, sl->ev[v * EV_ROW + s], sl->ev[v * EV_ROW + s + 1]) == cudaSuccess) ctx->stage_ms[s] += ms;
       }
     if (m) ctx->timed_views++;
-    ctx->ev_mask[v] = 0;
+    sl->ev_mask[v] = 0;
   }
   cudaGetLastError();
-  ctx->ev_views = 0;
+  sl->ev_views = 0;
 }
 
-// start a new event row for the next view
-void timing_begin_view(nbv_ctx* ctx, cudaStream_t st) {
+// start a new event row for the next view of this slot
+void timing_begin_view(nbv_ctx* ctx, ViewSlot* sl, cudaStream_t st) {
   if (!ctx->timing) return;
-  if (ctx->ev_views >= EV_MAX_VIEWS) { cudaStreamSynchronize(st); fold_timing(ctx); }
-  const size_t v = ctx->ev_views++;
-  if (ctx->ev.size() < (v + 1) * EV_ROW) {
-    const size_t old = ctx->ev.size();
-    ctx->ev.resize((v + 1) * EV_ROW);
-    for (size_t i = old; i < ctx->ev.size(); ++i) cudaEventCreate(&ctx->ev[i]);
-    ctx->ev_mask.resize(v + 1, 0u);
+  if (sl->ev_views >= EV_MAX_VIEWS) { cudaStreamSynchronize(st); fold_timing(ctx, sl); }
+  const size_t v = sl->ev_views++;
+  if (sl->ev.size() < (v + 1) * EV_ROW) {
+    const size_t old = sl->ev.size();
+    sl->ev.resize((v + 1) * EV_ROW);
+    for (size_t i = old; i < sl->ev.size(); ++i) cudaEventCreate(&sl->ev[i]);
+    sl->ev_mask.resize(v + 1, 0u);
   }
-  ctx->ev_mask[v] = 0;
+  sl->ev_mask[v] = 0;
 }
 
-// record boundary b (= start of stage b, end of stage b-1) of the current view
-void mark(nbv_ctx* ctx, int b, cudaStream_t st) {
-  if (!ctx->timing || ctx->ev_views == 0) return;
-  const size_t v = ctx->ev_views - 1;
-  cudaEventRecord(ctx->ev[v * EV_ROW + b], st);
-  ctx->ev_mask[v] |= 1u << b;
+// record boundary b (= start of stage b, end of stage b-1) of the slot's current view
+void mark(nbv_ctx* ctx, ViewSlot* sl, int b, cudaStream_t st) {
+  if (!ctx->timing || sl->ev_views == 0) return;
+  const size_t v = sl->ev_views - 1;
+  cudaEventRecord(sl->ev[v * EV_ROW + b], st);
+  sl->ev_mask[v] |= 1u << b;
+}
+
+void free_slot(ViewSlot* sl) {
+  if (!sl) return;
+  DevBuf* all[] = {&sl->splat, &sl->zkey, &sl->zkey_alt, &sl->ids, &sl->ids_alt, &sl->rect, &sl->abc, &sl->splat_sorted,
+                   &sl->rect_sorted, &sl->ncoarse, &sl->offsets, &sl->ckeys, &sl->ckeys_alt, &sl->crect, &sl->cranges, &sl->sort_tmp,
+                   &sl->scan_tmp, &sl->tile_counts, &sl->pix_rgb, &sl->pix_depth, &sl->pix_T, &sl->pix_nc, &sl->pix_last,
+                   &sl->tile_cend, &sl->tile_walk, &sl->moments, &sl->touched};
+  for (DevBuf* b : all) release(*b);
+  if (sl->d_counters) cudaFree(sl->d_counters);
+  if (sl->h_counters) cudaFreeHost(sl->h_counters);
+  for (cudaEvent_t e : sl->ev) cudaEventDestroy(e);
+  if (sl->done) cudaEventDestroy(sl->done);
+  if (sl->st) cudaStreamDestroy(sl->st);
+  delete sl;
+}
+
+// slot i, created on first use
+int get_slot(nbv_ctx* ctx, int i, ViewSlot** out) {
+  while ((int)ctx->slots.size() <= i) {
+    ViewSlot* sl = new ViewSlot;
+    bool ok = cudaStreamCreateWithFlags(&sl->st, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaEventCreateWithFlags(&sl->done, cudaEventDisableTiming) == cudaSuccess &&
+              cudaMalloc(&sl->d_counters, sizeof(ViewCounters)) == cudaSuccess &&
+              cudaMallocHost(&sl->h_counters, sizeof(ViewCounters)) == cudaSuccess;
+    if (!ok) {
+      cudaGetLastError();
+      free_slot(sl);
+      return fail(ctx, NBV_ERR_CUDA, "cannot create a view slot (stream, event or counters)");
+    }
+    std::memset(sl->h_counters, 0, sizeof(ViewCounters));
+    cudaMemset(sl->d_counters, 0, sizeof(ViewCounters));
+    ctx->slots.push_back(sl);
+  }
+  *out = ctx->slots[i];
+  return NBV_OK;
+}
+
+// supertile edge (in tiles, a power of two >= 8) such that the view has at most 256 supertiles
+TileGrid make_grid(int W, int H) {
+  TileGrid tg;
+  tg.tiles_x = (W + TILE - 1) / TILE;
+  tg.tiles_y = (H + TILE - 1) / TILE;
+  tg.sshift = 3;
+  for (;;) {
+    const int S = 1 << tg.sshift;
+    tg.super_x = (tg.tiles_x + S - 1) / S;
+    tg.super_y = (tg.tiles_y + S - 1) / S;
+    if ((long long)tg.super_x * tg.super_y <= 256) break;
+    ++tg.sshift;
+  }
+  return tg;
 }
 
 enum Stage { STAGE_PROJECT = 0, STAGE_BIN = 1, STAGE_FORWARD = 2, STAGE_BACKWARD = 3 };
 
-// S1..S4 for one camera.  Leaves the depth order in ctx->ids, rank-ordered splats, sorted keys, tile ranges,
-// per-pixel buffers and (STAGE_BACKWARD) the moment buffer.  Synchronises the stream once (key count read-back).
-int process_view(nbv_ctx* ctx, const nbv_camera& cam, int upto, bool want_abc, cudaStream_t st) {
+// S1..S4 for one camera on stream st, in the buffers of slot sl.  Leaves the depth order in sl->ids, rank-ordered splats,
+// the sorted coarse lists, per-pixel buffers and (STAGE_BACKWARD) the moment buffer + touched list.  Never synchronises.
+// full_pix: also write the colour / depth / count images (parity exports); the hot path needs only T and `last`.
+int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool want_abc, bool full_pix, cudaStream_t st) {
   if (!valid_camera(cam)) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
   const int N = ctx->N;
-  const int TX = (cam.width + TILE - 1) / TILE, TY = (cam.height + TILE - 1) / TILE;
-  const int n_tiles = TX * TY;
-  const int rank_bits = ceil_log2((size_t)N), tile_bits = ceil_log2((size_t)n_tiles);
-  if (rank_bits + tile_bits > 32)
-    return fail(ctx, NBV_ERR_INVALID_ARG, "N x tiles exceeds the 32-bit (tile | depth rank) key space");
-  ctx->rank_bits = rank_bits;
-  ctx->cur_W = cam.width; ctx->cur_H = cam.height;
+  const TileGrid tg = make_grid(cam.width, cam.height);
+  const int n_tiles = tg.tiles_x * tg.tiles_y, n_super = tg.super_x * tg.super_y;
+  const int rank_bits = ceil_log2((size_t)N), super_bits = ceil_log2((size_t)n_super);
+  if (rank_bits + super_bits > 32)
+    return fail(ctx, NBV_ERR_INVALID_ARG, "N x supertiles exceeds the 32-bit (supertile | depth rank) key space");
+  const unsigned long long worst = (unsigned long long)N * (unsigned long long)n_super;
+  if (worst > 0x40000000ull) return fail(ctx, NBV_ERR_CAPACITY, "N x supertiles exceeds the coarse key buffer limit (2^30)");
+  const uint32_t ccap = (uint32_t)worst;     // worst case: no overflow is possible, no count has to come back to the host
+  sl->tg = tg; sl->rank_bits = rank_bits; sl->ccap = ccap;
+  ctx->last_slot = sl;
   const SceneDev sc = scene_dev(ctx);
 
-  CKRET(ensure(ctx, ctx->splat, sizeof(Splat) * (size_t)N));
-  CKRET(ensure(ctx, ctx->zkey, 4 * (size_t)N)); CKRET(ensure(ctx, ctx->zkey_alt, 4 * (size_t)N));
-  CKRET(ensure(ctx, ctx->ids, 4 * (size_t)N)); CKRET(ensure(ctx, ctx->ids_alt, 4 * (size_t)N));
-  CKRET(ensure(ctx, ctx->rect, sizeof(ushort4) * (size_t)N));
-  if (want_abc) CKRET(ensure(ctx, ctx->abc, 12 * (size_t)N));
-  CKRET(ensure(ctx, ctx->sort_tmp, 4 * radix_temp_words((size_t)N)));
-  CKRET(ensure(ctx, ctx->scan_tmp, 4 * scan_temp_words((size_t)N + 1)));
+  CKRET(ensure(ctx, sl->splat, sizeof(Splat) * (size_t)N));
+  CKRET(ensure(ctx, sl->zkey, 4 * (size_t)N)); CKRET(ensure(ctx, sl->zkey_alt, 4 * (size_t)N));
+  CKRET(ensure(ctx, sl->ids, 4 * (size_t)N)); CKRET(ensure(ctx, sl->ids_alt, 4 * (size_t)N));
+  CKRET(ensure(ctx, sl->rect, sizeof(ushort4) * (size_t)N));
+  if (want_abc) CKRET(ensure(ctx, sl->abc, 12 * (size_t)N));
+  CKRET(ensure(ctx, sl->sort_tmp, 4 * radix_temp_words(std::max((size_t)N, (size_t)ccap))));
+  CKRET(ensure(ctx, sl->scan_tmp, 4 * scan_temp_words(std::max((size_t)N + 1, (size_t)n_tiles + 1))));
 
-  CK(cudaMemsetAsync(ctx->d_counters, 0, sizeof(ViewCounters), st));
-  timing_begin_view(ctx, st);
-  mark(ctx, NBV_STAGE_PROJECT, st);
-  launch_project(sc, cam, ctx->cfg, ctx->splat.as<Splat>(), ctx->zkey.as<uint32_t>(), ctx->ids.as<uint32_t>(),
-                 ctx->rect.as<ushort4>(), want_abc ? ctx->abc.as<float>() : nullptr, ctx->d_counters, st);
+  CK(cudaMemsetAsync(sl->d_counters, 0, sizeof(ViewCounters), st));
+  timing_begin_view(ctx, sl, st);
+  mark(ctx, sl, NBV_STAGE_PROJECT, st);
+  launch_project(sc, cam, ctx->cfg, sl->splat.as<Splat>(), sl->zkey.as<uint32_t>(), sl->ids.as<uint32_t>(),
+                 sl->rect.as<ushort4>(), want_abc ? sl->abc.as<float>() : nullptr, sl->d_counters, st);
   CK(cudaGetLastError());
   if (upto == STAGE_PROJECT) return NBV_OK;
 
   // depth sort: 4 stable passes of 8 bits on the z bits, Gaussian index as value (ties keep index order: R-7)
-  mark(ctx, NBV_STAGE_DEPTH_SORT, st);
+  mark(ctx, sl, NBV_STAGE_DEPTH_SORT, st);
   {
-    uint32_t *k0 = ctx->zkey.as<uint32_t>(), *k1 = ctx->zkey_alt.as<uint32_t>();
-    uint32_t *v0 = ctx->ids.as<uint32_t>(), *v1 = ctx->ids_alt.as<uint32_t>();
+    uint32_t *k0 = sl->zkey.as<uint32_t>(), *k1 = sl->zkey_alt.as<uint32_t>();
+    uint32_t *v0 = sl->ids.as<uint32_t>(), *v1 = sl->ids_alt.as<uint32_t>();
     for (int pass = 0; pass < 4; ++pass) {
-      radix_pass(k0, k1, v0, v1, (size_t)N, 8 * pass, 8, ctx->sort_tmp.as<uint32_t>(), st);
+      radix_pass(k0, k1, v0, v1, (size_t)N, nullptr, 8 * pass, 8, sl->sort_tmp.as<uint32_t>(), st);
       std::swap(k0, k1);
       std::swap(v0, v1);
     }
     CK(cudaGetLastError());
   }
-  mark(ctx, NBV_STAGE_BIN, st);
-  CKRET(ensure(ctx, ctx->splat_sorted, sizeof(Splat) * (size_t)N));
-  CKRET(ensure(ctx, ctx->rect_sorted, sizeof(ushort4) * (size_t)N));
-  CKRET(ensure(ctx, ctx->ntiles, 4 * (size_t)N));
-  CKRET(ensure(ctx, ctx->offsets, 4 * (size_t)N));
-  launch_gather(ctx->ids.as<uint32_t>(), ctx->splat.as<Splat>(), ctx->rect.as<ushort4>(), N, ctx->splat_sorted.as<Splat>(),
-                ctx->rect_sorted.as<ushort4>(), ctx->ntiles.as<uint32_t>(), st);
-  exclusive_scan_u32(ctx->ntiles.as<uint32_t>(), ctx->offsets.as<uint32_t>(), (size_t)N, ctx->scan_tmp.as<uint32_t>(), nullptr, st);
+  // coarse binning: rank-ordered splats, supertile counts, scan, keys (supertile | rank) emitted rank-major
+  mark(ctx, sl, NBV_STAGE_BIN, st);
+  CKRET(ensure(ctx, sl->splat_sorted, sizeof(Splat) * (size_t)N));
+  CKRET(ensure(ctx, sl->rect_sorted, sizeof(ushort4) * (size_t)N));
+  CKRET(ensure(ctx, sl->ncoarse, 4 * (size_t)N));
+  CKRET(ensure(ctx, sl->offsets, 4 * (size_t)N));
+  CKRET(ensure(ctx, sl->ckeys, 4 * (size_t)ccap)); CKRET(ensure(ctx, sl->ckeys_alt, 4 * (size_t)ccap));
+  CKRET(ensure(ctx, sl->crect, sizeof(ushort4) * (size_t)ccap));
+  CKRET(ensure(ctx, sl->cranges, sizeof(uint2) * 256));
+  launch_gather(sl->ids.as<uint32_t>(), sl->splat.as<Splat>(), sl->rect.as<ushort4>(), N, tg.sshift, sl->splat_sorted.as<Splat>(),
+                sl->rect_sorted.as<ushort4>(), sl->ncoarse.as<uint32_t>(), st);
+  exclusive_scan_u32(sl->ncoarse.as<uint32_t>(), sl->offsets.as<uint32_t>(), (size_t)N, sl->scan_tmp.as<uint32_t>(),
+                     &sl->d_counters->n_coarse, st);
+  launch_emit_coarse(sl->rect_sorted.as<ushort4>(), sl->offsets.as<uint32_t>(), N, tg.sshift, tg.super_x, rank_bits, ccap,
+                     sl->ckeys.as<uint32_t>(), st);
+  // one stable pass on the supertile digit (<= 8 bits); its scanned histogram gives the supertile ranges
+  mark(ctx, sl, NBV_STAGE_COARSE_SORT, st);
+  radix_pass(sl->ckeys.as<uint32_t>(), sl->ckeys_alt.as<uint32_t>(), nullptr, nullptr, (size_t)ccap, &sl->d_counters->n_coarse,
+             rank_bits, super_bits, sl->sort_tmp.as<uint32_t>(), st);
+  sl->ckeys_sorted = sl->ckeys_alt.as<uint32_t>();
+  launch_coarse_ranges(sl->sort_tmp.as<uint32_t>(), radix_blocks((size_t)ccap), n_super, 1 << super_bits, &sl->d_counters->n_coarse,
+                       ccap, sl->cranges.as<uint2>(), st);
+  launch_coarse_rect(sl->ckeys_sorted, &sl->d_counters->n_coarse, ccap, rank_bits, sl->rect_sorted.as<ushort4>(),
+                     sl->crect.as<ushort4>(), st);
   CK(cudaGetLastError());
-  CK(cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, sizeof(ViewCounters), cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-  const unsigned long long n_keys = ctx->h_counters->n_keys;
-  if (n_keys >= 0xfff00000ull) return fail(ctx, NBV_ERR_INVALID_ARG, "more than 2^32 (tile, Gaussian) keys in one view");
-  ctx->n_keys = (size_t)n_keys;
-
-  CKRET(ensure(ctx, ctx->keys, 4 * (size_t)n_keys, true));
-  CKRET(ensure(ctx, ctx->keys_alt, 4 * (size_t)n_keys, true));
-  CKRET(ensure(ctx, ctx->sort_tmp, 4 * radix_temp_words(std::max((size_t)n_keys, (size_t)N)), true));
-  CKRET(ensure(ctx, ctx->ranges, sizeof(uint2) * (size_t)n_tiles));
-  launch_emit_keys(ctx->rect_sorted.as<ushort4>(), ctx->offsets.as<uint32_t>(), N, TX, rank_bits, ctx->keys.as<uint32_t>(), st);
-  mark(ctx, NBV_STAGE_TILE_SORT, st);
-  {
-    uint32_t *k0 = ctx->keys.as<uint32_t>(), *k1 = ctx->keys_alt.as<uint32_t>();
-    const int npass = (tile_bits + 7) / 8;
-    const int bits = (tile_bits + npass - 1) / npass;
-    for (int pass = 0; pass < npass; ++pass) {
-      radix_pass(k0, k1, nullptr, nullptr, (size_t)n_keys, rank_bits + pass * bits, bits, ctx->sort_tmp.as<uint32_t>(), st);
-      std::swap(k0, k1);
-    }
-    ctx->keys_sorted = k0;
-  }
-  launch_tile_ranges(ctx->keys_sorted, (size_t)n_keys, rank_bits, ctx->ranges.as<uint2>(), n_tiles, st);
-  CK(cudaGetLastError());
-  mark(ctx, NBV_STAGE_FORWARD, st);
+  mark(ctx, sl, NBV_STAGE_FORWARD, st);
   if (upto == STAGE_BIN) return NBV_OK;
 
   const size_t npx = (size_t)cam.width * cam.height;
-  CKRET(ensure(ctx, ctx->pix_rgb, 12 * npx)); CKRET(ensure(ctx, ctx->pix_depth, 4 * npx)); CKRET(ensure(ctx, ctx->pix_T, 4 * npx));
-  CKRET(ensure(ctx, ctx->pix_nc, 4 * npx)); CKRET(ensure(ctx, ctx->pix_last, 4 * npx));
-  launch_forward(ctx->splat_sorted.as<Splat>(), ctx->keys_sorted, ctx->ranges.as<uint2>(), rank_bits, cam.width, cam.height,
-                 ctx->cfg, pixel_buf(ctx), ctx->d_counters, st);
+  CKRET(ensure(ctx, sl->pix_T, 4 * npx)); CKRET(ensure(ctx, sl->pix_last, 4 * npx));
+  CKRET(ensure(ctx, sl->tile_cend, 4 * (size_t)n_tiles)); CKRET(ensure(ctx, sl->tile_walk, 4 * (size_t)n_tiles));
+  PixelBuf pb;
+  pb.rgb = nullptr; pb.depth = nullptr; pb.ncontrib = nullptr;
+  if (full_pix) {
+    CKRET(ensure(ctx, sl->pix_rgb, 12 * npx)); CKRET(ensure(ctx, sl->pix_depth, 4 * npx)); CKRET(ensure(ctx, sl->pix_nc, 4 * npx));
+    pb.rgb = sl->pix_rgb.as<float>(); pb.depth = sl->pix_depth.as<float>(); pb.ncontrib = sl->pix_nc.as<int32_t>();
+  }
+  pb.T = sl->pix_T.as<float>(); pb.last = sl->pix_last.as<int32_t>();
+  launch_forward(sl->splat_sorted.as<Splat>(), sl->ckeys_sorted, sl->crect.as<ushort4>(), sl->cranges.as<uint2>(), tg, rank_bits,
+                 cam.width, cam.height, ctx->cfg, pb, sl->tile_cend.as<uint32_t>(), sl->tile_walk.as<uint32_t>(), sl->d_counters, st);
   CK(cudaGetLastError());
-  mark(ctx, NBV_STAGE_BACKWARD, st);
+  mark(ctx, sl, NBV_STAGE_BACKWARD, st);
   if (upto == STAGE_FORWARD) return NBV_OK;
 
-  CKRET(ensure(ctx, ctx->moments, 4 * (size_t)NMOM * N));
-  CK(cudaMemsetAsync(ctx->moments.p, 0, 4 * (size_t)NMOM * N, st));
-  launch_backward(ctx->splat_sorted.as<Splat>(), ctx->keys_sorted, ctx->ranges.as<uint2>(), rank_bits, cam.width, cam.height,
-                  ctx->cfg, pixel_buf(ctx), ctx->moments.as<float>(), st);
+  const size_t mom_bytes = 4 * (size_t)NMOM * N;
+  if (sl->moments.cap < mom_bytes || !sl->moments.p) sl->moments_clean = false;
+  CKRET(ensure(ctx, sl->moments, mom_bytes));
+  CKRET(ensure(ctx, sl->touched, 4 * (size_t)N));
+  if (!sl->moments_clean) CK(cudaMemsetAsync(sl->moments.p, 0, mom_bytes, st));
+  sl->moments_clean = false;     // dirty until an expand kernel has consumed the touched list
+  launch_backward(sl->splat_sorted.as<Splat>(), sl->ckeys_sorted, sl->crect.as<ushort4>(), sl->cranges.as<uint2>(), tg, rank_bits,
+                  cam.width, cam.height, ctx->cfg, pb, sl->tile_cend.as<uint32_t>(), sl->moments.as<float>(),
+                  sl->touched.as<uint32_t>(), sl->d_counters, st);
   CK(cudaGetLastError());
-  mark(ctx, NBV_STAGE_EXPAND, st);
+  mark(ctx, sl, NBV_STAGE_EXPAND, st);
   return NBV_OK;
+}
+
+// S5 (+S6) of the view process_view() left in the slot
+int expand_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int mode, float* out_blocks, float* score, float* gains,
+                cudaStream_t st) {
+  launch_expand(scene_dev(ctx), cam, ctx->cfg, sl->ids.as<uint32_t>(), sl->touched.as<uint32_t>(), sl->moments.as<float>(), mode,
+                ctx->H_T.as<float>(), out_blocks, ctx->conf.as<float>(), ctx->cholT.as<float>(), score, gains, sl->d_counters, st);
+  CK(cudaGetLastError());
+  sl->moments_clean = true;
+  mark(ctx, sl, NBV_N_STAGES, st);
+  return NBV_OK;
+}
+
+// Run S1..S6 for n cameras, round-robin over the view slots.  With more than one slot the slot streams fork from and
+// join back into the caller's stream through events, so the call stays asynchronous and stream-ordered for the caller.
+int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_scores, cudaStream_t st) {
+  const int S = std::max(1, std::min(ctx->concurrency, n));
+  std::vector<ViewSlot*> sl((size_t)S);
+  for (int i = 0; i < S; ++i) CKRET(get_slot(ctx, i, &sl[i]));
+  if (S > 1) {
+    CK(cudaEventRecord(ctx->ev_fork, st));
+    for (int i = 0; i < S; ++i) CK(cudaStreamWaitEvent(sl[i]->st, ctx->ev_fork, 0));
+  }
+  int rc = NBV_OK;
+  for (int i = 0; i < n && rc == NBV_OK; ++i) {
+    ViewSlot* s = sl[i % S];
+    cudaStream_t vs = S > 1 ? s->st : st;
+    rc = process_view(ctx, s, h_cams[i], STAGE_BACKWARD, false, false, vs);
+    if (rc == NBV_OK) rc = expand_view(ctx, s, h_cams[i], mode, nullptr, d_scores ? d_scores + i : nullptr, nullptr, vs);
+  }
+  if (S > 1)
+    for (int i = 0; i < S; ++i) {   // join even after an error: the caller's stream must not run ahead of the slots
+      cudaEventRecord(sl[i]->done, sl[i]->st);
+      cudaStreamWaitEvent(st, sl[i]->done, 0);
+    }
+  return rc;
 }
 
 int prepare_scoring(nbv_ctx* ctx, int target, cudaStream_t st) {
@@ -355,30 +458,37 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
   nbv_ctx* ctx = new nbv_ctx;
   ctx->cfg = c;
   ctx->device = dev;
-  if (cudaMalloc(&ctx->d_counters, sizeof(ViewCounters)) != cudaSuccess ||
-      cudaMallocHost(&ctx->h_counters, sizeof(ViewCounters)) != cudaSuccess) {
+  ViewSlot* s0 = nullptr;
+  if (cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess || get_slot(ctx, 0, &s0) != NBV_OK) {
     cudaGetLastError();
-    if (ctx->d_counters) cudaFree(ctx->d_counters);
-    delete ctx;
+    nbv_destroy(ctx);
     return NBV_ERR_CUDA;
   }
-  std::memset(ctx->h_counters, 0, sizeof(ViewCounters));
+  if (const char* e = std::getenv("NBV_CONCURRENCY")) {
+    const int v = std::atoi(e);
+    if (v >= 1 && v <= 16) ctx->concurrency = v;
+  }
   *out = ctx;
   return NBV_OK;
 }
 
 void nbv_destroy(nbv_ctx* ctx) {
   if (!ctx) return;
+  cudaDeviceSynchronize();
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
-                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->splat, &ctx->zkey, &ctx->zkey_alt, &ctx->ids, &ctx->ids_alt,
-                   &ctx->rect, &ctx->abc, &ctx->splat_sorted, &ctx->rect_sorted, &ctx->ntiles, &ctx->offsets, &ctx->keys,
-                   &ctx->keys_alt, &ctx->ranges, &ctx->sort_tmp, &ctx->scan_tmp, &ctx->tile_counts, &ctx->pix_rgb, &ctx->pix_depth,
-                   &ctx->pix_T, &ctx->pix_nc, &ctx->pix_last, &ctx->moments, &ctx->score_tmp};
+                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp};
   for (DevBuf* b : all) release(*b);
-  if (ctx->d_counters) cudaFree(ctx->d_counters);
-  if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
-  for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+  for (ViewSlot* sl : ctx->slots) free_slot(sl);
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  cudaGetLastError();
   delete ctx;
+}
+
+int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight) {
+  if (!ctx) return NBV_ERR_INVALID_ARG;
+  if (views_in_flight < 1 || views_in_flight > 16) return fail(ctx, NBV_ERR_INVALID_ARG, "views_in_flight must be in [1, 16]");
+  ctx->concurrency = views_in_flight;
+  return NBV_OK;
 }
 
 const char* nbv_last_error(const nbv_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
@@ -404,12 +514,15 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
   CK(cudaMemcpyAsync(ctx->rgb.p, d_rgb, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->logits.p, d_obj_logits, 4 * n * K, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemsetAsync(ctx->H_T.p, 0, 4 * (size_t)NBLK * n, st));
-  CK(cudaMemsetAsync(ctx->d_counters, 0, sizeof(ViewCounters), st));
-  launch_activate(scene_dev(ctx), ctx->d_counters, st);
+  ViewSlot* s0 = ctx->slots[0];
+  CK(cudaDeviceSynchronize());             // no view of a previous scene may still be in flight
+  CK(cudaMemsetAsync(s0->d_counters, 0, sizeof(ViewCounters), st));
+  launch_activate(scene_dev(ctx), s0->d_counters, st);
   CK(cudaGetLastError());
-  CK(cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, sizeof(ViewCounters), cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(s0->h_counters, s0->d_counters, sizeof(ViewCounters), cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
-  if (ctx->h_counters->bad_data)
+  for (ViewSlot* sl : ctx->slots) sl->moments_clean = false;
+  if (s0->h_counters->bad_data)
     return fail(ctx, NBV_ERR_BAD_DATA, "zero/non-finite quaternion, opacity outside (0,1) or non-finite parameter");
   ctx->n_train = 0;
   ctx->conf_target = -2;
@@ -433,15 +546,10 @@ int nbv_accumulate_training(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, v
   cudaStream_t st = (cudaStream_t)stream;
   for (int i = 0; i < n; ++i)
     if (!valid_camera(h_cams[i])) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
-  for (int i = 0; i < n; ++i) {
-    CKRET(process_view(ctx, h_cams[i], STAGE_BACKWARD, false, st));
-    launch_expand(scene_dev(ctx), h_cams[i], ctx->cfg, ctx->ids.as<uint32_t>(), ctx->moments.as<float>(), EXPAND_TRAIN,
-                  ctx->H_T.as<float>(), nullptr, nullptr, nullptr, nullptr, nullptr, ctx->d_counters, st);
-    CK(cudaGetLastError());
-    mark(ctx, NBV_N_STAGES, st);
-    ctx->n_train++;
-    ctx->conf_target = -2;
-  }
+  if (n == 0) return NBV_OK;
+  ctx->conf_target = -2;
+  CKRET(run_views(ctx, h_cams, n, EXPAND_TRAIN, nullptr, st));
+  ctx->n_train += n;
   return NBV_OK;
 }
 
@@ -457,14 +565,7 @@ int nbv_score_candidates(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int3
     if (!valid_camera(h_cams[i])) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
   CKRET(prepare_scoring(ctx, target_obj, st));
   CK(cudaMemsetAsync(d_scores, 0, 4 * (size_t)n, st));
-  for (int i = 0; i < n; ++i) {
-    CKRET(process_view(ctx, h_cams[i], STAGE_BACKWARD, false, st));
-    launch_expand(scene_dev(ctx), h_cams[i], ctx->cfg, ctx->ids.as<uint32_t>(), ctx->moments.as<float>(), EXPAND_GAIN,
-                  ctx->H_T.as<float>(), nullptr, ctx->conf.as<float>(), ctx->cholT.as<float>(), d_scores + i, nullptr,
-                  ctx->d_counters, st);
-    CK(cudaGetLastError());
-    mark(ctx, NBV_N_STAGES, st);
-  }
+  CKRET(run_views(ctx, h_cams, n, EXPAND_GAIN, d_scores, st));
   launch_argmax(d_scores, n, d_best, st);
   CK(cudaGetLastError());
   return NBV_OK;
@@ -489,21 +590,26 @@ int nbv_score_candidates_host(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n,
 int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream) {
   if (!ctx || !h_out) return NBV_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  CK(cudaMemcpyAsync(ctx->h_counters, ctx->d_counters, sizeof(ViewCounters), cudaMemcpyDeviceToHost, st));
+  ViewSlot* sl = ctx->last_slot ? ctx->last_slot : ctx->slots[0];
+  CK(cudaStreamSynchronize(st));           // joins the slot streams of the last call
+  CK(cudaMemcpyAsync(sl->h_counters, sl->d_counters, sizeof(ViewCounters), cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
-  h_out->n_visible = ctx->h_counters->n_visible;
-  h_out->n_keys = (int64_t)ctx->h_counters->n_keys;
-  h_out->n_entries = (int64_t)ctx->h_counters->n_entries;
-  h_out->n_pairs = (int64_t)ctx->h_counters->n_pairs;
-  h_out->n_touched = ctx->h_counters->n_touched;
+  h_out->n_visible = sl->h_counters->n_visible;
+  h_out->n_keys = (int64_t)sl->h_counters->n_keys;
+  h_out->n_entries = (int64_t)sl->h_counters->n_entries;
+  h_out->n_pairs = (int64_t)sl->h_counters->n_pairs;
+  h_out->n_touched = sl->h_counters->n_touched;
+  h_out->n_coarse = sl->h_counters->n_coarse;
   return NBV_OK;
 }
 
 int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream) {
   if (!ctx) return NBV_ERR_INVALID_ARG;
   CK(cudaStreamSynchronize((cudaStream_t)stream));
-  ctx->ev_views = 0;
-  for (auto& m : ctx->ev_mask) m = 0;
+  for (ViewSlot* sl : ctx->slots) {
+    sl->ev_views = 0;
+    for (auto& m : sl->ev_mask) m = 0;
+  }
   for (int s = 0; s < NBV_N_STAGES; ++s) ctx->stage_ms[s] = 0.0;
   ctx->timed_views = 0;
   ctx->timing = enable != 0;
@@ -513,7 +619,10 @@ int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream) {
 int nbv_stage_times(nbv_ctx* ctx, double* h_ms, int64_t* h_views, void* stream) {
   if (!ctx || !h_ms) return NBV_ERR_INVALID_ARG;
   CK(cudaStreamSynchronize((cudaStream_t)stream));
-  fold_timing(ctx);
+  for (ViewSlot* sl : ctx->slots) {
+    CK(cudaStreamSynchronize(sl->st));
+    fold_timing(ctx, sl);
+  }
   for (int s = 0; s < NBV_N_STAGES; ++s) h_ms[s] = ctx->stage_ms[s];
   if (h_views) *h_views = ctx->timed_views;
   return NBV_OK;
@@ -525,10 +634,11 @@ int nbv_projected(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t* d_visible, flo
   if (!ctx || !h_cam) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   cudaStream_t st = (cudaStream_t)stream;
-  CKRET(process_view(ctx, *h_cam, STAGE_PROJECT, true, st));
+  ViewSlot* sl = ctx->slots[0];
+  CKRET(process_view(ctx, sl, *h_cam, STAGE_PROJECT, true, false, st));
   ++g_kernel_launches;
-  export_projected_kernel<<<(ctx->N + 255) / 256, 256, 0, st>>>(ctx->N, ctx->splat.as<Splat>(), ctx->zkey.as<uint32_t>(),
-                                                                ctx->rect.as<ushort4>(), ctx->abc.as<float>(), d_visible, d_rec, d_rect);
+  export_projected_kernel<<<(ctx->N + 255) / 256, 256, 0, st>>>(ctx->N, sl->splat.as<Splat>(), sl->zkey.as<uint32_t>(),
+                                                                sl->rect.as<ushort4>(), sl->abc.as<float>(), d_visible, d_rec, d_rect);
   CK(cudaGetLastError());
   return NBV_OK;
 }
@@ -538,17 +648,28 @@ int nbv_tile_lists(nbv_ctx* ctx, const nbv_camera* h_cam, int64_t* d_offsets, in
   if (!ctx || !h_cam || !d_offsets || !h_total) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   cudaStream_t st = (cudaStream_t)stream;
-  CKRET(process_view(ctx, *h_cam, STAGE_BIN, false, st));
-  const int n_tiles = ((h_cam->width + TILE - 1) / TILE) * ((h_cam->height + TILE - 1) / TILE);
-  *h_total = (int64_t)ctx->n_keys;
-  CKRET(ensure(ctx, ctx->tile_counts, 4 * (size_t)n_tiles + 4));
-  CKRET(ensure(ctx, ctx->scan_tmp, 4 * scan_temp_words(std::max((size_t)n_tiles, (size_t)ctx->N + 1))));
-  const bool fits = d_ids && (int64_t)ctx->n_keys <= cap;
-  launch_export_lists(ctx->keys_sorted, ctx->n_keys, ctx->rank_bits, ctx->ids.as<uint32_t>(), ctx->ranges.as<uint2>(), n_tiles,
-                      d_offsets, fits ? d_ids : nullptr, ctx->tile_counts.as<uint32_t>(), ctx->scan_tmp.as<uint32_t>(), st);
+  ViewSlot* sl = ctx->slots[0];
+  CKRET(process_view(ctx, sl, *h_cam, STAGE_BIN, false, false, st));
+  const int n_tiles = sl->tg.tiles_x * sl->tg.tiles_y;
+  CKRET(ensure(ctx, sl->tile_counts, 4 * (2 * (size_t)n_tiles + 4)));
+  uint32_t* counts = sl->tile_counts.as<uint32_t>();
+  uint32_t* scanned = counts + n_tiles;
+  uint32_t* total = scanned + n_tiles;
+  launch_tile_counts(sl->ckeys_sorted, sl->crect.as<ushort4>(), sl->cranges.as<uint2>(), sl->tg, sl->rank_bits, counts, scanned, total,
+                     sl->scan_tmp.as<uint32_t>(), d_offsets, st);
   CK(cudaGetLastError());
+  uint32_t h_tot = 0;
+  CK(cudaMemcpyAsync(&h_tot, total, 4, cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
-  if (!fits && ctx->n_keys > 0) return fail(ctx, NBV_ERR_CAPACITY, "d_ids too small for the tile lists");
+  *h_total = (int64_t)h_tot;
+  const bool fits = d_ids && (int64_t)h_tot <= cap;
+  if (!fits && h_tot > 0) return fail(ctx, NBV_ERR_CAPACITY, "d_ids too small for the tile lists");
+  if (h_tot > 0) {
+    launch_tile_ids(sl->ckeys_sorted, sl->crect.as<ushort4>(), sl->cranges.as<uint2>(), sl->tg, sl->rank_bits, sl->ids.as<uint32_t>(),
+                    scanned, d_ids, st);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));
+  }
   return NBV_OK;
 }
 
@@ -556,12 +677,25 @@ int nbv_render(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_rgb, float* d_dep
   if (!ctx || !h_cam) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   cudaStream_t st = (cudaStream_t)stream;
-  CKRET(process_view(ctx, *h_cam, STAGE_FORWARD, false, st));
+  ViewSlot* sl = ctx->slots[0];
+  CKRET(process_view(ctx, sl, *h_cam, STAGE_FORWARD, false, true, st));
   const size_t npx = (size_t)h_cam->width * h_cam->height;
-  if (d_rgb) CK(cudaMemcpyAsync(d_rgb, ctx->pix_rgb.p, 12 * npx, cudaMemcpyDeviceToDevice, st));
-  if (d_depth) CK(cudaMemcpyAsync(d_depth, ctx->pix_depth.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
-  if (d_T) CK(cudaMemcpyAsync(d_T, ctx->pix_T.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
-  if (d_ncontrib) CK(cudaMemcpyAsync(d_ncontrib, ctx->pix_nc.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
+  if (d_rgb) CK(cudaMemcpyAsync(d_rgb, sl->pix_rgb.p, 12 * npx, cudaMemcpyDeviceToDevice, st));
+  if (d_depth) CK(cudaMemcpyAsync(d_depth, sl->pix_depth.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
+  if (d_T) CK(cudaMemcpyAsync(d_T, sl->pix_T.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
+  if (d_ncontrib) CK(cudaMemcpyAsync(d_ncontrib, sl->pix_nc.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
+  return NBV_OK;
+}
+
+int nbv_tile_walk(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t* d_walked, int32_t* d_last, void* stream) {
+  if (!ctx || !h_cam || !d_walked) return NBV_ERR_INVALID_ARG;
+  if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  cudaStream_t st = (cudaStream_t)stream;
+  ViewSlot* sl = ctx->slots[0];
+  CKRET(process_view(ctx, sl, *h_cam, STAGE_FORWARD, false, false, st));
+  const size_t n_tiles = (size_t)sl->tg.tiles_x * sl->tg.tiles_y;
+  CK(cudaMemcpyAsync(d_walked, sl->tile_walk.p, 4 * n_tiles, cudaMemcpyDeviceToDevice, st));
+  if (d_last) CK(cudaMemcpyAsync(d_last, sl->pix_last.p, 4 * (size_t)h_cam->width * h_cam->height, cudaMemcpyDeviceToDevice, st));
   return NBV_OK;
 }
 
@@ -569,11 +703,10 @@ int nbv_view_hessian(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_blocks, voi
   if (!ctx || !h_cam || !d_blocks) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   cudaStream_t st = (cudaStream_t)stream;
+  ViewSlot* sl = ctx->slots[0];
   CK(cudaMemsetAsync(d_blocks, 0, 4 * (size_t)NBLK * ctx->N, st));
-  CKRET(process_view(ctx, *h_cam, STAGE_BACKWARD, false, st));
-  launch_expand(scene_dev(ctx), *h_cam, ctx->cfg, ctx->ids.as<uint32_t>(), ctx->moments.as<float>(), EXPAND_VIEW, nullptr, d_blocks,
-                nullptr, nullptr, nullptr, nullptr, ctx->d_counters, st);
-  CK(cudaGetLastError());
+  CKRET(process_view(ctx, sl, *h_cam, STAGE_BACKWARD, false, false, st));
+  CKRET(expand_view(ctx, sl, *h_cam, EXPAND_VIEW, d_blocks, nullptr, nullptr, st));
   return NBV_OK;
 }
 
@@ -597,14 +730,13 @@ int nbv_gaussian_gains(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t target_obj
   if (!ctx || !h_cam || !d_gains) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   cudaStream_t st = (cudaStream_t)stream;
+  ViewSlot* sl = ctx->slots[0];
   CKRET(prepare_scoring(ctx, target_obj, st));
   CKRET(ensure(ctx, ctx->score_tmp, 64));
   CK(cudaMemsetAsync(ctx->score_tmp.p, 0, 64, st));
   CK(cudaMemsetAsync(d_gains, 0, 4 * (size_t)ctx->N, st));
-  CKRET(process_view(ctx, *h_cam, STAGE_BACKWARD, false, st));
-  launch_expand(scene_dev(ctx), *h_cam, ctx->cfg, ctx->ids.as<uint32_t>(), ctx->moments.as<float>(), EXPAND_GAIN, ctx->H_T.as<float>(),
-                nullptr, ctx->conf.as<float>(), ctx->cholT.as<float>(), ctx->score_tmp.as<float>(), d_gains, ctx->d_counters, st);
-  CK(cudaGetLastError());
+  CKRET(process_view(ctx, sl, *h_cam, STAGE_BACKWARD, false, false, st));
+  CKRET(expand_view(ctx, sl, *h_cam, EXPAND_GAIN, nullptr, ctx->score_tmp.as<float>(), d_gains, st));
   return NBV_OK;
 }
 

@@ -1,9 +1,12 @@
 // raster.cu -- S3 front-to-back compositing and S4 back-to-front Jacobian sweep, per 16x16 tile.
 //
 // Mapping: ONE WARP PER TILE, each lane owns a column of 8 pixels
-// (x = lane & 15, rows (lane >> 4) * 8 .. +7).  The tile's depth-sorted splats are staged 32 at a time in
-// shared memory; every lane evaluates each splat at its 8 pixels, so the 40 moment sums of S4 are reduced
-// over 8 pixels in registers before the cross-lane butterfly, and no block-level barrier exists at all.
+// (x = lane & 15, rows (lane >> 4) * 8 .. +7).  The warp streams its SUPERTILE's depth-ordered list (binning.cu),
+// keeps the entries whose tile rectangle contains this tile (ballot + compaction into a shared-memory queue: this
+// IS the tile list of R-5, produced lazily) and stages the splats 32 at a time in shared memory; every lane
+// evaluates each splat at its 8 pixels, so the 40 moment sums of S4 are reduced over 8 pixels in registers before
+// the cross-lane butterfly, and no block-level barrier exists at all.  S3 stops reading the list when all 256
+// pixels have terminated and records where (tile_cend); S4 walks the same list backwards from there.
 //
 // S3 is on the decision path (bit-exact power / alpha / transmittance chain).
 // S4 ("computes the Jacobian of the rendering with respect to Gaussian parameters", L189-191
@@ -26,35 +29,53 @@ constexpr unsigned FULL = 0xffffffffu;
 
 struct RasterParams {
   int W, H, tiles_x, rank_bits;
+  int sshift, super_x;                 // supertile = (1 << sshift)^2 tiles, super_x supertiles per row
   float alpha_min, alpha_max, t_stop;
   float bg[3];
   float omega[4];                      // channel weights, 0 for disabled channels
 };
 
-__device__ __forceinline__ void stage_batch(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ keys,
-                                            uint32_t first, uint32_t count, uint32_t rmask, float4* sm, uint32_t* sm_rank) {
+// lanes < count stage the splats of queue slots 0..count-1; slot j's coarse position + 1 rides in the pad field
+__device__ __forceinline__ void stage_queue(const Splat* __restrict__ splat_sorted, const uint32_t* q_rank, const uint32_t* q_cpos,
+                                            uint32_t count, float4* sm) {
   const int lane = threadIdx.x;
   if ((uint32_t)lane < count) {
-    const uint32_t r = keys[first + lane] & rmask;
-    const float4* s = reinterpret_cast<const float4*>(splat_sorted + r);
+    const float4* s = reinterpret_cast<const float4*>(splat_sorted + q_rank[lane]);
     sm[lane * 3 + 0] = s[0];
     sm[lane * 3 + 1] = s[1];
-    sm[lane * 3 + 2] = s[2];
-    if (sm_rank) sm_rank[lane] = r;
+    float4 c = s[2];
+    if (q_cpos) c.w = __uint_as_float(q_cpos[lane] + 1u);
+    sm[lane * 3 + 2] = c;
   }
   __syncwarp();
 }
 
-__global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ keys,
-                                                      const uint2* __restrict__ ranges, RasterParams prm, PixelBuf out,
-                                                      ViewCounters* counters) {
+// drop the first `count` queue slots
+__device__ __forceinline__ void shift_queue(uint32_t* q_rank, uint32_t* q_cpos, uint32_t& qn, uint32_t count) {
+  const int lane = threadIdx.x;
+  __syncwarp();
+  uint32_t r = 0, c = 0;
+  const bool mv = count + lane < qn;
+  if (mv) { r = q_rank[count + lane]; if (q_cpos) c = q_cpos[count + lane]; }
+  __syncwarp();
+  if (mv) { q_rank[lane] = r; if (q_cpos) q_cpos[lane] = c; }
+  qn -= count;
+  __syncwarp();
+}
+
+__global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ ckeys,
+                                                      const ushort4* __restrict__ crect, const uint2* __restrict__ cranges,
+                                                      RasterParams prm, PixelBuf out, uint32_t* __restrict__ tile_cend,
+                                                      uint32_t* __restrict__ tile_walk, ViewCounters* counters) {
   __shared__ float4 sm[32 * 3];
+  __shared__ uint32_t q_rank[64], q_cpos[64];
   const int tile = blockIdx.x, lane = threadIdx.x;
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
-  const uint2 range = ranges[tile];
+  const uint2 range = cranges[(ty >> prm.sshift) * prm.super_x + (tx >> prm.sshift)];
   const uint32_t rmask = (1u << prm.rank_bits) - 1u;
+  const uint32_t lt = (1u << lane) - 1u;
 
   float T[PPL], C0[PPL], C1[PPL], C2[PPL], D[PPL];
   int n[PPL], last[PPL];
@@ -64,14 +85,35 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
     T[k] = 1.0f; C0[k] = C1[k] = C2[k] = D[k] = 0.0f; n[k] = 0; last[k] = 0;
     if (x >= prm.W || y0 + k >= prm.H) done |= 1u << k;
   }
-  uint32_t walked = 0;
+  uint32_t walked = 0, cend = 0;
+  uint32_t pos = range.x, qn = 0;
+  int e_base = 0;
   bool finished = __all_sync(FULL, done == 0xffu);
-  for (uint32_t base = range.x; base < range.y && !finished; base += 32) {
-    const uint32_t cnt = min(32u, range.y - base);
-    stage_batch(splat_sorted, keys, base, cnt, rmask, sm, nullptr);
+  while (!finished) {
+    // fill the queue with the next entries of the supertile list whose rect contains this tile
+    while (qn < 32u && pos < range.y) {
+      const uint32_t i = pos + lane;
+      bool hit = false;
+      if (i < range.y) {
+        const ushort4 rc = crect[i];
+        hit = tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
+      }
+      const unsigned m = __ballot_sync(FULL, hit);
+      if (hit) {
+        const uint32_t slot = qn + __popc(m & lt);
+        q_rank[slot] = ckeys[i] & rmask;
+        q_cpos[slot] = i;
+      }
+      qn += __popc(m);
+      pos += 32;
+    }
+    if (qn == 0) break;
+    const uint32_t cnt = min(qn, 32u);
+    __syncwarp();
+    stage_queue(splat_sorted, q_rank, q_cpos, cnt, sm);
     for (uint32_t j = 0; j < cnt; ++j) {
       const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
-      const int e1 = (int)(base - range.x + j) + 1;
+      const int e1 = e_base + (int)j + 1;
       ++walked;
 #pragma unroll
       for (int k = 0; k < PPL; ++k) {
@@ -92,6 +134,7 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
                 T[k] = Tn;
                 ++n[k];
                 last[k] = e1;
+                cend = __float_as_uint(s2.w);             // coarse position + 1 of the last composited entry
               }
             }
           }
@@ -99,7 +142,8 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
       }
       if (__all_sync(FULL, done == 0xffu)) { finished = true; break; }
     }
-    __syncwarp();
+    e_base += (int)cnt;
+    shift_queue(q_rank, q_cpos, qn, cnt);
   }
   unsigned pairs = 0;
 #pragma unroll
@@ -119,8 +163,13 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
     }
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) pairs += __shfl_xor_sync(FULL, pairs, o);
+  for (int o = 16; o > 0; o >>= 1) {
+    pairs += __shfl_xor_sync(FULL, pairs, o);
+    cend = max(cend, __shfl_xor_sync(FULL, cend, o));
+  }
   if (lane == 0) {
+    tile_cend[tile] = cend;
+    if (tile_walk) tile_walk[tile] = walked;
     atomicAdd(&counters->n_entries, (unsigned long long)walked);
     atomicAdd(&counters->n_pairs, (unsigned long long)pairs);
   }
@@ -170,17 +219,19 @@ __device__ __forceinline__ void butterfly40(const float (&v)[NMOM], int lane, fl
 }
 
 template <int NCH>
-__global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ keys,
-                                                       const uint2* __restrict__ ranges, RasterParams prm, PixelBuf pix,
-                                                       float* __restrict__ moments) {
+__global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ ckeys,
+                                                       const ushort4* __restrict__ crect, const uint2* __restrict__ cranges,
+                                                       const uint32_t* __restrict__ tile_cend, RasterParams prm, PixelBuf pix,
+                                                       float* __restrict__ moments, uint32_t* __restrict__ touched,
+                                                       ViewCounters* counters) {
   __shared__ float4 sm[32 * 3];
-  __shared__ uint32_t sm_rank[32];
+  __shared__ uint32_t q_rank[64];
   const int tile = blockIdx.x, lane = threadIdx.x;
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
-  const uint2 range = ranges[tile];
   const uint32_t rmask = (1u << prm.rank_bits) - 1u;
+  const uint32_t lt = (1u << lane) - 1u;
 
   float Tc[PPL], S0[PPL], S1[PPL], S2[PPL], S3[PPL];
   int last[PPL];
@@ -200,13 +251,33 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
   for (int o = 16; o > 0; o >>= 1) maxlast = max(maxlast, __shfl_xor_sync(FULL, maxlast, o));
   if (maxlast == 0) return;
 
-  for (int bb = (maxlast - 1) / 32; bb >= 0; --bb) {
-    const int base_e = bb * 32;
-    const int cnt = min(32, maxlast - base_e);
-    stage_batch(splat_sorted, keys, range.x + (uint32_t)base_e, (uint32_t)cnt, rmask, sm, sm_rank);
-    for (int j = cnt - 1; j >= 0; --j) {
+  // walk the supertile list backwards from the last composited entry; the entries that pass the rect test are the
+  // tile-list entries maxlast-1, maxlast-2, ..., 0 in that order
+  const uint32_t cbegin = cranges[(ty >> prm.sshift) * prm.super_x + (tx >> prm.sshift)].x;
+  uint32_t pos_hi = tile_cend[tile], qn = 0;
+  int e_next = maxlast - 1;
+  for (;;) {
+    while (qn < 32u && pos_hi > cbegin) {
+      const uint32_t span = min(32u, pos_hi - cbegin);
+      bool hit = false;
+      uint32_t i = 0;
+      if ((uint32_t)lane < span) {
+        i = pos_hi - 1u - (uint32_t)lane;
+        const ushort4 rc = crect[i];
+        hit = tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
+      }
+      const unsigned m = __ballot_sync(FULL, hit);
+      if (hit) q_rank[qn + __popc(m & lt)] = ckeys[i] & rmask;
+      qn += __popc(m);
+      pos_hi -= span;
+    }
+    if (qn == 0) break;
+    const int cnt = (int)min(qn, 32u);
+    __syncwarp();
+    stage_queue(splat_sorted, q_rank, nullptr, (uint32_t)cnt, sm);
+    for (int j = 0; j < cnt; ++j) {
       const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
-      const int e = base_e + j;
+      const int e = e_next - j;
       const float cA = -2.0f * s0.z, cB = -s0.w, cC = -2.0f * s1.x;    // conic = Sigma2D^-1
       float acc[NMOM];
 #pragma unroll
@@ -265,44 +336,52 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
         float o0, o1;
         int i0, i1;
         butterfly40(acc, lane, o0, o1, i0, i1);
-        float* dst = moments + (size_t)sm_rank[j] * NMOM;
+        const uint32_t rank = q_rank[j];
+        float* dst = moments + (size_t)rank * NMOM;
         if (i0 >= 0) atomicAdd(dst + i0, o0);
-        if (i1 >= 0) atomicAdd(dst + i1, o1);
+        if (i1 >= 0) {
+          if (i1 == MOM_W2) {
+            // sum w^2 > 0 for every touched Gaussian: the first adder (old value 0) appends it to the touched list
+            if (atomicAdd(dst + i1, o1) == 0.0f) touched[atomicAdd(&counters->n_touched, 1u)] = rank;
+          } else {
+            atomicAdd(dst + i1, o1);
+          }
+        }
       }
     }
-    __syncwarp();
+    e_next -= cnt;
+    shift_queue(q_rank, nullptr, qn, (uint32_t)cnt);
   }
 }
 
-static RasterParams make_params(int rank_bits, int W, int H, const nbv_config& cfg) {
+static RasterParams make_params(const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg) {
   RasterParams p;
-  p.W = W; p.H = H; p.tiles_x = (W + TILE - 1) / TILE; p.rank_bits = rank_bits;
+  p.W = W; p.H = H; p.tiles_x = tg.tiles_x; p.rank_bits = rank_bits;
+  p.sshift = tg.sshift; p.super_x = tg.super_x;
   p.alpha_min = cfg.alpha_min; p.alpha_max = cfg.alpha_max; p.t_stop = cfg.t_stop;
   for (int c = 0; c < 3; ++c) p.bg[c] = cfg.bg[c];
   for (int c = 0; c < 4; ++c) p.omega[c] = ((cfg.channel_mask >> c) & 1) ? cfg.channel_weight[c] : 0.0f;
   return p;
 }
 
-void launch_forward(const Splat* splat_sorted, const uint32_t* keys, const uint2* ranges, int rank_bits, int W, int H,
-                    const nbv_config& cfg, PixelBuf px, ViewCounters* counters, cudaStream_t st) {
-  const RasterParams p = make_params(rank_bits, W, H, cfg);
-  const int tiles = p.tiles_x * ((H + TILE - 1) / TILE);
+void launch_forward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
+                    int rank_bits, int W, int H, const nbv_config& cfg, PixelBuf px, uint32_t* tile_cend, uint32_t* tile_walk,
+                    ViewCounters* counters, cudaStream_t st) {
+  const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
   ++g_kernel_launches;
-  forward_kernel<<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, counters);
+  forward_kernel<<<tg.tiles_x * tg.tiles_y, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, p, px, tile_cend, tile_walk, counters);
 }
 
-void launch_backward(const Splat* splat_sorted, const uint32_t* keys, const uint2* ranges, int rank_bits, int W, int H,
-                     const nbv_config& cfg, PixelBuf px, float* moments, cudaStream_t st) {
-  const RasterParams p = make_params(rank_bits, W, H, cfg);
-  const int tiles = p.tiles_x * ((H + TILE - 1) / TILE);
-  if (cfg.channel_mask & NBV_CH_DEPTH) {
-    ++g_kernel_launches;
-    backward_kernel<4><<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, moments);
-  }
-  else {
-    ++g_kernel_launches;
-    backward_kernel<3><<<tiles, 32, 0, st>>>(splat_sorted, keys, ranges, p, px, moments);
-  }
+void launch_backward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
+                     int rank_bits, int W, int H, const nbv_config& cfg, PixelBuf px, const uint32_t* tile_cend, float* moments,
+                     uint32_t* touched, ViewCounters* counters, cudaStream_t st) {
+  const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
+  const int tiles = tg.tiles_x * tg.tiles_y;
+  ++g_kernel_launches;
+  if (cfg.channel_mask & NBV_CH_DEPTH)
+    backward_kernel<4><<<tiles, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, tile_cend, p, px, moments, touched, counters);
+  else
+    backward_kernel<3><<<tiles, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, tile_cend, p, px, moments, touched, counters);
 }
 
 }  // namespace nbv

@@ -121,9 +121,10 @@ constexpr int RS_I = 16;
 constexpr int RS_TILE = RS_T * RS_I;   // 4096 keys per block
 constexpr int RS_W = RS_T / 32;        // 8 warps, 512 consecutive keys each
 
-__global__ void __launch_bounds__(RS_T) radix_hist_kernel(const uint32_t* __restrict__ keys, uint32_t n, int shift,
-                                                           uint32_t mask, uint32_t* __restrict__ hist, uint32_t nblocks) {
+__global__ void __launch_bounds__(RS_T) radix_hist_kernel(const uint32_t* __restrict__ keys, uint32_t n, const uint32_t* __restrict__ d_n,
+                                                           int shift, uint32_t mask, uint32_t* __restrict__ hist, uint32_t nblocks) {
   __shared__ uint32_t h[256];
+  if (d_n) n = min(n, *d_n);             // device-side length (n is then the capacity the grid was sized for)
   h[threadIdx.x] = 0;
   __syncthreads();
   const uint32_t base = blockIdx.x * RS_TILE;
@@ -139,8 +140,10 @@ __global__ void __launch_bounds__(RS_T) radix_hist_kernel(const uint32_t* __rest
 template <bool HAS_VALS>
 __global__ void __launch_bounds__(RS_T) radix_scatter_kernel(const uint32_t* __restrict__ keys_in, uint32_t* __restrict__ keys_out,
                                                               const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ vals_out,
-                                                              uint32_t n, int shift, uint32_t mask,
+                                                              uint32_t n, const uint32_t* __restrict__ d_n, int shift, uint32_t mask,
                                                               const uint32_t* __restrict__ hist_scanned, uint32_t nblocks) {
+  if (d_n) n = min(n, *d_n);
+  if (blockIdx.x * RS_TILE >= n) return;
   __shared__ uint32_t wh[RS_W][256];     // per-warp digit counts, then per-warp digit bases
   __shared__ uint32_t dstart[256];       // block-local start of each digit's run
   __shared__ uint32_t gofs[256];         // global position of local slot i with digit d = gofs[d] + i
@@ -209,6 +212,8 @@ __global__ void __launch_bounds__(RS_T) radix_scatter_kernel(const uint32_t* __r
   }
 }
 
+uint32_t radix_blocks(size_t n) { return (uint32_t)((n + RS_TILE - 1) / RS_TILE); }
+
 size_t radix_temp_words(size_t n) {
   size_t nb = (n + RS_TILE - 1) / RS_TILE;
   size_t hist = 256 * nb;
@@ -216,22 +221,22 @@ size_t radix_temp_words(size_t n) {
 }
 
 void radix_pass(const uint32_t* keys_in, uint32_t* keys_out, const uint32_t* vals_in, uint32_t* vals_out, size_t n,
-                int shift, int bits, uint32_t* tmp, cudaStream_t st) {
+                const uint32_t* d_n, int shift, int bits, uint32_t* tmp, cudaStream_t st) {
   if (n == 0) return;
   const uint32_t nb = (uint32_t)((n + RS_TILE - 1) / RS_TILE);
   const uint32_t mask = (1u << bits) - 1u;
   const size_t hist_n = (size_t)(mask + 1) * nb;
   uint32_t* hist = tmp;
   ++g_kernel_launches;
-  radix_hist_kernel<<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, shift, mask, hist, nb);
+  radix_hist_kernel<<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, d_n, shift, mask, hist, nb);
   exclusive_scan_u32(hist, hist, hist_n, tmp + 256 * (size_t)nb, nullptr, st);
   if (vals_in) {
     ++g_kernel_launches;
-    radix_scatter_kernel<true><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, shift, mask, hist, nb);
+    radix_scatter_kernel<true><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, d_n, shift, mask, hist, nb);
   }
   else {
     ++g_kernel_launches;
-    radix_scatter_kernel<false><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, shift, mask, hist, nb);
+    radix_scatter_kernel<false><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, d_n, shift, mask, hist, nb);
   }
 }
 
