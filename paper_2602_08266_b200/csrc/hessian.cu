@@ -136,6 +136,47 @@ __device__ void chain_f(const nbv_camera& cam, const float* mu, const float* ls,
   }
 }
 
+// S4 accumulates the moments in the monomials xi1^i xi2^j of the whitened pixel offset xi = L^-1 (p - m),
+// Sigma2D = L L^T (raster.cu).  The derivatives of alpha are monomials of u = Sigma2D^-1 d = L^-T xi, i.e.
+// ux = p00 xi1 + p01 xi2, uy = p11 xi2, so each homogeneous degree is mapped by the corresponding symmetric power of
+// that 2 x 2 matrix, once per touched Gaussian.  The two terms of ux are uncorrelated over the footprint (no
+// cancellation), which is why the whitened basis is used rather than plain pixel offsets.
+__device__ void moments_to_u_basis(float* m, float p00, float p01, float p10, float p11) {
+  float out[15];
+  out[0] = m[0];
+#pragma unroll
+  for (int n = 1; n <= 4; ++n)
+#pragma unroll
+    for (int j = 0; j <= n; ++j) {
+      // coefficients of ux^(n-j) uy^j in xi1^(n-t) xi2^t
+      float coef[5] = {1.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int sidx = 0; sidx < n; ++sidx) {
+        const float a0 = sidx < n - j ? p00 : p10, a1 = sidx < n - j ? p01 : p11;
+#pragma unroll
+        for (int t = 4; t >= 1; --t)
+          if (t <= sidx + 1) coef[t] = coef[t] * a0 + coef[t - 1] * a1;
+        coef[0] *= a0;
+      }
+      float v = 0.f;
+#pragma unroll
+      for (int t = 0; t <= n; ++t) v += coef[t] * m[mono_index(n - t, t)];
+      out[mono_index(n - j, j)] = v;
+    }
+#pragma unroll
+  for (int i = 0; i < 15; ++i) m[i] = out[i];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    float* x = m + MOM_X + 6 * c;          // (xi1, xi2, xi1^2, xi1 xi2, xi2^2, 1) -> (ux, uy, ux^2, ux uy, uy^2, 1)
+    const float x0 = x[0], x1 = x[1], x2 = x[2], x3 = x[3], x4 = x[4];
+    x[0] = p00 * x0 + p01 * x1;
+    x[1] = p10 * x0 + p11 * x1;
+    x[2] = p00 * p00 * x2 + 2.f * p00 * p01 * x3 + p01 * p01 * x4;
+    x[3] = p00 * p10 * x2 + (p00 * p11 + p01 * p10) * x3 + p01 * p11 * x4;
+    x[4] = p10 * p10 * x2 + 2.f * p10 * p11 * x3 + p11 * p11 * x4;
+  }
+}
+
 // moments (40) + chain -> packed block H[105]
 __device__ void build_block(const float* mom, const ChainF& ch, float kappa, const float* omega, float* H) {
   // A: 11 nonzero rows x 6
@@ -252,7 +293,7 @@ __device__ float gain_solve(float* B, const float* U) {
 }
 
 __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam, nbv_config cfg, const uint32_t* __restrict__ ids_sorted,
-                                                     const uint32_t* __restrict__ touched, float* __restrict__ moments, int mode,
+                                                     const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ touched, float* __restrict__ moments, int mode,
                                                      float* __restrict__ H_T, float* __restrict__ out_blocks,
                                                      const float* __restrict__ conf, const float* __restrict__ cholT,
                                                      float* __restrict__ score, float* __restrict__ gains, ViewCounters* counters) {
@@ -271,6 +312,12 @@ __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam,
       const float4 v = mom4[i];
       m[4 * i] = v.x; m[4 * i + 1] = v.y; m[4 * i + 2] = v.z; m[4 * i + 3] = v.w;
       mom4[i] = make_float4(0.f, 0.f, 0.f, 0.f);     // leave the buffer zeroed for the next view
+    }
+    {
+      const Splat sp = splat_sorted[r];                 // conic = Sigma2D^-1 = -(2 qa, qb, 2 qc), the one S4 evaluated with
+      const float cA = -2.f * sp.qa, cB = -sp.qb, cC = -2.f * sp.qc, icC = 1.0f / cC;
+      const float i11 = sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), sh = -cB * icC, i22 = sqrtf(cC);   // as in S4
+      moments_to_u_basis(m, i11, -sh * i22, 0.0f, i22);   // u = L^-T xi
     }
     ChainF ch;
     chain_f(cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
@@ -311,12 +358,12 @@ __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam,
 }
 
 void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
-                   const uint32_t* touched, float* moments, int mode, float* H_T, float* out_blocks, const float* conf,
+                   const Splat* splat_sorted, const uint32_t* touched, float* moments, int mode, float* H_T, float* out_blocks, const float* conf,
                    const float* cholT, float* score, float* gains, ViewCounters* counters, cudaStream_t st) {
   int blocks = (sc.N + 63) / 64;
   if (blocks > 148 * 8) blocks = 148 * 8;
   ++g_kernel_launches;
-  expand_kernel<<<blocks, 64, 0, st>>>(sc, cam, cfg, ids_sorted, touched, moments, mode, H_T, out_blocks, conf, cholT, score, gains,
+  expand_kernel<<<blocks, 64, 0, st>>>(sc, cam, cfg, ids_sorted, splat_sorted, touched, moments, mode, H_T, out_blocks, conf, cholT, score, gains,
                                        counters);
 }
 

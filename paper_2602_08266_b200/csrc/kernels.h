@@ -73,7 +73,7 @@ enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2 };
 // Consumes the touched list: reads the moments of every touched rank and writes zeros back (the moment buffer is
 // all-zero again afterwards).
 void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
-                   const uint32_t* touched, float* moments, int mode, float* H_T, float* out_blocks, const float* conf,
+                   const Splat* splat_sorted, const uint32_t* touched, float* moments, int mode, float* H_T, float* out_blocks, const float* conf,
                    const float* cholT, float* score, float* gains, ViewCounters* counters, cudaStream_t st);
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);
 void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);

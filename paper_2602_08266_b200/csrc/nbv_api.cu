@@ -354,7 +354,7 @@ int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bo
 // S5 (+S6) of the view process_view() left in the slot
 int expand_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int mode, float* out_blocks, float* score, float* gains,
                 cudaStream_t st) {
-  launch_expand(scene_dev(ctx), cam, ctx->cfg, sl->ids.as<uint32_t>(), sl->touched.as<uint32_t>(), sl->moments.as<float>(), mode,
+  launch_expand(scene_dev(ctx), cam, ctx->cfg, sl->ids.as<uint32_t>(), sl->splat_sorted.as<Splat>(), sl->touched.as<uint32_t>(), sl->moments.as<float>(), mode,
                 ctx->H_T.as<float>(), out_blocks, ctx->conf.as<float>(), ctx->cholT.as<float>(), score, gains, sl->d_counters, st);
   CK(cudaGetLastError());
   sl->moments_clean = true;

@@ -35,6 +35,31 @@ struct RasterParams {
   float omega[4];                      // channel weights, 0 for disabled channels
 };
 
+// Can any pixel centre of the tile whose first centre is (X0 + 0.5, Y0 + 0.5) reach power >= tau?  Conservative: the
+// maximum of the concave quadratic over the BOX of the 16 x 16 centres (at the centre if it lies inside, else on an
+// edge, where the 1-D optimum is clamped to the edge), plus a slack that covers the binary32 rounding of both this
+// evaluation and the per-pixel one.  An entry rejected here has no pixel that passes the footprint test of R-5 in
+// this tile, so dropping it changes no image, count, block or gain; S3 and S4 take the identical decision.
+__device__ __forceinline__ bool ellipse_reaches_tile(float mx, float my, float qa, float qb, float qc, float tau, float X0, float Y0) {
+  const float ax = sub_rn(X0 + 0.5f, mx), bx = add_rn(ax, (float)(TILE - 1));
+  const float ay = sub_rn(Y0 + 0.5f, my), by = add_rn(ay, (float)(TILE - 1));
+  if (ax <= 0.0f && bx >= 0.0f && ay <= 0.0f && by >= 0.0f) return true;
+  const float ry = div_rn(mul_rn(-0.5f, qb), qc), rx = div_rn(mul_rn(-0.5f, qb), qa);
+  const float thr = sub_rn(tau, 1e-3f);
+  bool keep = false;
+#pragma unroll
+  for (int e = 0; e < 4; ++e) {
+    float dx, dy;
+    if (e < 2) { dx = e == 0 ? ax : bx; dy = fminf(fmaxf(mul_rn(ry, dx), ay), by); }
+    else       { dy = e == 2 ? ay : by; dx = fminf(fmaxf(mul_rn(rx, dy), ax), bx); }
+    // explicit _rn operations: S3 and S4 must take bit-identical decisions, whatever the compiler would contract
+    const float t0 = mul_rn(mul_rn(qa, dx), dx), t1 = mul_rn(mul_rn(qb, dx), dy), t2 = mul_rn(mul_rn(qc, dy), dy);
+    const float p = add_rn(add_rn(t0, t1), t2), mag = add_rn(add_rn(fabsf(t0), fabsf(t1)), fabsf(t2));
+    keep = keep || !(add_rn(p, mul_rn(2e-5f, mag)) < thr);     // also keeps NaN / inf cases
+  }
+  return keep;
+}
+
 // lanes < count stage the splats of queue slots 0..count-1; slot j's coarse position + 1 rides in the pad field
 __device__ __forceinline__ void stage_queue(const Splat* __restrict__ splat_sorted, const uint32_t* q_rank, const uint32_t* q_cpos,
                                             uint32_t count, float4* sm) {
@@ -63,6 +88,11 @@ __device__ __forceinline__ void shift_queue(uint32_t* q_rank, uint32_t* q_cpos, 
   __syncwarp();
 }
 
+// FULLPIX = false is the timed path: S4 needs only the final transmittance and `last` of every pixel (it rebuilds the
+// suffix sums itself), so colour, depth and the contributor count are accumulated only for the parity exports.
+// The slot body is branch-free (predicated updates): the 8 pixels of a lane are 8 independent dependency chains the
+// scheduler can interleave, and after the ellipse test nearly every staged entry touches nearly every slot anyway.
+template <bool FULLPIX>
 __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ ckeys,
                                                       const ushort4* __restrict__ crect, const uint2* __restrict__ cranges,
                                                       RasterParams prm, PixelBuf out, uint32_t* __restrict__ tile_cend,
@@ -73,16 +103,18 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
+  const float X0 = (float)(tx * TILE), Y0 = (float)(ty * TILE);
   const uint2 range = cranges[(ty >> prm.sshift) * prm.super_x + (tx >> prm.sshift)];
   const uint32_t rmask = (1u << prm.rank_bits) - 1u;
   const uint32_t lt = (1u << lane) - 1u;
 
-  float T[PPL], C0[PPL], C1[PPL], C2[PPL], D[PPL];
+  float T[PPL], py[PPL], C0[PPL], C1[PPL], C2[PPL], D[PPL];
   int n[PPL], last[PPL];
   unsigned done = 0;
 #pragma unroll
   for (int k = 0; k < PPL; ++k) {
     T[k] = 1.0f; C0[k] = C1[k] = C2[k] = D[k] = 0.0f; n[k] = 0; last[k] = 0;
+    py[k] = (float)(y0 + k) + 0.5f;
     if (x >= prm.W || y0 + k >= prm.H) done |= 1u << k;
   }
   uint32_t walked = 0, cend = 0;
@@ -90,7 +122,7 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
   int e_base = 0;
   bool finished = __all_sync(FULL, done == 0xffu);
   while (!finished) {
-    // fill the queue with the next entries of the supertile list whose rect contains this tile
+    // fill the queue with the next entries of the supertile list that can contribute to this tile
     while (qn < 32u && pos < range.y) {
       const uint32_t i = pos + lane;
       bool hit = false;
@@ -98,10 +130,17 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
         const ushort4 rc = crect[i];
         hit = tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
       }
+      uint32_t r = 0;
+      if (hit) {
+        r = ckeys[i] & rmask;
+        const float4* sp = reinterpret_cast<const float4*>(splat_sorted + r);
+        const float4 a0 = sp[0], a1 = sp[1];
+        hit = ellipse_reaches_tile(a0.x, a0.y, a0.z, a0.w, a1.x, a1.w, X0, Y0);
+      }
       const unsigned m = __ballot_sync(FULL, hit);
       if (hit) {
         const uint32_t slot = qn + __popc(m & lt);
-        q_rank[slot] = ckeys[i] & rmask;
+        q_rank[slot] = r;
         q_cpos[slot] = i;
       }
       qn += __popc(m);
@@ -114,32 +153,32 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
     for (uint32_t j = 0; j < cnt; ++j) {
       const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
       const int e1 = e_base + (int)j + 1;
+      const float dx = sub_rn(px, s0.x);
+      bool anycomp = false;
       ++walked;
 #pragma unroll
       for (int k = 0; k < PPL; ++k) {
-        if (!((done >> k) & 1u)) {
-          const float dx = sub_rn(px, s0.x), dy = sub_rn((float)(y0 + k) + 0.5f, s0.y);
-          const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
-          if (power <= 0.0f && power >= s1.w) {          // s1.w = tau >= -6: pre-test, never decides (see project.cu)
-            const float a = mul_rn(s1.y, exp_spec(power));
-            if (a >= prm.alpha_min) {
-              const float alpha = fminf(a, prm.alpha_max);
-              const float Tn = mul_rn(T[k], sub_rn(1.0f, alpha));
-              if (Tn < prm.t_stop) {
-                done |= 1u << k;                          // stop BEFORE compositing (R-4)
-              } else {
-                const float w = alpha * T[k];
-                C0[k] = fmaf(s2.x, w, C0[k]); C1[k] = fmaf(s2.y, w, C1[k]); C2[k] = fmaf(s2.z, w, C2[k]);
-                D[k] = fmaf(s1.z, w, D[k]);
-                T[k] = Tn;
-                ++n[k];
-                last[k] = e1;
-                cend = __float_as_uint(s2.w);             // coarse position + 1 of the last composited entry
-              }
-            }
-          }
+        const float dy = sub_rn(py[k], s0.y);
+        const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
+        const float a = mul_rn(s1.y, exp_spec(power));       // garbage outside [tau, 0]: masked by `pass`
+        // s1.w = tau >= -6 is a pre-test that never decides (project.cu); the alpha test does (R-4, R-5)
+        const bool pass = power <= 0.0f && power >= s1.w && a >= prm.alpha_min && !((done >> k) & 1u);
+        const float alpha = fminf(a, prm.alpha_max);
+        const float Tn = mul_rn(T[k], sub_rn(1.0f, alpha));
+        const bool stop = Tn < prm.t_stop;                   // stop BEFORE compositing (R-4)
+        const bool comp = pass && !stop;
+        if (FULLPIX) {
+          const float w = comp ? alpha * T[k] : 0.0f;
+          C0[k] = fmaf(s2.x, w, C0[k]); C1[k] = fmaf(s2.y, w, C1[k]); C2[k] = fmaf(s2.z, w, C2[k]);
+          D[k] = fmaf(s1.z, w, D[k]);
+          n[k] += comp ? 1 : 0;
         }
+        T[k] = comp ? Tn : T[k];
+        last[k] = comp ? e1 : last[k];
+        if (pass && stop) done |= 1u << k;
+        anycomp = anycomp || comp;
       }
+      if (anycomp) cend = __float_as_uint(s2.w);               // coarse position + 1 of the last composited entry
       if (__all_sync(FULL, done == 0xffu)) { finished = true; break; }
     }
     e_base += (int)cnt;
@@ -148,31 +187,44 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
   unsigned pairs = 0;
 #pragma unroll
   for (int k = 0; k < PPL; ++k) {
-    pairs += n[k];
     if (x < prm.W && y0 + k < prm.H) {
       const size_t p = (size_t)(y0 + k) * prm.W + x;
-      if (out.rgb) {
+      if (FULLPIX) {
+        pairs += n[k];
         out.rgb[3 * p + 0] = fmaf(prm.bg[0], T[k], C0[k]);
         out.rgb[3 * p + 1] = fmaf(prm.bg[1], T[k], C1[k]);
         out.rgb[3 * p + 2] = fmaf(prm.bg[2], T[k], C2[k]);
+        out.depth[p] = D[k];
+        out.ncontrib[p] = n[k];
       }
-      if (out.depth) out.depth[p] = D[k];
       out.T[p] = T[k];
-      if (out.ncontrib) out.ncontrib[p] = n[k];
       out.last[p] = last[k];
     }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
-    pairs += __shfl_xor_sync(FULL, pairs, o);
+    if (FULLPIX) pairs += __shfl_xor_sync(FULL, pairs, o);
     cend = max(cend, __shfl_xor_sync(FULL, cend, o));
   }
   if (lane == 0) {
     tile_cend[tile] = cend;
-    if (tile_walk) tile_walk[tile] = walked;
-    atomicAdd(&counters->n_entries, (unsigned long long)walked);
-    atomicAdd(&counters->n_pairs, (unsigned long long)pairs);
+    tile_walk[tile] = walked;
+    if (FULLPIX) {
+      atomicAdd(&counters->n_entries, (unsigned long long)walked);
+      atomicAdd(&counters->n_pairs, (unsigned long long)pairs);
+    }
   }
+}
+
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 
 // Sum v[0..39] over the 32 lanes.  On return lane l holds the totals of moments idx0 and idx1 (or -1).
@@ -225,20 +277,23 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
                                                        float* __restrict__ moments, uint32_t* __restrict__ touched,
                                                        ViewCounters* counters) {
   __shared__ float4 sm[32 * 3];
+  __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22, -) of Sigma2D = L L^T
   __shared__ uint32_t q_rank[64];
   const int tile = blockIdx.x, lane = threadIdx.x;
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
+  const float X0 = (float)(tx * TILE), Y0 = (float)(ty * TILE);
   const uint32_t rmask = (1u << prm.rank_bits) - 1u;
   const uint32_t lt = (1u << lane) - 1u;
 
-  float Tc[PPL], S0[PPL], S1[PPL], S2[PPL], S3[PPL];
+  float Tc[PPL], S0[PPL], S1[PPL], S2[PPL], S3[PPL], py[PPL];
   int last[PPL];
   int maxlast = 0;
 #pragma unroll
   for (int k = 0; k < PPL; ++k) {
     last[k] = 0; Tc[k] = 1.0f;
+    py[k] = (float)(y0 + k) + 0.5f;
     if (x < prm.W && y0 + k < prm.H) {
       const size_t p = (size_t)(y0 + k) * prm.W + x;
       last[k] = pix.last[p];
@@ -266,8 +321,15 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
         const ushort4 rc = crect[i];
         hit = tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
       }
+      uint32_t r = 0;
+      if (hit) {
+        r = ckeys[i] & rmask;
+        const float4* sp = reinterpret_cast<const float4*>(splat_sorted + r);
+        const float4 a0 = sp[0], a1 = sp[1];
+        hit = ellipse_reaches_tile(a0.x, a0.y, a0.z, a0.w, a1.x, a1.w, X0, Y0);
+      }
       const unsigned m = __ballot_sync(FULL, hit);
-      if (hit) q_rank[qn + __popc(m & lt)] = ckeys[i] & rmask;
+      if (hit) q_rank[qn + __popc(m & lt)] = r;
       qn += __popc(m);
       pos_hi -= span;
     }
@@ -275,64 +337,119 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
     const int cnt = (int)min(qn, 32u);
     __syncwarp();
     stage_queue(splat_sorted, q_rank, nullptr, (uint32_t)cnt, sm);
+    if (lane < cnt) {
+      // Cholesky whitening of the footprint: xi = L^-1 d with Sigma2D = L L^T (L lower triangular), from the conic
+      // Sigma2D^-1 = [[cA, cB], [cB, cC]]:  1/l22 = sqrt(cC),  1/l11 = sqrt(det(conic) / cC),  l21/l11 = -cB / cC
+      const float4 q0 = sm[lane * 3], q1 = sm[lane * 3 + 1];
+      const float cA = -2.0f * q0.z, cB = -q0.w, cC = -2.0f * q1.x;
+      const float icC = 1.0f / cC;
+      sm_wh[lane] = make_float4(sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), -cB * icC, sqrtf(cC), 0.0f);
+    }
+    __syncwarp();
     for (int j = 0; j < cnt; ++j) {
       const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
       const int e = e_next - j;
-      const float cA = -2.0f * s0.z, cB = -s0.w, cC = -2.0f * s1.x;    // conic = Sigma2D^-1
-      float acc[NMOM];
+      const float dx = sub_rn(px, s0.x);
+      // pass 1 (decision path): power bit-identical to S3; alpha from the fast exp.  Wherever alpha comes within
+      // 8e-6 (relative) of a threshold of R-4 the exact exp_spec value is substituted below, so every decision
+      // (contributor or not, clamped or not) is the one S3 took; elsewhere the two exps agree to < 1e-6 relative.
+      float av[PPL];
+      unsigned inr = 0;
+      bool near = false;
 #pragma unroll
-      for (int m = 0; m < NMOM; ++m) acc[m] = 0.0f;
+      for (int k = 0; k < PPL; ++k) {
+        const float dy = sub_rn(py[k], s0.y);
+        const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
+        const float a = s1.y * ex2_approx(power * 0x1.715476p+0f);
+        const bool in = e < last[k] && power <= 0.0f && power >= s1.w;
+        av[k] = a;
+        inr |= in ? (1u << k) : 0u;
+        near = near || (in && (fabsf(a - prm.alpha_min) <= 8e-6f * prm.alpha_min || fabsf(a - prm.alpha_max) <= 8e-6f * prm.alpha_max));
+      }
+      if (__any_sync(FULL, near)) {
+#pragma unroll
+        for (int k = 0; k < PPL; ++k) {
+          const float dy = sub_rn(py[k], s0.y);
+          av[k] = mul_rn(s1.y, exp_spec(splat_power(s0.z, s0.w, s1.x, dx, dy)));
+        }
+      }
+      // pass 2 (value path): beta, suffix sums, and the sums  F_p = sum_k f_k t_k^p,  G_c,p = sum_k g_c,k t_k^p  over
+      // the lane's 8 pixels with t_k = k - 3.5 a compile-time constant (dy_k = dyc + t_k)
+      float F0 = 0.f, F1 = 0.f, F2 = 0.f, F3 = 0.f, F4 = 0.f, W2 = 0.f;
+      float G[NCH][3];
+#pragma unroll
+      for (int c = 0; c < NCH; ++c) G[c][0] = G[c][1] = G[c][2] = 0.f;
       bool any = false;
 #pragma unroll
       for (int k = 0; k < PPL; ++k) {
-        if (e < last[k]) {
-          const float dx = sub_rn(px, s0.x), dy = sub_rn((float)(y0 + k) + 0.5f, s0.y);
-          const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
-          if (power <= 0.0f && power >= s1.w) {
-            const float a = mul_rn(s1.y, exp_spec(power));
-            if (a >= prm.alpha_min) {                      // same tests as S3 -> same contributor set
-              any = true;
-              const bool clamped = a > prm.alpha_max;
-              const float alpha = fminf(a, prm.alpha_max);
-              const float rc = __fdividef(1.0f, 1.0f - alpha);
-              const float Ti = Tc[k] * rc;                 // T_i = T_{i+1} / (1 - alpha_i)
-              const float w = alpha * Ti;
-              // beta_ch = dy_ch/dalpha_i = T_i v_i - Splus_i / (1 - alpha_i)
-              const float b0 = Ti * s2.x - S0[k] * rc, b1 = Ti * s2.y - S1[k] * rc, b2 = Ti * s2.z - S2[k] * rc;
-              S0[k] = fmaf(s2.x, w, S0[k]); S1[k] = fmaf(s2.y, w, S1[k]); S2[k] = fmaf(s2.z, w, S2[k]);
-              float b3 = 0.0f;
-              if (NCH == 4) { b3 = Ti * s1.z - S3[k] * rc; S3[k] = fmaf(s1.z, w, S3[k]); }
-              Tc[k] = Ti;
-              acc[MOM_W2] = fmaf(w, w, acc[MOM_W2]);
-              if (!clamped) {                              // R-11: zero derivative at the 0.99 cap
-                const float ux = cA * dx + cB * dy, uy = cB * dx + cC * dy;
-                float B = prm.omega[0] * b0 * b0 + prm.omega[1] * b1 * b1 + prm.omega[2] * b2 * b2;
-                if (NCH == 4) B = fmaf(prm.omega[3] * b3, b3, B);
-                const float f = B * alpha * alpha;
-                const float ux2 = ux * ux, uxy = ux * uy, uy2 = uy * uy;
-                const float f10 = f * ux, f01 = f * uy, f20 = f * ux2, f11 = f * uxy, f02 = f * uy2;
-                acc[0] += f; acc[1] += f10; acc[2] += f01; acc[3] += f20; acc[4] += f11; acc[5] += f02;
-                acc[6] = fmaf(f20, ux, acc[6]); acc[7] = fmaf(f20, uy, acc[7]); acc[8] = fmaf(f02, ux, acc[8]); acc[9] = fmaf(f02, uy, acc[9]);
-                acc[10] = fmaf(f20, ux2, acc[10]); acc[11] = fmaf(f20, uxy, acc[11]); acc[12] = fmaf(f20, uy2, acc[12]);
-                acc[13] = fmaf(f02, uxy, acc[13]); acc[14] = fmaf(f02, uy2, acc[14]);
-                const float wa = w * alpha;
-                const float bch[4] = {b0, b1, b2, b3};
+        const float a = av[k];
+        const bool pass = ((inr >> k) & 1u) && a >= prm.alpha_min;      // same tests as S3 -> same contributor set
+        const bool active = pass && !(a > prm.alpha_max);                // R-11: zero derivative at the 0.99 cap
+        const float alpha = fminf(a, prm.alpha_max);
+        const float rc = rcp_approx(1.0f - alpha);
+        const float Ti = Tc[k] * rc;                                     // T_i = T_{i+1} / (1 - alpha_i)
+        const float w = alpha * Ti;
+        // beta_ch = dy_ch/dalpha_i = T_i v_i - Splus_i / (1 - alpha_i)
+        const float b0 = Ti * s2.x - S0[k] * rc, b1 = Ti * s2.y - S1[k] * rc, b2 = Ti * s2.z - S2[k] * rc;
+        float b3 = 0.0f;
+        if (NCH == 4) b3 = Ti * s1.z - S3[k] * rc;
+        const float wm = pass ? w : 0.0f;
+        S0[k] = fmaf(s2.x, wm, S0[k]); S1[k] = fmaf(s2.y, wm, S1[k]); S2[k] = fmaf(s2.z, wm, S2[k]);
+        if (NCH == 4) S3[k] = fmaf(s1.z, wm, S3[k]);
+        Tc[k] = pass ? Ti : Tc[k];
+        W2 = fmaf(wm, wm, W2);
+        float Bq = prm.omega[0] * b0 * b0 + prm.omega[1] * b1 * b1 + prm.omega[2] * b2 * b2;
+        if (NCH == 4) Bq = fmaf(prm.omega[3] * b3, b3, Bq);
+        const float aa = active ? alpha : 0.0f;
+        const float f = Bq * aa * aa;
+        const float wa = w * aa;
+        const float t1 = (float)k - 3.5f, t2 = t1 * t1, t3 = t2 * t1, t4 = t2 * t2;
+        F0 += f; F1 = fmaf(f, t1, F1); F2 = fmaf(f, t2, F2); F3 = fmaf(f, t3, F3); F4 = fmaf(f, t4, F4);
+        const float bch[4] = {b0, b1, b2, b3};
 #pragma unroll
-                for (int c = 0; c < NCH; ++c) {
-                  const float g = bch[c] * wa;
-                  acc[MOM_X + 6 * c + 0] = fmaf(g, ux, acc[MOM_X + 6 * c + 0]);
-                  acc[MOM_X + 6 * c + 1] = fmaf(g, uy, acc[MOM_X + 6 * c + 1]);
-                  acc[MOM_X + 6 * c + 2] = fmaf(g, ux2, acc[MOM_X + 6 * c + 2]);
-                  acc[MOM_X + 6 * c + 3] = fmaf(g, uxy, acc[MOM_X + 6 * c + 3]);
-                  acc[MOM_X + 6 * c + 4] = fmaf(g, uy2, acc[MOM_X + 6 * c + 4]);
-                  acc[MOM_X + 6 * c + 5] += g;
-                }
-              }
-            }
-          }
+        for (int c = 0; c < NCH; ++c) {
+          const float g = bch[c] * wa;
+          G[c][0] += g; G[c][1] = fmaf(g, t1, G[c][1]); G[c][2] = fmaf(g, t2, G[c][2]);
         }
+        any = any || pass;
       }
       if (__any_sync(FULL, any)) {
+        // The lane's 40 moments in the WHITENED coordinates xi = L^-1 (pixel - centre): xi1 = dx / l11 is the same for
+        // the lane's 8 pixels and xi2 = (dy - (l21 / l11) dx) / l22 = xc + h t_k steps with the row, so
+        // Y_b = sum_k f_k xi2_k^b follows from the F_p by a binomial shift, and the monomial sums are xi1^i Y_j.
+        // (The shear keeps the column structure; the whitening keeps the later change to the u basis free of the
+        // cancellation a plain pixel-offset basis has for elongated footprints.  DESIGN.md section 6.)
+        float acc[NMOM];
+        const float4 wh = sm_wh[j];
+        const float x1 = dx * wh.x;
+        const float h = wh.z, h2 = h * h;
+        const float c1 = (((py[0] + 3.5f) - s0.y) - wh.y * dx) * h, c2 = c1 * c1, c3 = c2 * c1, c4 = c2 * c2;
+        const float E1 = h * F1, E2 = h2 * F2, E3 = h2 * h * F3, E4 = h2 * h2 * F4;
+        const float Y0v = F0;
+        const float Y1v = fmaf(c1, F0, E1);
+        const float Y2v = fmaf(c2, F0, fmaf(2.0f * c1, E1, E2));
+        const float Y3v = fmaf(c3, F0, fmaf(3.0f * c2, E1, fmaf(3.0f * c1, E2, E3)));
+        const float Y4v = fmaf(c4, F0, fmaf(4.0f * c3, E1, fmaf(6.0f * c2, E2, fmaf(4.0f * c1, E3, E4))));
+        const float x2 = x1 * x1, x3 = x2 * x1, x4 = x2 * x2;
+        acc[0] = Y0v;
+        acc[1] = x1 * Y0v;  acc[2] = Y1v;
+        acc[3] = x2 * Y0v;  acc[4] = x1 * Y1v;  acc[5] = Y2v;
+        acc[6] = x3 * Y0v;  acc[7] = x2 * Y1v;  acc[8] = x1 * Y2v;  acc[9] = Y3v;
+        acc[10] = x4 * Y0v; acc[11] = x3 * Y1v; acc[12] = x2 * Y2v; acc[13] = x1 * Y3v; acc[14] = Y4v;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          float* xm = acc + MOM_X + 6 * c;
+          if (c < NCH) {
+            const int cc = c < NCH ? c : 0;
+            const float Z0 = G[cc][0], H1 = h * G[cc][1];
+            const float Z1 = fmaf(c1, Z0, H1);
+            const float Z2 = fmaf(c2, Z0, fmaf(2.0f * c1, H1, h2 * G[cc][2]));
+            xm[0] = x1 * Z0; xm[1] = Z1; xm[2] = x2 * Z0; xm[3] = x1 * Z1; xm[4] = Z2; xm[5] = Z0;
+          } else {
+            xm[0] = xm[1] = xm[2] = xm[3] = xm[4] = xm[5] = 0.0f;
+          }
+        }
+        acc[MOM_W2] = W2;
         float o0, o1;
         int i0, i1;
         butterfly40(acc, lane, o0, o1, i0, i1);
@@ -369,7 +486,10 @@ void launch_forward(const Splat* splat_sorted, const uint32_t* ckeys, const usho
                     ViewCounters* counters, cudaStream_t st) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
   ++g_kernel_launches;
-  forward_kernel<<<tg.tiles_x * tg.tiles_y, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, p, px, tile_cend, tile_walk, counters);
+  if (px.rgb)
+    forward_kernel<true><<<tg.tiles_x * tg.tiles_y, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, p, px, tile_cend, tile_walk, counters);
+  else
+    forward_kernel<false><<<tg.tiles_x * tg.tiles_y, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, p, px, tile_cend, tile_walk, counters);
 }
 
 void launch_backward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
