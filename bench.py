@@ -276,8 +276,11 @@ def main():
     # ---- counts of the same views (untimed pass) for the algorithmic work ----
     tot = dict(n_visible=0, n_keys=0, n_entries=0, n_pairs=0, n_touched=0, n_coarse=0)
     for cam in wl.cand_cams:
-        nbv.gaussian_gains(cam, wl.target_obj)
+        nbv.gaussian_gains(cam, wl.target_obj)          # hot kernels: n_visible, n_keys, n_coarse, n_touched
         st = nbv.last_view_stats()
+        nbv.render(cam)                                 # counting forward pass: n_entries, n_pairs
+        st_r = nbv.last_view_stats()
+        st["n_entries"], st["n_pairs"] = st_r["n_entries"], st_r["n_pairs"]
         for k in tot:
             tot[k] += st[k]
 
