@@ -101,10 +101,12 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg);
 void nbv_destroy(nbv_ctx* ctx);
 const char* nbv_last_error(const nbv_ctx* ctx);
 
-/* Number of views processed concurrently (each on its own internal stream, forked from and joined back into the
- * caller's stream with events; 1 = everything on the caller's stream).  Default 4; the NBV_CONCURRENCY environment
- * variable overrides the default at nbv_create.  Views are independent (the arg max is over per-view gains),
- * so this changes no result beyond the order of floating-point atomics.  Errors: INVALID_ARG outside [1, 16]. */
+/* Views per batch (default and maximum 8; the NBV_CONCURRENCY environment variable overrides the default at nbv_create).
+ * S1-S2 of the views of a batch run concurrently on internal streams (forked from and joined back into the caller's
+ * stream with events); S3, S4 and S5+S6 are ONE kernel launch each per batch (grid.y = view).  Two sets of work buffers
+ * alternate so the S1-S2 work of the next batch overlaps the S3-S6 launches of this one.  Views are independent
+ * (the arg max is over per-view gains), so this changes no result beyond the order of floating-point atomics.
+ * Errors: INVALID_ARG outside [1, 8]. */
 int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight);
 
 /* S0 -- load the Gaussian map G with object vectors: device arrays, row-major, float32.
@@ -155,8 +157,8 @@ int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream);
 #define NBV_STAGE_EXPAND 6
 #define NBV_N_STAGES 7
 
-/* enable != 0: record CUDA events on `stream` at every stage boundary of every view processed from now on
- * (a few microseconds per view); clears the accumulated times.  Synchronises `stream`. */
+/* enable != 0: bracket every stage launch (per view for S1-S2, per batch for S3-S6) with CUDA events on the stream it
+ * runs on, from now on (a few microseconds per view); clears the accumulated times.  Synchronises `stream`. */
 int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream);
 
 /* h_ms[NBV_N_STAGES] <- milliseconds spent per stage, summed over the *h_views views processed since timing was

@@ -215,12 +215,13 @@ __device__ void build_block(const float* mom, const ChainF& ch, float kappa, con
   for (int c = 0; c < 4; ++c) {
     const float om = omega[c];
     if (om == 0.f) continue;
+    const float som = sqrtf(om);
     float yv[11];
     for (int k = 0; k < 11; ++k) {
       float v = 0.f;
 #pragma unroll
       for (int i = 0; i < 6; ++i) v += A[k][i] * mom[MOM_X + 6 * c + i];
-      yv[k] = om * v;
+      yv[k] = som * v;                       // S4 delivers the cross moments scaled by sqrt(omega_ch)
     }
     if (c < 3) {
       for (int k = 0; k < 11; ++k) H[tri(k, 11 + c)] += yv[k];
@@ -292,12 +293,19 @@ __device__ float gain_solve(float* B, const float* U) {
   return ld;
 }
 
-__global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam, nbv_config cfg, const uint32_t* __restrict__ ids_sorted,
-                                                     const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ touched, float* __restrict__ moments, int mode,
-                                                     float* __restrict__ H_T, float* __restrict__ out_blocks,
-                                                     const float* __restrict__ conf, const float* __restrict__ cholT,
-                                                     float* __restrict__ score, float* __restrict__ gains, ViewCounters* counters) {
-  const uint32_t n_touched = counters->n_touched;
+__global__ void __launch_bounds__(64) expand_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
+                                                     const __grid_constant__ ExpandBatch batch, int mode, float* __restrict__ H_T,
+                                                     const float* __restrict__ conf, const float* __restrict__ cholT) {
+  const ExpandView& vw = batch.v[blockIdx.y];
+  const nbv_camera& cam = vw.cam;
+  const uint32_t* __restrict__ ids_sorted = vw.ids_sorted;
+  const Splat* __restrict__ splat_sorted = vw.splat_sorted;
+  const uint32_t* __restrict__ touched = vw.touched;
+  float* __restrict__ moments = vw.moments;
+  float* __restrict__ out_blocks = vw.out_blocks;
+  float* __restrict__ score = vw.score;
+  float* __restrict__ gains = vw.gains;
+  const uint32_t n_touched = vw.counters->n_touched;
   float gain = 0.f;
   float omega[4];
 #pragma unroll
@@ -357,14 +365,13 @@ __global__ void __launch_bounds__(64) expand_kernel(SceneDev sc, nbv_camera cam,
   }
 }
 
-void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
-                   const Splat* splat_sorted, const uint32_t* touched, float* moments, int mode, float* H_T, float* out_blocks, const float* conf,
-                   const float* cholT, float* score, float* gains, ViewCounters* counters, cudaStream_t st) {
+void launch_expand(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, float* H_T, const float* conf,
+                   const float* cholT, cudaStream_t st) {
   int blocks = (sc.N + 63) / 64;
-  if (blocks > 148 * 8) blocks = 148 * 8;
+  const int cap = (148 * 8 + batch.n - 1) / batch.n;
+  if (blocks > cap) blocks = cap;
   ++g_kernel_launches;
-  expand_kernel<<<blocks, 64, 0, st>>>(sc, cam, cfg, ids_sorted, splat_sorted, touched, moments, mode, H_T, out_blocks, conf, cholT, score, gains,
-                                       counters);
+  expand_kernel<<<dim3((unsigned)blocks, (unsigned)batch.n), 64, 0, st>>>(sc, cfg, batch, mode, H_T, conf, cholT);
 }
 
 // S0': confidence (Eq. 7; Eq. 12)

@@ -58,23 +58,55 @@ struct PixelBuf {            // per-pixel outputs of the forward pass (H x W eac
   int32_t* ncontrib;
   int32_t* last;             // list position (relative to the tile's range) after the last composited entry
 };
-void launch_forward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
-                    int rank_bits, int W, int H, const nbv_config& cfg, PixelBuf px, uint32_t* tile_cend, uint32_t* tile_walk,
-                    ViewCounters* counters, cudaStream_t st);
-// moments must be zero on entry for every Gaussian; `touched` receives the ranks with a non-zero block
-// (counters->n_touched of them, in no particular order)
-void launch_backward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
-                     int rank_bits, int W, int H, const nbv_config& cfg, PixelBuf px, const uint32_t* tile_cend, float* moments,
-                     uint32_t* touched, ViewCounters* counters, cudaStream_t st);
+// One launch of S3 / S4 / S5+S6 serves a BATCH of views (grid.y = view): per-view device pointers travel as a
+// __grid_constant__ kernel parameter.  All views of a batch share the image size.
+constexpr int MAX_BATCH = 8;
+struct RasterView {
+  const Splat* splat_sorted;
+  const uint32_t* ckeys;
+  const ushort4* crect;
+  const uint2* cranges;
+  PixelBuf pix;
+  uint32_t* tile_cend;       // per tile: coarse position + 1 of the last composited entry
+  uint32_t* tile_walk;       // per tile: list entries S3 consumed
+  float* moments;            // N x NMOM, zero on entry to S4 for every Gaussian
+  uint32_t* touched;         // ranks with a non-zero block (counters->n_touched of them, in no particular order)
+  ViewCounters* counters;
+};
+struct RasterBatch {
+  int n;
+  const uint32_t* tile_order;   // launch position -> tile: tiles by increasing distance from the image centre, so the
+                                // long-running central tiles of a look-at view start first and the tail is made of cheap ones
+  RasterView v[MAX_BATCH];
+};
+void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg, bool full_pix,
+                    cudaStream_t st);
+// S4, then the touched lists (ranks with sum w^2 != 0) of every view of the batch
+void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
+                     cudaStream_t st);
 
 // ---- hessian.cu
 enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2 };
 // EXPAND_TRAIN: H_T[id] += H ; EXPAND_VIEW: out_blocks[id] = H ; EXPAND_GAIN: gain vs H_T, sum into *score (and gains[id] if not null)
-// Consumes the touched list: reads the moments of every touched rank and writes zeros back (the moment buffer is
-// all-zero again afterwards).
-void launch_expand(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, const uint32_t* ids_sorted,
-                   const Splat* splat_sorted, const uint32_t* touched, float* moments, int mode, float* H_T, float* out_blocks, const float* conf,
-                   const float* cholT, float* score, float* gains, ViewCounters* counters, cudaStream_t st);
+// Consumes the touched list of every view of the batch: reads the moments of every touched rank and writes zeros back
+// (the moment buffers are all-zero again afterwards).
+struct ExpandView {
+  nbv_camera cam;
+  const uint32_t* ids_sorted;
+  const Splat* splat_sorted;
+  const uint32_t* touched;
+  float* moments;
+  float* out_blocks;         // EXPAND_VIEW
+  float* score;              // EXPAND_GAIN
+  float* gains;              // EXPAND_GAIN, may be null
+  ViewCounters* counters;
+};
+struct ExpandBatch {
+  int n;
+  ExpandView v[MAX_BATCH];
+};
+void launch_expand(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, float* H_T, const float* conf,
+                   const float* cholT, cudaStream_t st);
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);
 void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);

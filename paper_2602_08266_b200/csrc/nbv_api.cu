@@ -42,10 +42,12 @@ struct ViewSlot {
   uint32_t ccap = 0;                    // capacity of the coarse key buffers
   uint32_t* ckeys_sorted = nullptr;
   bool moments_clean = false;           // the moment buffer is known to be all zero
-  // per-stage timing: one event row per view, folded on read-out
-  std::vector<cudaEvent_t> ev;          // ev[view * (NBV_N_STAGES + 1) + boundary]
-  std::vector<unsigned> ev_mask;        // per view: bit b set when boundary b was recorded
-  size_t ev_views = 0;
+};
+
+// One timed interval of one stage: events a..b on the stream the stage ran on, covering `views` views.
+struct Span {
+  cudaEvent_t a, b;
+  int stage, views;
 };
 
 struct nbv_ctx {
@@ -58,13 +60,19 @@ struct nbv_ctx {
   // scene
   DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp;
   int conf_target = -2;                 // target the conf / cholT buffers were prepared for (-2 = stale)
-  // views in flight
+  // views in flight: S1-S2 of each view run on its slot's stream, S3-S6 of a whole batch in one launch per stage on
+  // the caller's stream; two sets of `concurrency` slots alternate so the next batch's S1-S2 overlap this batch's S3-S6
   std::vector<ViewSlot*> slots;
-  int concurrency = 4;
+  int concurrency = MAX_BATCH;
   cudaEvent_t ev_fork = nullptr;
+  cudaEvent_t ev_set_done[2] = {nullptr, nullptr};   // S3-S6 of the last batch that used slot set 0 / 1
   ViewSlot* last_slot = nullptr;        // slot of the last view processed (nbv_last_view_stats)
+  DevBuf tile_order;                    // centre-out launch order of the tiles of a tile_order_tx x tile_order_ty grid
+  int tile_order_tx = 0, tile_order_ty = 0;
   // optional per-stage timing (nbv_set_stage_timing)
   bool timing = false;
+  std::vector<Span> spans;
+  size_t spans_used = 0;
   double stage_ms[NBV_N_STAGES] = {0};
   long long timed_views = 0;
 };
@@ -152,45 +160,47 @@ SceneDev scene_dev(const nbv_ctx* c) {
   return s;
 }
 
-constexpr int EV_ROW = NBV_N_STAGES + 1;
-constexpr size_t EV_MAX_VIEWS = 1024;
+constexpr size_t MAX_SPANS = 1 << 15;
 
-// fold the recorded event rows of a slot into ctx->stage_ms (its stream must be idle)
-void fold_timing(nbv_ctx* ctx, ViewSlot* sl) {
-  for (size_t v = 0; v < sl->ev_views; ++v) {
-    const unsigned m = sl->ev_mask[v];
-    for (int s = 0; s < NBV_N_STAGES; ++s)
-      if (((m >> s) & 1u) && ((m >> (s + 1)) & 1u)) {
-        float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, sl->ev[v * EV_ROW + s], sl->ev[v * EV_ROW + s + 1]) == cudaSuccess) ctx->stage_ms[s] += ms;
-      }
-    if (m) ctx->timed_views++;
-    sl->ev_mask[v] = 0;
+// fold the recorded spans into ctx->stage_ms (every stream that recorded one must be idle)
+void fold_timing(nbv_ctx* ctx) {
+  for (size_t i = 0; i < ctx->spans_used; ++i) {
+    const Span& sp = ctx->spans[i];
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) {
+      ctx->stage_ms[sp.stage] += ms;
+      if (sp.stage == NBV_STAGE_PROJECT) ctx->timed_views += sp.views;
+    }
   }
   cudaGetLastError();
-  sl->ev_views = 0;
+  ctx->spans_used = 0;
 }
 
-// start a new event row for the next view of this slot
-void timing_begin_view(nbv_ctx* ctx, ViewSlot* sl, cudaStream_t st) {
-  if (!ctx->timing) return;
-  if (sl->ev_views >= EV_MAX_VIEWS) { cudaStreamSynchronize(st); fold_timing(ctx, sl); }
-  const size_t v = sl->ev_views++;
-  if (sl->ev.size() < (v + 1) * EV_ROW) {
-    const size_t old = sl->ev.size();
-    sl->ev.resize((v + 1) * EV_ROW);
-    for (size_t i = old; i < sl->ev.size(); ++i) cudaEventCreate(&sl->ev[i]);
-    sl->ev_mask.resize(v + 1, 0u);
+// open a span of `stage` on stream st; returns its index or -1 when timing is off
+int span_begin(nbv_ctx* ctx, int stage, int views, cudaStream_t st) {
+  if (!ctx->timing) return -1;
+  if (ctx->spans_used >= MAX_SPANS) { cudaDeviceSynchronize(); fold_timing(ctx); }
+  if (ctx->spans_used == ctx->spans.size()) {
+    Span sp;
+    sp.stage = 0; sp.views = 0;
+    if (cudaEventCreate(&sp.a) != cudaSuccess || cudaEventCreate(&sp.b) != cudaSuccess) { cudaGetLastError(); return -1; }
+    ctx->spans.push_back(sp);
   }
-  sl->ev_mask[v] = 0;
+  const size_t i = ctx->spans_used++;
+  ctx->spans[i].stage = stage;
+  ctx->spans[i].views = views;
+  cudaEventRecord(ctx->spans[i].a, st);
+  return (int)i;
 }
 
-// record boundary b (= start of stage b, end of stage b-1) of the slot's current view
-void mark(nbv_ctx* ctx, ViewSlot* sl, int b, cudaStream_t st) {
-  if (!ctx->timing || sl->ev_views == 0) return;
-  const size_t v = sl->ev_views - 1;
-  cudaEventRecord(sl->ev[v * EV_ROW + b], st);
-  sl->ev_mask[v] |= 1u << b;
+void span_end(nbv_ctx* ctx, int idx, cudaStream_t st) {
+  if (idx >= 0) cudaEventRecord(ctx->spans[(size_t)idx].b, st);
+}
+
+// close span `idx` and open the next stage's at the same point of the stream
+int span_next(nbv_ctx* ctx, int idx, int stage, int views, cudaStream_t st) {
+  span_end(ctx, idx, st);
+  return span_begin(ctx, stage, views, st);
 }
 
 void free_slot(ViewSlot* sl) {
@@ -202,7 +212,6 @@ void free_slot(ViewSlot* sl) {
   for (DevBuf* b : all) release(*b);
   if (sl->d_counters) cudaFree(sl->d_counters);
   if (sl->h_counters) cudaFreeHost(sl->h_counters);
-  for (cudaEvent_t e : sl->ev) cudaEventDestroy(e);
   if (sl->done) cudaEventDestroy(sl->done);
   if (sl->st) cudaStreamDestroy(sl->st);
   delete sl;
@@ -247,10 +256,9 @@ TileGrid make_grid(int W, int H) {
 
 enum Stage { STAGE_PROJECT = 0, STAGE_BIN = 1, STAGE_FORWARD = 2, STAGE_BACKWARD = 3 };
 
-// S1..S4 for one camera on stream st, in the buffers of slot sl.  Leaves the depth order in sl->ids, rank-ordered splats,
-// the sorted coarse lists, per-pixel buffers and (STAGE_BACKWARD) the moment buffer + touched list.  Never synchronises.
-// full_pix: also write the colour / depth / count images (parity exports); the hot path needs only T and `last`.
-int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool want_abc, bool full_pix, cudaStream_t st) {
+// S1..S2 for one camera on stream st, in the buffers of slot sl: leaves the depth order in sl->ids, the rank-ordered splats and
+// the sorted coarse lists, and makes sure the buffers S3/S4 will need exist (upto).  Never synchronises.
+int pre_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool want_abc, bool full_pix, cudaStream_t st) {
   if (!valid_camera(cam)) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
   const int N = ctx->N;
   const TileGrid tg = make_grid(cam.width, cam.height);
@@ -272,17 +280,41 @@ int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bo
   if (want_abc) CKRET(ensure(ctx, sl->abc, 12 * (size_t)N));
   CKRET(ensure(ctx, sl->sort_tmp, 4 * radix_temp_words(std::max((size_t)N, (size_t)ccap))));
   CKRET(ensure(ctx, sl->scan_tmp, 4 * scan_temp_words(std::max((size_t)N + 1, (size_t)n_tiles + 1))));
+  if (upto >= STAGE_BIN) {
+    CKRET(ensure(ctx, sl->splat_sorted, sizeof(Splat) * (size_t)N));
+    CKRET(ensure(ctx, sl->rect_sorted, sizeof(ushort4) * (size_t)N));
+    CKRET(ensure(ctx, sl->ncoarse, 4 * (size_t)N));
+    CKRET(ensure(ctx, sl->offsets, 4 * (size_t)N));
+    CKRET(ensure(ctx, sl->ckeys, 4 * (size_t)ccap)); CKRET(ensure(ctx, sl->ckeys_alt, 4 * (size_t)ccap));
+    CKRET(ensure(ctx, sl->crect, sizeof(ushort4) * (size_t)ccap));
+    CKRET(ensure(ctx, sl->cranges, sizeof(uint2) * 256));
+  }
+  if (upto >= STAGE_FORWARD) {
+    const size_t npx = (size_t)cam.width * cam.height;
+    CKRET(ensure(ctx, sl->pix_T, 4 * npx)); CKRET(ensure(ctx, sl->pix_last, 4 * npx));
+    CKRET(ensure(ctx, sl->tile_cend, 4 * (size_t)n_tiles)); CKRET(ensure(ctx, sl->tile_walk, 4 * (size_t)n_tiles));
+    if (full_pix) {
+      CKRET(ensure(ctx, sl->pix_rgb, 12 * npx)); CKRET(ensure(ctx, sl->pix_depth, 4 * npx)); CKRET(ensure(ctx, sl->pix_nc, 4 * npx));
+    }
+  }
+  if (upto >= STAGE_BACKWARD) {
+    const size_t mom_bytes = 4 * (size_t)NMOM * N;
+    if (sl->moments.cap < mom_bytes || !sl->moments.p) sl->moments_clean = false;
+    CKRET(ensure(ctx, sl->moments, mom_bytes));
+    CKRET(ensure(ctx, sl->touched, 4 * (size_t)N));
+    if (!sl->moments_clean) CK(cudaMemsetAsync(sl->moments.p, 0, mom_bytes, st));
+    sl->moments_clean = false;     // dirty until an expand kernel has consumed the touched list
+  }
 
   CK(cudaMemsetAsync(sl->d_counters, 0, sizeof(ViewCounters), st));
-  timing_begin_view(ctx, sl, st);
-  mark(ctx, sl, NBV_STAGE_PROJECT, st);
+  int sp = span_begin(ctx, NBV_STAGE_PROJECT, 1, st);
   launch_project(sc, cam, ctx->cfg, sl->splat.as<Splat>(), sl->zkey.as<uint32_t>(), sl->ids.as<uint32_t>(),
                  sl->rect.as<ushort4>(), want_abc ? sl->abc.as<float>() : nullptr, sl->d_counters, st);
   CK(cudaGetLastError());
-  if (upto == STAGE_PROJECT) return NBV_OK;
+  if (upto == STAGE_PROJECT) { span_end(ctx, sp, st); return NBV_OK; }
 
   // depth sort: 4 stable passes of 8 bits on the z bits, Gaussian index as value (ties keep index order: R-7)
-  mark(ctx, sl, NBV_STAGE_DEPTH_SORT, st);
+  sp = span_next(ctx, sp, NBV_STAGE_DEPTH_SORT, 1, st);
   {
     uint32_t *k0 = sl->zkey.as<uint32_t>(), *k1 = sl->zkey_alt.as<uint32_t>();
     uint32_t *v0 = sl->ids.as<uint32_t>(), *v1 = sl->ids_alt.as<uint32_t>();
@@ -294,14 +326,7 @@ int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bo
     CK(cudaGetLastError());
   }
   // coarse binning: rank-ordered splats, supertile counts, scan, keys (supertile | rank) emitted rank-major
-  mark(ctx, sl, NBV_STAGE_BIN, st);
-  CKRET(ensure(ctx, sl->splat_sorted, sizeof(Splat) * (size_t)N));
-  CKRET(ensure(ctx, sl->rect_sorted, sizeof(ushort4) * (size_t)N));
-  CKRET(ensure(ctx, sl->ncoarse, 4 * (size_t)N));
-  CKRET(ensure(ctx, sl->offsets, 4 * (size_t)N));
-  CKRET(ensure(ctx, sl->ckeys, 4 * (size_t)ccap)); CKRET(ensure(ctx, sl->ckeys_alt, 4 * (size_t)ccap));
-  CKRET(ensure(ctx, sl->crect, sizeof(ushort4) * (size_t)ccap));
-  CKRET(ensure(ctx, sl->cranges, sizeof(uint2) * 256));
+  sp = span_next(ctx, sp, NBV_STAGE_BIN, 1, st);
   launch_gather(sl->ids.as<uint32_t>(), sl->splat.as<Splat>(), sl->rect.as<ushort4>(), N, tg.sshift, sl->splat_sorted.as<Splat>(),
                 sl->rect_sorted.as<ushort4>(), sl->ncoarse.as<uint32_t>(), st);
   exclusive_scan_u32(sl->ncoarse.as<uint32_t>(), sl->offsets.as<uint32_t>(), (size_t)N, sl->scan_tmp.as<uint32_t>(),
@@ -309,7 +334,7 @@ int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bo
   launch_emit_coarse(sl->rect_sorted.as<ushort4>(), sl->offsets.as<uint32_t>(), N, tg.sshift, tg.super_x, rank_bits, ccap,
                      sl->ckeys.as<uint32_t>(), st);
   // one stable pass on the supertile digit (<= 8 bits); its scanned histogram gives the supertile ranges
-  mark(ctx, sl, NBV_STAGE_COARSE_SORT, st);
+  sp = span_next(ctx, sp, NBV_STAGE_COARSE_SORT, 1, st);
   radix_pass(sl->ckeys.as<uint32_t>(), sl->ckeys_alt.as<uint32_t>(), nullptr, nullptr, (size_t)ccap, &sl->d_counters->n_coarse,
              rank_bits, super_bits, sl->sort_tmp.as<uint32_t>(), st);
   sl->ckeys_sorted = sl->ckeys_alt.as<uint32_t>();
@@ -318,72 +343,123 @@ int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bo
   launch_coarse_rect(sl->ckeys_sorted, &sl->d_counters->n_coarse, ccap, rank_bits, sl->rect_sorted.as<ushort4>(),
                      sl->crect.as<ushort4>(), st);
   CK(cudaGetLastError());
-  mark(ctx, sl, NBV_STAGE_FORWARD, st);
-  if (upto == STAGE_BIN) return NBV_OK;
-
-  const size_t npx = (size_t)cam.width * cam.height;
-  CKRET(ensure(ctx, sl->pix_T, 4 * npx)); CKRET(ensure(ctx, sl->pix_last, 4 * npx));
-  CKRET(ensure(ctx, sl->tile_cend, 4 * (size_t)n_tiles)); CKRET(ensure(ctx, sl->tile_walk, 4 * (size_t)n_tiles));
-  PixelBuf pb;
-  pb.rgb = nullptr; pb.depth = nullptr; pb.ncontrib = nullptr;
-  if (full_pix) {
-    CKRET(ensure(ctx, sl->pix_rgb, 12 * npx)); CKRET(ensure(ctx, sl->pix_depth, 4 * npx)); CKRET(ensure(ctx, sl->pix_nc, 4 * npx));
-    pb.rgb = sl->pix_rgb.as<float>(); pb.depth = sl->pix_depth.as<float>(); pb.ncontrib = sl->pix_nc.as<int32_t>();
-  }
-  pb.T = sl->pix_T.as<float>(); pb.last = sl->pix_last.as<int32_t>();
-  launch_forward(sl->splat_sorted.as<Splat>(), sl->ckeys_sorted, sl->crect.as<ushort4>(), sl->cranges.as<uint2>(), tg, rank_bits,
-                 cam.width, cam.height, ctx->cfg, pb, sl->tile_cend.as<uint32_t>(), sl->tile_walk.as<uint32_t>(), sl->d_counters, st);
-  CK(cudaGetLastError());
-  mark(ctx, sl, NBV_STAGE_BACKWARD, st);
-  if (upto == STAGE_FORWARD) return NBV_OK;
-
-  const size_t mom_bytes = 4 * (size_t)NMOM * N;
-  if (sl->moments.cap < mom_bytes || !sl->moments.p) sl->moments_clean = false;
-  CKRET(ensure(ctx, sl->moments, mom_bytes));
-  CKRET(ensure(ctx, sl->touched, 4 * (size_t)N));
-  if (!sl->moments_clean) CK(cudaMemsetAsync(sl->moments.p, 0, mom_bytes, st));
-  sl->moments_clean = false;     // dirty until an expand kernel has consumed the touched list
-  launch_backward(sl->splat_sorted.as<Splat>(), sl->ckeys_sorted, sl->crect.as<ushort4>(), sl->cranges.as<uint2>(), tg, rank_bits,
-                  cam.width, cam.height, ctx->cfg, pb, sl->tile_cend.as<uint32_t>(), sl->moments.as<float>(),
-                  sl->touched.as<uint32_t>(), sl->d_counters, st);
-  CK(cudaGetLastError());
-  mark(ctx, sl, NBV_STAGE_EXPAND, st);
+  span_end(ctx, sp, st);
   return NBV_OK;
 }
 
-// S5 (+S6) of the view process_view() left in the slot
+// launch order of the tiles: by increasing distance from the image centre (ties by tile index)
+int ensure_tile_order(nbv_ctx* ctx, const TileGrid& tg, cudaStream_t st) {
+  if (ctx->tile_order.p && ctx->tile_order_tx == tg.tiles_x && ctx->tile_order_ty == tg.tiles_y) return NBV_OK;
+  const int n = tg.tiles_x * tg.tiles_y;
+  std::vector<uint32_t> order((size_t)n);
+  for (int i = 0; i < n; ++i) order[(size_t)i] = (uint32_t)i;
+  const double cx = 0.5 * (tg.tiles_x - 1), cy = 0.5 * (tg.tiles_y - 1);
+  auto d2 = [&](uint32_t t) { const double dx = (int)(t % tg.tiles_x) - cx, dy = (int)(t / tg.tiles_x) - cy; return dx * dx + dy * dy; };
+  std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) { return d2(a) < d2(b); });
+  CK(cudaStreamSynchronize(st));        // a launch reading the previous table may still be queued
+  CKRET(ensure(ctx, ctx->tile_order, 4 * (size_t)n));
+  CK(cudaMemcpyAsync(ctx->tile_order.p, order.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
+  CK(cudaStreamSynchronize(st));        // `order` is a pageable host buffer about to go out of scope
+  ctx->tile_order_tx = tg.tiles_x; ctx->tile_order_ty = tg.tiles_y;
+  return NBV_OK;
+}
+
+// S3 (+ S4) for a batch of views whose S1-S2 products sit in sl[0..n): ONE launch per stage, grid.y = view.
+// All views share the image size (same tile grid).  Stream st must already be ordered after the slots' S1-S2.
+int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int upto, bool full_pix, cudaStream_t st) {
+  RasterBatch rb;
+  rb.n = n;
+  for (int i = 0; i < n; ++i) {
+    ViewSlot* s = sl[i];
+    RasterView& v = rb.v[i];
+    v.splat_sorted = s->splat_sorted.as<Splat>(); v.ckeys = s->ckeys_sorted; v.crect = s->crect.as<ushort4>();
+    v.cranges = s->cranges.as<uint2>();
+    v.pix.rgb = full_pix ? s->pix_rgb.as<float>() : nullptr;
+    v.pix.depth = full_pix ? s->pix_depth.as<float>() : nullptr;
+    v.pix.ncontrib = full_pix ? s->pix_nc.as<int32_t>() : nullptr;
+    v.pix.T = s->pix_T.as<float>(); v.pix.last = s->pix_last.as<int32_t>();
+    v.tile_cend = s->tile_cend.as<uint32_t>(); v.tile_walk = s->tile_walk.as<uint32_t>();
+    v.moments = s->moments.as<float>(); v.touched = s->touched.as<uint32_t>(); v.counters = s->d_counters;
+  }
+  const TileGrid tg = sl[0]->tg;
+  CKRET(ensure_tile_order(ctx, tg, st));
+  rb.tile_order = ctx->tile_order.as<uint32_t>();
+  int sp = span_begin(ctx, NBV_STAGE_FORWARD, n, st);
+  launch_forward(rb, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, ctx->cfg, full_pix, st);
+  CK(cudaGetLastError());
+  if (upto == STAGE_FORWARD) { span_end(ctx, sp, st); return NBV_OK; }
+  sp = span_next(ctx, sp, NBV_STAGE_BACKWARD, n, st);
+  launch_backward(rb, ctx->N, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, ctx->cfg, st);
+  CK(cudaGetLastError());
+  span_end(ctx, sp, st);
+  return NBV_OK;
+}
+
+// S5 (+S6) of the views raster_batch() left in the slots.  out_blocks / gains: single-view exports (n == 1) only.
+int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int mode, float* out_blocks, float* d_scores,
+                 float* gains, cudaStream_t st) {
+  ExpandBatch eb;
+  eb.n = n;
+  for (int i = 0; i < n; ++i) {
+    ViewSlot* s = sl[i];
+    ExpandView& v = eb.v[i];
+    v.cam = cams[i];
+    v.ids_sorted = s->ids.as<uint32_t>(); v.splat_sorted = s->splat_sorted.as<Splat>(); v.touched = s->touched.as<uint32_t>();
+    v.moments = s->moments.as<float>(); v.out_blocks = out_blocks; v.score = d_scores ? d_scores + i : nullptr; v.gains = gains;
+    v.counters = s->d_counters;
+  }
+  const int sp = span_begin(ctx, NBV_STAGE_EXPAND, n, st);
+  launch_expand(scene_dev(ctx), ctx->cfg, eb, mode, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
+  CK(cudaGetLastError());
+  span_end(ctx, sp, st);
+  for (int i = 0; i < n; ++i) sl[i]->moments_clean = true;
+  return NBV_OK;
+}
+
+// one view through S1..S4 on the caller's stream in slot 0 (parity exports)
+int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool want_abc, bool full_pix, cudaStream_t st) {
+  CKRET(pre_view(ctx, sl, cam, upto, want_abc, full_pix, st));
+  if (upto >= STAGE_FORWARD) CKRET(raster_batch(ctx, &sl, &cam, 1, upto, full_pix, st));
+  return NBV_OK;
+}
+
 int expand_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int mode, float* out_blocks, float* score, float* gains,
                 cudaStream_t st) {
-  launch_expand(scene_dev(ctx), cam, ctx->cfg, sl->ids.as<uint32_t>(), sl->splat_sorted.as<Splat>(), sl->touched.as<uint32_t>(), sl->moments.as<float>(), mode,
-                ctx->H_T.as<float>(), out_blocks, ctx->conf.as<float>(), ctx->cholT.as<float>(), score, gains, sl->d_counters, st);
-  CK(cudaGetLastError());
-  sl->moments_clean = true;
-  mark(ctx, sl, NBV_N_STAGES, st);
-  return NBV_OK;
+  return expand_batch(ctx, &sl, &cam, 1, mode, out_blocks, score, gains, st);
 }
 
-// Run S1..S6 for n cameras, round-robin over the view slots.  With more than one slot the slot streams fork from and
-// join back into the caller's stream through events, so the call stays asynchronous and stream-ordered for the caller.
+// Run S1..S6 for n cameras in batches of up to `concurrency` views of equal image size.  S1-S2 of every view run on its slot's
+// stream; S3, S4 and S5+S6 of the whole batch are one launch each on the caller's stream.  Two slot sets alternate, so the
+// S1-S2 work of batch b+1 overlaps the S3-S6 launches of batch b.  Everything is ordered by events: the call never blocks.
 int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_scores, cudaStream_t st) {
-  const int S = std::max(1, std::min(ctx->concurrency, n));
-  std::vector<ViewSlot*> sl((size_t)S);
-  for (int i = 0; i < S; ++i) CKRET(get_slot(ctx, i, &sl[i]));
-  if (S > 1) {
-    CK(cudaEventRecord(ctx->ev_fork, st));
-    for (int i = 0; i < S; ++i) CK(cudaStreamWaitEvent(sl[i]->st, ctx->ev_fork, 0));
-  }
+  const int V = std::max(1, std::min(ctx->concurrency, MAX_BATCH));
+  CK(cudaEventRecord(ctx->ev_fork, st));
   int rc = NBV_OK;
-  for (int i = 0; i < n && rc == NBV_OK; ++i) {
-    ViewSlot* s = sl[i % S];
-    cudaStream_t vs = S > 1 ? s->st : st;
-    rc = process_view(ctx, s, h_cams[i], STAGE_BACKWARD, false, false, vs);
-    if (rc == NBV_OK) rc = expand_view(ctx, s, h_cams[i], mode, nullptr, d_scores ? d_scores + i : nullptr, nullptr, vs);
-  }
-  if (S > 1)
-    for (int i = 0; i < S; ++i) {   // join even after an error: the caller's stream must not run ahead of the slots
+  int batch_no = 0;
+  bool set_used[2] = {false, false};
+  for (int i0 = 0; i0 < n && rc == NBV_OK; ++batch_no) {
+    int nb = 1;
+    while (nb < V && i0 + nb < n && h_cams[i0 + nb].width == h_cams[i0].width && h_cams[i0 + nb].height == h_cams[i0].height) ++nb;
+    const int set = batch_no & 1;
+    ViewSlot* sl[MAX_BATCH];
+    for (int i = 0; i < nb && rc == NBV_OK; ++i) rc = get_slot(ctx, set * MAX_BATCH + i, &sl[i]);
+    if (rc != NBV_OK) break;
+    int started = 0;
+    for (int i = 0; i < nb; ++i) {
+      // the slot's buffers are free once the S3-S6 launches of the batch that last used this set have finished
+      cudaStreamWaitEvent(sl[i]->st, set_used[set] ? ctx->ev_set_done[set] : ctx->ev_fork, 0);
+      if (rc == NBV_OK) rc = pre_view(ctx, sl[i], h_cams[i0 + i], STAGE_BACKWARD, false, false, sl[i]->st);
       cudaEventRecord(sl[i]->done, sl[i]->st);
-      cudaStreamWaitEvent(st, sl[i]->done, 0);
+      cudaStreamWaitEvent(st, sl[i]->done, 0);      // join even after an error: the caller's stream must not run ahead
+      ++started;
     }
+    (void)started;
+    if (rc == NBV_OK) rc = raster_batch(ctx, sl, h_cams + i0, nb, STAGE_BACKWARD, false, st);
+    if (rc == NBV_OK) rc = expand_batch(ctx, sl, h_cams + i0, nb, mode, nullptr, d_scores ? d_scores + i0 : nullptr, nullptr, st);
+    cudaEventRecord(ctx->ev_set_done[set], st);
+    set_used[set] = true;
+    i0 += nb;
+  }
   return rc;
 }
 
@@ -459,14 +535,16 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
   ctx->cfg = c;
   ctx->device = dev;
   ViewSlot* s0 = nullptr;
-  if (cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess || get_slot(ctx, 0, &s0) != NBV_OK) {
+  if (cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_set_done[0], cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&ctx->ev_set_done[1], cudaEventDisableTiming) != cudaSuccess || get_slot(ctx, 0, &s0) != NBV_OK) {
     cudaGetLastError();
     nbv_destroy(ctx);
     return NBV_ERR_CUDA;
   }
   if (const char* e = std::getenv("NBV_CONCURRENCY")) {
     const int v = std::atoi(e);
-    if (v >= 1 && v <= 16) ctx->concurrency = v;
+    if (v >= 1 && v <= MAX_BATCH) ctx->concurrency = v;
   }
   *out = ctx;
   return NBV_OK;
@@ -476,17 +554,19 @@ void nbv_destroy(nbv_ctx* ctx) {
   if (!ctx) return;
   cudaDeviceSynchronize();
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
-                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp};
+                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->tile_order};
   for (DevBuf* b : all) release(*b);
   for (ViewSlot* sl : ctx->slots) free_slot(sl);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  for (cudaEvent_t e : ctx->ev_set_done) if (e) cudaEventDestroy(e);
+  for (const Span& sp : ctx->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   cudaGetLastError();
   delete ctx;
 }
 
 int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight) {
   if (!ctx) return NBV_ERR_INVALID_ARG;
-  if (views_in_flight < 1 || views_in_flight > 16) return fail(ctx, NBV_ERR_INVALID_ARG, "views_in_flight must be in [1, 16]");
+  if (views_in_flight < 1 || views_in_flight > MAX_BATCH) return fail(ctx, NBV_ERR_INVALID_ARG, "views_in_flight must be in [1, 8]");
   ctx->concurrency = views_in_flight;
   return NBV_OK;
 }
@@ -606,10 +686,7 @@ int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream) {
 int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream) {
   if (!ctx) return NBV_ERR_INVALID_ARG;
   CK(cudaStreamSynchronize((cudaStream_t)stream));
-  for (ViewSlot* sl : ctx->slots) {
-    sl->ev_views = 0;
-    for (auto& m : sl->ev_mask) m = 0;
-  }
+  ctx->spans_used = 0;
   for (int s = 0; s < NBV_N_STAGES; ++s) ctx->stage_ms[s] = 0.0;
   ctx->timed_views = 0;
   ctx->timing = enable != 0;
@@ -618,11 +695,9 @@ int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream) {
 
 int nbv_stage_times(nbv_ctx* ctx, double* h_ms, int64_t* h_views, void* stream) {
   if (!ctx || !h_ms) return NBV_ERR_INVALID_ARG;
-  CK(cudaStreamSynchronize((cudaStream_t)stream));
-  for (ViewSlot* sl : ctx->slots) {
-    CK(cudaStreamSynchronize(sl->st));
-    fold_timing(ctx, sl);
-  }
+  CK(cudaStreamSynchronize((cudaStream_t)stream));     // the slot streams are joined into the caller's stream
+  for (ViewSlot* sl : ctx->slots) CK(cudaStreamSynchronize(sl->st));
+  fold_timing(ctx);
   for (int s = 0; s < NBV_N_STAGES; ++s) h_ms[s] = ctx->stage_ms[s];
   if (h_views) *h_views = ctx->timed_views;
   return NBV_OK;

@@ -25,6 +25,9 @@
 namespace nbv {
 
 constexpr int PPL = 8;                 // pixels per lane
+#ifndef NBV_BWD_MIN_BLOCKS
+#define NBV_BWD_MIN_BLOCKS 16          // resident warps per SM the backward kernel is compiled for (register cap)
+#endif
 constexpr unsigned FULL = 0xffffffffu;
 
 struct RasterParams {
@@ -33,6 +36,8 @@ struct RasterParams {
   float alpha_min, alpha_max, t_stop;
   float bg[3];
   float omega[4];                      // channel weights, 0 for disabled channels
+  float somega[4];                     // their square roots
+  float ln_amax_over_amin;
 };
 
 // Can any pixel centre of the tile whose first centre is (X0 + 0.5, Y0 + 0.5) reach power >= tau?  Conservative: the
@@ -93,13 +98,19 @@ __device__ __forceinline__ void shift_queue(uint32_t* q_rank, uint32_t* q_cpos, 
 // The slot body is branch-free (predicated updates): the 8 pixels of a lane are 8 independent dependency chains the
 // scheduler can interleave, and after the ellipse test nearly every staged entry touches nearly every slot anyway.
 template <bool FULLPIX>
-__global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ ckeys,
-                                                      const ushort4* __restrict__ crect, const uint2* __restrict__ cranges,
-                                                      RasterParams prm, PixelBuf out, uint32_t* __restrict__ tile_cend,
-                                                      uint32_t* __restrict__ tile_walk, ViewCounters* counters) {
+__global__ void __launch_bounds__(32) forward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
+  const RasterView& vw = batch.v[blockIdx.y];          // one launch rasterises every view of the batch
+  const Splat* __restrict__ splat_sorted = vw.splat_sorted;
+  const uint32_t* __restrict__ ckeys = vw.ckeys;
+  const ushort4* __restrict__ crect = vw.crect;
+  const uint2* __restrict__ cranges = vw.cranges;
+  const PixelBuf out = vw.pix;
+  uint32_t* __restrict__ tile_cend = vw.tile_cend;
+  uint32_t* __restrict__ tile_walk = vw.tile_walk;
+  ViewCounters* counters = vw.counters;
   __shared__ float4 sm[32 * 3];
   __shared__ uint32_t q_rank[64], q_cpos[64];
-  const int tile = blockIdx.x, lane = threadIdx.x;
+  const int tile = batch.tile_order[blockIdx.x], lane = threadIdx.x;   // heaviest tiles first (launch order)
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -110,17 +121,19 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
 
   float T[PPL], py[PPL], C0[PPL], C1[PPL], C2[PPL], D[PPL];
   int n[PPL], last[PPL];
-  unsigned done = 0;
+  // A pixel that has terminated (or lies outside the image) gets py = +inf: its power evaluates to -inf or NaN and
+  // fails `power >= tau`, so no separate done mask has to be tested in the slot body.
+  int ndone = 0;
 #pragma unroll
   for (int k = 0; k < PPL; ++k) {
     T[k] = 1.0f; C0[k] = C1[k] = C2[k] = D[k] = 0.0f; n[k] = 0; last[k] = 0;
     py[k] = (float)(y0 + k) + 0.5f;
-    if (x >= prm.W || y0 + k >= prm.H) done |= 1u << k;
+    if (x >= prm.W || y0 + k >= prm.H) { py[k] = INFINITY; ++ndone; }
   }
   uint32_t walked = 0, cend = 0;
   uint32_t pos = range.x, qn = 0;
   int e_base = 0;
-  bool finished = __all_sync(FULL, done == 0xffu);
+  bool finished = __all_sync(FULL, ndone == PPL);
   while (!finished) {
     // fill the queue with the next entries of the supertile list that can contribute to this tile
     while (qn < 32u && pos < range.y) {
@@ -162,7 +175,7 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
         const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
         const float a = mul_rn(s1.y, exp_spec(power));       // garbage outside [tau, 0]: masked by `pass`
         // s1.w = tau >= -6 is a pre-test that never decides (project.cu); the alpha test does (R-4, R-5)
-        const bool pass = power <= 0.0f && power >= s1.w && a >= prm.alpha_min && !((done >> k) & 1u);
+        const bool pass = power <= 0.0f && power >= s1.w && a >= prm.alpha_min;
         const float alpha = fminf(a, prm.alpha_max);
         const float Tn = mul_rn(T[k], sub_rn(1.0f, alpha));
         const bool stop = Tn < prm.t_stop;                   // stop BEFORE compositing (R-4)
@@ -175,11 +188,11 @@ __global__ void __launch_bounds__(32) forward_kernel(const Splat* __restrict__ s
         }
         T[k] = comp ? Tn : T[k];
         last[k] = comp ? e1 : last[k];
-        if (pass && stop) done |= 1u << k;
+        if (pass && stop) { py[k] = INFINITY; ++ndone; }
         anycomp = anycomp || comp;
       }
       if (anycomp) cend = __float_as_uint(s2.w);               // coarse position + 1 of the last composited entry
-      if (__all_sync(FULL, done == 0xffu)) { finished = true; break; }
+      if (__all_sync(FULL, ndone == PPL)) { finished = true; break; }
     }
     e_base += (int)cnt;
     shift_queue(q_rank, q_cpos, qn, cnt);
@@ -227,59 +240,74 @@ __device__ __forceinline__ float rcp_approx(float x) {
   return y;
 }
 
-// Sum v[0..39] over the 32 lanes.  On return lane l holds the totals of moments idx0 and idx1 (or -1).
-// 40 shuffles instead of 200: at every level a lane keeps one half of its values and sends the other half.
-__device__ __forceinline__ void butterfly40(const float (&v)[NMOM], int lane, float& o0, float& o1, int& idx0, int& idx1) {
-  float a20[20], a10[10], a5[5], a3[3];
-  bool up = (lane & 16) != 0;
+// Cross-lane reduction of the 40 moments through shared memory: every lane stores its 40 values as one row of a
+// 32 x 44 array (row stride 44 words: the float4 stores and loads below are bank-conflict free up to one 2-way phase);
+// lane l < 30 then sums the float4 column q = l % 10 over the rows r = l / 10, l / 10 + 3, ... and two shuffles fold
+// the three row groups, leaving the totals of moments 4q .. 4q+3 in lane q < 10.  ~90 instructions per entry, none of
+// them on the half-rate select pipe, against ~160 for a register butterfly.
+constexpr int RED_STRIDE = 44;
+
+__device__ __forceinline__ float4 reduce40(const float (&v)[NMOM], float* red, int lane) {
+  float4* row = reinterpret_cast<float4*>(red + lane * RED_STRIDE);
 #pragma unroll
-  for (int i = 0; i < 20; ++i) {
-    const float keep = up ? v[20 + i] : v[i], send = up ? v[i] : v[20 + i];
-    a20[i] = keep + __shfl_xor_sync(FULL, send, 16);
-  }
-  up = (lane & 8) != 0;
+  for (int q = 0; q < NMOM / 4; ++q) row[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+  __syncwarp();
+  const int q = lane % 10, rg = lane / 10;
+  float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+  if (lane < 30) {
+    const float* col = red + 4 * q;
 #pragma unroll
-  for (int i = 0; i < 10; ++i) {
-    const float keep = up ? a20[10 + i] : a20[i], send = up ? a20[i] : a20[10 + i];
-    a10[i] = keep + __shfl_xor_sync(FULL, send, 8);
+    for (int i = 0; i < 10; i += 2) {
+      const float4 x = *reinterpret_cast<const float4*>(col + (rg + 3 * i) * RED_STRIDE);
+      const float4 y = *reinterpret_cast<const float4*>(col + (rg + 3 * i + 3) * RED_STRIDE);
+      a.x += x.x; a.y += x.y; a.z += x.z; a.w += x.w;
+      b.x += y.x; b.y += y.y; b.z += y.z; b.w += y.w;
+    }
+    if (rg < 2) {                                    // rows 30 and 31
+      const float4 x = *reinterpret_cast<const float4*>(col + (rg + 30) * RED_STRIDE);
+      a.x += x.x; a.y += x.y; a.z += x.z; a.w += x.w;
+    }
   }
-  up = (lane & 4) != 0;
-#pragma unroll
-  for (int i = 0; i < 5; ++i) {
-    const float keep = up ? a10[5 + i] : a10[i], send = up ? a10[i] : a10[5 + i];
-    a5[i] = keep + __shfl_xor_sync(FULL, send, 4);
-  }
-  up = (lane & 2) != 0;
-#pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    const float hi = (i < 2) ? a5[3 + i] : 0.0f;     // 5 -> 3 + 3 (one pad)
-    const float keep = up ? hi : a5[i], send = up ? a5[i] : hi;
-    a3[i] = keep + __shfl_xor_sync(FULL, send, 2);
-  }
-  up = (lane & 1) != 0;
-  {
-    const float keep0 = up ? a3[2] : a3[0], send0 = up ? a3[0] : a3[2];
-    const float keep1 = up ? 0.0f : a3[1], send1 = up ? a3[1] : 0.0f;   // 3 -> 2 + 2 (one pad)
-    o0 = keep0 + __shfl_xor_sync(FULL, send0, 1);
-    o1 = keep1 + __shfl_xor_sync(FULL, send1, 1);
-  }
-  const int b16 = (lane >> 4) & 1, b8 = (lane >> 3) & 1, b4 = (lane >> 2) & 1, b2 = (lane >> 1) & 1, b1 = lane & 1;
-  const int basei = 20 * b16 + 10 * b8 + 5 * b4 + 3 * b2;
-  const int s0 = 2 * b1, s1 = 2 * b1 + 1;
-  idx0 = (s0 < 3 && 3 * b2 + s0 < 5) ? basei + s0 : -1;
-  idx1 = (s1 < 3 && 3 * b2 + s1 < 5) ? basei + s1 : -1;
+  __syncwarp();                                      // the rows may be overwritten by the next entry
+  a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
+  float4 t;
+  t.x = __shfl_down_sync(FULL, a.x, 10); t.y = __shfl_down_sync(FULL, a.y, 10);
+  t.z = __shfl_down_sync(FULL, a.z, 10); t.w = __shfl_down_sync(FULL, a.w, 10);
+  float4 u;
+  u.x = __shfl_down_sync(FULL, a.x, 20); u.y = __shfl_down_sync(FULL, a.y, 20);
+  u.z = __shfl_down_sync(FULL, a.z, 20); u.w = __shfl_down_sync(FULL, a.w, 20);
+  a.x += t.x + u.x; a.y += t.y + u.y; a.z += t.z + u.z; a.w += t.w + u.w;
+  return a;                                          // valid in lanes 0..9
+}
+
+// 16-byte vector reductions into the L2 (sm_90+): one request per four moments
+__device__ __forceinline__ void red_add_v4(float* dst, const float4& v) {
+  asm volatile("red.global.v4.f32.add [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ float4 atom_add_v4(float* dst, const float4& v) {
+  float4 o;
+  asm volatile("atom.global.v4.f32.add {%0, %1, %2, %3}, [%4], {%5, %6, %7, %8};"
+               : "=f"(o.x), "=f"(o.y), "=f"(o.z), "=f"(o.w)
+               : "l"(dst), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w)
+               : "memory");
+  return o;
 }
 
 template <int NCH>
-__global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ ckeys,
-                                                       const ushort4* __restrict__ crect, const uint2* __restrict__ cranges,
-                                                       const uint32_t* __restrict__ tile_cend, RasterParams prm, PixelBuf pix,
-                                                       float* __restrict__ moments, uint32_t* __restrict__ touched,
-                                                       ViewCounters* counters) {
+__global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
+  const RasterView& vw = batch.v[blockIdx.y];
+  const Splat* __restrict__ splat_sorted = vw.splat_sorted;
+  const uint32_t* __restrict__ ckeys = vw.ckeys;
+  const ushort4* __restrict__ crect = vw.crect;
+  const uint2* __restrict__ cranges = vw.cranges;
+  const uint32_t* __restrict__ tile_cend = vw.tile_cend;
+  const PixelBuf pix = vw.pix;
+  float* __restrict__ moments = vw.moments;
   __shared__ float4 sm[32 * 3];
-  __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22, -) of Sigma2D = L L^T
+  __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
+  __shared__ __align__(16) float red[32 * RED_STRIDE];
   __shared__ uint32_t q_rank[64];
-  const int tile = blockIdx.x, lane = threadIdx.x;
+  const int tile = batch.tile_order[blockIdx.x], lane = threadIdx.x;   // heaviest tiles first (launch order)
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -299,7 +327,8 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
       last[k] = pix.last[p];
       Tc[k] = pix.T[p];
     }
-    S0[k] = prm.bg[0] * Tc[k]; S1[k] = prm.bg[1] * Tc[k]; S2[k] = prm.bg[2] * Tc[k]; S3[k] = 0.0f;
+    // suffix sums are carried pre-scaled by sqrt(omega_ch) (see pass 2)
+    S0[k] = prm.somega[0] * prm.bg[0] * Tc[k]; S1[k] = prm.somega[1] * prm.bg[1] * Tc[k]; S2[k] = prm.somega[2] * prm.bg[2] * Tc[k]; S3[k] = 0.0f;
     maxlast = max(maxlast, last[k]);
   }
 #pragma unroll
@@ -343,38 +372,48 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
       const float4 q0 = sm[lane * 3], q1 = sm[lane * 3 + 1];
       const float cA = -2.0f * q0.z, cB = -q0.w, cC = -2.0f * q1.x;
       const float icC = 1.0f / cC;
-      sm_wh[lane] = make_float4(sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), -cB * icC, sqrtf(cC), 0.0f);
+      sm_wh[lane] = make_float4(sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), -cB * icC, sqrtf(cC), __logf(prm.alpha_min / q1.y));
     }
     __syncwarp();
     for (int j = 0; j < cnt; ++j) {
       const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
       const int e = e_next - j;
       const float dx = sub_rn(px, s0.x);
-      // pass 1 (decision path): power bit-identical to S3; alpha from the fast exp.  Wherever alpha comes within
-      // 8e-6 (relative) of a threshold of R-4 the exact exp_spec value is substituted below, so every decision
-      // (contributor or not, clamped or not) is the one S3 took; elsewhere the two exps agree to < 1e-6 relative.
-      float av[PPL];
+      // pass 1 (decision path): power bit-identical to S3; alpha from the fast exp (MUFU.EX2).  The two exps agree to
+      // < 1e-6 relative, so they can only disagree on a decision of R-4 (contributor or not, clamped or not) when
+      // sigma exp(power) lies within ~1e-6 (relative) of alpha_min or alpha_max, i.e. when `power` lies within ~1e-6
+      // of P_min = ln(alpha_min / sigma) or P_max = ln(alpha_max / sigma).  If any pixel of the tile comes within 2e-5
+      // of either, the whole entry is evaluated with exp_spec instead, so every decision is the one S3 took.  The test
+      // reads only `power`: the MUFU results are first needed in pass 2, where 8 independent chains hide their latency.
+      const float4 wh = sm_wh[j];
+      const float Pmin = wh.w, Pmax = wh.w + prm.ln_amax_over_amin;
+      float pw[PPL], av[PPL];
       unsigned inr = 0;
       bool near = false;
 #pragma unroll
       for (int k = 0; k < PPL; ++k) {
         const float dy = sub_rn(py[k], s0.y);
         const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
-        const float a = s1.y * ex2_approx(power * 0x1.715476p+0f);
         const bool in = e < last[k] && power <= 0.0f && power >= s1.w;
-        av[k] = a;
+        pw[k] = power;
         inr |= in ? (1u << k) : 0u;
-        near = near || (in && (fabsf(a - prm.alpha_min) <= 8e-6f * prm.alpha_min || fabsf(a - prm.alpha_max) <= 8e-6f * prm.alpha_max));
+        near |= in & ((fabsf(power - Pmin) <= 2e-5f) | (fabsf(power - Pmax) <= 2e-5f));    // bitwise: no branches
       }
       if (__any_sync(FULL, near)) {
 #pragma unroll
-        for (int k = 0; k < PPL; ++k) {
-          const float dy = sub_rn(py[k], s0.y);
-          av[k] = mul_rn(s1.y, exp_spec(splat_power(s0.z, s0.w, s1.x, dx, dy)));
-        }
+        for (int k = 0; k < PPL; ++k) av[k] = mul_rn(s1.y, exp_spec(pw[k]));
+      } else {
+#pragma unroll
+        for (int k = 0; k < PPL; ++k) av[k] = s1.y * ex2_approx(pw[k] * 0x1.715476p+0f);
       }
       // pass 2 (value path): beta, suffix sums, and the sums  F_p = sum_k f_k t_k^p,  G_c,p = sum_k g_c,k t_k^p  over
-      // the lane's 8 pixels with t_k = k - 3.5 a compile-time constant (dy_k = dyc + t_k)
+      // the lane's 8 pixels with t_k = k - 3.5 a compile-time constant (dy_k = dyc + t_k).
+      // With T_i = T_{i+1} / (1 - alpha_i) =: Tc * rc,   beta_ch = dy_ch/dalpha_i = T_i v_i - Splus_i / (1 - alpha_i)
+      // = rc * d_ch,  d_ch = Tc v_ch - Splus_ch.  The channel weight enters as sqrt(omega_ch) folded into v_ch and
+      // Splus_ch (both linear), so  sum_ch omega_ch beta_ch^2 = rc^2 sum_ch d_ch^2  and the cross moments come out
+      // scaled by sqrt(omega_ch) (S5 applies the other sqrt).
+      const float v0 = prm.somega[0] * s2.x, v1 = prm.somega[1] * s2.y, v2 = prm.somega[2] * s2.z;
+      const float v3 = NCH == 4 ? prm.somega[3] * s1.z : 0.0f;
       float F0 = 0.f, F1 = 0.f, F2 = 0.f, F3 = 0.f, F4 = 0.f, W2 = 0.f;
       float G[NCH][3];
 #pragma unroll
@@ -387,29 +426,28 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
         const bool active = pass && !(a > prm.alpha_max);                // R-11: zero derivative at the 0.99 cap
         const float alpha = fminf(a, prm.alpha_max);
         const float rc = rcp_approx(1.0f - alpha);
-        const float Ti = Tc[k] * rc;                                     // T_i = T_{i+1} / (1 - alpha_i)
+        const float Ti = Tc[k] * rc;
         const float w = alpha * Ti;
-        // beta_ch = dy_ch/dalpha_i = T_i v_i - Splus_i / (1 - alpha_i)
-        const float b0 = Ti * s2.x - S0[k] * rc, b1 = Ti * s2.y - S1[k] * rc, b2 = Ti * s2.z - S2[k] * rc;
-        float b3 = 0.0f;
-        if (NCH == 4) b3 = Ti * s1.z - S3[k] * rc;
+        const float d0 = fmaf(Tc[k], v0, -S0[k]), d1 = fmaf(Tc[k], v1, -S1[k]), d2 = fmaf(Tc[k], v2, -S2[k]);
+        float d3 = 0.0f;
+        if (NCH == 4) d3 = fmaf(Tc[k], v3, -S3[k]);
         const float wm = pass ? w : 0.0f;
-        S0[k] = fmaf(s2.x, wm, S0[k]); S1[k] = fmaf(s2.y, wm, S1[k]); S2[k] = fmaf(s2.z, wm, S2[k]);
-        if (NCH == 4) S3[k] = fmaf(s1.z, wm, S3[k]);
+        S0[k] = fmaf(v0, wm, S0[k]); S1[k] = fmaf(v1, wm, S1[k]); S2[k] = fmaf(v2, wm, S2[k]);
+        if (NCH == 4) S3[k] = fmaf(v3, wm, S3[k]);
         Tc[k] = pass ? Ti : Tc[k];
         W2 = fmaf(wm, wm, W2);
-        float Bq = prm.omega[0] * b0 * b0 + prm.omega[1] * b1 * b1 + prm.omega[2] * b2 * b2;
-        if (NCH == 4) Bq = fmaf(prm.omega[3] * b3, b3, Bq);
-        const float aa = active ? alpha : 0.0f;
-        const float f = Bq * aa * aa;
-        const float wa = w * aa;
+        float Dq = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
+        if (NCH == 4) Dq = fmaf(d3, d3, Dq);
+        const float r1 = active ? rc * alpha : 0.0f;                     // rc * alpha, zero when inactive
+        const float f = Dq * r1 * r1;                                    // (sum_ch omega beta^2) alpha^2
+        const float gw = w * r1;                                         // beta_ch w alpha = d_ch * gw
         const float t1 = (float)k - 3.5f, t2 = t1 * t1, t3 = t2 * t1, t4 = t2 * t2;
         F0 += f; F1 = fmaf(f, t1, F1); F2 = fmaf(f, t2, F2); F3 = fmaf(f, t3, F3); F4 = fmaf(f, t4, F4);
-        const float bch[4] = {b0, b1, b2, b3};
+        const float dch[4] = {d0, d1, d2, d3};
+        const float gw1 = gw * t1, gw2 = gw * t2;
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
-          const float g = bch[c] * wa;
-          G[c][0] += g; G[c][1] = fmaf(g, t1, G[c][1]); G[c][2] = fmaf(g, t2, G[c][2]);
+          G[c][0] = fmaf(dch[c], gw, G[c][0]); G[c][1] = fmaf(dch[c], gw1, G[c][1]); G[c][2] = fmaf(dch[c], gw2, G[c][2]);
         }
         any = any || pass;
       }
@@ -420,7 +458,6 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
         // (The shear keeps the column structure; the whitening keeps the later change to the u basis free of the
         // cancellation a plain pixel-offset basis has for elongated footprints.  DESIGN.md section 6.)
         float acc[NMOM];
-        const float4 wh = sm_wh[j];
         const float x1 = dx * wh.x;
         const float h = wh.z, h2 = h * h;
         const float c1 = (((py[0] + 3.5f) - s0.y) - wh.y * dx) * h, c2 = c1 * c1, c3 = c2 * c1, c4 = c2 * c2;
@@ -450,20 +487,12 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
           }
         }
         acc[MOM_W2] = W2;
-        float o0, o1;
-        int i0, i1;
-        butterfly40(acc, lane, o0, o1, i0, i1);
+        const float4 tot = reduce40(acc, red, lane);
         const uint32_t rank = q_rank[j];
-        float* dst = moments + (size_t)rank * NMOM;
-        if (i0 >= 0) atomicAdd(dst + i0, o0);
-        if (i1 >= 0) {
-          if (i1 == MOM_W2) {
-            // sum w^2 > 0 for every touched Gaussian: the first adder (old value 0) appends it to the touched list
-            if (atomicAdd(dst + i1, o1) == 0.0f) touched[atomicAdd(&counters->n_touched, 1u)] = rank;
-          } else {
-            atomicAdd(dst + i1, o1);
-          }
-        }
+        float* dst = moments + (size_t)rank * NMOM + 4 * lane;
+        // no returning atomic here: a returned value would tie up a scoreboard for a full L2 round trip; the touched
+        // list is built afterwards from sum w^2 != 0 (touched_kernel)
+        if (lane < 10) red_add_v4(dst, tot);
       }
     }
     e_next -= cnt;
@@ -471,37 +500,57 @@ __global__ void __launch_bounds__(32) backward_kernel(const Splat* __restrict__ 
   }
 }
 
+// Touched list of every view of the batch: the ranks whose sum w^2 (moment 39) is non-zero, i.e. the Gaussians with at
+// least one composited pixel.  Warp-aggregated append; the order is not specified.
+__global__ void __launch_bounds__(256) touched_kernel(const __grid_constant__ RasterBatch batch, int N) {
+  const RasterView& vw = batch.v[blockIdx.y];
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool hit = r < N && vw.moments[(size_t)r * NMOM + MOM_W2] != 0.0f;
+  const unsigned m = __ballot_sync(FULL, hit);
+  if (m == 0u) return;
+  const int lane = threadIdx.x & 31;
+  uint32_t base = 0;
+  if (lane == 0) base = atomicAdd(&vw.counters->n_touched, (uint32_t)__popc(m));
+  base = __shfl_sync(FULL, base, 0);
+  if (hit) vw.touched[base + __popc(m & ((1u << lane) - 1u))] = (uint32_t)r;
+}
+
 static RasterParams make_params(const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg) {
   RasterParams p;
   p.W = W; p.H = H; p.tiles_x = tg.tiles_x; p.rank_bits = rank_bits;
   p.sshift = tg.sshift; p.super_x = tg.super_x;
   p.alpha_min = cfg.alpha_min; p.alpha_max = cfg.alpha_max; p.t_stop = cfg.t_stop;
+  p.ln_amax_over_amin = logf(cfg.alpha_max / cfg.alpha_min);
   for (int c = 0; c < 3; ++c) p.bg[c] = cfg.bg[c];
-  for (int c = 0; c < 4; ++c) p.omega[c] = ((cfg.channel_mask >> c) & 1) ? cfg.channel_weight[c] : 0.0f;
+  for (int c = 0; c < 4; ++c) {
+    p.omega[c] = ((cfg.channel_mask >> c) & 1) ? cfg.channel_weight[c] : 0.0f;
+    p.somega[c] = sqrtf(p.omega[c]);
+  }
   return p;
 }
 
-void launch_forward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
-                    int rank_bits, int W, int H, const nbv_config& cfg, PixelBuf px, uint32_t* tile_cend, uint32_t* tile_walk,
-                    ViewCounters* counters, cudaStream_t st) {
+void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg, bool full_pix,
+                    cudaStream_t st) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
+  const dim3 grid((unsigned)(tg.tiles_x * tg.tiles_y), (unsigned)batch.n);
   ++g_kernel_launches;
-  if (px.rgb)
-    forward_kernel<true><<<tg.tiles_x * tg.tiles_y, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, p, px, tile_cend, tile_walk, counters);
+  if (full_pix)
+    forward_kernel<true><<<grid, 32, 0, st>>>(batch, p);
   else
-    forward_kernel<false><<<tg.tiles_x * tg.tiles_y, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, p, px, tile_cend, tile_walk, counters);
+    forward_kernel<false><<<grid, 32, 0, st>>>(batch, p);
 }
 
-void launch_backward(const Splat* splat_sorted, const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg,
-                     int rank_bits, int W, int H, const nbv_config& cfg, PixelBuf px, const uint32_t* tile_cend, float* moments,
-                     uint32_t* touched, ViewCounters* counters, cudaStream_t st) {
+void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
+                     cudaStream_t st) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
-  const int tiles = tg.tiles_x * tg.tiles_y;
+  const dim3 grid((unsigned)(tg.tiles_x * tg.tiles_y), (unsigned)batch.n);
   ++g_kernel_launches;
   if (cfg.channel_mask & NBV_CH_DEPTH)
-    backward_kernel<4><<<tiles, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, tile_cend, p, px, moments, touched, counters);
+    backward_kernel<4><<<grid, 32, 0, st>>>(batch, p);
   else
-    backward_kernel<3><<<tiles, 32, 0, st>>>(splat_sorted, ckeys, crect, cranges, tile_cend, p, px, moments, touched, counters);
+    backward_kernel<3><<<grid, 32, 0, st>>>(batch, p);
+  ++g_kernel_launches;
+  touched_kernel<<<dim3((unsigned)((N + 255) / 256), (unsigned)batch.n), 256, 0, st>>>(batch, N);
 }
 
 }  // namespace nbv
