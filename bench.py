@@ -180,6 +180,28 @@ def workload_config(args, wl, where: str):
 
 
 # --------------------------------------------------------------------------------------------------
+def rank_candidates(cfg_index: int, wl, rank: int):
+    """Candidate cameras rank `rank` scores: rank 0 keeps the workload's own set; every other replica draws its own set
+    of the same size from a rank-seeded generator (same scene, same hemisphere recipe) -- independent units, no exchange."""
+    if rank == 0:
+        return wl.cand_cams
+    from paper_2602_08266_b200 import synth
+    c = synth.CONFIGS[cfg_index]
+    f = synth._intrinsics(c)
+    return synth.hemisphere_cameras(c["C"], c["radius"], c["W"], c["H"], f, f, np.random.default_rng(10_000 + rank))
+
+
+def gather_over_ranks(per_step, dist, device):
+    """(ranks, steps) array of every rank's per-step times; `dist` is torch.distributed or None (single process)."""
+    import torch
+    t = torch.tensor([list(per_step)], dtype=torch.float64, device=device)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        parts = [torch.zeros_like(t) for _ in range(dist.get_world_size())]
+        dist.all_gather(parts, t)
+        t = torch.cat(parts)
+    return t.cpu().numpy()
+
+
 def aggregate(step_ms_per_rank, views_per_rank_step):
     """Whole-job throughput: units of all ranks / slowest rank's time.  step_ms_per_rank: (ranks, steps)."""
     t = np.asarray(step_ms_per_rank, dtype=np.float64)
@@ -208,10 +230,7 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    if rank > 0:   # replicas score their own candidate sets (same scene): rank-seeded cameras
-        c = synth.CONFIGS[args.config]
-        f = synth._intrinsics(c)
-        wl.cand_cams = synth.hemisphere_cameras(c["C"], c["radius"], c["W"], c["H"], f, f, np.random.default_rng(10_000 + rank))
+    wl.cand_cams = rank_candidates(args.config, wl, rank)   # replicas score their own candidate sets
 
     nbv = api.NBV(channel_mask=wl.channel_mask)
     if args.concurrency:
@@ -285,16 +304,10 @@ def main():
             tot[k] += st[k]
 
     # ---- gather over ranks ----
-    t_all = torch.tensor([step_ms], dtype=torch.float64, device="cuda")
-    e_all = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        tl = [torch.zeros_like(t_all) for _ in range(world)]
-        el = [torch.zeros_like(e_all) for _ in range(world)]
-        dist.all_gather(tl, t_all)
-        dist.all_gather(el, e_all)
-        t_all, e_all = torch.cat(tl), torch.cat(el)
-    agg = aggregate(t_all.cpu().numpy(), C)
-    agg_e2e = aggregate(e_all.cpu().numpy() * 1e3, C)
+    t_all = gather_over_ranks(step_ms, dist, "cuda")
+    e_all = gather_over_ranks(e2e_s, dist, "cuda")
+    agg = aggregate(t_all, C)
+    agg_e2e = aggregate(e_all * 1e3, C)
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
