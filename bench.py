@@ -44,6 +44,10 @@ FLOP_TEST = 11            # (pixel, list entry) evaluated: dx, dy, power, two ra
 FLOP_FWD_PAIR = 31        # composited pair, S3: exp, alpha, T update, 4 blended channels
 FLOP_BWD_PAIR = {3: 134, 4: 154}   # composited pair, S4: exp, beta, 34 / 40 moment updates
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
+VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (grid.y = view)
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture
+# (profiles/r1b_ncu_raster_cfg2.md); known for config 2 only
+NCU_TRAFFIC_BYTES = {2: {"backward": 99.1e6, "forward": 37.7e6}}
 
 
 def parse_args():
@@ -329,14 +333,17 @@ def main():
     for k, (bound, amount, peak, unit) in work.items():
         sec = per_view_ms[k] * 1e-3
         ach = amount / sec if sec > 0 else 0.0
-        rl[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak, "traffic": None,
-                 "ms_per_launch": per_view_ms[k], "peak_source": peaks["source"] if bound == "hbm" else
+        batched = k in ("backward", "forward")
+        rl[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
+                 "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(k),
+                 "views_per_launch": VIEWS_PER_LAUNCH if batched else 1,
+                 "ms_per_launch": per_view_ms[k] * (VIEWS_PER_LAUNCH if batched else 1), "peak_source": peaks["source"] if bound == "hbm" else
                  "148 SM x 128 lanes x 2 x %.0f MHz (DESIGN.md section 8)" % peaks["sm_max_mhz"]}
     dominant = max(work, key=lambda k: per_view_ms[k])
     roofline = dict(rl[dominant], kernel=dominant)
     # whole-view bound: sum over stages of the stage's own lower bound
     t_min_ms = sum(1e3 * work[k][1] / work[k][2] for k in work)
-    view_ms = sum(per_view_ms.values())
+    view_ms = agg["ms_per_step"] / C                    # wall time per view (stages of different views overlap)
 
     out = {
         "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -349,7 +356,8 @@ def main():
         "roofline": roofline,
         "stage_ms_per_view": per_view_ms,
         "stage_rooflines": rl,
-        "view_roofline": {"t_min_ms": t_min_ms, "t_measured_ms": view_ms, "frac": t_min_ms / view_ms if view_ms else None},
+        "view_roofline": {"t_min_ms": t_min_ms, "t_measured_ms": view_ms, "frac": t_min_ms / view_ms if view_ms else None,
+                          "note": "sum over stages of (algorithmic work / peak) against wall time per view"},
         "counts_per_view": avg,
         "setup": {"load_s": load_s, "training_views_per_s": len(wl.train_cams) / (train_ms * 1e-3) if train_ms else None},
         "best": int(h_best),
