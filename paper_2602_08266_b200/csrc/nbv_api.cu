@@ -66,6 +66,7 @@ struct nbv_ctx {
   int concurrency = MAX_BATCH;
   cudaEvent_t ev_fork = nullptr;
   cudaEvent_t ev_set_done[2] = {nullptr, nullptr};   // S3-S6 of the last batch that used slot set 0 / 1
+  cudaStream_t raster_st[2] = {nullptr, nullptr};    // S3-S6 of the batches of slot set 0 / 1 (forked from / joined into the caller's stream)
   ViewSlot* last_slot = nullptr;        // slot of the last view processed (nbv_last_view_stats)
   DevBuf tile_order;                    // centre-out launch order of the tiles of a tile_order_tx x tile_order_ty grid
   int tile_order_tx = 0, tile_order_ty = 0;
@@ -221,7 +222,12 @@ void free_slot(ViewSlot* sl) {
 int get_slot(nbv_ctx* ctx, int i, ViewSlot** out) {
   while ((int)ctx->slots.size() <= i) {
     ViewSlot* sl = new ViewSlot;
-    bool ok = cudaStreamCreateWithFlags(&sl->st, cudaStreamNonBlocking) == cudaSuccess &&
+    // Highest stream priority: the work distributor hands out the blocks of a queued kernel only after every earlier
+    // kernel of the same priority has dispatched all of its blocks, so without it the ~30 small S1-S2 launches of the next
+    // batch would sit behind the 28,800 blocks of the running raster launch instead of slipping in between them.
+    int prio_least = 0, prio_greatest = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest);
+    bool ok = cudaStreamCreateWithPriority(&sl->st, cudaStreamNonBlocking, prio_greatest) == cudaSuccess &&
               cudaEventCreateWithFlags(&sl->done, cudaEventDisableTiming) == cudaSuccess &&
               cudaMalloc(&sl->d_counters, sizeof(ViewCounters)) == cudaSuccess &&
               cudaMallocHost(&sl->h_counters, sizeof(ViewCounters)) == cudaSuccess;
@@ -356,7 +362,7 @@ int ensure_tile_order(nbv_ctx* ctx, const TileGrid& tg, cudaStream_t st) {
   const double cx = 0.5 * (tg.tiles_x - 1), cy = 0.5 * (tg.tiles_y - 1);
   auto d2 = [&](uint32_t t) { const double dx = (int)(t % tg.tiles_x) - cx, dy = (int)(t / tg.tiles_x) - cy; return dx * dx + dy * dy; };
   std::stable_sort(order.begin(), order.end(), [&](uint32_t a, uint32_t b) { return d2(a) < d2(b); });
-  CK(cudaStreamSynchronize(st));        // a launch reading the previous table may still be queued
+  CK(cudaDeviceSynchronize());          // a launch reading the previous table may still be queued (on either raster stream)
   CKRET(ensure(ctx, ctx->tile_order, 4 * (size_t)n));
   CK(cudaMemcpyAsync(ctx->tile_order.p, order.data(), 4 * (size_t)n, cudaMemcpyHostToDevice, st));
   CK(cudaStreamSynchronize(st));        // `order` is a pageable host buffer about to go out of scope
@@ -434,6 +440,7 @@ int expand_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int mode, flo
 int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_scores, cudaStream_t st) {
   const int V = std::max(1, std::min(ctx->concurrency, MAX_BATCH));
   CK(cudaEventRecord(ctx->ev_fork, st));
+  for (int s = 0; s < 2; ++s) CK(cudaStreamWaitEvent(ctx->raster_st[s], ctx->ev_fork, 0));
   int rc = NBV_OK;
   int batch_no = 0;
   bool set_used[2] = {false, false};
@@ -441,25 +448,29 @@ int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_
     int nb = 1;
     while (nb < V && i0 + nb < n && h_cams[i0 + nb].width == h_cams[i0].width && h_cams[i0 + nb].height == h_cams[i0].height) ++nb;
     const int set = batch_no & 1;
+    // Consecutive batches raster on two different streams: the forward launch of batch b+1 fills the SMs that the
+    // draining backward launch of batch b leaves idle (a launch of 28,800 one-warp blocks that each run for hundreds of
+    // microseconds has a tail of about one block duration).  Batch b+2 follows batch b in stream order, which is also
+    // what the reuse of the slot set requires.
+    cudaStream_t rs = ctx->raster_st[set];
     ViewSlot* sl[MAX_BATCH];
     for (int i = 0; i < nb && rc == NBV_OK; ++i) rc = get_slot(ctx, set * MAX_BATCH + i, &sl[i]);
     if (rc != NBV_OK) break;
-    int started = 0;
     for (int i = 0; i < nb; ++i) {
       // the slot's buffers are free once the S3-S6 launches of the batch that last used this set have finished
       cudaStreamWaitEvent(sl[i]->st, set_used[set] ? ctx->ev_set_done[set] : ctx->ev_fork, 0);
       if (rc == NBV_OK) rc = pre_view(ctx, sl[i], h_cams[i0 + i], STAGE_BACKWARD, false, false, sl[i]->st);
       cudaEventRecord(sl[i]->done, sl[i]->st);
-      cudaStreamWaitEvent(st, sl[i]->done, 0);      // join even after an error: the caller's stream must not run ahead
-      ++started;
+      cudaStreamWaitEvent(rs, sl[i]->done, 0);      // join even after an error: no stream may run ahead
     }
-    (void)started;
-    if (rc == NBV_OK) rc = raster_batch(ctx, sl, h_cams + i0, nb, STAGE_BACKWARD, false, st);
-    if (rc == NBV_OK) rc = expand_batch(ctx, sl, h_cams + i0, nb, mode, nullptr, d_scores ? d_scores + i0 : nullptr, nullptr, st);
-    cudaEventRecord(ctx->ev_set_done[set], st);
+    if (rc == NBV_OK) rc = raster_batch(ctx, sl, h_cams + i0, nb, STAGE_BACKWARD, false, rs);
+    if (rc == NBV_OK) rc = expand_batch(ctx, sl, h_cams + i0, nb, mode, nullptr, d_scores ? d_scores + i0 : nullptr, nullptr, rs);
+    cudaEventRecord(ctx->ev_set_done[set], rs);
     set_used[set] = true;
     i0 += nb;
   }
+  for (int s = 0; s < 2; ++s)
+    if (set_used[s]) cudaStreamWaitEvent(st, ctx->ev_set_done[s], 0);
   return rc;
 }
 
@@ -537,7 +548,9 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
   ViewSlot* s0 = nullptr;
   if (cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&ctx->ev_set_done[0], cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&ctx->ev_set_done[1], cudaEventDisableTiming) != cudaSuccess || get_slot(ctx, 0, &s0) != NBV_OK) {
+      cudaEventCreateWithFlags(&ctx->ev_set_done[1], cudaEventDisableTiming) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&ctx->raster_st[0], cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&ctx->raster_st[1], cudaStreamNonBlocking) != cudaSuccess || get_slot(ctx, 0, &s0) != NBV_OK) {
     cudaGetLastError();
     nbv_destroy(ctx);
     return NBV_ERR_CUDA;
@@ -559,6 +572,7 @@ void nbv_destroy(nbv_ctx* ctx) {
   for (ViewSlot* sl : ctx->slots) free_slot(sl);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
   for (cudaEvent_t e : ctx->ev_set_done) if (e) cudaEventDestroy(e);
+  for (cudaStream_t r : ctx->raster_st) if (r) cudaStreamDestroy(r);
   for (const Span& sp : ctx->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   cudaGetLastError();
   delete ctx;

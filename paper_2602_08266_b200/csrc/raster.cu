@@ -98,8 +98,12 @@ __device__ __forceinline__ void shift_queue(uint32_t* q_rank, uint32_t* q_cpos, 
 // The slot body is branch-free (predicated updates): the 8 pixels of a lane are 8 independent dependency chains the
 // scheduler can interleave, and after the ellipse test nearly every staged entry touches nearly every slot anyway.
 template <bool FULLPIX>
-__global__ void __launch_bounds__(32) forward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
-  const RasterView& vw = batch.v[blockIdx.y];          // one launch rasterises every view of the batch
+__global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
+  // One launch rasterises every view of the batch.  Launch position -> (view, tile): the views are
+  // interleaved, so the launch starts with the central (long-running) tiles of ALL views and its tail is made of the
+  // edge tiles of all views.
+  const int bpos = blockIdx.x, vidx = bpos % batch.n;
+  const RasterView& vw = batch.v[vidx];
   const Splat* __restrict__ splat_sorted = vw.splat_sorted;
   const uint32_t* __restrict__ ckeys = vw.ckeys;
   const ushort4* __restrict__ crect = vw.crect;
@@ -110,7 +114,7 @@ __global__ void __launch_bounds__(32) forward_kernel(const __grid_constant__ Ras
   ViewCounters* counters = vw.counters;
   __shared__ float4 sm[32 * 3];
   __shared__ uint32_t q_rank[64], q_cpos[64];
-  const int tile = batch.tile_order[blockIdx.x], lane = threadIdx.x;   // heaviest tiles first (launch order)
+  const int tile = batch.tile_order[bpos / batch.n], lane = threadIdx.x;   // heaviest tiles first (launch order)
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -295,7 +299,8 @@ __device__ __forceinline__ float4 atom_add_v4(float* dst, const float4& v) {
 
 template <int NCH>
 __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
-  const RasterView& vw = batch.v[blockIdx.y];
+  const int bpos = blockIdx.x, vidx = bpos % batch.n;       // views interleaved (see forward_kernel)
+  const RasterView& vw = batch.v[vidx];
   const Splat* __restrict__ splat_sorted = vw.splat_sorted;
   const uint32_t* __restrict__ ckeys = vw.ckeys;
   const ushort4* __restrict__ crect = vw.crect;
@@ -307,7 +312,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
   __shared__ __align__(16) float red[32 * RED_STRIDE];
   __shared__ uint32_t q_rank[64];
-  const int tile = batch.tile_order[blockIdx.x], lane = threadIdx.x;   // heaviest tiles first (launch order)
+  const int tile = batch.tile_order[bpos / batch.n], lane = threadIdx.x;   // heaviest tiles first (launch order)
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -386,18 +391,20 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       // of either, the whole entry is evaluated with exp_spec instead, so every decision is the one S3 took.  The test
       // reads only `power`: the MUFU results are first needed in pass 2, where 8 independent chains hide their latency.
       const float4 wh = sm_wh[j];
-      const float Pmin = wh.w, Pmax = wh.w + prm.ln_amax_over_amin;
+      // |power - P_min| <= 2e-5 or |power - P_max| <= 2e-5   <=>   | |power - P_mid| - P_half | <= 2e-5 (up to a rounding
+      // of ~5e-7, far inside the 2e-5 guard band)
+      const float Phalf = 0.5f * prm.ln_amax_over_amin, Pmid = wh.w + Phalf;
       float pw[PPL], av[PPL];
-      unsigned inr = 0;
       bool near = false;
 #pragma unroll
       for (int k = 0; k < PPL; ++k) {
         const float dy = sub_rn(py[k], s0.y);
         const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
         const bool in = e < last[k] && power <= 0.0f && power >= s1.w;
-        pw[k] = power;
-        inr |= in ? (1u << k) : 0u;
-        near |= in & ((fabsf(power - Pmin) <= 2e-5f) | (fabsf(power - Pmax) <= 2e-5f));    // bitwise: no branches
+        // outside the footprint or behind the pixel's last contributor: power = -inf, whose exp is 0 (MUFU) or NaN
+        // (exp_spec); either fails `a >= alpha_min`
+        pw[k] = in ? power : -INFINITY;
+        near |= fabsf(fabsf(pw[k] - Pmid) - Phalf) <= 2e-5f;
       }
       if (__any_sync(FULL, near)) {
 #pragma unroll
@@ -422,25 +429,24 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
 #pragma unroll
       for (int k = 0; k < PPL; ++k) {
         const float a = av[k];
-        const bool pass = ((inr >> k) & 1u) && a >= prm.alpha_min;      // same tests as S3 -> same contributor set
+        const bool pass = a >= prm.alpha_min;                            // same tests as S3 -> same contributor set
         const bool active = pass && !(a > prm.alpha_max);                // R-11: zero derivative at the 0.99 cap
-        const float alpha = fminf(a, prm.alpha_max);
+        const float alpha = pass ? fminf(a, prm.alpha_max) : 0.0f;       // alpha = 0: T_i = Tc, w = 0, nothing moves
         const float rc = rcp_approx(1.0f - alpha);
         const float Ti = Tc[k] * rc;
-        const float w = alpha * Ti;
+        const float wm = alpha * Ti;
         const float d0 = fmaf(Tc[k], v0, -S0[k]), d1 = fmaf(Tc[k], v1, -S1[k]), d2 = fmaf(Tc[k], v2, -S2[k]);
         float d3 = 0.0f;
         if (NCH == 4) d3 = fmaf(Tc[k], v3, -S3[k]);
-        const float wm = pass ? w : 0.0f;
         S0[k] = fmaf(v0, wm, S0[k]); S1[k] = fmaf(v1, wm, S1[k]); S2[k] = fmaf(v2, wm, S2[k]);
         if (NCH == 4) S3[k] = fmaf(v3, wm, S3[k]);
-        Tc[k] = pass ? Ti : Tc[k];
+        Tc[k] = Ti;
         W2 = fmaf(wm, wm, W2);
         float Dq = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
         if (NCH == 4) Dq = fmaf(d3, d3, Dq);
         const float r1 = active ? rc * alpha : 0.0f;                     // rc * alpha, zero when inactive
         const float f = Dq * r1 * r1;                                    // (sum_ch omega beta^2) alpha^2
-        const float gw = w * r1;                                         // beta_ch w alpha = d_ch * gw
+        const float gw = wm * r1;                                        // beta_ch w alpha = d_ch * gw
         const float t1 = (float)k - 3.5f, t2 = t1 * t1, t3 = t2 * t1, t4 = t2 * t2;
         F0 += f; F1 = fmaf(f, t1, F1); F2 = fmaf(f, t2, F2); F3 = fmaf(f, t3, F3); F4 = fmaf(f, t4, F4);
         const float dch[4] = {d0, d1, d2, d3};
@@ -532,7 +538,7 @@ static RasterParams make_params(const TileGrid& tg, int rank_bits, int W, int H,
 void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg, bool full_pix,
                     cudaStream_t st) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
-  const dim3 grid((unsigned)(tg.tiles_x * tg.tiles_y), (unsigned)batch.n);
+  const dim3 grid((unsigned)(tg.tiles_x * tg.tiles_y * batch.n));
   ++g_kernel_launches;
   if (full_pix)
     forward_kernel<true><<<grid, 32, 0, st>>>(batch, p);
@@ -543,7 +549,7 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
                      cudaStream_t st) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
-  const dim3 grid((unsigned)(tg.tiles_x * tg.tiles_y), (unsigned)batch.n);
+  const dim3 grid((unsigned)(tg.tiles_x * tg.tiles_y * batch.n));
   ++g_kernel_launches;
   if (cfg.channel_mask & NBV_CH_DEPTH)
     backward_kernel<4><<<grid, 32, 0, st>>>(batch, p);
