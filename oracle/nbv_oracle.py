@@ -321,3 +321,64 @@ def score_candidates(scene: OracleScene, train_cams, cand_cams, target=-1, alpha
         scores.append(g.sum())
     scores = np.array(scores)
     return dict(H_T=H_T, scores=scores, best=argmax_lowest(scores), conf=conf, gains=np.array(gains))
+
+
+# ---------------------------------------------------------------------------------------------------
+# per-output normalisation and fusion (Eq. 10-11), greedy selection.
+# ---------------------------------------------------------------------------------------------------
+def normalized_gain(raw, training_gains):
+    """PAPER.md Eq. 10 (L251-257): IG~_f(T,c) = IG_f(T,c) / ( (1/|T|) sum_{t in T} IG_f(T,t) )."""
+    tg = np.asarray(training_gains, dtype=np.float64)
+    return np.asarray(raw, dtype=np.float64) / (tg.sum() / tg.size)
+
+
+def fused_gain(ig_rgb_n, ig_d_n, beta_d=10.0):
+    """PAPER.md Eq. 11 (L261-265) without the object-mask output (NEXT-2, not built): IG~ = IG~_rgb + beta_d IG~_d;
+    beta_d = 10 (L742)."""
+    return np.asarray(ig_rgb_n, dtype=np.float64) + beta_d * np.asarray(ig_d_n, dtype=np.float64)
+
+
+def score_candidates_fused(scene_rgb: OracleScene, scene_d: OracleScene, train_cams, cand_cams, target=-1, beta_d=10.0,
+                           alpha_obj=0.3, alpha_opa=0.3, prior=None):
+    """Per-output gains (L248: each output has its own Jacobian, hence its own Hessian and gain), normalised by the
+    mean gain of the training views re-scored as candidates on top of the full H_T (Eq. 10), fused (Eq. 11), arg-max
+    (Eq. 5).  scene_rgb / scene_d: the same map with channel masks {r,g,b} / {depth}.
+    Returns dict(raw (2,C), denom (2,), normalized (2,C), fused (C,), best)."""
+    raw, denom = [], []
+    for scn in (scene_rgb, scene_d):
+        H_T = np.zeros((scn.N, NB))
+        for cam in np.atleast_1d(train_cams):
+            scn.view_hessian(cam, out=H_T)
+        r_c = score_candidates(scn, train_cams[:0], cand_cams, target, alpha_obj, alpha_opa, prior, H_T=H_T)["scores"]
+        r_t = score_candidates(scn, train_cams[:0], train_cams, target, alpha_obj, alpha_opa, prior, H_T=H_T)["scores"]
+        raw.append(r_c)
+        denom.append(r_t.sum() / r_t.size)
+    raw, denom = np.array(raw), np.array(denom)
+    norm = np.array([normalized_gain(raw[0], [denom[0]]), normalized_gain(raw[1], [denom[1]])])
+    fused = fused_gain(norm[0], norm[1], beta_d)
+    return dict(raw=raw, denom=denom, normalized=norm, fused=fused, best=argmax_lowest(fused))
+
+
+def select_greedy(scene: OracleScene, train_cams, cand_cams, rounds, target=-1, alpha_obj=0.3, alpha_opa=0.3, prior=None):
+    """Greedy multi-view selection without retraining (Eq. 5 applied repeatedly; L746 "6 rounds"):
+    in every round score the not-yet-selected candidates against the current H_T, pick the arg-max (lowest index on
+    ties), and add that view's Hessian to H_T (Eq. 6: the sum over the view set).
+    Returns dict(order (rounds,), scores (rounds, C) with NaN at already selected candidates)."""
+    prior = np.ones(P) if prior is None else np.asarray(prior, dtype=np.float64)
+    cand_cams = np.atleast_1d(cand_cams)
+    H_T = np.zeros((scene.N, NB))
+    for cam in np.atleast_1d(train_cams):
+        scene.view_hessian(cam, out=H_T)
+    conf = confidence(scene.obj_logits, scene.opacity, alpha_obj, alpha_opa, target)
+    H_c = [scene.view_hessian(cam) for cam in cand_cams]       # a view's block does not depend on H_T
+    order, table = [], []
+    for _ in range(rounds):
+        row = np.full(len(cand_cams), np.nan)
+        for i in range(len(cand_cams)):
+            if i not in order:
+                row[i] = gaussian_gains(H_T, H_c[i], conf, prior).sum()
+        best = int(np.flatnonzero(row == np.nanmax(row))[0])
+        order.append(best)
+        table.append(row)
+        H_T = H_T + H_c[best]
+    return dict(order=np.array(order), scores=np.array(table))
