@@ -141,6 +141,37 @@ int nbv_score_candidates(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int3
 int nbv_score_candidates_host(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t target_obj,
                               float* h_scores, int32_t* h_best, void* stream);
 
+/* ---- view selection on top of the per-view gains ------------- */
+
+/* Per-output normalised gains and their fusion (Eq. 10-11), for the outputs RGB and depth
+ * (the object-mask output of Eq. 11 is not built; its term is absent).
+ *   raw_f[i]   = IG_f(T, c_i)                       the score nbv_score_candidates gives in the context of output f
+ *   denom_f    = (1/|T|) sum_t IG_f(T, t)           the training views re-scored as candidates on top of the full H_T
+ *   fused[i]   = raw_rgb[i] / denom_rgb + beta_d * raw_d[i] / denom_d        (beta_d = 10 in the paper)
+ *   *d_best    = arg max_i fused[i], lowest index on ties
+ * ctx_rgb / ctx_depth: two contexts holding the SAME map, created with channel_mask = NBV_CH_RGB and NBV_CH_DEPTH
+ * (every output has its own Jacobian, hence its own Hessian), each with the n_train cameras of h_train
+ * already accumulated.  h_train: HOST array of those training cameras (needed again for the denominators).
+ * DEVICE outputs: d_fused n floats; d_raw 2*n floats (rgb row, then depth row; may be NULL); d_denom 2 floats
+ * (may be NULL); d_best one int32.  A zero denominator (no training view sees anything) yields non-finite
+ * fused scores, not an error.  Errors: NOT_LOADED, EMPTY_CANDIDATES (n == 0), UNKNOWN_TARGET, INVALID_ARG (null
+ * pointers, n_train <= 0, contexts of different N or K, wrong channel masks, bad camera), OOM, CUDA. */
+int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, const nbv_camera* h_train, int32_t n_train,
+                               const nbv_camera* h_cams, int32_t n, int32_t target_obj, float beta_d,
+                               float* d_fused, float* d_raw, float* d_denom, int32_t* d_best, void* stream);
+
+/* Greedy selection of `rounds` views out of n candidates without retraining (Eq. 5 applied repeatedly, P:L185;
+ * P:L746 uses 6 rounds): in round r the candidates not yet selected are scored against the current H_T, the arg-max
+ * (lowest index on ties) becomes h_order[r], and that view's blocks are added to H_T (Eq. 6).  On return H_T
+ * contains the selected views (|T| grows by `rounds`).
+ * HOST output h_order: rounds int32.  DEVICE output d_scores (may be NULL): rounds x n floats, row r = the scores of
+ * round r, NaN at candidates selected in earlier rounds.  Synchronises `stream` once per round (the selected index
+ * has to reach the host, which holds the cameras).
+ * Errors: NOT_LOADED, EMPTY_CANDIDATES, UNKNOWN_TARGET, INVALID_ARG (rounds < 1 or > n, null pointers, bad camera),
+ * OOM, CUDA. */
+int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t rounds, int32_t target_obj,
+                      int32_t* h_order, float* d_scores, void* stream);
+
 /* Counters of the last view processed by any call (synchronises `stream`). */
 int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream);
 

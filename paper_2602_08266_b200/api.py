@@ -35,7 +35,7 @@ EXPORTS = [
     "nbv_accumulate_training", "nbv_score_candidates", "nbv_score_candidates_host", "nbv_last_view_stats",
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
     "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
-    "nbv_tile_walk",
+    "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy",
 ]
 
 STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
@@ -204,6 +204,18 @@ class NBV:
                                                        C.c_void_p(scores.ctypes.data), C.byref(best), _stream()))
         return scores[:n], int(best.value)
 
+    def select_greedy(self, cams, rounds: int, target_obj: int = -1, want_scores: bool = True):
+        """nbv_select_greedy: returns (order: numpy int32 (rounds,), scores: CUDA tensor (rounds, n) or None).
+        H_T contains the selected views afterwards."""
+        torch = self._torch
+        cams = _cams(cams)
+        n = int(cams.shape[0])
+        order = np.full(max(int(rounds), 1), -1, dtype=np.int32)
+        scores = torch.empty((max(int(rounds), 1), max(n, 1)), dtype=torch.float32, device=self.device) if want_scores else None
+        self._check(self.lib.nbv_select_greedy(self._h, C.c_void_p(cams.ctypes.data), n, int(rounds), int(target_obj),
+                                               C.c_void_p(order.ctypes.data), _ptr(scores), _stream()))
+        return order[:rounds], (scores[:rounds, :n] if want_scores else None)
+
     def set_concurrency(self, views_in_flight: int):
         self._check(self.lib.nbv_set_concurrency(self._h, int(views_in_flight)))
 
@@ -298,3 +310,22 @@ class NBV:
         gains = torch.empty(self.N, dtype=torch.float32, device=self.device)
         self._check(self.lib.nbv_gaussian_gains(self._h, C.c_void_p(cam.ctypes.data), int(target_obj), _ptr(gains), _stream()))
         return gains
+
+
+def score_candidates_fused(nbv_rgb: NBV, nbv_depth: NBV, train_cams, cams, target_obj: int = -1, beta_d: float = 10.0):
+    """nbv_score_candidates_fused (Eq. 10-11): returns dict(fused (n,), raw (2, n), denom (2,), best (1,)) of
+    CUDA tensors.  nbv_rgb / nbv_depth: contexts with channel masks RGB / DEPTH holding the same map, with
+    `train_cams` already accumulated in both."""
+    torch = nbv_rgb._torch
+    tc, cc = _cams(train_cams), _cams(cams)
+    n, nt = int(cc.shape[0]), int(tc.shape[0])
+    dev = nbv_rgb.device
+    fused = torch.empty(max(n, 1), dtype=torch.float32, device=dev)
+    raw = torch.empty((2, max(n, 1)), dtype=torch.float32, device=dev)
+    denom = torch.empty(2, dtype=torch.float32, device=dev)
+    best = torch.empty(1, dtype=torch.int32, device=dev)
+    rc = nbv_rgb.lib.nbv_score_candidates_fused(nbv_rgb._h, nbv_depth._h, C.c_void_p(tc.ctypes.data), nt,
+                                                C.c_void_p(cc.ctypes.data), n, int(target_obj), C.c_float(beta_d),
+                                                _ptr(fused), _ptr(raw), _ptr(denom), _ptr(best), _stream())
+    nbv_rgb._check(rc)
+    return dict(fused=fused[:n], raw=raw[:, :n] if n else raw[:, :0], denom=denom, best=best)

@@ -111,4 +111,11 @@ void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, fl
 void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);
 
+// ---- select.cu
+// Eq. 10-11 on raw (2 x n) and training (2 x n_train) gains: denominators, fused scores, arg-max
+void launch_fuse(const float* raw, const float* train, int n, int n_train, float beta_d, float* denom, float* fused, int32_t* best,
+                 cudaStream_t st);
+// one greedy round: row[remaining[j]] = tmp[j], NaN elsewhere; *pick = arg-max over the remaining candidates
+void launch_greedy_round(const float* tmp, const int32_t* remaining, int m, int n, float* row, int32_t* pick, cudaStream_t st);
+
 }  // namespace nbv

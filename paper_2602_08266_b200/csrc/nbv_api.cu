@@ -58,7 +58,7 @@ struct nbv_ctx {
   bool loaded = false;
   int n_train = 0;
   // scene
-  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp;
+  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp;
   int conf_target = -2;                 // target the conf / cholT buffers were prepared for (-2 = stale)
   // views in flight: S1-S2 of each view run on its slot's stream, S3-S6 of a whole batch in one launch per stage on
   // the caller's stream; two sets of `concurrency` slots alternate so the next batch's S1-S2 overlap this batch's S3-S6
@@ -567,7 +567,7 @@ void nbv_destroy(nbv_ctx* ctx) {
   if (!ctx) return;
   cudaDeviceSynchronize();
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
-                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->tile_order};
+                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order};
   for (DevBuf* b : all) release(*b);
   for (ViewSlot* sl : ctx->slots) free_slot(sl);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -678,6 +678,83 @@ int nbv_score_candidates_host(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n,
   CK(cudaMemcpyAsync(h_scores, d_scores, 4 * (size_t)n, cudaMemcpyDeviceToHost, st));
   CK(cudaMemcpyAsync(h_best, d_best, 4, cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
+  return NBV_OK;
+}
+
+int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, const nbv_camera* h_train, int32_t n_train,
+                               const nbv_camera* h_cams, int32_t n, int32_t target_obj, float beta_d, float* d_fused,
+                               float* d_raw, float* d_denom, int32_t* d_best, void* stream) {
+  nbv_ctx* ctx = ctx_rgb;
+  if (!ctx_rgb || !ctx_depth) return NBV_ERR_INVALID_ARG;
+  if (!ctx_rgb->loaded || !ctx_depth->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  if (n == 0) return fail(ctx, NBV_ERR_EMPTY_CANDIDATES, "no candidate cameras");
+  if (n < 0 || n_train <= 0 || !h_train || !h_cams || !d_fused || !d_best || !std::isfinite(beta_d))
+    return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_score_candidates_fused: bad arguments");
+  if (ctx_rgb == ctx_depth || ctx_rgb->N != ctx_depth->N || ctx_rgb->K != ctx_depth->K)
+    return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_score_candidates_fused: the two contexts must be distinct and hold the same map");
+  if ((ctx_rgb->cfg.channel_mask & NBV_CH_DEPTH) || !(ctx_rgb->cfg.channel_mask & NBV_CH_RGB) || ctx_depth->cfg.channel_mask != NBV_CH_DEPTH)
+    return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_score_candidates_fused: channel masks must be RGB and DEPTH");
+  if (target_obj < -1 || target_obj >= ctx->K) return fail(ctx, NBV_ERR_UNKNOWN_TARGET, "target_obj must be -1 or in [0, K)");
+  cudaStream_t st = (cudaStream_t)stream;
+  // work area in the rgb context: raw (2n) | training gains (2 n_train) | denominators (2) | scratch arg-max (1)
+  const size_t words = 2 * (size_t)n + 2 * (size_t)n_train + 4;
+  CKRET(ensure(ctx, ctx->fuse_tmp, 4 * words));
+  float* raw = ctx->fuse_tmp.as<float>();
+  float* train = raw + 2 * (size_t)n;
+  float* denom = train + 2 * (size_t)n_train;
+  int32_t* scratch = reinterpret_cast<int32_t*>(denom + 2);
+  nbv_ctx* cx[2] = {ctx_rgb, ctx_depth};
+  for (int f = 0; f < 2; ++f) {
+    int rc = nbv_score_candidates(cx[f], h_cams, n, target_obj, raw + (size_t)f * n, scratch, stream);
+    if (rc == NBV_OK) rc = nbv_score_candidates(cx[f], h_train, n_train, target_obj, train + (size_t)f * n_train, scratch, stream);
+    if (rc != NBV_OK) {
+      if (f == 1) ctx->err = ctx_depth->err;
+      return rc;
+    }
+  }
+  launch_fuse(raw, train, n, n_train, beta_d, denom, d_fused, d_best, st);
+  CK(cudaGetLastError());
+  if (d_raw) CK(cudaMemcpyAsync(d_raw, raw, 8 * (size_t)n, cudaMemcpyDeviceToDevice, st));
+  if (d_denom) CK(cudaMemcpyAsync(d_denom, denom, 8, cudaMemcpyDeviceToDevice, st));
+  return NBV_OK;
+}
+
+int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t rounds, int32_t target_obj, int32_t* h_order,
+                      float* d_scores, void* stream) {
+  if (!ctx) return NBV_ERR_INVALID_ARG;
+  if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  if (n == 0) return fail(ctx, NBV_ERR_EMPTY_CANDIDATES, "no candidate cameras");
+  if (n < 0 || !h_cams || !h_order || rounds < 1 || rounds > n) return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_select_greedy: bad arguments");
+  if (target_obj < -1 || target_obj >= ctx->K) return fail(ctx, NBV_ERR_UNKNOWN_TARGET, "target_obj must be -1 or in [0, K)");
+  for (int i = 0; i < n; ++i)
+    if (!valid_camera(h_cams[i])) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
+  cudaStream_t st = (cudaStream_t)stream;
+  // work area: scores of the remaining candidates (n) | their original indices (n) | row when d_scores == NULL (n) | pick (1)
+  CKRET(ensure(ctx, ctx->fuse_tmp, 4 * (3 * (size_t)n + 4)));
+  float* tmp = ctx->fuse_tmp.as<float>();
+  int32_t* d_remaining = reinterpret_cast<int32_t*>(tmp + n);
+  float* row_tmp = tmp + 2 * (size_t)n;
+  int32_t* d_pick = reinterpret_cast<int32_t*>(tmp + 3 * (size_t)n);
+  std::vector<nbv_camera> cams;
+  std::vector<int32_t> remaining;
+  std::vector<char> taken((size_t)n, 0);
+  for (int r = 0; r < rounds; ++r) {
+    cams.clear(); remaining.clear();
+    for (int i = 0; i < n; ++i)
+      if (!taken[(size_t)i]) { cams.push_back(h_cams[i]); remaining.push_back(i); }
+    const int m = (int)cams.size();
+    CKRET(nbv_score_candidates(ctx, cams.data(), m, target_obj, tmp, d_pick, stream));
+    CK(cudaMemcpyAsync(d_remaining, remaining.data(), 4 * (size_t)m, cudaMemcpyHostToDevice, st));
+    launch_greedy_round(tmp, d_remaining, m, n, d_scores ? d_scores + (size_t)r * n : row_tmp, d_pick, st);
+    CK(cudaGetLastError());
+    int32_t pick = -1;
+    CK(cudaMemcpyAsync(&pick, d_pick, 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));          // also covers the pageable `remaining` copy above
+    if (pick < 0 || pick >= n || taken[(size_t)pick]) return fail(ctx, NBV_ERR_CUDA, "nbv_select_greedy: inconsistent arg-max");
+    taken[(size_t)pick] = 1;
+    h_order[r] = pick;
+    CKRET(nbv_accumulate_training(ctx, h_cams + pick, 1, stream));    // Eq. 6: H_T += H(c*)
+  }
   return NBV_OK;
 }
 
