@@ -75,6 +75,9 @@ struct RasterView {
 };
 struct RasterBatch {
   int n;
+  uint32_t n_work;              // launch positions (tiles x views) of a raster launch
+  uint32_t* work_fwd;           // forward: zeroed work counter of the persistent warps (nullptr: one block per position)
+  uint32_t* work;               // backward: zeroed counter the persistent warps pull launch positions from (nullptr: one block per position)
   const uint32_t* tile_order;   // launch position -> tile: tiles by increasing distance from the image centre, so the
                                 // long-running central tiles of a look-at view start first and the tail is made of cheap ones
   RasterView v[MAX_BATCH];

@@ -68,6 +68,8 @@ struct nbv_ctx {
   cudaEvent_t ev_set_done[2] = {nullptr, nullptr};   // S3-S6 of the last batch that used slot set 0 / 1
   cudaStream_t raster_st[2] = {nullptr, nullptr};    // S3-S6 of the batches of slot set 0 / 1 (forked from / joined into the caller's stream)
   ViewSlot* last_slot = nullptr;        // slot of the last view processed (nbv_last_view_stats)
+  DevBuf work_counters;                 // 3 x 128 B: work counters of the persistent backward launches
+  bool persistent = true;
   DevBuf tile_order;                    // centre-out launch order of the tiles of a tile_order_tx x tile_order_ty grid
   int tile_order_tx = 0, tile_order_ty = 0;
   // optional per-stage timing (nbv_set_stage_timing)
@@ -375,6 +377,16 @@ int ensure_tile_order(nbv_ctx* ctx, const TileGrid& tg, cudaStream_t st) {
 int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int upto, bool full_pix, cudaStream_t st) {
   RasterBatch rb;
   rb.n = n;
+  rb.n_work = 0;
+  rb.work = nullptr;
+  rb.work_fwd = nullptr;
+  if (ctx->persistent) {
+    // one counter per raster stream (launches on a stream are ordered); the parity exports run on the caller's stream
+    const int wi = st == ctx->raster_st[0] ? 0 : st == ctx->raster_st[1] ? 1 : 2;
+    rb.work = ctx->work_counters.as<uint32_t>() + 32 * wi;
+    rb.work_fwd = rb.work + 1;
+    CK(cudaMemsetAsync(rb.work, 0, 8, st));
+  }
   for (int i = 0; i < n; ++i) {
     ViewSlot* s = sl[i];
     RasterView& v = rb.v[i];
@@ -555,6 +567,8 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
     nbv_destroy(ctx);
     return NBV_ERR_CUDA;
   }
+  if (ensure(ctx, ctx->work_counters, 3 * 128) != NBV_OK) { nbv_destroy(ctx); return NBV_ERR_OOM; }
+  if (const char* e = std::getenv("NBV_PERSISTENT")) ctx->persistent = std::atoi(e) != 0;
   if (const char* e = std::getenv("NBV_CONCURRENCY")) {
     const int v = std::atoi(e);
     if (v >= 1 && v <= MAX_BATCH) ctx->concurrency = v;
@@ -567,7 +581,7 @@ void nbv_destroy(nbv_ctx* ctx) {
   if (!ctx) return;
   cudaDeviceSynchronize();
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
-                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order};
+                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order, &ctx->work_counters};
   for (DevBuf* b : all) release(*b);
   for (ViewSlot* sl : ctx->slots) free_slot(sl);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);

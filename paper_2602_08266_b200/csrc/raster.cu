@@ -20,6 +20,8 @@
 //    1 sum   sum_px w^2
 // = 40 numbers per (tile, Gaussian) for RGB + depth.  The oracle forms explicit rows instead, so parity
 // checks this algebra.
+#include <algorithm>
+
 #include "kernels.h"
 
 namespace nbv {
@@ -102,7 +104,19 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   // One launch rasterises every view of the batch.  Launch position -> (view, tile): the views are
   // interleaved, so the launch starts with the central (long-running) tiles of ALL views and its tail is made of the
   // edge tiles of all views.
-  const int bpos = blockIdx.x, vidx = bpos % batch.n;
+  // Persistent warps (batch.work_fwd != nullptr): the grid is one wave of resident warps and every warp pulls launch
+  // positions from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
+  __shared__ float4 sm[32 * 3];
+  __shared__ uint32_t q_rank[64], q_cpos[64];
+  const int lane = threadIdx.x;
+  for (uint32_t bpos = blockIdx.x;; ) {
+  if (batch.work_fwd) {
+    if (lane == 0) bpos = atomicAdd(batch.work_fwd, 1u);
+    bpos = __shfl_sync(FULL, bpos, 0);
+  }
+  if (bpos >= batch.n_work) return;
+  __syncwarp();
+  const int vidx = (int)(bpos % (uint32_t)batch.n);
   const RasterView& vw = batch.v[vidx];
   const Splat* __restrict__ splat_sorted = vw.splat_sorted;
   const uint32_t* __restrict__ ckeys = vw.ckeys;
@@ -112,9 +126,7 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   uint32_t* __restrict__ tile_cend = vw.tile_cend;
   uint32_t* __restrict__ tile_walk = vw.tile_walk;
   ViewCounters* counters = vw.counters;
-  __shared__ float4 sm[32 * 3];
-  __shared__ uint32_t q_rank[64], q_cpos[64];
-  const int tile = batch.tile_order[bpos / batch.n], lane = threadIdx.x;   // heaviest tiles first (launch order)
+  const int tile = batch.tile_order[bpos / (uint32_t)batch.n];   // heaviest tiles first (launch order)
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -231,6 +243,8 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
       atomicAdd(&counters->n_pairs, (unsigned long long)pairs);
     }
   }
+  if (!batch.work_fwd) return;
+  }  // persistent loop
 }
 
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -299,7 +313,21 @@ __device__ __forceinline__ float4 atom_add_v4(float* dst, const float4& v) {
 
 template <int NCH>
 __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
-  const int bpos = blockIdx.x, vidx = bpos % batch.n;       // views interleaved (see forward_kernel)
+  __shared__ float4 sm[32 * 3];
+  __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
+  __shared__ __align__(16) float red[32 * RED_STRIDE];
+  __shared__ uint32_t q_rank[64];
+  const int lane = threadIdx.x;
+  // Persistent warps (batch.work != nullptr): the grid is one wave of resident warps and every warp pulls launch positions
+  // from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
+  for (uint32_t bpos = blockIdx.x;; ) {
+  if (batch.work) {
+    if (lane == 0) bpos = atomicAdd(batch.work, 1u);
+    bpos = __shfl_sync(FULL, bpos, 0);
+  }
+  if (bpos >= batch.n_work) return;
+  __syncwarp();
+  const int vidx = (int)(bpos % (uint32_t)batch.n);      // views interleaved (see forward_kernel)
   const RasterView& vw = batch.v[vidx];
   const Splat* __restrict__ splat_sorted = vw.splat_sorted;
   const uint32_t* __restrict__ ckeys = vw.ckeys;
@@ -308,11 +336,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   const uint32_t* __restrict__ tile_cend = vw.tile_cend;
   const PixelBuf pix = vw.pix;
   float* __restrict__ moments = vw.moments;
-  __shared__ float4 sm[32 * 3];
-  __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
-  __shared__ __align__(16) float red[32 * RED_STRIDE];
-  __shared__ uint32_t q_rank[64];
-  const int tile = batch.tile_order[bpos / batch.n], lane = threadIdx.x;   // heaviest tiles first (launch order)
+  const int tile = batch.tile_order[bpos / (uint32_t)batch.n];   // heaviest tiles first (launch order)
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -338,7 +362,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) maxlast = max(maxlast, __shfl_xor_sync(FULL, maxlast, o));
-  if (maxlast == 0) return;
+  if (maxlast == 0) { if (batch.work) continue; return; }
 
   // walk the supertile list backwards from the last composited entry; the entries that pass the rect test are the
   // tile-list entries maxlast-1, maxlast-2, ..., 0 in that order
@@ -504,6 +528,8 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
     e_next -= cnt;
     shift_queue(q_rank, nullptr, qn, (uint32_t)cnt);
   }
+  if (!batch.work) return;
+  }  // persistent loop
 }
 
 // Touched list of every view of the batch: the ranks whose sum w^2 (moment 39) is non-zero, i.e. the Gaussians with at
@@ -538,23 +564,31 @@ static RasterParams make_params(const TileGrid& tg, int rank_bits, int W, int H,
 void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg, bool full_pix,
                     cudaStream_t st) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
-  const dim3 grid((unsigned)(tg.tiles_x * tg.tiles_y * batch.n));
+  RasterBatch b = batch;
+  b.n_work = (uint32_t)(tg.tiles_x * tg.tiles_y * batch.n);
+  unsigned blocks = b.n_work;
+  if (b.work_fwd) blocks = std::min(blocks, 148u * (full_pix ? 16u : 32u));
+  const dim3 grid(blocks);
   ++g_kernel_launches;
   if (full_pix)
-    forward_kernel<true><<<grid, 32, 0, st>>>(batch, p);
+    forward_kernel<true><<<grid, 32, 0, st>>>(b, p);
   else
-    forward_kernel<false><<<grid, 32, 0, st>>>(batch, p);
+    forward_kernel<false><<<grid, 32, 0, st>>>(b, p);
 }
 
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
                      cudaStream_t st) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
-  const dim3 grid((unsigned)(tg.tiles_x * tg.tiles_y * batch.n));
+  RasterBatch b = batch;
+  b.n_work = (uint32_t)(tg.tiles_x * tg.tiles_y * batch.n);
+  unsigned blocks = b.n_work;
+  if (b.work) blocks = std::min(blocks, 148u * NBV_BWD_MIN_BLOCKS);
+  const dim3 grid(blocks);
   ++g_kernel_launches;
   if (cfg.channel_mask & NBV_CH_DEPTH)
-    backward_kernel<4><<<grid, 32, 0, st>>>(batch, p);
+    backward_kernel<4><<<grid, 32, 0, st>>>(b, p);
   else
-    backward_kernel<3><<<grid, 32, 0, st>>>(batch, p);
+    backward_kernel<3><<<grid, 32, 0, st>>>(b, p);
   ++g_kernel_launches;
   touched_kernel<<<dim3((unsigned)((N + 255) / 256), (unsigned)batch.n), 256, 0, st>>>(batch, N);
 }
