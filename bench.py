@@ -46,8 +46,8 @@ FLOP_BWD_PAIR = {3: 134, 4: 154}   # composited pair, S4: exp, beta, 34 / 40 mom
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
 VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (grid.y = view)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture
-# (profiles/r1b_ncu_raster_cfg2.md); known for config 2 only
-NCU_TRAFFIC_BYTES = {2: {"backward": 99.1e6, "forward": 37.7e6}}
+# (profiles/r1c_ncu_raster_cfg2.md); known for config 2 only
+NCU_TRAFFIC_BYTES = {2: {"backward": 98.9e6, "forward": 40.8e6}}
 
 
 def parse_args():
