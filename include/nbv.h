@@ -164,9 +164,13 @@ int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, const nbv_c
  * P:L746 uses 6 rounds): in round r the candidates not yet selected are scored against the current H_T, the arg-max
  * (lowest index on ties) becomes h_order[r], and that view's blocks are added to H_T (Eq. 6).  On return H_T
  * contains the selected views (|T| grows by `rounds`).
+ * A view's blocks do not depend on H_T, so every candidate is rasterised once (S1-S5) into a sparse pool of
+ * (Gaussian, 14x14 block) entries; each round then runs only S0' (new factors of H_T), S6 over the pool, the masked
+ * arg-max and the addition of the selected view's blocks, all on the device.  The pool is limited to 4 GiB (override:
+ * environment variable NBV_GREEDY_CACHE_MB at nbv_create); if the candidates' blocks do not fit, the call falls back to
+ * re-rasterising the remaining candidates every round (same results, one host synchronisation per round).
  * HOST output h_order: rounds int32.  DEVICE output d_scores (may be NULL): rounds x n floats, row r = the scores of
- * round r, NaN at candidates selected in earlier rounds.  Synchronises `stream` once per round (the selected index
- * has to reach the host, which holds the cameras).
+ * round r, NaN at candidates selected in earlier rounds.  Synchronises `stream`.
  * Errors: NOT_LOADED, EMPTY_CANDIDATES, UNKNOWN_TARGET, INVALID_ARG (rounds < 1 or > n, null pointers, bad camera),
  * OOM, CUDA. */
 int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t rounds, int32_t target_obj,

@@ -295,7 +295,8 @@ __device__ float gain_solve(float* B, const float* U) {
 
 __global__ void __launch_bounds__(64) expand_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
                                                      const __grid_constant__ ExpandBatch batch, int mode, float* __restrict__ H_T,
-                                                     const float* __restrict__ conf, const float* __restrict__ cholT) {
+                                                     const float* __restrict__ conf, const float* __restrict__ cholT,
+                                                     uint32_t* __restrict__ cache_ids, float* __restrict__ cache_blocks) {
   const ExpandView& vw = batch.v[blockIdx.y];
   const nbv_camera& cam = vw.cam;
   const uint32_t* __restrict__ ids_sorted = vw.ids_sorted;
@@ -339,6 +340,13 @@ __global__ void __launch_bounds__(64) expand_kernel(const __grid_constant__ Scen
     } else if (mode == EXPAND_VIEW) {
       float* dst = out_blocks + (size_t)g * NBLK;
       for (int i = 0; i < NBLK; ++i) dst[i] = H[i];
+    } else if (mode == EXPAND_CACHE) {
+      if (t < vw.cache_span[1]) {                      // span[1] = 0 when the pool overflowed: nothing is stored
+        const size_t e = (size_t)vw.cache_span[0] + t;
+        cache_ids[e] = g;
+        float* dst = cache_blocks + e * NBLK;
+        for (int i = 0; i < NBLK; ++i) dst[i] = H[i];
+      }
     } else {
       const float c = conf[g];
       float gn = 0.f;
@@ -371,7 +379,89 @@ void launch_expand(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch&
   const int cap = (148 * 8 + batch.n - 1) / batch.n;
   if (blocks > cap) blocks = cap;
   ++g_kernel_launches;
-  expand_kernel<<<dim3((unsigned)blocks, (unsigned)batch.n), 64, 0, st>>>(sc, cfg, batch, mode, H_T, conf, cholT);
+  expand_kernel<<<dim3((unsigned)blocks, (unsigned)batch.n), 64, 0, st>>>(sc, cfg, batch, mode, H_T, conf, cholT, nullptr, nullptr);
+}
+
+// ---- sparse block cache of greedy selection ----------------------------------------------------------------------
+__global__ void cache_reserve_kernel(const __grid_constant__ ExpandBatch batch, BlockCache cache, int first_candidate) {
+  const int v = threadIdx.x;
+  if (v >= batch.n) return;
+  const uint32_t cnt = batch.v[v].counters->n_touched;
+  const uint32_t base = atomicAdd(cache.cursor, cnt);
+  uint32_t* span = cache.spans + 2 * (size_t)(first_candidate + v);
+  if ((unsigned long long)base + cnt > cache.capacity) {
+    cache.cursor[1] = 1u;                                // overflow: the caller falls back to re-rasterising
+    span[0] = 0u; span[1] = 0u;
+  } else {
+    span[0] = base; span[1] = cnt;
+  }
+}
+
+void launch_cache_reserve(const ExpandBatch& batch, const BlockCache& cache, int first_candidate, cudaStream_t st) {
+  ++g_kernel_launches;
+  cache_reserve_kernel<<<1, 32, 0, st>>>(batch, cache, first_candidate);
+}
+
+void launch_expand_cache(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, const BlockCache& cache, cudaStream_t st) {
+  int blocks = (sc.N + 63) / 64;
+  const int cap = (148 * 8 + batch.n - 1) / batch.n;
+  if (blocks > cap) blocks = cap;
+  ++g_kernel_launches;
+  expand_kernel<<<dim3((unsigned)blocks, (unsigned)batch.n), 64, 0, st>>>(sc, cfg, batch, EXPAND_CACHE, nullptr, nullptr, nullptr, cache.ids,
+                                                                         cache.blocks);
+}
+
+// One thread per cached (candidate, Gaussian) entry: the gain of Eq. 5/6/9 of that block against the current factor U_g.
+__global__ void __launch_bounds__(64) cached_gain_kernel(BlockCache cache, const int32_t* __restrict__ taken, const float* __restrict__ conf,
+                                                         const float* __restrict__ cholT, float* __restrict__ scores) {
+  const int c = blockIdx.y;
+  float gain = 0.f;
+  if (!taken[c]) {
+    const uint32_t base = cache.spans[2 * c], cnt = cache.spans[2 * c + 1];
+    for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < cnt; t += gridDim.x * blockDim.x) {
+      const size_t e = (size_t)base + t;
+      const uint32_t g = cache.ids[e];
+      const float cg = conf[g];
+      if (cg > 0.f) {
+        float H[NBLK], U[NBLK];
+        const float* hb = cache.blocks + e * NBLK;
+        const float* ut = cholT + (size_t)g * NBLK;
+        for (int i = 0; i < NBLK; ++i) { U[i] = ut[i]; H[i] = cg * hb[i]; }
+        gain += gain_solve(H, U);
+      }
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) gain += __shfl_xor_sync(0xffffffffu, gain, o);
+  __shared__ float ws[2];
+  if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = gain;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const float t = ws[0] + ws[1];
+    if (t != 0.f) atomicAdd(scores + c, t);
+  }
+}
+
+void launch_cached_gain(const BlockCache& cache, int n_cand, const int32_t* taken, const float* conf, const float* cholT, float* scores,
+                        cudaStream_t st) {
+  ++g_kernel_launches;
+  cached_gain_kernel<<<dim3(64, (unsigned)n_cand), 64, 0, st>>>(cache, taken, conf, cholT, scores);
+}
+
+__global__ void __launch_bounds__(256) cache_accumulate_kernel(BlockCache cache, const int32_t* __restrict__ pick, float* __restrict__ H_T) {
+  const int c = *pick;
+  const uint32_t base = cache.spans[2 * c], cnt = cache.spans[2 * c + 1];
+  const size_t total = (size_t)cnt * NBLK;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t e = i / NBLK, k = i - e * NBLK;
+    const uint32_t g = cache.ids[base + e];              // a view lists every Gaussian at most once: no atomics needed
+    H_T[(size_t)g * NBLK + k] += cache.blocks[((size_t)base + e) * NBLK + k];
+  }
+}
+
+void launch_cache_accumulate(const BlockCache& cache, const int32_t* pick, float* H_T, cudaStream_t st) {
+  ++g_kernel_launches;
+  cache_accumulate_kernel<<<148 * 4, 256, 0, st>>>(cache, pick, H_T);
 }
 
 // S0': confidence (Eq. 7; Eq. 12)

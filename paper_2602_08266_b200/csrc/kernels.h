@@ -89,7 +89,7 @@ void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int ra
                      cudaStream_t st);
 
 // ---- hessian.cu
-enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2 };
+enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2, EXPAND_CACHE = 3 };
 // EXPAND_TRAIN: H_T[id] += H ; EXPAND_VIEW: out_blocks[id] = H ; EXPAND_GAIN: gain vs H_T, sum into *score (and gains[id] if not null)
 // Consumes the touched list of every view of the batch: reads the moments of every touched rank and writes zeros back
 // (the moment buffers are all-zero again afterwards).
@@ -103,6 +103,9 @@ struct ExpandView {
   float* score;              // EXPAND_GAIN
   float* gains;              // EXPAND_GAIN, may be null
   ViewCounters* counters;
+  // EXPAND_CACHE: the view's touched Gaussians and their unweighted blocks go to pool entries
+  // [cache_span[0], cache_span[0] + cache_span[1]) (reserved by cache_reserve_kernel; span[1] = 0 on overflow)
+  const uint32_t* cache_span;
 };
 struct ExpandBatch {
   int n;
@@ -110,6 +113,22 @@ struct ExpandBatch {
 };
 void launch_expand(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, float* H_T, const float* conf,
                    const float* cholT, cudaStream_t st);
+// Sparse per-candidate block cache of greedy selection (nbv_select_greedy): pool of (Gaussian id, 105-float block) entries.
+struct BlockCache {
+  uint32_t* ids;             // capacity entries
+  float* blocks;             // capacity x 105
+  uint32_t* spans;           // per candidate: (first entry, number of entries)
+  uint32_t* cursor;          // [0] entries reserved so far, [1] overflow flag
+  uint32_t capacity;
+};
+// reserve pool space for the views of a batch (after their touched lists are known); spans_of_view[i] = spans + 2 * candidate
+void launch_cache_reserve(const ExpandBatch& batch, const BlockCache& cache, int first_candidate, cudaStream_t st);
+void launch_expand_cache(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, const BlockCache& cache, cudaStream_t st);
+// scores[c] += sum over the cached entries of candidate c of the gain against cholT (skipped when taken[c] != 0)
+void launch_cached_gain(const BlockCache& cache, int n_cand, const int32_t* taken, const float* conf, const float* cholT, float* scores,
+                        cudaStream_t st);
+// H_T[g] += block for the cached entries of candidate *pick
+void launch_cache_accumulate(const BlockCache& cache, const int32_t* pick, float* H_T, cudaStream_t st);
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);
 void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);
@@ -120,5 +139,7 @@ void launch_fuse(const float* raw, const float* train, int n, int n_train, float
                  cudaStream_t st);
 // one greedy round: row[remaining[j]] = tmp[j], NaN elsewhere; *pick = arg-max over the remaining candidates
 void launch_greedy_round(const float* tmp, const int32_t* remaining, int m, int n, float* row, int32_t* pick, cudaStream_t st);
+// device-resident greedy round: row[i] = taken[i] ? NaN : scores[i]; *pick = order_r[0] = arg-max over the free ones; taken[*pick] = 1
+void launch_greedy_pick(const float* scores, int32_t* taken, int n, float* row, int32_t* pick, int32_t* order_r, cudaStream_t st);
 
 }  // namespace nbv

@@ -58,7 +58,8 @@ struct nbv_ctx {
   bool loaded = false;
   int n_train = 0;
   // scene
-  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp;
+  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp, cache_ids, cache_blocks, cache_meta;
+  size_t greedy_cache_bytes = (size_t)4 << 30;   // budget of the block cache of nbv_select_greedy (NBV_GREEDY_CACHE_MB)
   int conf_target = -2;                 // target the conf / cholT buffers were prepared for (-2 = stale)
   // views in flight: S1-S2 of each view run on its slot's stream, S3-S6 of a whole batch in one launch per stage on
   // the caller's stream; two sets of `concurrency` slots alternate so the next batch's S1-S2 overlap this batch's S3-S6
@@ -415,7 +416,7 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
 
 // S5 (+S6) of the views raster_batch() left in the slots.  out_blocks / gains: single-view exports (n == 1) only.
 int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int mode, float* out_blocks, float* d_scores,
-                 float* gains, cudaStream_t st) {
+                 float* gains, cudaStream_t st, const BlockCache* cache = nullptr, int first_candidate = 0) {
   ExpandBatch eb;
   eb.n = n;
   for (int i = 0; i < n; ++i) {
@@ -425,9 +426,15 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     v.ids_sorted = s->ids.as<uint32_t>(); v.splat_sorted = s->splat_sorted.as<Splat>(); v.touched = s->touched.as<uint32_t>();
     v.moments = s->moments.as<float>(); v.out_blocks = out_blocks; v.score = d_scores ? d_scores + i : nullptr; v.gains = gains;
     v.counters = s->d_counters;
+    v.cache_span = cache ? cache->spans + 2 * (size_t)(first_candidate + i) : nullptr;
   }
   const int sp = span_begin(ctx, NBV_STAGE_EXPAND, n, st);
-  launch_expand(scene_dev(ctx), ctx->cfg, eb, mode, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
+  if (mode == EXPAND_CACHE) {
+    launch_cache_reserve(eb, *cache, first_candidate, st);
+    launch_expand_cache(scene_dev(ctx), ctx->cfg, eb, *cache, st);
+  } else {
+    launch_expand(scene_dev(ctx), ctx->cfg, eb, mode, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
+  }
   CK(cudaGetLastError());
   span_end(ctx, sp, st);
   for (int i = 0; i < n; ++i) sl[i]->moments_clean = true;
@@ -449,7 +456,7 @@ int expand_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int mode, flo
 // Run S1..S6 for n cameras in batches of up to `concurrency` views of equal image size.  S1-S2 of every view run on its slot's
 // stream; S3, S4 and S5+S6 of the whole batch are one launch each on the caller's stream.  Two slot sets alternate, so the
 // S1-S2 work of batch b+1 overlaps the S3-S6 launches of batch b.  Everything is ordered by events: the call never blocks.
-int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_scores, cudaStream_t st) {
+int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_scores, cudaStream_t st, const BlockCache* cache = nullptr) {
   const int V = std::max(1, std::min(ctx->concurrency, MAX_BATCH));
   CK(cudaEventRecord(ctx->ev_fork, st));
   for (int s = 0; s < 2; ++s) CK(cudaStreamWaitEvent(ctx->raster_st[s], ctx->ev_fork, 0));
@@ -476,7 +483,7 @@ int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_
       cudaStreamWaitEvent(rs, sl[i]->done, 0);      // join even after an error: no stream may run ahead
     }
     if (rc == NBV_OK) rc = raster_batch(ctx, sl, h_cams + i0, nb, STAGE_BACKWARD, false, rs);
-    if (rc == NBV_OK) rc = expand_batch(ctx, sl, h_cams + i0, nb, mode, nullptr, d_scores ? d_scores + i0 : nullptr, nullptr, rs);
+    if (rc == NBV_OK) rc = expand_batch(ctx, sl, h_cams + i0, nb, mode, nullptr, d_scores ? d_scores + i0 : nullptr, nullptr, rs, cache, i0);
     cudaEventRecord(ctx->ev_set_done[set], rs);
     set_used[set] = true;
     i0 += nb;
@@ -569,6 +576,7 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
   }
   if (ensure(ctx, ctx->work_counters, 3 * 128) != NBV_OK) { nbv_destroy(ctx); return NBV_ERR_OOM; }
   if (const char* e = std::getenv("NBV_PERSISTENT")) ctx->persistent = std::atoi(e) != 0;
+  if (const char* e = std::getenv("NBV_GREEDY_CACHE_MB")) ctx->greedy_cache_bytes = (size_t)std::max(0, std::atoi(e)) << 20;
   if (const char* e = std::getenv("NBV_CONCURRENCY")) {
     const int v = std::atoi(e);
     if (v >= 1 && v <= MAX_BATCH) ctx->concurrency = v;
@@ -581,7 +589,8 @@ void nbv_destroy(nbv_ctx* ctx) {
   if (!ctx) return;
   cudaDeviceSynchronize();
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
-                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order, &ctx->work_counters};
+                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order, &ctx->work_counters, &ctx->cache_ids,
+                   &ctx->cache_blocks, &ctx->cache_meta};
   for (DevBuf* b : all) release(*b);
   for (ViewSlot* sl : ctx->slots) free_slot(sl);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -733,16 +742,9 @@ int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, const nbv_c
   return NBV_OK;
 }
 
-int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t rounds, int32_t target_obj, int32_t* h_order,
-                      float* d_scores, void* stream) {
-  if (!ctx) return NBV_ERR_INVALID_ARG;
-  if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
-  if (n == 0) return fail(ctx, NBV_ERR_EMPTY_CANDIDATES, "no candidate cameras");
-  if (n < 0 || !h_cams || !h_order || rounds < 1 || rounds > n) return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_select_greedy: bad arguments");
-  if (target_obj < -1 || target_obj >= ctx->K) return fail(ctx, NBV_ERR_UNKNOWN_TARGET, "target_obj must be -1 or in [0, K)");
-  for (int i = 0; i < n; ++i)
-    if (!valid_camera(h_cams[i])) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
-  cudaStream_t st = (cudaStream_t)stream;
+// greedy selection by re-rasterising the remaining candidates every round (fallback when the block cache is too small)
+static int select_greedy_rescore(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t rounds, int32_t target_obj, int32_t* h_order,
+                                 float* d_scores, cudaStream_t st) {
   // work area: scores of the remaining candidates (n) | their original indices (n) | row when d_scores == NULL (n) | pick (1)
   CKRET(ensure(ctx, ctx->fuse_tmp, 4 * (3 * (size_t)n + 4)));
   float* tmp = ctx->fuse_tmp.as<float>();
@@ -757,7 +759,7 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
     for (int i = 0; i < n; ++i)
       if (!taken[(size_t)i]) { cams.push_back(h_cams[i]); remaining.push_back(i); }
     const int m = (int)cams.size();
-    CKRET(nbv_score_candidates(ctx, cams.data(), m, target_obj, tmp, d_pick, stream));
+    CKRET(nbv_score_candidates(ctx, cams.data(), m, target_obj, tmp, d_pick, (void*)st));
     CK(cudaMemcpyAsync(d_remaining, remaining.data(), 4 * (size_t)m, cudaMemcpyHostToDevice, st));
     launch_greedy_round(tmp, d_remaining, m, n, d_scores ? d_scores + (size_t)r * n : row_tmp, d_pick, st);
     CK(cudaGetLastError());
@@ -767,8 +769,56 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
     if (pick < 0 || pick >= n || taken[(size_t)pick]) return fail(ctx, NBV_ERR_CUDA, "nbv_select_greedy: inconsistent arg-max");
     taken[(size_t)pick] = 1;
     h_order[r] = pick;
-    CKRET(nbv_accumulate_training(ctx, h_cams + pick, 1, stream));    // Eq. 6: H_T += H(c*)
+    CKRET(nbv_accumulate_training(ctx, h_cams + pick, 1, (void*)st));    // Eq. 6: H_T += H(c*)
   }
+  return NBV_OK;
+}
+
+int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t rounds, int32_t target_obj, int32_t* h_order,
+                      float* d_scores, void* stream) {
+  if (!ctx) return NBV_ERR_INVALID_ARG;
+  if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  if (n == 0) return fail(ctx, NBV_ERR_EMPTY_CANDIDATES, "no candidate cameras");
+  if (n < 0 || !h_cams || !h_order || rounds < 1 || rounds > n) return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_select_greedy: bad arguments");
+  if (target_obj < -1 || target_obj >= ctx->K) return fail(ctx, NBV_ERR_UNKNOWN_TARGET, "target_obj must be -1 or in [0, K)");
+  for (int i = 0; i < n; ++i)
+    if (!valid_camera(h_cams[i])) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
+  cudaStream_t st = (cudaStream_t)stream;
+  // A view's blocks do not depend on H_T, so every candidate is rasterised ONCE: S1-S5 leave its touched Gaussians and
+  // their unweighted 14x14 blocks in a sparse pool; every round then needs only S0' (new factors), S6 over the pool,
+  // the masked arg-max and H_T += (blocks of the selected view) -- all on the device, no camera and no host round trip.
+  const size_t entry_bytes = 4 * (size_t)NBLK + 4;
+  const size_t want = std::min((size_t)n * (size_t)ctx->N, ctx->greedy_cache_bytes / entry_bytes);
+  if (want == 0 || want > 0xfffffff0ull) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);
+  CKRET(ensure(ctx, ctx->cache_ids, 4 * want));
+  CKRET(ensure(ctx, ctx->cache_blocks, 4 * (size_t)NBLK * want));
+  // meta: spans (2n) | cursor + overflow flag (2) | taken (n) | scores (n) | pick (1) | order (rounds)
+  CKRET(ensure(ctx, ctx->cache_meta, 4 * (4 * (size_t)n + 4 + (size_t)rounds)));
+  BlockCache bc;
+  bc.ids = ctx->cache_ids.as<uint32_t>(); bc.blocks = ctx->cache_blocks.as<float>();
+  bc.spans = ctx->cache_meta.as<uint32_t>(); bc.cursor = bc.spans + 2 * (size_t)n; bc.capacity = (uint32_t)want;
+  int32_t* d_taken = reinterpret_cast<int32_t*>(bc.cursor + 2);
+  float* d_round = reinterpret_cast<float*>(d_taken + n);
+  int32_t* d_pick = reinterpret_cast<int32_t*>(d_round + n);
+  int32_t* d_order = d_pick + 1;
+  CK(cudaMemsetAsync(ctx->cache_meta.p, 0, 4 * (4 * (size_t)n + 4 + (size_t)rounds), st));
+  CKRET(run_views(ctx, h_cams, n, EXPAND_CACHE, nullptr, st, &bc));
+  uint32_t h_cursor[2] = {0, 0};
+  CK(cudaMemcpyAsync(h_cursor, bc.cursor, 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  if (h_cursor[1]) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);   // pool too small
+  for (int r = 0; r < rounds; ++r) {
+    CKRET(prepare_scoring(ctx, target_obj, st));
+    CK(cudaMemsetAsync(d_round, 0, 4 * (size_t)n, st));
+    launch_cached_gain(bc, n, d_taken, ctx->conf.as<float>(), ctx->cholT.as<float>(), d_round, st);
+    launch_greedy_pick(d_round, d_taken, n, d_scores ? d_scores + (size_t)r * n : nullptr, d_pick, d_order + r, st);
+    launch_cache_accumulate(bc, d_pick, ctx->H_T.as<float>(), st);      // Eq. 6: H_T += H(c*)
+    CK(cudaGetLastError());
+    ctx->conf_target = -2;                                                // the factors of H_T are stale
+    ++ctx->n_train;
+  }
+  CK(cudaMemcpyAsync(h_order, d_order, 4 * (size_t)rounds, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
   return NBV_OK;
 }
 

@@ -86,6 +86,34 @@ __global__ void __launch_bounds__(SEL_T) greedy_round_kernel(const float* __rest
   if (threadIdx.x == 0) *pick = bi == 0x7fffffff ? remaining[0] : bi;
 }
 
+// device-resident greedy round (nbv_select_greedy with the block cache)
+__global__ void __launch_bounds__(SEL_T) greedy_pick_kernel(const float* __restrict__ scores, int32_t* __restrict__ taken, int n,
+                                                            float* __restrict__ row, int32_t* __restrict__ pick, int32_t* __restrict__ order_r) {
+  float bv = -CUDART_INF_F;
+  int bi = 0x7fffffff;
+  for (int i = threadIdx.x; i < n; i += SEL_T) {
+    const bool tk = taken[i] != 0;
+    const float v = scores[i];
+    if (row) row[i] = tk ? CUDART_NAN_F : v;
+    if (!tk && (v > bv || (v == bv && i < bi))) { bv = v; bi = i; }
+  }
+  block_argmax(bv, bi);
+  if (threadIdx.x == 0) {
+    if (bi == 0x7fffffff) {                               // only non-comparable scores left: lowest free index
+      for (int i = 0; i < n; ++i)
+        if (!taken[i]) { bi = i; break; }
+    }
+    *pick = bi;
+    *order_r = bi;
+    taken[bi] = 1;
+  }
+}
+
+void launch_greedy_pick(const float* scores, int32_t* taken, int n, float* row, int32_t* pick, int32_t* order_r, cudaStream_t st) {
+  ++g_kernel_launches;
+  greedy_pick_kernel<<<1, SEL_T, 0, st>>>(scores, taken, n, row, pick, order_r);
+}
+
 void launch_fuse(const float* raw, const float* train, int n, int n_train, float beta_d, float* denom, float* fused, int32_t* best,
                  cudaStream_t st) {
   ++g_kernel_launches;

@@ -62,8 +62,10 @@ def test_fused_argument_errors():
     assert e.value.status == "NBV_ERR_UNKNOWN_TARGET"
 
 
-def test_greedy_selection_matches_the_oracle():
+@pytest.mark.parametrize("cache_mb", ["4096", "0"])      # block cache / fallback that re-rasterises every round
+def test_greedy_selection_matches_the_oracle(cache_mb, monkeypatch):
     from paper_2602_08266_b200 import api
+    monkeypatch.setenv("NBV_GREEDY_CACHE_MB", cache_mb)
     wl = _workload(2, 12)
     nbv = _ctx(wl.scene, api.CH_RGB, wl.train_cams)
     order, scores = nbv.select_greedy(wl.cand_cams, 4)
