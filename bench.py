@@ -60,6 +60,7 @@ def parse_args():
     ap.add_argument("--cpu-sample-views", type=int, default=0, help="oracle sample size (0 = automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--concurrency", type=int, default=0, help="views in flight (0 = library default)")
+    ap.add_argument("--no-selection", action="store_true", help="skip the greedy / fused-output timings (SURVEY 8(f) rows)")
     return ap.parse_args()
 
 
@@ -184,6 +185,46 @@ def workload_config(args, wl, where: str):
 
 
 # --------------------------------------------------------------------------------------------------
+def bench_selection(nbv, wl, api, torch):
+    """The rows SURVEY.md section 8(f) marks "next", timed on the same workload (extra keys, not the headline):
+    greedy selection of 6 views and per-output normalised, fused scoring (Eq. 10-11)."""
+    C, T = len(wl.cand_cams), len(wl.train_cams)
+    rounds = min(6, C)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def fresh(n):
+        n.reset_training()
+        n.accumulate_training(wl.train_cams)
+
+    res = {}
+    nbv.select_greedy(wl.cand_cams, rounds, wl.target_obj, want_scores=False)          # warm-up: pool allocation
+    fresh(nbv)
+    a, b = ev(), ev()
+    a.record()
+    order, _ = nbv.select_greedy(wl.cand_cams, rounds, wl.target_obj, want_scores=False)
+    b.record(); b.synchronize()
+    ms = a.elapsed_time(b)
+    scored = sum(C - r for r in range(rounds))
+    res["greedy"] = {"rounds": rounds, "candidates": C, "ms": ms, "candidate_scorings_per_s": scored / (ms * 1e-3),
+                     "order": [int(i) for i in order], "call": "nbv_select_greedy (every candidate rasterised once, rounds on cached blocks)"}
+    fresh(nbv)
+    n_rgb, n_d = api.NBV(channel_mask=api.CH_RGB), api.NBV(channel_mask=api.CH_DEPTH)
+    for n in (n_rgb, n_d):
+        n.load_scene(wl.scene)
+        n.accumulate_training(wl.train_cams)
+    api.score_candidates_fused(n_rgb, n_d, wl.train_cams, wl.cand_cams, wl.target_obj)  # warm-up
+    a, b = ev(), ev()
+    a.record()
+    out = api.score_candidates_fused(n_rgb, n_d, wl.train_cams, wl.cand_cams, wl.target_obj)
+    b.record(); b.synchronize()
+    ms = a.elapsed_time(b)
+    res["fused"] = {"candidates": C, "training_views_rescored": T, "ms": ms, "views_per_s": C / (ms * 1e-3),
+                    "best": int(out["best"].item()), "denominators": [float(x) for x in out["denom"].cpu()],
+                    "call": "nbv_score_candidates_fused (rgb and depth contexts; candidates and training views scored in both)"}
+    n_rgb.close(); n_d.close()
+    return res
+
+
 def rank_candidates(cfg_index: int, wl, rank: int):
     """Candidate cameras rank `rank` scores: rank 0 keeps the workload's own set; every other replica draws its own set
     of the same size from a rank-seeded generator (same scene, same hemisphere recipe) -- independent units, no exchange."""
@@ -368,6 +409,8 @@ def main():
         "setup": {"load_s": load_s, "training_views_per_s": len(wl.train_cams) / (train_ms * 1e-3) if train_ms else None},
         "best": int(h_best),
     }
+    if world == 1 and not args.no_selection:
+        out["selection"] = bench_selection(nbv, wl, api, torch)
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(wl, args.cpu_sample_views or auto_sample_views(args.config))
     print(json.dumps(out), flush=True)
