@@ -248,3 +248,23 @@ def test_error_codes():
     assert e.value.status == "NBV_ERR_INVALID_ARG"
     with pytest.raises(api.NBVError):
         api.NBV(alpha_min=0.001)  # below 1/255: the support bound is built for 1/255
+
+
+def test_mixed_image_sizes_and_batching_do_not_change_scores(wl):
+    """One scoring call over cameras of two image sizes (the batches split at every size change, the tile-order table is
+    rebuilt) and with 1 / 3 / 8 views in flight gives the scores of one-camera-at-a-time calls (up to the order of the
+    floating-point atomics)."""
+    rng = np.random.default_rng(9)
+    big = synth.hemisphere_cameras(5, (0.6, 0.6), 200, 136, 170.0, 170.0, rng)        # 13 x 9 tiles, ragged
+    small = synth.hemisphere_cameras(6, (0.6, 0.6), 64, 64, 55.43, 55.43, rng)
+    cams = np.concatenate([small[:2], big[:3], small[2:], big[3:]])
+    nbv = _nbv(wl.scene)
+    nbv.accumulate_training(wl.train_cams)
+    single = np.array([float(nbv.score_candidates(cams[i:i + 1])[0].item()) for i in range(len(cams))])
+    for conc in (1, 3, 8):
+        nbv.set_concurrency(conc)
+        s, best = nbv.score_candidates(cams)
+        np.testing.assert_allclose(s.cpu().numpy(), single, rtol=2e-5)
+        assert int(best.item()) == int(np.argmax(single))
+    ref = orc.score_candidates(make_oracle_scene(wl.scene), wl.train_cams, cams[[2, 7]])["scores"]
+    np.testing.assert_allclose(single[[2, 7]], ref, rtol=1e-3, atol=1e-6)
