@@ -2,13 +2,15 @@
 //
 // Two-level binning.  After the depth sort (rank r <-> Gaussian ids_sorted[r]) the splats are
 // gathered into rank order and every rank is duplicated into the SUPERTILES (S x S tiles, S a power of two chosen so
-// that there are at most 256 of them) its tile rectangle touches: keys (supertile << rank_bits | rank) are emitted
-// rank-major, so one stable radix pass on the supertile digit yields, per supertile, the ranks in depth order.
+// that there are at most 256 of them) its tile rectangle touches, by a stable multi-split (count, scan, write): per
+// supertile, the keys (supertile << rank_bits | rank) come out in rank = depth order.
 // The tile list of tile t (R-5: the visible Gaussians whose rect contains t, in depth order) is the sub-sequence of
 // its supertile's list that passes the rect test.  The rasteriser applies that test on the fly and only as far as the
 // tile needs (until all 256 pixels have terminated), so the ~98% of the (tile, Gaussian) pairs that lie behind the
 // termination depth in the dense configs are never materialised.  nbv_tile_lists materialises the full lists with the
 // same test (count, scan, write) for the bit-exact parity check.
+#include <algorithm>
+
 #include "kernels.h"
 
 namespace nbv {
@@ -20,88 +22,113 @@ __device__ __forceinline__ uint32_t coarse_count(ushort4 rc, int sshift) {
   return (sx1 - sx0 + 1u) * (sy1 - sy0 + 1u);
 }
 
-__global__ void __launch_bounds__(256) gather_kernel(const uint32_t* __restrict__ ids_sorted, const Splat* __restrict__ splat,
-                                                      const ushort4* __restrict__ rect, int N, int sshift,
-                                                      Splat* __restrict__ splat_sorted, ushort4* __restrict__ rect_sorted,
-                                                      uint32_t* __restrict__ ncoarse_sorted) {
-  const int r = blockIdx.x * blockDim.x + threadIdx.x;
-  if (r >= N) return;
-  const uint32_t g = ids_sorted[r];
-  const ushort4 rc = rect[g];
-  rect_sorted[r] = rc;
-  ncoarse_sorted[r] = coarse_count(rc, sshift);
-  const float4* src = reinterpret_cast<const float4*>(splat + g);
-  float4* dst = reinterpret_cast<float4*>(splat_sorted + r);
-  dst[0] = src[0];
-  dst[1] = src[1];
-  dst[2] = src[2];
+// tile rect -> inclusive supertile rect (x0, y0, x1, y1); an empty tile rect gives x0 > x1 (covers nothing)
+__device__ __forceinline__ uint4 super_rect(ushort4 rc, int sshift) {
+  if (rc.z <= rc.x || rc.w <= rc.y) return make_uint4(1u, 1u, 0u, 0u);
+  return make_uint4(rc.x >> sshift, rc.y >> sshift, ((uint32_t)rc.z - 1u) >> sshift, ((uint32_t)rc.w - 1u) >> sshift);
+}
+__device__ __forceinline__ bool covers_super(uint4 sr, uint32_t sx, uint32_t sy) {
+  return sx >= sr.x && sx <= sr.z && sy >= sr.y && sy <= sr.w;
 }
 
-void launch_gather(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, int sshift, Splat* splat_sorted,
-                   ushort4* rect_sorted, uint32_t* ncoarse_sorted, cudaStream_t st) {
-  ++g_kernel_launches;
-  gather_kernel<<<(N + 255) / 256, 256, 0, st>>>(ids_sorted, splat, rect, N, sshift, splat_sorted, rect_sorted, ncoarse_sorted);
+// Stable multi-split of the ranks into supertile lists, without materialising unsorted keys: block b owns the ranks
+// [b * MS_T, (b + 1) * MS_T).  Pass 1 (this kernel, fused with the gather of the splats into rank order) counts, per
+// supertile, the block's ranks that touch it; an exclusive scan of the (supertile-major) count table gives the start of
+// every (supertile, block) segment; pass 2 writes each (supertile, rank) key and its tile rect at
+// segment start + (number of earlier ranks of the block touching the same supertile), found with warp ballots.
+// Rank order inside a supertile is preserved by construction: the lists are in depth order.
+constexpr int MS_T = 1024;
+constexpr int MS_W = MS_T / 32;
+
+__global__ void __launch_bounds__(MS_T) msplit_count_kernel(const uint32_t* __restrict__ ids_sorted, const Splat* __restrict__ splat,
+                                                            const ushort4* __restrict__ rect, int N, int sshift, int super_x, int n_super,
+                                                            Splat* __restrict__ splat_sorted, ushort4* __restrict__ rect_sorted,
+                                                            uint32_t* __restrict__ counts, uint32_t nblk) {
+  __shared__ uint32_t cnt[256];
+  const int r = blockIdx.x * MS_T + threadIdx.x, lane = threadIdx.x & 31;
+  if (threadIdx.x < 256) cnt[threadIdx.x] = 0;
+  __syncthreads();
+  ushort4 rc = make_ushort4(0, 0, 0, 0);
+  if (r < N) {
+    const uint32_t g = ids_sorted[r];
+    rc = rect[g];
+    rect_sorted[r] = rc;
+    const float4* src = reinterpret_cast<const float4*>(splat + g);
+    float4* dst = reinterpret_cast<float4*>(splat_sorted + r);
+    dst[0] = src[0];
+    dst[1] = src[1];
+    dst[2] = src[2];
+  }
+  const uint4 sr = super_rect(rc, sshift);
+  for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {            // (sx, sy) walk the supertiles row-major: no division
+    const unsigned m = __ballot_sync(0xffffffffu, covers_super(sr, (uint32_t)sx, (uint32_t)sy));
+    if (lane == 0 && m) atomicAdd(&cnt[s], (uint32_t)__popc(m));
+    if (++sx == super_x) { sx = 0; ++sy; }
+  }
+  __syncthreads();
+  if ((int)threadIdx.x < n_super) counts[(size_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
 }
 
-// 8 ranks per warp (4 lanes each): a rank touches a handful of supertiles
-__global__ void __launch_bounds__(256) emit_coarse_kernel(const ushort4* __restrict__ rect_sorted, const uint32_t* __restrict__ offsets,
-                                                           int N, int sshift, int super_x, int rank_bits, uint32_t cap,
-                                                           uint32_t* __restrict__ keys) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  const int r = t >> 2, sub = t & 3;
-  if (r >= N) return;
-  const ushort4 rc = rect_sorted[r];
-  if (rc.z <= rc.x || rc.w <= rc.y) return;
-  const uint32_t sx0 = rc.x >> sshift, sx1 = ((uint32_t)rc.z - 1u) >> sshift;
-  const uint32_t sy0 = rc.y >> sshift, sy1 = ((uint32_t)rc.w - 1u) >> sshift;
-  const uint32_t w = sx1 - sx0 + 1u, n = w * (sy1 - sy0 + 1u);
-  const uint32_t off = offsets[r];
-  for (uint32_t i = sub; i < n; i += 4) {
-    const uint32_t sy = sy0 + i / w, sx = sx0 + i % w;
-    if (off + i < cap) keys[off + i] = ((sy * (uint32_t)super_x + sx) << rank_bits) | (uint32_t)r;
+__global__ void __launch_bounds__(MS_T) msplit_write_kernel(const ushort4* __restrict__ rect_sorted, int N, int sshift, int super_x,
+                                                            int n_super, int rank_bits, const uint32_t* __restrict__ scanned, uint32_t nblk,
+                                                            const uint32_t* __restrict__ d_total, uint32_t cap,
+                                                            uint32_t* __restrict__ keys, ushort4* __restrict__ crect,
+                                                            uint2* __restrict__ ranges) {
+  __shared__ uint16_t wc[256][MS_W];         // per supertile: ranks of warp w touching it, then the exclusive prefix over warps
+  const int r = blockIdx.x * MS_T + threadIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const uint32_t lt = (1u << lane) - 1u;
+  const ushort4 rc = r < N ? rect_sorted[r] : make_ushort4(0, 0, 0, 0);
+  const uint4 sr = super_rect(rc, sshift);
+  for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {
+    const unsigned m = __ballot_sync(0xffffffffu, covers_super(sr, (uint32_t)sx, (uint32_t)sy));
+    if (lane == 0) wc[s][w] = (uint16_t)__popc(m);
+    if (++sx == super_x) { sx = 0; ++sy; }
+  }
+  __syncthreads();
+  if ((int)threadIdx.x < n_super) {
+    uint32_t run = 0;
+    for (int k = 0; k < MS_W; ++k) {
+      const uint32_t c = wc[threadIdx.x][k];
+      wc[threadIdx.x][k] = (uint16_t)run;
+      run += c;
+    }
+    if (blockIdx.x == 0) {                    // supertile ranges: [start of (s, block 0), start of (s + 1, block 0))
+      const uint32_t b = scanned[(size_t)threadIdx.x * nblk];
+      const uint32_t e = ((int)threadIdx.x + 1 < n_super) ? scanned[(size_t)(threadIdx.x + 1) * nblk] : min(*d_total, cap);
+      ranges[threadIdx.x] = make_uint2(b, e);
+    }
+  }
+  __syncthreads();
+  for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {
+    const bool c = covers_super(sr, (uint32_t)sx, (uint32_t)sy);
+    const unsigned m = __ballot_sync(0xffffffffu, c);
+    if (++sx == super_x) { sx = 0; ++sy; }
+    if (c) {
+      const uint32_t pos = scanned[(size_t)s * nblk + blockIdx.x] + wc[s][w] + __popc(m & lt);
+      if (pos < cap) {
+        keys[pos] = ((uint32_t)s << rank_bits) | (uint32_t)r;
+        crect[pos] = rc;
+      }
+    }
   }
 }
 
-void launch_emit_coarse(const ushort4* rect_sorted, const uint32_t* offsets, int N, int sshift, int super_x, int rank_bits,
-                        uint32_t cap, uint32_t* keys, cudaStream_t st) {
-  const long long threads = (long long)N * 4;
+uint32_t msplit_blocks(int N) { return (uint32_t)((N + MS_T - 1) / MS_T); }
+
+void launch_msplit_count(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, const TileGrid& tg, Splat* splat_sorted,
+                         ushort4* rect_sorted, uint32_t* counts, cudaStream_t st) {
+  const uint32_t nblk = msplit_blocks(N);
   ++g_kernel_launches;
-  emit_coarse_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(rect_sorted, offsets, N, sshift, super_x, rank_bits, cap, keys);
+  msplit_count_kernel<<<nblk, MS_T, 0, st>>>(ids_sorted, splat, rect, N, tg.sshift, tg.super_x, tg.super_x * tg.super_y, splat_sorted,
+                                             rect_sorted, counts, nblk);
 }
 
-// After the single stable pass on the supertile digit the scanned histogram holds every digit's start:
-// range of supertile s = [hist[s * nb], hist[(s + 1) * nb]) (the last one ends at n).
-__global__ void __launch_bounds__(256) coarse_ranges_kernel(const uint32_t* __restrict__ hist_scanned, uint32_t nb, int n_super,
-                                                             int n_digits, const uint32_t* __restrict__ d_n, uint32_t cap,
-                                                             uint2* __restrict__ ranges) {
-  const int s = threadIdx.x;
-  if (s >= n_super) return;
-  const uint32_t n = min(*d_n, cap);
-  const uint32_t b = hist_scanned[(size_t)s * nb];
-  const uint32_t e = (s + 1 < n_digits) ? hist_scanned[(size_t)(s + 1) * nb] : n;
-  ranges[s] = make_uint2(b, e);
-}
-
-void launch_coarse_ranges(const uint32_t* hist_scanned, uint32_t nb, int n_super, int n_digits, const uint32_t* d_n, uint32_t cap,
-                          uint2* ranges, cudaStream_t st) {
+void launch_msplit_write(const ushort4* rect_sorted, int N, const TileGrid& tg, int rank_bits, const uint32_t* scanned,
+                         const uint32_t* d_total, uint32_t cap, uint32_t* keys, ushort4* crect, uint2* ranges, cudaStream_t st) {
+  const uint32_t nblk = msplit_blocks(N);
   ++g_kernel_launches;
-  coarse_ranges_kernel<<<1, 256, 0, st>>>(hist_scanned, nb, n_super, n_digits, d_n, cap, ranges);
-}
-
-// rect of every sorted coarse entry, in list order (coalesced reads for the rasteriser's rect test)
-__global__ void __launch_bounds__(256) coarse_rect_kernel(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ d_n, uint32_t cap,
-                                                           uint32_t rmask, const ushort4* __restrict__ rect_sorted,
-                                                           ushort4* __restrict__ crect) {
-  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= min(*d_n, cap)) return;
-  crect[i] = rect_sorted[keys[i] & rmask];
-}
-
-void launch_coarse_rect(const uint32_t* keys, const uint32_t* d_n, uint32_t cap, int rank_bits, const ushort4* rect_sorted,
-                        ushort4* crect, cudaStream_t st) {
-  if (cap == 0) return;
-  ++g_kernel_launches;
-  coarse_rect_kernel<<<(cap + 255) / 256, 256, 0, st>>>(keys, d_n, cap, (1u << rank_bits) - 1u, rect_sorted, crect);
+  msplit_write_kernel<<<nblk, MS_T, 0, st>>>(rect_sorted, N, tg.sshift, tg.super_x, tg.super_x * tg.super_y, rank_bits, scanned, nblk,
+                                             d_total, cap, keys, crect, ranges);
 }
 
 // ---- parity export: the full tile lists (R-5), by the same rect test the rasteriser applies on the fly.

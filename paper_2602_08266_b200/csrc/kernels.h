@@ -36,14 +36,14 @@ void launch_project(const SceneDev& sc, const nbv_camera& cam, const nbv_config&
                     uint32_t* ids, ushort4* rect, float* abc, ViewCounters* counters, cudaStream_t st);
 
 // ---- binning.cu
-void launch_gather(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, int sshift, Splat* splat_sorted,
-                   ushort4* rect_sorted, uint32_t* ncoarse_sorted, cudaStream_t st);
-void launch_emit_coarse(const ushort4* rect_sorted, const uint32_t* offsets, int N, int sshift, int super_x, int rank_bits,
-                        uint32_t cap, uint32_t* keys, cudaStream_t st);
-void launch_coarse_ranges(const uint32_t* hist_scanned, uint32_t nb, int n_super, int n_digits, const uint32_t* d_n, uint32_t cap,
-                          uint2* ranges, cudaStream_t st);
-void launch_coarse_rect(const uint32_t* keys, const uint32_t* d_n, uint32_t cap, int rank_bits, const ushort4* rect_sorted,
-                        ushort4* crect, cudaStream_t st);
+// stable multi-split of the depth ranks into supertile lists: pass 1 (with the gather of the splats into rank order) fills
+// the supertile-major count table counts[s * msplit_blocks(N) + block]; after an exclusive scan of that table (total =
+// number of coarse entries) pass 2 writes keys (supertile << rank_bits | rank), their tile rects and the supertile ranges
+uint32_t msplit_blocks(int N);
+void launch_msplit_count(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, const TileGrid& tg, Splat* splat_sorted,
+                         ushort4* rect_sorted, uint32_t* counts, cudaStream_t st);
+void launch_msplit_write(const ushort4* rect_sorted, int N, const TileGrid& tg, int rank_bits, const uint32_t* scanned,
+                         const uint32_t* d_total, uint32_t cap, uint32_t* keys, ushort4* crect, uint2* ranges, cudaStream_t st);
 // parity export of the full tile lists: counts -> scanned offsets (+ total) -> ids
 void launch_tile_counts(const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg, int rank_bits,
                         uint32_t* counts, uint32_t* scanned, uint32_t* total, uint32_t* scan_tmp, int64_t* offsets_out, cudaStream_t st);

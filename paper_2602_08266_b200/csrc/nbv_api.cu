@@ -31,8 +31,8 @@ struct DevBuf {
 struct ViewSlot {
   cudaStream_t st = nullptr;
   cudaEvent_t done = nullptr;
-  DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, ncoarse, offsets;
-  DevBuf ckeys, ckeys_alt, crect, cranges, sort_tmp, scan_tmp, tile_counts;
+  DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, msplit;
+  DevBuf ckeys, crect, cranges, sort_tmp, scan_tmp, tile_counts;
   DevBuf pix_rgb, pix_depth, pix_T, pix_nc, pix_last, tile_cend, tile_walk, moments, touched;
   ViewCounters* d_counters = nullptr;
   ViewCounters* h_counters = nullptr;   // pinned
@@ -210,7 +210,7 @@ int span_next(nbv_ctx* ctx, int idx, int stage, int views, cudaStream_t st) {
 void free_slot(ViewSlot* sl) {
   if (!sl) return;
   DevBuf* all[] = {&sl->splat, &sl->zkey, &sl->zkey_alt, &sl->ids, &sl->ids_alt, &sl->rect, &sl->abc, &sl->splat_sorted,
-                   &sl->rect_sorted, &sl->ncoarse, &sl->offsets, &sl->ckeys, &sl->ckeys_alt, &sl->crect, &sl->cranges, &sl->sort_tmp,
+                   &sl->rect_sorted, &sl->msplit, &sl->ckeys, &sl->crect, &sl->cranges, &sl->sort_tmp,
                    &sl->scan_tmp, &sl->tile_counts, &sl->pix_rgb, &sl->pix_depth, &sl->pix_T, &sl->pix_nc, &sl->pix_last,
                    &sl->tile_cend, &sl->tile_walk, &sl->moments, &sl->touched};
   for (DevBuf* b : all) release(*b);
@@ -287,14 +287,14 @@ int pre_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool w
   CKRET(ensure(ctx, sl->ids, 4 * (size_t)N)); CKRET(ensure(ctx, sl->ids_alt, 4 * (size_t)N));
   CKRET(ensure(ctx, sl->rect, sizeof(ushort4) * (size_t)N));
   if (want_abc) CKRET(ensure(ctx, sl->abc, 12 * (size_t)N));
-  CKRET(ensure(ctx, sl->sort_tmp, 4 * radix_temp_words(std::max((size_t)N, (size_t)ccap))));
+  CKRET(ensure(ctx, sl->sort_tmp, 4 * radix_temp_words((size_t)N)));
   CKRET(ensure(ctx, sl->scan_tmp, 4 * scan_temp_words(std::max((size_t)N + 1, (size_t)n_tiles + 1))));
   if (upto >= STAGE_BIN) {
     CKRET(ensure(ctx, sl->splat_sorted, sizeof(Splat) * (size_t)N));
     CKRET(ensure(ctx, sl->rect_sorted, sizeof(ushort4) * (size_t)N));
-    CKRET(ensure(ctx, sl->ncoarse, 4 * (size_t)N));
-    CKRET(ensure(ctx, sl->offsets, 4 * (size_t)N));
-    CKRET(ensure(ctx, sl->ckeys, 4 * (size_t)ccap)); CKRET(ensure(ctx, sl->ckeys_alt, 4 * (size_t)ccap));
+    const size_t n_counts = (size_t)n_super * msplit_blocks(N);
+    CKRET(ensure(ctx, sl->msplit, 4 * (n_counts + scan_temp_words(n_counts))));
+    CKRET(ensure(ctx, sl->ckeys, 4 * (size_t)ccap));
     CKRET(ensure(ctx, sl->crect, sizeof(ushort4) * (size_t)ccap));
     CKRET(ensure(ctx, sl->cranges, sizeof(uint2) * 256));
   }
@@ -334,23 +334,17 @@ int pre_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool w
     }
     CK(cudaGetLastError());
   }
-  // coarse binning: rank-ordered splats, supertile counts, scan, keys (supertile | rank) emitted rank-major
+  // coarse binning: rank-ordered splats + per-(supertile, rank block) counts | scan | keys, rects and supertile ranges
   sp = span_next(ctx, sp, NBV_STAGE_BIN, 1, st);
-  launch_gather(sl->ids.as<uint32_t>(), sl->splat.as<Splat>(), sl->rect.as<ushort4>(), N, tg.sshift, sl->splat_sorted.as<Splat>(),
-                sl->rect_sorted.as<ushort4>(), sl->ncoarse.as<uint32_t>(), st);
-  exclusive_scan_u32(sl->ncoarse.as<uint32_t>(), sl->offsets.as<uint32_t>(), (size_t)N, sl->scan_tmp.as<uint32_t>(),
-                     &sl->d_counters->n_coarse, st);
-  launch_emit_coarse(sl->rect_sorted.as<ushort4>(), sl->offsets.as<uint32_t>(), N, tg.sshift, tg.super_x, rank_bits, ccap,
-                     sl->ckeys.as<uint32_t>(), st);
-  // one stable pass on the supertile digit (<= 8 bits); its scanned histogram gives the supertile ranges
+  const size_t n_counts = (size_t)n_super * msplit_blocks(N);
+  uint32_t* counts = sl->msplit.as<uint32_t>();
+  launch_msplit_count(sl->ids.as<uint32_t>(), sl->splat.as<Splat>(), sl->rect.as<ushort4>(), N, tg, sl->splat_sorted.as<Splat>(),
+                      sl->rect_sorted.as<ushort4>(), counts, st);
   sp = span_next(ctx, sp, NBV_STAGE_COARSE_SORT, 1, st);
-  radix_pass(sl->ckeys.as<uint32_t>(), sl->ckeys_alt.as<uint32_t>(), nullptr, nullptr, (size_t)ccap, &sl->d_counters->n_coarse,
-             rank_bits, super_bits, sl->sort_tmp.as<uint32_t>(), st);
-  sl->ckeys_sorted = sl->ckeys_alt.as<uint32_t>();
-  launch_coarse_ranges(sl->sort_tmp.as<uint32_t>(), radix_blocks((size_t)ccap), n_super, 1 << super_bits, &sl->d_counters->n_coarse,
-                       ccap, sl->cranges.as<uint2>(), st);
-  launch_coarse_rect(sl->ckeys_sorted, &sl->d_counters->n_coarse, ccap, rank_bits, sl->rect_sorted.as<ushort4>(),
-                     sl->crect.as<ushort4>(), st);
+  exclusive_scan_u32(counts, counts, n_counts, counts + n_counts, &sl->d_counters->n_coarse, st);
+  launch_msplit_write(sl->rect_sorted.as<ushort4>(), N, tg, rank_bits, counts, &sl->d_counters->n_coarse, ccap, sl->ckeys.as<uint32_t>(),
+                      sl->crect.as<ushort4>(), sl->cranges.as<uint2>(), st);
+  sl->ckeys_sorted = sl->ckeys.as<uint32_t>();
   CK(cudaGetLastError());
   span_end(ctx, sp, st);
   return NBV_OK;

@@ -85,6 +85,32 @@ __global__ void __launch_bounds__(SCAN_T) scan_downsweep_kernel(const uint32_t* 
   if (total_out && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *total_out = (offsets ? offsets[blockIdx.x] : 0u) + total;
 }
 
+// Whole scan in ONE block (n up to a few tens of thousands: the digit histograms of the depth sort), so that a radix
+// pass is three dependent launches instead of five: the S1-S2 chain of a batch is latency bound.
+constexpr int SCAN1_T = 1024;
+constexpr uint32_t SCAN1_MAX = 32768;
+
+__global__ void __launch_bounds__(SCAN1_T) scan_single_block_kernel(const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* __restrict__ total_out) {
+  __shared__ uint32_t sm[32];
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < n; base += SCAN1_T * 4) {
+    const uint32_t i0 = base + threadIdx.x * 4;
+    uint32_t v[4];
+    uint32_t s = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { v[i] = i0 + i < n ? in[i0 + i] : 0u; s += v[i]; }
+    uint32_t total;
+    uint32_t off = carry + block_exclusive_scan(s, sm, total);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      if (i0 + i < n) out[i0 + i] = off;
+      off += v[i];
+    }
+    carry += total;
+  }
+  if (total_out && threadIdx.x == 0) *total_out = carry;
+}
+
 size_t scan_temp_words(size_t n) {
   size_t words = 0;
   while (n > (size_t)SCAN_TILE) {
@@ -100,6 +126,11 @@ void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* t
     return;
   }
   const uint32_t nb = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
+  if (nb > 1 && n <= SCAN1_MAX) {
+    ++g_kernel_launches;
+    scan_single_block_kernel<<<1, SCAN1_T, 0, st>>>(in, out, (uint32_t)n, total_out);
+    return;
+  }
   if (nb == 1) {
     ++g_kernel_launches;
     scan_downsweep_kernel<<<1, SCAN_T, 0, st>>>(in, out, (uint32_t)n, nullptr, total_out);
