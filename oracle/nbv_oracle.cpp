@@ -472,6 +472,83 @@ inline void pixel_value(const Config& cfg, double px, double py, const Contrib* 
 // ---------------------------------------------------------------------------
 // scene object
 // ---------------------------------------------------------------------------
+// ---------------------------------------------------------------------------
+// Object-mask output.
+//   O' = sum_i softmax(o_i) alpha_i T_i                                  P:L125-129 (Eq. 1)
+//   O  = O' + e_bg (1 - 1^T O') = O' + e_bg T_end   (softmax sums to 1)  P:L135-139 (Eq. 2)
+// "masks use the object vector" next to position, scale, rotation and opacity: the
+// block of a Gaussian has L = 11 + K parameters [mu(3) logscale(3) quat(4) opacity | logits(K)],
+// packed upper triangle row-major, idx(r,c) = r*L - r(r-1)/2 + (c-r).
+// Row of output channel k for contributor i:
+//   J_k = beta_k * dalpha_i/dtheta_geo  (+)  w_i * dp_k/do,   dp_k/do_j = p_k (delta_kj - p_j),
+//   beta_k = T_i p_ik - Splus_k / (1 - alpha_i),  Splus = sum_{j>i} p_j w_j + e_bg T_end.
+// Explicit rows, dense J^T J: no moment factorisation (the CUDA path has one).
+// ---------------------------------------------------------------------------
+inline size_t triL(int r, int c, int L) { return (size_t)r * L - (size_t)r * (r - 1) / 2 + (size_t)(c - r); }
+
+// prob: N x K softmax probabilities (binary64).  outK: K mask values of the pixel.
+// hadd(g) -> pointer to that Gaussian's L(L+1)/2 packed doubles, or nullptr to skip.
+template <class HAdd>
+inline void pixel_value_mask(const Config& cfg, int K, int bgch, double px, double py, const Contrib* cs, int n,
+                             const SplatV* sv, const Chain* chains, const double* prob, double* outK, double& Tend,
+                             bool want_hessian, HAdd&& hadd) {
+  const double amax = (double)cfg.alpha_max;
+  const int L = 11 + K;
+  std::vector<double> al(n), Ti(n);
+  double T = 1.0;
+  for (int k = 0; k < K; ++k) outK[k] = 0.0;
+  for (int i = 0; i < n; ++i) {
+    const SplatV& s = sv[cs[i].g];
+    double dx = px - s.mx, dy = py - s.my;
+    double power = -0.5 * (s.ca * dx * dx + s.cc * dy * dy) - s.cb * dx * dy;
+    double a = cs[i].clamped ? amax : s.sigma * std::exp(power);
+    al[i] = a;
+    Ti[i] = T;
+    const double w = a * T;
+    const double* p = prob + (size_t)cs[i].g * K;
+    for (int k = 0; k < K; ++k) outK[k] += p[k] * w;
+    T *= (1.0 - a);
+  }
+  Tend = T;
+  outK[bgch] += T;                                           // Eq. 2: the residual goes to the background channel
+  if (!want_hessian) return;
+  std::vector<double> Sp(K, 0.0), beta(K), Jr(L), da(11);
+  Sp[bgch] = T;
+  for (int i = n - 1; i >= 0; --i) {
+    const int g = cs[i].g;
+    const SplatV& s = sv[g];
+    const double* p = prob + (size_t)g * K;
+    const double a = al[i], w = a * Ti[i];
+    for (int k = 0; k < K; ++k) beta[k] = Ti[i] * p[k] - Sp[k] / (1.0 - a);
+    for (int k = 0; k < K; ++k) Sp[k] += p[k] * w;
+    double* H = hadd(g);
+    if (!H) continue;
+    for (int k = 0; k < 11; ++k) da[k] = 0.0;
+    if (!cs[i].clamped) {                                    // R-11: zero derivative at the 0.99 clamp
+      double dx = px - s.mx, dy = py - s.my;
+      double ux = s.ca * dx + s.cb * dy, uy = s.cb * dx + s.cc * dy;
+      const double h5[5] = {a * ux, a * uy, 0.5 * a * ux * ux, a * ux * uy, 0.5 * a * uy * uy};
+      const Chain& ch = chains[g];
+      for (int k = 0; k < 10; ++k) {
+        double acc2 = 0;
+        for (int e = 0; e < 5; ++e) acc2 += h5[e] * ch.G[e][k];
+        da[k] = acc2;
+      }
+      da[10] = cfg.opacity_coord == 0 ? a * (1.0 - s.sigma) : a / s.sigma;   // R-10
+    }
+    for (int k = 0; k < K; ++k) {
+      for (int r = 0; r < 11; ++r) Jr[r] = beta[k] * da[r];
+      for (int j = 0; j < K; ++j) Jr[11 + j] = w * p[k] * ((j == k ? 1.0 : 0.0) - p[j]);   // softmax Jacobian
+      for (int r = 0; r < L; ++r) {
+        const double jr = Jr[r];
+        if (jr == 0.0) continue;
+        double* row = H + triL(r, r, L);
+        for (int c = r; c < L; ++c) row[c - r] += jr * Jr[c];
+      }
+    }
+  }
+}
+
 struct Scene {
   int N = 0, K = 0;
   std::vector<float> mean, logscale, quat, opacity, rgb;
@@ -801,6 +878,122 @@ void orc_chain(const Camera* cam, const Config* cfg, const double* theta14, doub
   for (int e = 0; e < 5; ++e)
     for (int k = 0; k < 10; ++k) G50[10 * e + k] = ch.G[e][k];
   for (int k = 0; k < 3; ++k) dz3[k] = ch.dz[k];
+}
+
+// ---- object-mask output (NEXT-2) -------------------------------------------------------------------
+// prob: N x K softmax probabilities.  out: H*W*K mask values (Eq. 1-2).
+void orc_render_mask(void* h, const Camera* cam, int K, int bgch, const double* prob, double* out) {
+  Scene* sc = (Scene*)h;
+  View v = make_view(*sc, *cam);
+  std::vector<SplatV> sv;
+  fill_splatv(*sc, v, sv);
+  const int W = cam->width, H = cam->height;
+#pragma omp parallel
+  {
+    std::vector<Contrib> cs;
+#pragma omp for schedule(dynamic, 1)
+    for (int iy = 0; iy < H; ++iy)
+      for (int ix = 0; ix < W; ++ix) {
+        float t32;
+        walk_pixel(*sc, v, ix, iy, cs, t32);
+        double Tend;
+        pixel_value_mask(sc->cfg, K, bgch, ix + 0.5, iy + 0.5, cs.data(), (int)cs.size(), sv.data(), nullptr, prob,
+                         out + ((size_t)iy * W + ix) * K, Tend, false, [](int) -> double* { return nullptr; });
+      }
+  }
+}
+
+// blocks (N x L(L+1)/2 doubles, L = 11 + K) += sum over pixels and mask channels of J^T J.  Rows of the image are
+// processed serially per thread into a private copy (small scenes only: this is for parity tests).
+void orc_view_hessian_mask(void* h, const Camera* cam, int K, int bgch, const double* prob, double* blocks) {
+  Scene* sc = (Scene*)h;
+  View v = make_view(*sc, *cam);
+  std::vector<SplatV> sv;
+  fill_splatv(*sc, v, sv);
+  std::vector<Chain> chains(sc->N);
+  for (int g = 0; g < sc->N; ++g) {
+    if (!v.sp[g].visible) continue;
+    double mu[3], ls[3], q[4];
+    for (int k = 0; k < 3; ++k) { mu[k] = sc->mean[3 * g + k]; ls[k] = sc->logscale[3 * g + k]; }
+    for (int k = 0; k < 4; ++k) q[k] = sc->quat[4 * g + k];
+    chains[g] = chain(*cam, sc->cfg, mu, ls, q);
+  }
+  const int W = cam->width, H = cam->height, L = 11 + K;
+  const size_t LB = (size_t)L * (L + 1) / 2;
+#pragma omp parallel
+  {
+    std::vector<double> priv((size_t)sc->N * LB, 0.0);
+    std::vector<Contrib> cs;
+    std::vector<double> outK(K);
+#pragma omp for schedule(dynamic, 1)
+    for (int iy = 0; iy < H; ++iy)
+      for (int ix = 0; ix < W; ++ix) {
+        float t32;
+        walk_pixel(*sc, v, ix, iy, cs, t32);
+        double Tend;
+        pixel_value_mask(sc->cfg, K, bgch, ix + 0.5, iy + 0.5, cs.data(), (int)cs.size(), sv.data(), chains.data(), prob,
+                         outK.data(), Tend, true, [&](int g) -> double* { return priv.data() + (size_t)g * LB; });
+      }
+#pragma omp critical
+    for (size_t i = 0; i < priv.size(); ++i) blocks[i] += priv[i];
+  }
+}
+
+// smooth mode (finite-difference self-test): theta N x 11 = [mu | logscale | quat raw | opacity logit], logits N x K
+static void smooth_setup_mask(int N, int K, const double* theta11, const double* logits, const Camera* cam, const Config* cfg,
+                              std::vector<SplatV>& sv, std::vector<Chain>& chains, std::vector<double>& prob) {
+  std::vector<double> th14((size_t)N * P, 0.0);
+  for (int g = 0; g < N; ++g)
+    for (int k = 0; k < 11; ++k) th14[(size_t)g * P + k] = theta11[(size_t)g * 11 + k];
+  smooth_setup(N, th14.data(), cam, cfg, sv, chains);
+  prob.resize((size_t)N * K);
+  for (int g = 0; g < N; ++g) {
+    const double* o = logits + (size_t)g * K;
+    double m = o[0];
+    for (int k = 1; k < K; ++k) m = std::max(m, o[k]);
+    double z = 0;
+    for (int k = 0; k < K; ++k) z += std::exp(o[k] - m);
+    for (int k = 0; k < K; ++k) prob[(size_t)g * K + k] = std::exp(o[k] - m) / z;
+  }
+}
+
+void orc_render_mask_smooth(int N, int K, int bgch, const double* theta11, const double* logits, const Camera* cam,
+                            const Config* cfg, const int64_t* offsets, const int32_t* ids, const uint8_t* clamped, double* out) {
+  std::vector<SplatV> sv; std::vector<Chain> chains; std::vector<double> prob;
+  smooth_setup_mask(N, K, theta11, logits, cam, cfg, sv, chains, prob);
+  const int W = cam->width, H = cam->height;
+  std::vector<Contrib> cs;
+  for (int iy = 0; iy < H; ++iy)
+    for (int ix = 0; ix < W; ++ix) {
+      size_t p = (size_t)iy * W + ix;
+      cs.clear();
+      for (int64_t i = offsets[p]; i < offsets[p + 1]; ++i) cs.push_back({ids[i], clamped[i] != 0});
+      double Tend;
+      pixel_value_mask(*cfg, K, bgch, ix + 0.5, iy + 0.5, cs.data(), (int)cs.size(), sv.data(), nullptr, prob.data(), out + p * K,
+                       Tend, false, [](int) -> double* { return nullptr; });
+    }
+}
+
+void orc_view_hessian_mask_smooth(int N, int K, int bgch, const double* theta11, const double* logits, const Camera* cam,
+                                  const Config* cfg, const int64_t* offsets, const int32_t* ids, const uint8_t* clamped,
+                                  double* blocks) {
+  std::vector<SplatV> sv; std::vector<Chain> chains; std::vector<double> prob;
+  smooth_setup_mask(N, K, theta11, logits, cam, cfg, sv, chains, prob);
+  const int L = 11 + K;
+  const size_t LB = (size_t)L * (L + 1) / 2;
+  std::fill(blocks, blocks + (size_t)N * LB, 0.0);
+  const int W = cam->width, H = cam->height;
+  std::vector<Contrib> cs;
+  std::vector<double> outK(K);
+  for (int iy = 0; iy < H; ++iy)
+    for (int ix = 0; ix < W; ++ix) {
+      size_t p = (size_t)iy * W + ix;
+      cs.clear();
+      for (int64_t i = offsets[p]; i < offsets[p + 1]; ++i) cs.push_back({ids[i], clamped[i] != 0});
+      double Tend;
+      pixel_value_mask(*cfg, K, bgch, ix + 0.5, iy + 0.5, cs.data(), (int)cs.size(), sv.data(), chains.data(), prob.data(),
+                       outK.data(), Tend, true, [&](int g) -> double* { return blocks + (size_t)g * LB; });
+    }
 }
 
 int orc_num_threads() {

@@ -215,6 +215,91 @@ class OracleScene:
         return th
 
 
+# ---- object-mask output (Eq. 1-2) -----------------------------
+def mask_block_size(K: int) -> int:
+    L = 11 + K
+    return L * (L + 1) // 2
+
+
+def unpack_blocks_L(packed: np.ndarray, L: int) -> np.ndarray:
+    iu = np.triu_indices(L)
+    packed = np.asarray(packed, dtype=np.float64)
+    full = np.zeros(packed.shape[:-1] + (L, L))
+    full[..., iu[0], iu[1]] = packed
+    full[..., iu[1], iu[0]] = packed
+    return full
+
+
+def render_mask(scene: "OracleScene", cam, bg_channel: int = 0) -> np.ndarray:
+    """(H,W,K) per-pixel object vector: O' = sum_i softmax(o_i) alpha_i T_i (Eq. 1) plus the residual 1 - 1^T O' on the
+    background channel (Eq. 2)."""
+    cam = _cam(cam)
+    W, H = _wh(cam)
+    prob = np.ascontiguousarray(softmax(scene.obj_logits))
+    out = np.zeros((H, W, scene.K))
+    lib().orc_render_mask(scene._h, _p(cam), scene.K, int(bg_channel), _p(prob), _p(out))
+    return out
+
+
+def view_hessian_mask(scene: "OracleScene", cam, bg_channel: int = 0, out=None) -> np.ndarray:
+    """(N, L(L+1)/2), L = 11 + K: packed J^T J blocks of the mask output w.r.t. [mu, logscale, quat, opacity | logits];
+    accumulates into `out`."""
+    cam = _cam(cam)
+    prob = np.ascontiguousarray(softmax(scene.obj_logits))
+    if out is None:
+        out = np.zeros((scene.N, mask_block_size(scene.K)))
+    lib().orc_view_hessian_mask(scene._h, _p(cam), scene.K, int(bg_channel), _p(prob), _p(out))
+    return out
+
+
+def render_mask_smooth(theta11, logits, cam, cfg, offsets, ids, clamped, bg_channel: int = 0) -> np.ndarray:
+    cam = _cam(cam)
+    theta11 = np.ascontiguousarray(theta11, dtype=np.float64)
+    logits = np.ascontiguousarray(logits, dtype=np.float64)
+    W, H = _wh(cam)
+    N, K = logits.shape
+    out = np.zeros((H, W, K))
+    lib().orc_render_mask_smooth(N, K, int(bg_channel), _p(theta11), _p(logits), _p(cam), C.byref(cfg), _p(offsets), _p(ids),
+                                 _p(clamped), _p(out))
+    return out
+
+
+def view_hessian_mask_smooth(theta11, logits, cam, cfg, offsets, ids, clamped, bg_channel: int = 0) -> np.ndarray:
+    cam = _cam(cam)
+    theta11 = np.ascontiguousarray(theta11, dtype=np.float64)
+    logits = np.ascontiguousarray(logits, dtype=np.float64)
+    N, K = logits.shape
+    out = np.zeros((N, mask_block_size(K)))
+    lib().orc_view_hessian_mask_smooth(N, K, int(bg_channel), _p(theta11), _p(logits), _p(cam), C.byref(cfg), _p(offsets),
+                                       _p(ids), _p(clamped), _p(out))
+    return out
+
+
+def gaussian_gains_L(H_T, H_c, c, prior, L: int) -> np.ndarray:
+    """gaussian_gains for blocks of L x L parameters (prior: L diagonal entries of Lambda)."""
+    Lam = np.diag(np.asarray(prior, dtype=np.float64))
+    A, B = unpack_blocks_L(H_T, L), unpack_blocks_L(H_c, L)
+    c = np.asarray(c, dtype=np.float64)[:, None, None]
+    s1, l1 = np.linalg.slogdet(c * (A + B) + Lam)
+    s0, l0 = np.linalg.slogdet(c * A + Lam)
+    assert np.all(s1 > 0) and np.all(s0 > 0)
+    return l1 - l0
+
+
+def score_candidates_mask(scene: "OracleScene", train_cams, cand_cams, target=-1, alpha_obj=0.3, alpha_opa=0.3, prior=None,
+                          bg_channel: int = 0):
+    """IG_o(T, c) (Eq. 5, 6, 9 on the mask output's blocks).  Returns dict(H_T, scores, best)."""
+    L = 11 + scene.K
+    prior = np.ones(L) if prior is None else np.asarray(prior, dtype=np.float64)
+    H_T = np.zeros((scene.N, mask_block_size(scene.K)))
+    for cam in np.atleast_1d(train_cams):
+        view_hessian_mask(scene, cam, bg_channel, out=H_T)
+    conf = confidence(scene.obj_logits, scene.opacity, alpha_obj, alpha_opa, target)
+    scores = np.array([gaussian_gains_L(H_T, view_hessian_mask(scene, cam, bg_channel), conf, prior, L).sum()
+                       for cam in np.atleast_1d(cand_cams)])
+    return dict(H_T=H_T, scores=scores, best=argmax_lowest(scores))
+
+
 def render_smooth(theta, cam, cfg, offsets, ids, clamped) -> np.ndarray:
     cam = _cam(cam)
     theta = np.ascontiguousarray(theta, dtype=np.float64)
