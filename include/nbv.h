@@ -43,6 +43,8 @@ extern "C" {
 #define NBV_CH_RGB 7      /* channel_mask bits: 1 = r, 2 = g, 4 = b, 8 = depth */
 #define NBV_CH_DEPTH 8
 #define NBV_CH_RGBD 15
+#define NBV_CH_MASK 16    /* the object-mask output (Eq. 1-2): a context of its own, blocks of 11 + K parameters */
+#define NBV_MASK_KMAX 52  /* largest number of object channels a mask context supports */
 
 typedef enum nbv_status {
   NBV_OK = 0,
@@ -73,12 +75,15 @@ typedef struct nbv_config {
   float alpha_max;           /* 0.99   alpha cap (R-4) */
   float t_stop;              /* 1e-4   stop before T would fall below (R-4) */
   float bg[3];               /* background colour, default 0 (R-8); depth background is 0 (R-6) */
-  int32_t channel_mask;      /* NBV_CH_RGB or NBV_CH_RGBD or NBV_CH_DEPTH: outputs whose Jacobians enter H (R-12) */
+  int32_t channel_mask;      /* any non-empty subset of NBV_CH_RGBD: outputs whose Jacobians enter H (R-12); or NBV_CH_MASK */
   float channel_weight[4];   /* omega_ch, inverse noise variance per channel, default 1 (R-12) */
   int32_t opacity_coord;     /* 0 = logit (default), 1 = sigma (R-10) */
   float alpha_obj, alpha_opa;/* 0.3, 0.3 exponents of Eq. 7 / Eq. 12 */
   float p_floor, sigma_floor;/* 1e-4 floors inside Eq. 7 (R-14) */
   float prior_precision[14]; /* diagonal of Lambda (R-13), default 1.0 each */
+  /* mask contexts (channel_mask == NBV_CH_MASK) only: */
+  int32_t mask_bg_channel;   /* 0      object channel that receives the residual 1 - 1^T O' (Eq. 2: the background label) */
+  float prior_precision_obj; /* 1.0    diagonal of Lambda on the K object logits */
 } nbv_config;
 
 typedef struct nbv_ctx nbv_ctx;
@@ -143,22 +148,24 @@ int nbv_score_candidates_host(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n,
 
 /* ---- view selection on top of the per-view gains ------------- */
 
-/* Per-output normalised gains and their fusion (Eq. 10-11), for the outputs RGB and depth
- * (the object-mask output of Eq. 11 is not built; its term is absent).
+/* Per-output normalised gains and their fusion (Eq. 10-11) for the outputs RGB, depth and (optionally)
+ * object mask:
  *   raw_f[i]   = IG_f(T, c_i)                       the score nbv_score_candidates gives in the context of output f
  *   denom_f    = (1/|T|) sum_t IG_f(T, t)           the training views re-scored as candidates on top of the full H_T
- *   fused[i]   = raw_rgb[i] / denom_rgb + beta_d * raw_d[i] / denom_d        (beta_d = 10 in the paper)
+ *   fused[i]   = raw_rgb[i] / denom_rgb + beta_d raw_d[i] / denom_d + beta_o raw_o[i] / denom_o
+ *                (beta_d = 10, beta_o = 1 in the paper)
  *   *d_best    = arg max_i fused[i], lowest index on ties
- * ctx_rgb / ctx_depth: two contexts holding the SAME map, created with channel_mask = NBV_CH_RGB and NBV_CH_DEPTH
- * (every output has its own Jacobian, hence its own Hessian), each with the n_train cameras of h_train
- * already accumulated.  h_train: HOST array of those training cameras (needed again for the denominators).
- * DEVICE outputs: d_fused n floats; d_raw 2*n floats (rgb row, then depth row; may be NULL); d_denom 2 floats
+ * ctx_rgb / ctx_depth / ctx_mask: contexts holding the SAME map, created with channel_mask = NBV_CH_RGB, NBV_CH_DEPTH and
+ * NBV_CH_MASK (every output has its own Jacobian, hence its own Hessian), each with the n_train cameras of
+ * h_train already accumulated.  ctx_mask may be NULL: the mask term is then left out (F = 2 outputs instead of 3).
+ * h_train: HOST array of those training cameras (needed again for the denominators).
+ * DEVICE outputs: d_fused n floats; d_raw F*n floats (rgb row, depth row[, mask row]; may be NULL); d_denom F floats
  * (may be NULL); d_best one int32.  A zero denominator (no training view sees anything) yields non-finite
  * fused scores, not an error.  Errors: NOT_LOADED, EMPTY_CANDIDATES (n == 0), UNKNOWN_TARGET, INVALID_ARG (null
  * pointers, n_train <= 0, contexts of different N or K, wrong channel masks, bad camera), OOM, CUDA. */
-int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, const nbv_camera* h_train, int32_t n_train,
-                               const nbv_camera* h_cams, int32_t n, int32_t target_obj, float beta_d,
-                               float* d_fused, float* d_raw, float* d_denom, int32_t* d_best, void* stream);
+int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, nbv_ctx* ctx_mask, const nbv_camera* h_train,
+                               int32_t n_train, const nbv_camera* h_cams, int32_t n, int32_t target_obj, float beta_d,
+                               float beta_o, float* d_fused, float* d_raw, float* d_denom, int32_t* d_best, void* stream);
 
 /* Greedy selection of `rounds` views out of n candidates without retraining (Eq. 5 applied repeatedly, P:L185;
  * P:L746 uses 6 rounds): in round r the candidates not yet selected are scored against the current H_T, the arg-max
@@ -175,6 +182,15 @@ int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, const nbv_c
  * OOM, CUDA. */
 int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t rounds, int32_t target_obj,
                       int32_t* h_order, float* d_scores, void* stream);
+
+/* Number of floats of one packed block in this context: 105 for colour/depth contexts; L (L + 1) / 2 with L = 11 + K
+ * for a loaded mask context (parameter order [mu(3) logscale(3) quat(4) opacity | object logits (K)], upper triangle
+ * row-major, idx(r,c) = r L - r (r - 1) / 2 + (c - r)).  nbv_view_hessian / nbv_training_hessian use this size.
+ * Returns 0 for a mask context before nbv_load_gaussians. */
+int64_t nbv_block_size(const nbv_ctx* ctx);
+
+/* Parity export of a mask context: d_mask H x W x K, the blended object vector O of Eq. 1-2 (sums to 1 per pixel). */
+int nbv_render_mask(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_mask, void* stream);
 
 /* Counters of the last view processed by any call (synchronises `stream`). */
 int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream);

@@ -423,12 +423,19 @@ def fused_gain(ig_rgb_n, ig_d_n, beta_d=10.0):
     return np.asarray(ig_rgb_n, dtype=np.float64) + beta_d * np.asarray(ig_d_n, dtype=np.float64)
 
 
+def fused_gain3(ig_rgb_n, ig_d_n, ig_o_n, beta_d=10.0, beta_o=1.0):
+    """PAPER.md Eq. 11 (L261-265): IG~ = IG~_rgb + beta_d IG~_d + beta_o IG~_o; beta_d = 10, beta_o = 1 (L742)."""
+    return fused_gain(ig_rgb_n, ig_d_n, beta_d) + beta_o * np.asarray(ig_o_n, dtype=np.float64)
+
+
 def score_candidates_fused(scene_rgb: OracleScene, scene_d: OracleScene, train_cams, cand_cams, target=-1, beta_d=10.0,
-                           alpha_obj=0.3, alpha_opa=0.3, prior=None):
+                           alpha_obj=0.3, alpha_opa=0.3, prior=None, scene_mask: OracleScene | None = None, beta_o=1.0,
+                           bg_channel: int = 0):
     """Per-output gains (L248: each output has its own Jacobian, hence its own Hessian and gain), normalised by the
     mean gain of the training views re-scored as candidates on top of the full H_T (Eq. 10), fused (Eq. 11), arg-max
-    (Eq. 5).  scene_rgb / scene_d: the same map with channel masks {r,g,b} / {depth}.
-    Returns dict(raw (2,C), denom (2,), normalized (2,C), fused (C,), best)."""
+    (Eq. 5).  scene_rgb / scene_d: the same map with channel masks {r,g,b} / {depth}; scene_mask (optional): the same
+    map again, scored on its object-mask output.
+    Returns dict(raw (F,C), denom (F,), normalized (F,C), fused (C,), best), F = 2 or 3."""
     raw, denom = [], []
     for scn in (scene_rgb, scene_d):
         H_T = np.zeros((scn.N, NB))
@@ -438,9 +445,14 @@ def score_candidates_fused(scene_rgb: OracleScene, scene_d: OracleScene, train_c
         r_t = score_candidates(scn, train_cams[:0], train_cams, target, alpha_obj, alpha_opa, prior, H_T=H_T)["scores"]
         raw.append(r_c)
         denom.append(r_t.sum() / r_t.size)
+    if scene_mask is not None:
+        r_c = score_candidates_mask(scene_mask, train_cams, cand_cams, target, alpha_obj, alpha_opa, None, bg_channel)["scores"]
+        r_t = score_candidates_mask(scene_mask, train_cams, train_cams, target, alpha_obj, alpha_opa, None, bg_channel)["scores"]
+        raw.append(r_c)
+        denom.append(r_t.sum() / r_t.size)
     raw, denom = np.array(raw), np.array(denom)
-    norm = np.array([normalized_gain(raw[0], [denom[0]]), normalized_gain(raw[1], [denom[1]])])
-    fused = fused_gain(norm[0], norm[1], beta_d)
+    norm = np.array([normalized_gain(raw[f], [denom[f]]) for f in range(len(raw))])
+    fused = fused_gain(norm[0], norm[1], beta_d) if scene_mask is None else fused_gain3(norm[0], norm[1], norm[2], beta_d, beta_o)
     return dict(raw=raw, denom=denom, normalized=norm, fused=fused, best=argmax_lowest(fused))
 
 

@@ -21,7 +21,7 @@ LIB_PATH = _PKG / "libnbv.so"
 
 P = 14
 NBLK = 105
-CH_RGB, CH_DEPTH, CH_RGBD = 7, 8, 15
+CH_RGB, CH_DEPTH, CH_RGBD, CH_MASK = 7, 8, 15, 16
 
 STATUS = {
     0: "NBV_OK", -1: "NBV_ERR_INVALID_ARG", -2: "NBV_ERR_BAD_DATA", -3: "NBV_ERR_NOT_LOADED",
@@ -35,7 +35,7 @@ EXPORTS = [
     "nbv_accumulate_training", "nbv_score_candidates", "nbv_score_candidates_host", "nbv_last_view_stats",
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
     "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
-    "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy",
+    "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy", "nbv_block_size", "nbv_render_mask",
 ]
 
 STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
@@ -54,7 +54,8 @@ class Config(C.Structure):
         ("near_plane", C.c_float), ("blur", C.c_float), ("alpha_min", C.c_float), ("alpha_max", C.c_float),
         ("t_stop", C.c_float), ("bg", C.c_float * 3), ("channel_mask", C.c_int32), ("channel_weight", C.c_float * 4),
         ("opacity_coord", C.c_int32), ("alpha_obj", C.c_float), ("alpha_opa", C.c_float), ("p_floor", C.c_float),
-        ("sigma_floor", C.c_float), ("prior_precision", C.c_float * 14),
+        ("sigma_floor", C.c_float), ("prior_precision", C.c_float * 14), ("mask_bg_channel", C.c_int32),
+        ("prior_precision_obj", C.c_float),
     ]
 
 
@@ -85,6 +86,8 @@ def load_library(path: Path | None = None):
     lib.nbv_destroy.argtypes = [C.c_void_p]
     lib.nbv_default_config.restype = None
     lib.nbv_kernel_launches.restype = C.c_int64
+    lib.nbv_block_size.restype = C.c_int64
+    lib.nbv_block_size.argtypes = [C.c_void_p]
     if path is None:
         _lib = lib
     return lib
@@ -285,16 +288,29 @@ class NBV:
         self._check(self.lib.nbv_render(self._h, C.c_void_p(cam.ctypes.data), _ptr(rgb), _ptr(depth), _ptr(T), _ptr(nc), _stream()))
         return dict(rgb=rgb, depth=depth, T=T, ncontrib=nc)
 
+    def block_size(self) -> int:
+        """nbv_block_size: floats per packed block (105, or L (L + 1) / 2 with L = 11 + K in a mask context)"""
+        return int(self.lib.nbv_block_size(self._h))
+
+    def render_mask(self, cam):
+        """nbv_render_mask: (H, W, K) blended object vector (mask contexts)"""
+        torch = self._torch
+        cam = _cams(cam)
+        W, H = int(cam["width"][0]), int(cam["height"][0])
+        mask = torch.empty((H, W, self.K), dtype=torch.float32, device=self.device)
+        self._check(self.lib.nbv_render_mask(self._h, C.c_void_p(cam.ctypes.data), _ptr(mask), _stream()))
+        return mask
+
     def view_hessian(self, cam):
         torch = self._torch
         cam = _cams(cam)
-        blocks = torch.empty((self.N, NBLK), dtype=torch.float32, device=self.device)
+        blocks = torch.empty((self.N, self.block_size()), dtype=torch.float32, device=self.device)
         self._check(self.lib.nbv_view_hessian(self._h, C.c_void_p(cam.ctypes.data), _ptr(blocks), _stream()))
         return blocks
 
     def training_hessian(self):
         torch = self._torch
-        blocks = torch.empty((self.N, NBLK), dtype=torch.float32, device=self.device)
+        blocks = torch.empty((self.N, self.block_size()), dtype=torch.float32, device=self.device)
         self._check(self.lib.nbv_training_hessian(self._h, _ptr(blocks), _stream()))
         return blocks
 
@@ -312,20 +328,23 @@ class NBV:
         return gains
 
 
-def score_candidates_fused(nbv_rgb: NBV, nbv_depth: NBV, train_cams, cams, target_obj: int = -1, beta_d: float = 10.0):
-    """nbv_score_candidates_fused (Eq. 10-11): returns dict(fused (n,), raw (2, n), denom (2,), best (1,)) of
-    CUDA tensors.  nbv_rgb / nbv_depth: contexts with channel masks RGB / DEPTH holding the same map, with
-    `train_cams` already accumulated in both."""
+def score_candidates_fused(nbv_rgb: NBV, nbv_depth: NBV, train_cams, cams, target_obj: int = -1, beta_d: float = 10.0,
+                           nbv_mask: NBV | None = None, beta_o: float = 1.0):
+    """nbv_score_candidates_fused (Eq. 10-11): returns dict(fused (n,), raw (F, n), denom (F,), best (1,)) of
+    CUDA tensors, F = 2 (rgb, depth) or 3 (+ mask).  The contexts hold the same map with channel masks RGB / DEPTH /
+    MASK and have `train_cams` already accumulated."""
     torch = nbv_rgb._torch
     tc, cc = _cams(train_cams), _cams(cams)
     n, nt = int(cc.shape[0]), int(tc.shape[0])
+    F = 3 if nbv_mask is not None else 2
     dev = nbv_rgb.device
     fused = torch.empty(max(n, 1), dtype=torch.float32, device=dev)
-    raw = torch.empty((2, max(n, 1)), dtype=torch.float32, device=dev)
-    denom = torch.empty(2, dtype=torch.float32, device=dev)
+    raw = torch.empty((F, max(n, 1)), dtype=torch.float32, device=dev)
+    denom = torch.empty(F, dtype=torch.float32, device=dev)
     best = torch.empty(1, dtype=torch.int32, device=dev)
-    rc = nbv_rgb.lib.nbv_score_candidates_fused(nbv_rgb._h, nbv_depth._h, C.c_void_p(tc.ctypes.data), nt,
-                                                C.c_void_p(cc.ctypes.data), n, int(target_obj), C.c_float(beta_d),
-                                                _ptr(fused), _ptr(raw), _ptr(denom), _ptr(best), _stream())
+    rc = nbv_rgb.lib.nbv_score_candidates_fused(nbv_rgb._h, nbv_depth._h, nbv_mask._h if nbv_mask is not None else None,
+                                                C.c_void_p(tc.ctypes.data), nt, C.c_void_p(cc.ctypes.data), n, int(target_obj),
+                                                C.c_float(beta_d), C.c_float(beta_o), _ptr(fused), _ptr(raw), _ptr(denom),
+                                                _ptr(best), _stream())
     nbv_rgb._check(rc)
     return dict(fused=fused[:n], raw=raw[:, :n] if n else raw[:, :0], denom=denom, best=best)

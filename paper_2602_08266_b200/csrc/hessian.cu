@@ -527,4 +527,290 @@ __global__ void argmax_kernel(const float* __restrict__ scores, int n, int32_t* 
 
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st) { { ++g_kernel_launches; argmax_kernel<<<1, 32, 0, st>>>(scores, n, best); } }
 
+
+
+// =====================================================================================================================
+// Object-mask output (Eq. 1-2 "masks use the object vector").
+//   O = sum_i softmax(o_i) alpha_i T_i + e_bg T_end : compositing of the K "colours" p_i = softmax(o_i) over the
+//   background colour e_bg.  Block of a Gaussian: L = 11 + K parameters [mu, logscale, quat, opacity | logits].
+//   Row of channel k at a pixel:  J_k = beta_k alpha A m6  (+)  w dp_k/do,   dp_k/do_j = p_k (delta_kj - p_j).
+// S3 is shared with the other outputs; S4 is the SAME kernel, run once per group of four object channels on a copy of
+// the rank-ordered splats whose (r, g, b | z) fields hold (p_t0, p_t1, p_t2 | p_t3); group 0 starts with the background
+// channel (the only one with a background term, which the kernel has on its three colour slots).  Every group leaves
+// 40 moments per rank: the 15 monomial sums add up over the groups (sum_k beta_k^2), the 6 cross moments x_k per
+// channel stay apart.  Then, per touched Gaussian (S5'):
+//   geo-geo   (11 x 11)  A Q A^T
+//   geo-logit (11 x K)   sum_k (A x_k) dp_k/do_j = p_j (A x_j - sum_k p_k A x_k)
+//   logit-logit (K x K)  W2 sum_k dp_k/do_j dp_k/do_l = W2 (delta_jl p_j^2 - p_j p_l (p_j + p_l) + p_j p_l sum_k p_k^2)
+// and S6 is the same solve-form log-det gain on L x L blocks.
+// =====================================================================================================================
+__host__ __device__ __forceinline__ int mask_channel_of_slot(int t, int bgch) { return t == 0 ? bgch : (t <= bgch ? t - 1 : t); }
+__host__ __device__ __forceinline__ int mask_slot_of_channel(int c, int bgch) { return c == bgch ? 0 : (c < bgch ? c + 1 : c); }
+__device__ __forceinline__ int triL(int r, int c, int L) { return r * L - r * (r - 1) / 2 + (c - r); }
+
+__global__ void __launch_bounds__(256) mask_splat_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ ids_sorted,
+                                                         const float* __restrict__ logits, const float* __restrict__ lse, int N, int K,
+                                                         int group, int bgch, Splat* __restrict__ out) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= N) return;
+  Splat s = splat_sorted[r];
+  const uint32_t g = ids_sorted[r];
+  float p[4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int t = 4 * group + j;
+    p[j] = (g < (uint32_t)N && t < K) ? expf(logits[(size_t)g * K + mask_channel_of_slot(t, bgch)] - lse[g]) : 0.f;
+  }
+  s.r = p[0]; s.g = p[1]; s.b = p[2]; s.z = p[3];
+  out[r] = s;
+}
+
+void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uint32_t* ids_sorted, int group, int bgch, Splat* out,
+                        cudaStream_t st) {
+  ++g_kernel_launches;
+  mask_splat_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(splat_sorted, ids_sorted, sc.logits, sc.lse, sc.N, sc.K, group, bgch, out);
+}
+
+// upper Cholesky factor of a packed SPD L x L, in place (as cholesky_packed)
+__device__ void cholesky_L(float* Mx, int L) {
+  for (int j = 0; j < L; ++j) {
+    float d = Mx[triL(j, j, L)];
+    for (int k = 0; k < j; ++k) d -= Mx[triL(k, j, L)] * Mx[triL(k, j, L)];
+    d = fmaxf(d, 1e-30f);
+    const float inv = rsqrtf(d);
+    Mx[triL(j, j, L)] = d * inv;
+    for (int i = j + 1; i < L; ++i) {
+      float v = Mx[triL(j, i, L)];
+      for (int k = 0; k < j; ++k) v -= Mx[triL(k, j, L)] * Mx[triL(k, i, L)];
+      Mx[triL(j, i, L)] = v * inv;
+    }
+  }
+}
+
+// log det(I + U^-T B U^-1), packed L x L (as gain_solve)
+__device__ float gain_solve_L(float* B, const float* U, int L) {
+  for (int k = 0; k < L; ++k) {
+    const float inv = 1.0f / U[triL(k, k, L)];
+    const float bkk = B[triL(k, k, L)] * inv * inv;
+    B[triL(k, k, L)] = bkk;
+    if (k < L - 1) {
+      const float ct = -0.5f * bkk;
+      for (int j = k + 1; j < L; ++j) B[triL(k, j, L)] = fmaf(ct, U[triL(k, j, L)], B[triL(k, j, L)] * inv);
+      for (int i = k + 1; i < L; ++i) {
+        const float bki = B[triL(k, i, L)], uki = U[triL(k, i, L)];
+        for (int j = i; j < L; ++j) B[triL(i, j, L)] -= bki * U[triL(k, j, L)] + uki * B[triL(k, j, L)];
+      }
+      for (int j = k + 1; j < L; ++j) B[triL(k, j, L)] = fmaf(ct, U[triL(k, j, L)], B[triL(k, j, L)]);
+      for (int j = k + 1; j < L; ++j) {
+        float v = B[triL(k, j, L)];
+        for (int i = k + 1; i < j; ++i) v -= U[triL(i, j, L)] * B[triL(k, i, L)];
+        B[triL(k, j, L)] = v / U[triL(j, j, L)];
+      }
+    }
+  }
+  float ld = 0.f;
+  for (int j = 0; j < L; ++j) {
+    float e = B[triL(j, j, L)];
+    for (int k = 0; k < j; ++k) e -= B[triL(k, j, L)] * B[triL(k, j, L)];
+    e = fmaxf(e, 0.f);
+    ld += log1pf(e);
+    const float inv = rsqrtf(1.0f + e);
+    for (int i = j + 1; i < L; ++i) {
+      float v = B[triL(j, i, L)];
+      for (int k = 0; k < j; ++k) v -= B[triL(k, j, L)] * B[triL(k, i, L)];
+      B[triL(j, i, L)] = v * inv;
+    }
+  }
+  return ld;
+}
+
+// S5' (+ S6) of a mask context.  KMAX bounds the per-thread arrays: L <= 11 + KMAX.
+template <int KMAX>
+__global__ void __launch_bounds__(64) expand_mask_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
+                                                          const __grid_constant__ ExpandBatch batch, int mode, int groups,
+                                                          float* __restrict__ H_T, const float* __restrict__ conf,
+                                                          const float* __restrict__ cholT) {
+  constexpr int LMAX = 11 + KMAX, LBMAX = LMAX * (LMAX + 1) / 2;
+  const ExpandView& vw = batch.v[blockIdx.y];
+  const int K = sc.K, L = 11 + K, LB = L * (L + 1) / 2, bgch = cfg.mask_bg_channel;
+  const uint32_t n_touched = vw.counters->n_touched;
+  const int stride = NMOM * groups;
+  float gain = 0.f;
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < n_touched; t += gridDim.x * blockDim.x) {
+    const uint32_t r = vw.touched[t];
+    const uint32_t g = vw.ids_sorted[r];
+    const Splat sp = vw.splat_sorted[r];
+    const float cA = -2.f * sp.qa, cB = -sp.qb, cC = -2.f * sp.qc, icC = 1.0f / cC;
+    const float i11 = sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), sh = -cB * icC, i22 = sqrtf(cC);   // as in S4
+    float mono[15], x[KMAX][6], p[KMAX];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) mono[i] = 0.f;
+    float W2 = 0.f;
+    for (int gr = 0; gr < groups; ++gr) {
+      float4* mom4 = reinterpret_cast<float4*>(vw.moments + (size_t)r * stride + (size_t)gr * NMOM);
+      float m[NMOM];
+#pragma unroll
+      for (int i = 0; i < NMOM / 4; ++i) {
+        const float4 v = mom4[i];
+        m[4 * i] = v.x; m[4 * i + 1] = v.y; m[4 * i + 2] = v.z; m[4 * i + 3] = v.w;
+        mom4[i] = make_float4(0.f, 0.f, 0.f, 0.f);     // leave the buffer zeroed for the next view
+      }
+      moments_to_u_basis(m, i11, -sh * i22, 0.0f, i22);
+#pragma unroll
+      for (int i = 0; i < 15; ++i) mono[i] += m[i];
+      if (gr == 0) W2 = m[MOM_W2];                       // sum w^2 does not depend on the channel values
+      for (int j = 0; j < 4; ++j) {
+        const int slot = 4 * gr + j;
+        if (slot < K)
+          for (int i = 0; i < 6; ++i) x[slot][i] = m[MOM_X + 6 * j + i];
+      }
+    }
+    float S2 = 0.f;
+    for (int slot = 0; slot < K; ++slot) {
+      p[slot] = expf(sc.logits[(size_t)g * K + mask_channel_of_slot(slot, bgch)] - sc.lse[g]);
+      S2 += p[slot] * p[slot];
+    }
+    ChainF ch;
+    chain_f(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
+    const float sg = sc.sigma[g];
+    const float kappa = cfg.opacity_coord == 0 ? (1.f - sg) : 1.f / sg;       // R-10
+    float A[11][6];
+#pragma unroll
+    for (int k = 0; k < 10; ++k) {
+      A[k][0] = ch.G[0][k]; A[k][1] = ch.G[1][k]; A[k][2] = 0.5f * ch.G[2][k]; A[k][3] = ch.G[3][k]; A[k][4] = 0.5f * ch.G[4][k]; A[k][5] = 0.f;
+    }
+#pragma unroll
+    for (int e = 0; e < 5; ++e) A[10][e] = 0.f;
+    A[10][5] = kappa;
+    float H[LBMAX];
+    for (int i = 0; i < LB; ++i) H[i] = 0.f;
+    {   // geo-geo: A Q A^T
+      const int ex[6] = {1, 0, 2, 1, 0, 0}, ey[6] = {0, 1, 0, 1, 2, 0};
+      float AQ[11][6];
+      for (int k = 0; k < 11; ++k)
+        for (int j = 0; j < 6; ++j) {
+          float v = 0.f;
+          for (int i = 0; i < 6; ++i) v += A[k][i] * mono[mono_index(ex[i] + ex[j], ey[i] + ey[j])];
+          AQ[k][j] = v;
+        }
+      for (int k = 0; k < 11; ++k)
+        for (int l = k; l < 11; ++l) {
+          float v = 0.f;
+          for (int j = 0; j < 6; ++j) v += AQ[k][j] * A[l][j];
+          H[triL(k, l, L)] = v;
+        }
+    }
+    {   // geo-logit: p_j (A x_j - sum_k p_k A x_k)
+      float xbar[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+      for (int slot = 0; slot < K; ++slot)
+        for (int i = 0; i < 6; ++i) xbar[i] += p[slot] * x[slot][i];
+      for (int c = 0; c < K; ++c) {
+        const int slot = mask_slot_of_channel(c, bgch);
+        float dx6[6];
+        for (int i = 0; i < 6; ++i) dx6[i] = p[slot] * (x[slot][i] - xbar[i]);
+        for (int k = 0; k < 11; ++k) {
+          float v = 0.f;
+          for (int i = 0; i < 6; ++i) v += A[k][i] * dx6[i];
+          H[triL(k, 11 + c, L)] = v;
+        }
+      }
+    }
+    for (int c = 0; c < K; ++c) {   // logit-logit
+      const float pc = p[mask_slot_of_channel(c, bgch)];
+      for (int d = c; d < K; ++d) {
+        const float pd = p[mask_slot_of_channel(d, bgch)];
+        float v = pc * pd * (S2 - pc - pd);
+        if (d == c) v += pc * pc;
+        H[triL(11 + c, 11 + d, L)] = W2 * v;
+      }
+    }
+    if (mode == EXPAND_TRAIN) {
+      float* dst = H_T + (size_t)g * LB;
+      for (int i = 0; i < LB; ++i) atomicAdd(dst + i, H[i]);
+    } else if (mode == EXPAND_VIEW) {
+      float* dst = vw.out_blocks + (size_t)g * LB;
+      for (int i = 0; i < LB; ++i) dst[i] = H[i];
+    } else {
+      const float c = conf[g];
+      float gn = 0.f;
+      if (c > 0.f) {
+        float U[LBMAX];
+        const float* ut = cholT + (size_t)g * LB;
+        for (int i = 0; i < LB; ++i) { U[i] = ut[i]; H[i] *= c; }
+        gn = gain_solve_L(H, U, L);
+      }
+      if (vw.gains) vw.gains[g] = gn;
+      gain += gn;
+    }
+  }
+  if (mode == EXPAND_GAIN) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) gain += __shfl_xor_sync(0xffffffffu, gain, o);
+    __shared__ float ws[2];
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = gain;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const float t = ws[0] + ws[1];
+      if (t != 0.f) atomicAdd(vw.score, t);
+    }
+  }
+}
+
+void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, float* H_T,
+                        const float* conf, const float* cholT, cudaStream_t st) {
+  int blocks = (sc.N + 63) / 64;
+  const int cap = (148 * 8 + batch.n - 1) / batch.n;
+  if (blocks > cap) blocks = cap;
+  const dim3 grid((unsigned)blocks, (unsigned)batch.n);
+  ++g_kernel_launches;
+  if (sc.K <= 20)
+    expand_mask_kernel<20><<<grid, 64, 0, st>>>(sc, cfg, batch, mode, groups, H_T, conf, cholT);
+  else
+    expand_mask_kernel<NBV_MASK_KMAX><<<grid, 64, 0, st>>>(sc, cfg, batch, mode, groups, H_T, conf, cholT);
+}
+
+// once per scoring call of a mask context: U_g = upper Cholesky factor of c_g H_T,g + Lambda (L x L)
+template <int KMAX>
+__global__ void __launch_bounds__(64) prepare_mask_kernel(int N, int K, nbv_config cfg, const float* __restrict__ H_T,
+                                                           const float* __restrict__ conf, float* __restrict__ cholT) {
+  constexpr int LMAX = 11 + KMAX, LBMAX = LMAX * (LMAX + 1) / 2;
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= N) return;
+  const float c = conf[g];
+  if (!(c > 0.f)) return;
+  const int L = 11 + K, LB = L * (L + 1) / 2;
+  const float* ht = H_T + (size_t)g * LB;
+  float H[LBMAX];
+  for (int i = 0; i < LB; ++i) H[i] = c * ht[i];
+  for (int k = 0; k < L; ++k) H[triL(k, k, L)] += k < 11 ? cfg.prior_precision[k] : cfg.prior_precision_obj;
+  cholesky_L(H, L);
+  float* dst = cholT + (size_t)g * LB;
+  for (int i = 0; i < LB; ++i) dst[i] = H[i];
+}
+
+void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st) {
+  ++g_kernel_launches;
+  if (sc.K <= 20)
+    prepare_mask_kernel<20><<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, sc.K, cfg, H_T, conf, cholT);
+  else
+    prepare_mask_kernel<NBV_MASK_KMAX><<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, sc.K, cfg, H_T, conf, cholT);
+}
+
+// parity export: (rgb | depth) images of one group's forward pass -> mask channels of that group
+__global__ void __launch_bounds__(256) mask_scatter_kernel(const float* __restrict__ rgb, const float* __restrict__ depth, size_t npx, int K,
+                                                            int group, int bgch, float* __restrict__ mask) {
+  const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= npx) return;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int t = 4 * group + j;
+    if (t < K) mask[p * K + mask_channel_of_slot(t, bgch)] = j < 3 ? rgb[3 * p + j] : depth[p];
+  }
+}
+
+void launch_mask_scatter(const float* rgb, const float* depth, size_t npx, int K, int group, int bgch, float* mask, cudaStream_t st) {
+  ++g_kernel_launches;
+  mask_scatter_kernel<<<(unsigned)((npx + 255) / 256), 256, 0, st>>>(rgb, depth, npx, K, group, bgch, mask);
+}
+
 }  // namespace nbv

@@ -69,7 +69,8 @@ struct RasterView {
   PixelBuf pix;
   uint32_t* tile_cend;       // per tile: coarse position + 1 of the last composited entry
   uint32_t* tile_walk;       // per tile: list entries S3 consumed
-  float* moments;            // N x NMOM, zero on entry to S4 for every Gaussian
+  float* moments;            // rank r at moments + r * mom_stride (NMOM floats), zero on entry to S4 for every Gaussian
+  int mom_stride;            // NMOM, or groups * NMOM in a mask context (one group of 4 object channels per S4 launch)
   uint32_t* touched;         // ranks with a non-zero block (counters->n_touched of them, in no particular order)
   ViewCounters* counters;
 };
@@ -86,7 +87,7 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
                     cudaStream_t st);
 // S4, then the touched lists (ranks with sum w^2 != 0) of every view of the batch
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
-                     cudaStream_t st);
+                     cudaStream_t st, bool build_touched = true);
 
 // ---- hessian.cu
 enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2, EXPAND_CACHE = 3 };
@@ -133,10 +134,18 @@ void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, fl
 void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);
 
+// ---- hessian.cu, object-mask output (NEXT-2): groups of four object channels, blocks of L = 11 + K parameters
+void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uint32_t* ids_sorted, int group, int bgch, Splat* out,
+                        cudaStream_t st);
+void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, float* H_T,
+                        const float* conf, const float* cholT, cudaStream_t st);
+void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
+void launch_mask_scatter(const float* rgb, const float* depth, size_t npx, int K, int group, int bgch, float* mask, cudaStream_t st);
+
 // ---- select.cu
-// Eq. 10-11 on raw (2 x n) and training (2 x n_train) gains: denominators, fused scores, arg-max
-void launch_fuse(const float* raw, const float* train, int n, int n_train, float beta_d, float* denom, float* fused, int32_t* best,
-                 cudaStream_t st);
+// Eq. 10-11 on raw (F x n) and training (F x n_train) gains of F = 2 or 3 outputs: denominators, fused scores, arg-max
+void launch_fuse(const float* raw, const float* train, int n, int n_train, int F, float beta_d, float beta_o, float* denom, float* fused,
+                 int32_t* best, cudaStream_t st);
 // one greedy round: row[remaining[j]] = tmp[j], NaN elsewhere; *pick = arg-max over the remaining candidates
 void launch_greedy_round(const float* tmp, const int32_t* remaining, int m, int n, float* row, int32_t* pick, cudaStream_t st);
 // device-resident greedy round: row[i] = taken[i] ? NaN : scores[i]; *pick = order_r[0] = arg-max over the free ones; taken[*pick] = 1

@@ -31,7 +31,7 @@ struct DevBuf {
 struct ViewSlot {
   cudaStream_t st = nullptr;
   cudaEvent_t done = nullptr;
-  DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, msplit;
+  DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, msplit, gsplat;
   DevBuf ckeys, crect, cranges, sort_tmp, scan_tmp, tile_counts;
   DevBuf pix_rgb, pix_depth, pix_T, pix_nc, pix_last, tile_cend, tile_walk, moments, touched;
   ViewCounters* d_counters = nullptr;
@@ -56,6 +56,10 @@ struct nbv_ctx {
   int device = 0;
   int N = 0, K = 0;
   bool loaded = false;
+  // object-mask context (channel_mask == NBV_CH_MASK): groups of four object channels, blocks of LB = L (L + 1) / 2 floats
+  bool mask_mode = false;
+  int mask_groups = 1;                  // 1 in colour / depth contexts (it is the moment stride in units of NMOM)
+  size_t LB = NBLK;
   int n_train = 0;
   // scene
   DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp, cache_ids, cache_blocks, cache_meta;
@@ -210,7 +214,7 @@ int span_next(nbv_ctx* ctx, int idx, int stage, int views, cudaStream_t st) {
 void free_slot(ViewSlot* sl) {
   if (!sl) return;
   DevBuf* all[] = {&sl->splat, &sl->zkey, &sl->zkey_alt, &sl->ids, &sl->ids_alt, &sl->rect, &sl->abc, &sl->splat_sorted,
-                   &sl->rect_sorted, &sl->msplit, &sl->ckeys, &sl->crect, &sl->cranges, &sl->sort_tmp,
+                   &sl->rect_sorted, &sl->msplit, &sl->gsplat, &sl->ckeys, &sl->crect, &sl->cranges, &sl->sort_tmp,
                    &sl->scan_tmp, &sl->tile_counts, &sl->pix_rgb, &sl->pix_depth, &sl->pix_T, &sl->pix_nc, &sl->pix_last,
                    &sl->tile_cend, &sl->tile_walk, &sl->moments, &sl->touched};
   for (DevBuf* b : all) release(*b);
@@ -307,7 +311,8 @@ int pre_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool w
     }
   }
   if (upto >= STAGE_BACKWARD) {
-    const size_t mom_bytes = 4 * (size_t)NMOM * N;
+    const size_t mom_bytes = 4 * (size_t)NMOM * ctx->mask_groups * N;
+    if (ctx->mask_mode) CKRET(ensure(ctx, sl->gsplat, sizeof(Splat) * (size_t)N));
     if (sl->moments.cap < mom_bytes || !sl->moments.p) sl->moments_clean = false;
     CKRET(ensure(ctx, sl->moments, mom_bytes));
     CKRET(ensure(ctx, sl->touched, 4 * (size_t)N));
@@ -367,6 +372,20 @@ int ensure_tile_order(nbv_ctx* ctx, const TileGrid& tg, cudaStream_t st) {
   return NBV_OK;
 }
 
+// configuration of the S3 / S4 launch of group gr of a mask context: slots (r, g, b | depth) <- object channels
+// 4 gr .. 4 gr + 3 in the order "background channel first"; only the very first slot has a background term (Eq. 2)
+nbv_config mask_group_config(const nbv_ctx* ctx, int gr) {
+  nbv_config g = ctx->cfg;
+  g.channel_mask = 0;
+  for (int j = 0; j < 4; ++j) {
+    if (4 * gr + j < ctx->K) g.channel_mask |= 1 << j;
+    g.channel_weight[j] = 1.0f;
+  }
+  g.bg[0] = gr == 0 ? 1.0f : 0.0f;
+  g.bg[1] = g.bg[2] = 0.0f;
+  return g;
+}
+
 // S3 (+ S4) for a batch of views whose S1-S2 products sit in sl[0..n): ONE launch per stage, grid.y = view.
 // All views share the image size (same tile grid).  Stream st must already be ordered after the slots' S1-S2.
 int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int upto, bool full_pix, cudaStream_t st) {
@@ -392,7 +411,7 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     v.pix.ncontrib = full_pix ? s->pix_nc.as<int32_t>() : nullptr;
     v.pix.T = s->pix_T.as<float>(); v.pix.last = s->pix_last.as<int32_t>();
     v.tile_cend = s->tile_cend.as<uint32_t>(); v.tile_walk = s->tile_walk.as<uint32_t>();
-    v.moments = s->moments.as<float>(); v.touched = s->touched.as<uint32_t>(); v.counters = s->d_counters;
+    v.moments = s->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = s->touched.as<uint32_t>(); v.counters = s->d_counters;
   }
   const TileGrid tg = sl[0]->tg;
   CKRET(ensure_tile_order(ctx, tg, st));
@@ -402,7 +421,24 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
   CK(cudaGetLastError());
   if (upto == STAGE_FORWARD) { span_end(ctx, sp, st); return NBV_OK; }
   sp = span_next(ctx, sp, NBV_STAGE_BACKWARD, n, st);
-  launch_backward(rb, ctx->N, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, ctx->cfg, st);
+  if (!ctx->mask_mode) {
+    launch_backward(rb, ctx->N, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, ctx->cfg, st);
+  } else {
+    // one S4 launch per group of four object channels, on a copy of the splats that carries their probabilities
+    const SceneDev sc = scene_dev(ctx);
+    for (int gr = 0; gr < ctx->mask_groups; ++gr) {
+      const nbv_config gcfg = mask_group_config(ctx, gr);
+      RasterBatch gb = rb;
+      for (int i = 0; i < n; ++i) {
+        launch_mask_splats(sc, sl[i]->splat_sorted.as<Splat>(), sl[i]->ids.as<uint32_t>(), gr, ctx->cfg.mask_bg_channel,
+                           sl[i]->gsplat.as<Splat>(), st);
+        gb.v[i].splat_sorted = sl[i]->gsplat.as<Splat>();
+        gb.v[i].moments = sl[i]->moments.as<float>() + (size_t)gr * NMOM;
+      }
+      if (gr > 0 && gb.work) CK(cudaMemsetAsync(gb.work, 0, 4, st));     // a fresh work counter for every launch
+      launch_backward(gb, ctx->N, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, gcfg, st, gr == 0);
+    }
+  }
   CK(cudaGetLastError());
   span_end(ctx, sp, st);
   return NBV_OK;
@@ -426,6 +462,9 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
   if (mode == EXPAND_CACHE) {
     launch_cache_reserve(eb, *cache, first_candidate, st);
     launch_expand_cache(scene_dev(ctx), ctx->cfg, eb, *cache, st);
+  } else if (ctx->mask_mode) {
+    launch_expand_mask(scene_dev(ctx), ctx->cfg, eb, mode, ctx->mask_groups, ctx->H_T.as<float>(), ctx->conf.as<float>(),
+                       ctx->cholT.as<float>(), st);
   } else {
     launch_expand(scene_dev(ctx), ctx->cfg, eb, mode, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
   }
@@ -492,7 +531,10 @@ int prepare_scoring(nbv_ctx* ctx, int target, cudaStream_t st) {
   if (ctx->conf_target == target) return NBV_OK;
   const SceneDev sc = scene_dev(ctx);
   launch_confidence(sc, ctx->cfg, target, ctx->conf.as<float>(), st);
-  launch_prepare(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
+  if (ctx->mask_mode)
+    launch_prepare_mask(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
+  else
+    launch_prepare(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
   CK(cudaGetLastError());
   ctx->conf_target = target;
   return NBV_OK;
@@ -538,6 +580,8 @@ void nbv_default_config(nbv_config* cfg) {
   cfg->p_floor = 1e-4f;
   cfg->sigma_floor = 1e-4f;
   for (int k = 0; k < NBV_P; ++k) cfg->prior_precision[k] = 1.0f;
+  cfg->mask_bg_channel = 0;
+  cfg->prior_precision_obj = 1.0f;
 }
 
 int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
@@ -546,7 +590,9 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
   nbv_config c;
   if (cfg) c = *cfg; else nbv_default_config(&c);
   const bool ok = c.near_plane > 0.f && c.blur >= 0.f && c.alpha_min >= 1.0f / 255.0f && c.alpha_max > c.alpha_min &&
-                  c.alpha_max < 1.f && c.t_stop > 0.f && c.t_stop < 1.f && (c.channel_mask & 15) != 0 && (c.channel_mask & ~15) == 0 &&
+                  c.alpha_max < 1.f && c.t_stop > 0.f && c.t_stop < 1.f &&
+                  (c.channel_mask == NBV_CH_MASK || ((c.channel_mask & 15) != 0 && (c.channel_mask & ~15) == 0)) &&
+                  c.mask_bg_channel >= 0 && c.prior_precision_obj > 0.f && std::isfinite(c.prior_precision_obj) &&
                   (c.opacity_coord == 0 || c.opacity_coord == 1) && c.p_floor > 0.f && c.sigma_floor > 0.f;
   if (!ok) return NBV_ERR_INVALID_ARG;
   for (int k = 0; k < NBV_P; ++k)
@@ -557,6 +603,7 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
   if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return NBV_ERR_CUDA; }
   nbv_ctx* ctx = new nbv_ctx;
   ctx->cfg = c;
+  ctx->mask_mode = c.channel_mask == NBV_CH_MASK;
   ctx->device = dev;
   ViewSlot* s0 = nullptr;
   if (cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -611,20 +658,27 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
     return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_load_gaussians: N, K must be positive and all pointers non-null");
   cudaStream_t st = (cudaStream_t)stream;
   ctx->loaded = false;
+  if (ctx->mask_mode) {
+    if (K > NBV_MASK_KMAX || ctx->cfg.mask_bg_channel >= K)
+      return fail(ctx, NBV_ERR_INVALID_ARG, "mask context: K exceeds NBV_MASK_KMAX or mask_bg_channel >= K");
+    const size_t L = 11 + (size_t)K;
+    ctx->LB = L * (L + 1) / 2;
+    ctx->mask_groups = (K + 3) / 4;
+  }
   ctx->N = N; ctx->K = K;
   const size_t n = (size_t)N;
   CKRET(ensure(ctx, ctx->mean, 12 * n)); CKRET(ensure(ctx, ctx->logscale, 12 * n)); CKRET(ensure(ctx, ctx->quat, 16 * n));
   CKRET(ensure(ctx, ctx->sigma, 4 * n)); CKRET(ensure(ctx, ctx->rgb, 12 * n)); CKRET(ensure(ctx, ctx->logits, 4 * n * K));
   CKRET(ensure(ctx, ctx->M, 36 * n)); CKRET(ensure(ctx, ctx->pmax, 4 * n)); CKRET(ensure(ctx, ctx->amax, 4 * n));
-  CKRET(ensure(ctx, ctx->lse, 4 * n)); CKRET(ensure(ctx, ctx->H_T, 4 * (size_t)NBLK * n)); CKRET(ensure(ctx, ctx->conf, 4 * n));
-  CKRET(ensure(ctx, ctx->cholT, 4 * (size_t)NBLK * n));
+  CKRET(ensure(ctx, ctx->lse, 4 * n)); CKRET(ensure(ctx, ctx->H_T, 4 * ctx->LB * n)); CKRET(ensure(ctx, ctx->conf, 4 * n));
+  CKRET(ensure(ctx, ctx->cholT, 4 * ctx->LB * n));
   CK(cudaMemcpyAsync(ctx->mean.p, d_mean, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->logscale.p, d_logscale, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->quat.p, d_quat, 16 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->sigma.p, d_opacity, 4 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->rgb.p, d_rgb, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->logits.p, d_obj_logits, 4 * n * K, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemsetAsync(ctx->H_T.p, 0, 4 * (size_t)NBLK * n, st));
+  CK(cudaMemsetAsync(ctx->H_T.p, 0, 4 * ctx->LB * n, st));
   ViewSlot* s0 = ctx->slots[0];
   CK(cudaDeviceSynchronize());             // no view of a previous scene may still be in flight
   CK(cudaMemsetAsync(s0->d_counters, 0, sizeof(ViewCounters), st));
@@ -644,7 +698,7 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
 int nbv_reset_training(nbv_ctx* ctx, void* stream) {
   if (!ctx) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
-  CK(cudaMemsetAsync(ctx->H_T.p, 0, 4 * (size_t)NBLK * ctx->N, (cudaStream_t)stream));
+  CK(cudaMemsetAsync(ctx->H_T.p, 0, 4 * ctx->LB * ctx->N, (cudaStream_t)stream));
   ctx->n_train = 0;
   ctx->conf_target = -2;
   return NBV_OK;
@@ -698,41 +752,44 @@ int nbv_score_candidates_host(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n,
   return NBV_OK;
 }
 
-int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, const nbv_camera* h_train, int32_t n_train,
-                               const nbv_camera* h_cams, int32_t n, int32_t target_obj, float beta_d, float* d_fused,
+int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, nbv_ctx* ctx_mask, const nbv_camera* h_train, int32_t n_train,
+                               const nbv_camera* h_cams, int32_t n, int32_t target_obj, float beta_d, float beta_o, float* d_fused,
                                float* d_raw, float* d_denom, int32_t* d_best, void* stream) {
   nbv_ctx* ctx = ctx_rgb;
   if (!ctx_rgb || !ctx_depth) return NBV_ERR_INVALID_ARG;
-  if (!ctx_rgb->loaded || !ctx_depth->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  if (!ctx_rgb->loaded || !ctx_depth->loaded || (ctx_mask && !ctx_mask->loaded)) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   if (n == 0) return fail(ctx, NBV_ERR_EMPTY_CANDIDATES, "no candidate cameras");
-  if (n < 0 || n_train <= 0 || !h_train || !h_cams || !d_fused || !d_best || !std::isfinite(beta_d))
+  if (n < 0 || n_train <= 0 || !h_train || !h_cams || !d_fused || !d_best || !std::isfinite(beta_d) || !std::isfinite(beta_o))
     return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_score_candidates_fused: bad arguments");
-  if (ctx_rgb == ctx_depth || ctx_rgb->N != ctx_depth->N || ctx_rgb->K != ctx_depth->K)
-    return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_score_candidates_fused: the two contexts must be distinct and hold the same map");
-  if ((ctx_rgb->cfg.channel_mask & NBV_CH_DEPTH) || !(ctx_rgb->cfg.channel_mask & NBV_CH_RGB) || ctx_depth->cfg.channel_mask != NBV_CH_DEPTH)
-    return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_score_candidates_fused: channel masks must be RGB and DEPTH");
+  if (ctx_rgb == ctx_depth || ctx_rgb->N != ctx_depth->N || ctx_rgb->K != ctx_depth->K ||
+      (ctx_mask && (ctx_mask == ctx_rgb || ctx_mask == ctx_depth || ctx_mask->N != ctx_rgb->N || ctx_mask->K != ctx_rgb->K)))
+    return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_score_candidates_fused: the contexts must be distinct and hold the same map");
+  if ((ctx_rgb->cfg.channel_mask & ~NBV_CH_RGB) || !(ctx_rgb->cfg.channel_mask & NBV_CH_RGB) || ctx_depth->cfg.channel_mask != NBV_CH_DEPTH ||
+      (ctx_mask && !ctx_mask->mask_mode))
+    return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_score_candidates_fused: channel masks must be RGB, DEPTH and (optionally) MASK");
   if (target_obj < -1 || target_obj >= ctx->K) return fail(ctx, NBV_ERR_UNKNOWN_TARGET, "target_obj must be -1 or in [0, K)");
   cudaStream_t st = (cudaStream_t)stream;
-  // work area in the rgb context: raw (2n) | training gains (2 n_train) | denominators (2) | scratch arg-max (1)
-  const size_t words = 2 * (size_t)n + 2 * (size_t)n_train + 4;
+  const int F = ctx_mask ? 3 : 2;
+  // work area in the rgb context: raw (F n) | training gains (F n_train) | denominators (F, padded to 4) | scratch arg-max (1)
+  const size_t words = (size_t)F * n + (size_t)F * n_train + 8;
   CKRET(ensure(ctx, ctx->fuse_tmp, 4 * words));
   float* raw = ctx->fuse_tmp.as<float>();
-  float* train = raw + 2 * (size_t)n;
-  float* denom = train + 2 * (size_t)n_train;
-  int32_t* scratch = reinterpret_cast<int32_t*>(denom + 2);
-  nbv_ctx* cx[2] = {ctx_rgb, ctx_depth};
-  for (int f = 0; f < 2; ++f) {
+  float* train = raw + (size_t)F * n;
+  float* denom = train + (size_t)F * n_train;
+  int32_t* scratch = reinterpret_cast<int32_t*>(denom + 4);
+  nbv_ctx* cx[3] = {ctx_rgb, ctx_depth, ctx_mask};
+  for (int f = 0; f < F; ++f) {
     int rc = nbv_score_candidates(cx[f], h_cams, n, target_obj, raw + (size_t)f * n, scratch, stream);
     if (rc == NBV_OK) rc = nbv_score_candidates(cx[f], h_train, n_train, target_obj, train + (size_t)f * n_train, scratch, stream);
     if (rc != NBV_OK) {
-      if (f == 1) ctx->err = ctx_depth->err;
+      if (f > 0) ctx->err = cx[f]->err;
       return rc;
     }
   }
-  launch_fuse(raw, train, n, n_train, beta_d, denom, d_fused, d_best, st);
+  launch_fuse(raw, train, n, n_train, F, beta_d, beta_o, denom, d_fused, d_best, st);
   CK(cudaGetLastError());
-  if (d_raw) CK(cudaMemcpyAsync(d_raw, raw, 8 * (size_t)n, cudaMemcpyDeviceToDevice, st));
-  if (d_denom) CK(cudaMemcpyAsync(d_denom, denom, 8, cudaMemcpyDeviceToDevice, st));
+  if (d_raw) CK(cudaMemcpyAsync(d_raw, raw, 4 * (size_t)F * n, cudaMemcpyDeviceToDevice, st));
+  if (d_denom) CK(cudaMemcpyAsync(d_denom, denom, 4 * (size_t)F, cudaMemcpyDeviceToDevice, st));
   return NBV_OK;
 }
 
@@ -783,7 +840,7 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
   // the masked arg-max and H_T += (blocks of the selected view) -- all on the device, no camera and no host round trip.
   const size_t entry_bytes = 4 * (size_t)NBLK + 4;
   const size_t want = std::min((size_t)n * (size_t)ctx->N, ctx->greedy_cache_bytes / entry_bytes);
-  if (want == 0 || want > 0xfffffff0ull) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);
+  if (want == 0 || want > 0xfffffff0ull || ctx->mask_mode) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);
   CKRET(ensure(ctx, ctx->cache_ids, 4 * want));
   CKRET(ensure(ctx, ctx->cache_blocks, 4 * (size_t)NBLK * want));
   // meta: spans (2n) | cursor + overflow flag (2) | taken (n) | scores (n) | pick (1) | order (rounds)
@@ -900,6 +957,7 @@ int nbv_tile_lists(nbv_ctx* ctx, const nbv_camera* h_cam, int64_t* d_offsets, in
 int nbv_render(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_rgb, float* d_depth, float* d_T, int32_t* d_ncontrib, void* stream) {
   if (!ctx || !h_cam) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  if (ctx->mask_mode) return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_render: a mask context renders with nbv_render_mask");
   cudaStream_t st = (cudaStream_t)stream;
   ViewSlot* sl = ctx->slots[0];
   CKRET(process_view(ctx, sl, *h_cam, STAGE_FORWARD, false, true, st));
@@ -908,6 +966,42 @@ int nbv_render(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_rgb, float* d_dep
   if (d_depth) CK(cudaMemcpyAsync(d_depth, sl->pix_depth.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
   if (d_T) CK(cudaMemcpyAsync(d_T, sl->pix_T.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
   if (d_ncontrib) CK(cudaMemcpyAsync(d_ncontrib, sl->pix_nc.p, 4 * npx, cudaMemcpyDeviceToDevice, st));
+  return NBV_OK;
+}
+
+int64_t nbv_block_size(const nbv_ctx* ctx) {
+  if (!ctx) return 0;
+  if (ctx->mask_mode && !ctx->loaded) return 0;
+  return (int64_t)ctx->LB;
+}
+
+int nbv_render_mask(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_mask, void* stream) {
+  if (!ctx || !h_cam || !d_mask) return NBV_ERR_INVALID_ARG;
+  if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  if (!ctx->mask_mode) return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_render_mask needs a context created with channel_mask = NBV_CH_MASK");
+  cudaStream_t st = (cudaStream_t)stream;
+  ViewSlot* sl = ctx->slots[0];
+  CKRET(pre_view(ctx, sl, *h_cam, STAGE_BACKWARD, false, true, st));      // S1-S2 and every buffer the raster passes use
+  CKRET(ensure_tile_order(ctx, sl->tg, st));
+  const size_t npx = (size_t)h_cam->width * h_cam->height;
+  const SceneDev sc = scene_dev(ctx);
+  for (int gr = 0; gr < ctx->mask_groups; ++gr) {
+    const nbv_config gcfg = mask_group_config(ctx, gr);
+    launch_mask_splats(sc, sl->splat_sorted.as<Splat>(), sl->ids.as<uint32_t>(), gr, ctx->cfg.mask_bg_channel, sl->gsplat.as<Splat>(), st);
+    RasterBatch rb;
+    rb.n = 1; rb.n_work = 0; rb.work = nullptr; rb.work_fwd = nullptr;
+    rb.tile_order = ctx->tile_order.as<uint32_t>();
+    RasterView& v = rb.v[0];
+    v.splat_sorted = sl->gsplat.as<Splat>(); v.ckeys = sl->ckeys_sorted; v.crect = sl->crect.as<ushort4>(); v.cranges = sl->cranges.as<uint2>();
+    v.pix.rgb = sl->pix_rgb.as<float>(); v.pix.depth = sl->pix_depth.as<float>(); v.pix.ncontrib = sl->pix_nc.as<int32_t>();
+    v.pix.T = sl->pix_T.as<float>(); v.pix.last = sl->pix_last.as<int32_t>();
+    v.tile_cend = sl->tile_cend.as<uint32_t>(); v.tile_walk = sl->tile_walk.as<uint32_t>();
+    v.moments = sl->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = sl->touched.as<uint32_t>();
+    v.counters = sl->d_counters;
+    launch_forward(rb, sl->tg, sl->rank_bits, h_cam->width, h_cam->height, gcfg, true, st);
+    launch_mask_scatter(sl->pix_rgb.as<float>(), sl->pix_depth.as<float>(), npx, ctx->K, gr, ctx->cfg.mask_bg_channel, d_mask, st);
+    CK(cudaGetLastError());
+  }
   return NBV_OK;
 }
 
@@ -928,7 +1022,7 @@ int nbv_view_hessian(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_blocks, voi
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   cudaStream_t st = (cudaStream_t)stream;
   ViewSlot* sl = ctx->slots[0];
-  CK(cudaMemsetAsync(d_blocks, 0, 4 * (size_t)NBLK * ctx->N, st));
+  CK(cudaMemsetAsync(d_blocks, 0, 4 * ctx->LB * ctx->N, st));
   CKRET(process_view(ctx, sl, *h_cam, STAGE_BACKWARD, false, false, st));
   CKRET(expand_view(ctx, sl, *h_cam, EXPAND_VIEW, d_blocks, nullptr, nullptr, st));
   return NBV_OK;
@@ -937,7 +1031,7 @@ int nbv_view_hessian(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_blocks, voi
 int nbv_training_hessian(nbv_ctx* ctx, float* d_blocks, void* stream) {
   if (!ctx || !d_blocks) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
-  CK(cudaMemcpyAsync(d_blocks, ctx->H_T.p, 4 * (size_t)NBLK * ctx->N, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  CK(cudaMemcpyAsync(d_blocks, ctx->H_T.p, 4 * ctx->LB * ctx->N, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
   return NBV_OK;
 }
 

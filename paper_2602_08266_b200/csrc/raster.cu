@@ -519,7 +519,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
         acc[MOM_W2] = W2;
         const float4 tot = reduce40(acc, red, lane);
         const uint32_t rank = q_rank[j];
-        float* dst = moments + (size_t)rank * NMOM + 4 * lane;
+        float* dst = moments + (size_t)rank * vw.mom_stride + 4 * lane;
         // no returning atomic here: a returned value would tie up a scoreboard for a full L2 round trip; the touched
         // list is built afterwards from sum w^2 != 0 (touched_kernel)
         if (lane < 10) red_add_v4(dst, tot);
@@ -537,7 +537,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
 __global__ void __launch_bounds__(256) touched_kernel(const __grid_constant__ RasterBatch batch, int N) {
   const RasterView& vw = batch.v[blockIdx.y];
   const int r = blockIdx.x * blockDim.x + threadIdx.x;
-  const bool hit = r < N && vw.moments[(size_t)r * NMOM + MOM_W2] != 0.0f;
+  const bool hit = r < N && vw.moments[(size_t)r * vw.mom_stride + MOM_W2] != 0.0f;
   const unsigned m = __ballot_sync(FULL, hit);
   if (m == 0u) return;
   const int lane = threadIdx.x & 31;
@@ -577,7 +577,7 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
 }
 
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
-                     cudaStream_t st) {
+                     cudaStream_t st, bool build_touched) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
   RasterBatch b = batch;
   b.n_work = (uint32_t)(tg.tiles_x * tg.tiles_y * batch.n);
@@ -589,6 +589,7 @@ void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int ra
     backward_kernel<4><<<grid, 32, 0, st>>>(b, p);
   else
     backward_kernel<3><<<grid, 32, 0, st>>>(b, p);
+  if (!build_touched) return;
   ++g_kernel_launches;
   touched_kernel<<<dim3((unsigned)((N + 255) / 256), (unsigned)batch.n), 256, 0, st>>>(batch, N);
 }

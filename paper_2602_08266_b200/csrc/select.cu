@@ -1,7 +1,7 @@
 // select.cu -- view-selection arithmetic on top of the per-view gains.
 //   fuse_kernel:   PAPER.md Eq. 10 (L251-257: each output's gain divided by the mean gain of the training views scored
-//                  as candidates) and Eq. 11 (L261-265: IG~ = IG~_rgb + beta_d IG~_d; the object-mask output is not
-//                  built), then the arg-max of Eq. 5 (lowest index on ties, R-15).
+//                  as candidates) and Eq. 11 (L261-265: IG~ = IG~_rgb + beta_d IG~_d + beta_o IG~_o), then the arg-max
+//                  of Eq. 5 (lowest index on ties, R-15).
 //   greedy_round_kernel: one round of greedy selection -- scatter the scores of the remaining candidates into the
 //                  round's row (NaN at already selected candidates) and take the arg-max over the remaining ones.
 #include <math_constants.h>
@@ -46,22 +46,23 @@ __device__ float block_sum(float v) {
 
 }  // namespace
 
-// raw: 2 x n (rgb row, depth row); train: 2 x n_train; denom: 2; fused: n; best: 1
+// raw: F x n (rgb row, depth row[, mask row]); train: F x n_train; beta: F weights (beta[0] = 1); denom: F; fused: n; best: 1
 __global__ void __launch_bounds__(SEL_T) fuse_kernel(const float* __restrict__ raw, const float* __restrict__ train, int n, int n_train,
-                                                     float beta_d, float* __restrict__ denom, float* __restrict__ fused,
-                                                     int32_t* __restrict__ best) {
-  float den[2];
-#pragma unroll
-  for (int f = 0; f < 2; ++f) {
+                                                     int F, float beta_d, float beta_o, float* __restrict__ denom,
+                                                     float* __restrict__ fused, int32_t* __restrict__ best) {
+  float den[3] = {1.f, 1.f, 1.f};
+  const float beta[3] = {1.f, beta_d, beta_o};
+  for (int f = 0; f < F; ++f) {
     float s = 0.f;
     for (int t = threadIdx.x; t < n_train; t += SEL_T) s += train[(size_t)f * n_train + t];
     den[f] = block_sum(s) / (float)n_train;   // Eq. 10 denominator: (1/|T|) sum_t IG_f(T, t)
   }
-  if (threadIdx.x == 0) { denom[0] = den[0]; denom[1] = den[1]; }
+  if (threadIdx.x < F) denom[threadIdx.x] = den[threadIdx.x];
   float bv = -CUDART_INF_F;
   int bi = 0x7fffffff;
   for (int i = threadIdx.x; i < n; i += SEL_T) {
-    const float v = raw[i] / den[0] + beta_d * (raw[(size_t)n + i] / den[1]);     // Eq. 11
+    float v = 0.f;
+    for (int f = 0; f < F; ++f) v += beta[f] * (raw[(size_t)f * n + i] / den[f]);     // Eq. 11
     fused[i] = v;
     if (v > bv || (v == bv && i < bi)) { bv = v; bi = i; }
   }
@@ -114,10 +115,10 @@ void launch_greedy_pick(const float* scores, int32_t* taken, int n, float* row, 
   greedy_pick_kernel<<<1, SEL_T, 0, st>>>(scores, taken, n, row, pick, order_r);
 }
 
-void launch_fuse(const float* raw, const float* train, int n, int n_train, float beta_d, float* denom, float* fused, int32_t* best,
-                 cudaStream_t st) {
+void launch_fuse(const float* raw, const float* train, int n, int n_train, int F, float beta_d, float beta_o, float* denom, float* fused,
+                 int32_t* best, cudaStream_t st) {
   ++g_kernel_launches;
-  fuse_kernel<<<1, SEL_T, 0, st>>>(raw, train, n, n_train, beta_d, denom, fused, best);
+  fuse_kernel<<<1, SEL_T, 0, st>>>(raw, train, n, n_train, F, beta_d, beta_o, denom, fused, best);
 }
 
 void launch_greedy_round(const float* tmp, const int32_t* remaining, int m, int n, float* row, int32_t* pick, cudaStream_t st) {

@@ -107,3 +107,16 @@ def test_saturated_one_hot_logits_give_a_hard_mask_and_no_logit_information():
     np.testing.assert_allclose(O[..., 0], r["T"], atol=1e-12)                # background = what is left over
     H = orc.unpack_blocks_L(orc.view_hessian_mask(scn, cam), 14)
     assert np.abs(H[:, 11:, :]).max() < 1e-20 and np.abs(H[:, :11, :11]).max() > 0   # dp/do = p(delta - p) = 0
+
+
+def test_three_output_fusion_hand_numbers_and_unit_mean(wl0):
+    assert orc.fused_gain3(0.5, 0.2, 0.3, 10.0, 1.0) == pytest.approx(2.8, abs=1e-15)     # Eq. 11
+    wl = synth.make_workload(0, n_gaussians=200)
+    rng = np.random.default_rng(5)
+    train = synth.hemisphere_cameras(2, (0.6, 0.6), 24, 24, 20.0, 20.0, rng)
+    s7, s8, sm = make_oracle_scene(wl.scene, 7), make_oracle_scene(wl.scene, 8), make_oracle_scene(wl.scene, 7)
+    r = orc.score_candidates_fused(s7, s8, train, train, scene_mask=sm)
+    assert r["raw"].shape == (3, 2) and r["normalized"].mean(axis=1) == pytest.approx([1.0, 1.0, 1.0], abs=1e-12)
+    assert r["fused"].mean() == pytest.approx(12.0, abs=1e-10)                            # 1 + beta_d + beta_o
+    two = orc.score_candidates_fused(s7, s8, train, train)
+    assert r["raw"][:2] == pytest.approx(two["raw"], rel=1e-12)
