@@ -221,7 +221,33 @@ def bench_selection(nbv, wl, api, torch):
     res["fused"] = {"candidates": C, "training_views_rescored": T, "ms": ms, "views_per_s": C / (ms * 1e-3),
                     "best": int(out["best"].item()), "denominators": [float(x) for x in out["denom"].cpu()],
                     "call": "nbv_score_candidates_fused (rgb and depth contexts; candidates and training views scored in both)"}
-    n_rgb.close(); n_d.close()
+    # the object-mask output alone, and Eq. 11 with all three outputs
+    n_o = api.NBV(channel_mask=api.CH_MASK)
+    n_o.load_scene(wl.scene)
+    n_o.accumulate_training(wl.train_cams)
+    sc = torch.empty(C, dtype=torch.float32, device="cuda"); bb = torch.empty(1, dtype=torch.int32, device="cuda")
+    n_o.score_candidates(wl.cand_cams, wl.target_obj, sc, bb)                           # warm-up
+    n_o.set_stage_timing(True)
+    a, b = ev(), ev()
+    a.record()
+    n_o.score_candidates(wl.cand_cams, wl.target_obj, sc, bb)
+    b.record(); b.synchronize()
+    ms = a.elapsed_time(b)
+    st_ms, nv = n_o.stage_times()
+    n_o.set_stage_timing(False)
+    res["mask"] = {"candidates": C, "object_channels": int(wl.scene.K), "block_parameters": 11 + int(wl.scene.K), "ms": ms,
+                   "views_per_s": C / (ms * 1e-3), "stage_ms_per_view": {k: v / max(nv, 1) for k, v in st_ms.items()},
+                   "call": "nbv_score_candidates on a NBV_CH_MASK context (S4 once per group of 4 object channels)"}
+    api.score_candidates_fused(n_rgb, n_d, wl.train_cams, wl.cand_cams, wl.target_obj, nbv_mask=n_o)      # warm-up
+    a, b = ev(), ev()
+    a.record()
+    out = api.score_candidates_fused(n_rgb, n_d, wl.train_cams, wl.cand_cams, wl.target_obj, nbv_mask=n_o)
+    b.record(); b.synchronize()
+    ms = a.elapsed_time(b)
+    res["fused3"] = {"candidates": C, "training_views_rescored": T, "ms": ms, "views_per_s": C / (ms * 1e-3),
+                     "best": int(out["best"].item()), "denominators": [float(x) for x in out["denom"].cpu()],
+                     "call": "nbv_score_candidates_fused with the mask context (Eq. 11, all three outputs)"}
+    n_rgb.close(); n_d.close(); n_o.close()
     return res
 
 
