@@ -92,23 +92,19 @@ constexpr uint32_t SCAN1_MAX = 32768;
 
 __global__ void __launch_bounds__(SCAN1_T) scan_single_block_kernel(const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* __restrict__ total_out) {
   __shared__ uint32_t sm[32];
-  uint32_t carry = 0;
-  for (uint32_t base = 0; base < n; base += SCAN1_T * 4) {
-    const uint32_t i0 = base + threadIdx.x * 4;
-    uint32_t v[4];
-    uint32_t s = 0;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) { v[i] = i0 + i < n ? in[i0 + i] : 0u; s += v[i]; }
-    uint32_t total;
-    uint32_t off = carry + block_exclusive_scan(s, sm, total);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      if (i0 + i < n) out[i0 + i] = off;
-      off += v[i];
-    }
-    carry += total;
+  // thread t owns the contiguous chunk [t c, (t + 1) c): one block-wide scan of the chunk sums instead of one per 4096 elements
+  const uint32_t c = (n + SCAN1_T - 1) / SCAN1_T;
+  const uint32_t i0 = threadIdx.x * c, i1 = min(i0 + c, n);
+  uint32_t s = 0;
+  for (uint32_t i = i0; i < i1; ++i) s += in[i];
+  uint32_t total;
+  uint32_t off = block_exclusive_scan(s, sm, total);
+  for (uint32_t i = i0; i < i1; ++i) {
+    const uint32_t v = in[i];
+    out[i] = off;
+    off += v;
   }
-  if (total_out && threadIdx.x == 0) *total_out = carry;
+  if (total_out && threadIdx.x == 0) *total_out = total;
 }
 
 size_t scan_temp_words(size_t n) {

@@ -11,7 +11,8 @@ from conftest import make_oracle_scene
 pytestmark = pytest.mark.gpu
 
 
-def _scene(K, n=1500, seed=0):
+def _scene(K, n=None, seed=0):
+    n = (1500 if K <= 10 else 500) if n is None else n
     rng = np.random.default_rng(100 + seed)
     sc = synth.make_scene(n, K, -4.0, 0.5, rng)
     return sc
@@ -36,7 +37,7 @@ def _block_err(Hg, Ho, L):
     return np.abs(Hg - Ho) / (scale + 1e-3)
 
 
-@pytest.mark.parametrize("K,bg", [(3, 0), (6, 0), (6, 4), (9, 2)])
+@pytest.mark.parametrize("K,bg", [(3, 0), (6, 0), (6, 4), (9, 2), (22, 0)])      # K = 22: six groups, the K <= 52 instantiation
 def test_mask_image_and_blocks(K, bg):
     sc = _scene(K)
     cam = _cams(1, seed=K)[0]
