@@ -44,7 +44,7 @@ FLOP_TEST = 11            # (pixel, list entry) evaluated: dx, dy, power, two ra
 FLOP_FWD_PAIR = 31        # composited pair, S3: exp, alpha, T update, 4 blended channels
 FLOP_BWD_PAIR = {3: 134, 4: 154}   # composited pair, S4: exp, beta, 34 / 40 moment updates
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
-VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (grid.y = view)
+VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture
 # (profiles/r1c_ncu_raster_cfg2.md); known for config 2 only
 NCU_TRAFFIC_BYTES = {2: {"backward": 98.9e6, "forward": 40.8e6}}

@@ -58,7 +58,7 @@ struct PixelBuf {            // per-pixel outputs of the forward pass (H x W eac
   int32_t* ncontrib;
   int32_t* last;             // list position (relative to the tile's range) after the last composited entry
 };
-// One launch of S3 / S4 / S5+S6 serves a BATCH of views (grid.y = view): per-view device pointers travel as a
+// One launch of S3 / S4 / S5+S6 serves a BATCH of views (S3, S4: launch positions interleave the views; S5+S6: grid.y = view): per-view device pointers travel as a
 // __grid_constant__ kernel parameter.  All views of a batch share the image size.
 constexpr int MAX_BATCH = 8;
 struct RasterView {

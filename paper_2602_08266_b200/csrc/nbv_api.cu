@@ -386,7 +386,7 @@ nbv_config mask_group_config(const nbv_ctx* ctx, int gr) {
   return g;
 }
 
-// S3 (+ S4) for a batch of views whose S1-S2 products sit in sl[0..n): ONE launch per stage, grid.y = view.
+// S3 (+ S4) for a batch of views whose S1-S2 products sit in sl[0..n): ONE launch per stage (S3, S4: persistent warps over (view, tile) positions; S5+S6: grid.y = view).
 // All views share the image size (same tile grid).  Stream st must already be ordered after the slots' S1-S2.
 int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int upto, bool full_pix, cudaStream_t st) {
   RasterBatch rb;
