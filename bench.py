@@ -389,6 +389,7 @@ def main():
         return
 
     peaks = load_peaks()
+    ffma_tflops = api.measure_ffma_peak()               # measured fp32 CUDA-core peak (FFMA chains) on this box
     nch = 4 if wl.channel_mask & 8 else 3
     views = max(n_timed_views, 1)
     per_view_ms = {k: v / views for k, v in stage_ms.items()}
@@ -414,6 +415,9 @@ def main():
     # S1-S2 stage times are taken on slot streams that wait behind the raster launches and are not exclusive
     dominant = max(("backward", "forward"), key=lambda k: per_view_ms[k])
     roofline = dict(rl[dominant], kernel=dominant)
+    if roofline["bound"] == "alu":
+        roofline["peak_measured_ffma"] = ffma_tflops
+        roofline["frac_of_measured_ffma"] = roofline["achieved"] / ffma_tflops if ffma_tflops else None
     # whole-view bound: sum over stages of the stage's own lower bound
     t_min_ms = sum(1e3 * work[k][1] / work[k][2] for k in work)
     view_ms = agg["ms_per_step"] / C                    # wall time per view (stages of different views overlap)

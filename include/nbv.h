@@ -216,6 +216,11 @@ int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream);
  * enabled (h_views may be NULL).  Synchronises `stream`. */
 int nbv_stage_times(nbv_ctx* ctx, double* h_ms, int64_t* h_views, void* stream);
 
+/* FFMA-chain microbenchmark on the current device: *h_tflops <- best of six runs of 8 independent fused multiply-add
+ * chains per thread, 2 blocks of 1024 threads per SM (2 flop per FMA).  The fp32 CUDA-core peak at the clocks the GPU
+ * actually holds; bench.py reports it beside the nominal SMs x 128 lanes x 2 x clock.  Synchronises `stream`. */
+int nbv_measure_ffma_peak(double* h_tflops, void* stream);
+
 /* Number of CUDA kernels this library has launched in this process so far (all contexts). */
 int64_t nbv_kernel_launches(void);
 

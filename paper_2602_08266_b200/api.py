@@ -35,7 +35,7 @@ EXPORTS = [
     "nbv_accumulate_training", "nbv_score_candidates", "nbv_score_candidates_host", "nbv_last_view_stats",
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
     "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
-    "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy", "nbv_block_size", "nbv_render_mask",
+    "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy", "nbv_block_size", "nbv_render_mask", "nbv_measure_ffma_peak",
 ]
 
 STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
@@ -326,6 +326,18 @@ class NBV:
         gains = torch.empty(self.N, dtype=torch.float32, device=self.device)
         self._check(self.lib.nbv_gaussian_gains(self._h, C.c_void_p(cam.ctypes.data), int(target_obj), _ptr(gains), _stream()))
         return gains
+
+
+def measure_ffma_peak() -> float:
+    """nbv_measure_ffma_peak: TFLOP/s of an FFMA-chain microbenchmark on the current CUDA device."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("libnbv needs a CUDA device (sm_100a); there is no CPU fallback")
+    v = C.c_double(0.0)
+    rc = load_library().nbv_measure_ffma_peak(C.byref(v), _stream())
+    if rc != 0:
+        raise NBVError(rc, "nbv_measure_ffma_peak failed")
+    return float(v.value)
 
 
 def score_candidates_fused(nbv_rgb: NBV, nbv_depth: NBV, train_cams, cams, target_obj: int = -1, beta_d: float = 10.0,

@@ -1,0 +1,61 @@
+// peak.cu -- FFMA-chain microbenchmark: the fp32 CUDA-core peak of the device at the clocks it actually holds
+// (BASELINE.md section 4 asks for it; bench.py reports it beside the nominal 148 SM x 128 lanes x 2 x clock).
+// Eight independent fused-multiply-add chains per thread, 1024 threads per block, two blocks per SM.
+#include <algorithm>
+
+#include "kernels.h"
+
+namespace nbv {
+
+constexpr int PK_CHAINS = 8;
+constexpr int PK_UNROLL = 64;
+
+__global__ void __launch_bounds__(1024) ffma_chain_kernel(int iters, float a, float b, float* __restrict__ sink) {
+  float x[PK_CHAINS];
+#pragma unroll
+  for (int c = 0; c < PK_CHAINS; ++c) x[c] = (float)(threadIdx.x + c) * 1e-6f;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < PK_UNROLL; ++u)
+#pragma unroll
+      for (int c = 0; c < PK_CHAINS; ++c) x[c] = fmaf(x[c], a, b);
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int c = 0; c < PK_CHAINS; ++c) s += x[c];
+  if (s == 123.456f) sink[0] = s;            // never true in practice: keeps the chains alive
+}
+
+}  // namespace nbv
+
+extern "C" int nbv_measure_ffma_peak(double* h_tflops, void* stream) {
+  if (!h_tflops) return NBV_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return NBV_ERR_CUDA;
+  }
+  float* sink = nullptr;
+  cudaEvent_t e0, e1;
+  if (cudaMalloc(&sink, 4) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+    cudaGetLastError();
+    return NBV_ERR_CUDA;
+  }
+  const int blocks = 2 * sms, iters = 2000;
+  double best = 0.0;
+  for (int rep = 0; rep < 6; ++rep) {          // first repetitions warm the clocks up
+    cudaEventRecord(e0, st);
+    ++nbv::g_kernel_launches;
+    nbv::ffma_chain_kernel<<<blocks, 1024, 0, st>>>(iters, 0.999f, 0.001f, sink);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaGetLastError(); cudaFree(sink); return NBV_ERR_CUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flops = 2.0 * blocks * 1024.0 * nbv::PK_CHAINS * nbv::PK_UNROLL * (double)iters;
+    if (ms > 0.f) best = std::max(best, flops / (ms * 1e-3) / 1e12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+  *h_tflops = best;
+  return NBV_OK;
+}
