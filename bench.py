@@ -44,7 +44,7 @@ FLOP_TEST = 11            # (pixel, list entry) evaluated: dx, dy, power, two ra
 FLOP_FWD_PAIR = 31        # composited pair, S3: exp, alpha, T update, 4 blended channels
 FLOP_BWD_PAIR = {3: 134, 4: 154}   # composited pair, S4: exp, beta, 34 / 40 moment updates
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
-VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views
+VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (16 for images of fewer than 2,000 tiles)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture
 # (profiles/r1c_ncu_raster_cfg2.md); known for config 2 only
 NCU_TRAFFIC_BYTES = {2: {"backward": 98.9e6, "forward": 40.8e6}}
@@ -406,10 +406,13 @@ def main():
         sec = per_view_ms[k] * 1e-3
         ach = amount / sec if sec > 0 else 0.0
         batched = k in ("backward", "forward")
+        W_, H_ = int(wl.cand_cams[0]["width"]), int(wl.cand_cams[0]["height"])
+        vpl = args.concurrency or (16 if ((W_ + 15) // 16) * ((H_ + 15) // 16) < 2000 else VIEWS_PER_LAUNCH)
+        vpl = min(vpl, C)
         rl[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
                  "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(k),
-                 "views_per_launch": VIEWS_PER_LAUNCH if batched else 1,
-                 "ms_per_launch": per_view_ms[k] * (VIEWS_PER_LAUNCH if batched else 1), "peak_source": peaks["source"] if bound == "hbm" else
+                 "views_per_launch": vpl if batched else 1,
+                 "ms_per_launch": per_view_ms[k] * (vpl if batched else 1), "peak_source": peaks["source"] if bound == "hbm" else
                  "148 SM x 128 lanes x 2 x %.0f MHz (DESIGN.md section 8)" % peaks["sm_max_mhz"]}
     # dominant kernel = largest share of GPU time in the ncu launch list (profiles/): one of the two raster stages; the
     # S1-S2 stage times are taken on slot streams that wait behind the raster launches and are not exclusive

@@ -106,12 +106,13 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg);
 void nbv_destroy(nbv_ctx* ctx);
 const char* nbv_last_error(const nbv_ctx* ctx);
 
-/* Views per batch (default and maximum 8; the NBV_CONCURRENCY environment variable overrides the default at nbv_create).
+/* Views per batch (1..16; default: 8, or 16 for images of fewer than 2,000 tiles; the NBV_CONCURRENCY environment variable
+ * overrides the default at nbv_create).
  * S1-S2 of the views of a batch run concurrently on internal streams (forked from and joined back into the caller's
  * stream with events); S3, S4 and S5+S6 are ONE kernel launch each per batch (S3 and S4: persistent warps pulling
  * (view, tile) positions).  Two sets of work buffers and two internal raster streams alternate between batches.  Views are independent
  * (the arg max is over per-view gains), so this changes no result beyond the order of floating-point atomics.
- * Errors: INVALID_ARG outside [1, 8]. */
+ * Errors: INVALID_ARG outside [1, 16]. */
 int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight);
 
 /* S0 -- load the Gaussian map G with object vectors: device arrays, row-major, float32.

@@ -60,7 +60,7 @@ struct PixelBuf {            // per-pixel outputs of the forward pass (H x W eac
 };
 // One launch of S3 / S4 / S5+S6 serves a BATCH of views (S3, S4: launch positions interleave the views; S5+S6: grid.y = view): per-view device pointers travel as a
 // __grid_constant__ kernel parameter.  All views of a batch share the image size.
-constexpr int MAX_BATCH = 8;
+constexpr int MAX_BATCH = 16;
 struct RasterView {
   const Splat* splat_sorted;
   const uint32_t* ckeys;

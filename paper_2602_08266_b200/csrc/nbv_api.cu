@@ -68,7 +68,7 @@ struct nbv_ctx {
   // views in flight: S1-S2 of each view run on its slot's stream, S3-S6 of a whole batch in one launch per stage on
   // the caller's stream; two sets of `concurrency` slots alternate so the next batch's S1-S2 overlap this batch's S3-S6
   std::vector<ViewSlot*> slots;
-  int concurrency = MAX_BATCH;
+  int concurrency = 0;                  // views per batch; 0 = automatic (8, or 16 for images of fewer than 2,000 tiles)
   cudaEvent_t ev_fork = nullptr;
   cudaEvent_t ev_set_done[2] = {nullptr, nullptr};   // S3-S6 of the last batch that used slot set 0 / 1
   cudaStream_t raster_st[2] = {nullptr, nullptr};    // S3-S6 of the batches of slot set 0 / 1 (forked from / joined into the caller's stream)
@@ -490,7 +490,11 @@ int expand_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int mode, flo
 // stream; S3, S4 and S5+S6 of the whole batch are one launch each on the caller's stream.  Two slot sets alternate, so the
 // S1-S2 work of batch b+1 overlaps the S3-S6 launches of batch b.  Everything is ordered by events: the call never blocks.
 int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_scores, cudaStream_t st, const BlockCache* cache = nullptr) {
-  const int V = std::max(1, std::min(ctx->concurrency, MAX_BATCH));
+  // automatic batch size: 8 views of a 1280 x 720 image are 28,800 (view, tile) positions for the ~2,400 resident S4 warps;
+  // smaller images get 16 views per batch so that every warp still draws several positions
+  int V = ctx->concurrency;
+  if (V <= 0) V = (n > 0 && make_grid(h_cams[0].width, h_cams[0].height).tiles_x * make_grid(h_cams[0].width, h_cams[0].height).tiles_y < 2000) ? 16 : 8;
+  V = std::max(1, std::min(V, MAX_BATCH));
   CK(cudaEventRecord(ctx->ev_fork, st));
   for (int s = 0; s < 2; ++s) CK(cudaStreamWaitEvent(ctx->raster_st[s], ctx->ev_fork, 0));
   int rc = NBV_OK;
@@ -644,7 +648,7 @@ void nbv_destroy(nbv_ctx* ctx) {
 
 int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight) {
   if (!ctx) return NBV_ERR_INVALID_ARG;
-  if (views_in_flight < 1 || views_in_flight > MAX_BATCH) return fail(ctx, NBV_ERR_INVALID_ARG, "views_in_flight must be in [1, 8]");
+  if (views_in_flight < 1 || views_in_flight > MAX_BATCH) return fail(ctx, NBV_ERR_INVALID_ARG, "views_in_flight must be in [1, 16]");
   ctx->concurrency = views_in_flight;
   return NBV_OK;
 }
