@@ -11,6 +11,9 @@
 //     which is the same number without the binary32 cancellation of two log-dets of size ~100.
 //     U is factored once per scoring call (prepare_kernel); per candidate one thread per touched Gaussian does the
 //     two-sided triangular solve and a Cholesky of I + W whose pivots 1 + e_j enter as log1p(e_j).
+#include <algorithm>
+#include <cstdlib>
+
 #include "kernels.h"
 
 namespace nbv {
@@ -587,186 +590,236 @@ __device__ void cholesky_L(float* Mx, int L) {
   }
 }
 
-// log det(I + U^-T B U^-1), packed L x L (as gain_solve)
-__device__ float gain_solve_L(float* B, const float* U, int L) {
-  for (int k = 0; k < L; ++k) {
-    const float inv = 1.0f / U[triL(k, k, L)];
-    const float bkk = B[triL(k, k, L)] * inv * inv;
-    B[triL(k, k, L)] = bkk;
-    if (k < L - 1) {
-      const float ct = -0.5f * bkk;
-      for (int j = k + 1; j < L; ++j) B[triL(k, j, L)] = fmaf(ct, U[triL(k, j, L)], B[triL(k, j, L)] * inv);
-      for (int i = k + 1; i < L; ++i) {
-        const float bki = B[triL(k, i, L)], uki = U[triL(k, i, L)];
-        for (int j = i; j < L; ++j) B[triL(i, j, L)] -= bki * U[triL(k, j, L)] + uki * B[triL(k, j, L)];
-      }
-      for (int j = k + 1; j < L; ++j) B[triL(k, j, L)] = fmaf(ct, U[triL(k, j, L)], B[triL(k, j, L)]);
-      for (int j = k + 1; j < L; ++j) {
-        float v = B[triL(k, j, L)];
-        for (int i = k + 1; i < j; ++i) v -= U[triL(i, j, L)] * B[triL(k, i, L)];
-        B[triL(k, j, L)] = v / U[triL(j, j, L)];
-      }
-    }
-  }
-  float ld = 0.f;
-  for (int j = 0; j < L; ++j) {
-    float e = B[triL(j, j, L)];
-    for (int k = 0; k < j; ++k) e -= B[triL(k, j, L)] * B[triL(k, j, L)];
-    e = fmaxf(e, 0.f);
-    ld += log1pf(e);
-    const float inv = rsqrtf(1.0f + e);
-    for (int i = j + 1; i < L; ++i) {
-      float v = B[triL(j, i, L)];
-      for (int k = 0; k < j; ++k) v -= B[triL(k, j, L)] * B[triL(k, i, L)];
-      B[triL(j, i, L)] = v * inv;
-    }
-  }
-  return ld;
+// ---- S5' + S6 of a mask context, warp-cooperative: ONE WARP PER TOUCHED GAUSSIAN, the L x L block and the factor in shared
+// memory.  Lane l owns the columns (or rows) l, l + 32 of the matrices, so the triangular solves and the elimination run
+// on up to 63 columns at once (a first version ran one thread per Gaussian over 2 x 2016 floats of local memory).
+//   W = U^-T (c H) U^-1 : (a) every lane solves U^T x = h_j for its columns j, in place; (b) every lane solves
+//   U^T y = (row i of the result)^T for its rows i, in place.   log det(I + W): right-looking Cholesky on the excess
+//   (pivot 1 + e_j enters as log1p(e_j), as in gain_solve), one column per step, the trailing rows updated in parallel.
+struct MaskWarpLayout {
+  int LS;          // row stride of H and U (odd: conflict-free column and row walks)
+  int per_warp;    // floats per warp
+  int oH, oU, oA, oAQ, oMom, oX, oP, oMono;
+};
+__host__ __device__ inline MaskWarpLayout mask_warp_layout(int K, int groups) {
+  MaskWarpLayout m;
+  const int L = 11 + K;
+  m.LS = L | 1;
+  int o = 0;
+  m.oH = o; o += m.LS * L;
+  m.oU = o; o += m.LS * L;
+  m.oA = o; o += 66;
+  m.oAQ = o; o += 66;
+  m.oMom = o; o += groups * NMOM;
+  m.oX = o; o += K * 6;
+  m.oP = o; o += K;
+  m.oMono = o; o += 16;
+  m.per_warp = (o + 3) & ~3;
+  return m;
 }
 
-// S5' (+ S6) of a mask context.  KMAX bounds the per-thread arrays: L <= 11 + KMAX.
-template <int KMAX>
-__global__ void __launch_bounds__(64) expand_mask_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
-                                                          const __grid_constant__ ExpandBatch batch, int mode, int groups,
-                                                          float* __restrict__ H_T, const float* __restrict__ conf,
-                                                          const float* __restrict__ cholT) {
-  constexpr int LMAX = 11 + KMAX, LBMAX = LMAX * (LMAX + 1) / 2;
+__global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
+                                                                const __grid_constant__ ExpandBatch batch, int mode, int groups,
+                                                                float* __restrict__ H_T, const float* __restrict__ conf,
+                                                                const float* __restrict__ cholT) {
+  extern __shared__ __align__(16) float smem[];
   const ExpandView& vw = batch.v[blockIdx.y];
   const int K = sc.K, L = 11 + K, LB = L * (L + 1) / 2, bgch = cfg.mask_bg_channel;
+  const MaskWarpLayout lay = mask_warp_layout(K, groups);
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5, LS = lay.LS;
+  float* base = smem + (size_t)wib * lay.per_warp;
+  float *Hm = base + lay.oH, *Um = base + lay.oU, *As = base + lay.oA, *AQs = base + lay.oAQ, *mom = base + lay.oMom;
+  float *xs = base + lay.oX, *ps = base + lay.oP, *mono = base + lay.oMono;
   const uint32_t n_touched = vw.counters->n_touched;
   const int stride = NMOM * groups;
   float gain = 0.f;
-  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < n_touched; t += gridDim.x * blockDim.x) {
+  for (uint32_t t = blockIdx.x * wpb + wib; t < n_touched; t += gridDim.x * wpb) {
     const uint32_t r = vw.touched[t];
     const uint32_t g = vw.ids_sorted[r];
-    const Splat sp = vw.splat_sorted[r];
-    const float cA = -2.f * sp.qa, cB = -sp.qb, cC = -2.f * sp.qc, icC = 1.0f / cC;
-    const float i11 = sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), sh = -cB * icC, i22 = sqrtf(cC);   // as in S4
-    float mono[15], x[KMAX][6], p[KMAX];
+    __syncwarp();
+    // moments of all groups -> shared memory (and zero the buffer for the next view)
+    float* gm = vw.moments + (size_t)r * stride;
+    for (int i = lane; i < stride; i += 32) { mom[i] = gm[i]; gm[i] = 0.f; }
+    __syncwarp();
+    {   // whitened basis -> u basis, one lane per group
+      const Splat sp = vw.splat_sorted[r];
+      const float cA = -2.f * sp.qa, cB = -sp.qb, cC = -2.f * sp.qc, icC = 1.0f / cC;
+      const float i11 = sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), sh = -cB * icC, i22 = sqrtf(cC);   // as in S4
+      for (int gr = lane; gr < groups; gr += 32) {
+        float m[NMOM];
 #pragma unroll
-    for (int i = 0; i < 15; ++i) mono[i] = 0.f;
-    float W2 = 0.f;
-    for (int gr = 0; gr < groups; ++gr) {
-      float4* mom4 = reinterpret_cast<float4*>(vw.moments + (size_t)r * stride + (size_t)gr * NMOM);
-      float m[NMOM];
+        for (int i = 0; i < NMOM; ++i) m[i] = mom[gr * NMOM + i];
+        moments_to_u_basis(m, i11, -sh * i22, 0.0f, i22);
 #pragma unroll
-      for (int i = 0; i < NMOM / 4; ++i) {
-        const float4 v = mom4[i];
-        m[4 * i] = v.x; m[4 * i + 1] = v.y; m[4 * i + 2] = v.z; m[4 * i + 3] = v.w;
-        mom4[i] = make_float4(0.f, 0.f, 0.f, 0.f);     // leave the buffer zeroed for the next view
-      }
-      moments_to_u_basis(m, i11, -sh * i22, 0.0f, i22);
-#pragma unroll
-      for (int i = 0; i < 15; ++i) mono[i] += m[i];
-      if (gr == 0) W2 = m[MOM_W2];                       // sum w^2 does not depend on the channel values
-      for (int j = 0; j < 4; ++j) {
-        const int slot = 4 * gr + j;
-        if (slot < K)
-          for (int i = 0; i < 6; ++i) x[slot][i] = m[MOM_X + 6 * j + i];
+        for (int i = 0; i < NMOM; ++i) mom[gr * NMOM + i] = m[i];
       }
     }
-    float S2 = 0.f;
-    for (int slot = 0; slot < K; ++slot) {
-      p[slot] = expf(sc.logits[(size_t)g * K + mask_channel_of_slot(slot, bgch)] - sc.lse[g]);
-      S2 += p[slot] * p[slot];
+    __syncwarp();
+    if (lane < 15) {
+      float v = 0.f;
+      for (int gr = 0; gr < groups; ++gr) v += mom[gr * NMOM + lane];
+      mono[lane] = v;
     }
-    ChainF ch;
-    chain_f(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
-    const float sg = sc.sigma[g];
-    const float kappa = cfg.opacity_coord == 0 ? (1.f - sg) : 1.f / sg;       // R-10
-    float A[11][6];
-#pragma unroll
-    for (int k = 0; k < 10; ++k) {
-      A[k][0] = ch.G[0][k]; A[k][1] = ch.G[1][k]; A[k][2] = 0.5f * ch.G[2][k]; A[k][3] = ch.G[3][k]; A[k][4] = 0.5f * ch.G[4][k]; A[k][5] = 0.f;
+    if (lane == 15) mono[15] = mom[MOM_W2];
+    for (int i = lane; i < K * 6; i += 32) {
+      const int slot = i / 6, e = i - 6 * slot;
+      xs[i] = mom[(slot >> 2) * NMOM + MOM_X + 6 * (slot & 3) + e];
+    }
+    float s2p = 0.f;
+    for (int slot = lane; slot < K; slot += 32) {
+      const float pv = expf(sc.logits[(size_t)g * K + mask_channel_of_slot(slot, bgch)] - sc.lse[g]);
+      ps[slot] = pv;
+      s2p += pv * pv;
     }
 #pragma unroll
-    for (int e = 0; e < 5; ++e) A[10][e] = 0.f;
-    A[10][5] = kappa;
-    float H[LBMAX];
-    for (int i = 0; i < LB; ++i) H[i] = 0.f;
-    {   // geo-geo: A Q A^T
+    for (int o = 16; o > 0; o >>= 1) s2p += __shfl_xor_sync(0xffffffffu, s2p, o);
+    const float S2 = s2p;
+    {   // chain rule (every lane, redundantly), A and A Q into shared memory for dynamic indexing
+      ChainF ch;
+      chain_f(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
+      const float sg = sc.sigma[g];
+      const float kappa = cfg.opacity_coord == 0 ? (1.f - sg) : 1.f / sg;       // R-10
+      if (lane < 11) {
+        float a6[6];
+        if (lane < 10) {
+          a6[0] = ch.G[0][lane]; a6[1] = ch.G[1][lane]; a6[2] = 0.5f * ch.G[2][lane]; a6[3] = ch.G[3][lane]; a6[4] = 0.5f * ch.G[4][lane]; a6[5] = 0.f;
+        } else {
+          a6[0] = a6[1] = a6[2] = a6[3] = a6[4] = 0.f; a6[5] = kappa;
+        }
+#pragma unroll
+        for (int e = 0; e < 6; ++e) As[lane * 6 + e] = a6[e];
+      }
+    }
+    __syncwarp();
+    if (lane < 11) {
       const int ex[6] = {1, 0, 2, 1, 0, 0}, ey[6] = {0, 1, 0, 1, 2, 0};
-      float AQ[11][6];
-      for (int k = 0; k < 11; ++k)
-        for (int j = 0; j < 6; ++j) {
-          float v = 0.f;
-          for (int i = 0; i < 6; ++i) v += A[k][i] * mono[mono_index(ex[i] + ex[j], ey[i] + ey[j])];
-          AQ[k][j] = v;
-        }
-      for (int k = 0; k < 11; ++k)
-        for (int l = k; l < 11; ++l) {
-          float v = 0.f;
-          for (int j = 0; j < 6; ++j) v += AQ[k][j] * A[l][j];
-          H[triL(k, l, L)] = v;
-        }
+      for (int j = 0; j < 6; ++j) {
+        float v = 0.f;
+        for (int i = 0; i < 6; ++i) v += As[lane * 6 + i] * mono[mono_index(ex[i] + ex[j], ey[i] + ey[j])];
+        AQs[lane * 6 + j] = v;
+      }
     }
-    {   // geo-logit: p_j (A x_j - sum_k p_k A x_k)
-      float xbar[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-      for (int slot = 0; slot < K; ++slot)
-        for (int i = 0; i < 6; ++i) xbar[i] += p[slot] * x[slot][i];
-      for (int c = 0; c < K; ++c) {
-        const int slot = mask_slot_of_channel(c, bgch);
-        float dx6[6];
-        for (int i = 0; i < 6; ++i) dx6[i] = p[slot] * (x[slot][i] - xbar[i]);
-        for (int k = 0; k < 11; ++k) {
+    __syncwarp();
+    const float W2 = mono[15];
+    float xbar[6];
+#pragma unroll
+    for (int e = 0; e < 6; ++e) {
+      float v = 0.f;
+      for (int slot = 0; slot < K; ++slot) v += ps[slot] * xs[slot * 6 + e];
+      xbar[e] = v;
+    }
+    // the full symmetric block, column j by lane j (and j + 32)
+    for (int j = lane; j < L; j += 32) {
+      if (j < 11) {
+        for (int i = 0; i < 11; ++i) {
           float v = 0.f;
-          for (int i = 0; i < 6; ++i) v += A[k][i] * dx6[i];
-          H[triL(k, 11 + c, L)] = v;
+#pragma unroll
+          for (int e = 0; e < 6; ++e) v += AQs[i * 6 + e] * As[j * 6 + e];
+          Hm[i * LS + j] = v;
+        }
+        for (int c = 0; c < K; ++c) {
+          const int slot = mask_slot_of_channel(c, bgch);
+          float v = 0.f;
+#pragma unroll
+          for (int e = 0; e < 6; ++e) v += As[j * 6 + e] * (ps[slot] * (xs[slot * 6 + e] - xbar[e]));
+          Hm[(11 + c) * LS + j] = v;
+        }
+      } else {
+        const int c = j - 11, slot = mask_slot_of_channel(c, bgch);
+        const float pc = ps[slot];
+        for (int i = 0; i < 11; ++i) {
+          float v = 0.f;
+#pragma unroll
+          for (int e = 0; e < 6; ++e) v += As[i * 6 + e] * (pc * (xs[slot * 6 + e] - xbar[e]));
+          Hm[i * LS + j] = v;
+        }
+        for (int d = 0; d < K; ++d) {
+          const float pd = ps[mask_slot_of_channel(d, bgch)];
+          float v = pc * pd * (S2 - pc - pd);
+          if (d == c) v += pc * pc;
+          Hm[(11 + d) * LS + j] = W2 * v;
         }
       }
     }
-    for (int c = 0; c < K; ++c) {   // logit-logit
-      const float pc = p[mask_slot_of_channel(c, bgch)];
-      for (int d = c; d < K; ++d) {
-        const float pd = p[mask_slot_of_channel(d, bgch)];
-        float v = pc * pd * (S2 - pc - pd);
-        if (d == c) v += pc * pc;
-        H[triL(11 + c, 11 + d, L)] = W2 * v;
+    __syncwarp();
+    if (mode == EXPAND_TRAIN || mode == EXPAND_VIEW) {
+      float* dst = (mode == EXPAND_TRAIN ? H_T : vw.out_blocks) + (size_t)g * LB;
+      for (int rr = 0; rr < L; ++rr)
+        for (int c = rr + lane; c < L; c += 32) {
+          if (mode == EXPAND_TRAIN) atomicAdd(dst + triL(rr, c, L), Hm[rr * LS + c]);
+          else dst[triL(rr, c, L)] = Hm[rr * LS + c];
+        }
+      continue;
+    }
+    const float cg = conf[g];
+    float gn = 0.f;
+    if (cg > 0.f) {
+      const float* ut = cholT + (size_t)g * LB;
+      for (int rr = 0; rr < L; ++rr)
+        for (int c = rr + lane; c < L; c += 32) Um[rr * LS + c] = ut[triL(rr, c, L)];
+      __syncwarp();
+      // (a) columns: U^T x = c h_j
+      for (int j = lane; j < L; j += 32)
+        for (int i = 0; i < L; ++i) {
+          float v = cg * Hm[i * LS + j];
+          for (int k = 0; k < i; ++k) v -= Um[k * LS + i] * Hm[k * LS + j];
+          Hm[i * LS + j] = v / Um[i * LS + i];
+        }
+      __syncwarp();
+      // (b) rows: U^T y = (row i)^T
+      for (int i = lane; i < L; i += 32)
+        for (int c = 0; c < L; ++c) {
+          float v = Hm[i * LS + c];
+          for (int k = 0; k < c; ++k) v -= Um[k * LS + c] * Hm[i * LS + k];
+          Hm[i * LS + c] = v / Um[c * LS + c];
+        }
+      __syncwarp();
+      // log det(I + W): right-looking Cholesky on the excess, lower triangle
+      for (int j = 0; j < L; ++j) {
+        const float e = fmaxf(Hm[j * LS + j], 0.f);
+        gn += log1pf(e);
+        const float inv = rsqrtf(1.0f + e);
+        __syncwarp();
+        for (int i = j + 1 + lane; i < L; i += 32) Hm[i * LS + j] *= inv;
+        __syncwarp();
+        for (int i = j + 1 + lane; i < L; i += 32) {
+          const float li = Hm[i * LS + j];
+          for (int k = j + 1; k <= i; ++k) Hm[i * LS + k] -= li * Hm[k * LS + j];
+        }
+        __syncwarp();
       }
     }
-    if (mode == EXPAND_TRAIN) {
-      float* dst = H_T + (size_t)g * LB;
-      for (int i = 0; i < LB; ++i) atomicAdd(dst + i, H[i]);
-    } else if (mode == EXPAND_VIEW) {
-      float* dst = vw.out_blocks + (size_t)g * LB;
-      for (int i = 0; i < LB; ++i) dst[i] = H[i];
-    } else {
-      const float c = conf[g];
-      float gn = 0.f;
-      if (c > 0.f) {
-        float U[LBMAX];
-        const float* ut = cholT + (size_t)g * LB;
-        for (int i = 0; i < LB; ++i) { U[i] = ut[i]; H[i] *= c; }
-        gn = gain_solve_L(H, U, L);
-      }
+    if (lane == 0) {
       if (vw.gains) vw.gains[g] = gn;
       gain += gn;
     }
   }
   if (mode == EXPAND_GAIN) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) gain += __shfl_xor_sync(0xffffffffu, gain, o);
-    __shared__ float ws[2];
-    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = gain;
+    __shared__ float ws[8];
+    if (lane == 0) ws[wib] = gain;
     __syncthreads();
     if (threadIdx.x == 0) {
-      const float t = ws[0] + ws[1];
-      if (t != 0.f) atomicAdd(vw.score, t);
+      float tsum = 0.f;
+      for (int w = 0; w < wpb; ++w) tsum += ws[w];
+      if (tsum != 0.f) atomicAdd(vw.score, tsum);
     }
   }
 }
 
 void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, float* H_T,
                         const float* conf, const float* cholT, cudaStream_t st) {
-  int blocks = (sc.N + 63) / 64;
-  const int cap = (148 * 8 + batch.n - 1) / batch.n;
-  if (blocks > cap) blocks = cap;
-  const dim3 grid((unsigned)blocks, (unsigned)batch.n);
   ++g_kernel_launches;
-  if (sc.K <= 20)
-    expand_mask_kernel<20><<<grid, 64, 0, st>>>(sc, cfg, batch, mode, groups, H_T, conf, cholT);
-  else
-    expand_mask_kernel<NBV_MASK_KMAX><<<grid, 64, 0, st>>>(sc, cfg, batch, mode, groups, H_T, conf, cholT);
+  const MaskWarpLayout lay = mask_warp_layout(sc.K, groups);
+  int wpb = 8;
+  while (wpb > 1 && (size_t)wpb * lay.per_warp * 4 > 200 * 1024) wpb >>= 1;
+  const size_t smem = (size_t)wpb * lay.per_warp * 4;
+  static size_t configured = 0;
+  if (smem > configured) {
+    cudaFuncSetAttribute(expand_mask_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = smem;
+  }
+  const int blocks = std::max(1, (148 * 2 + batch.n - 1) / batch.n);
+  expand_mask_warp_kernel<<<dim3((unsigned)blocks, (unsigned)batch.n), wpb * 32, smem, st>>>(sc, cfg, batch, mode, groups, H_T, conf, cholT);
 }
 
 // once per scoring call of a mask context: U_g = upper Cholesky factor of c_g H_T,g + Lambda (L x L)
