@@ -17,6 +17,14 @@ def _small_workload(n_train=3, n_cand=4):
     return wl
 
 
+def test_fusion_weight_defaults_are_the_papers():
+    import inspect, json, os
+    gold = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "spec_examples.json")))["fusion_weights"]
+    sig = inspect.signature(orc.fused_gain3).parameters
+    assert sig["beta_d"].default == gold["beta_d"] and sig["beta_o"].default == gold["beta_o"]
+    assert inspect.signature(orc.score_candidates_fused).parameters["beta_d"].default == gold["beta_d"]
+
+
 def test_normalized_and_fused_gain_hand_numbers():
     # Eq. 10: 3 / mean(1, 2, 3) = 1.5 ; Eq. 11 with beta_d = 10: 0.5 + 10 * 0.2 = 2.5
     assert orc.normalized_gain(3.0, [1.0, 2.0, 3.0]) == pytest.approx(1.5, abs=1e-15)
