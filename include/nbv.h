@@ -84,6 +84,12 @@ typedef struct nbv_config {
   /* mask contexts (channel_mask == NBV_CH_MASK) only: */
   int32_t mask_bg_channel;   /* 0      object channel that receives the residual 1 - 1^T O' (Eq. 2: the background label) */
   float prior_precision_obj; /* 1.0    diagonal of Lambda on the K object logits */
+  /* where the confidence c_g acts (the paper's equation and its prose differ, R-14):
+   * 0 (default, R1) Eq. 9 literal, H := J^T C J for every view: IG_g = logdet(c (H_T + H_c) + L) - logdet(c H_T + L)
+   * 1 (R2) "weighting each Gaussian's information gain":  IG_g = c [logdet(H_T + H_c + L) - logdet(H_T + L)]
+   * 2 (R3) "scale each Jacobian ... during information gain computation", candidate only:
+   *        IG_g = logdet(H_T + c H_c + L) - logdet(H_T + L).      c_g = 0 gives exactly 0 in all three. */
+  int32_t weight_mode;
 } nbv_config;
 
 typedef struct nbv_ctx nbv_ctx;

@@ -369,18 +369,28 @@ def confidence(obj_logits, opacity, alpha_obj=0.3, alpha_opa=0.3, target=-1, p_f
     return np.where(am == target, c, 0.0)
 
 
-def gaussian_gains(H_T, H_c, c, prior) -> np.ndarray:
-    """Per-Gaussian information gain (Eq. 5, 6, 9; block-diagonal, L210):
-        IG_g = log det(c_g (H_T,g + H_c,g) + Lambda) - log det(c_g H_T,g + Lambda)
-    H_T, H_c: (N,105) packed; c: (N,); prior: (14,) diagonal of Lambda (reading R-13)."""
+def gaussian_gains(H_T, H_c, c, prior, weight_mode: int = 0) -> np.ndarray:
+    """Per-Gaussian information gain (PAPER.md Eq. 5, 6, 9; block-diagonal, L210).  H_T, H_c: (N,105) packed; c: (N,);
+    prior: (14,) diagonal of Lambda (reading R-13).  Where the confidence acts (reading R-14):
+      weight_mode 0 (R1, Eq. 9 literal "H := J^T C J"): log det(c (H_T + H_c) + Lambda) - log det(c H_T + Lambda)
+      weight_mode 1 (R2, L61 "weighting each Gaussian's information gain"): c [log det(H_T + H_c + Lambda) - log det(H_T + Lambda)]
+      weight_mode 2 (R3, L238 "scale each Jacobian ... during information gain computation", candidate only):
+                     log det(H_T + c H_c + Lambda) - log det(H_T + Lambda)"""
     Lam = np.diag(np.asarray(prior, dtype=np.float64))
     A = unpack_blocks(H_T)
     B = unpack_blocks(H_c)
-    c = np.asarray(c, dtype=np.float64)[:, None, None]
-    s1, l1 = np.linalg.slogdet(c * (A + B) + Lam)
-    s0, l0 = np.linalg.slogdet(c * A + Lam)
+    cv = np.asarray(c, dtype=np.float64)
+    c3 = cv[:, None, None]
+    if weight_mode == 0:
+        M1, M0, out_scale = c3 * (A + B) + Lam, c3 * A + Lam, 1.0
+    elif weight_mode == 1:
+        M1, M0, out_scale = A + B + Lam, A + Lam, cv
+    else:
+        M1, M0, out_scale = A + c3 * B + Lam, A + Lam, 1.0
+    s1, l1 = np.linalg.slogdet(M1)
+    s0, l0 = np.linalg.slogdet(M0)
     assert np.all(s1 > 0) and np.all(s0 > 0)
-    return l1 - l0
+    return out_scale * (l1 - l0)
 
 
 def argmax_lowest(scores) -> int:
@@ -390,7 +400,7 @@ def argmax_lowest(scores) -> int:
 
 
 def score_candidates(scene: OracleScene, train_cams, cand_cams, target=-1, alpha_obj=0.3, alpha_opa=0.3,
-                     prior=None, H_T=None):
+                     prior=None, H_T=None, weight_mode: int = 0):
     """The whole hot path on the CPU.  Returns dict(H_T, scores, best, conf, gains (C,N))."""
     prior = np.ones(P) if prior is None else np.asarray(prior, dtype=np.float64)
     if H_T is None:
@@ -401,7 +411,7 @@ def score_candidates(scene: OracleScene, train_cams, cand_cams, target=-1, alpha
     scores, gains = [], []
     for cam in np.atleast_1d(cand_cams):
         H_c = scene.view_hessian(cam)
-        g = gaussian_gains(H_T, H_c, conf, prior)
+        g = gaussian_gains(H_T, H_c, conf, prior, weight_mode)
         gains.append(g)
         scores.append(g.sum())
     scores = np.array(scores)

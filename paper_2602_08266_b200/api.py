@@ -55,7 +55,7 @@ class Config(C.Structure):
         ("t_stop", C.c_float), ("bg", C.c_float * 3), ("channel_mask", C.c_int32), ("channel_weight", C.c_float * 4),
         ("opacity_coord", C.c_int32), ("alpha_obj", C.c_float), ("alpha_opa", C.c_float), ("p_floor", C.c_float),
         ("sigma_floor", C.c_float), ("prior_precision", C.c_float * 14), ("mask_bg_channel", C.c_int32),
-        ("prior_precision_obj", C.c_float),
+        ("prior_precision_obj", C.c_float), ("weight_mode", C.c_int32),
     ]
 
 

@@ -356,8 +356,10 @@ __global__ void __launch_bounds__(64) expand_kernel(const __grid_constant__ Scen
       if (c > 0.f) {                       // c_g = 0 (Eq. 12, non-target): exactly zero gain
         float U[NBLK];
         const float* ut = cholT + (size_t)g * NBLK;
-        for (int i = 0; i < NBLK; ++i) { U[i] = ut[i]; H[i] *= c; }
+        const float cb = cfg.weight_mode == 1 ? 1.0f : c;         // R2 weights the gain, R1 / R3 the candidate block
+        for (int i = 0; i < NBLK; ++i) { U[i] = ut[i]; H[i] *= cb; }
         gn = gain_solve(H, U);
+        if (cfg.weight_mode == 1) gn *= c;
       }
       if (gains) gains[g] = gn;
       gain += gn;
@@ -416,7 +418,7 @@ void launch_expand_cache(const SceneDev& sc, const nbv_config& cfg, const Expand
 
 // One thread per cached (candidate, Gaussian) entry: the gain of Eq. 5/6/9 of that block against the current factor U_g.
 __global__ void __launch_bounds__(64) cached_gain_kernel(BlockCache cache, const int32_t* __restrict__ taken, const float* __restrict__ conf,
-                                                         const float* __restrict__ cholT, float* __restrict__ scores) {
+                                                         const float* __restrict__ cholT, float* __restrict__ scores, int weight_mode) {
   const int c = blockIdx.y;
   float gain = 0.f;
   if (!taken[c]) {
@@ -429,8 +431,10 @@ __global__ void __launch_bounds__(64) cached_gain_kernel(BlockCache cache, const
         float H[NBLK], U[NBLK];
         const float* hb = cache.blocks + e * NBLK;
         const float* ut = cholT + (size_t)g * NBLK;
-        for (int i = 0; i < NBLK; ++i) { U[i] = ut[i]; H[i] = cg * hb[i]; }
-        gain += gain_solve(H, U);
+        const float cb = weight_mode == 1 ? 1.0f : cg;
+        for (int i = 0; i < NBLK; ++i) { U[i] = ut[i]; H[i] = cb * hb[i]; }
+        const float gn = gain_solve(H, U);
+        gain += weight_mode == 1 ? cg * gn : gn;
       }
     }
   }
@@ -446,9 +450,9 @@ __global__ void __launch_bounds__(64) cached_gain_kernel(BlockCache cache, const
 }
 
 void launch_cached_gain(const BlockCache& cache, int n_cand, const int32_t* taken, const float* conf, const float* cholT, float* scores,
-                        cudaStream_t st) {
+                        int weight_mode, cudaStream_t st) {
   ++g_kernel_launches;
-  cached_gain_kernel<<<dim3(64, (unsigned)n_cand), 64, 0, st>>>(cache, taken, conf, cholT, scores);
+  cached_gain_kernel<<<dim3(64, (unsigned)n_cand), 64, 0, st>>>(cache, taken, conf, cholT, scores, weight_mode);
 }
 
 __global__ void __launch_bounds__(256) cache_accumulate_kernel(BlockCache cache, const int32_t* __restrict__ pick, float* __restrict__ H_T) {
@@ -498,7 +502,8 @@ __global__ void __launch_bounds__(64) prepare_kernel(int N, nbv_config cfg, cons
   if (!(c > 0.f)) return;
   const float* ht = H_T + (size_t)g * NBLK;
   float H[NBLK];
-  for (int i = 0; i < NBLK; ++i) H[i] = c * ht[i];
+  const float ct = cfg.weight_mode == 0 ? c : 1.0f;           // Eq. 9 literal (R1) weights H_T as well; R2 / R3 do not
+  for (int i = 0; i < NBLK; ++i) H[i] = ct * ht[i];
   for (int k = 0; k < P; ++k) H[tri(k, k)] += cfg.prior_precision[k];
   cholesky_packed(H);
   float* dst = cholT + (size_t)g * NBLK;
@@ -752,6 +757,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       continue;
     }
     const float cg = conf[g];
+    const float cb = cfg.weight_mode == 1 ? 1.0f : cg;
     float gn = 0.f;
     if (cg > 0.f) {
       const float* ut = cholT + (size_t)g * LB;
@@ -761,7 +767,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       // (a) columns: U^T x = c h_j
       for (int j = lane; j < L; j += 32)
         for (int i = 0; i < L; ++i) {
-          float v = cg * Hm[i * LS + j];
+          float v = cb * Hm[i * LS + j];
           for (int k = 0; k < i; ++k) v -= Um[k * LS + i] * Hm[k * LS + j];
           Hm[i * LS + j] = v / Um[i * LS + i];
         }
@@ -789,6 +795,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
         __syncwarp();
       }
     }
+    if (cfg.weight_mode == 1) gn *= cg;
     if (lane == 0) {
       if (vw.gains) vw.gains[g] = gn;
       gain += gn;
@@ -834,7 +841,8 @@ __global__ void __launch_bounds__(64) prepare_mask_kernel(int N, int K, nbv_conf
   const int L = 11 + K, LB = L * (L + 1) / 2;
   const float* ht = H_T + (size_t)g * LB;
   float H[LBMAX];
-  for (int i = 0; i < LB; ++i) H[i] = c * ht[i];
+  const float ct = cfg.weight_mode == 0 ? c : 1.0f;
+  for (int i = 0; i < LB; ++i) H[i] = ct * ht[i];
   for (int k = 0; k < L; ++k) H[triL(k, k, L)] += k < 11 ? cfg.prior_precision[k] : cfg.prior_precision_obj;
   cholesky_L(H, L);
   float* dst = cholT + (size_t)g * LB;

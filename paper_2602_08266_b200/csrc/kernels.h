@@ -127,7 +127,7 @@ void launch_cache_reserve(const ExpandBatch& batch, const BlockCache& cache, int
 void launch_expand_cache(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, const BlockCache& cache, cudaStream_t st);
 // scores[c] += sum over the cached entries of candidate c of the gain against cholT (skipped when taken[c] != 0)
 void launch_cached_gain(const BlockCache& cache, int n_cand, const int32_t* taken, const float* conf, const float* cholT, float* scores,
-                        cudaStream_t st);
+                        int weight_mode, cudaStream_t st);
 // H_T[g] += block for the cached entries of candidate *pick
 void launch_cache_accumulate(const BlockCache& cache, const int32_t* pick, float* H_T, cudaStream_t st);
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);

@@ -586,6 +586,7 @@ void nbv_default_config(nbv_config* cfg) {
   for (int k = 0; k < NBV_P; ++k) cfg->prior_precision[k] = 1.0f;
   cfg->mask_bg_channel = 0;
   cfg->prior_precision_obj = 1.0f;
+  cfg->weight_mode = 0;
 }
 
 int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
@@ -597,6 +598,7 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
                   c.alpha_max < 1.f && c.t_stop > 0.f && c.t_stop < 1.f &&
                   (c.channel_mask == NBV_CH_MASK || ((c.channel_mask & 15) != 0 && (c.channel_mask & ~15) == 0)) &&
                   c.mask_bg_channel >= 0 && c.prior_precision_obj > 0.f && std::isfinite(c.prior_precision_obj) &&
+                  c.weight_mode >= 0 && c.weight_mode <= 2 &&
                   (c.opacity_coord == 0 || c.opacity_coord == 1) && c.p_floor > 0.f && c.sigma_floor > 0.f;
   if (!ok) return NBV_ERR_INVALID_ARG;
   for (int k = 0; k < NBV_P; ++k)
@@ -865,7 +867,7 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
   for (int r = 0; r < rounds; ++r) {
     CKRET(prepare_scoring(ctx, target_obj, st));
     CK(cudaMemsetAsync(d_round, 0, 4 * (size_t)n, st));
-    launch_cached_gain(bc, n, d_taken, ctx->conf.as<float>(), ctx->cholT.as<float>(), d_round, st);
+    launch_cached_gain(bc, n, d_taken, ctx->conf.as<float>(), ctx->cholT.as<float>(), d_round, ctx->cfg.weight_mode, st);
     launch_greedy_pick(d_round, d_taken, n, d_scores ? d_scores + (size_t)r * n : nullptr, d_pick, d_order + r, st);
     launch_cache_accumulate(bc, d_pick, ctx->H_T.as<float>(), st);      // Eq. 6: H_T += H(c*)
     CK(cudaGetLastError());

@@ -268,3 +268,23 @@ def test_mixed_image_sizes_and_batching_do_not_change_scores(wl):
         assert int(best.item()) == int(np.argmax(single))
     ref = orc.score_candidates(make_oracle_scene(wl.scene), wl.train_cams, cams[[2, 7]])["scores"]
     np.testing.assert_allclose(single[[2, 7]], ref, rtol=1e-3, atol=1e-6)
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_weight_modes_match_the_oracle(wl, mode):
+    """R2 / R3 readings of where the confidence acts (nbv_config.weight_mode), scores, per-Gaussian gains, arg-max, and the
+    cached-block greedy path under the same mode."""
+    scn = make_oracle_scene(wl.scene)
+    nbv = _nbv(wl.scene, weight_mode=mode)
+    nbv.accumulate_training(wl.train_cams)
+    ref = orc.score_candidates(scn, wl.train_cams, wl.cand_cams, weight_mode=mode)
+    s, best = nbv.score_candidates(wl.cand_cams)
+    np.testing.assert_allclose(s.cpu().numpy(), ref["scores"], rtol=1e-3, atol=1e-6)
+    assert int(best.item()) == ref["best"]
+    g = nbv.gaussian_gains(wl.cand_cams[1]).cpu().numpy()
+    np.testing.assert_allclose(g, ref["gains"][1], rtol=1e-3, atol=1e-6)
+    base = orc.score_candidates(scn, wl.train_cams, wl.cand_cams, weight_mode=0)["scores"]
+    assert not np.allclose(ref["scores"], base, rtol=1e-3)          # the readings really differ on this scene
+    order, sc = nbv.select_greedy(wl.cand_cams, 1)
+    np.testing.assert_allclose(sc.cpu().numpy()[0], ref["scores"], rtol=1e-3, atol=1e-6)
+    assert order[0] == ref["best"]

@@ -164,3 +164,31 @@ def test_score_candidates_properties(wl0):
     for i, cam in enumerate(wl0.cand_cams):
         g = orc.gaussian_gains(res["H_T"], scn.view_hessian(cam), c_forced, np.ones(P))
         assert g.sum() == pytest.approx(rt["scores"][i], rel=1e-9)
+
+
+def test_weight_modes_closed_forms_and_limits():
+    """Where the confidence acts (reading R-14): scalar closed forms on a block a e1 e1^T + candidate b e1 e1^T, lambda = 1."""
+    a, b, c = 3.0, 5.0, 1.7
+    H_T = np.zeros((1, orc.NB)); H_c = np.zeros((1, orc.NB))
+    H_T[0, 0], H_c[0, 0] = a, b
+    one = np.ones(14)
+    g0 = orc.gaussian_gains(H_T, H_c, [c], one, 0)[0]
+    g1 = orc.gaussian_gains(H_T, H_c, [c], one, 1)[0]
+    g2 = orc.gaussian_gains(H_T, H_c, [c], one, 2)[0]
+    assert g0 == pytest.approx(np.log((c * (a + b) + 1) / (c * a + 1)), rel=1e-12)     # Eq. 9 literal
+    assert g1 == pytest.approx(c * np.log((a + b + 1) / (a + 1)), rel=1e-12)          # c weights the gain
+    assert g2 == pytest.approx(np.log((a + c * b + 1) / (a + 1)), rel=1e-12)          # c weights the candidate only
+    rng = np.random.default_rng(0)
+    X = rng.standard_normal((5, 14, 20)); Y = rng.standard_normal((5, 14, 6))
+    HT, HC = orc.pack_blocks(X @ X.transpose(0, 2, 1)), orc.pack_blocks(Y @ Y.transpose(0, 2, 1))
+    ones = np.ones(5)
+    ref = orc.gaussian_gains(HT, HC, ones, one, 0)
+    for m in (1, 2):
+        np.testing.assert_allclose(orc.gaussian_gains(HT, HC, ones, one, m), ref, rtol=1e-12)    # c = 1: all readings agree
+    cs = rng.uniform(0.5, 3.0, 5)
+    np.testing.assert_allclose(orc.gaussian_gains(HT, HC, 2 * cs, one, 1), 2 * orc.gaussian_gains(HT, HC, cs, one, 1), rtol=1e-12)
+    zero = np.zeros_like(HT)
+    np.testing.assert_allclose(orc.gaussian_gains(zero, HC, cs, one, 0), orc.gaussian_gains(zero, HC, cs, one, 2), rtol=1e-12)
+    for m in (0, 1, 2):
+        assert np.all(orc.gaussian_gains(HT, HC, np.zeros(5), one, m) == 0.0)                      # c = 0 (Eq. 12): exactly zero
+    assert np.all(orc.gaussian_gains(HT, HC, 2 * cs, one, 2) > orc.gaussian_gains(HT, HC, cs, one, 2))
