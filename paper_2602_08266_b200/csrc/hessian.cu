@@ -768,6 +768,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       for (int j = lane; j < L; j += 32)
         for (int i = 0; i < L; ++i) {
           float v = cb * Hm[i * LS + j];
+#pragma unroll 4
           for (int k = 0; k < i; ++k) v -= Um[k * LS + i] * Hm[k * LS + j];
           Hm[i * LS + j] = v / Um[i * LS + i];
         }
@@ -776,6 +777,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       for (int i = lane; i < L; i += 32)
         for (int c = 0; c < L; ++c) {
           float v = Hm[i * LS + c];
+#pragma unroll 4
           for (int k = 0; k < c; ++k) v -= Um[k * LS + c] * Hm[i * LS + k];
           Hm[i * LS + c] = v / Um[c * LS + c];
         }
@@ -790,6 +792,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
         __syncwarp();
         for (int i = j + 1 + lane; i < L; i += 32) {
           const float li = Hm[i * LS + j];
+#pragma unroll 4
           for (int k = j + 1; k <= i; ++k) Hm[i * LS + k] -= li * Hm[k * LS + j];
         }
         __syncwarp();
