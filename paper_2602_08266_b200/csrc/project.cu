@@ -153,14 +153,26 @@ __global__ void __launch_bounds__(256) project_kernel(SceneDev sc, nbv_camera ca
     rect[g] = rc;
     if (abc) { abc[3 * (size_t)g] = a; abc[3 * (size_t)g + 1] = b; abc[3 * (size_t)g + 2] = c; }
   }
-  // counters: warp-aggregated
+  // counters: aggregated over the block (one pair of atomics per block: thousands of same-address atomics per view would
+  // serialise in the L2 and cost more than the projection itself)
+  __shared__ unsigned int s_vis[8];
+  __shared__ unsigned long long s_nt[8];
   const unsigned vis_mask = __ballot_sync(0xffffffffu, visible);
   unsigned long long nt = ntiles;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) nt += __shfl_xor_sync(0xffffffffu, nt, o);
-  if ((threadIdx.x & 31) == 0 && vis_mask) {
-    atomicAdd(&counters->n_visible, (unsigned)__popc(vis_mask));
-    atomicAdd(&counters->n_keys, nt);
+  const int wid = threadIdx.x >> 5;
+  if ((threadIdx.x & 31) == 0) { s_vis[wid] = (unsigned)__popc(vis_mask); s_nt[wid] = nt; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned int v = 0;
+    unsigned long long t = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) { v += s_vis[w]; t += s_nt[w]; }
+    if (v) {
+      atomicAdd(&counters->n_visible, v);
+      atomicAdd(&counters->n_keys, t);
+    }
   }
 }
 
