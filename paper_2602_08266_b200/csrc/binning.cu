@@ -30,6 +30,15 @@ __device__ __forceinline__ uint4 super_rect(ushort4 rc, int sshift) {
 __device__ __forceinline__ bool covers_super(uint4 sr, uint32_t sx, uint32_t sy) {
   return sx >= sr.x && sx <= sr.z && sy >= sr.y && sy <= sr.w;
 }
+// bit s of the result = the supertile rect touches supertile s (row-major index); for grids of at most 64 supertiles the
+// per-supertile loops below test one bit instead of four comparisons
+__device__ __forceinline__ unsigned long long super_mask64(uint4 sr, int super_x) {
+  unsigned long long m = 0ull;
+  if (sr.x > sr.z) return m;
+  const unsigned long long row = ((2ull << (sr.z - sr.x)) - 1ull) << sr.x;      // columns x0..x1 of one row
+  for (uint32_t sy = sr.y; sy <= sr.w; ++sy) m |= row << (sy * (uint32_t)super_x);
+  return m;
+}
 
 // Stable multi-split of the ranks into supertile lists, without materialising unsorted keys: block b owns the ranks
 // [b * MS_T, (b + 1) * MS_T).  Pass 1 (this kernel, fused with the gather of the splats into rank order) counts, per
@@ -60,10 +69,18 @@ __global__ void __launch_bounds__(MS_T) msplit_count_kernel(const uint32_t* __re
     dst[2] = src[2];
   }
   const uint4 sr = super_rect(rc, sshift);
-  for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {            // (sx, sy) walk the supertiles row-major: no division
-    const unsigned m = __ballot_sync(0xffffffffu, covers_super(sr, (uint32_t)sx, (uint32_t)sy));
-    if (lane == 0 && m) atomicAdd(&cnt[s], (uint32_t)__popc(m));
-    if (++sx == super_x) { sx = 0; ++sy; }
+  if (n_super <= 64) {
+    const unsigned long long cm = super_mask64(sr, super_x);
+    for (int s = 0; s < n_super; ++s) {
+      const unsigned m = __ballot_sync(0xffffffffu, (cm >> s) & 1ull);
+      if (lane == 0 && m) atomicAdd(&cnt[s], (uint32_t)__popc(m));
+    }
+  } else {
+    for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {          // (sx, sy) walk the supertiles row-major: no division
+      const unsigned m = __ballot_sync(0xffffffffu, covers_super(sr, (uint32_t)sx, (uint32_t)sy));
+      if (lane == 0 && m) atomicAdd(&cnt[s], (uint32_t)__popc(m));
+      if (++sx == super_x) { sx = 0; ++sy; }
+    }
   }
   __syncthreads();
   if ((int)threadIdx.x < n_super) counts[(size_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
@@ -79,10 +96,13 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const ushort4* __res
   const uint32_t lt = (1u << lane) - 1u;
   const ushort4 rc = r < N ? rect_sorted[r] : make_ushort4(0, 0, 0, 0);
   const uint4 sr = super_rect(rc, sshift);
+  const bool small = n_super <= 64;
+  const unsigned long long cm = small ? super_mask64(sr, super_x) : 0ull;
   for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {
-    const unsigned m = __ballot_sync(0xffffffffu, covers_super(sr, (uint32_t)sx, (uint32_t)sy));
+    const bool c = small ? ((cm >> s) & 1ull) != 0ull : covers_super(sr, (uint32_t)sx, (uint32_t)sy);
+    const unsigned m = __ballot_sync(0xffffffffu, c);
     if (lane == 0) wc[s][w] = (uint16_t)__popc(m);
-    if (++sx == super_x) { sx = 0; ++sy; }
+    if (!small && ++sx == super_x) { sx = 0; ++sy; }
   }
   __syncthreads();
   if ((int)threadIdx.x < n_super) {
@@ -100,9 +120,9 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const ushort4* __res
   }
   __syncthreads();
   for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {
-    const bool c = covers_super(sr, (uint32_t)sx, (uint32_t)sy);
+    const bool c = small ? ((cm >> s) & 1ull) != 0ull : covers_super(sr, (uint32_t)sx, (uint32_t)sy);
     const unsigned m = __ballot_sync(0xffffffffu, c);
-    if (++sx == super_x) { sx = 0; ++sy; }
+    if (!small && ++sx == super_x) { sx = 0; ++sy; }
     if (c) {
       const uint32_t pos = scanned[(size_t)s * nblk + blockIdx.x] + wc[s][w] + __popc(m & lt);
       if (pos < cap) {
