@@ -92,6 +92,8 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const ushort4* __res
                                                             uint32_t* __restrict__ keys, ushort4* __restrict__ crect,
                                                             uint2* __restrict__ ranges) {
   __shared__ uint16_t wc[256][MS_W];         // per supertile: ranks of warp w touching it, then the exclusive prefix over warps
+  __shared__ uint32_t seg[256];              // start of this block's segment in every supertile list (one global load each,
+                                             // up front: a load inside the write loop would stall every iteration on the L2)
   const int r = blockIdx.x * MS_T + threadIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const uint32_t lt = (1u << lane) - 1u;
   const ushort4 rc = r < N ? rect_sorted[r] : make_ushort4(0, 0, 0, 0);
@@ -106,6 +108,7 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const ushort4* __res
   }
   __syncthreads();
   if ((int)threadIdx.x < n_super) {
+    seg[threadIdx.x] = scanned[(size_t)threadIdx.x * nblk + blockIdx.x];
     uint32_t run = 0;
     for (int k = 0; k < MS_W; ++k) {
       const uint32_t c = wc[threadIdx.x][k];
@@ -124,7 +127,7 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const ushort4* __res
     const unsigned m = __ballot_sync(0xffffffffu, c);
     if (!small && ++sx == super_x) { sx = 0; ++sy; }
     if (c) {
-      const uint32_t pos = scanned[(size_t)s * nblk + blockIdx.x] + wc[s][w] + __popc(m & lt);
+      const uint32_t pos = seg[s] + wc[s][w] + __popc(m & lt);
       if (pos < cap) {
         keys[pos] = ((uint32_t)s << rank_bits) | (uint32_t)r;
         crect[pos] = rc;
