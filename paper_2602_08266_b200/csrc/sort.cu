@@ -88,22 +88,27 @@ __global__ void __launch_bounds__(SCAN_T) scan_downsweep_kernel(const uint32_t* 
 // Whole scan in ONE block (n up to a few tens of thousands: the digit histograms of the depth sort), so that a radix
 // pass is three dependent launches instead of five: the S1-S2 chain of a batch is latency bound.
 constexpr int SCAN1_T = 1024;
-constexpr uint32_t SCAN1_MAX = 32768;
+constexpr uint32_t SCAN1_MAX = 56 * 1024;   // 224 KB of shared memory
 
 __global__ void __launch_bounds__(SCAN1_T) scan_single_block_kernel(const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* __restrict__ total_out) {
+  extern __shared__ uint32_t sdata[];       // the whole input (coalesced in, coalesced out)
   __shared__ uint32_t sm[32];
-  // thread t owns the contiguous chunk [t c, (t + 1) c): one block-wide scan of the chunk sums instead of one per 4096 elements
-  const uint32_t c = (n + SCAN1_T - 1) / SCAN1_T;
-  const uint32_t i0 = threadIdx.x * c, i1 = min(i0 + c, n);
+  for (uint32_t i = threadIdx.x; i < n; i += SCAN1_T) sdata[i] = in[i];
+  __syncthreads();
+  // thread t owns the contiguous chunk [t c, (t + 1) c), c odd: the chunk walks of a warp fall into distinct banks
+  const uint32_t c = ((n + SCAN1_T - 1) / SCAN1_T) | 1u;
+  const uint32_t i0 = min(threadIdx.x * c, n), i1 = min(i0 + c, n);
   uint32_t s = 0;
-  for (uint32_t i = i0; i < i1; ++i) s += in[i];
+  for (uint32_t i = i0; i < i1; ++i) s += sdata[i];
   uint32_t total;
   uint32_t off = block_exclusive_scan(s, sm, total);
   for (uint32_t i = i0; i < i1; ++i) {
-    const uint32_t v = in[i];
-    out[i] = off;
+    const uint32_t v = sdata[i];
+    sdata[i] = off;
     off += v;
   }
+  __syncthreads();
+  for (uint32_t i = threadIdx.x; i < n; i += SCAN1_T) out[i] = sdata[i];
   if (total_out && threadIdx.x == 0) *total_out = total;
 }
 
@@ -124,7 +129,12 @@ void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* t
   const uint32_t nb = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
   if (nb > 1 && n <= SCAN1_MAX) {
     ++g_kernel_launches;
-    scan_single_block_kernel<<<1, SCAN1_T, 0, st>>>(in, out, (uint32_t)n, total_out);
+    static bool configured = false;
+    if (!configured) {
+      cudaFuncSetAttribute(scan_single_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SCAN1_MAX * 4));
+      configured = true;
+    }
+    scan_single_block_kernel<<<1, SCAN1_T, n * 4, st>>>(in, out, (uint32_t)n, total_out);
     return;
   }
   if (nb == 1) {
@@ -144,12 +154,18 @@ void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* t
 // one stable radix pass on `bits` (<= 8) bits at `shift`
 // ------------------------------------------------------------------------------------------------
 constexpr int RS_T = 256;
-constexpr int RS_I = 16;
-constexpr int RS_TILE = RS_T * RS_I;   // 4096 keys per block
+// keys per thread: 16 (4096 keys per block) for long inputs, 4 (1024 per block) for short ones -- a pass over 200,000
+// keys is one partial wave of blocks either way, so its time is one block's critical path: shorter blocks, shorter pass
+constexpr int RS_I_LONG = 16, RS_I_SHORT = 4;
+constexpr size_t RS_SHORT_MAX = 512 * 1024;
+__host__ __device__ constexpr int rs_tile(int rs_i) { return RS_T * rs_i; }
+static int rs_i_for(size_t n) { return n <= RS_SHORT_MAX ? RS_I_SHORT : RS_I_LONG; }
 constexpr int RS_W = RS_T / 32;        // 8 warps, 512 consecutive keys each
 
+template <int RS_I>
 __global__ void __launch_bounds__(RS_T) radix_hist_kernel(const uint32_t* __restrict__ keys, uint32_t n, const uint32_t* __restrict__ d_n,
                                                            int shift, uint32_t mask, uint32_t* __restrict__ hist, uint32_t nblocks) {
+  constexpr int RS_TILE = RS_T * RS_I;
   __shared__ uint32_t h[256];
   if (d_n) n = min(n, *d_n);             // device-side length (n is then the capacity the grid was sized for)
   h[threadIdx.x] = 0;
@@ -164,11 +180,12 @@ __global__ void __launch_bounds__(RS_T) radix_hist_kernel(const uint32_t* __rest
   if (threadIdx.x <= mask) hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
 
-template <bool HAS_VALS>
+template <bool HAS_VALS, int RS_I>
 __global__ void __launch_bounds__(RS_T) radix_scatter_kernel(const uint32_t* __restrict__ keys_in, uint32_t* __restrict__ keys_out,
                                                               const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ vals_out,
                                                               uint32_t n, const uint32_t* __restrict__ d_n, int shift, uint32_t mask,
                                                               const uint32_t* __restrict__ hist_scanned, uint32_t nblocks) {
+  constexpr int RS_TILE = RS_T * RS_I;
   if (d_n) n = min(n, *d_n);
   if (blockIdx.x * RS_TILE >= n) return;
   __shared__ uint32_t wh[RS_W][256];     // per-warp digit counts, then per-warp digit bases
@@ -239,10 +256,10 @@ __global__ void __launch_bounds__(RS_T) radix_scatter_kernel(const uint32_t* __r
   }
 }
 
-uint32_t radix_blocks(size_t n) { return (uint32_t)((n + RS_TILE - 1) / RS_TILE); }
+uint32_t radix_blocks(size_t n) { const size_t t = (size_t)rs_tile(rs_i_for(n)); return (uint32_t)((n + t - 1) / t); }
 
 size_t radix_temp_words(size_t n) {
-  size_t nb = (n + RS_TILE - 1) / RS_TILE;
+  size_t nb = radix_blocks(n);
   size_t hist = 256 * nb;
   return hist + scan_temp_words(hist);
 }
@@ -250,20 +267,24 @@ size_t radix_temp_words(size_t n) {
 void radix_pass(const uint32_t* keys_in, uint32_t* keys_out, const uint32_t* vals_in, uint32_t* vals_out, size_t n,
                 const uint32_t* d_n, int shift, int bits, uint32_t* tmp, cudaStream_t st) {
   if (n == 0) return;
-  const uint32_t nb = (uint32_t)((n + RS_TILE - 1) / RS_TILE);
+  const uint32_t nb = radix_blocks(n);
+  const bool shrt = rs_i_for(n) == RS_I_SHORT;
   const uint32_t mask = (1u << bits) - 1u;
   const size_t hist_n = (size_t)(mask + 1) * nb;
   uint32_t* hist = tmp;
   ++g_kernel_launches;
-  radix_hist_kernel<<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, d_n, shift, mask, hist, nb);
+  if (shrt) radix_hist_kernel<RS_I_SHORT><<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, d_n, shift, mask, hist, nb);
+  else radix_hist_kernel<RS_I_LONG><<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, d_n, shift, mask, hist, nb);
   exclusive_scan_u32(hist, hist, hist_n, tmp + 256 * (size_t)nb, nullptr, st);
   if (vals_in) {
     ++g_kernel_launches;
-    radix_scatter_kernel<true><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, d_n, shift, mask, hist, nb);
+    if (shrt) radix_scatter_kernel<true, RS_I_SHORT><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, d_n, shift, mask, hist, nb);
+    else radix_scatter_kernel<true, RS_I_LONG><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, d_n, shift, mask, hist, nb);
   }
   else {
     ++g_kernel_launches;
-    radix_scatter_kernel<false><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, d_n, shift, mask, hist, nb);
+    if (shrt) radix_scatter_kernel<false, RS_I_SHORT><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, d_n, shift, mask, hist, nb);
+    else radix_scatter_kernel<false, RS_I_LONG><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, d_n, shift, mask, hist, nb);
   }
 }
 
