@@ -5,6 +5,8 @@
 // Gaussian index (4 passes of 8 bits), then keys (tile << rank_bits | depth_rank) are emitted in depth-rank
 // order and only the tile digit is sorted, by stable passes.  Stability makes the result identical to a full
 // sort on (tile, z bits, index) -- the definition of the tile lists (R-5, R-7).
+#include <cooperative_groups.h>
+
 #include "kernels.h"
 
 namespace nbv {
@@ -85,19 +87,31 @@ __global__ void __launch_bounds__(SCAN_T) scan_downsweep_kernel(const uint32_t* 
   if (total_out && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *total_out = (offsets ? offsets[blockIdx.x] : 0u) + total;
 }
 
-// Whole scan in ONE block (n up to a few tens of thousands: the digit histograms of the depth sort), so that a radix
-// pass is three dependent launches instead of five: the S1-S2 chain of a batch is latency bound.
+// Whole scan in ONE launch of ONE thread-block cluster (n up to 56k: the digit histograms of the depth sort and the
+// multi-split count table), so that a radix pass is three dependent launches instead of five: the S1-S2 chain of a batch is
+// latency bound.  Eight CTAs on eight SMs each stage an eighth of the input in shared memory
+// (coalesced in, coalesced out), scan it, publish their total, and read the totals of the lower-ranked CTAs through
+// distributed shared memory after one cluster barrier.
 constexpr int SCAN1_T = 1024;
-constexpr uint32_t SCAN1_MAX = 56 * 1024;   // 224 KB of shared memory
+constexpr int SCAN1_CTAS = 8;
+constexpr uint32_t SCAN1_PER_CTA = 7168;
+constexpr uint32_t SCAN1_MAX = SCAN1_CTAS * SCAN1_PER_CTA;
 
-__global__ void __launch_bounds__(SCAN1_T) scan_single_block_kernel(const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* __restrict__ total_out) {
-  extern __shared__ uint32_t sdata[];       // the whole input (coalesced in, coalesced out)
+__global__ void __cluster_dims__(SCAN1_CTAS, 1, 1) __launch_bounds__(SCAN1_T)
+scan_cluster_kernel(const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* __restrict__ total_out) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  __shared__ uint32_t sdata[SCAN1_PER_CTA];
   __shared__ uint32_t sm[32];
-  for (uint32_t i = threadIdx.x; i < n; i += SCAN1_T) sdata[i] = in[i];
+  __shared__ uint32_t cta_total;
+  const uint32_t rank = cluster.block_rank();
+  const uint32_t per = (n + SCAN1_CTAS - 1) / SCAN1_CTAS;
+  const uint32_t g0 = min(rank * per, n), g1 = min(g0 + per, n), m = g1 - g0;
+  for (uint32_t i = threadIdx.x; i < m; i += SCAN1_T) sdata[i] = in[g0 + i];
   __syncthreads();
   // thread t owns the contiguous chunk [t c, (t + 1) c), c odd: the chunk walks of a warp fall into distinct banks
-  const uint32_t c = ((n + SCAN1_T - 1) / SCAN1_T) | 1u;
-  const uint32_t i0 = min(threadIdx.x * c, n), i1 = min(i0 + c, n);
+  const uint32_t c = ((m + SCAN1_T - 1) / SCAN1_T) | 1u;
+  const uint32_t i0 = min(threadIdx.x * c, m), i1 = min(i0 + c, m);
   uint32_t s = 0;
   for (uint32_t i = i0; i < i1; ++i) s += sdata[i];
   uint32_t total;
@@ -107,9 +121,13 @@ __global__ void __launch_bounds__(SCAN1_T) scan_single_block_kernel(const uint32
     sdata[i] = off;
     off += v;
   }
-  __syncthreads();
-  for (uint32_t i = threadIdx.x; i < n; i += SCAN1_T) out[i] = sdata[i];
-  if (total_out && threadIdx.x == 0) *total_out = total;
+  if (threadIdx.x == 0) cta_total = total;
+  cluster.sync();
+  uint32_t base = 0;
+  for (uint32_t r = 0; r < rank; ++r) base += *cluster.map_shared_rank(&cta_total, r);
+  for (uint32_t i = threadIdx.x; i < m; i += SCAN1_T) out[g0 + i] = base + sdata[i];
+  if (total_out && rank == SCAN1_CTAS - 1 && threadIdx.x == 0) *total_out = base + total;
+  cluster.sync();                            // no CTA may exit while its shared memory can still be read
 }
 
 size_t scan_temp_words(size_t n) {
@@ -129,12 +147,7 @@ void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* t
   const uint32_t nb = (uint32_t)((n + SCAN_TILE - 1) / SCAN_TILE);
   if (nb > 1 && n <= SCAN1_MAX) {
     ++g_kernel_launches;
-    static bool configured = false;
-    if (!configured) {
-      cudaFuncSetAttribute(scan_single_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SCAN1_MAX * 4));
-      configured = true;
-    }
-    scan_single_block_kernel<<<1, SCAN1_T, n * 4, st>>>(in, out, (uint32_t)n, total_out);
+    scan_cluster_kernel<<<SCAN1_CTAS, SCAN1_T, 0, st>>>(in, out, (uint32_t)n, total_out);
     return;
   }
   if (nb == 1) {
