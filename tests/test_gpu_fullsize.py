@@ -198,3 +198,26 @@ def test_cfg4_sampled_pixels_and_block_properties():
     # ~2e-4 relative from run to run; the bar is the gain tolerance of B: north_star
     np.testing.assert_allclose(s4.cpu().numpy(), s1.cpu().numpy(), rtol=1e-3)
     assert int(b4.item()) == int(b1.item())
+
+
+@pytest.mark.parametrize("W,H,f", [(1296, 1104, 1100.0), (2576, 1680, 2200.0)])
+def test_large_supertile_grids(W, H, f):
+    """Grids of more than 64 supertiles (1296 x 1104: 11 x 9 = 99 of 8 x 8 tiles -- the comparison path of the multi-split)
+    and of more than 256 at 8 x 8 (2576 x 1680: 161 x 105 tiles -> supertiles of 16 x 16 tiles, 11 x 7): tile lists
+    bit-exact, blocks and gains against the oracle."""
+    wl = synth.make_workload(0)
+    cam = synth.hemisphere_cameras(1, (0.6, 0.6), W, H, f, f, np.random.default_rng(13))[0]
+    scn = make_oracle_scene(wl.scene)
+    nbv = _nbv(wl.scene)
+    off_o, ids_o = scn.tile_lists(cam)
+    off_g, ids_g = [t.cpu().numpy() for t in nbv.tile_lists(cam)]
+    np.testing.assert_array_equal(off_g, off_o)
+    np.testing.assert_array_equal(ids_g, ids_o)
+    Ho = scn.view_hessian(cam)
+    Hg = nbv.view_hessian(cam).cpu().numpy().astype(np.float64)
+    np.testing.assert_array_equal(np.abs(Hg).sum(axis=1) > 0, np.abs(Ho).sum(axis=1) > 0)
+    assert block_rel_err(Hg, Ho).max() < 1e-3
+    nbv.accumulate_training(wl.train_cams)
+    ref = orc.score_candidates(scn, wl.train_cams, np.array([cam]))
+    s, _ = nbv.score_candidates(np.array([cam]))
+    np.testing.assert_allclose(s.cpu().numpy(), ref["scores"], rtol=1e-3)
