@@ -87,14 +87,14 @@ __global__ void __launch_bounds__(SCAN_T) scan_downsweep_kernel(const uint32_t* 
   if (total_out && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) *total_out = (offsets ? offsets[blockIdx.x] : 0u) + total;
 }
 
-// Whole scan in ONE launch of ONE thread-block cluster (n up to 56k: the digit histograms of the depth sort and the
+// Whole scan in ONE launch of ONE thread-block cluster (n up to 64k: the digit histograms of the depth sort and the
 // multi-split count table), so that a radix pass is three dependent launches instead of five: the S1-S2 chain of a batch is
 // latency bound.  Eight CTAs on eight SMs each stage an eighth of the input in shared memory
 // (coalesced in, coalesced out), scan it, publish their total, and read the totals of the lower-ranked CTAs through
 // distributed shared memory after one cluster barrier.
 constexpr int SCAN1_T = 1024;
 constexpr int SCAN1_CTAS = 8;
-constexpr uint32_t SCAN1_PER_CTA = 7168;
+constexpr uint32_t SCAN1_PER_CTA = 8192;
 constexpr uint32_t SCAN1_MAX = SCAN1_CTAS * SCAN1_PER_CTA;
 
 __global__ void __cluster_dims__(SCAN1_CTAS, 1, 1) __launch_bounds__(SCAN1_T)
