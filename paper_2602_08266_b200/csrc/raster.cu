@@ -315,6 +315,7 @@ template <int NCH>
 __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
   __shared__ float4 sm[32 * 3];
   __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
+  __shared__ float sm_l2s[32];           // per staged entry: log2(sigma), folded into the exponent of the fast exp
   __shared__ __align__(16) float red[32 * RED_STRIDE];
   __shared__ uint32_t q_rank[64];
   const int lane = threadIdx.x;
@@ -402,6 +403,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       const float cA = -2.0f * q0.z, cB = -q0.w, cC = -2.0f * q1.x;
       const float icC = 1.0f / cC;
       sm_wh[lane] = make_float4(sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), -cB * icC, sqrtf(cC), __logf(prm.alpha_min / q1.y));
+      sm_l2s[lane] = log2f(q1.y);
     }
     __syncwarp();
     for (int j = 0; j < cnt; ++j) {
@@ -415,6 +417,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       // of either, the whole entry is evaluated with exp_spec instead, so every decision is the one S3 took.  The test
       // reads only `power`: the MUFU results are first needed in pass 2, where 8 independent chains hide their latency.
       const float4 wh = sm_wh[j];
+      const float l2s = sm_l2s[j];
       // |power - P_min| <= 2e-5 or |power - P_max| <= 2e-5   <=>   | |power - P_mid| - P_half | <= 2e-5 (up to a rounding
       // of ~5e-7, far inside the 2e-5 guard band)
       const float Phalf = 0.5f * prm.ln_amax_over_amin, Pmid = wh.w + Phalf;
@@ -435,7 +438,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
         for (int k = 0; k < PPL; ++k) av[k] = mul_rn(s1.y, exp_spec(pw[k]));
       } else {
 #pragma unroll
-        for (int k = 0; k < PPL; ++k) av[k] = s1.y * ex2_approx(pw[k] * 0x1.715476p+0f);
+        for (int k = 0; k < PPL; ++k) av[k] = ex2_approx(fmaf(pw[k], 0x1.715476p+0f, l2s));      // sigma exp(power) in one FMA + MUFU
       }
       // pass 2 (value path): beta, suffix sums, and the sums  F_p = sum_k f_k t_k^p,  G_c,p = sum_k g_c,k t_k^p  over
       // the lane's 8 pixels with t_k = k - 3.5 a compile-time constant (dy_k = dyc + t_k).
