@@ -204,8 +204,9 @@ int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream);
 
 /* ---- measurement ------------------------------------------------------------------------------------ */
 
-/* Stages of one view, in stream order: S1 | depth radix sort | gather + scan + coarse key
- * emission | supertile-digit radix pass + ranges + rect gather | S3 (with the lazy tile-list filter) | S4 | S5 + S6. */
+/* Stages of one view, in stream order: S1 | depth radix sort | multi-split pass 1 (gather of the
+ * splats into depth order + per-supertile counts) | count-table scan + multi-split pass 2 (keys, rects, supertile
+ * ranges) | S3 (with the lazy tile-list filter) | S4 | S5 + S6. */
 #define NBV_STAGE_PROJECT 0
 #define NBV_STAGE_DEPTH_SORT 1
 #define NBV_STAGE_BIN 2
