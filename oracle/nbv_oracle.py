@@ -21,6 +21,7 @@ import numpy as np
 
 _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "nbv_oracle.cpp"
+_EXT = _HERE / "nbv_oracle_ext.inc"
 _LIB = _HERE / "libnbv_oracle.so"
 
 P = 14
@@ -56,7 +57,7 @@ def default_config(channel_mask: int = 7, bg=(0.0, 0.0, 0.0), opacity_coord: int
 
 def build(force: bool = False) -> Path:
     """Compile the oracle shared library (g++, OpenMP, no FP contraction)."""
-    if _LIB.exists() and not force and _LIB.stat().st_mtime >= _SRC.stat().st_mtime:
+    if _LIB.exists() and not force and _LIB.stat().st_mtime >= max(_SRC.stat().st_mtime, _EXT.stat().st_mtime):
         return _LIB
     flags = ["-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"]
     try:

@@ -95,6 +95,7 @@ def test_greedy_tie_takes_the_lowest_index():
     scn = make_oracle_scene(wl.scene, 7)
     g = orc.select_greedy(scn, wl.train_cams, wl.cand_cams[[0, 0]], rounds=2)      # the same camera twice
     row = g["scores"][0]
-    assert row[0] == pytest.approx(row[1], rel=1e-12)          # equal up to the order of the OpenMP partial sums
-    assert g["order"][0] == orc.argmax_lowest(row) and sorted(g["order"].tolist()) == [0, 1]
+    # the oracle sums a view's pixels band by band in a fixed order: the same camera gives the same bits, run to run
+    assert row[0] == row[1]
+    assert g["order"].tolist() == [0, 1]
     assert orc.argmax_lowest(np.array([1.0, 3.0, 3.0, 2.0])) == 1                  # the rule itself (R-15)
