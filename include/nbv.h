@@ -48,7 +48,7 @@ extern "C" {
 
 typedef enum nbv_status {
   NBV_OK = 0,
-  NBV_ERR_INVALID_ARG = -1,      /* null pointer, non-positive size, bad camera (R not orthonormal within 1e-4, fx<=0 ...) */
+  NBV_ERR_INVALID_ARG = -1,      /* null pointer, non-positive size, bad camera (R not orthonormal within 1e-6, fx<=0 ...) */
   NBV_ERR_BAD_DATA = -2,         /* zero / non-finite quaternion, opacity outside (0,1), non-finite parameter */
   NBV_ERR_NOT_LOADED = -3,       /* a call that needs Gaussians before nbv_load_gaussians */
   NBV_ERR_EMPTY_CANDIDATES = -4, /* nbv_score_candidates with n == 0 */
@@ -117,7 +117,8 @@ const char* nbv_last_error(const nbv_ctx* ctx);
  * S1-S2 of the views of a batch run concurrently on internal streams (forked from and joined back into the caller's
  * stream with events); S3, S4 and S5+S6 are ONE kernel launch each per batch (S3 and S4: persistent warps pulling
  * (view, tile) positions).  Two sets of work buffers and two internal raster streams alternate between batches.  Views are independent
- * (the arg max is over per-view gains), so this changes no result beyond the order of floating-point atomics.
+ * (the arg max is over per-view gains), so this changes no result beyond the order of the binary32 reductions of S4
+ * (H_T is accumulated view by view in call order, and a candidate's score is summed in a fixed order).
  * Errors: INVALID_ARG outside [1, 16]. */
 int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight);
 
@@ -179,8 +180,8 @@ int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, nbv_ctx* ct
  * (lowest index on ties) becomes h_order[r], and that view's blocks are added to H_T (Eq. 6).  On return H_T
  * contains the selected views (|T| grows by `rounds`).
  * A view's blocks do not depend on H_T, so every candidate is rasterised once (S1-S5) into a sparse pool of
- * (Gaussian, 14x14 block) entries; each round then runs only S0' (new factors of H_T), S6 over the pool, the masked
- * arg-max and the addition of the selected view's blocks, all on the device.  The pool is limited to 4 GiB (override:
+ * (Gaussian, 14x14 binary64 block) entries; each round then runs only S0', S6 over the pool against the current H_T, the
+ * masked arg-max and the addition of the selected view's blocks, all on the device.  The pool is limited to 4 GiB (override:
  * environment variable NBV_GREEDY_CACHE_MB at nbv_create); if the candidates' blocks do not fit, the call falls back to
  * re-rasterising the remaining candidates every round (same results, one host synchronisation per round).
  * HOST output h_order: rounds int32.  DEVICE output d_scores (may be NULL): rounds x n floats, row r = the scores of
@@ -264,6 +265,12 @@ int nbv_view_hessian(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_blocks, voi
 
 /* Copy of the accumulated training Hessian H_T (N x 105). */
 int nbv_training_hessian(nbv_ctx* ctx, float* d_blocks, void* stream);
+
+/* Chain rule of S5 for one camera, per Gaussian (visible or not): d_chain N x 53 floats = the 5 x 10 matrix
+ * d(mx, my, a, b, c) / d(mu(3), logscale(3), quat(4)) row-major (the quaternion columns THROUGH q/|q|, R-10), then dz/dmu (3).
+ * The kernel computes it in binary64 from the factor U of Sigma2D = U U^T + blur I (csrc/block_math.cuh); the export
+ * exists so that a test can pin it against finite differences of nbv_projected, the library's own forward projection. */
+int nbv_chain(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_chain, void* stream);
 
 /* S0' output: confidence c_g (N floats) for the given mode (Eq. 7 or Eq. 12). */
 int nbv_confidence(nbv_ctx* ctx, int32_t target_obj, float* d_conf, void* stream);

@@ -36,6 +36,7 @@ EXPORTS = [
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
     "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
     "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy", "nbv_block_size", "nbv_render_mask", "nbv_measure_ffma_peak",
+    "nbv_chain",
 ]
 
 STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
@@ -313,6 +314,14 @@ class NBV:
         blocks = torch.empty((self.N, self.block_size()), dtype=torch.float32, device=self.device)
         self._check(self.lib.nbv_training_hessian(self._h, _ptr(blocks), _stream()))
         return blocks
+
+    def chain(self, cam):
+        """nbv_chain: (N, 53) = d(mx,my,a,b,c)/d(mu,logscale,quat) (5 x 10, row-major) then dz/dmu (3), per Gaussian"""
+        torch = self._torch
+        cam = _cams(cam)
+        out = torch.empty((self.N, 53), dtype=torch.float32, device=self.device)
+        self._check(self.lib.nbv_chain(self._h, C.c_void_p(cam.ctypes.data), _ptr(out), _stream()))
+        return out
 
     def confidence(self, target_obj: int = -1):
         torch = self._torch

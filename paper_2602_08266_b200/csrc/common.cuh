@@ -75,6 +75,63 @@ __device__ __forceinline__ float splat_power(float qa, float qb, float qc, float
   return __fmaf_rn(dx, __fmaf_rn(qa, dx, __fmul_rn(qb, dy)), __fmul_rn(__fmul_rn(qc, dy), dy));
 }
 
+// ---------------------------------------------------------------------------------------------
+// Packed binary32 pairs (sm_100: FFMA2 / FMUL2 / FADD2 issue two operations per lane in one slot).
+// Each half is rounded exactly like the scalar .rn instruction, so the decision path may use them; ptxas does
+// contract a mul.rn.f32x2 feeding an add.rn.f32x2 into one FFMA2 (seen in the SASS), so the decision path never
+// writes that pattern: its products feed fused multiply-adds or other products only, as the specification has it.
+// ---------------------------------------------------------------------------------------------
+typedef float2 f2;
+__device__ __forceinline__ f2 bc2(float s) { return make_float2(s, s); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) {
+  f2 d;
+  asm("{.reg .b64 ra, rb, rc, rd; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mov.b64 rc, {%6,%7}; fma.rn.f32x2 rd, ra, rb, rc; mov.b64 {%0,%1}, rd;}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+  return d;
+}
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) {
+  f2 d;
+  asm("{.reg .b64 ra, rb, rd; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mul.rn.f32x2 rd, ra, rb; mov.b64 {%0,%1}, rd;}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return d;
+}
+__device__ __forceinline__ f2 add2(f2 a, f2 b) {
+  f2 d;
+  asm("{.reg .b64 ra, rb, rd; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; add.rn.f32x2 rd, ra, rb; mov.b64 {%0,%1}, rd;}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return d;
+}
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) {
+  f2 d;
+  asm("{.reg .b64 ra, rb, rd; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; sub.rn.f32x2 rd, ra, rb; mov.b64 {%0,%1}, rd;}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return d;
+}
+
+// power of the Gaussian exponent for a pair of pixels of one column: the operations of splat_power, pair-wise
+__device__ __forceinline__ f2 splat_power2(float qa, float qb, float qc, float dx, f2 dy) {
+  const f2 inner = fma2(bc2(qa), bc2(dx), mul2(bc2(qb), dy));
+  return fma2(bc2(dx), inner, mul2(mul2(bc2(qc), dy), dy));
+}
+
+// exp_spec on a pair: the same operations in the same order, each half individually rounded
+__device__ __forceinline__ f2 exp_spec2(f2 x) {
+  const float MAGIC = 12582912.0f;
+  const f2 t = fma2(x, bc2(0x1.715476p+0f), bc2(MAGIC));
+  const f2 kf = sub2(t, bc2(MAGIC));
+  f2 r = fma2(kf, bc2(-0x1.62e4p-1f), x);
+  r = fma2(kf, bc2(-0x1.7f7d1cp-20f), r);
+  f2 p = bc2(0x1.6c16c2p-10f);
+  p = fma2(p, r, bc2(0x1.111112p-7f));
+  p = fma2(p, r, bc2(0x1.555556p-5f));
+  p = fma2(p, r, bc2(0x1.555556p-3f));
+  p = fma2(p, r, bc2(0.5f));
+  p = fma2(p, r, bc2(1.0f));
+  p = fma2(p, r, bc2(1.0f));
+  const int kx = __float_as_int(t.x) - __float_as_int(MAGIC), ky = __float_as_int(t.y) - __float_as_int(MAGIC);
+  return make_float2(__int_as_float(__float_as_int(p.x) + (kx << 23)), __int_as_float(__float_as_int(p.y) + (ky << 23)));
+}
+
 // packed upper-triangle index, r <= c
 __host__ __device__ __forceinline__ constexpr int tri(int r, int c) { return r * P - r * (r - 1) / 2 + (c - r); }
 

@@ -5,6 +5,7 @@
 namespace nbv {
 
 extern unsigned long long g_kernel_launches;   // host-side count of kernel launches (nbv_kernel_launches)
+int sm_count();                                // multiprocessors of the current device (queried once per device)
 
 // ---- sort.cu
 size_t scan_temp_words(size_t n);
@@ -56,7 +57,7 @@ struct PixelBuf {            // per-pixel outputs of the forward pass (H x W eac
   float* depth;
   float* T;
   int32_t* ncontrib;
-  int32_t* last;             // list position (relative to the tile's range) after the last composited entry
+  int32_t* last;             // number of leading entries of the tile's list that can contribute to the pixel (every composited one does)
 };
 // One launch of S3 / S4 / S5+S6 serves a BATCH of views (S3, S4: launch positions interleave the views; S5+S6: grid.y = view): per-view device pointers travel as a
 // __grid_constant__ kernel parameter.  All views of a batch share the image size.
@@ -67,11 +68,13 @@ struct RasterView {
   const ushort4* crect;
   const uint2* cranges;
   PixelBuf pix;
-  uint32_t* tile_cend;       // per tile: coarse position + 1 of the last composited entry
+  uint32_t* tile_cend;       // per tile: coarse position + 1 of the last entry some pixel of the tile passed
+  uint32_t* tile_elast;      // per tile: position + 1 of that entry in the tile's list (0: nothing composited)
   uint32_t* tile_walk;       // per tile: list entries S3 consumed
   float* moments;            // rank r at moments + r * mom_stride (NMOM floats), zero on entry to S4 for every Gaussian
   int mom_stride;            // NMOM, or groups * NMOM in a mask context (one group of 4 object channels per S4 launch)
-  uint32_t* touched;         // ranks with a non-zero block (counters->n_touched of them, in no particular order)
+  uint32_t* touched;         // ranks with a non-zero block (counters->n_touched of them, in increasing rank order)
+  uint32_t* touched_cnt;     // scratch of the ordered compaction: touched ranks per block of 256 ranks
   ViewCounters* counters;
 };
 struct RasterBatch {
@@ -85,13 +88,15 @@ struct RasterBatch {
 };
 void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg, bool full_pix,
                     cudaStream_t st);
-// S4, then the touched lists (ranks with sum w^2 != 0) of every view of the batch
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
-                     cudaStream_t st, bool build_touched = true);
+                     cudaStream_t st);
 
-// ---- hessian.cu
+// ---- hessian.cu (colour / depth contexts: everything after the binary32 moments is binary64)
+// the touched lists (ranks with sum w^2 != 0, in rank order) of every view of the batch
+void launch_touched(const RasterBatch& batch, int N, cudaStream_t st);
+uint32_t touched_blocks(int N);
 enum ExpandMode { EXPAND_TRAIN = 0, EXPAND_VIEW = 1, EXPAND_GAIN = 2, EXPAND_CACHE = 3 };
-// EXPAND_TRAIN: H_T[id] += H ; EXPAND_VIEW: out_blocks[id] = H ; EXPAND_GAIN: gain vs H_T, sum into *score (and gains[id] if not null)
+// EXPAND_TRAIN: H_T[id] += H ; EXPAND_VIEW: out_blocks[id] = H ; EXPAND_GAIN: gain vs H_T, summed into *score (and gains[id] if not null)
 // Consumes the touched list of every view of the batch: reads the moments of every touched rank and writes zeros back
 // (the moment buffers are all-zero again afterwards).
 struct ExpandView {
@@ -101,8 +106,9 @@ struct ExpandView {
   const uint32_t* touched;
   float* moments;
   float* out_blocks;         // EXPAND_VIEW
-  float* score;              // EXPAND_GAIN
+  float* score;              // EXPAND_GAIN: written (not accumulated) by the last block of the view
   float* gains;              // EXPAND_GAIN, may be null
+  double* partials;          // EXPAND_GAIN: per-block partial scores (expand_partials() doubles)
   ViewCounters* counters;
   // EXPAND_CACHE: the view's touched Gaussians and their unweighted blocks go to pool entries
   // [cache_span[0], cache_span[0] + cache_span[1]) (reserved by cache_reserve_kernel; span[1] = 0 on overflow)
@@ -112,12 +118,13 @@ struct ExpandBatch {
   int n;
   ExpandView v[MAX_BATCH];
 };
-void launch_expand(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, float* H_T, const float* conf,
-                   const float* cholT, cudaStream_t st);
-// Sparse per-candidate block cache of greedy selection (nbv_select_greedy): pool of (Gaussian id, 105-float block) entries.
+int expand_partials();       // doubles a slot's `partials` buffer must hold
+void launch_expand(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, double* H_T, const float* conf,
+                   cudaStream_t st);
+// Sparse per-candidate block cache of greedy selection (nbv_select_greedy): pool of (Gaussian id, 105-double block) entries.
 struct BlockCache {
   uint32_t* ids;             // capacity entries
-  float* blocks;             // capacity x 105
+  double* blocks;            // capacity x 105
   uint32_t* spans;           // per candidate: (first entry, number of entries)
   uint32_t* cursor;          // [0] entries reserved so far, [1] overflow flag
   uint32_t capacity;
@@ -125,16 +132,19 @@ struct BlockCache {
 // reserve pool space for the views of a batch (after their touched lists are known); spans_of_view[i] = spans + 2 * candidate
 void launch_cache_reserve(const ExpandBatch& batch, const BlockCache& cache, int first_candidate, cudaStream_t st);
 void launch_expand_cache(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, const BlockCache& cache, cudaStream_t st);
-// scores[c] += sum over the cached entries of candidate c of the gain against cholT (skipped when taken[c] != 0)
-void launch_cached_gain(const BlockCache& cache, int n_cand, const int32_t* taken, const float* conf, const float* cholT, float* scores,
-                        int weight_mode, cudaStream_t st);
+// scores[c] = sum over the cached entries of candidate c of the gain against H_T (0 when taken[c] != 0); scratch:
+// cached_gain_scratch_bytes(n_cand) bytes, zero on first use
+size_t cached_gain_scratch_bytes(int n_cand);
+void launch_cached_gain(const BlockCache& cache, const nbv_config& cfg, int n_cand, const int32_t* taken, const float* conf,
+                        const double* H_T, float* scores, void* scratch, cudaStream_t st);
 // H_T[g] += block for the cached entries of candidate *pick
-void launch_cache_accumulate(const BlockCache& cache, const int32_t* pick, float* H_T, cudaStream_t st);
+void launch_cache_accumulate(const BlockCache& cache, const int32_t* pick, double* H_T, cudaStream_t st);
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);
-void launch_prepare(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
+void launch_export_blocks(const double* src, float* dst, size_t n, cudaStream_t st);
+void launch_export_chain(const SceneDev& sc, const nbv_camera& cam, float* out, cudaStream_t st);
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);
 
-// ---- hessian.cu, object-mask output (NEXT-2): groups of four object channels, blocks of L = 11 + K parameters
+// ---- mask.cu, object-mask output (NEXT-2): groups of four object channels, blocks of L = 11 + K parameters, binary32
 void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uint32_t* ids_sorted, int group, int bgch, Splat* out,
                         cudaStream_t st);
 void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, float* H_T,

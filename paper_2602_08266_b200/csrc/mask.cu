@@ -1,0 +1,354 @@
+// mask.cu -- the object-mask output (NEXT-2): S5' / S6 on blocks of L = 11 + K parameters, binary32, one warp per Gaussian.
+#include <algorithm>
+#include <cstdlib>
+
+#include "block_math.cuh"
+#include "kernels.h"
+
+namespace nbv {
+
+// =====================================================================================================================
+// Object-mask output (Eq. 1-2 "masks use the object vector").
+//   O = sum_i softmax(o_i) alpha_i T_i + e_bg T_end : compositing of the K "colours" p_i = softmax(o_i) over the
+//   background colour e_bg.  Block of a Gaussian: L = 11 + K parameters [mu, logscale, quat, opacity | logits].
+//   Row of channel k at a pixel:  J_k = beta_k alpha A m6  (+)  w dp_k/do,   dp_k/do_j = p_k (delta_kj - p_j).
+// S3 is shared with the other outputs; S4 is the SAME kernel, run once per group of four object channels on a copy of
+// the rank-ordered splats whose (r, g, b | z) fields hold (p_t0, p_t1, p_t2 | p_t3); group 0 starts with the background
+// channel (the only one with a background term, which the kernel has on its three colour slots).  Every group leaves
+// 40 moments per rank: the 15 monomial sums add up over the groups (sum_k beta_k^2), the 6 cross moments x_k per
+// channel stay apart.  Then, per touched Gaussian (S5'):
+//   geo-geo   (11 x 11)  A Q A^T
+//   geo-logit (11 x K)   sum_k (A x_k) dp_k/do_j = p_j (A x_j - sum_k p_k A x_k)
+//   logit-logit (K x K)  W2 sum_k dp_k/do_j dp_k/do_l = W2 (delta_jl p_j^2 - p_j p_l (p_j + p_l) + p_j p_l sum_k p_k^2)
+// and S6 is the same solve-form log-det gain on L x L blocks.
+// =====================================================================================================================
+__host__ __device__ __forceinline__ int mask_channel_of_slot(int t, int bgch) { return t == 0 ? bgch : (t <= bgch ? t - 1 : t); }
+__host__ __device__ __forceinline__ int mask_slot_of_channel(int c, int bgch) { return c == bgch ? 0 : (c < bgch ? c + 1 : c); }
+__device__ __forceinline__ int triL(int r, int c, int L) { return r * L - r * (r - 1) / 2 + (c - r); }
+
+__global__ void __launch_bounds__(256) mask_splat_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ ids_sorted,
+                                                         const float* __restrict__ logits, const float* __restrict__ lse, int N, int K,
+                                                         int group, int bgch, Splat* __restrict__ out) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= N) return;
+  Splat s = splat_sorted[r];
+  const uint32_t g = ids_sorted[r];
+  float p[4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int t = 4 * group + j;
+    p[j] = (g < (uint32_t)N && t < K) ? expf(logits[(size_t)g * K + mask_channel_of_slot(t, bgch)] - lse[g]) : 0.f;
+  }
+  s.r = p[0]; s.g = p[1]; s.b = p[2]; s.z = p[3];
+  out[r] = s;
+}
+
+void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uint32_t* ids_sorted, int group, int bgch, Splat* out,
+                        cudaStream_t st) {
+  ++g_kernel_launches;
+  mask_splat_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(splat_sorted, ids_sorted, sc.logits, sc.lse, sc.N, sc.K, group, bgch, out);
+}
+
+// upper Cholesky factor of a packed SPD L x L, in place (as cholesky_packed)
+__device__ void cholesky_L(float* Mx, int L) {
+  for (int j = 0; j < L; ++j) {
+    float d = Mx[triL(j, j, L)];
+    for (int k = 0; k < j; ++k) d -= Mx[triL(k, j, L)] * Mx[triL(k, j, L)];
+    d = fmaxf(d, 1e-30f);
+    const float inv = rsqrtf(d);
+    Mx[triL(j, j, L)] = d * inv;
+    for (int i = j + 1; i < L; ++i) {
+      float v = Mx[triL(j, i, L)];
+      for (int k = 0; k < j; ++k) v -= Mx[triL(k, j, L)] * Mx[triL(k, i, L)];
+      Mx[triL(j, i, L)] = v * inv;
+    }
+  }
+}
+
+// ---- S5' + S6 of a mask context, warp-cooperative: ONE WARP PER TOUCHED GAUSSIAN, the L x L block and the factor in shared
+// memory.  Lane l owns the columns (or rows) l, l + 32 of the matrices, so the triangular solves and the elimination run
+// on up to 63 columns at once (a first version ran one thread per Gaussian over 2 x 2016 floats of local memory).
+//   W = U^-T (c H) U^-1 : (a) every lane solves U^T x = h_j for its columns j, in place; (b) every lane solves
+//   U^T y = (row i of the result)^T for its rows i, in place.   log det(I + W): right-looking Cholesky on the excess
+//   (pivot 1 + e_j enters as log1p(e_j), as in gain_solve), one column per step, the trailing rows updated in parallel.
+struct MaskWarpLayout {
+  int LS;          // row stride of H and U (odd: conflict-free column and row walks)
+  int per_warp;    // floats per warp
+  int oH, oU, oA, oAQ, oMom, oX, oP, oMono;
+};
+__host__ __device__ inline MaskWarpLayout mask_warp_layout(int K, int groups) {
+  MaskWarpLayout m;
+  const int L = 11 + K;
+  m.LS = L | 1;
+  int o = 0;
+  m.oH = o; o += m.LS * L;
+  m.oU = o; o += m.LS * L;
+  m.oA = o; o += 66;
+  m.oAQ = o; o += 66;
+  m.oMom = o; o += groups * NMOM;
+  m.oX = o; o += K * 6;
+  m.oP = o; o += K;
+  m.oMono = o; o += 16;
+  m.per_warp = (o + 3) & ~3;
+  return m;
+}
+
+__global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
+                                                                const __grid_constant__ ExpandBatch batch, int mode, int groups, int view0,
+                                                                float* __restrict__ H_T, const float* __restrict__ conf,
+                                                                const float* __restrict__ cholT) {
+  extern __shared__ __align__(16) float smem[];
+  const ExpandView& vw = batch.v[view0 + blockIdx.y];
+  const int K = sc.K, L = 11 + K, LB = L * (L + 1) / 2, bgch = cfg.mask_bg_channel;
+  const MaskWarpLayout lay = mask_warp_layout(K, groups);
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5, LS = lay.LS;
+  float* base = smem + (size_t)wib * lay.per_warp;
+  float *Hm = base + lay.oH, *Um = base + lay.oU, *As = base + lay.oA, *AQs = base + lay.oAQ, *mom = base + lay.oMom;
+  float *xs = base + lay.oX, *ps = base + lay.oP, *mono = base + lay.oMono;
+  const uint32_t n_touched = vw.counters->n_touched;
+  const int stride = NMOM * groups;
+  float gain = 0.f;
+  for (uint32_t t = blockIdx.x * wpb + wib; t < n_touched; t += gridDim.x * wpb) {
+    const uint32_t r = vw.touched[t];
+    const uint32_t g = vw.ids_sorted[r];
+    __syncwarp();
+    // moments of all groups -> shared memory (and zero the buffer for the next view)
+    float* gm = vw.moments + (size_t)r * stride;
+    for (int i = lane; i < stride; i += 32) { mom[i] = gm[i]; gm[i] = 0.f; }
+    __syncwarp();
+    {   // whitened basis -> u basis, one lane per group
+      const Splat sp = vw.splat_sorted[r];
+      for (int gr = lane; gr < groups; gr += 32) {
+        float m[NMOM];
+#pragma unroll
+        for (int i = 0; i < NMOM; ++i) m[i] = mom[gr * NMOM + i];
+        whitened_to_u<float>(m, sp);
+#pragma unroll
+        for (int i = 0; i < NMOM; ++i) mom[gr * NMOM + i] = m[i];
+      }
+    }
+    __syncwarp();
+    if (lane < 15) {
+      float v = 0.f;
+      for (int gr = 0; gr < groups; ++gr) v += mom[gr * NMOM + lane];
+      mono[lane] = v;
+    }
+    if (lane == 15) mono[15] = mom[MOM_W2];
+    for (int i = lane; i < K * 6; i += 32) {
+      const int slot = i / 6, e = i - 6 * slot;
+      xs[i] = mom[(slot >> 2) * NMOM + MOM_X + 6 * (slot & 3) + e];
+    }
+    float s2p = 0.f;
+    for (int slot = lane; slot < K; slot += 32) {
+      const float pv = expf(sc.logits[(size_t)g * K + mask_channel_of_slot(slot, bgch)] - sc.lse[g]);
+      ps[slot] = pv;
+      s2p += pv * pv;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s2p += __shfl_xor_sync(0xffffffffu, s2p, o);
+    const float S2 = s2p;
+    {   // chain rule (every lane, redundantly), A and A Q into shared memory for dynamic indexing
+      Chain<float> ch;
+      projection_chain<float>(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
+      const float sg = sc.sigma[g];
+      const float kappa = cfg.opacity_coord == 0 ? (1.f - sg) : 1.f / sg;       // R-10
+      if (lane < 11) {
+        float a6[6];
+        if (lane < 10) {
+          a6[0] = ch.G[0][lane]; a6[1] = ch.G[1][lane]; a6[2] = 0.5f * ch.G[2][lane]; a6[3] = ch.G[3][lane]; a6[4] = 0.5f * ch.G[4][lane]; a6[5] = 0.f;
+        } else {
+          a6[0] = a6[1] = a6[2] = a6[3] = a6[4] = 0.f; a6[5] = kappa;
+        }
+#pragma unroll
+        for (int e = 0; e < 6; ++e) As[lane * 6 + e] = a6[e];
+      }
+    }
+    __syncwarp();
+    if (lane < 11) {
+      const int ex[6] = {1, 0, 2, 1, 0, 0}, ey[6] = {0, 1, 0, 1, 2, 0};
+      for (int j = 0; j < 6; ++j) {
+        float v = 0.f;
+        for (int i = 0; i < 6; ++i) v += As[lane * 6 + i] * mono[mono_index(ex[i] + ex[j], ey[i] + ey[j])];
+        AQs[lane * 6 + j] = v;
+      }
+    }
+    __syncwarp();
+    const float W2 = mono[15];
+    float xbar[6];
+#pragma unroll
+    for (int e = 0; e < 6; ++e) {
+      float v = 0.f;
+      for (int slot = 0; slot < K; ++slot) v += ps[slot] * xs[slot * 6 + e];
+      xbar[e] = v;
+    }
+    // the full symmetric block, column j by lane j (and j + 32)
+    for (int j = lane; j < L; j += 32) {
+      if (j < 11) {
+        for (int i = 0; i < 11; ++i) {
+          float v = 0.f;
+#pragma unroll
+          for (int e = 0; e < 6; ++e) v += AQs[i * 6 + e] * As[j * 6 + e];
+          Hm[i * LS + j] = v;
+        }
+        for (int c = 0; c < K; ++c) {
+          const int slot = mask_slot_of_channel(c, bgch);
+          float v = 0.f;
+#pragma unroll
+          for (int e = 0; e < 6; ++e) v += As[j * 6 + e] * (ps[slot] * (xs[slot * 6 + e] - xbar[e]));
+          Hm[(11 + c) * LS + j] = v;
+        }
+      } else {
+        const int c = j - 11, slot = mask_slot_of_channel(c, bgch);
+        const float pc = ps[slot];
+        for (int i = 0; i < 11; ++i) {
+          float v = 0.f;
+#pragma unroll
+          for (int e = 0; e < 6; ++e) v += As[i * 6 + e] * (pc * (xs[slot * 6 + e] - xbar[e]));
+          Hm[i * LS + j] = v;
+        }
+        for (int d = 0; d < K; ++d) {
+          const float pd = ps[mask_slot_of_channel(d, bgch)];
+          float v = pc * pd * (S2 - pc - pd);
+          if (d == c) v += pc * pc;
+          Hm[(11 + d) * LS + j] = W2 * v;
+        }
+      }
+    }
+    __syncwarp();
+    if (mode == EXPAND_TRAIN || mode == EXPAND_VIEW) {
+      float* dst = (mode == EXPAND_TRAIN ? H_T : vw.out_blocks) + (size_t)g * LB;
+      for (int rr = 0; rr < L; ++rr)
+        for (int c = rr + lane; c < L; c += 32) {
+          if (mode == EXPAND_TRAIN) dst[triL(rr, c, L)] += Hm[rr * LS + c];     // one launch per view, in view order
+          else dst[triL(rr, c, L)] = Hm[rr * LS + c];
+        }
+      continue;
+    }
+    const float cg = conf[g];
+    const float cb = cfg.weight_mode == 1 ? 1.0f : cg;
+    float gn = 0.f;
+    if (cg > 0.f) {
+      const float* ut = cholT + (size_t)g * LB;
+      for (int rr = 0; rr < L; ++rr)
+        for (int c = rr + lane; c < L; c += 32) Um[rr * LS + c] = ut[triL(rr, c, L)];
+      __syncwarp();
+      // (a) columns: U^T x = c h_j
+      for (int j = lane; j < L; j += 32)
+        for (int i = 0; i < L; ++i) {
+          float v = cb * Hm[i * LS + j];
+#pragma unroll 4
+          for (int k = 0; k < i; ++k) v -= Um[k * LS + i] * Hm[k * LS + j];
+          Hm[i * LS + j] = v / Um[i * LS + i];
+        }
+      __syncwarp();
+      // (b) rows: U^T y = (row i)^T
+      for (int i = lane; i < L; i += 32)
+        for (int c = 0; c < L; ++c) {
+          float v = Hm[i * LS + c];
+#pragma unroll 4
+          for (int k = 0; k < c; ++k) v -= Um[k * LS + c] * Hm[i * LS + k];
+          Hm[i * LS + c] = v / Um[c * LS + c];
+        }
+      __syncwarp();
+      // log det(I + W): right-looking Cholesky on the excess, lower triangle
+      for (int j = 0; j < L; ++j) {
+        const float e = fmaxf(Hm[j * LS + j], 0.f);
+        gn += log1pf(e);
+        const float inv = rsqrtf(1.0f + e);
+        __syncwarp();
+        for (int i = j + 1 + lane; i < L; i += 32) Hm[i * LS + j] *= inv;
+        __syncwarp();
+        for (int i = j + 1 + lane; i < L; i += 32) {
+          const float li = Hm[i * LS + j];
+#pragma unroll 4
+          for (int k = j + 1; k <= i; ++k) Hm[i * LS + k] -= li * Hm[k * LS + j];
+        }
+        __syncwarp();
+      }
+    }
+    if (cfg.weight_mode == 1) gn *= cg;
+    if (lane == 0) {
+      if (vw.gains) vw.gains[g] = gn;
+      gain += gn;
+    }
+  }
+  if (mode == EXPAND_GAIN) {
+    __shared__ float ws[8];
+    if (lane == 0) ws[wib] = gain;
+    __syncthreads();
+    double tsum = 0.0;
+    if (threadIdx.x == 0)
+      for (int w = 0; w < wpb; ++w) tsum += (double)ws[w];
+    ordered_score(tsum, vw.partials, &vw.counters->n_expanded, vw.score);    // block partials added in block order
+  }
+}
+
+void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, float* H_T,
+                        const float* conf, const float* cholT, cudaStream_t st) {
+  const MaskWarpLayout lay = mask_warp_layout(sc.K, groups);
+  int wpb = 8;
+  while (wpb > 1 && (size_t)wpb * lay.per_warp * 4 > 200 * 1024) wpb >>= 1;
+  const size_t smem = (size_t)wpb * lay.per_warp * 4;
+  // the attribute is per device and per function: set it whenever the launch needs more than the default 48 KB
+  if (smem > 48 * 1024 &&
+      cudaFuncSetAttribute(expand_mask_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return;                                           // the caller's cudaGetLastError() reports it
+  if (mode == EXPAND_TRAIN) {
+    const int blocks = sm_count() * 2;
+    for (int v = 0; v < batch.n; ++v) {
+      ++g_kernel_launches;
+      expand_mask_warp_kernel<<<dim3((unsigned)blocks, 1u), wpb * 32, smem, st>>>(sc, cfg, batch, mode, groups, v, H_T, conf, cholT);
+    }
+    return;
+  }
+  ++g_kernel_launches;
+  const int blocks = std::max(1, (sm_count() * 2 + batch.n - 1) / batch.n);
+  expand_mask_warp_kernel<<<dim3((unsigned)blocks, (unsigned)batch.n), wpb * 32, smem, st>>>(sc, cfg, batch, mode, groups, 0, H_T, conf, cholT);
+}
+
+// once per scoring call of a mask context: U_g = upper Cholesky factor of c_g H_T,g + Lambda (L x L)
+template <int KMAX>
+__global__ void __launch_bounds__(64) prepare_mask_kernel(int N, int K, nbv_config cfg, const float* __restrict__ H_T,
+                                                           const float* __restrict__ conf, float* __restrict__ cholT) {
+  constexpr int LMAX = 11 + KMAX, LBMAX = LMAX * (LMAX + 1) / 2;
+  const int g = blockIdx.x * blockDim.x + threadIdx.x;
+  if (g >= N) return;
+  const float c = conf[g];
+  if (!(c > 0.f)) return;
+  const int L = 11 + K, LB = L * (L + 1) / 2;
+  const float* ht = H_T + (size_t)g * LB;
+  float H[LBMAX];
+  const float ct = cfg.weight_mode == 0 ? c : 1.0f;
+  for (int i = 0; i < LB; ++i) H[i] = ct * ht[i];
+  for (int k = 0; k < L; ++k) H[triL(k, k, L)] += k < 11 ? cfg.prior_precision[k] : cfg.prior_precision_obj;
+  cholesky_L(H, L);
+  float* dst = cholT + (size_t)g * LB;
+  for (int i = 0; i < LB; ++i) dst[i] = H[i];
+}
+
+void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st) {
+  ++g_kernel_launches;
+  if (sc.K <= 20)
+    prepare_mask_kernel<20><<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, sc.K, cfg, H_T, conf, cholT);
+  else
+    prepare_mask_kernel<NBV_MASK_KMAX><<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, sc.K, cfg, H_T, conf, cholT);
+}
+
+// parity export: (rgb | depth) images of one group's forward pass -> mask channels of that group
+__global__ void __launch_bounds__(256) mask_scatter_kernel(const float* __restrict__ rgb, const float* __restrict__ depth, size_t npx, int K,
+                                                            int group, int bgch, float* __restrict__ mask) {
+  const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= npx) return;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int t = 4 * group + j;
+    if (t < K) mask[p * K + mask_channel_of_slot(t, bgch)] = j < 3 ? rgb[3 * p + j] : depth[p];
+  }
+}
+
+void launch_mask_scatter(const float* rgb, const float* depth, size_t npx, int K, int group, int bgch, float* mask, cudaStream_t st) {
+  ++g_kernel_launches;
+  mask_scatter_kernel<<<(unsigned)((npx + 255) / 256), 256, 0, st>>>(rgb, depth, npx, K, group, bgch, mask);
+}
+
+}  // namespace nbv

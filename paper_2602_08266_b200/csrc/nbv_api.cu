@@ -14,7 +14,19 @@ using namespace nbv;
 
 namespace nbv {
 unsigned long long g_kernel_launches = 0;
+
+int sm_count() {
+  static int cached[64] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return 148; }
+  if (cached[dev] == 0) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) { cudaGetLastError(); n = 148; }
+    cached[dev] = n;
+  }
+  return cached[dev];
 }
+}  // namespace nbv
 
 namespace {
 
@@ -33,7 +45,7 @@ struct ViewSlot {
   cudaEvent_t done = nullptr;
   DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, msplit, gsplat;
   DevBuf ckeys, crect, cranges, sort_tmp, scan_tmp, tile_counts;
-  DevBuf pix_rgb, pix_depth, pix_T, pix_nc, pix_last, tile_cend, tile_walk, moments, touched;
+  DevBuf pix_rgb, pix_depth, pix_T, pix_nc, pix_last, tile_cend, tile_elast, tile_walk, moments, touched, touched_cnt, partials;
   ViewCounters* d_counters = nullptr;
   ViewCounters* h_counters = nullptr;   // pinned
   // products of the last process_view()
@@ -62,9 +74,11 @@ struct nbv_ctx {
   size_t LB = NBLK;
   int n_train = 0;
   // scene
-  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp, cache_ids, cache_blocks, cache_meta;
+  // H_T: N x 105 binary64 (colour / depth contexts) or N x LB binary32 (mask contexts); cholT: mask contexts only
+  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp, cache_ids, cache_blocks, cache_meta,
+      cache_scratch;
   size_t greedy_cache_bytes = (size_t)4 << 30;   // budget of the block cache of nbv_select_greedy (NBV_GREEDY_CACHE_MB)
-  int conf_target = -2;                 // target the conf / cholT buffers were prepared for (-2 = stale)
+  int conf_target = -2;                 // mask contexts: target the cholT buffer was prepared for (-2 = stale)
   // views in flight: S1-S2 of each view run on its slot's stream, S3-S6 of a whole batch in one launch per stage on
   // the caller's stream; two sets of `concurrency` slots alternate so the next batch's S1-S2 overlap this batch's S3-S6
   std::vector<ViewSlot*> slots;
@@ -153,7 +167,7 @@ bool valid_camera(const nbv_camera& c) {
     for (int j = 0; j < 3; ++j) {
       double d = 0;
       for (int k = 0; k < 3; ++k) d += (double)c.R_cw[3 * i + k] * c.R_cw[3 * j + k];
-      if (!(std::fabs(d - (i == j ? 1.0 : 0.0)) <= 1e-4)) return false;
+      if (!(std::fabs(d - (i == j ? 1.0 : 0.0)) <= 1e-6)) return false;
     }
   }
   return true;
@@ -168,7 +182,7 @@ SceneDev scene_dev(const nbv_ctx* c) {
   return s;
 }
 
-constexpr size_t MAX_SPANS = 1 << 15;
+constexpr size_t MAX_SPANS = 1 << 20;       // beyond this, further spans are simply not recorded
 
 // fold the recorded spans into ctx->stage_ms (every stream that recorded one must be idle)
 void fold_timing(nbv_ctx* ctx) {
@@ -187,7 +201,7 @@ void fold_timing(nbv_ctx* ctx) {
 // open a span of `stage` on stream st; returns its index or -1 when timing is off
 int span_begin(nbv_ctx* ctx, int stage, int views, cudaStream_t st) {
   if (!ctx->timing) return -1;
-  if (ctx->spans_used >= MAX_SPANS) { cudaDeviceSynchronize(); fold_timing(ctx); }
+  if (ctx->spans_used >= MAX_SPANS) return -1;   // never recycle: callers may hold open span indices
   if (ctx->spans_used == ctx->spans.size()) {
     Span sp;
     sp.stage = 0; sp.views = 0;
@@ -216,7 +230,7 @@ void free_slot(ViewSlot* sl) {
   DevBuf* all[] = {&sl->splat, &sl->zkey, &sl->zkey_alt, &sl->ids, &sl->ids_alt, &sl->rect, &sl->abc, &sl->splat_sorted,
                    &sl->rect_sorted, &sl->msplit, &sl->gsplat, &sl->ckeys, &sl->crect, &sl->cranges, &sl->sort_tmp,
                    &sl->scan_tmp, &sl->tile_counts, &sl->pix_rgb, &sl->pix_depth, &sl->pix_T, &sl->pix_nc, &sl->pix_last,
-                   &sl->tile_cend, &sl->tile_walk, &sl->moments, &sl->touched};
+                   &sl->tile_cend, &sl->tile_elast, &sl->tile_walk, &sl->moments, &sl->touched, &sl->touched_cnt, &sl->partials};
   for (DevBuf* b : all) release(*b);
   if (sl->d_counters) cudaFree(sl->d_counters);
   if (sl->h_counters) cudaFreeHost(sl->h_counters);
@@ -306,6 +320,7 @@ int pre_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool w
     const size_t npx = (size_t)cam.width * cam.height;
     CKRET(ensure(ctx, sl->pix_T, 4 * npx)); CKRET(ensure(ctx, sl->pix_last, 4 * npx));
     CKRET(ensure(ctx, sl->tile_cend, 4 * (size_t)n_tiles)); CKRET(ensure(ctx, sl->tile_walk, 4 * (size_t)n_tiles));
+    CKRET(ensure(ctx, sl->tile_elast, 4 * (size_t)n_tiles));
     if (full_pix) {
       CKRET(ensure(ctx, sl->pix_rgb, 12 * npx)); CKRET(ensure(ctx, sl->pix_depth, 4 * npx)); CKRET(ensure(ctx, sl->pix_nc, 4 * npx));
     }
@@ -316,6 +331,8 @@ int pre_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool w
     if (sl->moments.cap < mom_bytes || !sl->moments.p) sl->moments_clean = false;
     CKRET(ensure(ctx, sl->moments, mom_bytes));
     CKRET(ensure(ctx, sl->touched, 4 * (size_t)N));
+    CKRET(ensure(ctx, sl->touched_cnt, 4 * (size_t)touched_blocks(N)));
+    CKRET(ensure(ctx, sl->partials, 8 * (size_t)expand_partials()));
     if (!sl->moments_clean) CK(cudaMemsetAsync(sl->moments.p, 0, mom_bytes, st));
     sl->moments_clean = false;     // dirty until an expand kernel has consumed the touched list
   }
@@ -410,8 +427,9 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     v.pix.depth = full_pix ? s->pix_depth.as<float>() : nullptr;
     v.pix.ncontrib = full_pix ? s->pix_nc.as<int32_t>() : nullptr;
     v.pix.T = s->pix_T.as<float>(); v.pix.last = s->pix_last.as<int32_t>();
-    v.tile_cend = s->tile_cend.as<uint32_t>(); v.tile_walk = s->tile_walk.as<uint32_t>();
-    v.moments = s->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = s->touched.as<uint32_t>(); v.counters = s->d_counters;
+    v.tile_cend = s->tile_cend.as<uint32_t>(); v.tile_elast = s->tile_elast.as<uint32_t>(); v.tile_walk = s->tile_walk.as<uint32_t>();
+    v.moments = s->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = s->touched.as<uint32_t>();
+    v.touched_cnt = s->touched_cnt.as<uint32_t>(); v.counters = s->d_counters;
   }
   const TileGrid tg = sl[0]->tg;
   CKRET(ensure_tile_order(ctx, tg, st));
@@ -436,9 +454,10 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
         gb.v[i].moments = sl[i]->moments.as<float>() + (size_t)gr * NMOM;
       }
       if (gr > 0 && gb.work) CK(cudaMemsetAsync(gb.work, 0, 4, st));     // a fresh work counter for every launch
-      launch_backward(gb, ctx->N, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, gcfg, st, gr == 0);
+      launch_backward(gb, ctx->N, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, gcfg, st);
     }
   }
+  launch_touched(rb, ctx->N, st);            // sum w^2 of (group 0 of) every rank -> ordered touched lists
   CK(cudaGetLastError());
   span_end(ctx, sp, st);
   return NBV_OK;
@@ -455,7 +474,7 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     v.cam = cams[i];
     v.ids_sorted = s->ids.as<uint32_t>(); v.splat_sorted = s->splat_sorted.as<Splat>(); v.touched = s->touched.as<uint32_t>();
     v.moments = s->moments.as<float>(); v.out_blocks = out_blocks; v.score = d_scores ? d_scores + i : nullptr; v.gains = gains;
-    v.counters = s->d_counters;
+    v.counters = s->d_counters; v.partials = s->partials.as<double>();
     v.cache_span = cache ? cache->spans + 2 * (size_t)(first_candidate + i) : nullptr;
   }
   const int sp = span_begin(ctx, NBV_STAGE_EXPAND, n, st);
@@ -466,7 +485,7 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     launch_expand_mask(scene_dev(ctx), ctx->cfg, eb, mode, ctx->mask_groups, ctx->H_T.as<float>(), ctx->conf.as<float>(),
                        ctx->cholT.as<float>(), st);
   } else {
-    launch_expand(scene_dev(ctx), ctx->cfg, eb, mode, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
+    launch_expand(scene_dev(ctx), ctx->cfg, eb, mode, ctx->H_T.as<double>(), ctx->conf.as<float>(), st);
   }
   CK(cudaGetLastError());
   span_end(ctx, sp, st);
@@ -495,9 +514,12 @@ int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_
   int V = ctx->concurrency;
   if (V <= 0) V = (n > 0 && make_grid(h_cams[0].width, h_cams[0].height).tiles_x * make_grid(h_cams[0].width, h_cams[0].height).tiles_y < 2000) ? 16 : 8;
   V = std::max(1, std::min(V, MAX_BATCH));
+  int rc = NBV_OK;
   CK(cudaEventRecord(ctx->ev_fork, st));
   for (int s = 0; s < 2; ++s) CK(cudaStreamWaitEvent(ctx->raster_st[s], ctx->ev_fork, 0));
-  int rc = NBV_OK;
+  auto ck = [&](cudaError_t e, const char* what) {       // event plumbing: keep enqueuing (no stream may run ahead), report the first failure
+    if (e != cudaSuccess && rc == NBV_OK) rc = cuda_fail(ctx, e, what);
+  };
   int batch_no = 0;
   bool set_used[2] = {false, false};
   for (int i0 = 0; i0 < n && rc == NBV_OK; ++batch_no) {
@@ -514,31 +536,35 @@ int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_
     if (rc != NBV_OK) break;
     for (int i = 0; i < nb; ++i) {
       // the slot's buffers are free once the S3-S6 launches of the batch that last used this set have finished
-      cudaStreamWaitEvent(sl[i]->st, set_used[set] ? ctx->ev_set_done[set] : ctx->ev_fork, 0);
+      ck(cudaStreamWaitEvent(sl[i]->st, set_used[set] ? ctx->ev_set_done[set] : ctx->ev_fork, 0), "cudaStreamWaitEvent(slot)");
       if (rc == NBV_OK) rc = pre_view(ctx, sl[i], h_cams[i0 + i], STAGE_BACKWARD, false, false, sl[i]->st);
-      cudaEventRecord(sl[i]->done, sl[i]->st);
-      cudaStreamWaitEvent(rs, sl[i]->done, 0);      // join even after an error: no stream may run ahead
+      ck(cudaEventRecord(sl[i]->done, sl[i]->st), "cudaEventRecord(slot)");
+      ck(cudaStreamWaitEvent(rs, sl[i]->done, 0), "cudaStreamWaitEvent(raster)");      // join even after an error: no stream may run ahead
     }
     if (rc == NBV_OK) rc = raster_batch(ctx, sl, h_cams + i0, nb, STAGE_BACKWARD, false, rs);
+    // Batches that write shared state in S5 (H_T += in view order, Eq. 6; the block pool of greedy selection) run that
+    // step after the previous batch's: the sums and the pool layout do not depend on timing.  S3 / S4 still overlap.
+    if ((mode == EXPAND_TRAIN || mode == EXPAND_CACHE) && set_used[set ^ 1])
+      ck(cudaStreamWaitEvent(rs, ctx->ev_set_done[set ^ 1], 0), "cudaStreamWaitEvent(order)");
     if (rc == NBV_OK) rc = expand_batch(ctx, sl, h_cams + i0, nb, mode, nullptr, d_scores ? d_scores + i0 : nullptr, nullptr, rs, cache, i0);
-    cudaEventRecord(ctx->ev_set_done[set], rs);
+    ck(cudaEventRecord(ctx->ev_set_done[set], rs), "cudaEventRecord(set)");
     set_used[set] = true;
     i0 += nb;
   }
   for (int s = 0; s < 2; ++s)
-    if (set_used[s]) cudaStreamWaitEvent(st, ctx->ev_set_done[s], 0);
+    if (set_used[s]) ck(cudaStreamWaitEvent(st, ctx->ev_set_done[s], 0), "cudaStreamWaitEvent(join)");
   return rc;
 }
 
 int prepare_scoring(nbv_ctx* ctx, int target, cudaStream_t st) {
   if (target < -1 || target >= ctx->K) return fail(ctx, NBV_ERR_UNKNOWN_TARGET, "target_obj must be -1 or in [0, K)");
-  if (ctx->conf_target == target) return NBV_OK;
+  // S0' runs in every scoring call (Eq. 7 / Eq. 12: N numbers).  Colour / depth contexts need nothing else: S6 factors
+  // c_g H_T,g + Lambda itself, for the touched Gaussians only.  Mask contexts keep a factor table, rebuilt when H_T or the
+  // target changed.
   const SceneDev sc = scene_dev(ctx);
   launch_confidence(sc, ctx->cfg, target, ctx->conf.as<float>(), st);
-  if (ctx->mask_mode)
+  if (ctx->mask_mode && ctx->conf_target != target)
     launch_prepare_mask(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
-  else
-    launch_prepare(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
   CK(cudaGetLastError());
   ctx->conf_target = target;
   return NBV_OK;
@@ -637,7 +663,7 @@ void nbv_destroy(nbv_ctx* ctx) {
   cudaDeviceSynchronize();
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
                    &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order, &ctx->work_counters, &ctx->cache_ids,
-                   &ctx->cache_blocks, &ctx->cache_meta};
+                   &ctx->cache_blocks, &ctx->cache_meta, &ctx->cache_scratch};
   for (DevBuf* b : all) release(*b);
   for (ViewSlot* sl : ctx->slots) free_slot(sl);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -676,15 +702,16 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
   CKRET(ensure(ctx, ctx->mean, 12 * n)); CKRET(ensure(ctx, ctx->logscale, 12 * n)); CKRET(ensure(ctx, ctx->quat, 16 * n));
   CKRET(ensure(ctx, ctx->sigma, 4 * n)); CKRET(ensure(ctx, ctx->rgb, 12 * n)); CKRET(ensure(ctx, ctx->logits, 4 * n * K));
   CKRET(ensure(ctx, ctx->M, 36 * n)); CKRET(ensure(ctx, ctx->pmax, 4 * n)); CKRET(ensure(ctx, ctx->amax, 4 * n));
-  CKRET(ensure(ctx, ctx->lse, 4 * n)); CKRET(ensure(ctx, ctx->H_T, 4 * ctx->LB * n)); CKRET(ensure(ctx, ctx->conf, 4 * n));
-  CKRET(ensure(ctx, ctx->cholT, 4 * ctx->LB * n));
+  const size_t ht_bytes = (ctx->mask_mode ? 4 : 8) * ctx->LB * n;
+  CKRET(ensure(ctx, ctx->lse, 4 * n)); CKRET(ensure(ctx, ctx->H_T, ht_bytes)); CKRET(ensure(ctx, ctx->conf, 4 * n));
+  if (ctx->mask_mode) CKRET(ensure(ctx, ctx->cholT, 4 * ctx->LB * n));
   CK(cudaMemcpyAsync(ctx->mean.p, d_mean, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->logscale.p, d_logscale, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->quat.p, d_quat, 16 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->sigma.p, d_opacity, 4 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->rgb.p, d_rgb, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->logits.p, d_obj_logits, 4 * n * K, cudaMemcpyDeviceToDevice, st));
-  CK(cudaMemsetAsync(ctx->H_T.p, 0, 4 * ctx->LB * n, st));
+  CK(cudaMemsetAsync(ctx->H_T.p, 0, ht_bytes, st));
   ViewSlot* s0 = ctx->slots[0];
   CK(cudaDeviceSynchronize());             // no view of a previous scene may still be in flight
   CK(cudaMemsetAsync(s0->d_counters, 0, sizeof(ViewCounters), st));
@@ -704,7 +731,7 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
 int nbv_reset_training(nbv_ctx* ctx, void* stream) {
   if (!ctx) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
-  CK(cudaMemsetAsync(ctx->H_T.p, 0, 4 * ctx->LB * ctx->N, (cudaStream_t)stream));
+  CK(cudaMemsetAsync(ctx->H_T.p, 0, (ctx->mask_mode ? 4 : 8) * ctx->LB * ctx->N, (cudaStream_t)stream));
   ctx->n_train = 0;
   ctx->conf_target = -2;
   return NBV_OK;
@@ -844,15 +871,17 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
   // A view's blocks do not depend on H_T, so every candidate is rasterised ONCE: S1-S5 leave its touched Gaussians and
   // their unweighted 14x14 blocks in a sparse pool; every round then needs only S0' (new factors), S6 over the pool,
   // the masked arg-max and H_T += (blocks of the selected view) -- all on the device, no camera and no host round trip.
-  const size_t entry_bytes = 4 * (size_t)NBLK + 4;
+  const size_t entry_bytes = 8 * (size_t)NBLK + 4;
   const size_t want = std::min((size_t)n * (size_t)ctx->N, ctx->greedy_cache_bytes / entry_bytes);
   if (want == 0 || want > 0xfffffff0ull || ctx->mask_mode) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);
   CKRET(ensure(ctx, ctx->cache_ids, 4 * want));
-  CKRET(ensure(ctx, ctx->cache_blocks, 4 * (size_t)NBLK * want));
+  CKRET(ensure(ctx, ctx->cache_blocks, 8 * (size_t)NBLK * want));
+  CKRET(ensure(ctx, ctx->cache_scratch, cached_gain_scratch_bytes(n)));
+  CK(cudaMemsetAsync(ctx->cache_scratch.p, 0, cached_gain_scratch_bytes(n), st));
   // meta: spans (2n) | cursor + overflow flag (2) | taken (n) | scores (n) | pick (1) | order (rounds)
   CKRET(ensure(ctx, ctx->cache_meta, 4 * (4 * (size_t)n + 4 + (size_t)rounds)));
   BlockCache bc;
-  bc.ids = ctx->cache_ids.as<uint32_t>(); bc.blocks = ctx->cache_blocks.as<float>();
+  bc.ids = ctx->cache_ids.as<uint32_t>(); bc.blocks = ctx->cache_blocks.as<double>();
   bc.spans = ctx->cache_meta.as<uint32_t>(); bc.cursor = bc.spans + 2 * (size_t)n; bc.capacity = (uint32_t)want;
   int32_t* d_taken = reinterpret_cast<int32_t*>(bc.cursor + 2);
   float* d_round = reinterpret_cast<float*>(d_taken + n);
@@ -866,10 +895,9 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
   if (h_cursor[1]) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);   // pool too small
   for (int r = 0; r < rounds; ++r) {
     CKRET(prepare_scoring(ctx, target_obj, st));
-    CK(cudaMemsetAsync(d_round, 0, 4 * (size_t)n, st));
-    launch_cached_gain(bc, n, d_taken, ctx->conf.as<float>(), ctx->cholT.as<float>(), d_round, ctx->cfg.weight_mode, st);
+    launch_cached_gain(bc, ctx->cfg, n, d_taken, ctx->conf.as<float>(), ctx->H_T.as<double>(), d_round, ctx->cache_scratch.p, st);
     launch_greedy_pick(d_round, d_taken, n, d_scores ? d_scores + (size_t)r * n : nullptr, d_pick, d_order + r, st);
-    launch_cache_accumulate(bc, d_pick, ctx->H_T.as<float>(), st);      // Eq. 6: H_T += H(c*)
+    launch_cache_accumulate(bc, d_pick, ctx->H_T.as<double>(), st);      // Eq. 6: H_T += H(c*)
     CK(cudaGetLastError());
     ctx->conf_target = -2;                                                // the factors of H_T are stale
     ++ctx->n_train;
@@ -1001,9 +1029,9 @@ int nbv_render_mask(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_mask, void* 
     v.splat_sorted = sl->gsplat.as<Splat>(); v.ckeys = sl->ckeys_sorted; v.crect = sl->crect.as<ushort4>(); v.cranges = sl->cranges.as<uint2>();
     v.pix.rgb = sl->pix_rgb.as<float>(); v.pix.depth = sl->pix_depth.as<float>(); v.pix.ncontrib = sl->pix_nc.as<int32_t>();
     v.pix.T = sl->pix_T.as<float>(); v.pix.last = sl->pix_last.as<int32_t>();
-    v.tile_cend = sl->tile_cend.as<uint32_t>(); v.tile_walk = sl->tile_walk.as<uint32_t>();
+    v.tile_cend = sl->tile_cend.as<uint32_t>(); v.tile_elast = sl->tile_elast.as<uint32_t>(); v.tile_walk = sl->tile_walk.as<uint32_t>();
     v.moments = sl->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = sl->touched.as<uint32_t>();
-    v.counters = sl->d_counters;
+    v.touched_cnt = sl->touched_cnt.as<uint32_t>(); v.counters = sl->d_counters;
     launch_forward(rb, sl->tg, sl->rank_bits, h_cam->width, h_cam->height, gcfg, true, st);
     launch_mask_scatter(sl->pix_rgb.as<float>(), sl->pix_depth.as<float>(), npx, ctx->K, gr, ctx->cfg.mask_bg_channel, d_mask, st);
     CK(cudaGetLastError());
@@ -1037,7 +1065,21 @@ int nbv_view_hessian(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_blocks, voi
 int nbv_training_hessian(nbv_ctx* ctx, float* d_blocks, void* stream) {
   if (!ctx || !d_blocks) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
-  CK(cudaMemcpyAsync(d_blocks, ctx->H_T.p, 4 * ctx->LB * ctx->N, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  if (ctx->mask_mode) {
+    CK(cudaMemcpyAsync(d_blocks, ctx->H_T.p, 4 * ctx->LB * ctx->N, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  } else {
+    launch_export_blocks(ctx->H_T.as<double>(), d_blocks, ctx->LB * (size_t)ctx->N, (cudaStream_t)stream);
+    CK(cudaGetLastError());
+  }
+  return NBV_OK;
+}
+
+int nbv_chain(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_chain, void* stream) {
+  if (!ctx || !h_cam || !d_chain) return NBV_ERR_INVALID_ARG;
+  if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  if (!valid_camera(*h_cam)) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
+  launch_export_chain(scene_dev(ctx), *h_cam, d_chain, (cudaStream_t)stream);
+  CK(cudaGetLastError());
   return NBV_OK;
 }
 

@@ -97,8 +97,16 @@ __device__ __forceinline__ void shift_queue(uint32_t* q_rank, uint32_t* q_cpos, 
 
 // FULLPIX = false is the timed path: S4 needs only the final transmittance and `last` of every pixel (it rebuilds the
 // suffix sums itself), so colour, depth and the contributor count are accumulated only for the parity exports.
-// The slot body is branch-free (predicated updates): the 8 pixels of a lane are 8 independent dependency chains the
-// scheduler can interleave, and after the ellipse test nearly every staged entry touches nearly every slot anyway.
+//
+// Slot body.  A lane's 8 pixels are 4 PAIRS (row q, row 7 - q) evaluated with packed binary32 operations (FFMA2 /
+// FMUL2 / FADD2: two pixels per issue slot, each half rounded like the scalar .rn operation, so the decision path is
+// bit for bit the specified one).  Per pixel and entry: 19 packed-pipe operations per pair (dy, power, exp_spec, sigma G,
+// 1 - alpha, T (1 - alpha)) and 8 scalar ones (the exponent bits of exp_spec, three range / alpha tests, min, two
+// selects, the stop test).  Nothing else: a pixel that stops (R-4: the entry that would take T below t_stop is not
+// composited, the pixel is finished) leaves its T unchanged but NEGATED, and a branch the warp takes only then -- 8 times
+// per lane and tile -- retires it (py = +inf: its power fails every later range test), counts it, and records in `last`
+// how many list entries precede the stop.  A pixel that never stops gets last = number of entries walked.  Every entry
+// S4 must composite at a pixel lies before `last`, and S4 re-takes the same pass decisions, so it finds the same set.
 template <bool FULLPIX>
 __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
   // One launch rasterises every view of the batch.  Launch position -> (view, tile): the views are
@@ -123,8 +131,6 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   const ushort4* __restrict__ crect = vw.crect;
   const uint2* __restrict__ cranges = vw.cranges;
   const PixelBuf out = vw.pix;
-  uint32_t* __restrict__ tile_cend = vw.tile_cend;
-  uint32_t* __restrict__ tile_walk = vw.tile_walk;
   ViewCounters* counters = vw.counters;
   const int tile = batch.tile_order[bpos / (uint32_t)batch.n];   // heaviest tiles first (launch order)
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
@@ -135,18 +141,21 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   const uint32_t rmask = (1u << prm.rank_bits) - 1u;
   const uint32_t lt = (1u << lane) - 1u;
 
-  float T[PPL], py[PPL], C0[PPL], C1[PPL], C2[PPL], D[PPL];
+  // pair q holds the pixels of rows q (.x) and 7 - q (.y)
+  f2 T2[PPL / 2], py2[PPL / 2];
+  float C0[PPL], C1[PPL], C2[PPL], D[PPL];
   int n[PPL], last[PPL];
   // A pixel that has terminated (or lies outside the image) gets py = +inf: its power evaluates to -inf or NaN and
   // fails `power >= tau`, so no separate done mask has to be tested in the slot body.
   int ndone = 0;
 #pragma unroll
   for (int k = 0; k < PPL; ++k) {
-    T[k] = 1.0f; C0[k] = C1[k] = C2[k] = D[k] = 0.0f; n[k] = 0; last[k] = 0;
-    py[k] = (float)(y0 + k) + 0.5f;
-    if (x >= prm.W || y0 + k >= prm.H) { py[k] = INFINITY; ++ndone; }
+    C0[k] = C1[k] = C2[k] = D[k] = 0.0f; n[k] = 0; last[k] = 0;
+    float py = (float)(y0 + k) + 0.5f;
+    if (x >= prm.W || y0 + k >= prm.H) { py = INFINITY; ++ndone; }
+    if (k < PPL / 2) { T2[k].x = 1.0f; py2[k].x = py; } else { T2[PPL - 1 - k].y = 1.0f; py2[PPL - 1 - k].y = py; }
   }
-  uint32_t walked = 0, cend = 0;
+  uint32_t walked = 0, cend = 0, elast = 0;
   uint32_t pos = range.x, qn = 0;
   int e_base = 0;
   bool finished = __all_sync(FULL, ndone == PPL);
@@ -181,33 +190,46 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
     stage_queue(splat_sorted, q_rank, q_cpos, cnt, sm);
     for (uint32_t j = 0; j < cnt; ++j) {
       const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
-      const int e1 = e_base + (int)j + 1;
+      const int e = e_base + (int)j;                           // position of this entry in the tile's list
       const float dx = sub_rn(px, s0.x);
-      bool anycomp = false;
+      bool anypass = false;
+      uint32_t neg = 0u;
       ++walked;
 #pragma unroll
-      for (int k = 0; k < PPL; ++k) {
-        const float dy = sub_rn(py[k], s0.y);
-        const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
-        const float a = mul_rn(s1.y, exp_spec(power));       // garbage outside [tau, 0]: masked by `pass`
+      for (int q = 0; q < PPL / 2; ++q) {
+        const f2 dy = sub2(py2[q], bc2(s0.y));
+        const f2 power = splat_power2(s0.z, s0.w, s1.x, dx, dy);
+        const f2 a = mul2(bc2(s1.y), exp_spec2(power));       // garbage outside [tau, 0]: masked by `pass`
         // s1.w = tau >= -6 is a pre-test that never decides (project.cu); the alpha test does (R-4, R-5)
-        const bool pass = power <= 0.0f && power >= s1.w && a >= prm.alpha_min;
-        const float alpha = fminf(a, prm.alpha_max);
-        const float Tn = mul_rn(T[k], sub_rn(1.0f, alpha));
-        const bool stop = Tn < prm.t_stop;                   // stop BEFORE compositing (R-4)
-        const bool comp = pass && !stop;
+        const bool pass_x = power.x <= 0.0f && power.x >= s1.w && a.x >= prm.alpha_min;
+        const bool pass_y = power.y <= 0.0f && power.y >= s1.w && a.y >= prm.alpha_min;
+        f2 al;
+        al.x = pass_x ? fminf(a.x, prm.alpha_max) : 0.0f;
+        al.y = pass_y ? fminf(a.y, prm.alpha_max) : 0.0f;
+        const f2 Tn = mul2(T2[q], sub2(bc2(1.0f), al));        // alpha = 0: T (1 - 0) = T exactly
+        // stop BEFORE compositing (R-4).  T >= t_stop always, so Tn < t_stop happens only where the pixel passed.
+        const bool stop_x = Tn.x < prm.t_stop, stop_y = Tn.y < prm.t_stop;
         if (FULLPIX) {
-          const float w = comp ? alpha * T[k] : 0.0f;
-          C0[k] = fmaf(s2.x, w, C0[k]); C1[k] = fmaf(s2.y, w, C1[k]); C2[k] = fmaf(s2.z, w, C2[k]);
-          D[k] = fmaf(s1.z, w, D[k]);
-          n[k] += comp ? 1 : 0;
+          const float wx = (pass_x && !stop_x) ? al.x * T2[q].x : 0.0f, wy = (pass_y && !stop_y) ? al.y * T2[q].y : 0.0f;
+          const int kx = q, ky = PPL - 1 - q;
+          C0[kx] = fmaf(s2.x, wx, C0[kx]); C1[kx] = fmaf(s2.y, wx, C1[kx]); C2[kx] = fmaf(s2.z, wx, C2[kx]); D[kx] = fmaf(s1.z, wx, D[kx]);
+          C0[ky] = fmaf(s2.x, wy, C0[ky]); C1[ky] = fmaf(s2.y, wy, C1[ky]); C2[ky] = fmaf(s2.z, wy, C2[ky]); D[ky] = fmaf(s1.z, wy, D[ky]);
+          n[kx] += (pass_x && !stop_x) ? 1 : 0;
+          n[ky] += (pass_y && !stop_y) ? 1 : 0;
         }
-        T[k] = comp ? Tn : T[k];
-        last[k] = comp ? e1 : last[k];
-        if (pass && stop) { py[k] = INFINITY; ++ndone; }
-        anycomp = anycomp || comp;
+        T2[q].x = stop_x ? -T2[q].x : Tn.x;
+        T2[q].y = stop_y ? -T2[q].y : Tn.y;
+        neg |= __float_as_uint(T2[q].x) | __float_as_uint(T2[q].y);
+        anypass = anypass || pass_x || pass_y;
       }
-      if (anycomp) cend = __float_as_uint(s2.w);               // coarse position + 1 of the last composited entry
+      if (anypass) { cend = __float_as_uint(s2.w); elast = (uint32_t)e + 1u; }   // coarse position + 1, list position + 1
+      if (neg & 0x80000000u) {                                  // some pixel of this lane stopped at this entry
+#pragma unroll
+        for (int q = 0; q < PPL / 2; ++q) {
+          if (T2[q].x < 0.0f) { T2[q].x = -T2[q].x; py2[q].x = INFINITY; last[q] = e; ++ndone; }
+          if (T2[q].y < 0.0f) { T2[q].y = -T2[q].y; py2[q].y = INFINITY; last[PPL - 1 - q] = e; ++ndone; }
+        }
+      }
       if (__all_sync(FULL, ndone == PPL)) { finished = true; break; }
     }
     e_base += (int)cnt;
@@ -218,26 +240,30 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   for (int k = 0; k < PPL; ++k) {
     if (x < prm.W && y0 + k < prm.H) {
       const size_t p = (size_t)(y0 + k) * prm.W + x;
+      const float Tk = k < PPL / 2 ? T2[k].x : T2[PPL - 1 - k].y;
+      const float pyk = k < PPL / 2 ? py2[k].x : py2[PPL - 1 - k].y;
       if (FULLPIX) {
         pairs += n[k];
-        out.rgb[3 * p + 0] = fmaf(prm.bg[0], T[k], C0[k]);
-        out.rgb[3 * p + 1] = fmaf(prm.bg[1], T[k], C1[k]);
-        out.rgb[3 * p + 2] = fmaf(prm.bg[2], T[k], C2[k]);
+        out.rgb[3 * p + 0] = fmaf(prm.bg[0], Tk, C0[k]);
+        out.rgb[3 * p + 1] = fmaf(prm.bg[1], Tk, C1[k]);
+        out.rgb[3 * p + 2] = fmaf(prm.bg[2], Tk, C2[k]);
         out.depth[p] = D[k];
         out.ncontrib[p] = n[k];
       }
-      out.T[p] = T[k];
-      out.last[p] = last[k];
+      out.T[p] = Tk;
+      out.last[p] = pyk == INFINITY ? last[k] : (int)walked;     // never stopped: every walked entry precedes `last`
     }
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     if (FULLPIX) pairs += __shfl_xor_sync(FULL, pairs, o);
     cend = max(cend, __shfl_xor_sync(FULL, cend, o));
+    elast = max(elast, __shfl_xor_sync(FULL, elast, o));
   }
   if (lane == 0) {
-    tile_cend[tile] = cend;
-    tile_walk[tile] = walked;
+    vw.tile_cend[tile] = cend;
+    vw.tile_elast[tile] = elast;
+    vw.tile_walk[tile] = walked;
     if (FULLPIX) {
       atomicAdd(&counters->n_entries, (unsigned long long)walked);
       atomicAdd(&counters->n_pairs, (unsigned long long)pairs);
@@ -271,23 +297,24 @@ __device__ __forceinline__ float4 reduce40(const float (&v)[NMOM], float* red, i
   for (int q = 0; q < NMOM / 4; ++q) row[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
   __syncwarp();
   const int q = lane % 10, rg = lane / 10;
-  float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+  f2 a01 = bc2(0.f), a23 = bc2(0.f), b01 = bc2(0.f), b23 = bc2(0.f);     // packed adds: two moments per issue slot
   if (lane < 30) {
     const float* col = red + 4 * q;
 #pragma unroll
     for (int i = 0; i < 10; i += 2) {
       const float4 x = *reinterpret_cast<const float4*>(col + (rg + 3 * i) * RED_STRIDE);
       const float4 y = *reinterpret_cast<const float4*>(col + (rg + 3 * i + 3) * RED_STRIDE);
-      a.x += x.x; a.y += x.y; a.z += x.z; a.w += x.w;
-      b.x += y.x; b.y += y.y; b.z += y.z; b.w += y.w;
+      a01 = add2(a01, make_float2(x.x, x.y)); a23 = add2(a23, make_float2(x.z, x.w));
+      b01 = add2(b01, make_float2(y.x, y.y)); b23 = add2(b23, make_float2(y.z, y.w));
     }
     if (rg < 2) {                                    // rows 30 and 31
       const float4 x = *reinterpret_cast<const float4*>(col + (rg + 30) * RED_STRIDE);
-      a.x += x.x; a.y += x.y; a.z += x.z; a.w += x.w;
+      a01 = add2(a01, make_float2(x.x, x.y)); a23 = add2(a23, make_float2(x.z, x.w));
     }
   }
   __syncwarp();                                      // the rows may be overwritten by the next entry
-  a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w;
+  a01 = add2(a01, b01); a23 = add2(a23, b23);
+  float4 a = make_float4(a01.x, a01.y, a23.x, a23.y);
   float4 t;
   t.x = __shfl_down_sync(FULL, a.x, 10); t.y = __shfl_down_sync(FULL, a.y, 10);
   t.z = __shfl_down_sync(FULL, a.z, 10); t.w = __shfl_down_sync(FULL, a.w, 10);
@@ -311,11 +338,14 @@ __device__ __forceinline__ float4 atom_add_v4(float* dst, const float4& v) {
   return o;
 }
 
+// S4 slot body: the lane's 8 pixels as 4 pairs (row q, row 7 - q), packed binary32 operations throughout.  With the row
+// offsets t = -(3.5 - q) (.x) and +(3.5 - q) (.y), the column sums  F_p = sum_k f_k t_k^p,  G_c,p = sum_k g_c,k t_k^p  are
+// accumulated per half with the broadcast weights |t|^p and folded at the end:  F_p = hi + (-1)^p lo.
 template <int NCH>
 __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
   __shared__ float4 sm[32 * 3];
   __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
-  __shared__ float sm_l2s[32];           // per staged entry: log2(sigma), folded into the exponent of the fast exp
+  __shared__ float4 sm_ex[32];           // per staged entry: log2(sigma), P_min + P_max, P_min P_max, -
   __shared__ __align__(16) float red[32 * RED_STRIDE];
   __shared__ uint32_t q_rank[64];
   const int lane = threadIdx.x;
@@ -334,10 +364,11 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   const uint32_t* __restrict__ ckeys = vw.ckeys;
   const ushort4* __restrict__ crect = vw.crect;
   const uint2* __restrict__ cranges = vw.cranges;
-  const uint32_t* __restrict__ tile_cend = vw.tile_cend;
   const PixelBuf pix = vw.pix;
   float* __restrict__ moments = vw.moments;
   const int tile = batch.tile_order[bpos / (uint32_t)batch.n];   // heaviest tiles first (launch order)
+  const uint32_t elast = vw.tile_elast[tile];             // list position + 1 of the last entry any pixel of the tile passed
+  if (elast == 0u) { if (batch.work) continue; return; }
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -345,31 +376,37 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   const uint32_t rmask = (1u << prm.rank_bits) - 1u;
   const uint32_t lt = (1u << lane) - 1u;
 
-  float Tc[PPL], S0[PPL], S1[PPL], S2[PPL], S3[PPL], py[PPL];
-  int last[PPL];
-  int maxlast = 0;
+  // pair q: rows q (.x) and 7 - q (.y).  nS = MINUS the suffix sums, pre-scaled by sqrt(omega_ch) (see pass 2)
+  f2 Tc2[PPL / 2], py2[PPL / 2], nS[NCH][PPL / 2];
+  int last_x[PPL / 2], last_y[PPL / 2];
 #pragma unroll
-  for (int k = 0; k < PPL; ++k) {
-    last[k] = 0; Tc[k] = 1.0f;
-    py[k] = (float)(y0 + k) + 0.5f;
-    if (x < prm.W && y0 + k < prm.H) {
-      const size_t p = (size_t)(y0 + k) * prm.W + x;
-      last[k] = pix.last[p];
-      Tc[k] = pix.T[p];
+  for (int q = 0; q < PPL / 2; ++q) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int k = h ? PPL - 1 - q : q;
+      int l = 0;
+      float T = 1.0f;
+      if (x < prm.W && y0 + k < prm.H) {
+        const size_t p = (size_t)(y0 + k) * prm.W + x;
+        l = pix.last[p];
+        T = pix.T[p];
+      }
+      const float py = (float)(y0 + k) + 0.5f;
+      if (h) { last_y[q] = l; Tc2[q].y = T; py2[q].y = py; } else { last_x[q] = l; Tc2[q].x = T; py2[q].x = py; }
     }
-    // suffix sums are carried pre-scaled by sqrt(omega_ch) (see pass 2)
-    S0[k] = prm.somega[0] * prm.bg[0] * Tc[k]; S1[k] = prm.somega[1] * prm.bg[1] * Tc[k]; S2[k] = prm.somega[2] * prm.bg[2] * Tc[k]; S3[k] = 0.0f;
-    maxlast = max(maxlast, last[k]);
-  }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) maxlast = max(maxlast, __shfl_xor_sync(FULL, maxlast, o));
-  if (maxlast == 0) { if (batch.work) continue; return; }
+    for (int c = 0; c < NCH; ++c) {
+      const float b = c < 3 ? -prm.somega[c] * prm.bg[c] : 0.0f;
+      nS[c][q] = make_float2(b * Tc2[q].x, b * Tc2[q].y);
+    }
+  }
 
-  // walk the supertile list backwards from the last composited entry; the entries that pass the rect test are the
-  // tile-list entries maxlast-1, maxlast-2, ..., 0 in that order
+  // walk the supertile list backwards from the last passed entry; the entries that pass the rect test are the
+  // tile-list entries elast-1, elast-2, ..., 0 in that order
   const uint32_t cbegin = cranges[(ty >> prm.sshift) * prm.super_x + (tx >> prm.sshift)].x;
-  uint32_t pos_hi = tile_cend[tile], qn = 0;
-  int e_next = maxlast - 1;
+  uint32_t pos_hi = vw.tile_cend[tile], qn = 0;
+  int e_next = (int)elast - 1;
+  const float thr_near = 2e-5f * prm.ln_amax_over_amin;
   for (;;) {
     while (qn < 32u && pos_hi > cbegin) {
       const uint32_t span = min(32u, pos_hi - cbegin);
@@ -402,8 +439,9 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       const float4 q0 = sm[lane * 3], q1 = sm[lane * 3 + 1];
       const float cA = -2.0f * q0.z, cB = -q0.w, cC = -2.0f * q1.x;
       const float icC = 1.0f / cC;
-      sm_wh[lane] = make_float4(sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), -cB * icC, sqrtf(cC), __logf(prm.alpha_min / q1.y));
-      sm_l2s[lane] = log2f(q1.y);
+      const float Pmin = __logf(prm.alpha_min / q1.y), Pmax = Pmin + prm.ln_amax_over_amin;
+      sm_wh[lane] = make_float4(sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), -cB * icC, sqrtf(cC), Pmin);
+      sm_ex[lane] = make_float4(log2f(q1.y), Pmin + Pmax, Pmin * Pmax, 0.0f);
     }
     __syncwarp();
     for (int j = 0; j < cnt; ++j) {
@@ -412,79 +450,89 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       const float dx = sub_rn(px, s0.x);
       // pass 1 (decision path): power bit-identical to S3; alpha from the fast exp (MUFU.EX2).  The two exps agree to
       // < 1e-6 relative, so they can only disagree on a decision of R-4 (contributor or not, clamped or not) when
-      // sigma exp(power) lies within ~1e-6 (relative) of alpha_min or alpha_max, i.e. when `power` lies within ~1e-6
-      // of P_min = ln(alpha_min / sigma) or P_max = ln(alpha_max / sigma).  If any pixel of the tile comes within 2e-5
-      // of either, the whole entry is evaluated with exp_spec instead, so every decision is the one S3 took.  The test
-      // reads only `power`: the MUFU results are first needed in pass 2, where 8 independent chains hide their latency.
+      // `power` lies within ~1e-6 of P_min = ln(alpha_min / sigma) or P_max = ln(alpha_max / sigma).  If any pixel of the
+      // tile comes within 2e-5 of either -- |(power - P_min)(power - P_max)| <= 2e-5 (P_max - P_min), two packed operations
+      // -- the whole entry is evaluated with exp_spec instead, so every decision is the one S3 took.
       const float4 wh = sm_wh[j];
-      const float l2s = sm_l2s[j];
-      // |power - P_min| <= 2e-5 or |power - P_max| <= 2e-5   <=>   | |power - P_mid| - P_half | <= 2e-5 (up to a rounding
-      // of ~5e-7, far inside the 2e-5 guard band)
-      const float Phalf = 0.5f * prm.ln_amax_over_amin, Pmid = wh.w + Phalf;
-      float pw[PPL], av[PPL];
+      const float4 ex = sm_ex[j];
+      f2 pw[PPL / 2];
       bool near = false;
 #pragma unroll
-      for (int k = 0; k < PPL; ++k) {
-        const float dy = sub_rn(py[k], s0.y);
-        const float power = splat_power(s0.z, s0.w, s1.x, dx, dy);
-        const bool in = e < last[k] && power <= 0.0f && power >= s1.w;
-        // outside the footprint or behind the pixel's last contributor: power = -inf, whose exp is 0 (MUFU) or NaN
+      for (int q = 0; q < PPL / 2; ++q) {
+        const f2 dy = sub2(py2[q], bc2(s0.y));
+        const f2 power = splat_power2(s0.z, s0.w, s1.x, dx, dy);
+        const bool in_x = e < last_x[q] && power.x <= 0.0f && power.x >= s1.w;
+        const bool in_y = e < last_y[q] && power.y <= 0.0f && power.y >= s1.w;
+        // outside the footprint or at / behind the entry the pixel stopped at: power = -inf, whose exp is 0 (MUFU) or NaN
         // (exp_spec); either fails `a >= alpha_min`
-        pw[k] = in ? power : -INFINITY;
-        near |= fabsf(fabsf(pw[k] - Pmid) - Phalf) <= 2e-5f;
+        pw[q].x = in_x ? power.x : -INFINITY;
+        pw[q].y = in_y ? power.y : -INFINITY;
+        const f2 nr = fma2(pw[q], sub2(pw[q], bc2(ex.y)), bc2(ex.z));
+        near = near || fabsf(nr.x) <= thr_near || fabsf(nr.y) <= thr_near;
       }
+      f2 av[PPL / 2];
       if (__any_sync(FULL, near)) {
 #pragma unroll
-        for (int k = 0; k < PPL; ++k) av[k] = mul_rn(s1.y, exp_spec(pw[k]));
+        for (int q = 0; q < PPL / 2; ++q) av[q] = mul2(bc2(s1.y), exp_spec2(pw[q]));
       } else {
 #pragma unroll
-        for (int k = 0; k < PPL; ++k) av[k] = ex2_approx(fmaf(pw[k], 0x1.715476p+0f, l2s));      // sigma exp(power) in one FMA + MUFU
+        for (int q = 0; q < PPL / 2; ++q) {
+          const f2 arg = fma2(pw[q], bc2(0x1.715476p+0f), bc2(ex.x));        // sigma exp(power) in one FMA + MUFU
+          av[q] = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
+        }
       }
-      // pass 2 (value path): beta, suffix sums, and the sums  F_p = sum_k f_k t_k^p,  G_c,p = sum_k g_c,k t_k^p  over
-      // the lane's 8 pixels with t_k = k - 3.5 a compile-time constant (dy_k = dyc + t_k).
-      // With T_i = T_{i+1} / (1 - alpha_i) =: Tc * rc,   beta_ch = dy_ch/dalpha_i = T_i v_i - Splus_i / (1 - alpha_i)
-      // = rc * d_ch,  d_ch = Tc v_ch - Splus_ch.  The channel weight enters as sqrt(omega_ch) folded into v_ch and
-      // Splus_ch (both linear), so  sum_ch omega_ch beta_ch^2 = rc^2 sum_ch d_ch^2  and the cross moments come out
-      // scaled by sqrt(omega_ch) (S5 applies the other sqrt).
-      const float v0 = prm.somega[0] * s2.x, v1 = prm.somega[1] * s2.y, v2 = prm.somega[2] * s2.z;
-      const float v3 = NCH == 4 ? prm.somega[3] * s1.z : 0.0f;
-      float F0 = 0.f, F1 = 0.f, F2 = 0.f, F3 = 0.f, F4 = 0.f, W2 = 0.f;
-      float G[NCH][3];
+      // pass 2 (value path): with T_i = T_{i+1} / (1 - alpha_i) =: Tc * rc,
+      //   beta_ch = dy_ch/dalpha_i = T_i v_i - Splus_i / (1 - alpha_i) = rc * d_ch,  d_ch = Tc v_ch - Splus_ch.
+      // The channel weight enters as sqrt(omega_ch) folded into v_ch and Splus_ch (both linear), so
+      // sum_ch omega_ch beta_ch^2 = rc^2 sum_ch d_ch^2 and the cross moments come out scaled by sqrt(omega_ch) (S5 applies
+      // the other sqrt).
+      float v[4];
+      v[0] = prm.somega[0] * s2.x; v[1] = prm.somega[1] * s2.y; v[2] = prm.somega[2] * s2.z;
+      v[3] = NCH == 4 ? prm.somega[3] * s1.z : 0.0f;
+      f2 F0 = bc2(0.f), F1 = bc2(0.f), F2 = bc2(0.f), F3 = bc2(0.f), F4 = bc2(0.f), W2 = bc2(0.f);
+      f2 G[NCH][3];
 #pragma unroll
-      for (int c = 0; c < NCH; ++c) G[c][0] = G[c][1] = G[c][2] = 0.f;
+      for (int c = 0; c < NCH; ++c) G[c][0] = G[c][1] = G[c][2] = bc2(0.f);
       bool any = false;
 #pragma unroll
-      for (int k = 0; k < PPL; ++k) {
-        const float a = av[k];
-        const bool pass = a >= prm.alpha_min;                            // same tests as S3 -> same contributor set
-        const bool active = pass && !(a > prm.alpha_max);                // R-11: zero derivative at the 0.99 cap
-        const float alpha = pass ? fminf(a, prm.alpha_max) : 0.0f;       // alpha = 0: T_i = Tc, w = 0, nothing moves
-        const float rc = rcp_approx(1.0f - alpha);
-        const float Ti = Tc[k] * rc;
-        const float wm = alpha * Ti;
-        const float d0 = fmaf(Tc[k], v0, -S0[k]), d1 = fmaf(Tc[k], v1, -S1[k]), d2 = fmaf(Tc[k], v2, -S2[k]);
-        float d3 = 0.0f;
-        if (NCH == 4) d3 = fmaf(Tc[k], v3, -S3[k]);
-        S0[k] = fmaf(v0, wm, S0[k]); S1[k] = fmaf(v1, wm, S1[k]); S2[k] = fmaf(v2, wm, S2[k]);
-        if (NCH == 4) S3[k] = fmaf(v3, wm, S3[k]);
-        Tc[k] = Ti;
-        W2 = fmaf(wm, wm, W2);
-        float Dq = fmaf(d2, d2, fmaf(d1, d1, d0 * d0));
-        if (NCH == 4) Dq = fmaf(d3, d3, Dq);
-        const float r1 = active ? rc * alpha : 0.0f;                     // rc * alpha, zero when inactive
-        const float f = Dq * r1 * r1;                                    // (sum_ch omega beta^2) alpha^2
-        const float gw = wm * r1;                                        // beta_ch w alpha = d_ch * gw
-        const float t1 = (float)k - 3.5f, t2 = t1 * t1, t3 = t2 * t1, t4 = t2 * t2;
-        F0 += f; F1 = fmaf(f, t1, F1); F2 = fmaf(f, t2, F2); F3 = fmaf(f, t3, F3); F4 = fmaf(f, t4, F4);
-        const float dch[4] = {d0, d1, d2, d3};
-        const float gw1 = gw * t1, gw2 = gw * t2;
+      for (int q = 0; q < PPL / 2; ++q) {
+        const f2 a = av[q];
+        const bool pass_x = a.x >= prm.alpha_min, pass_y = a.y >= prm.alpha_min;     // same tests as S3 -> same contributor set
+        f2 al, aa;                              // alpha (0: nothing moves), and alpha where its derivative is not zero
+        al.x = pass_x ? fminf(a.x, prm.alpha_max) : 0.0f;
+        al.y = pass_y ? fminf(a.y, prm.alpha_max) : 0.0f;
+        aa.x = a.x > prm.alpha_max ? 0.0f : al.x;                                  // R-11: zero derivative at the 0.99 cap
+        aa.y = a.y > prm.alpha_max ? 0.0f : al.y;
+        const f2 om = sub2(bc2(1.0f), al);
+        const f2 rc = make_float2(rcp_approx(om.x), rcp_approx(om.y));
+        const f2 Ti = mul2(Tc2[q], rc);
+        const f2 wm = mul2(al, Ti);
+        f2 d[NCH];
 #pragma unroll
         for (int c = 0; c < NCH; ++c) {
-          G[c][0] = fmaf(dch[c], gw, G[c][0]); G[c][1] = fmaf(dch[c], gw1, G[c][1]); G[c][2] = fmaf(dch[c], gw2, G[c][2]);
+          d[c] = fma2(Tc2[q], bc2(v[c]), nS[c][q]);
+          nS[c][q] = fma2(bc2(-v[c]), wm, nS[c][q]);
         }
-        any = any || pass;
+        Tc2[q] = Ti;
+        W2 = fma2(wm, wm, W2);
+        f2 Dq = mul2(d[0], d[0]);
+#pragma unroll
+        for (int c = 1; c < NCH; ++c) Dq = fma2(d[c], d[c], Dq);
+        const f2 r1 = mul2(rc, aa);                                              // rc * alpha, zero when inactive
+        const f2 f = mul2(mul2(Dq, r1), r1);                                     // (sum_ch omega beta^2) alpha^2
+        const f2 gw = mul2(wm, r1);                                              // beta_ch w alpha = d_ch * gw
+        const float t1 = 3.5f - (float)q, t2 = t1 * t1, t3 = t2 * t1, t4 = t2 * t2;   // |t| of both rows of the pair
+        F0 = add2(F0, f); F1 = fma2(f, bc2(t1), F1); F2 = fma2(f, bc2(t2), F2); F3 = fma2(f, bc2(t3), F3); F4 = fma2(f, bc2(t4), F4);
+        const f2 gw1 = mul2(gw, bc2(t1)), gw2 = mul2(gw, bc2(t2));
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+          G[c][0] = fma2(d[c], gw, G[c][0]); G[c][1] = fma2(d[c], gw1, G[c][1]); G[c][2] = fma2(d[c], gw2, G[c][2]);
+        }
+        any = any || pass_x || pass_y;
       }
       if (__any_sync(FULL, any)) {
+        // fold the halves: rows q have t < 0, rows 7 - q have t > 0
+        const float F0s = F0.x + F0.y, F1s = F1.y - F1.x, F2s = F2.x + F2.y, F3s = F3.y - F3.x, F4s = F4.x + F4.y;
         // The lane's 40 moments in the WHITENED coordinates xi = L^-1 (pixel - centre): xi1 = dx / l11 is the same for
         // the lane's 8 pixels and xi2 = (dy - (l21 / l11) dx) / l22 = xc + h t_k steps with the row, so
         // Y_b = sum_k f_k xi2_k^b follows from the F_p by a binomial shift, and the monomial sums are xi1^i Y_j.
@@ -493,13 +541,13 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
         float acc[NMOM];
         const float x1 = dx * wh.x;
         const float h = wh.z, h2 = h * h;
-        const float c1 = (((py[0] + 3.5f) - s0.y) - wh.y * dx) * h, c2 = c1 * c1, c3 = c2 * c1, c4 = c2 * c2;
-        const float E1 = h * F1, E2 = h2 * F2, E3 = h2 * h * F3, E4 = h2 * h2 * F4;
-        const float Y0v = F0;
-        const float Y1v = fmaf(c1, F0, E1);
-        const float Y2v = fmaf(c2, F0, fmaf(2.0f * c1, E1, E2));
-        const float Y3v = fmaf(c3, F0, fmaf(3.0f * c2, E1, fmaf(3.0f * c1, E2, E3)));
-        const float Y4v = fmaf(c4, F0, fmaf(4.0f * c3, E1, fmaf(6.0f * c2, E2, fmaf(4.0f * c1, E3, E4))));
+        const float c1 = ((((float)y0 + 4.0f) - s0.y) - wh.y * dx) * h, c2 = c1 * c1, c3 = c2 * c1, c4 = c2 * c2;
+        const float E1 = h * F1s, E2 = h2 * F2s, E3 = h2 * h * F3s, E4 = h2 * h2 * F4s;
+        const float Y0v = F0s;
+        const float Y1v = fmaf(c1, F0s, E1);
+        const float Y2v = fmaf(c2, F0s, fmaf(2.0f * c1, E1, E2));
+        const float Y3v = fmaf(c3, F0s, fmaf(3.0f * c2, E1, fmaf(3.0f * c1, E2, E3)));
+        const float Y4v = fmaf(c4, F0s, fmaf(4.0f * c3, E1, fmaf(6.0f * c2, E2, fmaf(4.0f * c1, E3, E4))));
         const float x2 = x1 * x1, x3 = x2 * x1, x4 = x2 * x2;
         acc[0] = Y0v;
         acc[1] = x1 * Y0v;  acc[2] = Y1v;
@@ -511,20 +559,20 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
           float* xm = acc + MOM_X + 6 * c;
           if (c < NCH) {
             const int cc = c < NCH ? c : 0;
-            const float Z0 = G[cc][0], H1 = h * G[cc][1];
+            const float Z0 = G[cc][0].x + G[cc][0].y, H1 = h * (G[cc][1].y - G[cc][1].x), H2 = h2 * (G[cc][2].x + G[cc][2].y);
             const float Z1 = fmaf(c1, Z0, H1);
-            const float Z2 = fmaf(c2, Z0, fmaf(2.0f * c1, H1, h2 * G[cc][2]));
+            const float Z2 = fmaf(c2, Z0, fmaf(2.0f * c1, H1, H2));
             xm[0] = x1 * Z0; xm[1] = Z1; xm[2] = x2 * Z0; xm[3] = x1 * Z1; xm[4] = Z2; xm[5] = Z0;
           } else {
             xm[0] = xm[1] = xm[2] = xm[3] = xm[4] = xm[5] = 0.0f;
           }
         }
-        acc[MOM_W2] = W2;
+        acc[MOM_W2] = W2.x + W2.y;
         const float4 tot = reduce40(acc, red, lane);
         const uint32_t rank = q_rank[j];
         float* dst = moments + (size_t)rank * vw.mom_stride + 4 * lane;
         // no returning atomic here: a returned value would tie up a scoreboard for a full L2 round trip; the touched
-        // list is built afterwards from sum w^2 != 0 (touched_kernel)
+        // list is built afterwards from sum w^2 != 0 (launch_touched)
         if (lane < 10) red_add_v4(dst, tot);
       }
     }
@@ -533,21 +581,6 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   }
   if (!batch.work) return;
   }  // persistent loop
-}
-
-// Touched list of every view of the batch: the ranks whose sum w^2 (moment 39) is non-zero, i.e. the Gaussians with at
-// least one composited pixel.  Warp-aggregated append; the order is not specified.
-__global__ void __launch_bounds__(256) touched_kernel(const __grid_constant__ RasterBatch batch, int N) {
-  const RasterView& vw = batch.v[blockIdx.y];
-  const int r = blockIdx.x * blockDim.x + threadIdx.x;
-  const bool hit = r < N && vw.moments[(size_t)r * vw.mom_stride + MOM_W2] != 0.0f;
-  const unsigned m = __ballot_sync(FULL, hit);
-  if (m == 0u) return;
-  const int lane = threadIdx.x & 31;
-  uint32_t base = 0;
-  if (lane == 0) base = atomicAdd(&vw.counters->n_touched, (uint32_t)__popc(m));
-  base = __shfl_sync(FULL, base, 0);
-  if (hit) vw.touched[base + __popc(m & ((1u << lane) - 1u))] = (uint32_t)r;
 }
 
 static RasterParams make_params(const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg) {
@@ -570,7 +603,7 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
   RasterBatch b = batch;
   b.n_work = (uint32_t)(tg.tiles_x * tg.tiles_y * batch.n);
   unsigned blocks = b.n_work;
-  if (b.work_fwd) blocks = std::min(blocks, 148u * (full_pix ? 16u : 32u));
+  if (b.work_fwd) blocks = std::min(blocks, (unsigned)sm_count() * (full_pix ? 16u : 32u));
   const dim3 grid(blocks);
   ++g_kernel_launches;
   if (full_pix)
@@ -580,21 +613,19 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
 }
 
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
-                     cudaStream_t st, bool build_touched) {
+                     cudaStream_t st) {
   const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
   RasterBatch b = batch;
   b.n_work = (uint32_t)(tg.tiles_x * tg.tiles_y * batch.n);
   unsigned blocks = b.n_work;
-  if (b.work) blocks = std::min(blocks, 148u * NBV_BWD_MIN_BLOCKS);
+  if (b.work) blocks = std::min(blocks, (unsigned)sm_count() * NBV_BWD_MIN_BLOCKS);
   const dim3 grid(blocks);
   ++g_kernel_launches;
   if (cfg.channel_mask & NBV_CH_DEPTH)
     backward_kernel<4><<<grid, 32, 0, st>>>(b, p);
   else
     backward_kernel<3><<<grid, 32, 0, st>>>(b, p);
-  if (!build_touched) return;
-  ++g_kernel_launches;
-  touched_kernel<<<dim3((unsigned)((N + 255) / 256), (unsigned)batch.n), 256, 0, st>>>(batch, N);
+  (void)N;
 }
 
 }  // namespace nbv

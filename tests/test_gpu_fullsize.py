@@ -100,10 +100,10 @@ def test_cfg1_scoring_call_matches_the_oracle():
     scores, best = nbv.score_candidates(cand)
     np.testing.assert_allclose(scores.cpu().numpy(), res["scores"], rtol=1e-3, atol=1e-6)
     assert int(best.item()) == res["best"]
-    # the number of views in flight changes nothing but the order of float atomics
+    # the number of views in flight changes nothing but the order of S4's binary32 reductions
     nbv.set_concurrency(1)
     s1, b1 = nbv.score_candidates(cand)
-    np.testing.assert_allclose(s1.cpu().numpy(), scores.cpu().numpy(), rtol=1e-4)
+    np.testing.assert_allclose(s1.cpu().numpy(), scores.cpu().numpy(), rtol=1e-5)
     assert int(b1.item()) == int(best.item())
     _check_walk_invariants(nbv, cand[0])
 
@@ -148,16 +148,10 @@ def _full_view_check(wl, target):
     scores, best = nbv.score_candidates(cand, target_obj=target)
     np.testing.assert_allclose(scores.cpu().numpy(), res["scores"], rtol=1e-3, atol=1e-6)
     assert int(best.item()) == res["best"]
-    # Per-Gaussian terms (a debug export; the graded quantity is their sum, checked above).  A term is
-    # log det(I + U^-T H_c U^-1) with U^T U = c H_T + Lambda: where H_T is ill-conditioned (diagonal spanning 1e6 : 1e2)
-    # and H_c is small, a 1e-6 relative perturbation of the binary32 H_T block -- the block tolerance is 1e-3 -- already
-    # moves the term by ~1e-3 relative (measured: DESIGN.md section 6).  So: 1e-3 for all but at most 1 in 10^4
-    # Gaussians, and 5e-3 for every one.
+    # per-Gaussian terms: the tolerance of B: north_star, every Gaussian
     g = nbv.gaussian_gains(cand[0], target_obj=target).cpu().numpy()
     go = res["gains"][0]
-    err = np.abs(g - go) / (np.abs(go) + 1e-6 / 1e-3)
-    assert (err > 1e-3).mean() <= 1e-4, float((err > 1e-3).mean())
-    assert err.max() < 5e-3, float(err.max())
+    np.testing.assert_allclose(g, go, rtol=1e-3, atol=1e-6)
     return nbv, res, g
 
 
@@ -177,6 +171,12 @@ def test_cfg3_object_centric_full_view():
     assert (res["conf"] > 0).sum() < 0.2 * len(conf)
 
 
+def test_cfg4_full_view_blocks_and_gains():
+    """config 4 (1,000,000 Gaussians, dense small splats, RGB): H_T of one training view, every block of one candidate, its
+    per-Gaussian gains and the score, against the oracle"""
+    _full_view_check(synth.make_workload(4), -1)
+
+
 def test_cfg4_sampled_pixels_and_block_properties():
     """config 4 (1,000,000 Gaussians, dense small splats): 1,500 random pixels + 2 tiles bit-exact; block invariants"""
     wl = synth.make_workload(4)
@@ -193,10 +193,8 @@ def test_cfg4_sampled_pixels_and_block_properties():
     s4, b4 = nbv.score_candidates(cands)
     nbv.set_concurrency(1)
     s1, b1 = nbv.score_candidates(cands)
-    # float atomics: the order varies, and without training views (prior only) the rank-deficient blocks of the few
-    # Gaussians with H_kk ~ 1e7 carry binary32 noise of ~0.1 per null pivot: a score moves by up to
-    # ~2e-4 relative from run to run; the bar is the gain tolerance of B: north_star
-    np.testing.assert_allclose(s4.cpu().numpy(), s1.cpu().numpy(), rtol=1e-3)
+    # the order of S4's binary32 reductions is all that varies with the number of views in flight
+    np.testing.assert_allclose(s4.cpu().numpy(), s1.cpu().numpy(), rtol=1e-5)
     assert int(b4.item()) == int(b1.item())
 
 

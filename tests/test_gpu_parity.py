@@ -163,7 +163,8 @@ def test_reset_training_and_repeatability(wl):
     assert float(nbv.training_hessian().abs().sum()) == 0.0
     nbv.accumulate_training(wl.train_cams)
     s2, b2 = nbv.score_candidates(wl.cand_cams)
-    np.testing.assert_allclose(s2.cpu().numpy(), s1, rtol=1e-5)  # float atomics: order varies, values agree
+    # H_T is added up view by view and a score block by block in a fixed order; only the binary32 reductions of S4 vary
+    np.testing.assert_allclose(s2.cpu().numpy(), s1, rtol=2e-6)
     assert int(b1.item()) == int(b2.item())
 
 
@@ -288,3 +289,68 @@ def test_weight_modes_match_the_oracle(wl, mode):
     order, sc = nbv.select_greedy(wl.cand_cams, 1)
     np.testing.assert_allclose(sc.cpu().numpy()[0], ref["scores"], rtol=1e-3, atol=1e-6)
     assert order[0] == ref["best"]
+
+
+# ------------------------------------------------------------------ the product's own chain rule, its own prior
+def test_chain_rule_against_finite_differences_of_the_librarys_own_projection(wl):
+    """nbv_chain (S5's d(mx,my,a,b,c,z)/d(mu,logscale,quat), derived from the factor U of Sigma2D = U U^T + blur I) against
+    central differences of nbv_projected -- the library's own binary32 forward projection, not the oracle."""
+    sub = wl.scene.subset(np.arange(400))
+    cam = wl.cand_cams[1]
+    nbv = _nbv(sub)
+    G = nbv.chain(cam).cpu().numpy().astype(np.float64)
+    vis0, rec0, _ = [t.cpu().numpy() for t in nbv.projected(cam)]
+    cols = [("mean", 0), ("mean", 1), ("mean", 2), ("logscale", 0), ("logscale", 1), ("logscale", 2),
+            ("quat", 0), ("quat", 1), ("quat", 2), ("quat", 3)]
+    steps = dict(mean=2e-3, logscale=1e-2, quat=1e-2)
+    out_idx = [0, 1, 6, 7, 8]                       # mx, my, a, b, c in the nbv_projected record
+    FD = np.zeros((sub.N, 5, 10))
+    FDz = np.zeros((sub.N, 3))
+    ok = vis0.astype(bool).copy()
+    for k, (name, j) in enumerate(cols):
+        h = steps[name]
+        recs = []
+        for sgn in (+1, -1):
+            pert = sub.subset(np.arange(sub.N))
+            getattr(pert, name)[:, j] += np.float32(sgn * h)
+            n2 = _nbv(pert)
+            v, r, _ = [t.cpu().numpy() for t in n2.projected(cam)]
+            ok &= v.astype(bool)
+            recs.append((r.astype(np.float64), getattr(pert, name)[:, j].astype(np.float64)))
+        dx = recs[0][1] - recs[1][1]               # the step actually taken in binary32
+        FD[:, :, k] = (recs[0][0][:, out_idx] - recs[1][0][:, out_idx]) / dx[:, None]
+        if name == "mean":
+            FDz[:, j] = (recs[0][0][:, 5] - recs[1][0][:, 5]) / dx
+    assert ok.sum() > 300
+    Gm, dz = G[:, :50].reshape(-1, 5, 10), G[:, 50:]
+    # scale of a row of the 5 x 10 matrix per parameter group; binary32 outputs differenced over a finite step: 1%
+    for grp in (slice(0, 3), slice(3, 6), slice(6, 10)):
+        ref = FD[ok][:, :, grp]
+        scale = np.abs(ref).max(axis=2, keepdims=True) + 1e-9 * np.abs(ref).max()
+        err = np.abs(Gm[ok][:, :, grp] - ref) / scale
+        # centre rows do not depend on scale / rotation: exactly zero on both sides there
+        assert np.nanmax(np.where(np.abs(ref).max(axis=2, keepdims=True) > 0, err, 0)) < 2e-2, grp
+    np.testing.assert_allclose(dz[ok], FDz[ok], atol=2e-3)
+    assert np.all(Gm[:, 0:2, 3:] == 0)            # the centre does not move with scale or rotation
+    # the raw quaternion enters through q / |q|: no first-order change along q itself (R-10)
+    q = sub.quat.astype(np.float64)
+    radial = np.einsum("nek,nk->ne", Gm[:, :, 6:10], q)
+    assert np.abs(radial[ok]).max() <= 1e-5 * np.abs(Gm[ok][:, :, 6:10]).max()
+
+
+@pytest.mark.parametrize("prior", ["1e-2", "1e-4", "nonuniform"])
+def test_prior_precisions_other_than_one(wl, prior):
+    """Lambda is an API parameter (R-13).  S5/S6 run in binary64, so small and non-uniform priors hold the same tolerances:
+    scores, per-Gaussian gains and the arg-max against the oracle."""
+    lam = {"1e-2": np.full(14, 1e-2), "1e-4": np.full(14, 1e-4),
+           "nonuniform": np.array([1e4, 1e4, 1e4, 1.0, 1.0, 1.0, 0.5, 0.5, 0.5, 0.5, 1e-2, 3.0, 3.0, 3.0])}[prior]
+    scn = make_oracle_scene(wl.scene, channel_mask=15)
+    nbv = _nbv(wl.scene, channel_mask=15, prior_precision=lam)
+    train = np.concatenate([wl.train_cams, wl.cand_cams[3:4]])
+    nbv.accumulate_training(train)
+    ref = orc.score_candidates(scn, train, wl.cand_cams, prior=lam)
+    s, best = nbv.score_candidates(wl.cand_cams)
+    np.testing.assert_allclose(s.cpu().numpy(), ref["scores"], rtol=1e-3, atol=1e-6)
+    assert int(best.item()) == ref["best"]
+    g = nbv.gaussian_gains(wl.cand_cams[2]).cpu().numpy()
+    np.testing.assert_allclose(g, ref["gains"][2], rtol=1e-3, atol=1e-6)
