@@ -69,10 +69,23 @@ def run_config(cfg: int, work: Path, progress: Path, deadline: float) -> bool:
     if ht_file.exists():
         H_T = np.load(ht_file)
     else:
+        # H_T = sum over the training views (Eq. 6), in view order; checkpointed every few views (a time-limited job may stop)
+        part_file, part_meta = work / (tag + "_HT_partial.npy"), work / (tag + "_HT_partial.json")
+        done = 0
         H_T = np.zeros((s.N, orc.NB))
-        for i, cam in enumerate(wl.train_cams):
-            scn.view_hessian(cam, out=H_T)
+        if part_file.exists() and part_meta.exists():
+            meta = json.loads(part_meta.read_text())
+            if meta.get("input_sha256") == input_checksum(wl) and meta.get("hashes") == oracle_hashes():
+                H_T, done = np.load(part_file), int(meta["views_done"])
+        for i in range(done, T):
+            if time.time() > deadline:
+                print("%s: time budget used, %d/%d training views done" % (tag, i, T), flush=True)
+                return False
+            scn.view_hessian(wl.train_cams[i], out=H_T)
             print("%s training view %d/%d  %.0f s" % (tag, i + 1, T, time.time() - t0), flush=True)
+            if (i + 1) % 4 == 0 and i + 1 < T:
+                np.save(part_file, H_T)
+                part_meta.write_text(json.dumps(dict(views_done=i + 1, input_sha256=input_checksum(wl), hashes=oracle_hashes())))
         np.save(ht_file, H_T)
     prog = json.loads(prog_file.read_text()) if prog_file.exists() else dict(scores={}, touched={})
     if prog.get("input_sha256", input_checksum(wl)) != input_checksum(wl) or prog.get("hashes", oracle_hashes()) != oracle_hashes():
