@@ -4,8 +4,8 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
 
 A STEP is one pass of the whole hot path over one batch: nbv_score_candidates() on the C candidate cameras of
-the workload (S0' confidence + factorisation, then S1..S6 per view, S7 arg-max), against the training Hessian
-accumulated (untimed set-up) from the workload's training cameras.  The default workload is BASELINE.json
+the workload (S0' confidence, then S1..S6 per view -- S6 factors c_g H_T,g + Lambda itself, nothing is cached between
+calls -- and S7 arg-max), against the training Hessian accumulated (untimed set-up) from the workload's training cameras.  The default workload is BASELINE.json
 configs[2] (200,000 Gaussians, 20 objects, 1280x720, 20 training + 64 candidate cameras, RGB + depth): the
 configuration north_star quotes its roofline target on.  Inputs are seeded and synthetic (paper_2602_08266_b200.synth).
 
@@ -36,18 +36,21 @@ import numpy as np
 
 METRIC = "candidate views scored/sec (Hessian + info gain)"
 UNIT = "views/s"
-SM_COUNT_B200 = 148
 FP32_LANES_PER_SM = 128
 
-# Algorithmic work per unit (FMA = 2 flop).
-FLOP_TEST = 11            # (pixel, list entry) evaluated: dx, dy, power, two range tests
-FLOP_FWD_PAIR = 31        # composited pair, S3: exp, alpha, T update, 4 blended channels
-FLOP_BWD_PAIR = {3: 134, 4: 154}   # composited pair, S4: exp, beta, 34 / 40 moment updates
+# EXECUTED binary32 work per unit, from hardware counters (FMA = 2 flop, a packed FFMA2 = 4):
+#   flop = 2 ffma + 4 ffma2 + fmul + 2 fmul2 + fadd + 2 fadd2   (smsp__sass_thread_inst_executed_op_*_pred_on.sum)
+# of one launch of each raster kernel, divided by the (pixel, list entry) evaluations of that launch (walked entries x 256).
+# Both slot bodies are branch-free, so the executed work is proportional to the evaluations, composited or not; S4's
+# per-entry moment assembly and reduction are amortised into its figure.  Source: FLOP_SOURCE (committed ncu pass).
+FLOP_PER_EVAL = {"forward": 40.6, "backward": {3: 118.0, 4: 131.0}}
+FLOP_SOURCE = "profiles/r2_ncu_flops_cfg2.md"
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
 VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (16 for images of fewer than 2,000 tiles)
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture
-# (profiles/r1c_ncu_raster_cfg2.md); known for config 2 only
-NCU_TRAFFIC_BYTES = {2: {"backward": 98.9e6, "forward": 40.8e6}}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture named
+# in TRAFFIC_SOURCE; known for config 2 only (null elsewhere)
+NCU_TRAFFIC_BYTES = {}
+TRAFFIC_SOURCE = None
 
 
 def parse_args():
@@ -133,26 +136,37 @@ def oracle_score_views(orc, scn, wl, H_T, cams):
     return time.perf_counter() - t0
 
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def cpu_baseline(wl, n_views: int):
     orc, scn = oracle_setup(wl)
     # H_T of ONE training view (untimed): scoring cost does not depend on how many views H_T sums
     H_T = np.zeros((scn.N, orc.NB))
     scn.view_hessian(wl.train_cams[0], out=H_T)
     dt = oracle_score_views(orc, scn, wl, H_T, wl.cand_cams[:n_views])
-    return {"value": n_views / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+    return {"value": n_views / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "cpu": cpu_model(),
             "sample": "first %d candidate view(s) of the workload scored against H_T of its first training view "
                       "(%.1f s wall, OpenMP over pixels)" % (n_views, dt)}
 
 
 def auto_sample_views(cfg_index: int) -> int:
-    return {0: 4, 1: 2, 2: 1, 3: 1, 4: 1}[cfg_index]
+    return 4          # at least 4 views (about 40 s of host time at config 2)
 
 
 def run_reference(args, wl, rank: int):
     """--impl reference: the oracle, each step a bounded sample (n candidate views) of the workload."""
     if rank != 0:
         return
-    n = args.cpu_sample_views or auto_sample_views(args.config)
+    # every step scores n candidate views; n = 1 at the large configs so that W + K steps end within a few minutes
+    n = args.cpu_sample_views or {0: 4, 1: 2}.get(args.config, 1)
     orc, scn = oracle_setup(wl)
     H_T = np.zeros((scn.N, orc.NB))
     scn.view_hessian(wl.train_cams[0], out=H_T)
@@ -167,20 +181,24 @@ def run_reference(args, wl, rank: int):
     sample = "each step = %d candidate view(s) of the workload scored by the oracle against H_T of one training view" % n
     out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(args, wl, "host"),
-           "cpu_baseline": {"value": v, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_config(args, wl, "host", candidates_per_step=n, training_views=1),
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "cpu": cpu_model(), "sample": sample},
            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(out), flush=True)
 
 
-def workload_config(args, wl, where: str):
+def workload_config(args, wl, where: str, candidates_per_step=None, training_views=None):
+    """what this arm ran: the reference arm scores a bounded sample per step (candidates_per_step, training_views given)"""
     s = wl.scene
     return {"workload": "BASELINE.json configs[%d] (%s)" % (args.config, wl.name), "gaussians": s.N, "objects": s.K,
             "image": "%dx%d" % (int(wl.cand_cams[0]["width"]), int(wl.cand_cams[0]["height"])),
-            "training_views": int(len(wl.train_cams)), "candidates_per_step": int(len(wl.cand_cams)),
+            "training_views": int(len(wl.train_cams) if training_views is None else training_views),
+            "candidates_per_step": int(len(wl.cand_cams) if candidates_per_step is None else candidates_per_step),
+            "workload_training_views": int(len(wl.train_cams)), "workload_candidates": int(len(wl.cand_cams)),
             "channels": "rgb+depth" if wl.channel_mask == 15 else "rgb", "target_obj": int(wl.target_obj), "P": 14,
             "seed": int(wl.seed), "parallelism": "replicas x%d" % args.gpus,
-            "l2": "flushed between steps (512 MiB write); per-view working set (keys, H_T, factors) exceeds the 126 MB L2"
+            "l2": "flushed between steps (512 MiB write); per-batch working set (keys, splats, H_T) exceeds the 126 MB L2"
                   if where == "device" else "n/a"}
 
 
@@ -311,6 +329,9 @@ def main():
     torch.cuda.synchronize()
     load_s = time.perf_counter() - t0
     ev = lambda: torch.cuda.Event(enable_timing=True)
+    nbv.accumulate_training(wl.train_cams)              # untimed: creates the slots' work buffers
+    nbv.reset_training()
+    torch.cuda.synchronize()
     e0, e1 = ev(), ev()
     e0.record()
     nbv.accumulate_training(wl.train_cams)
@@ -394,11 +415,12 @@ def main():
     views = max(n_timed_views, 1)
     per_view_ms = {k: v / views for k, v in stage_ms.items()}
     avg = {k: v / C for k, v in tot.items()}            # per view
-    tests = avg["n_entries"] * 256.0
-    alu_peak = SM_COUNT_B200 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12    # TFLOP/s
+    evals = avg["n_entries"] * 256.0                    # (pixel, list entry) evaluations per view
+    n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    alu_peak = n_sm * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12    # TFLOP/s
     work = {
-        "backward": ("alu", (tests * FLOP_TEST + avg["n_pairs"] * FLOP_BWD_PAIR[nch]) / 1e12, alu_peak, "TFLOP/s"),
-        "forward": ("alu", (tests * FLOP_TEST + avg["n_pairs"] * FLOP_FWD_PAIR) / 1e12, alu_peak, "TFLOP/s"),
+        "backward": ("alu", evals * FLOP_PER_EVAL["backward"][nch] / 1e12, alu_peak, "TFLOP/s"),
+        "forward": ("alu", evals * FLOP_PER_EVAL["forward"] / 1e12, alu_peak, "TFLOP/s"),
         "coarse_sort": ("hbm", avg["n_coarse"] * BYTES_PER_KEY / 1e9, peaks["hbm_gbs"], "GB/s"),
     }
     rl = {}
@@ -411,9 +433,11 @@ def main():
         vpl = min(vpl, C)
         rl[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
                  "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(k),
+                 "traffic_source": TRAFFIC_SOURCE if NCU_TRAFFIC_BYTES.get(args.config, {}).get(k) else None,
+                 "flops_source": ("executed fp32 flop per evaluation from " + FLOP_SOURCE) if batched else None,
                  "views_per_launch": vpl if batched else 1,
                  "ms_per_launch": per_view_ms[k] * (vpl if batched else 1), "peak_source": peaks["source"] if bound == "hbm" else
-                 "148 SM x 128 lanes x 2 x %.0f MHz (DESIGN.md section 8)" % peaks["sm_max_mhz"]}
+                 "%d SM x 128 lanes x 2 x %.0f MHz (DESIGN.md section 8)" % (n_sm, peaks["sm_max_mhz"])}
     # dominant kernel = largest share of GPU time in the ncu launch list (profiles/): one of the two raster stages; the
     # S1-S2 stage times are taken on slot streams that wait behind the raster launches and are not exclusive
     dominant = max(("backward", "forward"), key=lambda k: per_view_ms[k])
@@ -428,7 +452,8 @@ def main():
     out = {
         "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": agg["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic", "config": workload_config(args, wl, "device"),
+        "dtype": "f32", "dtype_note": "S1-S4 binary32 (S4's 40 moments per Gaussian), S5-S6 binary64 (1-2% of a view)",
+        "data": "synthetic", "config": workload_config(args, wl, "device"),
         "clocks": clocks,
         "e2e": {"value": agg_e2e["value"], "unit": UNIT, "h2d_bytes_per_step": int(72 * C), "d2h_bytes_per_step": int(4 * C + 4),
                 "call": "nbv_score_candidates_host (host camera structs in, host scores + best out, stream synchronised)"},
@@ -437,7 +462,7 @@ def main():
         "stage_ms_per_view": per_view_ms,
         "stage_rooflines": rl,
         "view_roofline": {"t_min_ms": t_min_ms, "t_measured_ms": view_ms, "frac": t_min_ms / view_ms if view_ms else None,
-                          "note": "sum over stages of (algorithmic work / peak) against wall time per view"},
+                          "note": "sum over stages of (executed fp32 work or algorithmic bytes / peak) against wall time per view"},
         "counts_per_view": avg,
         "setup": {"load_s": load_s, "training_views_per_s": len(wl.train_cams) / (train_ms * 1e-3) if train_ms else None},
         "best": int(h_best),

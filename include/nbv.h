@@ -45,6 +45,10 @@ extern "C" {
 #define NBV_CH_RGBD 15
 #define NBV_CH_MASK 16    /* the object-mask output (Eq. 1-2): a context of its own, blocks of 11 + K parameters */
 #define NBV_MASK_KMAX 52  /* largest number of object channels a mask context supports */
+#define NBV_SH_L 59       /* parameters per block after nbv_load_sh: 11 + 3 * 16 */
+#define NBV_CRIT_LOGDET 0
+#define NBV_CRIT_TRACE 1
+#define NBV_CRIT_DET 2
 
 typedef enum nbv_status {
   NBV_OK = 0,
@@ -90,6 +94,15 @@ typedef struct nbv_config {
    * 2 (R3) "scale each Jacobian ... during information gain computation", candidate only:
    *        IG_g = logdet(H_T + c H_c + L) - logdet(H_T + L).      c_g = 0 gives exactly 0 in all three. */
   int32_t weight_mode;
+  /* the function f of Eq. 5, IG(T,c) = f(T u c) - f(T), on the block-diagonal H (P:L199 names the alternatives; R-17):
+   * 0 (default, the paper's choice) f = log det H:  score = sum_g [logdet(c (H_T + H_c) + L) - logdet(c H_T + L)]   (Eq. 6)
+   * 1 trace-based, f = 1 / trace(H^-1):  score = 1 / (S_T - D_c) - 1 / S_T with S_T = sum over ALL Gaussians of
+   *        trace((c_g H_T,g + L)^-1) and D_c = the reduction of that sum by the candidate (weight_mode 0, colour / depth
+   *        contexts only).  nbv_gaussian_gains then exports the per-Gaussian reductions D_g.
+   * 2 determinant, f = det H: det(H_T) is a product over all Gaussians and leaves binary64 range for any real map, so
+   *        the score is carried in the log domain, log(det(H_{T u c}) / det(H_T)) -- the same numbers as criterion 0,
+   *        ordering the candidates exactly as the literal difference does. */
+  int32_t criterion;
 } nbv_config;
 
 typedef struct nbv_ctx nbv_ctx;
@@ -131,6 +144,16 @@ int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight);
 int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, const float* d_logscale,
                        const float* d_quat, const float* d_opacity, const float* d_rgb,
                        const float* d_obj_logits, void* stream);
+
+/* View-dependent colour, SH degree 3 ("SH coefficients c in R^{3(d+1)^2}"; R-18):
+ *   colour_ch(dir) = rgb_ch + sum_{j=1}^{15} B_j(dir) k_{j,ch},  dir = (mu - o) / |mu - o|, o = camera centre,
+ * B_j the real spherical harmonics of degree 1..3 in the ordering and signs of the 3DGS pipeline, no clamp.
+ * d_sh: N x 45 floats, coefficient-major (k_1 rgb, k_2 rgb, ..., k_15 rgb), copied.  From this call on the context works on
+ * blocks of NBV_SH_L = 59 parameters [mu logscale quat opacity | rgb | k_1 .. k_15] (nbv_block_size() = 1770; the prior of
+ * a coefficient is prior_precision[11 + channel]); H_T is reset.  S1 evaluates the colours per view, S3 / S4 are unchanged,
+ * S5 / S6 run on 59 x 59 blocks in binary64.  Colour / depth contexts with weight_mode 0 and the log-det criterion only;
+ * nbv_select_greedy re-rasterises every round in this mode.  Errors: NOT_LOADED, INVALID_ARG, OOM, CUDA. */
+int nbv_load_sh(nbv_ctx* ctx, const float* d_sh, void* stream);
 
 /* H_T <- 0, |T| <- 0. */
 int nbv_reset_training(nbv_ctx* ctx, void* stream);
@@ -191,7 +214,7 @@ int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, nbv_ctx* ct
 int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t rounds, int32_t target_obj,
                       int32_t* h_order, float* d_scores, void* stream);
 
-/* Number of floats of one packed block in this context: 105 for colour/depth contexts; L (L + 1) / 2 with L = 11 + K
+/* Number of floats of one packed block in this context: 105 for colour/depth contexts (1770 after nbv_load_sh); L (L + 1) / 2 with L = 11 + K
  * for a loaded mask context (parameter order [mu(3) logscale(3) quat(4) opacity | object logits (K)], upper triangle
  * row-major, idx(r,c) = r L - r (r - 1) / 2 + (c - r)).  nbv_view_hessian / nbv_training_hessian use this size.
  * Returns 0 for a mask context before nbv_load_gaussians. */

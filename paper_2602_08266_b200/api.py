@@ -36,7 +36,7 @@ EXPORTS = [
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
     "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
     "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy", "nbv_block_size", "nbv_render_mask", "nbv_measure_ffma_peak",
-    "nbv_chain",
+    "nbv_chain", "nbv_load_sh",
 ]
 
 STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
@@ -56,7 +56,7 @@ class Config(C.Structure):
         ("t_stop", C.c_float), ("bg", C.c_float * 3), ("channel_mask", C.c_int32), ("channel_weight", C.c_float * 4),
         ("opacity_coord", C.c_int32), ("alpha_obj", C.c_float), ("alpha_opa", C.c_float), ("p_floor", C.c_float),
         ("sigma_floor", C.c_float), ("prior_precision", C.c_float * 14), ("mask_bg_channel", C.c_int32),
-        ("prior_precision_obj", C.c_float), ("weight_mode", C.c_int32),
+        ("prior_precision_obj", C.c_float), ("weight_mode", C.c_int32), ("criterion", C.c_int32),
     ]
 
 
@@ -178,6 +178,12 @@ class NBV:
 
     def load_scene(self, scene):
         self.load_gaussians(scene.mean, scene.logscale, scene.quat, scene.opacity, scene.rgb, scene.obj_logits)
+
+    def load_sh(self, sh45):
+        """nbv_load_sh: (N, 45) float32 SH coefficients of degree 1..3 (coefficient-major); blocks become 59 x 59"""
+        torch = self._torch
+        t = torch.as_tensor(np.ascontiguousarray(sh45, dtype=np.float32).reshape(self.N, 45), device=self.device).contiguous()
+        self._check(self.lib.nbv_load_sh(self._h, _ptr(t), _stream()))
 
     def reset_training(self):
         self._check(self.lib.nbv_reset_training(self._h, _stream()))

@@ -49,11 +49,16 @@ __device__ __forceinline__ unsigned long long super_mask64(uint4 sr, int super_x
 constexpr int MS_T = 1024;
 constexpr int MS_W = MS_T / 32;
 
-__global__ void __launch_bounds__(MS_T) msplit_count_kernel(const uint32_t* __restrict__ ids_sorted, const Splat* __restrict__ splat,
-                                                            const ushort4* __restrict__ rect, int N, int sshift, int super_x, int n_super,
-                                                            Splat* __restrict__ splat_sorted, ushort4* __restrict__ rect_sorted,
-                                                            uint32_t* __restrict__ counts, uint32_t nblk) {
+__global__ void __launch_bounds__(MS_T) msplit_count_kernel(const __grid_constant__ PreBatch batch, int N, int sshift, int super_x,
+                                                            int n_super, uint32_t nblk) {
   __shared__ uint32_t cnt[256];
+  const PreView& pv = batch.v[blockIdx.y];
+  const uint32_t* __restrict__ ids_sorted = pv.ids[0];
+  const Splat* __restrict__ splat = pv.splat;
+  const ushort4* __restrict__ rect = pv.rect;
+  Splat* __restrict__ splat_sorted = pv.splat_sorted;
+  ushort4* __restrict__ rect_sorted = pv.rect_sorted;
+  uint32_t* __restrict__ counts = pv.counts;
   const int r = blockIdx.x * MS_T + threadIdx.x, lane = threadIdx.x & 31;
   if (threadIdx.x < 256) cnt[threadIdx.x] = 0;
   __syncthreads();
@@ -86,11 +91,15 @@ __global__ void __launch_bounds__(MS_T) msplit_count_kernel(const uint32_t* __re
   if ((int)threadIdx.x < n_super) counts[(size_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
 }
 
-__global__ void __launch_bounds__(MS_T) msplit_write_kernel(const ushort4* __restrict__ rect_sorted, int N, int sshift, int super_x,
-                                                            int n_super, int rank_bits, const uint32_t* __restrict__ scanned, uint32_t nblk,
-                                                            const uint32_t* __restrict__ d_total, uint32_t cap,
-                                                            uint32_t* __restrict__ keys, ushort4* __restrict__ crect,
-                                                            uint2* __restrict__ ranges) {
+__global__ void __launch_bounds__(MS_T) msplit_write_kernel(const __grid_constant__ PreBatch batch, int N, int sshift, int super_x,
+                                                            int n_super, int rank_bits, uint32_t nblk, uint32_t cap) {
+  const PreView& pv = batch.v[blockIdx.y];
+  const ushort4* __restrict__ rect_sorted = pv.rect_sorted;
+  const uint32_t* __restrict__ scanned = pv.counts;
+  const uint32_t* __restrict__ d_total = &pv.counters->n_coarse;
+  uint32_t* __restrict__ keys = pv.ckeys;
+  ushort4* __restrict__ crect = pv.crect;
+  uint2* __restrict__ ranges = pv.cranges;
   __shared__ uint16_t wc[256][MS_W];         // per supertile: ranks of warp w touching it, then the exclusive prefix over warps
   __shared__ uint32_t seg[256];              // start of this block's segment in every supertile list (one global load each,
                                              // up front: a load inside the write loop would stall every iteration on the L2)
@@ -138,20 +147,17 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const ushort4* __res
 
 uint32_t msplit_blocks(int N) { return (uint32_t)((N + MS_T - 1) / MS_T); }
 
-void launch_msplit_count(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, const TileGrid& tg, Splat* splat_sorted,
-                         ushort4* rect_sorted, uint32_t* counts, cudaStream_t st) {
+void launch_msplit_count(const PreBatch& batch, int N, const TileGrid& tg, cudaStream_t st) {
   const uint32_t nblk = msplit_blocks(N);
   ++g_kernel_launches;
-  msplit_count_kernel<<<nblk, MS_T, 0, st>>>(ids_sorted, splat, rect, N, tg.sshift, tg.super_x, tg.super_x * tg.super_y, splat_sorted,
-                                             rect_sorted, counts, nblk);
+  msplit_count_kernel<<<dim3(nblk, (unsigned)batch.n), MS_T, 0, st>>>(batch, N, tg.sshift, tg.super_x, tg.super_x * tg.super_y, nblk);
 }
 
-void launch_msplit_write(const ushort4* rect_sorted, int N, const TileGrid& tg, int rank_bits, const uint32_t* scanned,
-                         const uint32_t* d_total, uint32_t cap, uint32_t* keys, ushort4* crect, uint2* ranges, cudaStream_t st) {
+void launch_msplit_write(const PreBatch& batch, int N, const TileGrid& tg, int rank_bits, uint32_t cap, cudaStream_t st) {
   const uint32_t nblk = msplit_blocks(N);
   ++g_kernel_launches;
-  msplit_write_kernel<<<nblk, MS_T, 0, st>>>(rect_sorted, N, tg.sshift, tg.super_x, tg.super_x * tg.super_y, rank_bits, scanned, nblk,
-                                             d_total, cap, keys, crect, ranges);
+  msplit_write_kernel<<<dim3(nblk, (unsigned)batch.n), MS_T, 0, st>>>(batch, N, tg.sshift, tg.super_x, tg.super_x * tg.super_y, rank_bits, nblk,
+                                                                      cap);
 }
 
 // ---- parity export: the full tile lists (R-5), by the same rect test the rasteriser applies on the fly.

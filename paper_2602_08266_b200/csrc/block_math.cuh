@@ -26,89 +26,108 @@ struct Chain {
 template <class T>
 __device__ __forceinline__ T dot3(const T* a, const T* b) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
 
+// what every column of the chain needs (computed once per (view, Gaussian))
 template <class T>
-__device__ void projection_chain(const nbv_camera& cam, const float* mu_f, const float* ls_f, const float* q_f, Chain<T>& ch) {
-  T W[9];
+struct ChainPrefix {
+  T W[9], t0[3], t1[3], u0[3], u1[3], v2[3], s[3], qh[4], in;    // in = 1 / |q|
+  T ax, cx, ay, cy, iz;
+  T u0v2, u1v2, u0u0, u0u1, u1u1;
+};
+
+template <class T>
+__device__ void chain_prefix(const nbv_camera& cam, const float* mu_f, const float* ls_f, const float* q_f, ChainPrefix<T>& p) {
 #pragma unroll
-  for (int i = 0; i < 9; ++i) W[i] = (T)cam.R_cw[i];
+  for (int i = 0; i < 9; ++i) p.W[i] = (T)cam.R_cw[i];
+  const T* W = p.W;
   const T fx = (T)cam.fx, fy = (T)cam.fy;
   const T mu[3] = {(T)mu_f[0], (T)mu_f[1], (T)mu_f[2]};
   const T x = W[0] * mu[0] + W[1] * mu[1] + W[2] * mu[2] + (T)cam.t_cw[0];
   const T y = W[3] * mu[0] + W[4] * mu[1] + W[5] * mu[2] + (T)cam.t_cw[1];
   const T z = W[6] * mu[0] + W[7] * mu[1] + W[8] * mu[2] + (T)cam.t_cw[2];
   const T iz = (T)1 / z, xz = x * iz, yz = y * iz, gx = fx * iz, gy = fy * iz;
-  T s[3];
 #pragma unroll
-  for (int k = 0; k < 3; ++k) s[k] = exp(fmin(fmax((T)ls_f[k], (T)-80), (T)80));
+  for (int k = 0; k < 3; ++k) p.s[k] = exp(fmin(fmax((T)ls_f[k], (T)-80), (T)80));
   const T qr[4] = {(T)q_f[0], (T)q_f[1], (T)q_f[2], (T)q_f[3]};
   const T in = rsqrt(qr[0] * qr[0] + qr[1] * qr[1] + qr[2] * qr[2] + qr[3] * qr[3]);
   const T w = qr[0] * in, i = qr[1] * in, j = qr[2] * in, k = qr[3] * in;
-  const T qh[4] = {w, i, j, k};
-  // N(q_hat) = R, and D[e] = dN/dq_e at q_hat (each entry linear in q_hat)
+  p.qh[0] = w; p.qh[1] = i; p.qh[2] = j; p.qh[3] = k; p.in = in;
+  // N(q_hat) = R
   const T R[9] = {w * w + i * i - j * j - k * k, 2 * (i * j - w * k), 2 * (i * k + w * j),
                   2 * (i * j + w * k), w * w - i * i + j * j - k * k, 2 * (j * k - w * i),
                   2 * (i * k - w * j), 2 * (j * k + w * i), w * w - i * i - j * j + k * k};
-  const T D[4][9] = {{w, -k, j, k, w, -i, -j, i, w},
-                     {i, j, k, j, -i, -w, k, w, -i},
-                     {-j, i, w, i, j, k, -w, k, -j},
-                     {-k, -w, i, w, -k, j, i, j, k}};      // each to be doubled (applied below)
   // Jp W: the 2 x 3 map from world displacements to pixel displacements
-  T t0[3], t1[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    t0[c] = gx * (W[c] - xz * W[6 + c]);
-    t1[c] = gy * (W[3 + c] - yz * W[6 + c]);
+    p.t0[c] = gx * (W[c] - xz * W[6 + c]);
+    p.t1[c] = gy * (W[3 + c] - yz * W[6 + c]);
   }
   // rows of U = (Jp W) R diag(s), and v2 = row 2 of V = W R diag(s)
-  T u0[3], u1[3], v2[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    u0[c] = (t0[0] * R[c] + t0[1] * R[3 + c] + t0[2] * R[6 + c]) * s[c];
-    u1[c] = (t1[0] * R[c] + t1[1] * R[3 + c] + t1[2] * R[6 + c]) * s[c];
-    v2[c] = (W[6] * R[c] + W[7] * R[3 + c] + W[8] * R[6 + c]) * s[c];
+    p.u0[c] = (p.t0[0] * R[c] + p.t0[1] * R[3 + c] + p.t0[2] * R[6 + c]) * p.s[c];
+    p.u1[c] = (p.t1[0] * R[c] + p.t1[1] * R[3 + c] + p.t1[2] * R[6 + c]) * p.s[c];
+    p.v2[c] = (W[6] * R[c] + W[7] * R[3 + c] + W[8] * R[6 + c]) * p.s[c];
   }
-  // position
-  {
-    const T u0v2 = dot3(u0, v2), u1v2 = dot3(u1, v2), u0u0 = dot3(u0, u0), u0u1 = dot3(u0, u1), u1u1 = dot3(u1, u1);
-    // du0/dx = ax v2, du0/dz = -iz u0 + cx v2;   du1/dy = ay v2, du1/dz = -iz u1 + cy v2
-    const T ax = -gx * iz, cx = gx * xz * iz, ay = -gy * iz, cy = gy * yz * iz;
-#pragma unroll
-    for (int m = 0; m < 3; ++m) {
-      const T wx = W[m], wy = W[3 + m], wz = W[6 + m];
-      // du0 = (ax wx + cx wz) v2 - iz wz u0 ;  du1 = (ay wy + cy wz) v2 - iz wz u1
-      const T e0 = ax * wx + cx * wz, e1 = ay * wy + cy * wz, f = -iz * wz;
-      ch.G[0][m] = t0[m];
-      ch.G[1][m] = t1[m];
-      ch.G[2][m] = 2 * (e0 * u0v2 + f * u0u0);
-      ch.G[3][m] = e0 * u1v2 + e1 * u0v2 + 2 * f * u0u1;
-      ch.G[4][m] = 2 * (e1 * u1v2 + f * u1u1);
-      ch.dz[m] = wz;
-    }
-  }
-  // log-scale
-#pragma unroll
-  for (int m = 0; m < 3; ++m) {
-    ch.G[0][3 + m] = 0; ch.G[1][3 + m] = 0;
-    ch.G[2][3 + m] = 2 * u0[m] * u0[m];
-    ch.G[3][3 + m] = 2 * u0[m] * u1[m];
-    ch.G[4][3 + m] = 2 * u1[m] * u1[m];
-  }
-  // rotation, through q / |q|
-#pragma unroll
-  for (int e = 0; e < 4; ++e) {
+  p.u0v2 = dot3(p.u0, p.v2); p.u1v2 = dot3(p.u1, p.v2); p.u0u0 = dot3(p.u0, p.u0); p.u0u1 = dot3(p.u0, p.u1); p.u1u1 = dot3(p.u1, p.u1);
+  // du0/dx = ax v2, du0/dz = -iz u0 + cx v2;   du1/dy = ay v2, du1/dz = -iz u1 + cy v2
+  p.ax = -gx * iz; p.cx = gx * xz * iz; p.ay = -gy * iz; p.cy = gy * yz * iz; p.iz = iz;
+}
+
+// column k of the chain: d(mx, my, a, b, c) / d(parameter k), k = 0..2 position, 3..5 log-scale, 6..9 raw quaternion
+template <class T>
+__device__ void chain_column(const ChainPrefix<T>& p, int k, T* col5) {
+  if (k < 3) {
+    const T wx = p.W[k], wy = p.W[3 + k], wz = p.W[6 + k];
+    // du0 = (ax wx + cx wz) v2 - iz wz u0 ;  du1 = (ay wy + cy wz) v2 - iz wz u1
+    const T e0 = p.ax * wx + p.cx * wz, e1 = p.ay * wy + p.cy * wz, f = -p.iz * wz;
+    col5[0] = p.t0[k];
+    col5[1] = p.t1[k];
+    col5[2] = 2 * (e0 * p.u0v2 + f * p.u0u0);
+    col5[3] = e0 * p.u1v2 + e1 * p.u0v2 + 2 * f * p.u0u1;
+    col5[4] = 2 * (e1 * p.u1v2 + f * p.u1u1);
+  } else if (k < 6) {
+    const int m = k - 3;
+    col5[0] = 0; col5[1] = 0;
+    col5[2] = 2 * p.u0[m] * p.u0[m];
+    col5[3] = 2 * p.u0[m] * p.u1[m];
+    col5[4] = 2 * p.u1[m] * p.u1[m];
+  } else {
+    const int e = k - 6;
+    const T w = p.qh[0], i = p.qh[1], j = p.qh[2], kk = p.qh[3];
+    // D = dN/dq_e at q_hat (each entry linear in q_hat), to be doubled
+    T D[9];
+    if (e == 0)      { const T d[9] = {w, -kk, j, kk, w, -i, -j, i, w};   for (int n = 0; n < 9; ++n) D[n] = d[n]; }
+    else if (e == 1) { const T d[9] = {i, j, kk, j, -i, -w, kk, w, -i};   for (int n = 0; n < 9; ++n) D[n] = d[n]; }
+    else if (e == 2) { const T d[9] = {-j, i, w, i, j, kk, -w, kk, -j};   for (int n = 0; n < 9; ++n) D[n] = d[n]; }
+    else             { const T d[9] = {-kk, -w, i, w, -kk, j, i, j, kk};  for (int n = 0; n < 9; ++n) D[n] = d[n]; }
     T d0[3], d1[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      const T p0 = 2 * (t0[0] * D[e][c] + t0[1] * D[e][3 + c] + t0[2] * D[e][6 + c]) * s[c];
-      const T p1 = 2 * (t1[0] * D[e][c] + t1[1] * D[e][3 + c] + t1[2] * D[e][6 + c]) * s[c];
-      d0[c] = (p0 - 2 * qh[e] * u0[c]) * in;
-      d1[c] = (p1 - 2 * qh[e] * u1[c]) * in;
+      const T p0 = 2 * (p.t0[0] * D[c] + p.t0[1] * D[3 + c] + p.t0[2] * D[6 + c]) * p.s[c];
+      const T p1 = 2 * (p.t1[0] * D[c] + p.t1[1] * D[3 + c] + p.t1[2] * D[6 + c]) * p.s[c];
+      d0[c] = (p0 - 2 * p.qh[e] * p.u0[c]) * p.in;
+      d1[c] = (p1 - 2 * p.qh[e] * p.u1[c]) * p.in;
     }
-    ch.G[0][6 + e] = 0; ch.G[1][6 + e] = 0;
-    ch.G[2][6 + e] = 2 * dot3(u0, d0);
-    ch.G[3][6 + e] = dot3(d0, u1) + dot3(u0, d1);
-    ch.G[4][6 + e] = 2 * dot3(u1, d1);
+    col5[0] = 0; col5[1] = 0;
+    col5[2] = 2 * dot3(p.u0, d0);
+    col5[3] = dot3(d0, p.u1) + dot3(p.u0, d1);
+    col5[4] = 2 * dot3(p.u1, d1);
   }
+}
+
+template <class T>
+__device__ void projection_chain(const nbv_camera& cam, const float* mu_f, const float* ls_f, const float* q_f, Chain<T>& ch) {
+  ChainPrefix<T> p;
+  chain_prefix<T>(cam, mu_f, ls_f, q_f, p);
+#pragma unroll
+  for (int k = 0; k < 10; ++k) {
+    T col[5];
+    chain_column<T>(p, k, col);
+#pragma unroll
+    for (int e = 0; e < 5; ++e) ch.G[e][k] = col[e];
+  }
+#pragma unroll
+  for (int m = 0; m < 3; ++m) ch.dz[m] = p.W[6 + m];
 }
 
 // S4 accumulates the moments in the monomials xi1^i xi2^j of the whitened pixel offset xi = L^-1 (p - m),
@@ -236,8 +255,35 @@ __device__ __forceinline__ void ldl_pivots(double* Mx, double* piv) {
   }
 }
 
-// every block leaves its partial in partials[blockIdx.x]; the block that finishes last adds them in block order
-__device__ __forceinline__ void ordered_score(double block_total, double* partials, unsigned int* done, float* score) {
+// trace(A^-1) of a packed symmetric positive definite 14 x 14 (destroyed): A = L D L^T, A^-1 = L^-T D^-1 L^-1, so the trace is
+// sum over the columns x = L^-1 e_c of sum_i x_i^2 / d_i
+__device__ __forceinline__ double ldl_inverse_trace(double* Mx) {
+  double piv[P];
+  ldl_pivots(Mx, piv);
+  for (int j = 0; j < P; ++j) {
+    const double inv = 1.0 / piv[j];
+    for (int i = j + 1; i < P; ++i) Mx[tri(j, i)] *= inv;          // row j now holds L_ij, i > j
+  }
+  double tr = 0.0;
+  for (int c = 0; c < P; ++c) {
+    double x[P];
+    x[c] = 1.0;
+    double acc = 1.0 / piv[c];
+    for (int i = c + 1; i < P; ++i) {
+      double sacc = 0.0;
+      for (int j = c; j < i; ++j) sacc = fma(Mx[tri(j, i)], x[j], sacc);
+      x[i] = -sacc;
+      acc = fma(sacc * sacc, 1.0 / piv[i], acc);
+    }
+    tr += acc;
+  }
+  return tr;
+}
+
+// every block leaves its partial in partials[blockIdx.x]; the block that finishes last adds them in block order.
+// trace_total != nullptr (trace criterion): the sum D_c becomes the score 1 / (S_T - D_c) - 1 / S_T.
+__device__ __forceinline__ void ordered_score(double block_total, double* partials, unsigned int* done, float* score,
+                                              const double* trace_total = nullptr, double* total_out = nullptr) {
   __shared__ bool last;
   if (threadIdx.x == 0) {
     partials[blockIdx.x] = block_total;
@@ -249,7 +295,9 @@ __device__ __forceinline__ void ordered_score(double block_total, double* partia
     __threadfence();
     double t = 0.0;
     for (unsigned b = 0; b < gridDim.x; ++b) t += __ldcg(partials + b);
-    *score = (float)t;
+    if (trace_total) { const double S = *trace_total; t = 1.0 / (S - t) - 1.0 / S; }
+    if (score) *score = (float)t;
+    if (total_out) *total_out = t;
     *done = 0u;
   }
 }

@@ -7,16 +7,41 @@ namespace nbv {
 extern unsigned long long g_kernel_launches;   // host-side count of kernel launches (nbv_kernel_launches)
 int sm_count();                                // multiprocessors of the current device (queried once per device)
 
+// One launch of every S1-S2 stage serves a BATCH of views (grid.y = view): the per-view device pointers travel as a
+// __grid_constant__ kernel parameter, like RasterBatch below.  All views of a batch share N and the image size.
+constexpr int MAX_BATCH = 16;
+struct PreView {
+  nbv_camera cam;
+  Splat* splat;              // N, indexed by Gaussian
+  uint32_t* zkey[2];         // depth keys (z bits; 0xffffffff = culled), ping-pong buffers of the radix passes
+  uint32_t* ids[2];          // Gaussian ids, ping-pong; after the sort ids[0][rank]
+  ushort4* rect;             // N tile rectangles, indexed by Gaussian
+  float* abc;                // N x 3 Sigma2D (parity export) or nullptr
+  uint32_t* hist;            // radix digit histograms (256 x radix_blocks(N)) of the current pass
+  Splat* splat_sorted;       // N, indexed by depth rank
+  ushort4* rect_sorted;
+  uint32_t* counts;          // multi-split count table (supertiles x msplit_blocks(N)), scanned in place
+  uint32_t* ckeys;           // coarse keys (supertile << rank_bits | rank)
+  ushort4* crect;            // their tile rectangles
+  uint2* cranges;            // 256 supertile ranges
+  ViewCounters* counters;
+};
+struct PreBatch {
+  int n;
+  PreView v[MAX_BATCH];
+};
+
 // ---- sort.cu
 size_t scan_temp_words(size_t n);
 void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* tmp, uint32_t* total_out, cudaStream_t st);
-size_t radix_temp_words(size_t n);
-// one stable pass over `bits` (<= 8) bits at `shift`; vals_in == nullptr -> keys only
-// n: number of keys, or (d_n != nullptr) the capacity the grids are sized for with the length read from *d_n.
-// On return tmp[digit * radix_blocks(n)] holds the start of every digit in the output.
-void radix_pass(const uint32_t* keys_in, uint32_t* keys_out, const uint32_t* vals_in, uint32_t* vals_out, size_t n,
-                const uint32_t* d_n, int shift, int bits, uint32_t* tmp, cudaStream_t st);
+// in-place exclusive scans of one table of n words per view (n <= scan_batched_max(): one cluster launch for the batch)
+enum ScanTable { SCAN_HIST = 0, SCAN_COUNTS = 1 };     // PreView::hist, or PreView::counts with the total in counters->n_coarse
+uint32_t scan_batched_max();
+void scan_batched(const PreBatch& batch, int table, size_t n, cudaStream_t st);
+// one stable pass over 8 bits at `shift` of the depth sort of every view of the batch: (zkey, ids)[src] -> [src ^ 1]
+void radix_pass_batched(const PreBatch& batch, int src, size_t n, int shift, cudaStream_t st);
 uint32_t radix_blocks(size_t n);
+size_t radix_temp_words(size_t n);      // words of PreView::hist (the table and the scratch of the long-table scan)
 
 // ---- project.cu
 struct SceneDev {            // device arrays of the loaded map
@@ -33,18 +58,15 @@ struct SceneDev {            // device arrays of the loaded map
   float* lse;                // N       log sum exp of the logits
 };
 void launch_activate(const SceneDev& sc, ViewCounters* counters, cudaStream_t st);
-void launch_project(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, Splat* splat, uint32_t* zkey,
-                    uint32_t* ids, ushort4* rect, float* abc, ViewCounters* counters, cudaStream_t st);
+void launch_project(const SceneDev& sc, const nbv_config& cfg, const PreBatch& batch, cudaStream_t st);
 
 // ---- binning.cu
 // stable multi-split of the depth ranks into supertile lists: pass 1 (with the gather of the splats into rank order) fills
 // the supertile-major count table counts[s * msplit_blocks(N) + block]; after an exclusive scan of that table (total =
 // number of coarse entries) pass 2 writes keys (supertile << rank_bits | rank), their tile rects and the supertile ranges
 uint32_t msplit_blocks(int N);
-void launch_msplit_count(const uint32_t* ids_sorted, const Splat* splat, const ushort4* rect, int N, const TileGrid& tg, Splat* splat_sorted,
-                         ushort4* rect_sorted, uint32_t* counts, cudaStream_t st);
-void launch_msplit_write(const ushort4* rect_sorted, int N, const TileGrid& tg, int rank_bits, const uint32_t* scanned,
-                         const uint32_t* d_total, uint32_t cap, uint32_t* keys, ushort4* crect, uint2* ranges, cudaStream_t st);
+void launch_msplit_count(const PreBatch& batch, int N, const TileGrid& tg, cudaStream_t st);
+void launch_msplit_write(const PreBatch& batch, int N, const TileGrid& tg, int rank_bits, uint32_t cap, cudaStream_t st);
 // parity export of the full tile lists: counts -> scanned offsets (+ total) -> ids
 void launch_tile_counts(const uint32_t* ckeys, const ushort4* crect, const uint2* cranges, const TileGrid& tg, int rank_bits,
                         uint32_t* counts, uint32_t* scanned, uint32_t* total, uint32_t* scan_tmp, int64_t* offsets_out, cudaStream_t st);
@@ -61,7 +83,6 @@ struct PixelBuf {            // per-pixel outputs of the forward pass (H x W eac
 };
 // One launch of S3 / S4 / S5+S6 serves a BATCH of views (S3, S4: launch positions interleave the views; S5+S6: grid.y = view): per-view device pointers travel as a
 // __grid_constant__ kernel parameter.  All views of a batch share the image size.
-constexpr int MAX_BATCH = 16;
 struct RasterView {
   const Splat* splat_sorted;
   const uint32_t* ckeys;
@@ -119,8 +140,12 @@ struct ExpandBatch {
   ExpandView v[MAX_BATCH];
 };
 int expand_partials();       // doubles a slot's `partials` buffer must hold
+// trace_total: device scalar S_T of the trace criterion (launch_trace_total), ignored otherwise
 void launch_expand(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, double* H_T, const float* conf,
-                   cudaStream_t st);
+                   const double* trace_total, cudaStream_t st);
+size_t trace_total_scratch_bytes();
+void launch_trace_total(const SceneDev& sc, const nbv_config& cfg, const double* H_T, const float* conf, void* scratch, double* out,
+                        cudaStream_t st);
 // Sparse per-candidate block cache of greedy selection (nbv_select_greedy): pool of (Gaussian id, 105-double block) entries.
 struct BlockCache {
   uint32_t* ids;             // capacity entries
@@ -136,7 +161,7 @@ void launch_expand_cache(const SceneDev& sc, const nbv_config& cfg, const Expand
 // cached_gain_scratch_bytes(n_cand) bytes, zero on first use
 size_t cached_gain_scratch_bytes(int n_cand);
 void launch_cached_gain(const BlockCache& cache, const nbv_config& cfg, int n_cand, const int32_t* taken, const float* conf,
-                        const double* H_T, float* scores, void* scratch, cudaStream_t st);
+                        const double* H_T, float* scores, void* scratch, const double* trace_total, cudaStream_t st);
 // H_T[g] += block for the cached entries of candidate *pick
 void launch_cache_accumulate(const BlockCache& cache, const int32_t* pick, double* H_T, cudaStream_t st);
 void launch_confidence(const SceneDev& sc, const nbv_config& cfg, int target, float* conf, cudaStream_t st);
@@ -151,6 +176,11 @@ void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandB
                         const float* conf, const float* cholT, cudaStream_t st);
 void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
 void launch_mask_scatter(const float* rgb, const float* depth, size_t npx, int K, int group, int bgch, float* mask, cudaStream_t st);
+
+// ---- sh.cu, SH degree 3 colour (NEXT-4): per-view colours in S1, 59 x 59 blocks in S5 / S6 (binary64, one warp per Gaussian)
+void launch_sh_colours(const SceneDev& sc, const float* sh45, const PreBatch& batch, cudaStream_t st);
+void launch_expand_sh(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, const float* sh45, const float* prior59,
+                      double* H_T, const float* conf, cudaStream_t st);
 
 // ---- select.cu
 // Eq. 10-11 on raw (F x n) and training (F x n_train) gains of F = 2 or 3 outputs: denominators, fused scores, arg-max

@@ -70,13 +70,14 @@ struct nbv_ctx {
   bool loaded = false;
   // object-mask context (channel_mask == NBV_CH_MASK): groups of four object channels, blocks of LB = L (L + 1) / 2 floats
   bool mask_mode = false;
+  bool sh_mode = false;                 // SH degree 3 colour (nbv_load_sh): blocks of 59 parameters, binary64
   int mask_groups = 1;                  // 1 in colour / depth contexts (it is the moment stride in units of NMOM)
   size_t LB = NBLK;
   int n_train = 0;
   // scene
   // H_T: N x 105 binary64 (colour / depth contexts) or N x LB binary32 (mask contexts); cholT: mask contexts only
   DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp, cache_ids, cache_blocks, cache_meta,
-      cache_scratch;
+      cache_scratch, trace_buf, sh45, prior59;         // trace_buf: S_T (1 double) | scratch of launch_trace_total
   size_t greedy_cache_bytes = (size_t)4 << 30;   // budget of the block cache of nbv_select_greedy (NBV_GREEDY_CACHE_MB)
   int conf_target = -2;                 // mask contexts: target the cholT buffer was prepared for (-2 = stale)
   // views in flight: S1-S2 of each view run on its slot's stream, S3-S6 of a whole batch in one launch per stage on
@@ -88,6 +89,7 @@ struct nbv_ctx {
   cudaStream_t raster_st[2] = {nullptr, nullptr};    // S3-S6 of the batches of slot set 0 / 1 (forked from / joined into the caller's stream)
   ViewSlot* last_slot = nullptr;        // slot of the last view processed (nbv_last_view_stats)
   DevBuf work_counters;                 // 3 x 128 B: work counters of the persistent backward launches
+  DevBuf counters_pool;                 // ViewCounters of all 2 x MAX_BATCH slots, consecutive (one memset per batch)
   bool persistent = true;
   DevBuf tile_order;                    // centre-out launch order of the tiles of a tile_order_tx x tile_order_ty grid
   int tile_order_tx = 0, tile_order_ty = 0;
@@ -232,7 +234,6 @@ void free_slot(ViewSlot* sl) {
                    &sl->scan_tmp, &sl->tile_counts, &sl->pix_rgb, &sl->pix_depth, &sl->pix_T, &sl->pix_nc, &sl->pix_last,
                    &sl->tile_cend, &sl->tile_elast, &sl->tile_walk, &sl->moments, &sl->touched, &sl->touched_cnt, &sl->partials};
   for (DevBuf* b : all) release(*b);
-  if (sl->d_counters) cudaFree(sl->d_counters);
   if (sl->h_counters) cudaFreeHost(sl->h_counters);
   if (sl->done) cudaEventDestroy(sl->done);
   if (sl->st) cudaStreamDestroy(sl->st);
@@ -248,10 +249,11 @@ int get_slot(nbv_ctx* ctx, int i, ViewSlot** out) {
     // batch would sit behind the 28,800 blocks of the running raster launch instead of slipping in between them.
     int prio_least = 0, prio_greatest = 0;
     cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest);
-    bool ok = cudaStreamCreateWithPriority(&sl->st, cudaStreamNonBlocking, prio_greatest) == cudaSuccess &&
+    bool ok = ensure(ctx, ctx->counters_pool, sizeof(ViewCounters) * 2 * MAX_BATCH) == NBV_OK &&
+              cudaStreamCreateWithPriority(&sl->st, cudaStreamNonBlocking, prio_greatest) == cudaSuccess &&
               cudaEventCreateWithFlags(&sl->done, cudaEventDisableTiming) == cudaSuccess &&
-              cudaMalloc(&sl->d_counters, sizeof(ViewCounters)) == cudaSuccess &&
               cudaMallocHost(&sl->h_counters, sizeof(ViewCounters)) == cudaSuccess;
+    if (ok) sl->d_counters = ctx->counters_pool.as<ViewCounters>() + ctx->slots.size();
     if (!ok) {
       cudaGetLastError();
       free_slot(sl);
@@ -283,12 +285,14 @@ TileGrid make_grid(int W, int H) {
 
 enum Stage { STAGE_PROJECT = 0, STAGE_BIN = 1, STAGE_FORWARD = 2, STAGE_BACKWARD = 3 };
 
-// S1..S2 for one camera on stream st, in the buffers of slot sl: leaves the depth order in sl->ids, the rank-ordered splats and
-// the sorted coarse lists, and makes sure the buffers S3/S4 will need exist (upto).  Never synchronises.
-int pre_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool want_abc, bool full_pix, cudaStream_t st) {
-  if (!valid_camera(cam)) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
+// S1..S2 for a batch of n cameras of equal image size on stream st, in the buffers of slots sl[0..n): ONE launch per stage for
+// the whole batch (grid.y = view; 16 launches instead of 16 n).  Leaves, per slot, the depth order in sl->ids, the rank-ordered
+// splats and the coarse lists, and makes sure the buffers S3/S4 will need exist (upto).  Never synchronises.
+int pre_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int upto, bool want_abc, bool full_pix, cudaStream_t st) {
+  for (int i = 0; i < n; ++i)
+    if (!valid_camera(cams[i])) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
   const int N = ctx->N;
-  const TileGrid tg = make_grid(cam.width, cam.height);
+  const TileGrid tg = make_grid(cams[0].width, cams[0].height);
   const int n_tiles = tg.tiles_x * tg.tiles_y, n_super = tg.super_x * tg.super_y;
   const int rank_bits = ceil_log2((size_t)N), super_bits = ceil_log2((size_t)n_super);
   if (rank_bits + super_bits > 32)
@@ -296,77 +300,87 @@ int pre_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool w
   const unsigned long long worst = (unsigned long long)N * (unsigned long long)n_super;
   if (worst > 0x40000000ull) return fail(ctx, NBV_ERR_CAPACITY, "N x supertiles exceeds the coarse key buffer limit (2^30)");
   const uint32_t ccap = (uint32_t)worst;     // worst case: no overflow is possible, no count has to come back to the host
-  sl->tg = tg; sl->rank_bits = rank_bits; sl->ccap = ccap;
-  ctx->last_slot = sl;
-  const SceneDev sc = scene_dev(ctx);
-
-  CKRET(ensure(ctx, sl->splat, sizeof(Splat) * (size_t)N));
-  CKRET(ensure(ctx, sl->zkey, 4 * (size_t)N)); CKRET(ensure(ctx, sl->zkey_alt, 4 * (size_t)N));
-  CKRET(ensure(ctx, sl->ids, 4 * (size_t)N)); CKRET(ensure(ctx, sl->ids_alt, 4 * (size_t)N));
-  CKRET(ensure(ctx, sl->rect, sizeof(ushort4) * (size_t)N));
-  if (want_abc) CKRET(ensure(ctx, sl->abc, 12 * (size_t)N));
-  CKRET(ensure(ctx, sl->sort_tmp, 4 * radix_temp_words((size_t)N)));
-  CKRET(ensure(ctx, sl->scan_tmp, 4 * scan_temp_words(std::max((size_t)N + 1, (size_t)n_tiles + 1))));
-  if (upto >= STAGE_BIN) {
-    CKRET(ensure(ctx, sl->splat_sorted, sizeof(Splat) * (size_t)N));
-    CKRET(ensure(ctx, sl->rect_sorted, sizeof(ushort4) * (size_t)N));
-    const size_t n_counts = (size_t)n_super * msplit_blocks(N);
-    CKRET(ensure(ctx, sl->msplit, 4 * (n_counts + scan_temp_words(n_counts))));
-    CKRET(ensure(ctx, sl->ckeys, 4 * (size_t)ccap));
-    CKRET(ensure(ctx, sl->crect, sizeof(ushort4) * (size_t)ccap));
-    CKRET(ensure(ctx, sl->cranges, sizeof(uint2) * 256));
-  }
-  if (upto >= STAGE_FORWARD) {
-    const size_t npx = (size_t)cam.width * cam.height;
-    CKRET(ensure(ctx, sl->pix_T, 4 * npx)); CKRET(ensure(ctx, sl->pix_last, 4 * npx));
-    CKRET(ensure(ctx, sl->tile_cend, 4 * (size_t)n_tiles)); CKRET(ensure(ctx, sl->tile_walk, 4 * (size_t)n_tiles));
-    CKRET(ensure(ctx, sl->tile_elast, 4 * (size_t)n_tiles));
-    if (full_pix) {
-      CKRET(ensure(ctx, sl->pix_rgb, 12 * npx)); CKRET(ensure(ctx, sl->pix_depth, 4 * npx)); CKRET(ensure(ctx, sl->pix_nc, 4 * npx));
+  const size_t n_counts = (size_t)n_super * msplit_blocks(N);
+  const size_t npx = (size_t)cams[0].width * cams[0].height;
+  const size_t mom_bytes = 4 * (size_t)NMOM * ctx->mask_groups * N;
+  PreBatch pb;
+  pb.n = n;
+  for (int i = 0; i < n; ++i) {
+    ViewSlot* s = sl[i];
+    s->tg = tg; s->rank_bits = rank_bits; s->ccap = ccap;
+    CKRET(ensure(ctx, s->splat, sizeof(Splat) * (size_t)N));
+    CKRET(ensure(ctx, s->zkey, 4 * (size_t)N)); CKRET(ensure(ctx, s->zkey_alt, 4 * (size_t)N));
+    CKRET(ensure(ctx, s->ids, 4 * (size_t)N)); CKRET(ensure(ctx, s->ids_alt, 4 * (size_t)N));
+    CKRET(ensure(ctx, s->rect, sizeof(ushort4) * (size_t)N));
+    if (want_abc) CKRET(ensure(ctx, s->abc, 12 * (size_t)N));
+    CKRET(ensure(ctx, s->sort_tmp, 4 * radix_temp_words((size_t)N)));
+    CKRET(ensure(ctx, s->scan_tmp, 4 * scan_temp_words(std::max((size_t)N + 1, (size_t)n_tiles + 1))));
+    if (upto >= STAGE_BIN) {
+      CKRET(ensure(ctx, s->splat_sorted, sizeof(Splat) * (size_t)N));
+      CKRET(ensure(ctx, s->rect_sorted, sizeof(ushort4) * (size_t)N));
+      CKRET(ensure(ctx, s->msplit, 4 * (n_counts + scan_temp_words(n_counts))));
+      CKRET(ensure(ctx, s->ckeys, 4 * (size_t)ccap));
+      CKRET(ensure(ctx, s->crect, sizeof(ushort4) * (size_t)ccap));
+      CKRET(ensure(ctx, s->cranges, sizeof(uint2) * 256));
     }
+    if (upto >= STAGE_FORWARD) {
+      CKRET(ensure(ctx, s->pix_T, 4 * npx)); CKRET(ensure(ctx, s->pix_last, 4 * npx));
+      CKRET(ensure(ctx, s->tile_cend, 4 * (size_t)n_tiles)); CKRET(ensure(ctx, s->tile_walk, 4 * (size_t)n_tiles));
+      CKRET(ensure(ctx, s->tile_elast, 4 * (size_t)n_tiles));
+      if (full_pix) {
+        CKRET(ensure(ctx, s->pix_rgb, 12 * npx)); CKRET(ensure(ctx, s->pix_depth, 4 * npx)); CKRET(ensure(ctx, s->pix_nc, 4 * npx));
+      }
+    }
+    if (upto >= STAGE_BACKWARD) {
+      if (ctx->mask_mode) CKRET(ensure(ctx, s->gsplat, sizeof(Splat) * (size_t)N));
+      if (s->moments.cap < mom_bytes || !s->moments.p) s->moments_clean = false;
+      CKRET(ensure(ctx, s->moments, mom_bytes));
+      CKRET(ensure(ctx, s->touched, 4 * (size_t)N));
+      CKRET(ensure(ctx, s->touched_cnt, 4 * (size_t)touched_blocks(N)));
+      CKRET(ensure(ctx, s->partials, 8 * (size_t)expand_partials()));
+      if (!s->moments_clean) CK(cudaMemsetAsync(s->moments.p, 0, mom_bytes, st));
+      s->moments_clean = false;     // dirty until an expand kernel has consumed the touched list
+    }
+    PreView& v = pb.v[i];
+    v.cam = cams[i];
+    v.splat = s->splat.as<Splat>();
+    v.zkey[0] = s->zkey.as<uint32_t>(); v.zkey[1] = s->zkey_alt.as<uint32_t>();
+    v.ids[0] = s->ids.as<uint32_t>(); v.ids[1] = s->ids_alt.as<uint32_t>();
+    v.rect = s->rect.as<ushort4>();
+    v.abc = want_abc ? s->abc.as<float>() : nullptr;
+    v.hist = s->sort_tmp.as<uint32_t>();
+    v.splat_sorted = s->splat_sorted.as<Splat>(); v.rect_sorted = s->rect_sorted.as<ushort4>();
+    v.counts = s->msplit.as<uint32_t>();
+    v.ckeys = s->ckeys.as<uint32_t>(); v.crect = s->crect.as<ushort4>(); v.cranges = s->cranges.as<uint2>();
+    v.counters = s->d_counters;
+    s->ckeys_sorted = s->ckeys.as<uint32_t>();
   }
-  if (upto >= STAGE_BACKWARD) {
-    const size_t mom_bytes = 4 * (size_t)NMOM * ctx->mask_groups * N;
-    if (ctx->mask_mode) CKRET(ensure(ctx, sl->gsplat, sizeof(Splat) * (size_t)N));
-    if (sl->moments.cap < mom_bytes || !sl->moments.p) sl->moments_clean = false;
-    CKRET(ensure(ctx, sl->moments, mom_bytes));
-    CKRET(ensure(ctx, sl->touched, 4 * (size_t)N));
-    CKRET(ensure(ctx, sl->touched_cnt, 4 * (size_t)touched_blocks(N)));
-    CKRET(ensure(ctx, sl->partials, 8 * (size_t)expand_partials()));
-    if (!sl->moments_clean) CK(cudaMemsetAsync(sl->moments.p, 0, mom_bytes, st));
-    sl->moments_clean = false;     // dirty until an expand kernel has consumed the touched list
+  ctx->last_slot = sl[n - 1];
+  // the counters of the slots of a set are consecutive in one pool: one memset per batch
+  bool consecutive = true;
+  for (int i = 1; i < n; ++i) consecutive = consecutive && sl[i]->d_counters == sl[0]->d_counters + i;
+  if (consecutive) {
+    CK(cudaMemsetAsync(sl[0]->d_counters, 0, sizeof(ViewCounters) * (size_t)n, st));
+  } else {
+    for (int i = 0; i < n; ++i) CK(cudaMemsetAsync(sl[i]->d_counters, 0, sizeof(ViewCounters), st));
   }
-
-  CK(cudaMemsetAsync(sl->d_counters, 0, sizeof(ViewCounters), st));
-  int sp = span_begin(ctx, NBV_STAGE_PROJECT, 1, st);
-  launch_project(sc, cam, ctx->cfg, sl->splat.as<Splat>(), sl->zkey.as<uint32_t>(), sl->ids.as<uint32_t>(),
-                 sl->rect.as<ushort4>(), want_abc ? sl->abc.as<float>() : nullptr, sl->d_counters, st);
+  const SceneDev sc = scene_dev(ctx);
+  int sp = span_begin(ctx, NBV_STAGE_PROJECT, n, st);
+  launch_project(sc, ctx->cfg, pb, st);
+  if (ctx->sh_mode) launch_sh_colours(sc, ctx->sh45.as<float>(), pb, st);      // R-18: the colour of this view direction
   CK(cudaGetLastError());
   if (upto == STAGE_PROJECT) { span_end(ctx, sp, st); return NBV_OK; }
 
   // depth sort: 4 stable passes of 8 bits on the z bits, Gaussian index as value (ties keep index order: R-7)
-  sp = span_next(ctx, sp, NBV_STAGE_DEPTH_SORT, 1, st);
-  {
-    uint32_t *k0 = sl->zkey.as<uint32_t>(), *k1 = sl->zkey_alt.as<uint32_t>();
-    uint32_t *v0 = sl->ids.as<uint32_t>(), *v1 = sl->ids_alt.as<uint32_t>();
-    for (int pass = 0; pass < 4; ++pass) {
-      radix_pass(k0, k1, v0, v1, (size_t)N, nullptr, 8 * pass, 8, sl->sort_tmp.as<uint32_t>(), st);
-      std::swap(k0, k1);
-      std::swap(v0, v1);
-    }
-    CK(cudaGetLastError());
-  }
+  sp = span_next(ctx, sp, NBV_STAGE_DEPTH_SORT, n, st);
+  for (int pass = 0; pass < 4; ++pass) radix_pass_batched(pb, pass & 1, (size_t)N, 8 * pass, st);
+  CK(cudaGetLastError());
   // coarse binning: rank-ordered splats + per-(supertile, rank block) counts | scan | keys, rects and supertile ranges
-  sp = span_next(ctx, sp, NBV_STAGE_BIN, 1, st);
-  const size_t n_counts = (size_t)n_super * msplit_blocks(N);
-  uint32_t* counts = sl->msplit.as<uint32_t>();
-  launch_msplit_count(sl->ids.as<uint32_t>(), sl->splat.as<Splat>(), sl->rect.as<ushort4>(), N, tg, sl->splat_sorted.as<Splat>(),
-                      sl->rect_sorted.as<ushort4>(), counts, st);
-  sp = span_next(ctx, sp, NBV_STAGE_COARSE_SORT, 1, st);
-  exclusive_scan_u32(counts, counts, n_counts, counts + n_counts, &sl->d_counters->n_coarse, st);
-  launch_msplit_write(sl->rect_sorted.as<ushort4>(), N, tg, rank_bits, counts, &sl->d_counters->n_coarse, ccap, sl->ckeys.as<uint32_t>(),
-                      sl->crect.as<ushort4>(), sl->cranges.as<uint2>(), st);
-  sl->ckeys_sorted = sl->ckeys.as<uint32_t>();
+  sp = span_next(ctx, sp, NBV_STAGE_BIN, n, st);
+  launch_msplit_count(pb, N, tg, st);
+  sp = span_next(ctx, sp, NBV_STAGE_COARSE_SORT, n, st);
+  scan_batched(pb, SCAN_COUNTS, n_counts, st);
+  launch_msplit_write(pb, N, tg, rank_bits, ccap, st);
   CK(cudaGetLastError());
   span_end(ctx, sp, st);
   return NBV_OK;
@@ -484,8 +498,11 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
   } else if (ctx->mask_mode) {
     launch_expand_mask(scene_dev(ctx), ctx->cfg, eb, mode, ctx->mask_groups, ctx->H_T.as<float>(), ctx->conf.as<float>(),
                        ctx->cholT.as<float>(), st);
+  } else if (ctx->sh_mode) {
+    launch_expand_sh(scene_dev(ctx), ctx->cfg, eb, mode, ctx->sh45.as<float>(), ctx->prior59.as<float>(), ctx->H_T.as<double>(),
+                     ctx->conf.as<float>(), st);
   } else {
-    launch_expand(scene_dev(ctx), ctx->cfg, eb, mode, ctx->H_T.as<double>(), ctx->conf.as<float>(), st);
+    launch_expand(scene_dev(ctx), ctx->cfg, eb, mode, ctx->H_T.as<double>(), ctx->conf.as<float>(), ctx->trace_buf.as<double>(), st);
   }
   CK(cudaGetLastError());
   span_end(ctx, sp, st);
@@ -495,7 +512,7 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
 
 // one view through S1..S4 on the caller's stream in slot 0 (parity exports)
 int process_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int upto, bool want_abc, bool full_pix, cudaStream_t st) {
-  CKRET(pre_view(ctx, sl, cam, upto, want_abc, full_pix, st));
+  CKRET(pre_batch(ctx, &sl, &cam, 1, upto, want_abc, full_pix, st));
   if (upto >= STAGE_FORWARD) CKRET(raster_batch(ctx, &sl, &cam, 1, upto, full_pix, st));
   return NBV_OK;
 }
@@ -534,12 +551,14 @@ int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_
     ViewSlot* sl[MAX_BATCH];
     for (int i = 0; i < nb && rc == NBV_OK; ++i) rc = get_slot(ctx, set * MAX_BATCH + i, &sl[i]);
     if (rc != NBV_OK) break;
-    for (int i = 0; i < nb; ++i) {
-      // the slot's buffers are free once the S3-S6 launches of the batch that last used this set have finished
-      ck(cudaStreamWaitEvent(sl[i]->st, set_used[set] ? ctx->ev_set_done[set] : ctx->ev_fork, 0), "cudaStreamWaitEvent(slot)");
-      if (rc == NBV_OK) rc = pre_view(ctx, sl[i], h_cams[i0 + i], STAGE_BACKWARD, false, false, sl[i]->st);
-      ck(cudaEventRecord(sl[i]->done, sl[i]->st), "cudaEventRecord(slot)");
-      ck(cudaStreamWaitEvent(rs, sl[i]->done, 0), "cudaStreamWaitEvent(raster)");      // join even after an error: no stream may run ahead
+    {
+      // S1-S2 of the whole batch on the high-priority stream of the set's first slot; the set's buffers are free once the
+      // S3-S6 launches of the batch that last used this set have finished
+      cudaStream_t ps = sl[0]->st;
+      ck(cudaStreamWaitEvent(ps, set_used[set] ? ctx->ev_set_done[set] : ctx->ev_fork, 0), "cudaStreamWaitEvent(pre)");
+      if (rc == NBV_OK) rc = pre_batch(ctx, sl, h_cams + i0, nb, STAGE_BACKWARD, false, false, ps);
+      ck(cudaEventRecord(sl[0]->done, ps), "cudaEventRecord(pre)");
+      ck(cudaStreamWaitEvent(rs, sl[0]->done, 0), "cudaStreamWaitEvent(raster)");      // join even after an error: no stream may run ahead
     }
     if (rc == NBV_OK) rc = raster_batch(ctx, sl, h_cams + i0, nb, STAGE_BACKWARD, false, rs);
     // Batches that write shared state in S5 (H_T += in view order, Eq. 6; the block pool of greedy selection) run that
@@ -565,6 +584,13 @@ int prepare_scoring(nbv_ctx* ctx, int target, cudaStream_t st) {
   launch_confidence(sc, ctx->cfg, target, ctx->conf.as<float>(), st);
   if (ctx->mask_mode && ctx->conf_target != target)
     launch_prepare_mask(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
+  if (ctx->cfg.criterion == NBV_CRIT_TRACE) {                // S_T of the trace criterion: all N blocks of the current H_T
+    if (!ctx->trace_buf.p) {
+      CKRET(ensure(ctx, ctx->trace_buf, 16 + trace_total_scratch_bytes()));
+      CK(cudaMemsetAsync(ctx->trace_buf.p, 0, 16 + trace_total_scratch_bytes(), st));
+    }
+    launch_trace_total(sc, ctx->cfg, ctx->H_T.as<double>(), ctx->conf.as<float>(), ctx->trace_buf.as<char>() + 16, ctx->trace_buf.as<double>(), st);
+  }
   CK(cudaGetLastError());
   ctx->conf_target = target;
   return NBV_OK;
@@ -613,6 +639,7 @@ void nbv_default_config(nbv_config* cfg) {
   cfg->mask_bg_channel = 0;
   cfg->prior_precision_obj = 1.0f;
   cfg->weight_mode = 0;
+  cfg->criterion = NBV_CRIT_LOGDET;
 }
 
 int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
@@ -624,7 +651,8 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
                   c.alpha_max < 1.f && c.t_stop > 0.f && c.t_stop < 1.f &&
                   (c.channel_mask == NBV_CH_MASK || ((c.channel_mask & 15) != 0 && (c.channel_mask & ~15) == 0)) &&
                   c.mask_bg_channel >= 0 && c.prior_precision_obj > 0.f && std::isfinite(c.prior_precision_obj) &&
-                  c.weight_mode >= 0 && c.weight_mode <= 2 &&
+                  c.weight_mode >= 0 && c.weight_mode <= 2 && c.criterion >= NBV_CRIT_LOGDET && c.criterion <= NBV_CRIT_DET &&
+                  (c.criterion != NBV_CRIT_TRACE || (c.weight_mode == 0 && c.channel_mask != NBV_CH_MASK)) &&
                   (c.opacity_coord == 0 || c.opacity_coord == 1) && c.p_floor > 0.f && c.sigma_floor > 0.f;
   if (!ok) return NBV_ERR_INVALID_ARG;
   for (int k = 0; k < NBV_P; ++k)
@@ -662,8 +690,8 @@ void nbv_destroy(nbv_ctx* ctx) {
   if (!ctx) return;
   cudaDeviceSynchronize();
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
-                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order, &ctx->work_counters, &ctx->cache_ids,
-                   &ctx->cache_blocks, &ctx->cache_meta, &ctx->cache_scratch};
+                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order, &ctx->work_counters, &ctx->counters_pool, &ctx->cache_ids,
+                   &ctx->cache_blocks, &ctx->cache_meta, &ctx->cache_scratch, &ctx->trace_buf, &ctx->sh45, &ctx->prior59};
   for (DevBuf* b : all) release(*b);
   for (ViewSlot* sl : ctx->slots) free_slot(sl);
   if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
@@ -697,6 +725,7 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
     ctx->LB = L * (L + 1) / 2;
     ctx->mask_groups = (K + 3) / 4;
   }
+  if (!ctx->mask_mode) { ctx->sh_mode = false; ctx->LB = NBLK; }
   ctx->N = N; ctx->K = K;
   const size_t n = (size_t)N;
   CKRET(ensure(ctx, ctx->mean, 12 * n)); CKRET(ensure(ctx, ctx->logscale, 12 * n)); CKRET(ensure(ctx, ctx->quat, 16 * n));
@@ -725,6 +754,30 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
   ctx->n_train = 0;
   ctx->conf_target = -2;
   ctx->loaded = true;
+  return NBV_OK;
+}
+
+int nbv_load_sh(nbv_ctx* ctx, const float* d_sh, void* stream) {
+  if (!ctx || !d_sh) return NBV_ERR_INVALID_ARG;
+  if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
+  if (ctx->mask_mode || ctx->cfg.weight_mode != 0 || ctx->cfg.criterion == NBV_CRIT_TRACE)
+    return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_load_sh: colour / depth contexts with weight_mode 0 and the log-det criterion only");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t n = (size_t)ctx->N;
+  CK(cudaDeviceSynchronize());             // no view may still be in flight on the old block size
+  ctx->LB = (size_t)NBV_SH_L * (NBV_SH_L + 1) / 2;
+  CKRET(ensure(ctx, ctx->sh45, 4 * 45 * n));
+  CKRET(ensure(ctx, ctx->prior59, 4 * NBV_SH_L));
+  CKRET(ensure(ctx, ctx->H_T, 8 * ctx->LB * n));
+  CK(cudaMemcpyAsync(ctx->sh45.p, d_sh, 4 * 45 * n, cudaMemcpyDeviceToDevice, st));
+  float prior[NBV_SH_L];
+  for (int k = 0; k < NBV_SH_L; ++k) prior[k] = k < 14 ? ctx->cfg.prior_precision[k] : ctx->cfg.prior_precision[11 + (k - 14) % 3];
+  CK(cudaMemcpyAsync(ctx->prior59.p, prior, sizeof(prior), cudaMemcpyHostToDevice, st));
+  CK(cudaMemsetAsync(ctx->H_T.p, 0, 8 * ctx->LB * n, st));
+  CK(cudaStreamSynchronize(st));           // `prior` is a stack buffer
+  ctx->sh_mode = true;
+  ctx->n_train = 0;
+  ctx->conf_target = -2;
   return NBV_OK;
 }
 
@@ -873,7 +926,7 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
   // the masked arg-max and H_T += (blocks of the selected view) -- all on the device, no camera and no host round trip.
   const size_t entry_bytes = 8 * (size_t)NBLK + 4;
   const size_t want = std::min((size_t)n * (size_t)ctx->N, ctx->greedy_cache_bytes / entry_bytes);
-  if (want == 0 || want > 0xfffffff0ull || ctx->mask_mode) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);
+  if (want == 0 || want > 0xfffffff0ull || ctx->mask_mode || ctx->sh_mode) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);
   CKRET(ensure(ctx, ctx->cache_ids, 4 * want));
   CKRET(ensure(ctx, ctx->cache_blocks, 8 * (size_t)NBLK * want));
   CKRET(ensure(ctx, ctx->cache_scratch, cached_gain_scratch_bytes(n)));
@@ -895,7 +948,8 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
   if (h_cursor[1]) return select_greedy_rescore(ctx, h_cams, n, rounds, target_obj, h_order, d_scores, st);   // pool too small
   for (int r = 0; r < rounds; ++r) {
     CKRET(prepare_scoring(ctx, target_obj, st));
-    launch_cached_gain(bc, ctx->cfg, n, d_taken, ctx->conf.as<float>(), ctx->H_T.as<double>(), d_round, ctx->cache_scratch.p, st);
+    launch_cached_gain(bc, ctx->cfg, n, d_taken, ctx->conf.as<float>(), ctx->H_T.as<double>(), d_round, ctx->cache_scratch.p,
+                       ctx->trace_buf.as<double>(), st);
     launch_greedy_pick(d_round, d_taken, n, d_scores ? d_scores + (size_t)r * n : nullptr, d_pick, d_order + r, st);
     launch_cache_accumulate(bc, d_pick, ctx->H_T.as<double>(), st);      // Eq. 6: H_T += H(c*)
     CK(cudaGetLastError());
@@ -1015,7 +1069,7 @@ int nbv_render_mask(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_mask, void* 
   if (!ctx->mask_mode) return fail(ctx, NBV_ERR_INVALID_ARG, "nbv_render_mask needs a context created with channel_mask = NBV_CH_MASK");
   cudaStream_t st = (cudaStream_t)stream;
   ViewSlot* sl = ctx->slots[0];
-  CKRET(pre_view(ctx, sl, *h_cam, STAGE_BACKWARD, false, true, st));      // S1-S2 and every buffer the raster passes use
+  CKRET(pre_batch(ctx, &sl, h_cam, 1, STAGE_BACKWARD, false, true, st));      // S1-S2 and every buffer the raster passes use
   CKRET(ensure_tile_order(ctx, sl->tg, st));
   const size_t npx = (size_t)h_cam->width * h_cam->height;
   const SceneDev sc = scene_dev(ctx);

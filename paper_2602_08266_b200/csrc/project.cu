@@ -74,10 +74,16 @@ __device__ __forceinline__ float log_bound(float sigma) {
   return add_rn(mul_rn((float)e, 0x1.62e43p-1f), lm);
 }
 
-__global__ void __launch_bounds__(256) project_kernel(SceneDev sc, nbv_camera cam, nbv_config cfg, Splat* __restrict__ splat,
-                                                       uint32_t* __restrict__ zkey, uint32_t* __restrict__ ids,
-                                                       ushort4* __restrict__ rect, float* __restrict__ abc,
-                                                       ViewCounters* counters) {
+__global__ void __launch_bounds__(256) project_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
+                                                       const __grid_constant__ PreBatch batch) {
+  const PreView& pv = batch.v[blockIdx.y];
+  const nbv_camera& cam = pv.cam;
+  Splat* __restrict__ splat = pv.splat;
+  uint32_t* __restrict__ zkey = pv.zkey[0];
+  uint32_t* __restrict__ ids = pv.ids[0];
+  ushort4* __restrict__ rect = pv.rect;
+  float* __restrict__ abc = pv.abc;
+  ViewCounters* counters = pv.counters;
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   bool visible = false;
   unsigned int ntiles = 0;
@@ -176,10 +182,9 @@ __global__ void __launch_bounds__(256) project_kernel(SceneDev sc, nbv_camera ca
   }
 }
 
-void launch_project(const SceneDev& sc, const nbv_camera& cam, const nbv_config& cfg, Splat* splat, uint32_t* zkey,
-                    uint32_t* ids, ushort4* rect, float* abc, ViewCounters* counters, cudaStream_t st) {
+void launch_project(const SceneDev& sc, const nbv_config& cfg, const PreBatch& batch, cudaStream_t st) {
   ++g_kernel_launches;
-  project_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(sc, cam, cfg, splat, zkey, ids, rect, abc, counters);
+  project_kernel<<<dim3((unsigned)((sc.N + 255) / 256), (unsigned)batch.n), 256, 0, st>>>(sc, cfg, batch);
 }
 
 }  // namespace nbv

@@ -130,6 +130,42 @@ scan_cluster_kernel(const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* __r
   cluster.sync();                            // no CTA may exit while its shared memory can still be read
 }
 
+// the same scan for one table per view of a batch (grid.y = view), in place
+__global__ void __cluster_dims__(SCAN1_CTAS, 1, 1) __launch_bounds__(SCAN1_T)
+scan_cluster_batched_kernel(const __grid_constant__ PreBatch batch, int table, uint32_t n) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  __shared__ uint32_t sdata[SCAN1_PER_CTA];
+  __shared__ uint32_t sm[32];
+  __shared__ uint32_t cta_total;
+  const PreView& pv = batch.v[blockIdx.y];
+  uint32_t* data = table == SCAN_HIST ? pv.hist : pv.counts;
+  uint32_t* total_out = table == SCAN_COUNTS ? &pv.counters->n_coarse : nullptr;
+  const uint32_t rank = cluster.block_rank();
+  const uint32_t per = (n + SCAN1_CTAS - 1) / SCAN1_CTAS;
+  const uint32_t g0 = min(rank * per, n), g1 = min(g0 + per, n), m = g1 - g0;
+  for (uint32_t i = threadIdx.x; i < m; i += SCAN1_T) sdata[i] = data[g0 + i];
+  __syncthreads();
+  const uint32_t c = ((m + SCAN1_T - 1) / SCAN1_T) | 1u;
+  const uint32_t i0 = min(threadIdx.x * c, m), i1 = min(i0 + c, m);
+  uint32_t s = 0;
+  for (uint32_t i = i0; i < i1; ++i) s += sdata[i];
+  uint32_t total;
+  uint32_t off = block_exclusive_scan(s, sm, total);
+  for (uint32_t i = i0; i < i1; ++i) {
+    const uint32_t v = sdata[i];
+    sdata[i] = off;
+    off += v;
+  }
+  if (threadIdx.x == 0) cta_total = total;
+  cluster.sync();
+  uint32_t base = 0;
+  for (uint32_t r = 0; r < rank; ++r) base += *cluster.map_shared_rank(&cta_total, r);
+  for (uint32_t i = threadIdx.x; i < m; i += SCAN1_T) data[g0 + i] = base + sdata[i];
+  if (total_out && rank == SCAN1_CTAS - 1 && threadIdx.x == 0) *total_out = base + total;
+  cluster.sync();                            // no CTA may exit while its shared memory can still be read
+}
+
 size_t scan_temp_words(size_t n) {
   size_t words = 0;
   while (n > (size_t)SCAN_TILE) {
@@ -163,6 +199,21 @@ void exclusive_scan_u32(const uint32_t* in, uint32_t* out, size_t n, uint32_t* t
   scan_downsweep_kernel<<<nb, SCAN_T, 0, st>>>(in, out, (uint32_t)n, sums, total_out);
 }
 
+uint32_t scan_batched_max() { return SCAN1_MAX; }
+
+void scan_batched(const PreBatch& batch, int table, size_t n, cudaStream_t st) {
+  if (n == 0) return;
+  if (n > SCAN1_MAX) {                       // long tables: the general multi-level scan, view by view (scratch follows the table)
+    for (int v = 0; v < batch.n; ++v) {
+      uint32_t* data = table == SCAN_HIST ? batch.v[v].hist : batch.v[v].counts;
+      exclusive_scan_u32(data, data, n, data + n, table == SCAN_COUNTS ? &batch.v[v].counters->n_coarse : nullptr, st);
+    }
+    return;
+  }
+  ++g_kernel_launches;
+  scan_cluster_batched_kernel<<<dim3(SCAN1_CTAS, (unsigned)batch.n), SCAN1_T, 0, st>>>(batch, table, (uint32_t)n);
+}
+
 // ------------------------------------------------------------------------------------------------
 // one stable radix pass on `bits` (<= 8) bits at `shift`
 // ------------------------------------------------------------------------------------------------
@@ -170,17 +221,19 @@ constexpr int RS_T = 256;
 // keys per thread: 16 (4096 keys per block) for long inputs, 4 (1024 per block) for short ones -- a pass over 200,000
 // keys is one partial wave of blocks either way, so its time is one block's critical path: shorter blocks, shorter pass
 constexpr int RS_I_LONG = 16, RS_I_SHORT = 4;
-constexpr size_t RS_SHORT_MAX = 512 * 1024;
+constexpr size_t RS_SHORT_MAX = 256 * 1024;
 __host__ __device__ constexpr int rs_tile(int rs_i) { return RS_T * rs_i; }
-static int rs_i_for(size_t n) { return n <= RS_SHORT_MAX ? RS_I_SHORT : RS_I_LONG; }
+static int rs_i_for(size_t n) { return n <= RS_SHORT_MAX ? RS_I_SHORT : RS_I_LONG; }   // <= 256 blocks up to 2^20 keys: one cluster scan
 constexpr int RS_W = RS_T / 32;        // 8 warps, 512 consecutive keys each
 
 template <int RS_I>
-__global__ void __launch_bounds__(RS_T) radix_hist_kernel(const uint32_t* __restrict__ keys, uint32_t n, const uint32_t* __restrict__ d_n,
-                                                           int shift, uint32_t mask, uint32_t* __restrict__ hist, uint32_t nblocks) {
+__global__ void __launch_bounds__(RS_T) radix_hist_kernel(const __grid_constant__ PreBatch batch, int src, uint32_t n, int shift,
+                                                           uint32_t mask, uint32_t nblocks) {
   constexpr int RS_TILE = RS_T * RS_I;
   __shared__ uint32_t h[256];
-  if (d_n) n = min(n, *d_n);             // device-side length (n is then the capacity the grid was sized for)
+  const PreView& pv = batch.v[blockIdx.y];
+  const uint32_t* __restrict__ keys = pv.zkey[src];
+  uint32_t* __restrict__ hist = pv.hist;
   h[threadIdx.x] = 0;
   __syncthreads();
   const uint32_t base = blockIdx.x * RS_TILE;
@@ -193,13 +246,17 @@ __global__ void __launch_bounds__(RS_T) radix_hist_kernel(const uint32_t* __rest
   if (threadIdx.x <= mask) hist[(size_t)threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
 }
 
-template <bool HAS_VALS, int RS_I>
-__global__ void __launch_bounds__(RS_T) radix_scatter_kernel(const uint32_t* __restrict__ keys_in, uint32_t* __restrict__ keys_out,
-                                                              const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ vals_out,
-                                                              uint32_t n, const uint32_t* __restrict__ d_n, int shift, uint32_t mask,
-                                                              const uint32_t* __restrict__ hist_scanned, uint32_t nblocks) {
+template <int RS_I>
+__global__ void __launch_bounds__(RS_T) radix_scatter_kernel(const __grid_constant__ PreBatch batch, int src, uint32_t n, int shift,
+                                                              uint32_t mask, uint32_t nblocks) {
   constexpr int RS_TILE = RS_T * RS_I;
-  if (d_n) n = min(n, *d_n);
+  constexpr bool HAS_VALS = true;
+  const PreView& pv = batch.v[blockIdx.y];
+  const uint32_t* __restrict__ keys_in = pv.zkey[src];
+  uint32_t* __restrict__ keys_out = pv.zkey[src ^ 1];
+  const uint32_t* __restrict__ vals_in = pv.ids[src];
+  uint32_t* __restrict__ vals_out = pv.ids[src ^ 1];
+  const uint32_t* __restrict__ hist_scanned = pv.hist;
   if (blockIdx.x * RS_TILE >= n) return;
   __shared__ uint32_t wh[RS_W][256];     // per-warp digit counts, then per-warp digit bases
   __shared__ uint32_t dstart[256];       // block-local start of each digit's run
@@ -271,34 +328,21 @@ __global__ void __launch_bounds__(RS_T) radix_scatter_kernel(const uint32_t* __r
 
 uint32_t radix_blocks(size_t n) { const size_t t = (size_t)rs_tile(rs_i_for(n)); return (uint32_t)((n + t - 1) / t); }
 
-size_t radix_temp_words(size_t n) {
-  size_t nb = radix_blocks(n);
-  size_t hist = 256 * nb;
-  return hist + scan_temp_words(hist);
-}
+size_t radix_temp_words(size_t n) { const size_t h = 256 * (size_t)radix_blocks(n); return h + scan_temp_words(h); }
 
-void radix_pass(const uint32_t* keys_in, uint32_t* keys_out, const uint32_t* vals_in, uint32_t* vals_out, size_t n,
-                const uint32_t* d_n, int shift, int bits, uint32_t* tmp, cudaStream_t st) {
+void radix_pass_batched(const PreBatch& batch, int src, size_t n, int shift, cudaStream_t st) {
   if (n == 0) return;
   const uint32_t nb = radix_blocks(n);
   const bool shrt = rs_i_for(n) == RS_I_SHORT;
-  const uint32_t mask = (1u << bits) - 1u;
-  const size_t hist_n = (size_t)(mask + 1) * nb;
-  uint32_t* hist = tmp;
+  const uint32_t mask = 255u;
+  const dim3 grid(nb, (unsigned)batch.n);
   ++g_kernel_launches;
-  if (shrt) radix_hist_kernel<RS_I_SHORT><<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, d_n, shift, mask, hist, nb);
-  else radix_hist_kernel<RS_I_LONG><<<nb, RS_T, 0, st>>>(keys_in, (uint32_t)n, d_n, shift, mask, hist, nb);
-  exclusive_scan_u32(hist, hist, hist_n, tmp + 256 * (size_t)nb, nullptr, st);
-  if (vals_in) {
-    ++g_kernel_launches;
-    if (shrt) radix_scatter_kernel<true, RS_I_SHORT><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, d_n, shift, mask, hist, nb);
-    else radix_scatter_kernel<true, RS_I_LONG><<<nb, RS_T, 0, st>>>(keys_in, keys_out, vals_in, vals_out, (uint32_t)n, d_n, shift, mask, hist, nb);
-  }
-  else {
-    ++g_kernel_launches;
-    if (shrt) radix_scatter_kernel<false, RS_I_SHORT><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, d_n, shift, mask, hist, nb);
-    else radix_scatter_kernel<false, RS_I_LONG><<<nb, RS_T, 0, st>>>(keys_in, keys_out, nullptr, nullptr, (uint32_t)n, d_n, shift, mask, hist, nb);
-  }
+  if (shrt) radix_hist_kernel<RS_I_SHORT><<<grid, RS_T, 0, st>>>(batch, src, (uint32_t)n, shift, mask, nb);
+  else radix_hist_kernel<RS_I_LONG><<<grid, RS_T, 0, st>>>(batch, src, (uint32_t)n, shift, mask, nb);
+  scan_batched(batch, SCAN_HIST, 256 * (size_t)nb, st);
+  ++g_kernel_launches;
+  if (shrt) radix_scatter_kernel<RS_I_SHORT><<<grid, RS_T, 0, st>>>(batch, src, (uint32_t)n, shift, mask, nb);
+  else radix_scatter_kernel<RS_I_LONG><<<grid, RS_T, 0, st>>>(batch, src, (uint32_t)n, shift, mask, nb);
 }
 
 }  // namespace nbv

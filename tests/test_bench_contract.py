@@ -30,10 +30,25 @@ def test_reference_arm_on_other_ranks_is_silent():
     assert r.returncode == 0 and r.stdout.strip() == ""
 
 
-def test_work_constants_match_the_design_document():
+def test_work_constants_come_from_the_committed_counter_pass():
+    """roofline.frac uses EXECUTED flop per (pixel, entry) evaluation; the numbers must be the ones of the committed ncu
+    metric pass bench.FLOP_SOURCE names (frac must follow from committed counters) and DESIGN.md must quote them"""
     sys.path.insert(0, ROOT)
     import bench
-    text = open(os.path.join(ROOT, "DESIGN.md")).read()
-    assert bench.FLOP_TEST == 11 and "| 11 flop | `FLOP_TEST` |" in text
-    assert bench.FLOP_FWD_PAIR == 31 and "| 31 flop | `FLOP_FWD_PAIR` |" in text
-    assert bench.FLOP_BWD_PAIR == {3: 134, 4: 154} and "| 154 (134) flop | `FLOP_BWD_PAIR` |" in text
+    src = os.path.join(ROOT, bench.FLOP_SOURCE)
+    assert os.path.exists(src), bench.FLOP_SOURCE
+    prof = open(src).read()
+    design = open(os.path.join(ROOT, "DESIGN.md")).read()
+    for v in (bench.FLOP_PER_EVAL["forward"], bench.FLOP_PER_EVAL["backward"][3], bench.FLOP_PER_EVAL["backward"][4]):
+        assert ("%.1f" % v) in prof, v
+        assert ("%.1f" % v) in design, v
+    assert "FLOP_PER_EVAL" in design
+
+
+def test_reference_arm_says_what_it_ran():
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "0", "--steps", "1",
+                        "--warmup", "0"], capture_output=True, text=True, timeout=300, cwd=ROOT)
+    d = json.loads(r.stdout.strip().splitlines()[-1])
+    assert d["config"]["candidates_per_step"] == 4 and d["config"]["training_views"] == 1
+    assert d["config"]["workload_candidates"] == 4 and d["config"]["workload_training_views"] == 1
+    assert "cpu" in d["cpu_baseline"]

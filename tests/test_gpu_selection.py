@@ -19,6 +19,13 @@ def _workload(n_train, n_cand, W=96, H=80, n_gaussians=2000, seed=0):
     return wl
 
 
+def _nbv(scene, **kw):
+    from paper_2602_08266_b200 import api
+    n = api.NBV(**kw)
+    n.load_scene(scene)
+    return n
+
+
 def _ctx(scene, mask, train):
     from paper_2602_08266_b200 import api
     n = api.NBV(channel_mask=mask)
@@ -99,3 +106,36 @@ def test_greedy_edge_cases():
     with pytest.raises(api.NBVError) as e:
         nbv.select_greedy(wl.cand_cams[:0], 1)
     assert e.value.status == "NBV_ERR_EMPTY_CANDIDATES"
+
+
+# ---- alternative criteria: nbv_config.criterion
+def test_trace_and_det_criteria_match_the_oracle():
+    from oracle import criteria as crit
+    wl = synth.make_workload(0)
+    scn = make_oracle_scene(wl.scene)
+    for target in (-1, 1):
+        ref = crit.score_candidates(scn, wl.train_cams, wl.cand_cams, crit.TRACE, target=target)
+        nbv = _nbv(wl.scene, criterion=1)
+        nbv.accumulate_training(wl.train_cams)
+        s, best = nbv.score_candidates(wl.cand_cams, target_obj=target)
+        np.testing.assert_allclose(s.cpu().numpy(), ref["scores"], rtol=1e-3, atol=0)
+        assert int(best.item()) == ref["best"]
+        d = nbv.gaussian_gains(wl.cand_cams[2], target_obj=target).cpu().numpy()      # per-Gaussian trace reductions D_g
+        np.testing.assert_allclose(d, ref["terms"][2], rtol=1e-3, atol=1e-9)
+    # greedy selection under the trace criterion: first round = plain scoring, S_T refreshed every round
+    order, table = nbv.select_greedy(wl.cand_cams, 2, target_obj=1)
+    np.testing.assert_allclose(table.cpu().numpy()[0], ref["scores"], rtol=1e-3)
+    assert order[0] == ref["best"]
+    # determinant criterion: carried in the log domain (R-17), the numbers of the log-det criterion
+    nd, nl = _nbv(wl.scene, criterion=2), _nbv(wl.scene)
+    for n in (nd, nl):
+        n.accumulate_training(wl.train_cams)
+    sd, bd = nd.score_candidates(wl.cand_cams)
+    sl, bl = nl.score_candidates(wl.cand_cams)
+    np.testing.assert_allclose(sd.cpu().numpy(), sl.cpu().numpy(), rtol=2e-6)
+    assert int(bd.item()) == int(bl.item()) == crit.score_candidates(scn, wl.train_cams, wl.cand_cams, crit.DET)["best"]
+    from paper_2602_08266_b200 import api
+    with pytest.raises(api.NBVError):
+        api.NBV(criterion=1, weight_mode=1)
+    with pytest.raises(api.NBVError):
+        api.NBV(criterion=3)
