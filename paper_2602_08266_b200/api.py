@@ -182,7 +182,10 @@ class NBV:
     def load_sh(self, sh45):
         """nbv_load_sh: (N, 45) float32 SH coefficients of degree 1..3 (coefficient-major); blocks become 59 x 59"""
         torch = self._torch
-        t = torch.as_tensor(np.ascontiguousarray(sh45, dtype=np.float32).reshape(self.N, 45), device=self.device).contiguous()
+        a = np.ascontiguousarray(sh45, dtype=np.float32)
+        if a.size != self.N * 45:
+            raise ValueError("load_sh expects N x 45 coefficients for the %d Gaussians loaded, got %d values" % (self.N, a.size))
+        t = torch.as_tensor(a.reshape(-1), device=self.device).contiguous()
         self._check(self.lib.nbv_load_sh(self._h, _ptr(t), _stream()))
 
     def reset_training(self):

@@ -85,263 +85,341 @@ __device__ __forceinline__ double block_sum(double v, double* ws) {
   return t;
 }
 
-// ---- S5 + S6, ONE WARP PER TOUCHED GAUSSIAN, everything in shared memory (packed 105-double blocks, coalesced H_T rows).
-// A thread-per-Gaussian version kept ~3 KB of dynamically indexed binary64 arrays per thread in local memory; with a few
-// hundred resident threads per SM that working set fell out of the L1 and the kernel took 0.64 ms per 8-view batch for
-// 2e8 binary64 operations.  Here the 32 lanes share one Gaussian: lane k computes column k of the chain rule, the 66 + 44
-// entries of A Q and A x_ch and the 105 entries of H are dealt to the lanes, and the two L D L^T factorisations update the
-// trailing packed entries in parallel (one __syncwarp per pivot).
-constexpr int EXP_WARPS = 8;
-constexpr int EXP_T = EXP_WARPS * 32;
+// ---- S5 + S6, ONE THREAD PER TOUCHED GAUSSIAN, the 105-double blocks in shared memory.
+// Two earlier versions -- one thread per Gaussian with its arrays in local memory, then one warp per Gaussian with the
+// chain rule computed redundantly in every lane and dynamically indexed per-thread scratch -- both spent their time waiting
+// on LOCAL memory (ncu, profiles/r2b_ncu_expand.md: long-scoreboard 18.7 of 26 stall cycles per issue, 870k local stores per
+// view) and took 0.57 ms per 8-view batch for ~3e8 binary64 operations.  Here every array a thread indexes lives either in
+// registers with compile-time indices (all loops fully unrolled) or in shared memory: a block of 64 threads owns two
+// 64 x 105 binary64 arrays S0, S1 (row stride 105, odd: the 16 lanes of a 64-bit shared-memory phase hit 16 different
+// bank pairs).  A thread builds its Gaussian's block into its row of S1 (its row of S0 holds the 11 x 6 chain matrix A
+// meanwhile); then, per mode, the block stores the rows cooperatively and coalesced (TRAIN / VIEW / CACHE) or loads
+// c H_T + Lambda into S0 and c (H_T + H) + Lambda into S1 the same way and every thread factors its two rows in place
+// (GAIN): two interleaved right-looking L D L^T with the pivot row in registers.
+constexpr int TPG = 64;                              // threads = Gaussians per block
+constexpr int TPG_SMEM = 2 * TPG * NBLK * 8;         // bytes of dynamic shared memory
 
-struct WarpScratch {
-  double mom[NMOM];      // S4's moments (whitened basis)
-  double mu[NMOM];       // the same in the u basis
-  double A[11][6];
-  double AQ[11][6];
-  double yv[4][11];      // sqrt(omega_ch) A x_ch
-  double H[NBLK];        // the view's block
-  double M[NBLK];        // the matrix being factored
-  double piv0[P], piv1[P];
-  double dz[4];
-};
-
-// in-place L D L^T of the packed symmetric positive definite M, all lanes; pivots -> piv
-__device__ __forceinline__ void warp_ldl14(double* M, double* piv, const uint8_t* tr, const uint8_t* tc, int lane) {
-  for (int j = 0; j < P; ++j) {
-    __syncwarp();
-    const int jj = tri(j, j);
-    const double d = fmax(M[jj], 1e-300);
-    if (lane == 0) piv[j] = d;
-    const double inv = 1.0 / d;
-    for (int t = tri(j + 1, j + 1) + lane; t < NBLK; t += 32) {          // the rows below the pivot: contiguous in packed order
-      const int r = tr[t], c = tc[t];
-      M[t] = fma(-(M[jj + (r - j)] * inv), M[jj + (c - j)], M[t]);
-    }
-  }
-  __syncwarp();
+__device__ __forceinline__ double binom_d(int n, int k) {     // folds to a constant after unrolling
+  return (k == 0 || k == n) ? 1.0 : (n == 2) ? 2.0 : (n == 3) ? 3.0 : (k == 2) ? 6.0 : 4.0;
 }
 
-// trace(A^-1) from the factorisation warp_ldl14 left in M / piv: lane c solves L x = e_c
-__device__ __forceinline__ double warp_inverse_trace14(const double* M, const double* piv, int lane) {
-  double acc = 0.0;
-  if (lane < P) {
+// S4's 40 moments (whitened basis xi = L^-1 d) -> the u basis (u = L^-T xi: ux = p00 xi1 + p01 xi2, uy = p11 xi2):
+//   sum f ux^a uy^b = p11^b sum_t C(a,t) p00^(a-t) p01^t  sum f xi1^(a-t) xi2^(t+b)
+__device__ __forceinline__ void moments_whitened_to_u(const double (&m)[NMOM], double p00, double p01, double p11, double (&u)[NMOM]) {
+  double P0[5], P1[5], P2[5];
+  P0[0] = P1[0] = P2[0] = 1.0;
+#pragma unroll
+  for (int e = 1; e < 5; ++e) { P0[e] = P0[e - 1] * p00; P1[e] = P1[e - 1] * p01; P2[e] = P2[e - 1] * p11; }
+#pragma unroll
+  for (int n = 0; n <= 4; ++n)
+#pragma unroll
+    for (int b = 0; b <= n; ++b) {
+      const int a = n - b;
+      double v = 0.0;
+#pragma unroll
+      for (int t = 0; t <= a; ++t) v = fma(binom_d(a, t) * P0[a - t] * P1[t], m[mono_index(a - t, t + b)], v);
+      u[mono_index(a, b)] = v * P2[b];
+    }
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const int o = MOM_X + 6 * c;               // (xi1, xi2, xi1^2, xi1 xi2, xi2^2, 1) -> (ux, uy, ux^2, ux uy, uy^2, 1)
+    u[o + 0] = fma(p00, m[o + 0], p01 * m[o + 1]);
+    u[o + 1] = p11 * m[o + 1];
+    u[o + 2] = fma(P0[2], m[o + 2], fma(2.0 * p00 * p01, m[o + 3], P1[2] * m[o + 4]));
+    u[o + 3] = p11 * fma(p00, m[o + 3], p01 * m[o + 4]);
+    u[o + 4] = P2[2] * m[o + 4];
+    u[o + 5] = m[o + 5];
+  }
+  u[MOM_W2] = m[MOM_W2];
+}
+
+// structural non-zeros of A (11 x 6): position rows use (ux, uy, ux^2, ux uy, uy^2), log-scale and quaternion rows only the
+// quadratic monomials (they move Sigma2D, not the centre), the opacity row only the constant
+__device__ __forceinline__ constexpr bool a_nz(int k, int i) { return k < 3 ? i < 5 : k < 10 ? (i >= 2 && i < 5) : i == 5; }
+
+// S5 of one Gaussian: moments + chain rule -> packed 14 x 14 block H (row `Hrow` of S1); `Arow` (66 doubles) is scratch
+__device__ __forceinline__ void tpg_build_block(const SceneDev& sc, const nbv_config& cfg, const ExpandView& vw, uint32_t r, uint32_t g,
+                                                const float (&omega)[4], double* __restrict__ Arow, double* __restrict__ Hrow) {
+  double u[NMOM];
+  {
+    double m[NMOM];
+    float4* mom4 = reinterpret_cast<float4*>(vw.moments + (size_t)r * NMOM);
+#pragma unroll
+    for (int q = 0; q < NMOM / 4; ++q) {
+      const float4 v = mom4[q];
+      mom4[q] = make_float4(0.f, 0.f, 0.f, 0.f);             // leave the buffer zeroed for the next view
+      m[4 * q] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w;
+    }
+    // the whitening S4 used, from the splat's conic (-2 qa, -qb, -2 qc) = Sigma2D^-1
+    const float4 s0 = *reinterpret_cast<const float4*>(vw.splat_sorted + r);
+    const float4 s1 = *(reinterpret_cast<const float4*>(vw.splat_sorted + r) + 1);
+    const double cA = -2.0 * (double)s0.z, cB = -(double)s0.w, cC = -2.0 * (double)s1.x, icC = 1.0 / cC;
+    const double p00 = sqrt(fmax(cA * cC - cB * cB, 0.0) * icC), p11 = sqrt(cC), p01 = cB * icC * p11;
+    moments_whitened_to_u(m, p00, p01, p11, u);
+  }
+  double dz[3];
+  {
+    ChainPrefix<double> pf;
+    chain_prefix<double>(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, pf);
+#pragma unroll
+    for (int k = 0; k < 10; ++k) {
+      double col[5];
+      chain_column<double>(pf, k, col);
+      if (k < 3) { Arow[6 * k + 0] = col[0]; Arow[6 * k + 1] = col[1]; }
+      Arow[6 * k + 2] = 0.5 * col[2]; Arow[6 * k + 3] = col[3]; Arow[6 * k + 4] = 0.5 * col[4];
+    }
+    const double sg = (double)sc.sigma[g];
+    Arow[6 * 10 + 5] = cfg.opacity_coord == 0 ? (1.0 - sg) : 1.0 / sg;       // R-10
+#pragma unroll
+    for (int k = 0; k < 3; ++k) dz[k] = pf.W[6 + k];
+  }
+  const int ex[6] = {1, 0, 2, 1, 0, 0}, ey[6] = {0, 1, 0, 1, 2, 0};
+  const double W2 = u[MOM_W2];
+  const bool depth = omega[3] != 0.f;
+  // y_3[l] = sqrt(omega_3) A x_3 (depth channel; S4 delivers x_ch scaled by sqrt(omega_ch)): needed for every l by the rows k < 3
+  double y3[11];
+  if (depth) {
+    const double som = sqrt((double)omega[3]);
+#pragma unroll
+    for (int l = 0; l < 11; ++l) {
+      double v = 0.0;
+#pragma unroll
+      for (int i = 0; i < 6; ++i)
+        if (a_nz(l, i)) v = fma(Arow[6 * l + i], u[MOM_X + 18 + i], v);
+      y3[l] = som * v;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 11; ++k) {
+    double ak[6], aq[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) ak[i] = a_nz(k, i) ? Arow[6 * k + i] : 0.0;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {                               // row k of A Q
+      double v = 0.0;
+#pragma unroll
+      for (int i = 0; i < 6; ++i)
+        if (a_nz(k, i)) v = fma(ak[i], u[mono_index(ex[i] + ex[j], ey[i] + ey[j])], v);
+      aq[j] = v;
+    }
+#pragma unroll
+    for (int l = k; l < 11; ++l) {                              // H = A Q A^T + sum_ch [y e^T + e y^T + omega W2 e e^T]
+      double v = 0.0;
+#pragma unroll
+      for (int j = 0; j < 6; ++j)
+        if (a_nz(l, j)) v = fma(aq[j], l == k ? ak[j] : Arow[6 * l + j], v);
+      if (depth && k < 3) {                                     // depth: e = (dz/dmu, 0, ...)
+        const double el = l < 3 ? dz[l] : 0.0;
+        v += y3[k] * el + dz[k] * y3[l] + (double)omega[3] * W2 * dz[k] * el;
+      }
+      Hrow[tri(k, l)] = v;
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {                               // colour ch: e = unit vector on its parameter
+      double v = 0.0;
+      if (omega[c] != 0.f) {
+#pragma unroll
+        for (int i = 0; i < 6; ++i)
+          if (a_nz(k, i)) v = fma(ak[i], u[MOM_X + 6 * c + i], v);
+        v *= sqrt((double)omega[c]);
+      }
+      Hrow[tri(k, 11 + c)] = v;
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c)
+#pragma unroll
+    for (int d = c; d < 3; ++d) Hrow[tri(11 + c, 11 + d)] = c == d ? (double)omega[c] * W2 : 0.0;
+}
+
+// S6 on the thread's two rows: a0 = c H_T + Lambda, a1 = c (H_T + H) + Lambda (packed, destroyed).  Two interleaved
+// right-looking L D L^T; the pivot ratios d1_j / d0_j are multiplied up in two halves (each ratio is >= 1 up to rounding
+// and far below 1e20, so neither product leaves binary64 range) and enter as two logarithms.  The rows are accessed as
+// `volatile`: otherwise the compiler promotes the whole packed block to registers across the unrolled pivot steps and
+// spills it to local memory (2.4 KB of spill stores per thread).
+// TRACE: this Gaussian's reduction of trace(H^-1) instead, from the same factors.
+__device__ __forceinline__ double tpg_inverse_trace(const volatile double* a) {
+  // a = the rows U_j = d_j L_j^T left by the elimination; A^-1 = L^-T D^-1 L^-1, trace = sum_c sum_i x_i^2 / d_i, x = L^-1 e_c
+  double inv[P];
+#pragma unroll
+  for (int j = 0; j < P; ++j) inv[j] = 1.0 / fmax(a[tri(j, j)], 1e-300);
+  double tr = 0.0;
+#pragma unroll
+  for (int c = 0; c < P; ++c) {
     double x[P];
-    x[lane] = 1.0;
-    acc = 1.0 / piv[lane];
-    for (int i = lane + 1; i < P; ++i) {
-      double sacc = 0.0;
-      for (int j = lane; j < i; ++j) sacc = fma(M[tri(j, i)] / piv[j], x[j], sacc);
-      x[i] = -sacc;
-      acc = fma(sacc * sacc, 1.0 / piv[i], acc);
+    x[c] = 1.0;
+    double acc = inv[c];
+#pragma unroll
+    for (int i = c + 1; i < P; ++i) {
+      double s = 0.0;
+#pragma unroll
+      for (int j = c; j < i; ++j) s = fma(a[tri(j, i)] * inv[j], x[j], s);
+      x[i] = -s;
+      acc = fma(s * s, inv[i], acc);
+    }
+    tr += acc;
+  }
+  return tr;
+}
+
+template <bool TRACE>
+__device__ __forceinline__ double tpg_gain(volatile double* a0, volatile double* a1) {
+  double prod_lo = 1.0, prod_hi = 1.0;
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    const int jj = tri(j, j);
+    double r0[P], r1[P];                        // the pivot rows (compile-time indices: registers)
+#pragma unroll
+    for (int c = j; c < P; ++c) { r0[c] = a0[jj + c - j]; r1[c] = a1[jj + c - j]; }
+    const double d0 = fmax(r0[j], 1e-300), d1 = fmax(r1[j], 1e-300);
+    const double i0 = 1.0 / d0;
+    if (j < P / 2) prod_lo *= d1 * i0; else prod_hi *= d1 * i0;
+    if (j + 1 < P) {
+      const double i1 = 1.0 / d1;
+#pragma unroll
+      for (int r = j + 1; r < P; ++r) {
+        const double l0 = -r0[r] * i0, l1 = -r1[r] * i1;
+        const int rr = tri(r, r);
+#pragma unroll
+        for (int c = r; c < P; ++c) {
+          a0[rr + c - r] = fma(l0, r0[c], a0[rr + c - r]);
+          a1[rr + c - r] = fma(l1, r1[c], a1[rr + c - r]);
+        }
+      }
     }
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  return acc;
+  if (TRACE) return tpg_inverse_trace(a0) - tpg_inverse_trace(a1);
+  return log(prod_lo) + log(prod_hi);
 }
 
-// S6 for one block held in shared memory (ws.H) against H_T,g, all lanes; returns the term in every lane
-__device__ double warp_block_gain(const double* __restrict__ ht, WarpScratch& ws, double c, const nbv_config& cfg, const uint8_t* tr,
-                                  const uint8_t* tc, int lane) {
-  const double ct = cfg.weight_mode == 0 ? c : 1.0;          // Eq. 9 literal (R1) weights H_T as well; R2 / R3 do not
-  const double cb = cfg.weight_mode == 1 ? 1.0 : c;          // R2 weights the gain, R1 / R3 the candidate block
-  double hreg[4];
+// cooperative, coalesced: for the block's Gaussian i (id gs[i], confidence cs[i]):
+//   S0 row i = ct H_T,g + Lambda,   S1 row i = S0 row i + cb * S1 row i      (R-14: which of the two the confidence weights)
+__device__ __forceinline__ void tpg_load_combine(const double* __restrict__ H_T, const nbv_config& cfg, const uint32_t* gs, const double* cs,
+                                                 int n, double* S0, double* S1) {
+#pragma unroll 4
+  for (int i = 0; i < n; ++i) {
+    const double c = cs[i];
+    if (!(c > 0.0)) continue;
+    const double ct = cfg.weight_mode == 0 ? c : 1.0;          // Eq. 9 literal (R1) weights H_T as well; R2 / R3 do not
+    const double cb = cfg.weight_mode == 1 ? 1.0 : c;          // R2 weights the gain, R1 / R3 the candidate block
+    const double* ht = H_T + (size_t)gs[i] * NBLK;
+    for (int idx = threadIdx.x; idx < NBLK; idx += TPG) {
+      // packed index -> diagonal?  row r starts at tri(r, r)
+      int r = 0;
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int t = lane + 32 * i;
-    hreg[i] = t < NBLK ? ct * ht[t] : 0.0;
-    if (t < NBLK) ws.M[t] = hreg[i] + (tr[t] == tc[t] ? (double)cfg.prior_precision[tr[t]] : 0.0);
+      for (int q = 1; q < P; ++q) r += idx >= tri(q, q) ? 1 : 0;
+      const double m0 = fma(ct, ht[idx], idx == tri(r, r) ? (double)cfg.prior_precision[r] : 0.0);
+      S0[i * NBLK + idx] = m0;
+      S1[i * NBLK + idx] = fma(cb, S1[i * NBLK + idx], m0);
+    }
   }
-  warp_ldl14(ws.M, ws.piv0, tr, tc, lane);
-  const double t0 = cfg.criterion == NBV_CRIT_TRACE ? warp_inverse_trace14(ws.M, ws.piv0, lane) : 0.0;
-  __syncwarp();
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int t = lane + 32 * i;
-    if (t < NBLK) ws.M[t] = fma(cb, ws.H[t], hreg[i]) + (tr[t] == tc[t] ? (double)cfg.prior_precision[tr[t]] : 0.0);
-  }
-  warp_ldl14(ws.M, ws.piv1, tr, tc, lane);
-  if (cfg.criterion == NBV_CRIT_TRACE) return t0 - warp_inverse_trace14(ws.M, ws.piv1, lane);   // this Gaussian's reduction of trace(H^-1)
-  double gn = lane < P ? log(ws.piv1[lane] / ws.piv0[lane]) : 0.0;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) gn += __shfl_xor_sync(0xffffffffu, gn, o);
-  return cfg.weight_mode == 1 ? c * gn : gn;
 }
 
-// one entry of the basis change u = L^-T xi (ux = p00 xi1 + p01 xi2, uy = p11 xi2):
-//   sum f ux^a uy^b = p11^b sum_t C(a,t) p00^(a-t) p01^t  sum f xi1^(a-t) xi2^(t+b);   src[mono_index(i,j) - off] holds sum f xi1^i xi2^j
-__device__ __forceinline__ double ubasis_entry(int a, int b, const double* src, int off, double p00, double p01, double p11) {
-  const double binom[5][5] = {{1, 0, 0, 0, 0}, {1, 1, 0, 0, 0}, {1, 2, 1, 0, 0}, {1, 3, 3, 1, 0}, {1, 4, 6, 4, 1}};
-  double v = 0.0, pa = 1.0;                 // pa = p01^t
-  for (int t = 0; t <= a; ++t) {
-    double q = binom[a][t] * pa;
-    for (int e = 0; e < a - t; ++e) q *= p00;
-    v = fma(q, src[mono_index(a - t, t + b) - off], v);
-    pa *= p01;
-  }
-  for (int e = 0; e < b; ++e) v *= p11;
-  return v;
-}
-
-__global__ void __launch_bounds__(EXP_T) expand_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
-                                                        const __grid_constant__ ExpandBatch batch, int mode, int view0,
-                                                        double* __restrict__ H_T, const float* __restrict__ conf,
-                                                        uint32_t* __restrict__ cache_ids, double* __restrict__ cache_blocks,
-                                                        const double* __restrict__ trace_total) {
-  __shared__ WarpScratch scratch[EXP_WARPS];
-  __shared__ uint8_t tr[NBLK], tc[NBLK];
-  __shared__ double wsum[EXP_WARPS];
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  if (threadIdx.x < P) {                                      // packed index -> (row, column)
-    int t = tri(threadIdx.x, threadIdx.x);
-    for (int c = threadIdx.x; c < P; ++c, ++t) { tr[t] = (uint8_t)threadIdx.x; tc[t] = (uint8_t)c; }
-  }
-  __syncthreads();
-  WarpScratch& ws = scratch[wib];
+template <int MODE, bool TRACE>
+__global__ void __launch_bounds__(TPG) expand_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
+                                                      const __grid_constant__ ExpandBatch batch, int view0, double* __restrict__ H_T,
+                                                      const float* __restrict__ conf, uint32_t* __restrict__ cache_ids,
+                                                      double* __restrict__ cache_blocks, const double* __restrict__ trace_total) {
+  extern __shared__ __align__(16) double tpg_smem[];
+  double* S0 = tpg_smem;
+  double* S1 = tpg_smem + TPG * NBLK;
+  __shared__ uint32_t gs[TPG];
+  __shared__ double cs[TPG];
+  __shared__ double wsum[TPG / 32];
   const ExpandView& vw = batch.v[view0 + blockIdx.y];
   const uint32_t n_touched = vw.counters->n_touched;
   float omega[4];
 #pragma unroll
   for (int c = 0; c < 4; ++c) omega[c] = ((cfg.channel_mask >> c) & 1) ? cfg.channel_weight[c] : 0.f;
   double gain = 0.0;
-  for (uint32_t t = blockIdx.x * EXP_WARPS + wib; t < n_touched; t += gridDim.x * EXP_WARPS) {
-    const uint32_t r = vw.touched[t];
-    const uint32_t g = vw.ids_sorted[r];
-    __syncwarp();
-    if (lane < NMOM / 4) {
-      float4* mom4 = reinterpret_cast<float4*>(vw.moments + (size_t)r * NMOM) + lane;
-      const float4 v = *mom4;
-      *mom4 = make_float4(0.f, 0.f, 0.f, 0.f);                // leave the buffer zeroed for the next view
-      ws.mom[4 * lane] = v.x; ws.mom[4 * lane + 1] = v.y; ws.mom[4 * lane + 2] = v.z; ws.mom[4 * lane + 3] = v.w;
+  for (uint32_t base = blockIdx.x * TPG; base < n_touched; base += gridDim.x * TPG) {
+    const int n = (int)min((uint32_t)TPG, n_touched - base);
+    const bool valid = (int)threadIdx.x < n;
+    uint32_t g = 0;
+    __syncthreads();                                          // the previous chunk's rows are no longer read
+    if (valid) {
+      const uint32_t r = vw.touched[base + threadIdx.x];
+      g = vw.ids_sorted[r];
+      gs[threadIdx.x] = g;
+      if (MODE == EXPAND_GAIN) cs[threadIdx.x] = (double)conf[g];
+      tpg_build_block(sc, cfg, vw, r, g, omega, S0 + threadIdx.x * NBLK, S1 + threadIdx.x * NBLK);
     }
-    // the whitening S4 used, from the splat's conic (-2 qa, -qb, -2 qc) = Sigma2D^-1:  u = L^-T xi
-    const Splat sp = vw.splat_sorted[r];
-    const double cA = -2.0 * (double)sp.qa, cB = -(double)sp.qb, cC = -2.0 * (double)sp.qc, icC = 1.0 / cC;
-    const double p00 = sqrt(fmax(cA * cC - cB * cB, 0.0) * icC), p11 = sqrt(cC), p01 = cB * icC * p11;
-    __syncwarp();
-    if (lane < 15) {                                          // monomial sums: degree n, index j within the degree
-      const int n = lane < 1 ? 0 : lane < 3 ? 1 : lane < 6 ? 2 : lane < 10 ? 3 : 4;
-      const int j = lane - n * (n + 1) / 2;
-      ws.mu[lane] = ubasis_entry(n - j, j, ws.mom, 0, p00, p01, p11);
-    }
-    if (lane < 20) {                                          // cross moments of channel c: (ux, uy, ux^2, ux uy, uy^2 | 1)
-      const int c = lane / 5, e = lane - 5 * c;
-      const int ea[5] = {1, 0, 2, 1, 0}, eb[5] = {0, 1, 0, 1, 2};
-      ws.mu[MOM_X + 6 * c + e] = ubasis_entry(ea[e], eb[e], ws.mom + MOM_X + 6 * c, 1, p00, p01, p11);
-    } else if (lane < 24) {
-      ws.mu[MOM_X + 6 * (lane - 20) + 5] = ws.mom[MOM_X + 6 * (lane - 20) + 5];
-    } else if (lane == 24) {
-      ws.mu[MOM_W2] = ws.mom[MOM_W2];
-    }
-    // chain rule: the prefix in every lane, column k in lane k; row k of A (14 x 6)
-    {
-      ChainPrefix<double> pf;
-      chain_prefix<double>(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, pf);
-      if (lane < 10) {
-        double col[5];
-        chain_column<double>(pf, lane, col);
-        ws.A[lane][0] = col[0]; ws.A[lane][1] = col[1]; ws.A[lane][2] = 0.5 * col[2]; ws.A[lane][3] = col[3]; ws.A[lane][4] = 0.5 * col[4];
-        ws.A[lane][5] = 0.0;
-      } else if (lane == 10) {
-        const double sg = (double)sc.sigma[g];
-#pragma unroll
-        for (int e = 0; e < 5; ++e) ws.A[10][e] = 0.0;
-        ws.A[10][5] = cfg.opacity_coord == 0 ? (1.0 - sg) : 1.0 / sg;       // R-10
-      } else if (lane < 14) {
-        ws.dz[lane - 11] = pf.W[6 + lane - 11];
+    __syncthreads();
+    if (MODE == EXPAND_TRAIN) {
+      // one launch per view, in view order: a view lists a Gaussian once, so these are plain binary64 additions
+      for (int i = 0; i < n; ++i) {
+        double* dst = H_T + (size_t)gs[i] * NBLK;
+        for (int idx = threadIdx.x; idx < NBLK; idx += TPG) dst[idx] += S1[i * NBLK + idx];
       }
-    }
-    __syncwarp();
-    {
-      const int ex[6] = {1, 0, 2, 1, 0, 0}, ey[6] = {0, 1, 0, 1, 2, 0};
-      for (int idx = lane; idx < 66; idx += 32) {             // A Q
-        const int k = idx / 6, j = idx - 6 * k;
-        double v = 0.0;
-#pragma unroll
-        for (int i = 0; i < 6; ++i) v = fma(ws.A[k][i], ws.mu[mono_index(ex[i] + ex[j], ey[i] + ey[j])], v);
-        ws.AQ[k][j] = v;
+    } else if (MODE == EXPAND_VIEW) {
+      for (int i = 0; i < n; ++i) {
+        float* dst = vw.out_blocks + (size_t)gs[i] * NBLK;
+        for (int idx = threadIdx.x; idx < NBLK; idx += TPG) dst[idx] = (float)S1[i * NBLK + idx];
       }
-      for (int idx = lane; idx < 44; idx += 32) {             // sqrt(omega_ch) A x_ch (S4 delivers x_ch scaled by sqrt(omega_ch))
-        const int c = idx / 11, k = idx - 11 * c;
-        double v = 0.0;
-#pragma unroll
-        for (int i = 0; i < 6; ++i) v = fma(ws.A[k][i], ws.mu[MOM_X + 6 * c + i], v);
-        ws.yv[c][k] = sqrt((double)omega[c]) * v;
-      }
-    }
-    __syncwarp();
-    const double W2 = ws.mu[MOM_W2];
-    for (int idx = lane; idx < NBLK; idx += 32) {             // H = A Q A^T + sum_ch [y e^T + e y^T + omega W2 e e^T]
-      const int rr = tr[idx], cc = tc[idx];
-      double v = 0.0;
-      if (cc < 11) {
-#pragma unroll
-        for (int j = 0; j < 6; ++j) v = fma(ws.AQ[rr][j], ws.A[cc][j], v);
-        if (omega[3] != 0.f) {                                // depth: e = (dz/dmu, 0, ...)
-          const double ek = rr < 3 ? ws.dz[rr] : 0.0, el = cc < 3 ? ws.dz[cc] : 0.0;
-          v += ws.yv[3][rr] * el + ek * ws.yv[3][cc] + (double)omega[3] * W2 * ek * el;
-        }
-      } else if (rr < 11) {
-        v = omega[cc - 11] != 0.f ? ws.yv[cc - 11][rr] : 0.0;  // colour ch: e = unit vector on its parameter
-      } else if (rr == cc) {
-        v = (double)omega[rr - 11] * W2;
-      }
-      ws.H[idx] = v;
-    }
-    __syncwarp();
-    if (mode == EXPAND_TRAIN) {
-      double* dst = H_T + (size_t)g * NBLK;                   // one launch per view, in view order: a view lists a Gaussian once
-      for (int idx = lane; idx < NBLK; idx += 32) dst[idx] += ws.H[idx];
-    } else if (mode == EXPAND_VIEW) {
-      float* dst = vw.out_blocks + (size_t)g * NBLK;
-      for (int idx = lane; idx < NBLK; idx += 32) dst[idx] = (float)ws.H[idx];
-    } else if (mode == EXPAND_CACHE) {
-      if (t < vw.cache_span[1]) {                              // span[1] = 0 when the pool overflowed: nothing is stored
-        const size_t e = (size_t)vw.cache_span[0] + t;
-        if (lane == 0) cache_ids[e] = g;
+    } else if (MODE == EXPAND_CACHE) {
+      // span[1] = 0 when the pool overflowed: nothing is stored
+      for (int i = 0; i < n; ++i) {
+        if (base + i >= vw.cache_span[1]) break;
+        const size_t e = (size_t)vw.cache_span[0] + base + i;
+        if (threadIdx.x == 0) cache_ids[e] = gs[i];
         double* dst = cache_blocks + e * NBLK;
-        for (int idx = lane; idx < NBLK; idx += 32) dst[idx] = ws.H[idx];
+        for (int idx = threadIdx.x; idx < NBLK; idx += TPG) dst[idx] = S1[i * NBLK + idx];
       }
     } else {
-      const double c = (double)conf[g];
+      tpg_load_combine(H_T, cfg, gs, cs, n, S0, S1);
+      __syncthreads();
       double gn = 0.0;
-      if (c > 0.0) gn = warp_block_gain(H_T + (size_t)g * NBLK, ws, c, cfg, tr, tc, lane);   // c_g = 0 (Eq. 12): exactly zero gain
-      if (lane == 0 && vw.gains) vw.gains[g] = (float)gn;
+      if (valid) {
+        const double c = cs[threadIdx.x];
+        if (c > 0.0) {                                          // c_g = 0 (Eq. 12): exactly zero gain
+          gn = tpg_gain<TRACE>(S0 + threadIdx.x * NBLK, S1 + threadIdx.x * NBLK);
+          if (cfg.weight_mode == 1) gn *= c;
+        }
+        if (vw.gains) vw.gains[g] = (float)gn;
+      }
       gain += gn;
     }
   }
-  if (mode == EXPAND_GAIN) {
-    if (lane == 0) wsum[wib] = gain;
+  if (MODE == EXPAND_GAIN) {
     __syncthreads();
-    double tot = 0.0;
-    if (threadIdx.x == 0)
-      for (int w = 0; w < EXP_WARPS; ++w) tot += wsum[w];
+    const double tot = block_sum<TPG>(gain, wsum);
     ordered_score(tot, vw.partials, &vw.counters->n_expanded, vw.score, trace_total);
   }
 }
 
+// blocks per view: at most two resident blocks per SM over the whole batch, and never more than the partial buffers hold
 static int expand_blocks(int N, int n_views) {
-  int blocks = (N + EXP_WARPS - 1) / EXP_WARPS;
-  const int cap = (sm_count() * 8 + n_views - 1) / n_views;
+  const int blocks = (N + TPG - 1) / TPG;
+  const int cap = std::min(expand_partials(), (sm_count() * 2 + n_views - 1) / n_views);
   return std::max(1, std::min(blocks, cap));
 }
 int expand_partials() { return sm_count() * 8; }
+
+template <int MODE, bool TRACE>
+static void launch_expand_mode(dim3 grid, const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int view0, double* H_T,
+                               const float* conf, uint32_t* cache_ids, double* cache_blocks, const double* trace_total, cudaStream_t st) {
+  // the attribute is per device and per function; setting it is cheap and idempotent
+  if (cudaFuncSetAttribute(expand_kernel<MODE, TRACE>, cudaFuncAttributeMaxDynamicSharedMemorySize, TPG_SMEM) != cudaSuccess) return;
+  ++g_kernel_launches;
+  expand_kernel<MODE, TRACE><<<grid, TPG, TPG_SMEM, st>>>(sc, cfg, batch, view0, H_T, conf, cache_ids, cache_blocks, trace_total);
+}
 
 void launch_expand(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, double* H_T, const float* conf,
                    const double* trace_total, cudaStream_t st) {
   if (mode == EXPAND_TRAIN) {
     // H_T += H(view), view after view (Eq. 6): a fixed order of binary64 additions, no atomics
-    const int blocks = expand_blocks(sc.N, 1);
-    for (int v = 0; v < batch.n; ++v) {
-      ++g_kernel_launches;
-      expand_kernel<<<dim3((unsigned)blocks, 1u), EXP_T, 0, st>>>(sc, cfg, batch, mode, v, H_T, conf, nullptr, nullptr, nullptr);
-    }
+    const dim3 grid((unsigned)expand_blocks(sc.N, 1), 1u);
+    for (int v = 0; v < batch.n; ++v)
+      launch_expand_mode<EXPAND_TRAIN, false>(grid, sc, cfg, batch, v, H_T, conf, nullptr, nullptr, nullptr, st);
     return;
   }
-  ++g_kernel_launches;
-  expand_kernel<<<dim3((unsigned)expand_blocks(sc.N, batch.n), (unsigned)batch.n), EXP_T, 0, st>>>(
-      sc, cfg, batch, mode, 0, H_T, conf, nullptr, nullptr, cfg.criterion == NBV_CRIT_TRACE ? trace_total : nullptr);
+  const dim3 grid((unsigned)expand_blocks(sc.N, batch.n), (unsigned)batch.n);
+  if (mode == EXPAND_VIEW)
+    launch_expand_mode<EXPAND_VIEW, false>(grid, sc, cfg, batch, 0, H_T, conf, nullptr, nullptr, nullptr, st);
+  else if (cfg.criterion == NBV_CRIT_TRACE)
+    launch_expand_mode<EXPAND_GAIN, true>(grid, sc, cfg, batch, 0, H_T, conf, nullptr, nullptr, trace_total, st);
+  else
+    launch_expand_mode<EXPAND_GAIN, false>(grid, sc, cfg, batch, 0, H_T, conf, nullptr, nullptr, nullptr, st);
 }
 
 // ---- sparse block cache of greedy selection ----------------------------------------------------------------------
@@ -368,48 +446,53 @@ void launch_cache_reserve(const ExpandBatch& batch, const BlockCache& cache, int
 }
 
 void launch_expand_cache(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, const BlockCache& cache, cudaStream_t st) {
-  ++g_kernel_launches;
-  expand_kernel<<<dim3((unsigned)expand_blocks(sc.N, batch.n), (unsigned)batch.n), EXP_T, 0, st>>>(sc, cfg, batch, EXPAND_CACHE, 0, nullptr,
-                                                                                                     nullptr, cache.ids, cache.blocks, nullptr);
+  const dim3 grid((unsigned)expand_blocks(sc.N, batch.n), (unsigned)batch.n);
+  launch_expand_mode<EXPAND_CACHE, false>(grid, sc, cfg, batch, 0, nullptr, nullptr, cache.ids, cache.blocks, nullptr, st);
 }
 
-// One warp per cached (candidate, Gaussian) entry: the gain of Eq. 5/6/9 of that block against the current H_T,g.
+// One thread per cached (candidate, Gaussian) entry: the gain of Eq. 5/6/9 of that block against the current H_T,g
+// (the S6 of expand_kernel on blocks read back from the pool instead of rebuilt).
 constexpr int CG_BLOCKS = 64;
-__global__ void __launch_bounds__(EXP_T) cached_gain_kernel(BlockCache cache, const __grid_constant__ nbv_config cfg,
-                                                            const int32_t* __restrict__ taken, const float* __restrict__ conf,
-                                                            const double* __restrict__ H_T, float* __restrict__ scores,
-                                                            double* __restrict__ partials, unsigned int* __restrict__ done,
-                                                            const double* __restrict__ trace_total) {
-  __shared__ WarpScratch scratch[EXP_WARPS];
-  __shared__ uint8_t tr[NBLK], tc[NBLK];
-  __shared__ double wsum[EXP_WARPS];
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  if (threadIdx.x < P) {
-    int t = tri(threadIdx.x, threadIdx.x);
-    for (int c = threadIdx.x; c < P; ++c, ++t) { tr[t] = (uint8_t)threadIdx.x; tc[t] = (uint8_t)c; }
-  }
-  __syncthreads();
-  WarpScratch& ws = scratch[wib];
+template <bool TRACE>
+__global__ void __launch_bounds__(TPG) cached_gain_kernel(BlockCache cache, const __grid_constant__ nbv_config cfg,
+                                                          const int32_t* __restrict__ taken, const float* __restrict__ conf,
+                                                          const double* __restrict__ H_T, float* __restrict__ scores,
+                                                          double* __restrict__ partials, unsigned int* __restrict__ done,
+                                                          const double* __restrict__ trace_total) {
+  extern __shared__ __align__(16) double tpg_smem[];
+  double* S0 = tpg_smem;
+  double* S1 = tpg_smem + TPG * NBLK;
+  __shared__ uint32_t gs[TPG];
+  __shared__ double cs[TPG];
+  __shared__ double wsum[TPG / 32];
   const int c = blockIdx.y;
   double gain = 0.0;
   if (!taken[c]) {
-    const uint32_t base = cache.spans[2 * c], cnt = cache.spans[2 * c + 1];
-    for (uint32_t t = blockIdx.x * EXP_WARPS + wib; t < cnt; t += gridDim.x * EXP_WARPS) {
-      const size_t e = (size_t)base + t;
-      const uint32_t g = cache.ids[e];
-      const double cg = (double)conf[g];
-      if (!(cg > 0.0)) continue;
-      __syncwarp();
-      for (int idx = lane; idx < NBLK; idx += 32) ws.H[idx] = cache.blocks[e * NBLK + idx];
-      __syncwarp();
-      gain += warp_block_gain(H_T + (size_t)g * NBLK, ws, cg, cfg, tr, tc, lane);
+    const uint32_t first = cache.spans[2 * c], cnt = cache.spans[2 * c + 1];
+    for (uint32_t base = blockIdx.x * TPG; base < cnt; base += gridDim.x * TPG) {
+      const int n = (int)min((uint32_t)TPG, cnt - base);
+      __syncthreads();
+      if ((int)threadIdx.x < n) {
+        const uint32_t g = cache.ids[(size_t)first + base + threadIdx.x];
+        gs[threadIdx.x] = g;
+        cs[threadIdx.x] = (double)conf[g];
+      }
+      const double* src = cache.blocks + ((size_t)first + base) * NBLK;            // n consecutive blocks: one coalesced copy
+      for (int i = threadIdx.x; i < n * NBLK; i += TPG) S1[i] = src[i];
+      __syncthreads();
+      tpg_load_combine(H_T, cfg, gs, cs, n, S0, S1);
+      __syncthreads();
+      if ((int)threadIdx.x < n) {
+        const double cg = cs[threadIdx.x];
+        if (cg > 0.0) {
+          const double gn = tpg_gain<TRACE>(S0 + threadIdx.x * NBLK, S1 + threadIdx.x * NBLK);
+          gain += cfg.weight_mode == 1 ? cg * gn : gn;
+        }
+      }
     }
   }
-  if (lane == 0) wsum[wib] = gain;
   __syncthreads();
-  double tot = 0.0;
-  if (threadIdx.x == 0)
-    for (int w = 0; w < EXP_WARPS; ++w) tot += wsum[w];
+  const double tot = block_sum<TPG>(gain, wsum);
   ordered_score(tot, partials + (size_t)c * CG_BLOCKS, done + c, scores + c, trace_total);
 }
 
@@ -420,8 +503,14 @@ void launch_cached_gain(const BlockCache& cache, const nbv_config& cfg, int n_ca
   ++g_kernel_launches;
   double* partials = reinterpret_cast<double*>(scratch);
   unsigned int* done = reinterpret_cast<unsigned int*>(partials + (size_t)n_cand * CG_BLOCKS);     // zero on entry, zero on exit
-  cached_gain_kernel<<<dim3(CG_BLOCKS, (unsigned)n_cand), EXP_T, 0, st>>>(cache, cfg, taken, conf, H_T, scores, partials, done,
-                                                                          cfg.criterion == NBV_CRIT_TRACE ? trace_total : nullptr);
+  const dim3 grid(CG_BLOCKS, (unsigned)n_cand);
+  if (cfg.criterion == NBV_CRIT_TRACE) {
+    if (cudaFuncSetAttribute(cached_gain_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TPG_SMEM) != cudaSuccess) return;
+    cached_gain_kernel<true><<<grid, TPG, TPG_SMEM, st>>>(cache, cfg, taken, conf, H_T, scores, partials, done, trace_total);
+  } else {
+    if (cudaFuncSetAttribute(cached_gain_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TPG_SMEM) != cudaSuccess) return;
+    cached_gain_kernel<false><<<grid, TPG, TPG_SMEM, st>>>(cache, cfg, taken, conf, H_T, scores, partials, done, nullptr);
+  }
 }
 
 __global__ void __launch_bounds__(256) cache_accumulate_kernel(BlockCache cache, const int32_t* __restrict__ pick, double* __restrict__ H_T) {

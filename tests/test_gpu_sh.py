@@ -74,7 +74,11 @@ def test_sh_zero_coefficients_and_reload():
     H14 = orc.unpack_blocks(base.view_hessian(cam).cpu().numpy().astype(np.float64))
     sc = np.sqrt(np.einsum("nii->ni", H14))[:, :, None] * np.sqrt(np.einsum("nii->ni", H14))[:, None, :] + 1e-3
     assert np.max(np.abs(H59[:, :14, :14] - H14) / sc) < 1e-5
+    mctx = api.NBV(channel_mask=api.CH_MASK)
+    with pytest.raises(ValueError):
+        mctx.load_sh(k)                                   # nothing loaded yet: the binding refuses the size
+    mctx.load_scene(wl.scene)
     with pytest.raises(api.NBVError):
-        api.NBV(channel_mask=api.CH_MASK).load_sh(k)
+        mctx.load_sh(k)                                   # the library refuses SH colour on the object-mask output
     nbv.load_scene(wl.scene)
     assert nbv.block_size() == 105
