@@ -373,6 +373,18 @@ def main():
         flush.fill_(1)
         nbv.score_candidates(wl.cand_cams, wl.target_obj, scores, best)
     stage_ms, n_timed_views = nbv.stage_times()
+    # ---- and once more ONE BATCH PER CALL: in the full call the S3 launch of batch b+1 shares the SMs with the S4 launch of
+    # batch b (two raster streams), so a launch's event-to-event duration there includes time the other kernel ran; with one
+    # batch per call every raster launch has the GPU to itself and its duration is the kernel's own (`roofline` uses these) ----
+    W_, H_ = int(wl.cand_cams[0]["width"]), int(wl.cand_cams[0]["height"])
+    vpl = args.concurrency or (16 if ((W_ + 15) // 16) * ((H_ + 15) // 16) < 2000 else VIEWS_PER_LAUNCH)
+    vpl = min(vpl, C)
+    nbv.set_stage_timing(True)                          # clears the accumulated times of the pass above
+    for _ in range(args.steps):
+        flush.fill_(1)
+        for c0 in range(0, C, vpl):
+            nbv.score_candidates(wl.cand_cams[c0:c0 + vpl], wl.target_obj, scores[c0:c0 + vpl], best)
+    stage_ms_x, n_timed_views_x = nbv.stage_times()
     nbv.set_stage_timing(False)
 
     # ---- e2e: host cameras in, host scores out, through nbv_score_candidates_host ----
@@ -414,6 +426,7 @@ def main():
     nch = 4 if wl.channel_mask & 8 else 3
     views = max(n_timed_views, 1)
     per_view_ms = {k: v / views for k, v in stage_ms.items()}
+    per_view_ms_x = {k: v / max(n_timed_views_x, 1) for k, v in stage_ms_x.items()}       # one batch per call: exclusive
     avg = {k: v / C for k, v in tot.items()}            # per view
     evals = avg["n_entries"] * 256.0                    # (pixel, list entry) evaluations per view
     n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
@@ -425,22 +438,23 @@ def main():
     }
     rl = {}
     for k, (bound, amount, peak, unit) in work.items():
-        sec = per_view_ms[k] * 1e-3
-        ach = amount / sec if sec > 0 else 0.0
         batched = k in ("backward", "forward")
-        W_, H_ = int(wl.cand_cams[0]["width"]), int(wl.cand_cams[0]["height"])
-        vpl = args.concurrency or (16 if ((W_ + 15) // 16) * ((H_ + 15) // 16) < 2000 else VIEWS_PER_LAUNCH)
-        vpl = min(vpl, C)
+        sec = (per_view_ms_x[k] if batched else per_view_ms[k]) * 1e-3
+        ach = amount / sec if sec > 0 else 0.0
         rl[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
                  "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(k),
                  "traffic_source": TRAFFIC_SOURCE if NCU_TRAFFIC_BYTES.get(args.config, {}).get(k) else None,
                  "flops_source": ("executed fp32 flop per evaluation from " + FLOP_SOURCE) if batched else None,
                  "views_per_launch": vpl if batched else 1,
-                 "ms_per_launch": per_view_ms[k] * (vpl if batched else 1), "peak_source": peaks["source"] if bound == "hbm" else
+                 "ms_per_launch": (per_view_ms_x[k] * vpl) if batched else per_view_ms[k],
+                 "ms_per_launch_in_full_call": per_view_ms[k] * (vpl if batched else 1),
+                 "timing": ("CUDA events around the launch on its own stream, one batch per call (the launch has the GPU to itself); "
+                            "in the full call launches of two batches overlap: ms_per_launch_in_full_call") if batched else
+                           "CUDA events on the slot stream in the full call", "peak_source": peaks["source"] if bound == "hbm" else
                  "%d SM x 128 lanes x 2 x %.0f MHz (DESIGN.md section 8)" % (n_sm, peaks["sm_max_mhz"])}
     # dominant kernel = largest share of GPU time in the ncu launch list (profiles/): one of the two raster stages; the
     # S1-S2 stage times are taken on slot streams that wait behind the raster launches and are not exclusive
-    dominant = max(("backward", "forward"), key=lambda k: per_view_ms[k])
+    dominant = max(("backward", "forward"), key=lambda k: per_view_ms_x[k])
     roofline = dict(rl[dominant], kernel=dominant)
     if roofline["bound"] == "alu":
         roofline["peak_measured_ffma"] = ffma_tflops
@@ -460,6 +474,7 @@ def main():
         "gpu_launches": int(launches),
         "roofline": roofline,
         "stage_ms_per_view": per_view_ms,
+        "stage_ms_per_view_exclusive": per_view_ms_x,
         "stage_rooflines": rl,
         "view_roofline": {"t_min_ms": t_min_ms, "t_measured_ms": view_ms, "frac": t_min_ms / view_ms if view_ms else None,
                           "note": "sum over stages of (executed fp32 work or algorithmic bytes / peak) against wall time per view"},

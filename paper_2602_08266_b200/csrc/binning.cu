@@ -15,43 +15,57 @@
 
 namespace nbv {
 
-__device__ __forceinline__ uint32_t coarse_count(ushort4 rc, int sshift) {
-  if (rc.z <= rc.x || rc.w <= rc.y) return 0u;
-  const uint32_t sx0 = rc.x >> sshift, sx1 = ((uint32_t)rc.z - 1u) >> sshift;
-  const uint32_t sy0 = rc.y >> sshift, sy1 = ((uint32_t)rc.w - 1u) >> sshift;
-  return (sx1 - sx0 + 1u) * (sy1 - sy0 + 1u);
-}
-
 // tile rect -> inclusive supertile rect (x0, y0, x1, y1); an empty tile rect gives x0 > x1 (covers nothing)
 __device__ __forceinline__ uint4 super_rect(ushort4 rc, int sshift) {
   if (rc.z <= rc.x || rc.w <= rc.y) return make_uint4(1u, 1u, 0u, 0u);
   return make_uint4(rc.x >> sshift, rc.y >> sshift, ((uint32_t)rc.z - 1u) >> sshift, ((uint32_t)rc.w - 1u) >> sshift);
 }
-__device__ __forceinline__ bool covers_super(uint4 sr, uint32_t sx, uint32_t sy) {
-  return sx >= sr.x && sx <= sr.z && sy >= sr.y && sy <= sr.w;
+// Coverage of a supertile rect as a bit mask over the (at most 256) supertiles, row-major: bit s of word s / 32.
+constexpr int MS_WORDS = 8;
+__device__ __forceinline__ void super_mask(uint4 sr, int super_x, int words, uint32_t (&cm)[MS_WORDS]) {
+#pragma unroll
+  for (int w = 0; w < MS_WORDS; ++w) cm[w] = 0u;
+  if (sr.x > sr.z) return;
+  const uint32_t len = sr.z - sr.x + 1u;
+  for (uint32_t sy = sr.y; sy <= sr.w; ++sy) {
+    const uint32_t lo = sy * (uint32_t)super_x + sr.x, hi = lo + len;       // bits [lo, hi)
+#pragma unroll
+    for (int w = 0; w < MS_WORDS; ++w) {
+      if (w < words) {
+        const uint32_t a = max(lo, 32u * w), e = min(hi, 32u * w + 32u);
+        if (a < e) cm[w] |= (e - a == 32u ? 0xffffffffu : ((1u << (e - a)) - 1u) << (a - 32u * w));
+      }
+    }
+  }
 }
-// bit s of the result = the supertile rect touches supertile s (row-major index); for grids of at most 64 supertiles the
-// per-supertile loops below test one bit instead of four comparisons
-__device__ __forceinline__ unsigned long long super_mask64(uint4 sr, int super_x) {
-  unsigned long long m = 0ull;
-  if (sr.x > sr.z) return m;
-  const unsigned long long row = ((2ull << (sr.z - sr.x)) - 1ull) << sr.x;      // columns x0..x1 of one row
-  for (uint32_t sy = sr.y; sy <= sr.w; ++sy) m |= row << (sy * (uint32_t)super_x);
-  return m;
+
+// 32 x 32 bit-matrix transpose across the warp: lane i gives row i and receives column i (bit c of the result = bit i of
+// lane c's input).  Applied to the lanes' coverage words it yields, in lane i, the ballot "which lanes touch supertile
+// 32 w + i" -- 5 shuffles per 32 supertiles instead of 32 votes.
+__device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane) {
+#pragma unroll
+  for (int j = 16; j > 0; j >>= 1) {
+    const uint32_t m = j == 16 ? 0x0000ffffu : j == 8 ? 0x00ff00ffu : j == 4 ? 0x0f0f0f0fu : j == 2 ? 0x33333333u : 0x55555555u;
+    const uint32_t y = __shfl_xor_sync(0xffffffffu, x, j);
+    x = (lane & j) ? ((x & ~m) | ((y >> j) & m)) : ((x & m) | ((y << j) & ~m));
+  }
+  return x;
 }
 
 // Stable multi-split of the ranks into supertile lists, without materialising unsorted keys: block b owns the ranks
 // [b * MS_T, (b + 1) * MS_T).  Pass 1 (this kernel, fused with the gather of the splats into rank order) counts, per
 // supertile, the block's ranks that touch it; an exclusive scan of the (supertile-major) count table gives the start of
 // every (supertile, block) segment; pass 2 writes each (supertile, rank) key and its tile rect at
-// segment start + (number of earlier ranks of the block touching the same supertile), found with warp ballots.
+// segment start + (number of earlier ranks of the block touching the same supertile).
 // Rank order inside a supertile is preserved by construction: the lists are in depth order.
+// Both passes were issue-bound on one vote per (warp, supertile) (ncu r2c: 64-106 M warp instructions per 8-view batch);
+// now a warp transposes its 32 coverage masks, which gives every per-supertile lane mask at once.
 constexpr int MS_T = 1024;
 constexpr int MS_W = MS_T / 32;
 
 __global__ void __launch_bounds__(MS_T) msplit_count_kernel(const __grid_constant__ PreBatch batch, int N, int sshift, int super_x,
                                                             int n_super, uint32_t nblk) {
-  __shared__ uint32_t cnt[256];
+  __shared__ uint16_t wc[256][MS_W + 2];     // [supertile][warp]; row stride 34 halves = 17 words (odd): conflict-free column sums
   const PreView& pv = batch.v[blockIdx.y];
   const uint32_t* __restrict__ ids_sorted = pv.ids[0];
   const Splat* __restrict__ splat = pv.splat;
@@ -59,9 +73,8 @@ __global__ void __launch_bounds__(MS_T) msplit_count_kernel(const __grid_constan
   Splat* __restrict__ splat_sorted = pv.splat_sorted;
   ushort4* __restrict__ rect_sorted = pv.rect_sorted;
   uint32_t* __restrict__ counts = pv.counts;
-  const int r = blockIdx.x * MS_T + threadIdx.x, lane = threadIdx.x & 31;
-  if (threadIdx.x < 256) cnt[threadIdx.x] = 0;
-  __syncthreads();
+  const int r = blockIdx.x * MS_T + threadIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int words = (n_super + 31) >> 5;
   ushort4 rc = make_ushort4(0, 0, 0, 0);
   if (r < N) {
     const uint32_t g = ids_sorted[r];
@@ -73,22 +86,18 @@ __global__ void __launch_bounds__(MS_T) msplit_count_kernel(const __grid_constan
     dst[1] = src[1];
     dst[2] = src[2];
   }
-  const uint4 sr = super_rect(rc, sshift);
-  if (n_super <= 64) {
-    const unsigned long long cm = super_mask64(sr, super_x);
-    for (int s = 0; s < n_super; ++s) {
-      const unsigned m = __ballot_sync(0xffffffffu, (cm >> s) & 1ull);
-      if (lane == 0 && m) atomicAdd(&cnt[s], (uint32_t)__popc(m));
-    }
-  } else {
-    for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {          // (sx, sy) walk the supertiles row-major: no division
-      const unsigned m = __ballot_sync(0xffffffffu, covers_super(sr, (uint32_t)sx, (uint32_t)sy));
-      if (lane == 0 && m) atomicAdd(&cnt[s], (uint32_t)__popc(m));
-      if (++sx == super_x) { sx = 0; ++sy; }
-    }
-  }
+  uint32_t cm[MS_WORDS];
+  super_mask(super_rect(rc, sshift), super_x, words, cm);
+#pragma unroll
+  for (int k = 0; k < MS_WORDS; ++k)
+    if (k < words) wc[32 * k + lane][w] = (uint16_t)__popc(transpose32(cm[k], lane));
   __syncthreads();
-  if ((int)threadIdx.x < n_super) counts[(size_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
+  if ((int)threadIdx.x < n_super) {
+    uint32_t c = 0;
+#pragma unroll
+    for (int k = 0; k < MS_W; ++k) c += wc[threadIdx.x][k];
+    counts[(size_t)threadIdx.x * nblk + blockIdx.x] = c;
+  }
 }
 
 __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const __grid_constant__ PreBatch batch, int N, int sshift, int super_x,
@@ -100,29 +109,38 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const __grid_constan
   uint32_t* __restrict__ keys = pv.ckeys;
   ushort4* __restrict__ crect = pv.crect;
   uint2* __restrict__ ranges = pv.cranges;
-  __shared__ uint16_t wc[256][MS_W];         // per supertile: ranks of warp w touching it, then the exclusive prefix over warps
-  __shared__ uint32_t seg[256];              // start of this block's segment in every supertile list (one global load each,
-                                             // up front: a load inside the write loop would stall every iteration on the L2)
+  extern __shared__ __align__(16) uint32_t ms_smem[];
+  // per supertile: start of this block's segment in its list + the ranks of earlier warps touching it (seg), and per
+  // (warp, supertile) the lanes of that warp touching it (bm)
+  uint32_t* seg = ms_smem;                              // [n_super]
+  uint32_t* bm = ms_smem + 256;                         // [MS_W][n_super]
+  uint16_t* wc = reinterpret_cast<uint16_t*>(bm + MS_W * n_super);      // [n_super][MS_W + 2]
   const int r = blockIdx.x * MS_T + threadIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int words = (n_super + 31) >> 5;
   const uint32_t lt = (1u << lane) - 1u;
   const ushort4 rc = r < N ? rect_sorted[r] : make_ushort4(0, 0, 0, 0);
-  const uint4 sr = super_rect(rc, sshift);
-  const bool small = n_super <= 64;
-  const unsigned long long cm = small ? super_mask64(sr, super_x) : 0ull;
-  for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {
-    const bool c = small ? ((cm >> s) & 1ull) != 0ull : covers_super(sr, (uint32_t)sx, (uint32_t)sy);
-    const unsigned m = __ballot_sync(0xffffffffu, c);
-    if (lane == 0) wc[s][w] = (uint16_t)__popc(m);
-    if (!small && ++sx == super_x) { sx = 0; ++sy; }
-  }
+  uint32_t cm[MS_WORDS];
+  super_mask(super_rect(rc, sshift), super_x, words, cm);
+#pragma unroll
+  for (int k = 0; k < MS_WORDS; ++k)
+    if (k < words) {                                    // uniform over the warp: the shuffles inside are warp-wide
+      const uint32_t m = transpose32(cm[k], lane);
+      if (32 * k + lane < n_super) {
+        bm[w * n_super + 32 * k + lane] = m;
+        wc[(32 * k + lane) * (MS_W + 2) + w] = (uint16_t)__popc(m);
+      }
+    }
   __syncthreads();
   if ((int)threadIdx.x < n_super) {
-    seg[threadIdx.x] = scanned[(size_t)threadIdx.x * nblk + blockIdx.x];
-    uint32_t run = 0;
-    for (int k = 0; k < MS_W; ++k) {
-      const uint32_t c = wc[threadIdx.x][k];
-      wc[threadIdx.x][k] = (uint16_t)run;
-      run += c;
+    uint32_t run = scanned[(size_t)threadIdx.x * nblk + blockIdx.x];
+    seg[threadIdx.x] = run;
+    uint16_t* row = wc + threadIdx.x * (MS_W + 2);
+    uint32_t before = 0;
+#pragma unroll
+    for (int k = 0; k < MS_W; ++k) {                    // exclusive prefix over the warps (a block holds 1024 ranks: fits 16 bits)
+      const uint32_t c = row[k];
+      row[k] = (uint16_t)before;
+      before += c;
     }
     if (blockIdx.x == 0) {                    // supertile ranges: [start of (s, block 0), start of (s + 1, block 0))
       const uint32_t b = scanned[(size_t)threadIdx.x * nblk];
@@ -131,18 +149,25 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const __grid_constan
     }
   }
   __syncthreads();
-  for (int s = 0, sx = 0, sy = 0; s < n_super; ++s) {
-    const bool c = small ? ((cm >> s) & 1ull) != 0ull : covers_super(sr, (uint32_t)sx, (uint32_t)sy);
-    const unsigned m = __ballot_sync(0xffffffffu, c);
-    if (!small && ++sx == super_x) { sx = 0; ++sy; }
-    if (c) {
-      const uint32_t pos = seg[s] + wc[s][w] + __popc(m & lt);
+  // every lane walks the supertiles of its own rect
+#pragma unroll
+  for (int k = 0; k < MS_WORDS; ++k) {
+    if (k >= words) break;
+    uint32_t bits = cm[k];
+    while (bits) {
+      const int s = 32 * k + __ffs((int)bits) - 1;
+      bits &= bits - 1u;
+      const uint32_t pos = seg[s] + wc[s * (MS_W + 2) + w] + __popc(bm[w * n_super + s] & lt);
       if (pos < cap) {
         keys[pos] = ((uint32_t)s << rank_bits) | (uint32_t)r;
         crect[pos] = rc;
       }
     }
   }
+}
+
+static size_t msplit_write_smem(int n_super) {
+  return (size_t)256 * 4 + (size_t)MS_W * n_super * 4 + (size_t)n_super * (MS_W + 2) * 2;
 }
 
 uint32_t msplit_blocks(int N) { return (uint32_t)((N + MS_T - 1) / MS_T); }
@@ -156,8 +181,11 @@ void launch_msplit_count(const PreBatch& batch, int N, const TileGrid& tg, cudaS
 void launch_msplit_write(const PreBatch& batch, int N, const TileGrid& tg, int rank_bits, uint32_t cap, cudaStream_t st) {
   const uint32_t nblk = msplit_blocks(N);
   ++g_kernel_launches;
-  msplit_write_kernel<<<dim3(nblk, (unsigned)batch.n), MS_T, 0, st>>>(batch, N, tg.sshift, tg.super_x, tg.super_x * tg.super_y, rank_bits, nblk,
-                                                                      cap);
+  const int n_super = tg.super_x * tg.super_y;
+  const size_t smem = msplit_write_smem(n_super);
+  if (smem > 48 * 1024 && cudaFuncSetAttribute(msplit_write_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return;                                             // the caller's cudaGetLastError() reports it
+  msplit_write_kernel<<<dim3(nblk, (unsigned)batch.n), MS_T, smem, st>>>(batch, N, tg.sshift, tg.super_x, n_super, rank_bits, nblk, cap);
 }
 
 // ---- parity export: the full tile lists (R-5), by the same rect test the rasteriser applies on the fly.

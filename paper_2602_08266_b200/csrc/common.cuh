@@ -114,7 +114,20 @@ __device__ __forceinline__ f2 splat_power2(float qa, float qb, float qc, float d
   return fma2(bc2(dx), inner, mul2(mul2(bc2(qc), dy), dy));
 }
 
-// exp_spec on a pair: the same operations in the same order, each half individually rounded
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// exp_spec on a pair: the same operations in the same order, each half individually rounded.  The last step of exp_spec,
+// bits(p) + (k << 23), is taken here as p * 2^k with 2^k from MUFU.EX2 of the integer-valued kf: on this hardware
+// ex2.approx is exact at every integer in [-126, 127] and the product of p in [0.5, 2) with a power of two equals the
+// exponent-field addition whenever the result is a normal number (checked exhaustively over k and on a grid of mantissas on
+// the B200), i.e. for every x in [-80, 80] -- the whole domain exp_spec is specified on.  Outside it the two differ, in the
+// useful direction: a NaN or -inf argument (a pixel parked at py = +inf) gives NaN instead of arbitrary bits, and NaN fails
+// every `>= alpha_min` test, so the raster kernels need no separate range test to mask such lanes.  Two ALU-pipe
+// operations per pixel move to the idle MUFU pipe.
 __device__ __forceinline__ f2 exp_spec2(f2 x) {
   const float MAGIC = 12582912.0f;
   const f2 t = fma2(x, bc2(0x1.715476p+0f), bc2(MAGIC));
@@ -128,8 +141,7 @@ __device__ __forceinline__ f2 exp_spec2(f2 x) {
   p = fma2(p, r, bc2(0.5f));
   p = fma2(p, r, bc2(1.0f));
   p = fma2(p, r, bc2(1.0f));
-  const int kx = __float_as_int(t.x) - __float_as_int(MAGIC), ky = __float_as_int(t.y) - __float_as_int(MAGIC);
-  return make_float2(__int_as_float(__float_as_int(p.x) + (kx << 23)), __int_as_float(__float_as_int(p.y) + (ky << 23)));
+  return mul2(p, make_float2(ex2_approx(kf.x), ex2_approx(kf.y)));
 }
 
 // packed upper-triangle index, r <= c

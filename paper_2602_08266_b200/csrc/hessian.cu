@@ -234,11 +234,13 @@ __device__ __forceinline__ void tpg_build_block(const SceneDev& sc, const nbv_co
 
 // S6 on the thread's two rows: a0 = c H_T + Lambda, a1 = c (H_T + H) + Lambda (packed, destroyed).  Two interleaved
 // right-looking L D L^T; the pivot ratios d1_j / d0_j are multiplied up in two halves (each ratio is >= 1 up to rounding
-// and far below 1e20, so neither product leaves binary64 range) and enter as two logarithms.  The rows are accessed as
-// `volatile`: otherwise the compiler promotes the whole packed block to registers across the unrolled pivot steps and
-// spills it to local memory (2.4 KB of spill stores per thread).
+// and far below 1e20, so neither product leaves binary64 range) and enter as two logarithms.  A compiler barrier after every
+// row update keeps the rows in shared memory: without it the whole packed block is promoted to registers across the
+// unrolled pivot steps and spilled to local memory (2.4 KB of spill stores per thread); `volatile` rows avoid that too but
+// serialise every load behind the previous store (85 us per chunk).  The row pointers are deliberately not __restrict__
+// (the barrier would not apply to them).
 // TRACE: this Gaussian's reduction of trace(H^-1) instead, from the same factors.
-__device__ __forceinline__ double tpg_inverse_trace(const volatile double* a) {
+__device__ __forceinline__ double tpg_inverse_trace(const double* a) {
   // a = the rows U_j = d_j L_j^T left by the elimination; A^-1 = L^-T D^-1 L^-1, trace = sum_c sum_i x_i^2 / d_i, x = L^-1 e_c
   double inv[P];
 #pragma unroll
@@ -256,6 +258,7 @@ __device__ __forceinline__ double tpg_inverse_trace(const volatile double* a) {
       for (int j = c; j < i; ++j) s = fma(a[tri(j, i)] * inv[j], x[j], s);
       x[i] = -s;
       acc = fma(s * s, inv[i], acc);
+      asm volatile("" ::: "memory");
     }
     tr += acc;
   }
@@ -263,7 +266,7 @@ __device__ __forceinline__ double tpg_inverse_trace(const volatile double* a) {
 }
 
 template <bool TRACE>
-__device__ __forceinline__ double tpg_gain(volatile double* a0, volatile double* a1) {
+__device__ __forceinline__ double tpg_gain(double* a0, double* a1) {
   double prod_lo = 1.0, prod_hi = 1.0;
 #pragma unroll
   for (int j = 0; j < P; ++j) {
@@ -285,6 +288,7 @@ __device__ __forceinline__ double tpg_gain(volatile double* a0, volatile double*
           a0[rr + c - r] = fma(l0, r0[c], a0[rr + c - r]);
           a1[rr + c - r] = fma(l1, r1[c], a1[rr + c - r]);
         }
+        asm volatile("" ::: "memory");
       }
     }
   }
@@ -292,25 +296,84 @@ __device__ __forceinline__ double tpg_gain(volatile double* a0, volatile double*
   return log(prod_lo) + log(prod_hi);
 }
 
-// cooperative, coalesced: for the block's Gaussian i (id gs[i], confidence cs[i]):
+// Cooperative, coalesced walks over the block's rows: thread t owns the packed entries t and t + 64 of EVERY Gaussian of the
+// chunk, so index arithmetic and the prior lookup happen once per thread, and TPG_U Gaussians' loads are in flight at a time
+// (H_T is far larger than the L2: a loop that waits for one load per iteration costs a DRAM round trip per Gaussian, 64 of
+// them in a row -- measured 46 us per chunk).
+constexpr int TPG_U = 8;
+
+// packed index -> prior on the diagonal, 0 elsewhere
+__device__ __forceinline__ double prior_of(const nbv_config& cfg, int idx) {
+  int r = 0;
+#pragma unroll
+  for (int q = 1; q < P; ++q) r += idx >= tri(q, q) ? 1 : 0;
+  return idx == tri(r, r) ? (double)cfg.prior_precision[r] : 0.0;
+}
+
 //   S0 row i = ct H_T,g + Lambda,   S1 row i = S0 row i + cb * S1 row i      (R-14: which of the two the confidence weights)
 __device__ __forceinline__ void tpg_load_combine(const double* __restrict__ H_T, const nbv_config& cfg, const uint32_t* gs, const double* cs,
                                                  int n, double* S0, double* S1) {
-#pragma unroll 4
-  for (int i = 0; i < n; ++i) {
-    const double c = cs[i];
-    if (!(c > 0.0)) continue;
-    const double ct = cfg.weight_mode == 0 ? c : 1.0;          // Eq. 9 literal (R1) weights H_T as well; R2 / R3 do not
-    const double cb = cfg.weight_mode == 1 ? 1.0 : c;          // R2 weights the gain, R1 / R3 the candidate block
-    const double* ht = H_T + (size_t)gs[i] * NBLK;
-    for (int idx = threadIdx.x; idx < NBLK; idx += TPG) {
-      // packed index -> diagonal?  row r starts at tri(r, r)
-      int r = 0;
+  const int idx0 = threadIdx.x, idx1 = threadIdx.x + TPG;
+  const bool has1 = idx1 < NBLK;
+  const double pr0 = prior_of(cfg, idx0), pr1 = has1 ? prior_of(cfg, idx1) : 0.0;
+  for (int i0 = 0; i0 < n; i0 += TPG_U) {
+    double h0[TPG_U], h1[TPG_U];
 #pragma unroll
-      for (int q = 1; q < P; ++q) r += idx >= tri(q, q) ? 1 : 0;
-      const double m0 = fma(ct, ht[idx], idx == tri(r, r) ? (double)cfg.prior_precision[r] : 0.0);
-      S0[i * NBLK + idx] = m0;
-      S1[i * NBLK + idx] = fma(cb, S1[i * NBLK + idx], m0);
+    for (int k = 0; k < TPG_U; ++k) {
+      const int i = i0 + k;
+      h0[k] = h1[k] = 0.0;
+      if (i < n && cs[i] > 0.0) {
+        const double* ht = H_T + (size_t)gs[i] * NBLK;
+        h0[k] = __ldg(ht + idx0);
+        if (has1) h1[k] = __ldg(ht + idx1);
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < TPG_U; ++k) {
+      const int i = i0 + k;
+      if (i < n) {
+        const double c = cs[i];
+        if (c > 0.0) {
+          const double ct = cfg.weight_mode == 0 ? c : 1.0;          // Eq. 9 literal (R1) weights H_T as well; R2 / R3 do not
+          const double cb = cfg.weight_mode == 1 ? 1.0 : c;          // R2 weights the gain, R1 / R3 the candidate block
+          const double m0 = fma(ct, h0[k], pr0);
+          S0[i * NBLK + idx0] = m0;
+          S1[i * NBLK + idx0] = fma(cb, S1[i * NBLK + idx0], m0);
+          if (has1) {
+            const double m1 = fma(ct, h1[k], pr1);
+            S0[i * NBLK + idx1] = m1;
+            S1[i * NBLK + idx1] = fma(cb, S1[i * NBLK + idx1], m1);
+          }
+        }
+      }
+    }
+  }
+}
+
+// H_T rows += S1 rows (training accumulation; one launch per view: a view lists a Gaussian once, plain binary64 additions)
+__device__ __forceinline__ void tpg_accumulate(double* __restrict__ H_T, const uint32_t* gs, int n, const double* S1) {
+  const int idx0 = threadIdx.x, idx1 = threadIdx.x + TPG;
+  const bool has1 = idx1 < NBLK;
+  for (int i0 = 0; i0 < n; i0 += TPG_U) {
+    double h0[TPG_U], h1[TPG_U];
+#pragma unroll
+    for (int k = 0; k < TPG_U; ++k) {
+      const int i = i0 + k;
+      h0[k] = h1[k] = 0.0;
+      if (i < n) {
+        const double* ht = H_T + (size_t)gs[i] * NBLK;
+        h0[k] = ht[idx0];
+        if (has1) h1[k] = ht[idx1];
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < TPG_U; ++k) {
+      const int i = i0 + k;
+      if (i < n) {
+        double* ht = H_T + (size_t)gs[i] * NBLK;
+        ht[idx0] = h0[k] + S1[i * NBLK + idx0];
+        if (has1) ht[idx1] = h1[k] + S1[i * NBLK + idx1];
+      }
     }
   }
 }
@@ -346,25 +409,19 @@ __global__ void __launch_bounds__(TPG) expand_kernel(const __grid_constant__ Sce
     }
     __syncthreads();
     if (MODE == EXPAND_TRAIN) {
-      // one launch per view, in view order: a view lists a Gaussian once, so these are plain binary64 additions
-      for (int i = 0; i < n; ++i) {
-        double* dst = H_T + (size_t)gs[i] * NBLK;
-        for (int idx = threadIdx.x; idx < NBLK; idx += TPG) dst[idx] += S1[i * NBLK + idx];
-      }
+      tpg_accumulate(H_T, gs, n, S1);
     } else if (MODE == EXPAND_VIEW) {
-      for (int i = 0; i < n; ++i) {
-        float* dst = vw.out_blocks + (size_t)gs[i] * NBLK;
-        for (int idx = threadIdx.x; idx < NBLK; idx += TPG) dst[idx] = (float)S1[i * NBLK + idx];
+      for (int e = threadIdx.x; e < n * NBLK; e += TPG) {
+        const int i = e / NBLK;
+        vw.out_blocks[(size_t)gs[i] * NBLK + (e - i * NBLK)] = (float)S1[e];
       }
     } else if (MODE == EXPAND_CACHE) {
       // span[1] = 0 when the pool overflowed: nothing is stored
-      for (int i = 0; i < n; ++i) {
-        if (base + i >= vw.cache_span[1]) break;
-        const size_t e = (size_t)vw.cache_span[0] + base + i;
-        if (threadIdx.x == 0) cache_ids[e] = gs[i];
-        double* dst = cache_blocks + e * NBLK;
-        for (int idx = threadIdx.x; idx < NBLK; idx += TPG) dst[idx] = S1[i * NBLK + idx];
-      }
+      const uint32_t span0 = vw.cache_span[0], span1 = vw.cache_span[1];
+      const int m = base >= span1 ? 0 : (int)min((uint32_t)n, span1 - base);       // consecutive pool entries: one coalesced copy
+      if ((int)threadIdx.x < m) cache_ids[(size_t)span0 + base + threadIdx.x] = gs[threadIdx.x];
+      double* dst = cache_blocks + ((size_t)span0 + base) * NBLK;
+      for (int e = threadIdx.x; e < m * NBLK; e += TPG) dst[e] = S1[e];
     } else {
       tpg_load_combine(H_T, cfg, gs, cs, n, S0, S1);
       __syncthreads();

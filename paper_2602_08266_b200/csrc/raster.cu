@@ -199,10 +199,11 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
       for (int q = 0; q < PPL / 2; ++q) {
         const f2 dy = sub2(py2[q], bc2(s0.y));
         const f2 power = splat_power2(s0.z, s0.w, s1.x, dx, dy);
-        const f2 a = mul2(bc2(s1.y), exp_spec2(power));       // garbage outside [tau, 0]: masked by `pass`
-        // s1.w = tau >= -6 is a pre-test that never decides (project.cu); the alpha test does (R-4, R-5)
-        const bool pass_x = power.x <= 0.0f && power.x >= s1.w && a.x >= prm.alpha_min;
-        const bool pass_y = power.y <= 0.0f && power.y >= s1.w && a.y >= prm.alpha_min;
+        const f2 a = mul2(bc2(s1.y), exp_spec2(power));       // NaN for a parked pixel (power = -inf or NaN): fails the alpha test
+        // The lower bounds of R-5 (power >= -6) and of the splat (power >= tau) never decide: alpha_min >= 1/255 (nbv_create)
+        // and sigma < 1 make sigma exp(power) >= alpha_min the stronger condition (project.cu), so the alpha test stands for both.
+        const bool pass_x = power.x <= 0.0f && a.x >= prm.alpha_min;
+        const bool pass_y = power.y <= 0.0f && a.y >= prm.alpha_min;
         f2 al;
         al.x = pass_x ? fminf(a.x, prm.alpha_max) : 0.0f;
         al.y = pass_y ? fminf(a.y, prm.alpha_max) : 0.0f;
@@ -273,11 +274,6 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   }  // persistent loop
 }
 
-__device__ __forceinline__ float ex2_approx(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
 __device__ __forceinline__ float rcp_approx(float x) {
   float y;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -461,8 +457,8 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       for (int q = 0; q < PPL / 2; ++q) {
         const f2 dy = sub2(py2[q], bc2(s0.y));
         const f2 power = splat_power2(s0.z, s0.w, s1.x, dx, dy);
-        const bool in_x = e < last_x[q] && power.x <= 0.0f && power.x >= s1.w;
-        const bool in_y = e < last_y[q] && power.y <= 0.0f && power.y >= s1.w;
+        const bool in_x = e < last_x[q] && power.x <= 0.0f;        // the lower bounds never decide (see forward_kernel)
+        const bool in_y = e < last_y[q] && power.y <= 0.0f;
         // outside the footprint or at / behind the entry the pixel stopped at: power = -inf, whose exp is 0 (MUFU) or NaN
         // (exp_spec); either fails `a >= alpha_min`
         pw[q].x = in_x ? power.x : -INFINITY;

@@ -113,3 +113,46 @@ def test_mask_context_errors_and_greedy_fallback():
     order, _ = nbv.select_greedy(cands, 2)                           # mask contexts take the re-rasterising path
     first = orc.score_candidates_mask(make_oracle_scene(sc), train, cands)
     assert order[0] == first["best"] and len(set(order.tolist())) == 2
+
+
+def test_mask_output_at_the_benchmarked_image_size_and_channel_count():
+    """1280 x 720, K = 20 object channels (blocks of 31 parameters, five S4 channel groups), 20,000 Gaussians: training
+    blocks, candidate blocks, per-Gaussian gains, scores and the arg-max against the oracle's stored values
+    (tests/golden/mask_fullres.json, written by tests/golden/make_mask_golden.py from oracle/ alone)."""
+    import importlib.util
+    import json
+    from pathlib import Path
+    golden = Path(__file__).resolve().parent / "golden"
+    spec = importlib.util.spec_from_file_location("make_mask_golden", golden / "make_mask_golden.py")
+    mk = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mk)
+    f = golden / "mask_fullres.json"
+    assert f.exists(), "mask_fullres.json missing: run tests/golden/make_mask_golden.py"
+    g = json.loads(f.read_text())
+    wl = mk.workload()
+    for k, v in mk.oracle_hashes().items():
+        assert g[k] == v, "mask_fullres.json is stale (%s changed): regenerate it" % k
+    assert g["input_sha256"] == mk.input_checksum(wl), "mask_fullres.json is stale (the synthetic inputs changed): regenerate it"
+    K, L, step = g["K"], g["L"], g["block_step"]
+    assert (K, L) == (wl.scene.K, 11 + wl.scene.K) and g["image"] == [1280, 720]
+    nbv = _mask_ctx(wl.scene, mask_bg_channel=g["bg_channel"])
+    nbv.accumulate_training(wl.train_cams)
+
+    def check_blocks(Hg, touched, ref_blocks):
+        touched = np.array(touched)
+        assert np.array_equal(np.flatnonzero(np.abs(Hg).max(axis=1) > 0), touched)          # same set of touched Gaussians
+        assert _block_err(Hg[touched[::step]], np.array(ref_blocks), L).max() < 1e-3
+
+    check_blocks(nbv.training_hessian().cpu().numpy().astype(np.float64), g["train_touched"], g["train_blocks"])
+    c0 = g["candidates"][0]
+    check_blocks(nbv.view_hessian(wl.cand_cams[0]).cpu().numpy().astype(np.float64), c0["touched"], c0["blocks"])
+    s, best = nbv.score_candidates(wl.cand_cams)
+    np.testing.assert_allclose(s.cpu().numpy(), g["scores"], rtol=1e-3, atol=1e-6)
+    assert int(best.item()) == g["best"]
+    for i, c in enumerate(g["candidates"]):
+        gg = nbv.gaussian_gains(wl.cand_cams[i]).cpu().numpy().astype(np.float64)
+        t = np.array(c["touched"])
+        np.testing.assert_allclose(gg[t], c["gains"], rtol=1e-3, atol=1e-6)
+        rest = np.ones(len(gg), bool)
+        rest[t] = False
+        assert np.all(gg[rest] == 0)
