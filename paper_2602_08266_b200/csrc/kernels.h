@@ -169,12 +169,12 @@ void launch_export_blocks(const double* src, float* dst, size_t n, cudaStream_t 
 void launch_export_chain(const SceneDev& sc, const nbv_camera& cam, float* out, cudaStream_t st);
 void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);
 
-// ---- mask.cu, object-mask output (NEXT-2): groups of four object channels, blocks of L = 11 + K parameters, binary32
+// ---- mask.cu, object-mask output (NEXT-2): groups of four object channels, blocks of L = 11 + K parameters, binary64
 void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uint32_t* ids_sorted, int group, int bgch, Splat* out,
                         cudaStream_t st);
-void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, float* H_T,
-                        const float* conf, const float* cholT, cudaStream_t st);
-void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st);
+void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, double* H_T,
+                        const float* conf, const double* cholT, cudaStream_t st);
+void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const double* H_T, const float* conf, double* cholT, cudaStream_t st);
 void launch_mask_scatter(const float* rgb, const float* depth, size_t npx, int K, int group, int bgch, float* mask, cudaStream_t st);
 
 // ---- sh.cu, SH degree 3 colour (NEXT-4): per-view colours in S1, 59 x 59 blocks in S5 / S6 (binary64, one warp per Gaussian)

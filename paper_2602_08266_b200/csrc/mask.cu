@@ -1,4 +1,5 @@
-// mask.cu -- the object-mask output (NEXT-2): S5' / S6 on blocks of L = 11 + K parameters, binary32, one warp per Gaussian.
+// mask.cu -- the object-mask output (NEXT-2): S5' / S6 on blocks of L = 11 + K parameters, binary64 (as the colour / depth
+// contexts, and for the same reason: hessian.cu), one warp per Gaussian.
 #include <algorithm>
 #include <cstdlib>
 
@@ -50,15 +51,15 @@ void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uin
 }
 
 // upper Cholesky factor of a packed SPD L x L, in place (as cholesky_packed)
-__device__ void cholesky_L(float* Mx, int L) {
+__device__ void cholesky_L(double* Mx, int L) {
   for (int j = 0; j < L; ++j) {
-    float d = Mx[triL(j, j, L)];
+    double d = Mx[triL(j, j, L)];
     for (int k = 0; k < j; ++k) d -= Mx[triL(k, j, L)] * Mx[triL(k, j, L)];
-    d = fmaxf(d, 1e-30f);
-    const float inv = rsqrtf(d);
+    d = fmax(d, 1e-300);
+    const double inv = rsqrt(d);
     Mx[triL(j, j, L)] = d * inv;
     for (int i = j + 1; i < L; ++i) {
-      float v = Mx[triL(j, i, L)];
+      double v = Mx[triL(j, i, L)];
       for (int k = 0; k < j; ++k) v -= Mx[triL(k, j, L)] * Mx[triL(k, i, L)];
       Mx[triL(j, i, L)] = v * inv;
     }
@@ -73,7 +74,7 @@ __device__ void cholesky_L(float* Mx, int L) {
 //   (pivot 1 + e_j enters as log1p(e_j), as in gain_solve), one column per step, the trailing rows updated in parallel.
 struct MaskWarpLayout {
   int LS;          // row stride of H and U (odd: conflict-free column and row walks)
-  int per_warp;    // floats per warp
+  int per_warp;    // doubles per warp
   int oH, oU, oA, oAQ, oMom, oX, oP, oMono;
 };
 __host__ __device__ inline MaskWarpLayout mask_warp_layout(int K, int groups) {
@@ -95,41 +96,41 @@ __host__ __device__ inline MaskWarpLayout mask_warp_layout(int K, int groups) {
 
 __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
                                                                 const __grid_constant__ ExpandBatch batch, int mode, int groups, int view0,
-                                                                float* __restrict__ H_T, const float* __restrict__ conf,
-                                                                const float* __restrict__ cholT) {
-  extern __shared__ __align__(16) float smem[];
+                                                                double* __restrict__ H_T, const float* __restrict__ conf,
+                                                                const double* __restrict__ cholT) {
+  extern __shared__ __align__(16) double smem[];
   const ExpandView& vw = batch.v[view0 + blockIdx.y];
   const int K = sc.K, L = 11 + K, LB = L * (L + 1) / 2, bgch = cfg.mask_bg_channel;
   const MaskWarpLayout lay = mask_warp_layout(K, groups);
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5, LS = lay.LS;
-  float* base = smem + (size_t)wib * lay.per_warp;
-  float *Hm = base + lay.oH, *Um = base + lay.oU, *As = base + lay.oA, *AQs = base + lay.oAQ, *mom = base + lay.oMom;
-  float *xs = base + lay.oX, *ps = base + lay.oP, *mono = base + lay.oMono;
+  double* base = smem + (size_t)wib * lay.per_warp;
+  double *Hm = base + lay.oH, *Um = base + lay.oU, *As = base + lay.oA, *AQs = base + lay.oAQ, *mom = base + lay.oMom;
+  double *xs = base + lay.oX, *ps = base + lay.oP, *mono = base + lay.oMono;
   const uint32_t n_touched = vw.counters->n_touched;
   const int stride = NMOM * groups;
-  float gain = 0.f;
+  double gain = 0.0;
   for (uint32_t t = blockIdx.x * wpb + wib; t < n_touched; t += gridDim.x * wpb) {
     const uint32_t r = vw.touched[t];
     const uint32_t g = vw.ids_sorted[r];
     __syncwarp();
     // moments of all groups -> shared memory (and zero the buffer for the next view)
     float* gm = vw.moments + (size_t)r * stride;
-    for (int i = lane; i < stride; i += 32) { mom[i] = gm[i]; gm[i] = 0.f; }
+    for (int i = lane; i < stride; i += 32) { mom[i] = (double)gm[i]; gm[i] = 0.f; }
     __syncwarp();
     {   // whitened basis -> u basis, one lane per group
       const Splat sp = vw.splat_sorted[r];
       for (int gr = lane; gr < groups; gr += 32) {
-        float m[NMOM];
+        double m[NMOM];
 #pragma unroll
         for (int i = 0; i < NMOM; ++i) m[i] = mom[gr * NMOM + i];
-        whitened_to_u<float>(m, sp);
+        whitened_to_u<double>(m, sp);
 #pragma unroll
         for (int i = 0; i < NMOM; ++i) mom[gr * NMOM + i] = m[i];
       }
     }
     __syncwarp();
     if (lane < 15) {
-      float v = 0.f;
+      double v = 0.0;
       for (int gr = 0; gr < groups; ++gr) v += mom[gr * NMOM + lane];
       mono[lane] = v;
     }
@@ -138,26 +139,26 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       const int slot = i / 6, e = i - 6 * slot;
       xs[i] = mom[(slot >> 2) * NMOM + MOM_X + 6 * (slot & 3) + e];
     }
-    float s2p = 0.f;
+    double s2p = 0.0;
     for (int slot = lane; slot < K; slot += 32) {
-      const float pv = expf(sc.logits[(size_t)g * K + mask_channel_of_slot(slot, bgch)] - sc.lse[g]);
+      const double pv = exp(sc.logits[(size_t)g * K + mask_channel_of_slot(slot, bgch)] - sc.lse[g]);
       ps[slot] = pv;
       s2p += pv * pv;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s2p += __shfl_xor_sync(0xffffffffu, s2p, o);
-    const float S2 = s2p;
+    const double S2 = s2p;
     {   // chain rule (every lane, redundantly), A and A Q into shared memory for dynamic indexing
-      Chain<float> ch;
-      projection_chain<float>(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
-      const float sg = sc.sigma[g];
-      const float kappa = cfg.opacity_coord == 0 ? (1.f - sg) : 1.f / sg;       // R-10
+      Chain<double> ch;
+      projection_chain<double>(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);
+      const double sg = sc.sigma[g];
+      const double kappa = cfg.opacity_coord == 0 ? (1.0 - sg) : 1.0 / sg;       // R-10
       if (lane < 11) {
-        float a6[6];
+        double a6[6];
         if (lane < 10) {
-          a6[0] = ch.G[0][lane]; a6[1] = ch.G[1][lane]; a6[2] = 0.5f * ch.G[2][lane]; a6[3] = ch.G[3][lane]; a6[4] = 0.5f * ch.G[4][lane]; a6[5] = 0.f;
+          a6[0] = ch.G[0][lane]; a6[1] = ch.G[1][lane]; a6[2] = 0.5 * ch.G[2][lane]; a6[3] = ch.G[3][lane]; a6[4] = 0.5 * ch.G[4][lane]; a6[5] = 0.0;
         } else {
-          a6[0] = a6[1] = a6[2] = a6[3] = a6[4] = 0.f; a6[5] = kappa;
+          a6[0] = a6[1] = a6[2] = a6[3] = a6[4] = 0.0; a6[5] = kappa;
         }
 #pragma unroll
         for (int e = 0; e < 6; ++e) As[lane * 6 + e] = a6[e];
@@ -167,17 +168,17 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
     if (lane < 11) {
       const int ex[6] = {1, 0, 2, 1, 0, 0}, ey[6] = {0, 1, 0, 1, 2, 0};
       for (int j = 0; j < 6; ++j) {
-        float v = 0.f;
+        double v = 0.0;
         for (int i = 0; i < 6; ++i) v += As[lane * 6 + i] * mono[mono_index(ex[i] + ex[j], ey[i] + ey[j])];
         AQs[lane * 6 + j] = v;
       }
     }
     __syncwarp();
-    const float W2 = mono[15];
-    float xbar[6];
+    const double W2 = mono[15];
+    double xbar[6];
 #pragma unroll
     for (int e = 0; e < 6; ++e) {
-      float v = 0.f;
+      double v = 0.0;
       for (int slot = 0; slot < K; ++slot) v += ps[slot] * xs[slot * 6 + e];
       xbar[e] = v;
     }
@@ -185,30 +186,30 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
     for (int j = lane; j < L; j += 32) {
       if (j < 11) {
         for (int i = 0; i < 11; ++i) {
-          float v = 0.f;
+          double v = 0.0;
 #pragma unroll
           for (int e = 0; e < 6; ++e) v += AQs[i * 6 + e] * As[j * 6 + e];
           Hm[i * LS + j] = v;
         }
         for (int c = 0; c < K; ++c) {
           const int slot = mask_slot_of_channel(c, bgch);
-          float v = 0.f;
+          double v = 0.0;
 #pragma unroll
           for (int e = 0; e < 6; ++e) v += As[j * 6 + e] * (ps[slot] * (xs[slot * 6 + e] - xbar[e]));
           Hm[(11 + c) * LS + j] = v;
         }
       } else {
         const int c = j - 11, slot = mask_slot_of_channel(c, bgch);
-        const float pc = ps[slot];
+        const double pc = ps[slot];
         for (int i = 0; i < 11; ++i) {
-          float v = 0.f;
+          double v = 0.0;
 #pragma unroll
           for (int e = 0; e < 6; ++e) v += As[i * 6 + e] * (pc * (xs[slot * 6 + e] - xbar[e]));
           Hm[i * LS + j] = v;
         }
         for (int d = 0; d < K; ++d) {
-          const float pd = ps[mask_slot_of_channel(d, bgch)];
-          float v = pc * pd * (S2 - pc - pd);
+          const double pd = ps[mask_slot_of_channel(d, bgch)];
+          double v = pc * pd * (S2 - pc - pd);
           if (d == c) v += pc * pc;
           Hm[(11 + d) * LS + j] = W2 * v;
         }
@@ -216,26 +217,26 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
     }
     __syncwarp();
     if (mode == EXPAND_TRAIN || mode == EXPAND_VIEW) {
-      float* dst = (mode == EXPAND_TRAIN ? H_T : vw.out_blocks) + (size_t)g * LB;
       for (int rr = 0; rr < L; ++rr)
         for (int c = rr + lane; c < L; c += 32) {
-          if (mode == EXPAND_TRAIN) dst[triL(rr, c, L)] += Hm[rr * LS + c];     // one launch per view, in view order
-          else dst[triL(rr, c, L)] = Hm[rr * LS + c];
+          const size_t o = (size_t)g * LB + triL(rr, c, L);
+          if (mode == EXPAND_TRAIN) H_T[o] += Hm[rr * LS + c];                  // one launch per view, in view order
+          else vw.out_blocks[o] = (float)Hm[rr * LS + c];
         }
       continue;
     }
-    const float cg = conf[g];
-    const float cb = cfg.weight_mode == 1 ? 1.0f : cg;
-    float gn = 0.f;
-    if (cg > 0.f) {
-      const float* ut = cholT + (size_t)g * LB;
+    const double cg = conf[g];
+    const double cb = cfg.weight_mode == 1 ? 1.0 : cg;
+    double gn = 0.0;
+    if (cg > 0.0) {
+      const double* ut = cholT + (size_t)g * LB;
       for (int rr = 0; rr < L; ++rr)
         for (int c = rr + lane; c < L; c += 32) Um[rr * LS + c] = ut[triL(rr, c, L)];
       __syncwarp();
       // (a) columns: U^T x = c h_j
       for (int j = lane; j < L; j += 32)
         for (int i = 0; i < L; ++i) {
-          float v = cb * Hm[i * LS + j];
+          double v = cb * Hm[i * LS + j];
 #pragma unroll 4
           for (int k = 0; k < i; ++k) v -= Um[k * LS + i] * Hm[k * LS + j];
           Hm[i * LS + j] = v / Um[i * LS + i];
@@ -244,7 +245,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       // (b) rows: U^T y = (row i)^T
       for (int i = lane; i < L; i += 32)
         for (int c = 0; c < L; ++c) {
-          float v = Hm[i * LS + c];
+          double v = Hm[i * LS + c];
 #pragma unroll 4
           for (int k = 0; k < c; ++k) v -= Um[k * LS + c] * Hm[i * LS + k];
           Hm[i * LS + c] = v / Um[c * LS + c];
@@ -252,14 +253,14 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       __syncwarp();
       // log det(I + W): right-looking Cholesky on the excess, lower triangle
       for (int j = 0; j < L; ++j) {
-        const float e = fmaxf(Hm[j * LS + j], 0.f);
-        gn += log1pf(e);
-        const float inv = rsqrtf(1.0f + e);
+        const double e = fmax(Hm[j * LS + j], 0.0);
+        gn += log1p(e);
+        const double inv = rsqrt(1.0 + e);
         __syncwarp();
         for (int i = j + 1 + lane; i < L; i += 32) Hm[i * LS + j] *= inv;
         __syncwarp();
         for (int i = j + 1 + lane; i < L; i += 32) {
-          const float li = Hm[i * LS + j];
+          const double li = Hm[i * LS + j];
 #pragma unroll 4
           for (int k = j + 1; k <= i; ++k) Hm[i * LS + k] -= li * Hm[k * LS + j];
         }
@@ -273,7 +274,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
     }
   }
   if (mode == EXPAND_GAIN) {
-    __shared__ float ws[8];
+    __shared__ double ws[8];
     if (lane == 0) ws[wib] = gain;
     __syncthreads();
     double tsum = 0.0;
@@ -283,12 +284,12 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
   }
 }
 
-void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, float* H_T,
-                        const float* conf, const float* cholT, cudaStream_t st) {
+void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, double* H_T,
+                        const float* conf, const double* cholT, cudaStream_t st) {
   const MaskWarpLayout lay = mask_warp_layout(sc.K, groups);
   int wpb = 8;
-  while (wpb > 1 && (size_t)wpb * lay.per_warp * 4 > 200 * 1024) wpb >>= 1;
-  const size_t smem = (size_t)wpb * lay.per_warp * 4;
+  while (wpb > 1 && (size_t)wpb * lay.per_warp * 8 > 200 * 1024) wpb >>= 1;
+  const size_t smem = (size_t)wpb * lay.per_warp * 8;
   // the attribute is per device and per function: set it whenever the launch needs more than the default 48 KB
   if (smem > 48 * 1024 &&
       cudaFuncSetAttribute(expand_mask_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
@@ -308,25 +309,25 @@ void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandB
 
 // once per scoring call of a mask context: U_g = upper Cholesky factor of c_g H_T,g + Lambda (L x L)
 template <int KMAX>
-__global__ void __launch_bounds__(64) prepare_mask_kernel(int N, int K, nbv_config cfg, const float* __restrict__ H_T,
-                                                           const float* __restrict__ conf, float* __restrict__ cholT) {
+__global__ void __launch_bounds__(64) prepare_mask_kernel(int N, int K, nbv_config cfg, const double* __restrict__ H_T,
+                                                           const float* __restrict__ conf, double* __restrict__ cholT) {
   constexpr int LMAX = 11 + KMAX, LBMAX = LMAX * (LMAX + 1) / 2;
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   if (g >= N) return;
-  const float c = conf[g];
-  if (!(c > 0.f)) return;
+  const double c = conf[g];
+  if (!(c > 0.0)) return;
   const int L = 11 + K, LB = L * (L + 1) / 2;
-  const float* ht = H_T + (size_t)g * LB;
-  float H[LBMAX];
-  const float ct = cfg.weight_mode == 0 ? c : 1.0f;
+  const double* ht = H_T + (size_t)g * LB;
+  double H[LBMAX];
+  const double ct = cfg.weight_mode == 0 ? c : 1.0;
   for (int i = 0; i < LB; ++i) H[i] = ct * ht[i];
   for (int k = 0; k < L; ++k) H[triL(k, k, L)] += k < 11 ? cfg.prior_precision[k] : cfg.prior_precision_obj;
   cholesky_L(H, L);
-  float* dst = cholT + (size_t)g * LB;
+  double* dst = cholT + (size_t)g * LB;
   for (int i = 0; i < LB; ++i) dst[i] = H[i];
 }
 
-void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const float* H_T, const float* conf, float* cholT, cudaStream_t st) {
+void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const double* H_T, const float* conf, double* cholT, cudaStream_t st) {
   ++g_kernel_launches;
   if (sc.K <= 20)
     prepare_mask_kernel<20><<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, sc.K, cfg, H_T, conf, cholT);

@@ -75,7 +75,7 @@ struct nbv_ctx {
   size_t LB = NBLK;
   int n_train = 0;
   // scene
-  // H_T: N x 105 binary64 (colour / depth contexts) or N x LB binary32 (mask contexts); cholT: mask contexts only
+  // H_T: N x LB binary64 (LB = 105, or L (L + 1) / 2 in mask / SH contexts); cholT: mask contexts only, binary64
   DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp, cache_ids, cache_blocks, cache_meta,
       cache_scratch, trace_buf, sh45, prior59;         // trace_buf: S_T (1 double) | scratch of launch_trace_total
   size_t greedy_cache_bytes = (size_t)4 << 30;   // budget of the block cache of nbv_select_greedy (NBV_GREEDY_CACHE_MB)
@@ -496,8 +496,8 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     launch_cache_reserve(eb, *cache, first_candidate, st);
     launch_expand_cache(scene_dev(ctx), ctx->cfg, eb, *cache, st);
   } else if (ctx->mask_mode) {
-    launch_expand_mask(scene_dev(ctx), ctx->cfg, eb, mode, ctx->mask_groups, ctx->H_T.as<float>(), ctx->conf.as<float>(),
-                       ctx->cholT.as<float>(), st);
+    launch_expand_mask(scene_dev(ctx), ctx->cfg, eb, mode, ctx->mask_groups, ctx->H_T.as<double>(), ctx->conf.as<float>(),
+                       ctx->cholT.as<double>(), st);
   } else if (ctx->sh_mode) {
     launch_expand_sh(scene_dev(ctx), ctx->cfg, eb, mode, ctx->sh45.as<float>(), ctx->prior59.as<float>(), ctx->H_T.as<double>(),
                      ctx->conf.as<float>(), st);
@@ -583,7 +583,7 @@ int prepare_scoring(nbv_ctx* ctx, int target, cudaStream_t st) {
   const SceneDev sc = scene_dev(ctx);
   launch_confidence(sc, ctx->cfg, target, ctx->conf.as<float>(), st);
   if (ctx->mask_mode && ctx->conf_target != target)
-    launch_prepare_mask(sc, ctx->cfg, ctx->H_T.as<float>(), ctx->conf.as<float>(), ctx->cholT.as<float>(), st);
+    launch_prepare_mask(sc, ctx->cfg, ctx->H_T.as<double>(), ctx->conf.as<float>(), ctx->cholT.as<double>(), st);
   if (ctx->cfg.criterion == NBV_CRIT_TRACE) {                // S_T of the trace criterion: all N blocks of the current H_T
     if (!ctx->trace_buf.p) {
       CKRET(ensure(ctx, ctx->trace_buf, 16 + trace_total_scratch_bytes()));
@@ -731,9 +731,9 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
   CKRET(ensure(ctx, ctx->mean, 12 * n)); CKRET(ensure(ctx, ctx->logscale, 12 * n)); CKRET(ensure(ctx, ctx->quat, 16 * n));
   CKRET(ensure(ctx, ctx->sigma, 4 * n)); CKRET(ensure(ctx, ctx->rgb, 12 * n)); CKRET(ensure(ctx, ctx->logits, 4 * n * K));
   CKRET(ensure(ctx, ctx->M, 36 * n)); CKRET(ensure(ctx, ctx->pmax, 4 * n)); CKRET(ensure(ctx, ctx->amax, 4 * n));
-  const size_t ht_bytes = (ctx->mask_mode ? 4 : 8) * ctx->LB * n;
+  const size_t ht_bytes = 8 * (size_t)ctx->LB * n;
   CKRET(ensure(ctx, ctx->lse, 4 * n)); CKRET(ensure(ctx, ctx->H_T, ht_bytes)); CKRET(ensure(ctx, ctx->conf, 4 * n));
-  if (ctx->mask_mode) CKRET(ensure(ctx, ctx->cholT, 4 * ctx->LB * n));
+  if (ctx->mask_mode) CKRET(ensure(ctx, ctx->cholT, 8 * (size_t)ctx->LB * n));
   CK(cudaMemcpyAsync(ctx->mean.p, d_mean, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->logscale.p, d_logscale, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->quat.p, d_quat, 16 * n, cudaMemcpyDeviceToDevice, st));
@@ -784,7 +784,7 @@ int nbv_load_sh(nbv_ctx* ctx, const float* d_sh, void* stream) {
 int nbv_reset_training(nbv_ctx* ctx, void* stream) {
   if (!ctx) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
-  CK(cudaMemsetAsync(ctx->H_T.p, 0, (ctx->mask_mode ? 4 : 8) * ctx->LB * ctx->N, (cudaStream_t)stream));
+  CK(cudaMemsetAsync(ctx->H_T.p, 0, 8 * (size_t)ctx->LB * ctx->N, (cudaStream_t)stream));
   ctx->n_train = 0;
   ctx->conf_target = -2;
   return NBV_OK;
@@ -1119,12 +1119,8 @@ int nbv_view_hessian(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_blocks, voi
 int nbv_training_hessian(nbv_ctx* ctx, float* d_blocks, void* stream) {
   if (!ctx || !d_blocks) return NBV_ERR_INVALID_ARG;
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
-  if (ctx->mask_mode) {
-    CK(cudaMemcpyAsync(d_blocks, ctx->H_T.p, 4 * ctx->LB * ctx->N, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
-  } else {
-    launch_export_blocks(ctx->H_T.as<double>(), d_blocks, ctx->LB * (size_t)ctx->N, (cudaStream_t)stream);
-    CK(cudaGetLastError());
-  }
+  launch_export_blocks(ctx->H_T.as<double>(), d_blocks, ctx->LB * (size_t)ctx->N, (cudaStream_t)stream);
+  CK(cudaGetLastError());
   return NBV_OK;
 }
 
