@@ -43,7 +43,7 @@ FP32_LANES_PER_SM = 128
 # of one launch of each raster kernel, divided by the (pixel, list entry) evaluations of that launch (walked entries x 256).
 # Both slot bodies are branch-free, so the executed work is proportional to the evaluations, composited or not; S4's
 # per-entry moment assembly and reduction are amortised into its figure.  Source: FLOP_SOURCE (committed ncu pass).
-FLOP_PER_EVAL = {"forward": 40.6, "backward": {3: 118.0, 4: 131.0}}
+FLOP_PER_EVAL = {"forward": 30.8, "backward": {3: 87.0, 4: 102.4}}
 FLOP_SOURCE = "profiles/r2_ncu_flops_cfg2.md"
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
 VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (16 for images of fewer than 2,000 tiles)
