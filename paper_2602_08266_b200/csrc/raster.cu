@@ -437,7 +437,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       const float icC = 1.0f / cC;
       const float Pmin = __logf(prm.alpha_min / q1.y), Pmax = Pmin + prm.ln_amax_over_amin;
       sm_wh[lane] = make_float4(sqrtf(fmaxf(cA * cC - cB * cB, 0.0f) * icC), -cB * icC, sqrtf(cC), Pmin);
-      sm_ex[lane] = make_float4(log2f(q1.y), Pmin + Pmax, Pmin * Pmax, 0.0f);
+      sm_ex[lane] = make_float4(log2f(q1.y), Pmin + Pmax, Pmin * Pmax, cC);               // .w = h^2 = 1 / l22^2
     }
     __syncwarp();
     for (int j = 0; j < cnt; ++j) {
@@ -536,14 +536,14 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
         // cancellation a plain pixel-offset basis has for elongated footprints.  DESIGN.md section 6.)
         float acc[NMOM];
         const float x1 = dx * wh.x;
-        const float h = wh.z, h2 = h * h;
-        const float c1 = ((((float)y0 + 4.0f) - s0.y) - wh.y * dx) * h, c2 = c1 * c1, c3 = c2 * c1, c4 = c2 * c2;
-        const float E1 = h * F1s, E2 = h2 * F2s, E3 = h2 * h * F3s, E4 = h2 * h2 * F4s;
-        const float Y0v = F0s;
-        const float Y1v = fmaf(c1, F0s, E1);
-        const float Y2v = fmaf(c2, F0s, fmaf(2.0f * c1, E1, E2));
-        const float Y3v = fmaf(c3, F0s, fmaf(3.0f * c2, E1, fmaf(3.0f * c1, E2, E3)));
-        const float Y4v = fmaf(c4, F0s, fmaf(4.0f * c3, E1, fmaf(6.0f * c2, E2, fmaf(4.0f * c1, E3, E4))));
+        const float h = wh.z, h2 = ex.w;
+        const float c1 = ((((float)y0 + 4.0f) - s0.y) - wh.y * dx) * h;
+        // Y_j = sum_p C(j, p) c1^(j - p) h^p F_p by the Pascal recurrence a_p <- c1 a_p + a_(p+1) (ten FMAs, no powers of c1)
+        const float a0 = F0s, a1 = h * F1s, a2 = h2 * F2s, a3 = (h2 * h) * F3s, a4 = (h2 * h2) * F4s;
+        const float b0 = fmaf(c1, a0, a1), b1 = fmaf(c1, a1, a2), b2 = fmaf(c1, a2, a3), b3 = fmaf(c1, a3, a4);
+        const float d0 = fmaf(c1, b0, b1), d1 = fmaf(c1, b1, b2), d2 = fmaf(c1, b2, b3);
+        const float g0 = fmaf(c1, d0, d1), g1 = fmaf(c1, d1, d2);
+        const float Y0v = a0, Y1v = b0, Y2v = d0, Y3v = g0, Y4v = fmaf(c1, g0, g1);
         const float x2 = x1 * x1, x3 = x2 * x1, x4 = x2 * x2;
         acc[0] = Y0v;
         acc[1] = x1 * Y0v;  acc[2] = Y1v;
@@ -557,7 +557,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
             const int cc = c < NCH ? c : 0;
             const float Z0 = G[cc][0].x + G[cc][0].y, H1 = h * (G[cc][1].y - G[cc][1].x), H2 = h2 * (G[cc][2].x + G[cc][2].y);
             const float Z1 = fmaf(c1, Z0, H1);
-            const float Z2 = fmaf(c2, Z0, fmaf(2.0f * c1, H1, H2));
+            const float Z2 = fmaf(c1, Z1 + H1, H2);                      // c1^2 Z0 + 2 c1 H1 + H2
             xm[0] = x1 * Z0; xm[1] = Z1; xm[2] = x2 * Z0; xm[3] = x1 * Z1; xm[4] = Z2; xm[5] = Z0;
           } else {
             xm[0] = xm[1] = xm[2] = xm[3] = xm[4] = xm[5] = 0.0f;
