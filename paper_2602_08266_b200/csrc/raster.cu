@@ -280,46 +280,7 @@ __device__ __forceinline__ float rcp_approx(float x) {
   return y;
 }
 
-// Cross-lane reduction of the 40 moments through shared memory: every lane stores its 40 values as one row of a
-// 32 x 44 array (row stride 44 words: the float4 stores and loads below are bank-conflict free up to one 2-way phase);
-// lane l < 30 then sums the float4 column q = l % 10 over the rows r = l / 10, l / 10 + 3, ... and two shuffles fold
-// the three row groups, leaving the totals of moments 4q .. 4q+3 in lane q < 10.  ~90 instructions per entry, none of
-// them on the half-rate select pipe, against ~160 for a register butterfly.
-constexpr int RED_STRIDE = 44;
-
-__device__ __forceinline__ float4 reduce40(const float (&v)[NMOM], float* red, int lane) {
-  float4* row = reinterpret_cast<float4*>(red + lane * RED_STRIDE);
-#pragma unroll
-  for (int q = 0; q < NMOM / 4; ++q) row[q] = make_float4(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
-  __syncwarp();
-  const int q = lane % 10, rg = lane / 10;
-  f2 a01 = bc2(0.f), a23 = bc2(0.f), b01 = bc2(0.f), b23 = bc2(0.f);     // packed adds: two moments per issue slot
-  if (lane < 30) {
-    const float* col = red + 4 * q;
-#pragma unroll
-    for (int i = 0; i < 10; i += 2) {
-      const float4 x = *reinterpret_cast<const float4*>(col + (rg + 3 * i) * RED_STRIDE);
-      const float4 y = *reinterpret_cast<const float4*>(col + (rg + 3 * i + 3) * RED_STRIDE);
-      a01 = add2(a01, make_float2(x.x, x.y)); a23 = add2(a23, make_float2(x.z, x.w));
-      b01 = add2(b01, make_float2(y.x, y.y)); b23 = add2(b23, make_float2(y.z, y.w));
-    }
-    if (rg < 2) {                                    // rows 30 and 31
-      const float4 x = *reinterpret_cast<const float4*>(col + (rg + 30) * RED_STRIDE);
-      a01 = add2(a01, make_float2(x.x, x.y)); a23 = add2(a23, make_float2(x.z, x.w));
-    }
-  }
-  __syncwarp();                                      // the rows may be overwritten by the next entry
-  a01 = add2(a01, b01); a23 = add2(a23, b23);
-  float4 a = make_float4(a01.x, a01.y, a23.x, a23.y);
-  float4 t;
-  t.x = __shfl_down_sync(FULL, a.x, 10); t.y = __shfl_down_sync(FULL, a.y, 10);
-  t.z = __shfl_down_sync(FULL, a.z, 10); t.w = __shfl_down_sync(FULL, a.w, 10);
-  float4 u;
-  u.x = __shfl_down_sync(FULL, a.x, 20); u.y = __shfl_down_sync(FULL, a.y, 20);
-  u.z = __shfl_down_sync(FULL, a.z, 20); u.w = __shfl_down_sync(FULL, a.w, 20);
-  a.x += t.x + u.x; a.y += t.y + u.y; a.z += t.z + u.z; a.w += t.w + u.w;
-  return a;                                          // valid in lanes 0..9
-}
+constexpr int RED_STRIDE = 44;      // row stride (words) of the 32 x 40 reduction buffer: float4 rows, bank-conflict free
 
 // 16-byte vector reductions into the L2 (sm_90+): one request per four moments
 __device__ __forceinline__ void red_add_v4(float* dst, const float4& v) {
@@ -334,6 +295,97 @@ __device__ __forceinline__ float4 atom_add_v4(float* dst, const float4& v) {
   return o;
 }
 
+// ---- S4 group tail.  After its slot body a lane holds, per entry, 18 column sums over its 8 pixels: F_p = sum_k f_k t_k^p
+// (p <= 4), sum w^2, and G_c,p = sum_k g_c,k t_k^p (p <= 2) per channel.  Turning them into the lane's 40 moments (binomial
+// shift to the Gaussian's centre line, powers of xi1) and reducing those over the 32 lanes once per entry cost as much as the
+// slot body itself (ncu r2a: 41% of the kernel's instructions).  Instead the column sums of GE = 4 entries are parked in
+// shared memory and ONE tail serves them all: lane l takes entry l / 8 and the four source lanes l % 8 + 8 k, assembles
+// their moments (the source lane's pixel column and row block follow from its index) and accumulates them in registers;
+// one shared-memory transpose then folds the eight partial sums of every entry, and the lanes issue the 16-byte reductions
+// into the L2 -- every lane assembles 4 (entry, lane) pairs instead of 4 entries x 1 lane, but the 32-row reduction per
+// entry becomes an 8-row reduction per FOUR entries.
+constexpr int GE = 4;
+
+template <int NCH>
+__device__ __forceinline__ void group_tail(const float4* rawA, const float2* rawB, float* red, const float4* sm, const float4* sm_wh,
+                                           const float4* sm_ex, const uint32_t* q_rank, int gcount, uint32_t gpack, int tx, int ty,
+                                           float* __restrict__ moments, int mom_stride, int lane) {
+  __syncwarp();                                            // the parked column sums are visible
+  const int ge = lane >> 3, part = lane & 7;
+  float acc[NMOM];
+#pragma unroll
+  for (int i = 0; i < NMOM; ++i) acc[i] = 0.0f;
+  if (ge < gcount) {
+    const int je = (int)((gpack >> (8 * ge)) & 0xffu);
+    const float4 s0 = sm[je * 3], wh = sm_wh[je];
+    const float h = wh.z, h2 = sm_ex[je].w;
+    // The lane's 40 moments in the WHITENED coordinates xi = L^-1 (pixel - centre): xi1 = dx / l11 is the same for
+    // a source lane's 8 pixels and xi2 = (dy - (l21 / l11) dx) / l22 = c1 + h t_k steps with the row, so
+    // Y_b = sum_k f_k xi2_k^b follows from the F_p by a binomial shift, and the monomial sums are xi1^i Y_j.
+    // (The shear keeps the column structure; the whitening keeps the later change to the u basis free of the
+    // cancellation a plain pixel-offset basis has for elongated footprints.  DESIGN.md section 6.)
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int sl = part + 8 * k;                         // source lane: column sl & 15, row block sl >> 4
+      const float4* ra = rawA + ge * 4 * 32 + sl;
+      const float4 r0 = ra[0], r1 = ra[32], r2 = ra[64], r3 = ra[96];
+      const float2 r4 = rawB[ge * 32 + sl];
+      const float dx = sub_rn((float)(tx * TILE + (sl & 15)) + 0.5f, s0.x);
+      const float x1 = dx * wh.x;
+      const float c1 = ((((float)(ty * TILE + (sl >> 4) * PPL) + 4.0f) - s0.y) - wh.y * dx) * h;
+      // Y_j = sum_p C(j, p) c1^(j - p) h^p F_p by the Pascal recurrence a_p <- c1 a_p + a_(p+1) (ten FMAs, no powers of c1)
+      const float a0 = r0.x, a1 = h * r0.y, a2 = h2 * r0.z, a3 = (h2 * h) * r0.w, a4 = (h2 * h2) * r1.x;
+      const float b0 = fmaf(c1, a0, a1), b1 = fmaf(c1, a1, a2), b2 = fmaf(c1, a2, a3), b3 = fmaf(c1, a3, a4);
+      const float d0 = fmaf(c1, b0, b1), d1 = fmaf(c1, b1, b2), d2 = fmaf(c1, b2, b3);
+      const float g0 = fmaf(c1, d0, d1), g1 = fmaf(c1, d1, d2);
+      const float Y0v = a0, Y1v = b0, Y2v = d0, Y3v = g0, Y4v = fmaf(c1, g0, g1);
+      const float x2 = x1 * x1, x3 = x2 * x1, x4 = x2 * x2;
+      acc[0] += Y0v;
+      acc[1] = fmaf(x1, Y0v, acc[1]);   acc[2] += Y1v;
+      acc[3] = fmaf(x2, Y0v, acc[3]);   acc[4] = fmaf(x1, Y1v, acc[4]);   acc[5] += Y2v;
+      acc[6] = fmaf(x3, Y0v, acc[6]);   acc[7] = fmaf(x2, Y1v, acc[7]);   acc[8] = fmaf(x1, Y2v, acc[8]);   acc[9] += Y3v;
+      acc[10] = fmaf(x4, Y0v, acc[10]); acc[11] = fmaf(x3, Y1v, acc[11]); acc[12] = fmaf(x2, Y2v, acc[12]);
+      acc[13] = fmaf(x1, Y3v, acc[13]); acc[14] += Y4v;
+      const float gvv[12] = {r1.z, r1.w, r2.x, r2.y, r2.z, r2.w, r3.x, r3.y, r3.z, r3.w, r4.x, r4.y};
+#pragma unroll
+      for (int c = 0; c < NCH; ++c) {
+        float* xm = acc + MOM_X + 6 * c;
+        const float Z0 = gvv[3 * c], H1 = h * gvv[3 * c + 1], H2 = h2 * gvv[3 * c + 2];
+        const float Z1 = fmaf(c1, Z0, H1);
+        const float Z2 = fmaf(c1, Z1 + H1, H2);            // c1^2 Z0 + 2 c1 H1 + H2
+        xm[0] = fmaf(x1, Z0, xm[0]); xm[1] += Z1; xm[2] = fmaf(x2, Z0, xm[2]); xm[3] = fmaf(x1, Z1, xm[3]); xm[4] += Z2; xm[5] += Z0;
+      }
+      acc[MOM_W2] += r1.y;
+    }
+  }
+  __syncwarp();                                            // every lane has read its sources: rawA now serves as `red`
+  {
+    float4* row = reinterpret_cast<float4*>(red + lane * RED_STRIDE);
+#pragma unroll
+    for (int q = 0; q < NMOM / 4; ++q) row[q] = make_float4(acc[4 * q], acc[4 * q + 1], acc[4 * q + 2], acc[4 * q + 3]);
+  }
+  __syncwarp();
+  // 4 entries x 10 float4 columns, each the sum of the 8 rows of its entry: columns 0..7 by all lanes, 8 and 9 by lanes 0..7.
+  // No returning atomic: a returned value would tie up a scoreboard for a full L2 round trip; the touched list is built
+  // afterwards from sum w^2 != 0 (launch_touched)
+#pragma unroll
+  for (int round = 0; round < 2; ++round) {
+    const int e1 = round == 0 ? lane >> 3 : lane >> 1, q = round == 0 ? lane & 7 : 8 + (lane & 1);
+    if ((round == 0 || lane < 8) && e1 < gcount) {
+      const float* col = red + (e1 * 8) * RED_STRIDE + 4 * q;
+      f2 a01 = bc2(0.f), a23 = bc2(0.f);
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const float4 x = *reinterpret_cast<const float4*>(col + r * RED_STRIDE);
+        a01 = add2(a01, make_float2(x.x, x.y)); a23 = add2(a23, make_float2(x.z, x.w));
+      }
+      const uint32_t rank = q_rank[(gpack >> (8 * e1)) & 0xffu];
+      red_add_v4(moments + (size_t)rank * mom_stride + 4 * q, make_float4(a01.x, a01.y, a23.x, a23.y));
+    }
+  }
+  __syncwarp();                                            // the buffers may be refilled
+}
+
 // S4 slot body: the lane's 8 pixels as 4 pairs (row q, row 7 - q), packed binary32 operations throughout.  With the row
 // offsets t = -(3.5 - q) (.x) and +(3.5 - q) (.y), the column sums  F_p = sum_k f_k t_k^p,  G_c,p = sum_k g_c,k t_k^p  are
 // accumulated per half with the broadcast weights |t|^p and folded at the end:  F_p = hi + (-1)^p lo.
@@ -342,8 +394,12 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   __shared__ float4 sm[32 * 3];
   __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
   __shared__ float4 sm_ex[32];           // per staged entry: log2(sigma), P_min + P_max, P_min P_max, -
-  __shared__ __align__(16) float red[32 * RED_STRIDE];
+  // folded column sums of up to GE entries awaiting their group tail: values 0..15 of lane l, entry slot g at
+  // rawA[(g * 4 + m) * 32 + l] (m = 0..3), values 16, 17 at rawB[g * 32 + l]; the reduction buffer of the tail aliases rawA
+  __shared__ float4 rawA[GE * 4 * 32];
+  __shared__ float2 rawB[GE * 32];
   __shared__ uint32_t q_rank[64];
+  float* red = reinterpret_cast<float*>(rawA);
   const int lane = threadIdx.x;
   // Persistent warps (batch.work != nullptr): the grid is one wave of resident warps and every warp pulls launch positions
   // from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
@@ -402,6 +458,8 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   const uint32_t cbegin = cranges[(ty >> prm.sshift) * prm.super_x + (tx >> prm.sshift)].x;
   uint32_t pos_hi = vw.tile_cend[tile], qn = 0;
   int e_next = (int)elast - 1;
+  int gcount = 0;                      // entries parked for the group tail, and their positions j in the staged batch (8 bits each)
+  uint32_t gpack = 0u;
   const float thr_near = 2e-5f * prm.ln_amax_over_amin;
   for (;;) {
     while (qn < 32u && pos_hi > cbegin) {
@@ -440,7 +498,8 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       sm_ex[lane] = make_float4(log2f(q1.y), Pmin + Pmax, Pmin * Pmax, cC);               // .w = h^2 = 1 / l22^2
     }
     __syncwarp();
-    for (int j = 0; j < cnt; ++j) {
+    for (int j = 0; j <= cnt; ++j) {                         // j == cnt: only the group tail of what is still pending
+      if (j < cnt) {
       const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
       const int e = e_next - j;
       const float dx = sub_rn(px, s0.x);
@@ -527,50 +586,29 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
         any = any || pass_x || pass_y;
       }
       if (__any_sync(FULL, any)) {
-        // fold the halves: rows q have t < 0, rows 7 - q have t > 0
+        // fold the halves (rows q have t < 0, rows 7 - q have t > 0) and park the lane's 18 column sums; the moment assembly
+        // and the cross-lane reduction happen once per GE entries (group tail below)
         const float F0s = F0.x + F0.y, F1s = F1.y - F1.x, F2s = F2.x + F2.y, F3s = F3.y - F3.x, F4s = F4.x + F4.y;
-        // The lane's 40 moments in the WHITENED coordinates xi = L^-1 (pixel - centre): xi1 = dx / l11 is the same for
-        // the lane's 8 pixels and xi2 = (dy - (l21 / l11) dx) / l22 = xc + h t_k steps with the row, so
-        // Y_b = sum_k f_k xi2_k^b follows from the F_p by a binomial shift, and the monomial sums are xi1^i Y_j.
-        // (The shear keeps the column structure; the whitening keeps the later change to the u basis free of the
-        // cancellation a plain pixel-offset basis has for elongated footprints.  DESIGN.md section 6.)
-        float acc[NMOM];
-        const float x1 = dx * wh.x;
-        const float h = wh.z, h2 = ex.w;
-        const float c1 = ((((float)y0 + 4.0f) - s0.y) - wh.y * dx) * h;
-        // Y_j = sum_p C(j, p) c1^(j - p) h^p F_p by the Pascal recurrence a_p <- c1 a_p + a_(p+1) (ten FMAs, no powers of c1)
-        const float a0 = F0s, a1 = h * F1s, a2 = h2 * F2s, a3 = (h2 * h) * F3s, a4 = (h2 * h2) * F4s;
-        const float b0 = fmaf(c1, a0, a1), b1 = fmaf(c1, a1, a2), b2 = fmaf(c1, a2, a3), b3 = fmaf(c1, a3, a4);
-        const float d0 = fmaf(c1, b0, b1), d1 = fmaf(c1, b1, b2), d2 = fmaf(c1, b2, b3);
-        const float g0 = fmaf(c1, d0, d1), g1 = fmaf(c1, d1, d2);
-        const float Y0v = a0, Y1v = b0, Y2v = d0, Y3v = g0, Y4v = fmaf(c1, g0, g1);
-        const float x2 = x1 * x1, x3 = x2 * x1, x4 = x2 * x2;
-        acc[0] = Y0v;
-        acc[1] = x1 * Y0v;  acc[2] = Y1v;
-        acc[3] = x2 * Y0v;  acc[4] = x1 * Y1v;  acc[5] = Y2v;
-        acc[6] = x3 * Y0v;  acc[7] = x2 * Y1v;  acc[8] = x1 * Y2v;  acc[9] = Y3v;
-        acc[10] = x4 * Y0v; acc[11] = x3 * Y1v; acc[12] = x2 * Y2v; acc[13] = x1 * Y3v; acc[14] = Y4v;
+        float gv[12];
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
-          float* xm = acc + MOM_X + 6 * c;
-          if (c < NCH) {
-            const int cc = c < NCH ? c : 0;
-            const float Z0 = G[cc][0].x + G[cc][0].y, H1 = h * (G[cc][1].y - G[cc][1].x), H2 = h2 * (G[cc][2].x + G[cc][2].y);
-            const float Z1 = fmaf(c1, Z0, H1);
-            const float Z2 = fmaf(c1, Z1 + H1, H2);                      // c1^2 Z0 + 2 c1 H1 + H2
-            xm[0] = x1 * Z0; xm[1] = Z1; xm[2] = x2 * Z0; xm[3] = x1 * Z1; xm[4] = Z2; xm[5] = Z0;
-          } else {
-            xm[0] = xm[1] = xm[2] = xm[3] = xm[4] = xm[5] = 0.0f;
-          }
+          const int cc = c < NCH ? c : 0;
+          gv[3 * c + 0] = c < NCH ? G[cc][0].x + G[cc][0].y : 0.0f;
+          gv[3 * c + 1] = c < NCH ? G[cc][1].y - G[cc][1].x : 0.0f;
+          gv[3 * c + 2] = c < NCH ? G[cc][2].x + G[cc][2].y : 0.0f;
         }
-        acc[MOM_W2] = W2.x + W2.y;
-        const float4 tot = reduce40(acc, red, lane);
-        const uint32_t rank = q_rank[j];
-        float* dst = moments + (size_t)rank * vw.mom_stride + 4 * lane;
-        // no returning atomic here: a returned value would tie up a scoreboard for a full L2 round trip; the touched
-        // list is built afterwards from sum w^2 != 0 (launch_touched)
-        if (lane < 10) red_add_v4(dst, tot);
+        float4* ra = rawA + gcount * 4 * 32 + lane;
+        ra[0] = make_float4(F0s, F1s, F2s, F3s);
+        ra[32] = make_float4(F4s, W2.x + W2.y, gv[0], gv[1]);
+        ra[64] = make_float4(gv[2], gv[3], gv[4], gv[5]);
+        ra[96] = make_float4(gv[6], gv[7], gv[8], gv[9]);
+        rawB[gcount * 32 + lane] = make_float2(gv[10], gv[11]);
+        gpack |= (uint32_t)j << (8 * gcount);
+        ++gcount;
       }
+      }  // j < cnt
+      if (gcount == GE || (j == cnt && gcount > 0)) group_tail<NCH>(rawA, rawB, red, sm, sm_wh, sm_ex, q_rank, gcount, gpack, tx, ty, moments, vw.mom_stride, lane);
+      if (gcount == GE || j == cnt) { gcount = 0; gpack = 0u; }
     }
     e_next -= cnt;
     shift_queue(q_rank, nullptr, qn, (uint32_t)cnt);
