@@ -37,7 +37,7 @@ def _block_err(Hg, Ho, L):
     return np.abs(Hg - Ho) / (scale + 1e-3)
 
 
-@pytest.mark.parametrize("K,bg", [(3, 0), (6, 0), (6, 4), (9, 2), (22, 0)])      # K = 22: six groups, the K <= 52 instantiation
+@pytest.mark.parametrize("K,bg", [(3, 0), (6, 0), (6, 4), (9, 2), (22, 0), (50, 0), (52, 51)])      # K = 22: six groups; 50: config 4; 52 = NBV_MASK_KMAX
 def test_mask_image_and_blocks(K, bg):
     sc = _scene(K)
     cam = _cams(1, seed=K)[0]
