@@ -22,15 +22,15 @@
 
 namespace nbv {
 
-// ---- ordered touched list: the ranks whose sum w^2 (moment 39) is non-zero, i.e. the Gaussians with at least one
-// composited pixel, in increasing rank (= depth) order.  Pass 1 counts per block of 256 ranks, pass 2 offsets every block
+// ---- ordered touched list: the ranks S4 flagged (RasterView::touched_flag: it added moments to them, i.e. the Gaussians
+// with at least one composited pixel, sum w^2 != 0), in increasing rank (= depth) order.  Pass 1 counts per block of 256 ranks, pass 2 offsets every block
 // by the counts before it (each block sums them itself: at most a few thousand numbers) and writes its ranks in order.
 constexpr int TOUCH_T = 256;
 
 __global__ void __launch_bounds__(TOUCH_T) touched_count_kernel(const __grid_constant__ RasterBatch batch, int N) {
   const RasterView& vw = batch.v[blockIdx.y];
   const int r = blockIdx.x * TOUCH_T + threadIdx.x;
-  const bool hit = r < N && vw.moments[(size_t)r * vw.mom_stride + MOM_W2] != 0.0f;
+  const bool hit = r < N && vw.touched_flag[r] != 0;
   const int c = __syncthreads_count(hit);
   if (threadIdx.x == 0) vw.touched_cnt[blockIdx.x] = (uint32_t)c;
 }
@@ -44,7 +44,8 @@ __global__ void __launch_bounds__(TOUCH_T) touched_write_kernel(const __grid_con
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) before += __shfl_xor_sync(0xffffffffu, before, o);
   const int r = blockIdx.x * TOUCH_T + threadIdx.x;
-  const bool hit = r < N && vw.moments[(size_t)r * vw.mom_stride + MOM_W2] != 0.0f;
+  const bool hit = r < N && vw.touched_flag[r] != 0;
+  if (hit) vw.touched_flag[r] = 0;                          // this is the last reader: all-zero again for the next view
   const unsigned m = __ballot_sync(0xffffffffu, hit);
   if (lane == 0) { wsum[wid] = before; wcnt[wid] = (uint32_t)__popc(m); }
   __syncthreads();

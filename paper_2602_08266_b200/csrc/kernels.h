@@ -94,6 +94,8 @@ struct RasterView {
   uint32_t* tile_walk;       // per tile: list entries S3 consumed
   float* moments;            // rank r at moments + r * mom_stride (NMOM floats), zero on entry to S4 for every Gaussian
   int mom_stride;            // NMOM, or groups * NMOM in a mask context (one group of 4 object channels per S4 launch)
+  uint8_t* touched_flag;     // N bytes, zero on entry to S4: S4 sets flag[rank] for every rank it adds moments to (= sum w^2 != 0),
+                             // the ordered compaction reads and clears it (32x less traffic than testing moment 39 of every rank)
   uint32_t* touched;         // ranks with a non-zero block (counters->n_touched of them, in increasing rank order)
   uint32_t* touched_cnt;     // scratch of the ordered compaction: touched ranks per block of 256 ranks
   ViewCounters* counters;

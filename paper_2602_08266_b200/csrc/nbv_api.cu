@@ -333,12 +333,13 @@ int pre_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, 
     }
     if (upto >= STAGE_BACKWARD) {
       if (ctx->mask_mode) CKRET(ensure(ctx, s->gsplat, sizeof(Splat) * (size_t)N));
-      if (s->moments.cap < mom_bytes || !s->moments.p) s->moments_clean = false;
-      CKRET(ensure(ctx, s->moments, mom_bytes));
+      // the moments, then one flag byte per rank (kernels.h: touched_flag); both are all-zero between views
+      if (s->moments.cap < mom_bytes + (size_t)N || !s->moments.p) s->moments_clean = false;
+      CKRET(ensure(ctx, s->moments, mom_bytes + (size_t)N));
       CKRET(ensure(ctx, s->touched, 4 * (size_t)N));
       CKRET(ensure(ctx, s->touched_cnt, 4 * (size_t)touched_blocks(N)));
       CKRET(ensure(ctx, s->partials, 8 * (size_t)expand_partials()));
-      if (!s->moments_clean) CK(cudaMemsetAsync(s->moments.p, 0, mom_bytes, st));
+      if (!s->moments_clean) CK(cudaMemsetAsync(s->moments.p, 0, mom_bytes + (size_t)N, st));
       s->moments_clean = false;     // dirty until an expand kernel has consumed the touched list
     }
     PreView& v = pb.v[i];
@@ -443,6 +444,7 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     v.pix.T = s->pix_T.as<float>(); v.pix.last = s->pix_last.as<int32_t>();
     v.tile_cend = s->tile_cend.as<uint32_t>(); v.tile_elast = s->tile_elast.as<uint32_t>(); v.tile_walk = s->tile_walk.as<uint32_t>();
     v.moments = s->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = s->touched.as<uint32_t>();
+    v.touched_flag = reinterpret_cast<uint8_t*>(s->moments.p) + sizeof(float) * NMOM * (size_t)ctx->mask_groups * (size_t)ctx->N;
     v.touched_cnt = s->touched_cnt.as<uint32_t>(); v.counters = s->d_counters;
   }
   const TileGrid tg = sl[0]->tg;
@@ -1085,6 +1087,7 @@ int nbv_render_mask(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_mask, void* 
     v.pix.T = sl->pix_T.as<float>(); v.pix.last = sl->pix_last.as<int32_t>();
     v.tile_cend = sl->tile_cend.as<uint32_t>(); v.tile_elast = sl->tile_elast.as<uint32_t>(); v.tile_walk = sl->tile_walk.as<uint32_t>();
     v.moments = sl->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = sl->touched.as<uint32_t>();
+    v.touched_flag = nullptr;                            // forward pass only
     v.touched_cnt = sl->touched_cnt.as<uint32_t>(); v.counters = sl->d_counters;
     launch_forward(rb, sl->tg, sl->rank_bits, h_cam->width, h_cam->height, gcfg, true, st);
     launch_mask_scatter(sl->pix_rgb.as<float>(), sl->pix_depth.as<float>(), npx, ctx->K, gr, ctx->cfg.mask_bg_channel, d_mask, st);

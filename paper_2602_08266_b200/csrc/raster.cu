@@ -309,7 +309,7 @@ constexpr int GE = 4;
 template <int NCH>
 __device__ __forceinline__ void group_tail(const float4* rawA, const float2* rawB, float* red, const float4* sm, const float4* sm_wh,
                                            const float4* sm_ex, const uint32_t* q_rank, int gcount, uint32_t gpack, int tx, int ty,
-                                           float* __restrict__ moments, int mom_stride, int lane) {
+                                           float* __restrict__ moments, int mom_stride, uint8_t* __restrict__ flag, int lane) {
   __syncwarp();                                            // the parked column sums are visible
   const int ge = lane >> 3, part = lane & 7;
   float acc[NMOM];
@@ -367,7 +367,7 @@ __device__ __forceinline__ void group_tail(const float4* rawA, const float2* raw
   __syncwarp();
   // 4 entries x 10 float4 columns, each the sum of the 8 rows of its entry: columns 0..7 by all lanes, 8 and 9 by lanes 0..7.
   // No returning atomic: a returned value would tie up a scoreboard for a full L2 round trip; the touched list is built
-  // afterwards from sum w^2 != 0 (launch_touched)
+  // afterwards from one flag byte per rank (launch_touched)
 #pragma unroll
   for (int round = 0; round < 2; ++round) {
     const int e1 = round == 0 ? lane >> 3 : lane >> 1, q = round == 0 ? lane & 7 : 8 + (lane & 1);
@@ -381,6 +381,7 @@ __device__ __forceinline__ void group_tail(const float4* rawA, const float2* raw
       }
       const uint32_t rank = q_rank[(gpack >> (8 * e1)) & 0xffu];
       red_add_v4(moments + (size_t)rank * mom_stride + 4 * q, make_float4(a01.x, a01.y, a23.x, a23.y));
+      if (q == 0) flag[rank] = 1;                          // touched: the compaction of launch_touched reads these bytes
     }
   }
   __syncwarp();                                            // the buffers may be refilled
@@ -607,7 +608,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
         ++gcount;
       }
       }  // j < cnt
-      if (gcount == GE || (j == cnt && gcount > 0)) group_tail<NCH>(rawA, rawB, red, sm, sm_wh, sm_ex, q_rank, gcount, gpack, tx, ty, moments, vw.mom_stride, lane);
+      if (gcount == GE || (j == cnt && gcount > 0)) group_tail<NCH>(rawA, rawB, red, sm, sm_wh, sm_ex, q_rank, gcount, gpack, tx, ty, moments, vw.mom_stride, vw.touched_flag, lane);
       if (gcount == GE || j == cnt) { gcount = 0; gpack = 0u; }
     }
     e_next -= cnt;
