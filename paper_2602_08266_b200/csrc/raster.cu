@@ -430,7 +430,8 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   const uint32_t lt = (1u << lane) - 1u;
 
   // pair q: rows q (.x) and 7 - q (.y).  nS = MINUS the suffix sums, pre-scaled by sqrt(omega_ch) (see pass 2)
-  f2 Tc2[PPL / 2], py2[PPL / 2], nS[NCH][PPL / 2];
+  f2 Tc2[PPL / 2], nS[NCH][PPL / 2];
+  const float y0f = (float)y0;          // pixel centres py = y0f + (k + 0.5): small integers + 0.5, exact in binary32 (= S3's py bit for bit)
   int last_x[PPL / 2], last_y[PPL / 2];
 #pragma unroll
   for (int q = 0; q < PPL / 2; ++q) {
@@ -444,8 +445,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
         l = pix.last[p];
         T = pix.T[p];
       }
-      const float py = (float)(y0 + k) + 0.5f;
-      if (h) { last_y[q] = l; Tc2[q].y = T; py2[q].y = py; } else { last_x[q] = l; Tc2[q].x = T; py2[q].x = py; }
+      if (h) { last_y[q] = l; Tc2[q].y = T; } else { last_x[q] = l; Tc2[q].x = T; }
     }
 #pragma unroll
     for (int c = 0; c < NCH; ++c) {
@@ -515,7 +515,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       bool near = false;
 #pragma unroll
       for (int q = 0; q < PPL / 2; ++q) {
-        const f2 dy = sub2(py2[q], bc2(s0.y));
+        const f2 dy = sub2(add2(bc2(y0f), make_float2((float)q + 0.5f, (float)(PPL - 1 - q) + 0.5f)), bc2(s0.y));
         const f2 power = splat_power2(s0.z, s0.w, s1.x, dx, dy);
         const bool in_x = e < last_x[q] && power.x <= 0.0f;        // the lower bounds never decide (see forward_kernel)
         const bool in_y = e < last_y[q] && power.y <= 0.0f;
