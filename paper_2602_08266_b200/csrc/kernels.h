@@ -175,8 +175,7 @@ void launch_argmax(const float* scores, int n, int32_t* best, cudaStream_t st);
 void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uint32_t* ids_sorted, int group, int bgch, Splat* out,
                         cudaStream_t st);
 void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, double* H_T,
-                        const float* conf, const double* cholT, cudaStream_t st);
-void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const double* H_T, const float* conf, double* cholT, cudaStream_t st);
+                        const float* conf, cudaStream_t st);
 void launch_mask_scatter(const float* rgb, const float* depth, size_t npx, int K, int group, int bgch, float* mask, cudaStream_t st);
 
 // ---- sh.cu, SH degree 3 colour (NEXT-4): per-view colours in S1, 59 x 59 blocks in S5 / S6 (binary64, one warp per Gaussian)

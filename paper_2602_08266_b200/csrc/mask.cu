@@ -21,7 +21,7 @@ namespace nbv {
 //   geo-geo   (11 x 11)  A Q A^T
 //   geo-logit (11 x K)   sum_k (A x_k) dp_k/do_j = p_j (A x_j - sum_k p_k A x_k)
 //   logit-logit (K x K)  W2 sum_k dp_k/do_j dp_k/do_l = W2 (delta_jl p_j^2 - p_j p_l (p_j + p_l) + p_j p_l sum_k p_k^2)
-// and S6 is the same solve-form log-det gain on L x L blocks.
+// and S6 is the same pivot-ratio log-det gain on L x L blocks.
 // =====================================================================================================================
 __host__ __device__ __forceinline__ int mask_channel_of_slot(int t, int bgch) { return t == 0 ? bgch : (t <= bgch ? t - 1 : t); }
 __host__ __device__ __forceinline__ int mask_slot_of_channel(int c, int bgch) { return c == bgch ? 0 : (c < bgch ? c + 1 : c); }
@@ -50,32 +50,15 @@ void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uin
   mask_splat_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(splat_sorted, ids_sorted, sc.logits, sc.lse, sc.N, sc.K, group, bgch, out);
 }
 
-// upper Cholesky factor of a packed SPD L x L, in place (as cholesky_packed)
-__device__ void cholesky_L(double* Mx, int L) {
-  for (int j = 0; j < L; ++j) {
-    double d = Mx[triL(j, j, L)];
-    for (int k = 0; k < j; ++k) d -= Mx[triL(k, j, L)] * Mx[triL(k, j, L)];
-    d = fmax(d, 1e-300);
-    const double inv = rsqrt(d);
-    Mx[triL(j, j, L)] = d * inv;
-    for (int i = j + 1; i < L; ++i) {
-      double v = Mx[triL(j, i, L)];
-      for (int k = 0; k < j; ++k) v -= Mx[triL(k, j, L)] * Mx[triL(k, i, L)];
-      Mx[triL(j, i, L)] = v * inv;
-    }
-  }
-}
-
-// ---- S5' + S6 of a mask context, warp-cooperative: ONE WARP PER TOUCHED GAUSSIAN, the L x L block and the factor in shared
-// memory.  Lane l owns the columns (or rows) l, l + 32 of the matrices, so the triangular solves and the elimination run
-// on up to 63 columns at once (a first version ran one thread per Gaussian over 2 x 2016 floats of local memory).
-//   W = U^-T (c H) U^-1 : (a) every lane solves U^T x = h_j for its columns j, in place; (b) every lane solves
-//   U^T y = (row i of the result)^T for its rows i, in place.   log det(I + W): right-looking Cholesky on the excess
-//   (pivot 1 + e_j enters as log1p(e_j), as in gain_solve), one column per step, the trailing rows updated in parallel.
+// ---- S5' + S6 of a mask context, warp-cooperative: ONE WARP PER TOUCHED GAUSSIAN, two L x L matrices in shared memory
+// (a first version ran one thread per Gaussian over 2 x 2016 floats of local memory).  Lane l owns the columns (building the
+// block) or rows (elimination) l, l + 32.  S6 is the pivot-ratio form of the colour / depth contexts: M0 = c H_T + Lambda and
+// M1 = c (H_T + H) + Lambda are eliminated side by side (right-looking L D L^T, one column per step, the trailing rows updated
+// in parallel) and the gain is sum_j log(d1_j / d0_j).  No factor table, nothing cached between scoring calls.
 struct MaskWarpLayout {
   int LS;          // row stride of H and U (odd: conflict-free column and row walks)
   int per_warp;    // doubles per warp
-  int oH, oU, oA, oAQ, oMom, oX, oP, oMono;
+  int oH, oU, oA, oAQ, oMom, oX, oP, oMono, oPiv;
 };
 __host__ __device__ inline MaskWarpLayout mask_warp_layout(int K, int groups) {
   MaskWarpLayout m;
@@ -90,14 +73,14 @@ __host__ __device__ inline MaskWarpLayout mask_warp_layout(int K, int groups) {
   m.oX = o; o += K * 6;
   m.oP = o; o += K;
   m.oMono = o; o += 16;
+  m.oPiv = o; o += 2 * L;
   m.per_warp = (o + 3) & ~3;
   return m;
 }
 
 __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
                                                                 const __grid_constant__ ExpandBatch batch, int mode, int groups, int view0,
-                                                                double* __restrict__ H_T, const float* __restrict__ conf,
-                                                                const double* __restrict__ cholT) {
+                                                                double* __restrict__ H_T, const float* __restrict__ conf) {
   extern __shared__ __align__(16) double smem[];
   const ExpandView& vw = batch.v[view0 + blockIdx.y];
   const int K = sc.K, L = 11 + K, LB = L * (L + 1) / 2, bgch = cfg.mask_bg_channel;
@@ -105,7 +88,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5, LS = lay.LS;
   double* base = smem + (size_t)wib * lay.per_warp;
   double *Hm = base + lay.oH, *Um = base + lay.oU, *As = base + lay.oA, *AQs = base + lay.oAQ, *mom = base + lay.oMom;
-  double *xs = base + lay.oX, *ps = base + lay.oP, *mono = base + lay.oMono;
+  double *xs = base + lay.oX, *ps = base + lay.oP, *mono = base + lay.oMono, *piv = base + lay.oPiv;
   const uint32_t n_touched = vw.counters->n_touched;
   const int stride = NMOM * groups;
   double gain = 0.0;
@@ -226,46 +209,41 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       continue;
     }
     const double cg = conf[g];
-    const double cb = cfg.weight_mode == 1 ? 1.0 : cg;
+    const double ct = cfg.weight_mode == 0 ? cg : 1.0;        // Eq. 9 literal (R1) weights H_T as well; R2 / R3 do not
+    const double cb = cfg.weight_mode == 1 ? 1.0 : cg;        // R2 weights the gain, R1 / R3 the candidate block
     double gn = 0.0;
     if (cg > 0.0) {
-      const double* ut = cholT + (size_t)g * LB;
-      for (int rr = 0; rr < L; ++rr)
-        for (int c = rr + lane; c < L; c += 32) Um[rr * LS + c] = ut[triL(rr, c, L)];
-      __syncwarp();
-      // (a) columns: U^T x = c h_j
-      for (int j = lane; j < L; j += 32)
-        for (int i = 0; i < L; ++i) {
-          double v = cb * Hm[i * LS + j];
-#pragma unroll 4
-          for (int k = 0; k < i; ++k) v -= Um[k * LS + i] * Hm[k * LS + j];
-          Hm[i * LS + j] = v / Um[i * LS + i];
+      // M0 = ct H_T + Lambda -> Um,  M1 = M0 + cb H -> Hm  (lower triangles; H_T is stored packed upper, row-major)
+      const double* ht = H_T + (size_t)g * LB;
+      for (int rr = 0; rr < L; ++rr) {
+        const double pr = rr < 11 ? (double)cfg.prior_precision[rr] : (double)cfg.prior_precision_obj;
+        for (int c = rr + lane; c < L; c += 32) {
+          const double m0 = fma(ct, ht[triL(rr, c, L)], c == rr ? pr : 0.0);
+          Um[c * LS + rr] = m0;
+          Hm[c * LS + rr] = fma(cb, Hm[c * LS + rr], m0);
         }
+      }
       __syncwarp();
-      // (b) rows: U^T y = (row i)^T
-      for (int i = lane; i < L; i += 32)
-        for (int c = 0; c < L; ++c) {
-          double v = Hm[i * LS + c];
-#pragma unroll 4
-          for (int k = 0; k < c; ++k) v -= Um[k * LS + c] * Hm[i * LS + k];
-          Hm[i * LS + c] = v / Um[c * LS + c];
-        }
-      __syncwarp();
-      // log det(I + W): right-looking Cholesky on the excess, lower triangle
+      // two interleaved right-looking L D L^T (lower triangles, lane i owns rows i and i + 32); the gain is the sum of
+      // log(d1_j / d0_j) over the pivots, as in the colour / depth contexts (hessian.cu): 2 x L^3 / 6 multiply-adds instead of
+      // the two L^3 / 2 triangular solves + a Cholesky of the solve form used while this path was binary32
       for (int j = 0; j < L; ++j) {
-        const double e = fmax(Hm[j * LS + j], 0.0);
-        gn += log1p(e);
-        const double inv = rsqrt(1.0 + e);
-        __syncwarp();
-        for (int i = j + 1 + lane; i < L; i += 32) Hm[i * LS + j] *= inv;
-        __syncwarp();
+        const double d0 = fmax(Um[j * LS + j], 1e-300), d1 = fmax(Hm[j * LS + j], 1e-300);
+        if (lane == 0) { piv[j] = d0; piv[L + j] = d1; }
+        const double i0 = 1.0 / d0, i1 = 1.0 / d1;
         for (int i = j + 1 + lane; i < L; i += 32) {
-          const double li = Hm[i * LS + j];
+          const double l0 = Um[i * LS + j] * i0, l1 = Hm[i * LS + j] * i1;
 #pragma unroll 4
-          for (int k = j + 1; k <= i; ++k) Hm[i * LS + k] -= li * Hm[k * LS + j];
+          for (int k = j + 1; k <= i; ++k) {
+            Um[i * LS + k] = fma(-l0, Um[k * LS + j], Um[i * LS + k]);
+            Hm[i * LS + k] = fma(-l1, Hm[k * LS + j], Hm[i * LS + k]);
+          }
         }
         __syncwarp();
       }
+      for (int j = lane; j < L; j += 32) gn += log(piv[L + j] / piv[j]);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) gn += __shfl_xor_sync(0xffffffffu, gn, o);
     }
     if (cfg.weight_mode == 1) gn *= cg;
     if (lane == 0) {
@@ -285,7 +263,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
 }
 
 void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandBatch& batch, int mode, int groups, double* H_T,
-                        const float* conf, const double* cholT, cudaStream_t st) {
+                        const float* conf, cudaStream_t st) {
   const MaskWarpLayout lay = mask_warp_layout(sc.K, groups);
   int wpb = 8;
   while (wpb > 1 && (size_t)wpb * lay.per_warp * 8 > 200 * 1024) wpb >>= 1;
@@ -298,41 +276,13 @@ void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandB
     const int blocks = sm_count() * 2;
     for (int v = 0; v < batch.n; ++v) {
       ++g_kernel_launches;
-      expand_mask_warp_kernel<<<dim3((unsigned)blocks, 1u), wpb * 32, smem, st>>>(sc, cfg, batch, mode, groups, v, H_T, conf, cholT);
+      expand_mask_warp_kernel<<<dim3((unsigned)blocks, 1u), wpb * 32, smem, st>>>(sc, cfg, batch, mode, groups, v, H_T, conf);
     }
     return;
   }
   ++g_kernel_launches;
   const int blocks = std::max(1, (sm_count() * 2 + batch.n - 1) / batch.n);
-  expand_mask_warp_kernel<<<dim3((unsigned)blocks, (unsigned)batch.n), wpb * 32, smem, st>>>(sc, cfg, batch, mode, groups, 0, H_T, conf, cholT);
-}
-
-// once per scoring call of a mask context: U_g = upper Cholesky factor of c_g H_T,g + Lambda (L x L)
-template <int KMAX>
-__global__ void __launch_bounds__(64) prepare_mask_kernel(int N, int K, nbv_config cfg, const double* __restrict__ H_T,
-                                                           const float* __restrict__ conf, double* __restrict__ cholT) {
-  constexpr int LMAX = 11 + KMAX, LBMAX = LMAX * (LMAX + 1) / 2;
-  const int g = blockIdx.x * blockDim.x + threadIdx.x;
-  if (g >= N) return;
-  const double c = conf[g];
-  if (!(c > 0.0)) return;
-  const int L = 11 + K, LB = L * (L + 1) / 2;
-  const double* ht = H_T + (size_t)g * LB;
-  double H[LBMAX];
-  const double ct = cfg.weight_mode == 0 ? c : 1.0;
-  for (int i = 0; i < LB; ++i) H[i] = ct * ht[i];
-  for (int k = 0; k < L; ++k) H[triL(k, k, L)] += k < 11 ? cfg.prior_precision[k] : cfg.prior_precision_obj;
-  cholesky_L(H, L);
-  double* dst = cholT + (size_t)g * LB;
-  for (int i = 0; i < LB; ++i) dst[i] = H[i];
-}
-
-void launch_prepare_mask(const SceneDev& sc, const nbv_config& cfg, const double* H_T, const float* conf, double* cholT, cudaStream_t st) {
-  ++g_kernel_launches;
-  if (sc.K <= 20)
-    prepare_mask_kernel<20><<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, sc.K, cfg, H_T, conf, cholT);
-  else
-    prepare_mask_kernel<NBV_MASK_KMAX><<<(sc.N + 63) / 64, 64, 0, st>>>(sc.N, sc.K, cfg, H_T, conf, cholT);
+  expand_mask_warp_kernel<<<dim3((unsigned)blocks, (unsigned)batch.n), wpb * 32, smem, st>>>(sc, cfg, batch, mode, groups, 0, H_T, conf);
 }
 
 // parity export: (rgb | depth) images of one group's forward pass -> mask channels of that group

@@ -75,11 +75,10 @@ struct nbv_ctx {
   size_t LB = NBLK;
   int n_train = 0;
   // scene
-  // H_T: N x LB binary64 (LB = 105, or L (L + 1) / 2 in mask / SH contexts); cholT: mask contexts only, binary64
-  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, cholT, score_tmp, fuse_tmp, cache_ids, cache_blocks, cache_meta,
+  // H_T: N x LB binary64 (LB = 105, or L (L + 1) / 2 in mask / SH contexts)
+  DevBuf mean, logscale, quat, sigma, rgb, logits, M, pmax, amax, lse, H_T, conf, score_tmp, fuse_tmp, cache_ids, cache_blocks, cache_meta,
       cache_scratch, trace_buf, sh45, prior59;         // trace_buf: S_T (1 double) | scratch of launch_trace_total
   size_t greedy_cache_bytes = (size_t)4 << 30;   // budget of the block cache of nbv_select_greedy (NBV_GREEDY_CACHE_MB)
-  int conf_target = -2;                 // mask contexts: target the cholT buffer was prepared for (-2 = stale)
   // views in flight: S1-S2 of each view run on its slot's stream, S3-S6 of a whole batch in one launch per stage on
   // the caller's stream; two sets of `concurrency` slots alternate so the next batch's S1-S2 overlap this batch's S3-S6
   std::vector<ViewSlot*> slots;
@@ -498,8 +497,7 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     launch_cache_reserve(eb, *cache, first_candidate, st);
     launch_expand_cache(scene_dev(ctx), ctx->cfg, eb, *cache, st);
   } else if (ctx->mask_mode) {
-    launch_expand_mask(scene_dev(ctx), ctx->cfg, eb, mode, ctx->mask_groups, ctx->H_T.as<double>(), ctx->conf.as<float>(),
-                       ctx->cholT.as<double>(), st);
+    launch_expand_mask(scene_dev(ctx), ctx->cfg, eb, mode, ctx->mask_groups, ctx->H_T.as<double>(), ctx->conf.as<float>(), st);
   } else if (ctx->sh_mode) {
     launch_expand_sh(scene_dev(ctx), ctx->cfg, eb, mode, ctx->sh45.as<float>(), ctx->prior59.as<float>(), ctx->H_T.as<double>(),
                      ctx->conf.as<float>(), st);
@@ -579,13 +577,10 @@ int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_
 
 int prepare_scoring(nbv_ctx* ctx, int target, cudaStream_t st) {
   if (target < -1 || target >= ctx->K) return fail(ctx, NBV_ERR_UNKNOWN_TARGET, "target_obj must be -1 or in [0, K)");
-  // S0' runs in every scoring call (Eq. 7 / Eq. 12: N numbers).  Colour / depth contexts need nothing else: S6 factors
-  // c_g H_T,g + Lambda itself, for the touched Gaussians only.  Mask contexts keep a factor table, rebuilt when H_T or the
-  // target changed.
+  // S0' runs in every scoring call (Eq. 7 / Eq. 12: N numbers).  Nothing else is needed in any context: S6 factors
+  // c_g H_T,g + Lambda itself, for the touched Gaussians only.
   const SceneDev sc = scene_dev(ctx);
   launch_confidence(sc, ctx->cfg, target, ctx->conf.as<float>(), st);
-  if (ctx->mask_mode && ctx->conf_target != target)
-    launch_prepare_mask(sc, ctx->cfg, ctx->H_T.as<double>(), ctx->conf.as<float>(), ctx->cholT.as<double>(), st);
   if (ctx->cfg.criterion == NBV_CRIT_TRACE) {                // S_T of the trace criterion: all N blocks of the current H_T
     if (!ctx->trace_buf.p) {
       CKRET(ensure(ctx, ctx->trace_buf, 16 + trace_total_scratch_bytes()));
@@ -594,7 +589,6 @@ int prepare_scoring(nbv_ctx* ctx, int target, cudaStream_t st) {
     launch_trace_total(sc, ctx->cfg, ctx->H_T.as<double>(), ctx->conf.as<float>(), ctx->trace_buf.as<char>() + 16, ctx->trace_buf.as<double>(), st);
   }
   CK(cudaGetLastError());
-  ctx->conf_target = target;
   return NBV_OK;
 }
 
@@ -692,7 +686,7 @@ void nbv_destroy(nbv_ctx* ctx) {
   if (!ctx) return;
   cudaDeviceSynchronize();
   DevBuf* all[] = {&ctx->mean, &ctx->logscale, &ctx->quat, &ctx->sigma, &ctx->rgb, &ctx->logits, &ctx->M, &ctx->pmax, &ctx->amax,
-                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->cholT, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order, &ctx->work_counters, &ctx->counters_pool, &ctx->cache_ids,
+                   &ctx->lse, &ctx->H_T, &ctx->conf, &ctx->score_tmp, &ctx->fuse_tmp, &ctx->tile_order, &ctx->work_counters, &ctx->counters_pool, &ctx->cache_ids,
                    &ctx->cache_blocks, &ctx->cache_meta, &ctx->cache_scratch, &ctx->trace_buf, &ctx->sh45, &ctx->prior59};
   for (DevBuf* b : all) release(*b);
   for (ViewSlot* sl : ctx->slots) free_slot(sl);
@@ -735,7 +729,6 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
   CKRET(ensure(ctx, ctx->M, 36 * n)); CKRET(ensure(ctx, ctx->pmax, 4 * n)); CKRET(ensure(ctx, ctx->amax, 4 * n));
   const size_t ht_bytes = 8 * (size_t)ctx->LB * n;
   CKRET(ensure(ctx, ctx->lse, 4 * n)); CKRET(ensure(ctx, ctx->H_T, ht_bytes)); CKRET(ensure(ctx, ctx->conf, 4 * n));
-  if (ctx->mask_mode) CKRET(ensure(ctx, ctx->cholT, 8 * (size_t)ctx->LB * n));
   CK(cudaMemcpyAsync(ctx->mean.p, d_mean, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->logscale.p, d_logscale, 12 * n, cudaMemcpyDeviceToDevice, st));
   CK(cudaMemcpyAsync(ctx->quat.p, d_quat, 16 * n, cudaMemcpyDeviceToDevice, st));
@@ -754,7 +747,6 @@ int nbv_load_gaussians(nbv_ctx* ctx, int32_t N, int32_t K, const float* d_mean, 
   if (s0->h_counters->bad_data)
     return fail(ctx, NBV_ERR_BAD_DATA, "zero/non-finite quaternion, opacity outside (0,1) or non-finite parameter");
   ctx->n_train = 0;
-  ctx->conf_target = -2;
   ctx->loaded = true;
   return NBV_OK;
 }
@@ -779,7 +771,6 @@ int nbv_load_sh(nbv_ctx* ctx, const float* d_sh, void* stream) {
   CK(cudaStreamSynchronize(st));           // `prior` is a stack buffer
   ctx->sh_mode = true;
   ctx->n_train = 0;
-  ctx->conf_target = -2;
   return NBV_OK;
 }
 
@@ -788,7 +779,6 @@ int nbv_reset_training(nbv_ctx* ctx, void* stream) {
   if (!ctx->loaded) return fail(ctx, NBV_ERR_NOT_LOADED, "no Gaussians loaded");
   CK(cudaMemsetAsync(ctx->H_T.p, 0, 8 * (size_t)ctx->LB * ctx->N, (cudaStream_t)stream));
   ctx->n_train = 0;
-  ctx->conf_target = -2;
   return NBV_OK;
 }
 
@@ -800,7 +790,6 @@ int nbv_accumulate_training(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, v
   for (int i = 0; i < n; ++i)
     if (!valid_camera(h_cams[i])) return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
   if (n == 0) return NBV_OK;
-  ctx->conf_target = -2;
   CKRET(run_views(ctx, h_cams, n, EXPAND_TRAIN, nullptr, st));
   ctx->n_train += n;
   return NBV_OK;
@@ -955,7 +944,6 @@ int nbv_select_greedy(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n, int32_t
     launch_greedy_pick(d_round, d_taken, n, d_scores ? d_scores + (size_t)r * n : nullptr, d_pick, d_order + r, st);
     launch_cache_accumulate(bc, d_pick, ctx->H_T.as<double>(), st);      // Eq. 6: H_T += H(c*)
     CK(cudaGetLastError());
-    ctx->conf_target = -2;                                                // the factors of H_T are stale
     ++ctx->n_train;
   }
   CK(cudaMemcpyAsync(h_order, d_order, 4 * (size_t)rounds, cudaMemcpyDeviceToHost, st));
