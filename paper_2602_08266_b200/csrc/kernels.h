@@ -1,10 +1,12 @@
 // kernels.h -- host-side launchers of the CUDA kernels (internal to libnbv).
 #pragma once
+#include <atomic>
+
 #include "common.cuh"
 
 namespace nbv {
 
-extern unsigned long long g_kernel_launches;   // host-side count of kernel launches (nbv_kernel_launches)
+extern std::atomic<unsigned long long> g_kernel_launches;   // host-side count of kernel launches (nbv_kernel_launches)
 int sm_count();                                // multiprocessors of the current device (queried once per device)
 
 // One launch of every S1-S2 stage serves a BATCH of views (grid.y = view): the per-view device pointers travel as a

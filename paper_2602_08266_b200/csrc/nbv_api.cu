@@ -13,7 +13,7 @@
 using namespace nbv;
 
 namespace nbv {
-unsigned long long g_kernel_launches = 0;
+std::atomic<unsigned long long> g_kernel_launches{0};
 
 int sm_count() {
   static int cached[64] = {0};
@@ -987,7 +987,7 @@ int nbv_stage_times(nbv_ctx* ctx, double* h_ms, int64_t* h_views, void* stream) 
   return NBV_OK;
 }
 
-int64_t nbv_kernel_launches(void) { return (int64_t)nbv::g_kernel_launches; }
+int64_t nbv_kernel_launches(void) { return (int64_t)nbv::g_kernel_launches.load(); }
 
 int nbv_projected(nbv_ctx* ctx, const nbv_camera* h_cam, int32_t* d_visible, float* d_rec, int32_t* d_rect, void* stream) {
   if (!ctx || !h_cam) return NBV_ERR_INVALID_ARG;
