@@ -119,6 +119,8 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const __grid_constan
   const int words = (n_super + 31) >> 5;
   const uint32_t lt = (1u << lane) - 1u;
   const ushort4 rc = r < N ? rect_sorted[r] : make_ushort4(0, 0, 0, 0);
+  // this block's row of the scanned count table (supertile-major: one sector per supertile), needed after the first barrier
+  const uint32_t seg0 = (int)threadIdx.x < n_super ? scanned[(size_t)threadIdx.x * nblk + blockIdx.x] : 0u;
   uint32_t cm[MS_WORDS];
   super_mask(super_rect(rc, sshift), super_x, words, cm);
 #pragma unroll
@@ -132,8 +134,7 @@ __global__ void __launch_bounds__(MS_T) msplit_write_kernel(const __grid_constan
     }
   __syncthreads();
   if ((int)threadIdx.x < n_super) {
-    uint32_t run = scanned[(size_t)threadIdx.x * nblk + blockIdx.x];
-    seg[threadIdx.x] = run;
+    seg[threadIdx.x] = seg0;
     uint16_t* row = wc + threadIdx.x * (MS_W + 2);
     uint32_t before = 0;
 #pragma unroll
