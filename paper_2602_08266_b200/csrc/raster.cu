@@ -42,6 +42,12 @@ struct RasterParams {
   float ln_amax_over_amin;
 };
 
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
 // Can any pixel centre of the tile whose first centre is (X0 + 0.5, Y0 + 0.5) reach power >= tau?  Conservative: the
 // maximum of the concave quadratic over the BOX of the 16 x 16 centres (at the centre if it lies inside, else on an
 // edge, where the 1-D optimum is clamped to the edge), plus a slack that covers the binary32 rounding of both this
@@ -51,7 +57,10 @@ __device__ __forceinline__ bool ellipse_reaches_tile(float mx, float my, float q
   const float ax = sub_rn(X0 + 0.5f, mx), bx = add_rn(ax, (float)(TILE - 1));
   const float ay = sub_rn(Y0 + 0.5f, my), by = add_rn(ay, (float)(TILE - 1));
   if (ax <= 0.0f && bx >= 0.0f && ay <= 0.0f && by >= 0.0f) return true;
-  const float ry = div_rn(mul_rn(-0.5f, qb), qc), rx = div_rn(mul_rn(-0.5f, qb), qa);
+  // the 1-D optima -qb dx / (2 qc), -qb dy / (2 qa): approximate reciprocals (MUFU) instead of two IEEE divisions -- the test
+  // is conservative by the slack below, far above their 1-ulp error, and S3 / S4 still evaluate the very same expressions
+  const float hb = mul_rn(-0.5f, qb);
+  const float ry = mul_rn(hb, rcp_approx(qc)), rx = mul_rn(hb, rcp_approx(qa));
   const float thr = sub_rn(tau, 1e-3f);
   bool keep = false;
 #pragma unroll
@@ -159,18 +168,25 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   uint32_t pos = range.x, qn = 0;
   int e_base = 0;
   bool finished = __all_sync(FULL, ndone == PPL);
+  // The filter is a chain of dependent loads (rect -> key -> splat -> ellipse test) and was a third of this kernel's stall
+  // samples: the rect and key of the NEXT chunk of 32 list entries are requested as soon as the current chunk has been taken,
+  // so they are in flight during the splat loads of this chunk and the whole entry loop; only key -> splat remains exposed.
+  ushort4 nrc = make_ushort4(1, 1, 0, 0);                  // empty rect: covers no tile
+  uint32_t nkey = 0;
+  if (!finished && pos + lane < range.y) { nrc = crect[pos + lane]; nkey = ckeys[pos + lane]; }
   while (!finished) {
     // fill the queue with the next entries of the supertile list that can contribute to this tile
     while (qn < 32u && pos < range.y) {
       const uint32_t i = pos + lane;
-      bool hit = false;
-      if (i < range.y) {
-        const ushort4 rc = crect[i];
-        hit = tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
-      }
+      const ushort4 rc = nrc;
+      const uint32_t key = nkey;
+      bool hit = i < range.y && tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
+      pos += 32;
+      nrc = make_ushort4(1, 1, 0, 0);
+      if (pos + lane < range.y) { nrc = crect[pos + lane]; nkey = ckeys[pos + lane]; }
       uint32_t r = 0;
       if (hit) {
-        r = ckeys[i] & rmask;
+        r = key & rmask;
         const float4* sp = reinterpret_cast<const float4*>(splat_sorted + r);
         const float4 a0 = sp[0], a1 = sp[1];
         hit = ellipse_reaches_tile(a0.x, a0.y, a0.z, a0.w, a1.x, a1.w, X0, Y0);
@@ -182,7 +198,6 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
         q_cpos[slot] = i;
       }
       qn += __popc(m);
-      pos += 32;
     }
     if (qn == 0) break;
     const uint32_t cnt = min(qn, 32u);
@@ -274,11 +289,6 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   }  // persistent loop
 }
 
-__device__ __forceinline__ float rcp_approx(float x) {
-  float y;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
 
 constexpr int RED_STRIDE = 44;      // row stride (words) of the 32 x 40 reduction buffer: float4 rows, bank-conflict free
 
@@ -462,19 +472,22 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   int gcount = 0;                      // entries parked for the group tail, and their positions j in the staged batch (8 bits each)
   uint32_t gpack = 0u;
   const float thr_near = 2e-5f * prm.ln_amax_over_amin;
+  // rect and key of the next chunk (walking down from pos_hi) are requested one chunk ahead, as in forward_kernel
+  ushort4 nrc = make_ushort4(1, 1, 0, 0);
+  uint32_t nkey = 0;
+  if (pos_hi > cbegin && (uint32_t)lane < pos_hi - cbegin) { nrc = crect[pos_hi - 1u - (uint32_t)lane]; nkey = ckeys[pos_hi - 1u - (uint32_t)lane]; }
   for (;;) {
     while (qn < 32u && pos_hi > cbegin) {
       const uint32_t span = min(32u, pos_hi - cbegin);
-      bool hit = false;
-      uint32_t i = 0;
-      if ((uint32_t)lane < span) {
-        i = pos_hi - 1u - (uint32_t)lane;
-        const ushort4 rc = crect[i];
-        hit = tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
-      }
+      const ushort4 rc = nrc;
+      const uint32_t key = nkey;
+      bool hit = (uint32_t)lane < span && tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
+      pos_hi -= span;
+      nrc = make_ushort4(1, 1, 0, 0);
+      if (pos_hi > cbegin && (uint32_t)lane < pos_hi - cbegin) { nrc = crect[pos_hi - 1u - (uint32_t)lane]; nkey = ckeys[pos_hi - 1u - (uint32_t)lane]; }
       uint32_t r = 0;
       if (hit) {
-        r = ckeys[i] & rmask;
+        r = key & rmask;
         const float4* sp = reinterpret_cast<const float4*>(splat_sorted + r);
         const float4 a0 = sp[0], a1 = sp[1];
         hit = ellipse_reaches_tile(a0.x, a0.y, a0.z, a0.w, a1.x, a1.w, X0, Y0);
@@ -482,7 +495,6 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       const unsigned m = __ballot_sync(FULL, hit);
       if (hit) q_rank[qn + __popc(m & lt)] = r;
       qn += __popc(m);
-      pos_hi -= span;
     }
     if (qn == 0) break;
     const int cnt = (int)min(qn, 32u);
