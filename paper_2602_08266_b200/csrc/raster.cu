@@ -48,6 +48,8 @@ __device__ __forceinline__ float rcp_approx(float x) {
   return y;
 }
 
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 // Can any pixel centre of the tile whose first centre is (X0 + 0.5, Y0 + 0.5) reach power >= tau?  Conservative: the
 // maximum of the concave quadratic over the BOX of the 16 x 16 centres (at the centre if it lies inside, else on an
 // edge, where the 1-D optimum is clamped to the edge), plus a slack that covers the binary32 rounding of both this
@@ -168,22 +170,31 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   uint32_t pos = range.x, qn = 0;
   int e_base = 0;
   bool finished = __all_sync(FULL, ndone == PPL);
-  // The filter is a chain of dependent loads (rect -> key -> splat -> ellipse test) and was a third of this kernel's stall
-  // samples: the rect and key of the NEXT chunk of 32 list entries are requested as soon as the current chunk has been taken,
-  // so they are in flight during the splat loads of this chunk and the whole entry loop; only key -> splat remains exposed.
-  ushort4 nrc = make_ushort4(1, 1, 0, 0);                  // empty rect: covers no tile
-  uint32_t nkey = 0;
-  if (!finished && pos + lane < range.y) { nrc = crect[pos + lane]; nkey = ckeys[pos + lane]; }
+  // The lazy tile filter is a chain of dependent loads per chunk of 32 list entries (rect -> key -> splat record gathered by
+  // rank -> ellipse test) and was a third of this kernel's stall samples.  It is software-pipelined two chunks deep in
+  // registers: while chunk c is tested, rect and key of chunk c + 1 are already here -- its rect test is taken at once and the
+  // splat records it will need are requested into the L1 -- and rect and key of chunk c + 2 are in flight.
+  ushort4 rcA = make_ushort4(1, 1, 0, 0), rcB = rcA;       // empty rect: covers no tile
+  uint32_t keyA = 0, keyB = 0;
+  if (!finished) {
+    if (pos + lane < range.y) { rcA = crect[pos + lane]; keyA = ckeys[pos + lane]; }
+    if (pos + 32u + lane < range.y) { rcB = crect[pos + 32u + lane]; keyB = ckeys[pos + 32u + lane]; }
+  }
   while (!finished) {
     // fill the queue with the next entries of the supertile list that can contribute to this tile
     while (qn < 32u && pos < range.y) {
       const uint32_t i = pos + lane;
-      const ushort4 rc = nrc;
-      const uint32_t key = nkey;
+      const ushort4 rc = rcA;
+      const uint32_t key = keyA;
       bool hit = i < range.y && tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
       pos += 32;
-      nrc = make_ushort4(1, 1, 0, 0);
-      if (pos + lane < range.y) { nrc = crect[pos + lane]; nkey = ckeys[pos + lane]; }
+      rcA = rcB; keyA = keyB;
+      rcB = make_ushort4(1, 1, 0, 0);
+      if (pos + 32u + lane < range.y) { rcB = crect[pos + 32u + lane]; keyB = ckeys[pos + 32u + lane]; }
+      if (tx >= rcA.x && tx < rcA.z && ty >= rcA.y && ty < rcA.w) {      // next chunk's records (48 B: one or two sectors)
+        const char* nx = reinterpret_cast<const char*>(splat_sorted + (keyA & rmask));
+        prefetch_l1(nx); prefetch_l1(nx + 16);
+      }
       uint32_t r = 0;
       if (hit) {
         r = key & rmask;
@@ -472,19 +483,31 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   int gcount = 0;                      // entries parked for the group tail, and their positions j in the staged batch (8 bits each)
   uint32_t gpack = 0u;
   const float thr_near = 2e-5f * prm.ln_amax_over_amin;
-  // rect and key of the next chunk (walking down from pos_hi) are requested one chunk ahead, as in forward_kernel
-  ushort4 nrc = make_ushort4(1, 1, 0, 0);
-  uint32_t nkey = 0;
-  if (pos_hi > cbegin && (uint32_t)lane < pos_hi - cbegin) { nrc = crect[pos_hi - 1u - (uint32_t)lane]; nkey = ckeys[pos_hi - 1u - (uint32_t)lane]; }
+  // the lazy tile filter, software-pipelined two chunks deep as in forward_kernel (walking down from pos_hi)
+  ushort4 rcA = make_ushort4(1, 1, 0, 0), rcB = rcA;
+  uint32_t keyA = 0, keyB = 0;
+  {
+    const uint32_t left = pos_hi - min(pos_hi, cbegin);
+    if ((uint32_t)lane < left) { rcA = crect[pos_hi - 1u - (uint32_t)lane]; keyA = ckeys[pos_hi - 1u - (uint32_t)lane]; }
+    if ((uint32_t)lane + 32u < left) { rcB = crect[pos_hi - 33u - (uint32_t)lane]; keyB = ckeys[pos_hi - 33u - (uint32_t)lane]; }
+  }
   for (;;) {
     while (qn < 32u && pos_hi > cbegin) {
       const uint32_t span = min(32u, pos_hi - cbegin);
-      const ushort4 rc = nrc;
-      const uint32_t key = nkey;
+      const ushort4 rc = rcA;
+      const uint32_t key = keyA;
       bool hit = (uint32_t)lane < span && tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
       pos_hi -= span;
-      nrc = make_ushort4(1, 1, 0, 0);
-      if (pos_hi > cbegin && (uint32_t)lane < pos_hi - cbegin) { nrc = crect[pos_hi - 1u - (uint32_t)lane]; nkey = ckeys[pos_hi - 1u - (uint32_t)lane]; }
+      rcA = rcB; keyA = keyB;
+      rcB = make_ushort4(1, 1, 0, 0);
+      {
+        const uint32_t left = pos_hi - cbegin;               // entries not yet taken; chunk A covers the first 32 of them
+        if ((uint32_t)lane + 32u < left) { rcB = crect[pos_hi - 33u - (uint32_t)lane]; keyB = ckeys[pos_hi - 33u - (uint32_t)lane]; }
+      }
+      if (tx >= rcA.x && tx < rcA.z && ty >= rcA.y && ty < rcA.w) {
+        const char* nx = reinterpret_cast<const char*>(splat_sorted + (keyA & rmask));
+        prefetch_l1(nx); prefetch_l1(nx + 16);
+      }
       uint32_t r = 0;
       if (hit) {
         r = key & rmask;
