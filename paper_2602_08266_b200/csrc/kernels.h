@@ -85,6 +85,7 @@ struct PixelBuf {            // per-pixel outputs of the forward pass (H x W eac
 };
 // One launch of S3 / S4 / S5+S6 serves a BATCH of views (S3, S4: launch positions interleave the views; S5+S6: grid.y = view): per-view device pointers travel as a
 // __grid_constant__ kernel parameter.  All views of a batch share the image size.
+constexpr int TL_CAP = 1024;    // list entries per tile S3 hands to S4 (config 2 walks 138 on average)
 struct RasterView {
   const Splat* splat_sorted;
   const uint32_t* ckeys;
@@ -94,6 +95,8 @@ struct RasterView {
   uint32_t* tile_cend;       // per tile: coarse position + 1 of the last entry some pixel of the tile passed
   uint32_t* tile_elast;      // per tile: position + 1 of that entry in the tile's list (0: nothing composited)
   uint32_t* tile_walk;       // per tile: list entries S3 consumed
+  uint32_t* tlist;           // per tile TL_CAP ranks: the tile's list as S3 walked it (entry e at tlist[tile * TL_CAP + e]); S4 reads it
+                             // backwards instead of filtering the supertile list again (tiles that walked more fall back to the filter)
   float* moments;            // rank r at moments + r * mom_stride (NMOM floats), zero on entry to S4 for every Gaussian
   int mom_stride;            // NMOM, or groups * NMOM in a mask context (one group of 4 object channels per S4 launch)
   uint8_t* touched_flag;     // N bytes, zero on entry to S4: S4 sets flag[rank] for every rank it adds moments to (= sum w^2 != 0),
@@ -107,6 +110,8 @@ struct RasterBatch {
   uint32_t n_work;              // launch positions (tiles x views) of a raster launch
   uint32_t* work_fwd;           // forward: zeroed work counter of the persistent warps (nullptr: one block per position)
   uint32_t* work;               // backward: zeroed counter the persistent warps pull launch positions from (nullptr: one block per position)
+  uint32_t* work_fb;            // the same for the fallback launch of S4 (tiles whose list outgrew TL_CAP)
+  uint32_t* overflow;           // number of such tiles in the batch (S3 counts them; zero -> the fallback launch exits at once)
   const uint32_t* tile_order;   // launch position -> tile: tiles by increasing distance from the image centre, so the
                                 // long-running central tiles of a look-at view start first and the tail is made of cheap ones
   RasterView v[MAX_BATCH];

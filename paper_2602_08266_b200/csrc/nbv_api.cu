@@ -45,7 +45,7 @@ struct ViewSlot {
   cudaEvent_t done = nullptr;
   DevBuf splat, zkey, zkey_alt, ids, ids_alt, rect, abc, splat_sorted, rect_sorted, msplit, gsplat;
   DevBuf ckeys, crect, cranges, sort_tmp, scan_tmp, tile_counts;
-  DevBuf pix_rgb, pix_depth, pix_T, pix_nc, pix_last, tile_cend, tile_elast, tile_walk, moments, touched, touched_cnt, partials;
+  DevBuf pix_rgb, pix_depth, pix_T, pix_nc, pix_last, tile_cend, tile_elast, tile_walk, tlist, moments, touched, touched_cnt, partials;
   ViewCounters* d_counters = nullptr;
   ViewCounters* h_counters = nullptr;   // pinned
   // products of the last process_view()
@@ -231,7 +231,7 @@ void free_slot(ViewSlot* sl) {
   DevBuf* all[] = {&sl->splat, &sl->zkey, &sl->zkey_alt, &sl->ids, &sl->ids_alt, &sl->rect, &sl->abc, &sl->splat_sorted,
                    &sl->rect_sorted, &sl->msplit, &sl->gsplat, &sl->ckeys, &sl->crect, &sl->cranges, &sl->sort_tmp,
                    &sl->scan_tmp, &sl->tile_counts, &sl->pix_rgb, &sl->pix_depth, &sl->pix_T, &sl->pix_nc, &sl->pix_last,
-                   &sl->tile_cend, &sl->tile_elast, &sl->tile_walk, &sl->moments, &sl->touched, &sl->touched_cnt, &sl->partials};
+                   &sl->tile_cend, &sl->tile_elast, &sl->tile_walk, &sl->tlist, &sl->moments, &sl->touched, &sl->touched_cnt, &sl->partials};
   for (DevBuf* b : all) release(*b);
   if (sl->h_counters) cudaFreeHost(sl->h_counters);
   if (sl->done) cudaEventDestroy(sl->done);
@@ -326,6 +326,7 @@ int pre_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, 
       CKRET(ensure(ctx, s->pix_T, 4 * npx)); CKRET(ensure(ctx, s->pix_last, 4 * npx));
       CKRET(ensure(ctx, s->tile_cend, 4 * (size_t)n_tiles)); CKRET(ensure(ctx, s->tile_walk, 4 * (size_t)n_tiles));
       CKRET(ensure(ctx, s->tile_elast, 4 * (size_t)n_tiles));
+      CKRET(ensure(ctx, s->tlist, 4 * (size_t)n_tiles * TL_CAP));
       if (full_pix) {
         CKRET(ensure(ctx, s->pix_rgb, 12 * npx)); CKRET(ensure(ctx, s->pix_depth, 4 * npx)); CKRET(ensure(ctx, s->pix_nc, 4 * npx));
       }
@@ -425,12 +426,16 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
   rb.n_work = 0;
   rb.work = nullptr;
   rb.work_fwd = nullptr;
+  rb.work_fb = nullptr;
+  rb.overflow = nullptr;
   if (ctx->persistent) {
     // one counter per raster stream (launches on a stream are ordered); the parity exports run on the caller's stream
     const int wi = st == ctx->raster_st[0] ? 0 : st == ctx->raster_st[1] ? 1 : 2;
-    rb.work = ctx->work_counters.as<uint32_t>() + 32 * wi;
-    rb.work_fwd = rb.work + 1;
-    CK(cudaMemsetAsync(rb.work, 0, 8, st));
+    rb.work = ctx->work_counters.as<uint32_t>() + 32 * wi;      // [work, work_fb, work_fwd, overflow]
+    rb.work_fb = rb.work + 1;
+    rb.work_fwd = rb.work + 2;
+    rb.overflow = rb.work + 3;
+    CK(cudaMemsetAsync(rb.work, 0, 16, st));
   }
   for (int i = 0; i < n; ++i) {
     ViewSlot* s = sl[i];
@@ -442,6 +447,7 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     v.pix.ncontrib = full_pix ? s->pix_nc.as<int32_t>() : nullptr;
     v.pix.T = s->pix_T.as<float>(); v.pix.last = s->pix_last.as<int32_t>();
     v.tile_cend = s->tile_cend.as<uint32_t>(); v.tile_elast = s->tile_elast.as<uint32_t>(); v.tile_walk = s->tile_walk.as<uint32_t>();
+    v.tlist = s->tlist.as<uint32_t>();
     v.moments = s->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = s->touched.as<uint32_t>();
     v.touched_flag = reinterpret_cast<uint8_t*>(s->moments.p) + sizeof(float) * NMOM * (size_t)ctx->mask_groups * (size_t)ctx->N;
     v.touched_cnt = s->touched_cnt.as<uint32_t>(); v.counters = s->d_counters;
@@ -468,7 +474,7 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
         gb.v[i].splat_sorted = sl[i]->gsplat.as<Splat>();
         gb.v[i].moments = sl[i]->moments.as<float>() + (size_t)gr * NMOM;
       }
-      if (gr > 0 && gb.work) CK(cudaMemsetAsync(gb.work, 0, 4, st));     // a fresh work counter for every launch
+      if (gr > 0 && gb.work) CK(cudaMemsetAsync(gb.work, 0, 8, st));     // fresh work counters (main + fallback) for every launch
       launch_backward(gb, ctx->N, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, gcfg, st);
     }
   }
@@ -1067,13 +1073,14 @@ int nbv_render_mask(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_mask, void* 
     const nbv_config gcfg = mask_group_config(ctx, gr);
     launch_mask_splats(sc, sl->splat_sorted.as<Splat>(), sl->ids.as<uint32_t>(), gr, ctx->cfg.mask_bg_channel, sl->gsplat.as<Splat>(), st);
     RasterBatch rb;
-    rb.n = 1; rb.n_work = 0; rb.work = nullptr; rb.work_fwd = nullptr;
+    rb.n = 1; rb.n_work = 0; rb.work = nullptr; rb.work_fwd = nullptr; rb.work_fb = nullptr; rb.overflow = nullptr;
     rb.tile_order = ctx->tile_order.as<uint32_t>();
     RasterView& v = rb.v[0];
     v.splat_sorted = sl->gsplat.as<Splat>(); v.ckeys = sl->ckeys_sorted; v.crect = sl->crect.as<ushort4>(); v.cranges = sl->cranges.as<uint2>();
     v.pix.rgb = sl->pix_rgb.as<float>(); v.pix.depth = sl->pix_depth.as<float>(); v.pix.ncontrib = sl->pix_nc.as<int32_t>();
     v.pix.T = sl->pix_T.as<float>(); v.pix.last = sl->pix_last.as<int32_t>();
     v.tile_cend = sl->tile_cend.as<uint32_t>(); v.tile_elast = sl->tile_elast.as<uint32_t>(); v.tile_walk = sl->tile_walk.as<uint32_t>();
+    v.tlist = nullptr;                                   // forward pass only
     v.moments = sl->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = sl->touched.as<uint32_t>();
     v.touched_flag = nullptr;                            // forward pass only
     v.touched_cnt = sl->touched_cnt.as<uint32_t>(); v.counters = sl->d_counters;

@@ -213,6 +213,9 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
     if (qn == 0) break;
     const uint32_t cnt = min(qn, 32u);
     __syncwarp();
+    // hand the tile's list to S4: entry e_base + lane is rank q_rank[lane] (S4 reads it backwards and filters nothing)
+    if (vw.tlist && (uint32_t)lane < cnt && (uint32_t)e_base + lane < (uint32_t)TL_CAP)
+      vw.tlist[(size_t)tile * TL_CAP + e_base + lane] = q_rank[lane];
     stage_queue(splat_sorted, q_rank, q_cpos, cnt, sm);
     for (uint32_t j = 0; j < cnt; ++j) {
       const float4 s0 = sm[j * 3], s1 = sm[j * 3 + 1], s2 = sm[j * 3 + 2];
@@ -291,6 +294,7 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
     vw.tile_cend[tile] = cend;
     vw.tile_elast[tile] = elast;
     vw.tile_walk[tile] = walked;
+    if (elast > (uint32_t)TL_CAP && batch.overflow) atomicAdd(batch.overflow, 1u);     // S4's fallback launch takes this tile
     if (FULLPIX) {
       atomicAdd(&counters->n_entries, (unsigned long long)walked);
       atomicAdd(&counters->n_pairs, (unsigned long long)pairs);
@@ -411,7 +415,10 @@ __device__ __forceinline__ void group_tail(const float4* rawA, const float2* raw
 // S4 slot body: the lane's 8 pixels as 4 pairs (row q, row 7 - q), packed binary32 operations throughout.  With the row
 // offsets t = -(3.5 - q) (.x) and +(3.5 - q) (.y), the column sums  F_p = sum_k f_k t_k^p,  G_c,p = sum_k g_c,k t_k^p  are
 // accumulated per half with the broadcast weights |t|^p and folded at the end:  F_p = hi + (-1)^p lo.
-template <int NCH>
+// FROM_LIST: the tile's entries come from the list S3 wrote (RasterView::tlist), read backwards one chunk of 32 ranks ahead --
+// no rect test, no ellipse test, no gather before the staging; tiles whose list outgrew TL_CAP are left to the instantiation
+// without FROM_LIST, which filters the supertile list again as S3 did and exits at once when the batch has no such tile.
+template <int NCH, bool FROM_LIST>
 __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
   __shared__ float4 sm[32 * 3];
   __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
@@ -425,9 +432,11 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   const int lane = threadIdx.x;
   // Persistent warps (batch.work != nullptr): the grid is one wave of resident warps and every warp pulls launch positions
   // from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
+  uint32_t* const work = FROM_LIST ? batch.work : batch.work_fb;
+  if (!FROM_LIST && batch.overflow && *batch.overflow == 0u) return;      // no tile of the batch outgrew its list
   for (uint32_t bpos = blockIdx.x;; ) {
-  if (batch.work) {
-    if (lane == 0) bpos = atomicAdd(batch.work, 1u);
+  if (work) {
+    if (lane == 0) bpos = atomicAdd(work, 1u);
     bpos = __shfl_sync(FULL, bpos, 0);
   }
   if (bpos >= batch.n_work) return;
@@ -442,7 +451,9 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   float* __restrict__ moments = vw.moments;
   const int tile = batch.tile_order[bpos / (uint32_t)batch.n];   // heaviest tiles first (launch order)
   const uint32_t elast = vw.tile_elast[tile];             // list position + 1 of the last entry any pixel of the tile passed
-  if (elast == 0u) { if (batch.work) continue; return; }
+  // which instantiation owns the tile: the list holds the first TL_CAP entries only
+  const bool listed = vw.tlist != nullptr && elast <= (uint32_t)TL_CAP;
+  if (elast == 0u || listed != FROM_LIST) { if (work) continue; return; }
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -475,54 +486,76 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
     }
   }
 
-  // walk the supertile list backwards from the last passed entry; the entries that pass the rect test are the
-  // tile-list entries elast-1, elast-2, ..., 0 in that order
-  const uint32_t cbegin = cranges[(ty >> prm.sshift) * prm.super_x + (tx >> prm.sshift)].x;
-  uint32_t pos_hi = vw.tile_cend[tile], qn = 0;
   int e_next = (int)elast - 1;
   int gcount = 0;                      // entries parked for the group tail, and their positions j in the staged batch (8 bits each)
   uint32_t gpack = 0u;
   const float thr_near = 2e-5f * prm.ln_amax_over_amin;
-  // the lazy tile filter, software-pipelined two chunks deep as in forward_kernel (walking down from pos_hi)
-  ushort4 rcA = make_ushort4(1, 1, 0, 0), rcB = rcA;
+  // FROM_LIST: entries elast-1, ..., 0 of the list S3 wrote, 32 at a time; the ranks of the next chunk are loaded before the
+  // entry loop of this one and their splat records requested into the L1, so the staging finds them there
+  const uint32_t* __restrict__ tl = FROM_LIST ? vw.tlist + (size_t)tile * TL_CAP : nullptr;
+  uint32_t nrank = 0;
+  if (FROM_LIST && lane <= e_next) nrank = tl[e_next - lane];
+  // !FROM_LIST: walk the supertile list backwards from the last passed entry; the entries that pass the rect and ellipse tests
+  // are the tile-list entries elast-1, elast-2, ..., 0 in that order
+  uint32_t cbegin = 0, pos_hi = 0, qn = 0;
+  ushort4 rcA = make_ushort4(1, 1, 0, 0), rcB = rcA;       // the lazy tile filter, software-pipelined two chunks deep as in forward_kernel
   uint32_t keyA = 0, keyB = 0;
-  {
+  if (!FROM_LIST) {
+    cbegin = cranges[(ty >> prm.sshift) * prm.super_x + (tx >> prm.sshift)].x;
+    pos_hi = vw.tile_cend[tile];
     const uint32_t left = pos_hi - min(pos_hi, cbegin);
     if ((uint32_t)lane < left) { rcA = crect[pos_hi - 1u - (uint32_t)lane]; keyA = ckeys[pos_hi - 1u - (uint32_t)lane]; }
     if ((uint32_t)lane + 32u < left) { rcB = crect[pos_hi - 33u - (uint32_t)lane]; keyB = ckeys[pos_hi - 33u - (uint32_t)lane]; }
   }
   for (;;) {
-    while (qn < 32u && pos_hi > cbegin) {
-      const uint32_t span = min(32u, pos_hi - cbegin);
-      const ushort4 rc = rcA;
-      const uint32_t key = keyA;
-      bool hit = (uint32_t)lane < span && tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
-      pos_hi -= span;
-      rcA = rcB; keyA = keyB;
-      rcB = make_ushort4(1, 1, 0, 0);
-      {
-        const uint32_t left = pos_hi - cbegin;               // entries not yet taken; chunk A covers the first 32 of them
-        if ((uint32_t)lane + 32u < left) { rcB = crect[pos_hi - 33u - (uint32_t)lane]; keyB = ckeys[pos_hi - 33u - (uint32_t)lane]; }
+    int cnt;
+    if (FROM_LIST) {
+      if (e_next < 0) break;
+      cnt = min(32, e_next + 1);
+      __syncwarp();
+      if (lane < cnt) q_rank[lane] = nrank;                 // staged slot j <-> list entry e_next - j
+      const int e_after = e_next - cnt;                     // first entry of the next chunk
+      nrank = 0;
+      if (lane <= e_after) nrank = tl[e_after - lane];
+      __syncwarp();
+      stage_queue(splat_sorted, q_rank, nullptr, (uint32_t)cnt, sm);
+      if (lane <= e_after) {                                // 48-byte records: two sectors
+        const char* nx = reinterpret_cast<const char*>(splat_sorted + nrank);
+        prefetch_l1(nx); prefetch_l1(nx + 32);
       }
-      if (tx >= rcA.x && tx < rcA.z && ty >= rcA.y && ty < rcA.w) {
-        const char* nx = reinterpret_cast<const char*>(splat_sorted + (keyA & rmask));
-        prefetch_l1(nx); prefetch_l1(nx + 16);
+    } else {
+      while (qn < 32u && pos_hi > cbegin) {
+        const uint32_t span = min(32u, pos_hi - cbegin);
+        const ushort4 rc = rcA;
+        const uint32_t key = keyA;
+        bool hit = (uint32_t)lane < span && tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
+        pos_hi -= span;
+        rcA = rcB; keyA = keyB;
+        rcB = make_ushort4(1, 1, 0, 0);
+        {
+          const uint32_t left = pos_hi - cbegin;             // entries not yet taken; chunk A covers the first 32 of them
+          if ((uint32_t)lane + 32u < left) { rcB = crect[pos_hi - 33u - (uint32_t)lane]; keyB = ckeys[pos_hi - 33u - (uint32_t)lane]; }
+        }
+        if (tx >= rcA.x && tx < rcA.z && ty >= rcA.y && ty < rcA.w) {
+          const char* nx = reinterpret_cast<const char*>(splat_sorted + (keyA & rmask));
+          prefetch_l1(nx); prefetch_l1(nx + 16);
+        }
+        uint32_t r = 0;
+        if (hit) {
+          r = key & rmask;
+          const float4* sp = reinterpret_cast<const float4*>(splat_sorted + r);
+          const float4 a0 = sp[0], a1 = sp[1];
+          hit = ellipse_reaches_tile(a0.x, a0.y, a0.z, a0.w, a1.x, a1.w, X0, Y0);
+        }
+        const unsigned m = __ballot_sync(FULL, hit);
+        if (hit) q_rank[qn + __popc(m & lt)] = r;
+        qn += __popc(m);
       }
-      uint32_t r = 0;
-      if (hit) {
-        r = key & rmask;
-        const float4* sp = reinterpret_cast<const float4*>(splat_sorted + r);
-        const float4 a0 = sp[0], a1 = sp[1];
-        hit = ellipse_reaches_tile(a0.x, a0.y, a0.z, a0.w, a1.x, a1.w, X0, Y0);
-      }
-      const unsigned m = __ballot_sync(FULL, hit);
-      if (hit) q_rank[qn + __popc(m & lt)] = r;
-      qn += __popc(m);
+      if (qn == 0) break;
+      cnt = (int)min(qn, 32u);
+      __syncwarp();
+      stage_queue(splat_sorted, q_rank, nullptr, (uint32_t)cnt, sm);
     }
-    if (qn == 0) break;
-    const int cnt = (int)min(qn, 32u);
-    __syncwarp();
-    stage_queue(splat_sorted, q_rank, nullptr, (uint32_t)cnt, sm);
     if (lane < cnt) {
       // Cholesky whitening of the footprint: xi = L^-1 d with Sigma2D = L L^T (L lower triangular), from the conic
       // Sigma2D^-1 = [[cA, cB], [cB, cC]]:  1/l22 = sqrt(cC),  1/l11 = sqrt(det(conic) / cC),  l21/l11 = -cB / cC
@@ -647,9 +680,9 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       if (gcount == GE || j == cnt) { gcount = 0; gpack = 0u; }
     }
     e_next -= cnt;
-    shift_queue(q_rank, nullptr, qn, (uint32_t)cnt);
+    if (!FROM_LIST) shift_queue(q_rank, nullptr, qn, (uint32_t)cnt);
   }
-  if (!batch.work) return;
+  if (!work) return;
   }  // persistent loop
 }
 
@@ -691,10 +724,15 @@ void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int ra
   if (b.work) blocks = std::min(blocks, (unsigned)sm_count() * NBV_BWD_MIN_BLOCKS);
   const dim3 grid(blocks);
   ++g_kernel_launches;
-  if (cfg.channel_mask & NBV_CH_DEPTH)
-    backward_kernel<4><<<grid, 32, 0, st>>>(b, p);
-  else
-    backward_kernel<3><<<grid, 32, 0, st>>>(b, p);
+  // main launch: the tiles whose list S3 handed over; fallback launch: the tiles that outgrew it (exits at once if none did)
+  if (cfg.channel_mask & NBV_CH_DEPTH) {
+    backward_kernel<4, true><<<grid, 32, 0, st>>>(b, p);
+    backward_kernel<4, false><<<grid, 32, 0, st>>>(b, p);
+  } else {
+    backward_kernel<3, true><<<grid, 32, 0, st>>>(b, p);
+    backward_kernel<3, false><<<grid, 32, 0, st>>>(b, p);
+  }
+  ++g_kernel_launches;
   (void)N;
 }
 

@@ -354,3 +354,34 @@ def test_prior_precisions_other_than_one(wl, prior):
     assert int(best.item()) == ref["best"]
     g = nbv.gaussian_gains(wl.cand_cams[2]).cpu().numpy()
     np.testing.assert_allclose(g, ref["gains"][2], rtol=1e-3, atol=1e-6)
+
+
+def test_tile_lists_longer_than_the_handover_capacity_take_the_fallback_path():
+    """S3 hands S4 the first 1,024 entries of every tile's list (kernels.h: TL_CAP); a tile that walks more is processed by
+    the S4 instantiation that filters the supertile list again.  3,000 faint Gaussians (sigma = 0.006: alpha barely above
+    1/255, the transmittance needs ~1,500 of them to fall below 1e-4) stacked in the middle of a 48 x 40 image make the
+    central tiles do that while the outer ones stay short, at two distances: images, counts, blocks, gains and scores against the oracle."""
+    rng = np.random.default_rng(77)
+    n = 3000
+    mean = np.c_[rng.uniform(-0.02, 0.02, n), rng.uniform(-0.02, 0.02, n), rng.uniform(-0.05, 0.05, n)]
+    sc = scene_from_arrays(mean, np.full((n, 3), -2.8), np.c_[np.ones(n), rng.normal(0, 0.2, (n, 3))], np.full(n, 0.006),
+                           rng.uniform(0, 1, (n, 3)))
+    cams = [synth.simple_camera(48, 40, 60.0, dist=0.5), synth.simple_camera(48, 40, 60.0, dist=3.0)]
+    scn = make_oracle_scene(sc, channel_mask=15)
+    nbv = _nbv(sc, channel_mask=15)
+    walked, _ = [t.cpu().numpy() for t in nbv.tile_walk(cams[0])]
+    assert walked.max() > 1024 and walked.min() <= 1024, (walked.min(), walked.max())      # both S4 instantiations have tiles
+    for cam in cams:
+        ro = scn.render(cam)
+        rg = {k: v.cpu().numpy() for k, v in nbv.render(cam).items()}
+        np.testing.assert_array_equal(rg["ncontrib"], ro["ncontrib"])
+        np.testing.assert_allclose(rg["rgb"], ro["rgb"], atol=1e-5, rtol=0)
+        Ho = scn.view_hessian(cam)
+        Hg = nbv.view_hessian(cam).cpu().numpy().astype(np.float64)
+        np.testing.assert_array_equal(np.abs(Hg).sum(axis=1) > 0, np.abs(Ho).sum(axis=1) > 0)
+        assert block_rel_err(Hg, Ho).max() < 1e-3
+    nbv.accumulate_training(cams[1:])
+    ref = orc.score_candidates(scn, cams[1:], cams, -1)
+    s, best = nbv.score_candidates(cams)
+    np.testing.assert_allclose(s.cpu().numpy(), ref["scores"], rtol=1e-3, atol=1e-6)
+    assert int(best.item()) == ref["best"]
