@@ -43,13 +43,13 @@ FP32_LANES_PER_SM = 128
 # of one launch of each raster kernel, divided by the (pixel, list entry) evaluations of that launch (walked entries x 256).
 # Both slot bodies are branch-free, so the executed work is proportional to the evaluations, composited or not; S4's
 # per-entry moment assembly and reduction are amortised into its figure.  Source: FLOP_SOURCE (committed ncu pass).
-FLOP_PER_EVAL = {"forward": 31.8, "backward": {3: 85.5, 4: 100.8}}
+FLOP_PER_EVAL = {"forward": 31.6, "backward": {3: 84.7, 4: 99.9}}
 FLOP_SOURCE = "profiles/r2_ncu_flops_cfg2.md"
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
 VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (16 for images of fewer than 2,000 tiles)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture named
 # in TRAFFIC_SOURCE; known for config 2 only (null elsewhere)
-NCU_TRAFFIC_BYTES = {2: {"backward": 98.45e6, "forward": 40.94e6}}
+NCU_TRAFFIC_BYTES = {2: {"backward": 102.9e6, "forward": 56.3e6}}
 TRAFFIC_SOURCE = "profiles/r2_ncu_raster_cfg2.md (ncu --set full of the first candidate batch; a stored figure, not measured by this run)"
 
 
