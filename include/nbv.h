@@ -253,6 +253,13 @@ int nbv_stage_times(nbv_ctx* ctx, double* h_ms, int64_t* h_views, void* stream);
  * actually holds; bench.py reports it beside the nominal SMs x 128 lanes x 2 x clock.  Synchronises `stream`. */
 int nbv_measure_ffma_peak(double* h_tflops, void* stream);
 
+/* Parity export of the decision path's exponential as the raster kernels evaluate it (exp_spec): the
+ * packed routine takes its last step, bits(p) + (k << 23), as p * 2^k with 2^k from MUFU.EX2 -- bit-identical on the whole
+ * domain [-80, 80] on hardware whose ex2.approx is exact at integers; tests compare it bit for bit with the oracle's
+ * exp_spec so that a device where that does not hold fails loudly.  DEVICE in d_x (n floats), DEVICE out d_y (n floats);
+ * elements are processed in pairs (2i, 2i + 1) as the kernels do.  Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA. */
+int nbv_exp_spec_pairs(const float* d_x, float* d_y, int64_t n, void* stream);
+
 /* Number of CUDA kernels this library has launched in this process so far (all contexts). */
 int64_t nbv_kernel_launches(void);
 

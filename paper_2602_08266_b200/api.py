@@ -36,7 +36,7 @@ EXPORTS = [
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
     "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
     "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy", "nbv_block_size", "nbv_render_mask", "nbv_measure_ffma_peak",
-    "nbv_chain", "nbv_load_sh",
+    "nbv_chain", "nbv_load_sh", "nbv_exp_spec_pairs",
 ]
 
 STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
@@ -344,6 +344,17 @@ class NBV:
         gains = torch.empty(self.N, dtype=torch.float32, device=self.device)
         self._check(self.lib.nbv_gaussian_gains(self._h, C.c_void_p(cam.ctypes.data), int(target_obj), _ptr(gains), _stream()))
         return gains
+
+
+def exp_spec_pairs(x):
+    """nbv_exp_spec_pairs: the raster kernels' packed exp_spec on a CUDA float32 tensor (returns a tensor of the same shape)."""
+    import torch
+    x = x.contiguous()
+    y = torch.empty_like(x)
+    rc = load_library().nbv_exp_spec_pairs(_ptr(x), _ptr(y), C.c_int64(x.numel()), _stream())
+    if rc != 0:
+        raise NBVError(rc, "nbv_exp_spec_pairs failed")
+    return y
 
 
 def measure_ffma_peak() -> float:

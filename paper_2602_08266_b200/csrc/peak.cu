@@ -26,7 +26,25 @@ __global__ void __launch_bounds__(1024) ffma_chain_kernel(int iters, float a, fl
   if (s == 123.456f) sink[0] = s;            // never true in practice: keeps the chains alive
 }
 
+// parity export: the raster kernels' packed exp_spec on pairs of arguments
+__global__ void __launch_bounds__(256) exp_spec_pairs_kernel(const float* __restrict__ x, float* __restrict__ y, long long n) {
+  const long long i = 2 * ((long long)blockIdx.x * blockDim.x + threadIdx.x);
+  if (i >= n) return;
+  const bool two = i + 1 < n;
+  const f2 r = exp_spec2(make_float2(x[i], two ? x[i + 1] : 0.0f));
+  y[i] = r.x;
+  if (two) y[i + 1] = r.y;
+}
+
 }  // namespace nbv
+
+extern "C" int nbv_exp_spec_pairs(const float* d_x, float* d_y, int64_t n, void* stream) {
+  if (!d_x || !d_y || n < 0) return NBV_ERR_INVALID_ARG;
+  if (n == 0) return NBV_OK;
+  ++nbv::g_kernel_launches;
+  nbv::exp_spec_pairs_kernel<<<(unsigned)((n / 2 + 256) / 256), 256, 0, (cudaStream_t)stream>>>(d_x, d_y, (long long)n);
+  return cudaGetLastError() == cudaSuccess ? NBV_OK : NBV_ERR_CUDA;
+}
 
 extern "C" int nbv_measure_ffma_peak(double* h_tflops, void* stream) {
   if (!h_tflops) return NBV_ERR_INVALID_ARG;

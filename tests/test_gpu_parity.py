@@ -385,3 +385,25 @@ def test_tile_lists_longer_than_the_handover_capacity_take_the_fallback_path():
     s, best = nbv.score_candidates(cams)
     np.testing.assert_allclose(s.cpu().numpy(), ref["scores"], rtol=1e-3, atol=1e-6)
     assert int(best.item()) == ref["best"]
+
+
+def test_packed_exp_spec_is_the_specified_exp_spec_bit_for_bit():
+    """The raster kernels take the last step of exp_spec (bits(p) + (k << 23)) as p * 2^k with 2^k from
+    MUFU.EX2.  That is the same binary32 number only where ex2.approx is exact at integers and the product is normal: every
+    argument the decision path can see, [-80, 80] -- checked here against the oracle's exp_spec on a grid that covers the
+    whole footprint range [-6, 0] densely, every integer and half-integer multiple of ln 2 neighbourhood, and the clamp range."""
+    import torch
+    from paper_2602_08266_b200 import api
+    rng = np.random.default_rng(3)
+    ln2 = np.log(2.0)
+    x = np.concatenate([np.linspace(-6.0, 0.0, 40001), rng.uniform(-80.0, 80.0, 20000), rng.uniform(-6.0, 0.0, 20000),
+                        (np.arange(-115, 116)[:, None] * ln2 + np.linspace(-1e-4, 1e-4, 21)[None, :]).ravel(),
+                        ((np.arange(-115, 116)[:, None] + 0.5) * ln2 + np.linspace(-1e-4, 1e-4, 21)[None, :]).ravel(),
+                        [0.0, -0.0, -80.0, 80.0, -5.5412635, 1e-30, -1e-30]]).astype(np.float32)
+    x = x[(x >= -80.0) & (x <= 80.0)]
+    y = api.exp_spec_pairs(torch.as_tensor(x, device="cuda")).cpu().numpy()
+    ref = orc.exp_spec(x)
+    assert np.array_equal(y.view(np.uint32), ref.view(np.uint32)), int((y.view(np.uint32) != ref.view(np.uint32)).sum())
+    # a parked pixel: -inf and NaN arguments give NaN, which fails every `>= alpha_min` test
+    bad = api.exp_spec_pairs(torch.tensor([-np.inf, np.nan, 0.0], device="cuda")).cpu().numpy()
+    assert np.isnan(bad[0]) and np.isnan(bad[1]) and bad[2] == 1.0
