@@ -271,7 +271,10 @@ TileGrid make_grid(int W, int H) {
   TileGrid tg;
   tg.tiles_x = (W + TILE - 1) / TILE;
   tg.tiles_y = (H + TILE - 1) / TILE;
-  tg.sshift = 3;
+  // supertiles of 8 x 8 tiles; 4 x 4 for images of fewer than 2,000 tiles: a tile then scans a list a third as long (S3 -18% at
+  // config 1) and the multi-split, which writes 2.4x the entries, is still small.  At 1280 x 720 the trade goes the other way
+  // (S3 -13%, multi-split 0.11 -> 0.40 ms per 8-view batch, 1943 -> 1838 views/s at config 2).
+  tg.sshift = tg.tiles_x * tg.tiles_y < 2000 ? 2 : 3;
   for (;;) {
     const int S = 1 << tg.sshift;
     tg.super_x = (tg.tiles_x + S - 1) / S;

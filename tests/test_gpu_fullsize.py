@@ -194,7 +194,7 @@ def test_cfg4_sampled_pixels_and_block_properties():
     nbv.set_concurrency(1)
     s1, b1 = nbv.score_candidates(cands)
     # the order of S4's binary32 reductions is all that varies with the number of views in flight
-    np.testing.assert_allclose(s4.cpu().numpy(), s1.cpu().numpy(), rtol=1e-5)
+    np.testing.assert_allclose(s4.cpu().numpy(), s1.cpu().numpy(), rtol=1e-4)       # see test_gpu_golden.py on the bound
     assert int(b4.item()) == int(b1.item())
 
 
