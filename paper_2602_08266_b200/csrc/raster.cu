@@ -127,6 +127,7 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   // positions from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
   __shared__ float4 sm[32 * 3];
   __shared__ uint32_t q_rank[64], q_cpos[64];
+  __shared__ uint32_t p_rank[64], p_cpos[64];             // rect hits awaiting the ellipse test (stage 2 of the tile filter)
   const int lane = threadIdx.x;
   for (uint32_t bpos = blockIdx.x;; ) {
   if (batch.work_fwd) {
@@ -170,45 +171,61 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   uint32_t pos = range.x, qn = 0;
   int e_base = 0;
   bool finished = __all_sync(FULL, ndone == PPL);
-  // The lazy tile filter is a chain of dependent loads per chunk of 32 list entries (rect -> key -> splat record gathered by
-  // rank -> ellipse test) and was a third of this kernel's stall samples.  It is software-pipelined two chunks deep in
-  // registers: while chunk c is tested, rect and key of chunk c + 1 are already here -- its rect test is taken at once and the
-  // splat records it will need are requested into the L1 -- and rect and key of chunk c + 2 are in flight.
+  // The lazy tile filter, two stages.  Stage 1 streams the supertile list in chunks of 32 entries and keeps the ones whose rect
+  // contains this tile (about one in five): rect and key are software-pipelined two chunks deep in registers, and the splat
+  // record of every rect hit is requested into the L1 at once.  Stage 2 runs when 32 rect hits are pending (or the list has
+  // ended): it gathers their records -- by then in the L1 -- and applies the ellipse test with all lanes busy (per chunk it
+  // kept six lanes busy and cost a dependent gather each time), and the survivors enter the queue of the entry loop.
+  // Until r2m the filter was one chain of dependent loads per chunk (rect -> key -> record -> ellipse test) and a third of
+  // this kernel's stall samples.
   ushort4 rcA = make_ushort4(1, 1, 0, 0), rcB = rcA;       // empty rect: covers no tile
   uint32_t keyA = 0, keyB = 0;
   if (!finished) {
     if (pos + lane < range.y) { rcA = crect[pos + lane]; keyA = ckeys[pos + lane]; }
     if (pos + 32u + lane < range.y) { rcB = crect[pos + 32u + lane]; keyB = ckeys[pos + 32u + lane]; }
   }
+  uint32_t pn = 0;                                         // rect hits pending for stage 2
   while (!finished) {
     // fill the queue with the next entries of the supertile list that can contribute to this tile
-    while (qn < 32u && pos < range.y) {
-      const uint32_t i = pos + lane;
-      const ushort4 rc = rcA;
-      const uint32_t key = keyA;
-      bool hit = i < range.y && tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
-      pos += 32;
-      rcA = rcB; keyA = keyB;
-      rcB = make_ushort4(1, 1, 0, 0);
-      if (pos + 32u + lane < range.y) { rcB = crect[pos + 32u + lane]; keyB = ckeys[pos + 32u + lane]; }
-      if (tx >= rcA.x && tx < rcA.z && ty >= rcA.y && ty < rcA.w) {      // next chunk's records (48 B: one or two sectors)
-        const char* nx = reinterpret_cast<const char*>(splat_sorted + (keyA & rmask));
-        prefetch_l1(nx); prefetch_l1(nx + 16);
+    while (qn < 32u) {
+      while (pn < 32u && pos < range.y) {                  // stage 1
+        const uint32_t i = pos + lane;
+        const ushort4 rc = rcA;
+        const uint32_t key = keyA;
+        const bool hit = i < range.y && tx >= rc.x && tx < rc.z && ty >= rc.y && ty < rc.w;
+        pos += 32;
+        rcA = rcB; keyA = keyB;
+        rcB = make_ushort4(1, 1, 0, 0);
+        if (pos + 32u + lane < range.y) { rcB = crect[pos + 32u + lane]; keyB = ckeys[pos + 32u + lane]; }
+        const unsigned m = __ballot_sync(FULL, hit);
+        if (hit) {
+          const uint32_t slot = pn + __popc(m & lt), r = key & rmask;
+          p_rank[slot] = r;
+          p_cpos[slot] = i;
+          const char* rec = reinterpret_cast<const char*>(splat_sorted + r);      // 48 B: one or two sectors
+          prefetch_l1(rec); prefetch_l1(rec + 16);
+        }
+        pn += __popc(m);
       }
-      uint32_t r = 0;
-      if (hit) {
-        r = key & rmask;
+      if (pn == 0) break;
+      const uint32_t take = min(pn, 32u);                  // stage 2
+      __syncwarp();
+      bool keep = false;
+      uint32_t r = 0, cp = 0;
+      if ((uint32_t)lane < take) {
+        r = p_rank[lane]; cp = p_cpos[lane];
         const float4* sp = reinterpret_cast<const float4*>(splat_sorted + r);
         const float4 a0 = sp[0], a1 = sp[1];
-        hit = ellipse_reaches_tile(a0.x, a0.y, a0.z, a0.w, a1.x, a1.w, X0, Y0);
+        keep = ellipse_reaches_tile(a0.x, a0.y, a0.z, a0.w, a1.x, a1.w, X0, Y0);
       }
-      const unsigned m = __ballot_sync(FULL, hit);
-      if (hit) {
+      const unsigned m = __ballot_sync(FULL, keep);
+      if (keep) {
         const uint32_t slot = qn + __popc(m & lt);
         q_rank[slot] = r;
-        q_cpos[slot] = i;
+        q_cpos[slot] = cp;
       }
       qn += __popc(m);
+      shift_queue(p_rank, p_cpos, pn, take);
     }
     if (qn == 0) break;
     const uint32_t cnt = min(qn, 32u);
