@@ -466,7 +466,7 @@ def main():
     out = {
         "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": agg["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "dtype_note": "S1-S4 binary32 (S4's 40 moments per Gaussian), S5-S6 binary64 (1-2% of a view)",
+        "dtype": "f32", "dtype_note": "S1-S4 binary32 (S4's 40 moments per (tile, Gaussian)), their sum across tiles and S5-S6 binary64 (1-2% of a view)",
         "data": "synthetic", "config": workload_config(args, wl, "device"),
         "clocks": clocks,
         "e2e": {"value": agg_e2e["value"], "unit": UNIT, "h2d_bytes_per_step": int(72 * C), "d2h_bytes_per_step": int(4 * C + 4),

@@ -5,7 +5,7 @@
 //     PAPER.md L189-191 (H ~= J^T J), L210 (per-Gaussian blocks), L248.
 // S6: IG_g = log det(c_g (H_T,g + H_c,g) + Lambda) - log det(c_g H_T,g + Lambda)   (Eq. 5, 6, 9; R-13, R-14)
 //     as the difference of the pivots of two L D L^T factorisations, sum_j log(d1_j / d0_j).
-// PRECISION: everything after the 40 binary32 moments is binary64 -- the chain rule, A Q A^T, H_T itself, the two
+// PRECISION: everything after S4's binary32 per-tile moment sums is binary64 -- their sum across tiles, the chain rule, A Q A^T, H_T itself, the two
 //     factorisations.  A block has exact null directions (R-10; single-view blocks have rank ~8 of 14) next to entries of
 //     1e5-1e7: in binary32 the product A Q A^T and the storage of H_T alone leave rounding noise of eps H_kk ~ 0.1-1 on
 //     pivots whose exact value is the prior, which is what limited round 1 to Lambda = 1 and 5e-3 on single gains.  In
@@ -13,7 +13,8 @@
 //     ~2.5 kflop (binary64) per touched Gaussian, 1-2% of a view.
 // DETERMINISM: the touched list is built in rank order (touched_count / touched_write), a thread's partial gain and a block's
 //     partial score depend only on (view, block), and the last block of a view adds the partials in block order; H_T is
-//     accumulated view by view without atomics.  What is left run-to-run is the order of the binary32 `red.add` of S4.
+//     accumulated view by view without atomics.  What is left run-to-run is the order of S4's
+//     `red.global.add.f64` across tiles, whose addends (widened binary32) sum exactly in binary64 for any realistic footprint.
 #include <algorithm>
 #include <cstdlib>
 
@@ -144,12 +145,12 @@ __device__ __forceinline__ void tpg_build_block(const SceneDev& sc, const nbv_co
   double u[NMOM];
   {
     double m[NMOM];
-    float4* mom4 = reinterpret_cast<float4*>(vw.moments + (size_t)r * NMOM);
+    double2* mom2 = reinterpret_cast<double2*>(vw.moments + (size_t)r * NMOM);
 #pragma unroll
-    for (int q = 0; q < NMOM / 4; ++q) {
-      const float4 v = mom4[q];
-      mom4[q] = make_float4(0.f, 0.f, 0.f, 0.f);             // leave the buffer zeroed for the next view
-      m[4 * q] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w;
+    for (int q = 0; q < NMOM / 2; ++q) {
+      const double2 v = mom2[q];
+      mom2[q] = make_double2(0.0, 0.0);                       // leave the buffer zeroed for the next view
+      m[2 * q] = v.x; m[2 * q + 1] = v.y;
     }
     // the whitening S4 used, from the splat's conic (-2 qa, -qb, -2 qc) = Sigma2D^-1
     const float4 s0 = *reinterpret_cast<const float4*>(vw.splat_sorted + r);

@@ -97,7 +97,7 @@ struct RasterView {
   uint32_t* tile_walk;       // per tile: list entries S3 consumed
   uint32_t* tlist;           // per tile TL_CAP ranks: the tile's list as S3 walked it (entry e at tlist[tile * TL_CAP + e]); S4 reads it
                              // backwards instead of filtering the supertile list again (tiles that walked more fall back to the filter)
-  float* moments;            // rank r at moments + r * mom_stride (NMOM floats), zero on entry to S4 for every Gaussian
+  double* moments;           // rank r at moments + r * mom_stride (NMOM doubles: the tiles' binary32 sums are added up in binary64), zero on entry to S4 for every Gaussian
   int mom_stride;            // NMOM, or groups * NMOM in a mask context (one group of 4 object channels per S4 launch)
   uint8_t* touched_flag;     // N bytes, zero on entry to S4: S4 sets flag[rank] for every rank it adds moments to (= sum w^2 != 0),
                              // the ordered compaction reads and clears it (32x less traffic than testing moment 39 of every rank)
@@ -121,7 +121,7 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
                      cudaStream_t st);
 
-// ---- hessian.cu (colour / depth contexts: everything after the binary32 moments is binary64)
+// ---- hessian.cu (colour / depth contexts: everything after S4's binary32 per-tile moment sums is binary64)
 // the touched lists (ranks with sum w^2 != 0, in rank order) of every view of the batch
 void launch_touched(const RasterBatch& batch, int N, cudaStream_t st);
 uint32_t touched_blocks(int N);
@@ -134,7 +134,7 @@ struct ExpandView {
   const uint32_t* ids_sorted;
   const Splat* splat_sorted;
   const uint32_t* touched;
-  float* moments;
+  double* moments;
   float* out_blocks;         // EXPAND_VIEW
   float* score;              // EXPAND_GAIN: written (not accumulated) by the last block of the view
   float* gains;              // EXPAND_GAIN, may be null

@@ -97,8 +97,8 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
     const uint32_t g = vw.ids_sorted[r];
     __syncwarp();
     // moments of all groups -> shared memory (and zero the buffer for the next view)
-    float* gm = vw.moments + (size_t)r * stride;
-    for (int i = lane; i < stride; i += 32) { mom[i] = (double)gm[i]; gm[i] = 0.f; }
+    double* gm = vw.moments + (size_t)r * stride;
+    for (int i = lane; i < stride; i += 32) { mom[i] = gm[i]; gm[i] = 0.0; }
     __syncwarp();
     {   // whitened basis -> u basis, one lane per group
       const Splat sp = vw.splat_sorted[r];

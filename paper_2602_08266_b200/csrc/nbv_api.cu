@@ -304,7 +304,7 @@ int pre_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, 
   const uint32_t ccap = (uint32_t)worst;     // worst case: no overflow is possible, no count has to come back to the host
   const size_t n_counts = (size_t)n_super * msplit_blocks(N);
   const size_t npx = (size_t)cams[0].width * cams[0].height;
-  const size_t mom_bytes = 4 * (size_t)NMOM * ctx->mask_groups * N;
+  const size_t mom_bytes = 8 * (size_t)NMOM * ctx->mask_groups * N;
   PreBatch pb;
   pb.n = n;
   for (int i = 0; i < n; ++i) {
@@ -451,8 +451,8 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     v.pix.T = s->pix_T.as<float>(); v.pix.last = s->pix_last.as<int32_t>();
     v.tile_cend = s->tile_cend.as<uint32_t>(); v.tile_elast = s->tile_elast.as<uint32_t>(); v.tile_walk = s->tile_walk.as<uint32_t>();
     v.tlist = s->tlist.as<uint32_t>();
-    v.moments = s->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = s->touched.as<uint32_t>();
-    v.touched_flag = reinterpret_cast<uint8_t*>(s->moments.p) + sizeof(float) * NMOM * (size_t)ctx->mask_groups * (size_t)ctx->N;
+    v.moments = s->moments.as<double>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = s->touched.as<uint32_t>();
+    v.touched_flag = reinterpret_cast<uint8_t*>(s->moments.p) + sizeof(double) * NMOM * (size_t)ctx->mask_groups * (size_t)ctx->N;
     v.touched_cnt = s->touched_cnt.as<uint32_t>(); v.counters = s->d_counters;
   }
   const TileGrid tg = sl[0]->tg;
@@ -475,7 +475,7 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
         launch_mask_splats(sc, sl[i]->splat_sorted.as<Splat>(), sl[i]->ids.as<uint32_t>(), gr, ctx->cfg.mask_bg_channel,
                            sl[i]->gsplat.as<Splat>(), st);
         gb.v[i].splat_sorted = sl[i]->gsplat.as<Splat>();
-        gb.v[i].moments = sl[i]->moments.as<float>() + (size_t)gr * NMOM;
+        gb.v[i].moments = sl[i]->moments.as<double>() + (size_t)gr * NMOM;
       }
       if (gr > 0 && gb.work) CK(cudaMemsetAsync(gb.work, 0, 8, st));     // fresh work counters (main + fallback) for every launch
       launch_backward(gb, ctx->N, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, gcfg, st);
@@ -497,7 +497,7 @@ int expand_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     ExpandView& v = eb.v[i];
     v.cam = cams[i];
     v.ids_sorted = s->ids.as<uint32_t>(); v.splat_sorted = s->splat_sorted.as<Splat>(); v.touched = s->touched.as<uint32_t>();
-    v.moments = s->moments.as<float>(); v.out_blocks = out_blocks; v.score = d_scores ? d_scores + i : nullptr; v.gains = gains;
+    v.moments = s->moments.as<double>(); v.out_blocks = out_blocks; v.score = d_scores ? d_scores + i : nullptr; v.gains = gains;
     v.counters = s->d_counters; v.partials = s->partials.as<double>();
     v.cache_span = cache ? cache->spans + 2 * (size_t)(first_candidate + i) : nullptr;
   }
@@ -1084,7 +1084,7 @@ int nbv_render_mask(nbv_ctx* ctx, const nbv_camera* h_cam, float* d_mask, void* 
     v.pix.T = sl->pix_T.as<float>(); v.pix.last = sl->pix_last.as<int32_t>();
     v.tile_cend = sl->tile_cend.as<uint32_t>(); v.tile_elast = sl->tile_elast.as<uint32_t>(); v.tile_walk = sl->tile_walk.as<uint32_t>();
     v.tlist = nullptr;                                   // forward pass only
-    v.moments = sl->moments.as<float>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = sl->touched.as<uint32_t>();
+    v.moments = sl->moments.as<double>(); v.mom_stride = NMOM * ctx->mask_groups; v.touched = sl->touched.as<uint32_t>();
     v.touched_flag = nullptr;                            // forward pass only
     v.touched_cnt = sl->touched_cnt.as<uint32_t>(); v.counters = sl->d_counters;
     launch_forward(rb, sl->tg, sl->rank_bits, h_cam->width, h_cam->height, gcfg, true, st);

@@ -324,18 +324,11 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
 
 constexpr int RED_STRIDE = 44;      // row stride (words) of the 32 x 40 reduction buffer: float4 rows, bank-conflict free
 
-// 16-byte vector reductions into the L2 (sm_90+): one request per four moments
-__device__ __forceinline__ void red_add_v4(float* dst, const float4& v) {
-  asm volatile("red.global.v4.f32.add [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
-}
-__device__ __forceinline__ float4 atom_add_v4(float* dst, const float4& v) {
-  float4 o;
-  asm volatile("atom.global.v4.f32.add {%0, %1, %2, %3}, [%4], {%5, %6, %7, %8};"
-               : "=f"(o.x), "=f"(o.y), "=f"(o.z), "=f"(o.w)
-               : "l"(dst), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w)
-               : "memory");
-  return o;
-}
+// Cross-tile sum of a Gaussian's moments, in the L2, without a return value.  Binary64: the addends are binary32 tile sums
+// widened, so the sum over a few hundred tiles is exact (and the same in any order) unless their exponents span more than
+// 2^29; a binary32 sum here (red.global.v4.f32.add, a quarter of the requests) left per-Gaussian gains of Gaussians a few
+// pixels from the camera 2e-3 off the oracle and moving from call to call (Determinism).
+__device__ __forceinline__ void red_add_f64(double* dst, double v) { asm volatile("red.global.add.f64 [%0], %1;" ::"l"(dst), "d"(v) : "memory"); }
 
 // ---- S4 group tail.  After its slot body a lane holds, per entry, 18 column sums over its 8 pixels: F_p = sum_k f_k t_k^p
 // (p <= 4), sum w^2, and G_c,p = sum_k g_c,k t_k^p (p <= 2) per channel.  Turning them into the lane's 40 moments (binomial
@@ -351,7 +344,7 @@ constexpr int GE = 4;
 template <int NCH>
 __device__ __forceinline__ void group_tail(const float4* rawA, const float2* rawB, float* red, const float4* sm, const float4* sm_wh,
                                            const float4* sm_ex, const uint32_t* q_rank, int gcount, uint32_t gpack, int tx, int ty,
-                                           float* __restrict__ moments, int mom_stride, uint8_t* __restrict__ flag, int lane) {
+                                           double* __restrict__ moments, int mom_stride, uint8_t* __restrict__ flag, int lane) {
   __syncwarp();                                            // the parked column sums are visible
   const int ge = lane >> 3, part = lane & 7;
   float acc[NMOM];
@@ -422,7 +415,10 @@ __device__ __forceinline__ void group_tail(const float4* rawA, const float2* raw
         a01 = add2(a01, make_float2(x.x, x.y)); a23 = add2(a23, make_float2(x.z, x.w));
       }
       const uint32_t rank = q_rank[(gpack >> (8 * e1)) & 0xffu];
-      red_add_v4(moments + (size_t)rank * mom_stride + 4 * q, make_float4(a01.x, a01.y, a23.x, a23.y));
+      // across the tiles a Gaussian covers the sums are taken in binary64: in binary32 their order-dependent rounding (a few 1e-7
+      // of the total) was amplified to 2e-3 on the gains of Gaussians filling hundreds of tiles (near-singular moment matrices)
+      double* dst = moments + (size_t)rank * mom_stride + 4 * q;
+      red_add_f64(dst, (double)a01.x); red_add_f64(dst + 1, (double)a01.y); red_add_f64(dst + 2, (double)a23.x); red_add_f64(dst + 3, (double)a23.y);
       if (q == 0) flag[rank] = 1;                          // touched: the compaction of launch_touched reads these bytes
     }
   }
@@ -465,7 +461,7 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   const ushort4* __restrict__ crect = vw.crect;
   const uint2* __restrict__ cranges = vw.cranges;
   const PixelBuf pix = vw.pix;
-  float* __restrict__ moments = vw.moments;
+  double* __restrict__ moments = vw.moments;
   const int tile = batch.tile_order[bpos / (uint32_t)batch.n];   // heaviest tiles first (launch order)
   const uint32_t elast = vw.tile_elast[tile];             // list position + 1 of the last entry any pixel of the tile passed
   // which instantiation owns the tile: the list holds the first TL_CAP entries only

@@ -139,15 +139,15 @@ __global__ void __launch_bounds__(SH_WARPS * 32) expand_sh_kernel(const __grid_c
     // every lane reads the 40 moments (broadcast loads); lane 0 zeroes them for the next view afterwards
     double m[NMOM];
     {
-      const float4* mom4 = reinterpret_cast<const float4*>(vw.moments + (size_t)r * NMOM);
+      const double2* mom2 = reinterpret_cast<const double2*>(vw.moments + (size_t)r * NMOM);
 #pragma unroll
-      for (int i = 0; i < NMOM / 4; ++i) {
-        const float4 v = mom4[i];
-        m[4 * i] = v.x; m[4 * i + 1] = v.y; m[4 * i + 2] = v.z; m[4 * i + 3] = v.w;
+      for (int i = 0; i < NMOM / 2; ++i) {
+        const double2 v = mom2[i];
+        m[2 * i] = v.x; m[2 * i + 1] = v.y;
       }
     }
     __syncwarp();
-    if (lane < NMOM / 4) reinterpret_cast<float4*>(vw.moments + (size_t)r * NMOM)[lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (lane < NMOM / 2) reinterpret_cast<double2*>(vw.moments + (size_t)r * NMOM)[lane] = make_double2(0.0, 0.0);
     whitened_to_u<double>(m, vw.splat_sorted[r]);
     Chain<double> ch;
     projection_chain<double>(vw.cam, sc.mean + 3 * (size_t)g, sc.logscale + 3 * (size_t)g, sc.quat + 4 * (size_t)g, ch);

@@ -193,8 +193,8 @@ def test_cfg4_sampled_pixels_and_block_properties():
     s4, b4 = nbv.score_candidates(cands)
     nbv.set_concurrency(1)
     s1, b1 = nbv.score_candidates(cands)
-    # the order of S4's binary32 reductions is all that varies with the number of views in flight
-    np.testing.assert_allclose(s4.cpu().numpy(), s1.cpu().numpy(), rtol=1e-4)       # see test_gpu_golden.py on the bound
+    # the order of S4's cross-tile red.global.add.f64 is all that varies with the number of views in flight
+    np.testing.assert_allclose(s4.cpu().numpy(), s1.cpu().numpy(), rtol=1e-9)       # see test_gpu_golden.py on the bound
     assert int(b4.item()) == int(b1.item())
 
 

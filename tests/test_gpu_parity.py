@@ -163,8 +163,9 @@ def test_reset_training_and_repeatability(wl):
     assert float(nbv.training_hessian().abs().sum()) == 0.0
     nbv.accumulate_training(wl.train_cams)
     s2, b2 = nbv.score_candidates(wl.cand_cams)
-    # H_T is added up view by view and a score block by block in a fixed order; only the binary32 reductions of S4 vary
-    np.testing.assert_allclose(s2.cpu().numpy(), s1, rtol=2e-6)
+    # H_T is added up view by view and a score block by block in a fixed order; only the order of S4's cross-tile
+    # red.global.add.f64 varies, and a binary64 sum of widened binary32 tile sums is exact for these data
+    np.testing.assert_allclose(s2.cpu().numpy(), s1, rtol=1e-9)
     assert int(b1.item()) == int(b2.item())
 
 
