@@ -49,7 +49,7 @@ BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written on
 VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (16 for images of fewer than 2,000 tiles)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture named
 # in TRAFFIC_SOURCE; known for config 2 only (null elsewhere)
-NCU_TRAFFIC_BYTES = {2: {"backward": 105.4e6, "forward": 54.5e6}}
+NCU_TRAFFIC_BYTES = {2: {"backward": 113.8e6, "forward": 55.2e6}}
 TRAFFIC_SOURCE = "profiles/r2_ncu_raster_cfg2.md (ncu --set full of the first candidate batch; a stored figure, not measured by this run)"
 
 
