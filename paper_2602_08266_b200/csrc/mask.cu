@@ -91,6 +91,11 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
   double *xs = base + lay.oX, *ps = base + lay.oP, *mono = base + lay.oMono, *piv = base + lay.oPiv;
   const uint32_t n_touched = vw.counters->n_touched;
   const int stride = NMOM * groups;
+  // entry e of the row-major lower triangle -> (row << 8) | column, behind the warps' areas
+  uint16_t* tri = reinterpret_cast<uint16_t*>(smem + (size_t)wpb * lay.per_warp);
+  for (int i = threadIdx.x; i < L - 1; i += blockDim.x)
+    for (int k = 0; k <= i; ++k) tri[i * (i + 1) / 2 + k] = (uint16_t)((i << 8) | k);
+  __syncthreads();
   double gain = 0.0;
   for (uint32_t t = blockIdx.x * wpb + wib; t < n_touched; t += gridDim.x * wpb) {
     const uint32_t r = vw.touched[t];
@@ -227,17 +232,23 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       // two interleaved right-looking L D L^T (lower triangles, lane i owns rows i and i + 32); the gain is the sum of
       // log(d1_j / d0_j) over the pivots, as in the colour / depth contexts (hessian.cu): 2 x L^3 / 6 multiply-adds instead of
       // the two L^3 / 2 triangular solves + a Cholesky of the solve form used while this path was binary32
+      // The trailing triangle of step j (m = L - j - 1 rows, m (m + 1) / 2 entries) is dealt to the lanes entry by entry
+      // through `tri` (entry e of the row-major lower triangle -> (row, column); the triangle of m rows is a prefix of the
+      // larger ones, so one table serves every step): a lane per ROW left the lanes with 1 ... m entries each and the warp
+      // waiting for the longest row, 3 x the serial length.
       for (int j = 0; j < L; ++j) {
         const double d0 = fmax(Um[j * LS + j], 1e-300), d1 = fmax(Hm[j * LS + j], 1e-300);
         if (lane == 0) { piv[j] = d0; piv[L + j] = d1; }
-        const double i0 = 1.0 / d0, i1 = 1.0 / d1;
-        for (int i = j + 1 + lane; i < L; i += 32) {
-          const double l0 = Um[i * LS + j] * i0, l1 = Hm[i * LS + j] * i1;
-#pragma unroll 4
-          for (int k = j + 1; k <= i; ++k) {
-            Um[i * LS + k] = fma(-l0, Um[k * LS + j], Um[i * LS + k]);
-            Hm[i * LS + k] = fma(-l1, Hm[k * LS + j], Hm[i * LS + k]);
-          }
+        const double i0 = -1.0 / d0, i1 = -1.0 / d1;
+        const int m = L - j - 1, n = m * (m + 1) / 2;
+        const double *u0 = Um + (j + 1) * LS + j, *h0 = Hm + (j + 1) * LS + j;        // column j below the pivot
+        double *ut = Um + (j + 1) * (LS + 1), *ht2 = Hm + (j + 1) * (LS + 1);           // the trailing block
+#pragma unroll 2
+        for (int e = lane; e < n; e += 32) {
+          const int ik = tri[e], i = ik >> 8, k = ik & 255;
+          const double l0 = u0[i * LS] * i0, l1 = h0[i * LS] * i1;
+          ut[i * LS + k] = fma(l0, u0[k * LS], ut[i * LS + k]);
+          ht2[i * LS + k] = fma(l1, h0[k * LS], ht2[i * LS + k]);
         }
         __syncwarp();
       }
@@ -267,7 +278,8 @@ void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandB
   const MaskWarpLayout lay = mask_warp_layout(sc.K, groups);
   int wpb = 8;
   while (wpb > 1 && (size_t)wpb * lay.per_warp * 8 > 200 * 1024) wpb >>= 1;
-  const size_t smem = (size_t)wpb * lay.per_warp * 8;
+  const int L = 11 + sc.K;
+  const size_t smem = (size_t)wpb * lay.per_warp * 8 + (((size_t)L * (L - 1) / 2 * 2 + 15) & ~(size_t)15);
   // the attribute is per device and per function: set it whenever the launch needs more than the default 48 KB
   if (smem > 48 * 1024 &&
       cudaFuncSetAttribute(expand_mask_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)

@@ -96,17 +96,25 @@ constexpr int SH_WARPS = 3;
 
 // in-place right-looking L D L^T of the symmetric matrix in M (full storage, upper triangle used), pivots -> piv (or the
 // log of pivot ratios accumulated when ref != nullptr).  All 32 lanes cooperate; returns sum_j log(d_j / ref_j) or 0.
-__device__ double warp_ldl(double* M, double* piv, const double* ref, int lane) {
+// `tri`: entry e of a row-major lower triangle -> (a << 8) | b, b <= a (filled once per block); the trailing triangle of
+// step j is a prefix of it, and its entries are dealt to the lanes one by one (a lane per row leaves the warp waiting for
+// the longest row: 3 x the serial length).
+constexpr int SH_TRI = SH_L * (SH_L - 1) / 2;
+__device__ double warp_ldl(double* M, double* piv, const double* ref, const uint16_t* tri, int lane) {
   double ld = 0.0;
   for (int j = 0; j < SH_L; ++j) {
     __syncwarp();
     const double d = fmax(M[j * SH_LS + j], 1e-300);
     if (ref) ld += log(d / ref[j]); else if (lane == 0) piv[j] = d;
-    const double inv = 1.0 / d;
-    // trailing update: row i (i > j) -= (M[j][i] / d) * row j, columns >= i; rows dealt to lanes round-robin
-    for (int i = j + 1 + lane; i < SH_L; i += 32) {
-      const double l = M[j * SH_LS + i] * inv;
-      for (int k = i; k < SH_L; ++k) M[i * SH_LS + k] = fma(-l, M[j * SH_LS + k], M[i * SH_LS + k]);
+    const double inv = -1.0 / d;
+    // trailing update: M[i][k] -= (M[j][i] / d) M[j][k] for j < i <= k
+    const int m = SH_L - j - 1, n = m * (m + 1) / 2;
+    const double* rowj = M + j * SH_LS + j + 1;
+    double* tr = M + (j + 1) * (SH_LS + 1);
+#pragma unroll 2
+    for (int e = lane; e < n; e += 32) {
+      const int ab = tri[e], k = ab >> 8, i = ab & 255;
+      tr[i * SH_LS + k] = fma(rowj[i] * inv, rowj[k], tr[i * SH_LS + k]);
     }
   }
   __syncwarp();
@@ -119,6 +127,10 @@ __global__ void __launch_bounds__(SH_WARPS * 32) expand_sh_kernel(const __grid_c
                                                                     double* __restrict__ H_T, const float* __restrict__ conf) {
   extern __shared__ __align__(16) double shm[];
   __shared__ double ws[SH_WARPS];
+  __shared__ uint16_t tri[SH_TRI];
+  for (int i = threadIdx.x; i < SH_L - 1; i += blockDim.x)
+    for (int k = 0; k <= i; ++k) tri[i * (i + 1) / 2 + k] = (uint16_t)((i << 8) | k);
+  __syncthreads();
   const ExpandView& vw = batch.v[view0 + blockIdx.y];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   double* Hc = shm + (size_t)wib * SH_WARP_DOUBLES;
@@ -246,11 +258,11 @@ __global__ void __launch_bounds__(SH_WARPS * 32) expand_sh_kernel(const __grid_c
       const double* ht = H_T + (size_t)g * SH_LB;
       for (int rr = 0; rr < SH_L; ++rr)
         for (int cc = rr + lane; cc < SH_L; cc += 32) Ha[rr * SH_LS + cc] = c * ht[triS(rr, cc)] + (rr == cc ? (double)prior59[rr] : 0.0);
-      warp_ldl(Ha, piv0, nullptr, lane);
+      warp_ldl(Ha, piv0, nullptr, tri, lane);
       for (int rr = 0; rr < SH_L; ++rr)
         for (int cc = rr + lane; cc < SH_L; cc += 32)
           Ha[rr * SH_LS + cc] = c * (ht[triS(rr, cc)] + Hc[rr * SH_LS + cc]) + (rr == cc ? (double)prior59[rr] : 0.0);
-      gn = warp_ldl(Ha, nullptr, piv0, lane);
+      gn = warp_ldl(Ha, nullptr, piv0, tri, lane);
     }
     if (lane == 0) {
       if (vw.gains) vw.gains[g] = (float)gn;
