@@ -26,6 +26,7 @@ namespace nbv {
 __host__ __device__ __forceinline__ int mask_channel_of_slot(int t, int bgch) { return t == 0 ? bgch : (t <= bgch ? t - 1 : t); }
 __host__ __device__ __forceinline__ int mask_slot_of_channel(int c, int bgch) { return c == bgch ? 0 : (c < bgch ? c + 1 : c); }
 __device__ __forceinline__ int triL(int r, int c, int L) { return r * L - r * (r - 1) / 2 + (c - r); }
+__device__ __forceinline__ int rtri(int r) { return r * (r + 1) / 2; }      // start of row r of a row-major lower triangle
 
 __global__ void __launch_bounds__(256) mask_splat_kernel(const Splat* __restrict__ splat_sorted, const uint32_t* __restrict__ ids_sorted,
                                                          const float* __restrict__ logits, const float* __restrict__ lse, int N, int K,
@@ -50,23 +51,24 @@ void launch_mask_splats(const SceneDev& sc, const Splat* splat_sorted, const uin
   mask_splat_kernel<<<(sc.N + 255) / 256, 256, 0, st>>>(splat_sorted, ids_sorted, sc.logits, sc.lse, sc.N, sc.K, group, bgch, out);
 }
 
-// ---- S5' + S6 of a mask context, warp-cooperative: ONE WARP PER TOUCHED GAUSSIAN, two L x L matrices in shared memory
-// (a first version ran one thread per Gaussian over 2 x 2016 floats of local memory).  Lane l owns the columns (building the
-// block) or rows (elimination) l, l + 32.  S6 is the pivot-ratio form of the colour / depth contexts: M0 = c H_T + Lambda and
-// M1 = c (H_T + H) + Lambda are eliminated side by side (right-looking L D L^T, one column per step, the trailing rows updated
-// in parallel) and the gain is sum_j log(d1_j / d0_j).  No factor table, nothing cached between scoring calls.
+// ---- S5' + S6 of a mask context, warp-cooperative: ONE WARP PER TOUCHED GAUSSIAN, two packed symmetric L x L matrices in
+// shared memory (a first version ran one thread per Gaussian over 2 x 2016 floats of local memory).  Lane l builds the columns
+// l, l + 32 of the block.  S6 is the pivot-ratio form of the colour / depth contexts: M0 = c H_T + Lambda and
+// M1 = c (H_T + H) + Lambda are eliminated side by side (right-looking L D L^T, one column per step, the entries of the
+// trailing block dealt to the lanes one by one) and the gain is sum_j log(d1_j / d0_j).  No factor table, nothing cached
+// between scoring calls.  K = 20: 12.3 KB per warp, two blocks of 8 warps per SM.
 struct MaskWarpLayout {
-  int LS;          // row stride of H and U (odd: conflict-free column and row walks)
+  int LB;          // packed size of a symmetric L x L matrix
   int per_warp;    // doubles per warp
   int oH, oU, oA, oAQ, oMom, oX, oP, oMono, oPiv;
 };
 __host__ __device__ inline MaskWarpLayout mask_warp_layout(int K, int groups) {
   MaskWarpLayout m;
   const int L = 11 + K;
-  m.LS = L | 1;
+  m.LB = L * (L + 1) / 2;
   int o = 0;
-  m.oH = o; o += m.LS * L;
-  m.oU = o; o += m.LS * L;
+  m.oH = o; o += m.LB;
+  m.oU = o; o += m.LB;
   m.oA = o; o += 66;
   m.oAQ = o; o += 66;
   m.oMom = o; o += groups * NMOM;
@@ -85,7 +87,7 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
   const ExpandView& vw = batch.v[view0 + blockIdx.y];
   const int K = sc.K, L = 11 + K, LB = L * (L + 1) / 2, bgch = cfg.mask_bg_channel;
   const MaskWarpLayout lay = mask_warp_layout(K, groups);
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5, LS = lay.LS;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5, wpb = blockDim.x >> 5;
   double* base = smem + (size_t)wib * lay.per_warp;
   double *Hm = base + lay.oH, *Um = base + lay.oU, *As = base + lay.oA, *AQs = base + lay.oAQ, *mom = base + lay.oMom;
   double *xs = base + lay.oX, *ps = base + lay.oP, *mono = base + lay.oMono, *piv = base + lay.oPiv;
@@ -170,21 +172,17 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       for (int slot = 0; slot < K; ++slot) v += ps[slot] * xs[slot * 6 + e];
       xbar[e] = v;
     }
-    // the full symmetric block, column j by lane j (and j + 32)
+    // the upper triangle of the block, column j by lane j (and j + 32), in REVERSED packed storage: entry (i, j >= i) sits at
+    // r (r + 1) / 2 + c with r = L - 1 - i, c = L - 1 - j.  In that order the trailing block of elimination step j is the prefix
+    // [0, m (m + 1) / 2), m = L - 1 - j, of the array, the pivot row follows it directly, and an entry's address is its number.
     for (int j = lane; j < L; j += 32) {
+      const int cj = L - 1 - j;
       if (j < 11) {
-        for (int i = 0; i < 11; ++i) {
+        for (int i = 0; i <= j; ++i) {
           double v = 0.0;
 #pragma unroll
           for (int e = 0; e < 6; ++e) v += AQs[i * 6 + e] * As[j * 6 + e];
-          Hm[i * LS + j] = v;
-        }
-        for (int c = 0; c < K; ++c) {
-          const int slot = mask_slot_of_channel(c, bgch);
-          double v = 0.0;
-#pragma unroll
-          for (int e = 0; e < 6; ++e) v += As[j * 6 + e] * (ps[slot] * (xs[slot * 6 + e] - xbar[e]));
-          Hm[(11 + c) * LS + j] = v;
+          Hm[rtri(L - 1 - i) + cj] = v;
         }
       } else {
         const int c = j - 11, slot = mask_slot_of_channel(c, bgch);
@@ -193,13 +191,13 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
           double v = 0.0;
 #pragma unroll
           for (int e = 0; e < 6; ++e) v += As[i * 6 + e] * (pc * (xs[slot * 6 + e] - xbar[e]));
-          Hm[i * LS + j] = v;
+          Hm[rtri(L - 1 - i) + cj] = v;
         }
-        for (int d = 0; d < K; ++d) {
+        for (int d = 0; d <= c; ++d) {
           const double pd = ps[mask_slot_of_channel(d, bgch)];
           double v = pc * pd * (S2 - pc - pd);
           if (d == c) v += pc * pc;
-          Hm[(11 + d) * LS + j] = W2 * v;
+          Hm[rtri(L - 12 - d) + cj] = W2 * v;
         }
       }
     }
@@ -208,8 +206,9 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
       for (int rr = 0; rr < L; ++rr)
         for (int c = rr + lane; c < L; c += 32) {
           const size_t o = (size_t)g * LB + triL(rr, c, L);
-          if (mode == EXPAND_TRAIN) H_T[o] += Hm[rr * LS + c];                  // one launch per view, in view order
-          else vw.out_blocks[o] = (float)Hm[rr * LS + c];
+          const double v = Hm[rtri(L - 1 - rr) + L - 1 - c];
+          if (mode == EXPAND_TRAIN) H_T[o] += v;                  // one launch per view, in view order
+          else vw.out_blocks[o] = (float)v;
         }
       continue;
     }
@@ -218,37 +217,34 @@ __global__ void __launch_bounds__(256) expand_mask_warp_kernel(const __grid_cons
     const double cb = cfg.weight_mode == 1 ? 1.0 : cg;        // R2 weights the gain, R1 / R3 the candidate block
     double gn = 0.0;
     if (cg > 0.0) {
-      // M0 = ct H_T + Lambda -> Um,  M1 = M0 + cb H -> Hm  (lower triangles; H_T is stored packed upper, row-major)
+      // M0 = ct H_T + Lambda -> Um,  M1 = M0 + cb H -> Hm  (H_T is stored packed upper, row-major)
       const double* ht = H_T + (size_t)g * LB;
       for (int rr = 0; rr < L; ++rr) {
         const double pr = rr < 11 ? (double)cfg.prior_precision[rr] : (double)cfg.prior_precision_obj;
+        const int rb = rtri(L - 1 - rr) + L - 1;
         for (int c = rr + lane; c < L; c += 32) {
           const double m0 = fma(ct, ht[triL(rr, c, L)], c == rr ? pr : 0.0);
-          Um[c * LS + rr] = m0;
-          Hm[c * LS + rr] = fma(cb, Hm[c * LS + rr], m0);
+          Um[rb - c] = m0;
+          Hm[rb - c] = fma(cb, Hm[rb - c], m0);
         }
       }
       __syncwarp();
-      // two interleaved right-looking L D L^T (lower triangles, lane i owns rows i and i + 32); the gain is the sum of
-      // log(d1_j / d0_j) over the pivots, as in the colour / depth contexts (hessian.cu): 2 x L^3 / 6 multiply-adds instead of
-      // the two L^3 / 2 triangular solves + a Cholesky of the solve form used while this path was binary32
-      // The trailing triangle of step j (m = L - j - 1 rows, m (m + 1) / 2 entries) is dealt to the lanes entry by entry
-      // through `tri` (entry e of the row-major lower triangle -> (row, column); the triangle of m rows is a prefix of the
-      // larger ones, so one table serves every step): a lane per ROW left the lanes with 1 ... m entries each and the warp
-      // waiting for the longest row, 3 x the serial length.
+      // two interleaved right-looking L D L^T; the gain is the sum of log(d1_j / d0_j) over the pivots, as in the colour /
+      // depth contexts (hessian.cu): 2 x L^3 / 6 multiply-adds instead of the two L^3 / 2 triangular solves + a Cholesky of
+      // the solve form used while this path was binary32.  Step j: pivot row = entries [n, n + m] of the array (n = m (m + 1)
+      // / 2), trailing block = entries [0, n), dealt to the lanes entry by entry through `tri` (entry -> (row, column)): a lane
+      // per ROW left the lanes with 1 ... m entries each and the warp waiting for the longest row, 3 x the serial length.
       for (int j = 0; j < L; ++j) {
-        const double d0 = fmax(Um[j * LS + j], 1e-300), d1 = fmax(Hm[j * LS + j], 1e-300);
+        const int m = L - 1 - j, n = m * (m + 1) / 2;
+        const double *v0 = Um + n, *v1 = Hm + n;
+        const double d0 = fmax(v0[m], 1e-300), d1 = fmax(v1[m], 1e-300);
         if (lane == 0) { piv[j] = d0; piv[L + j] = d1; }
         const double i0 = -1.0 / d0, i1 = -1.0 / d1;
-        const int m = L - j - 1, n = m * (m + 1) / 2;
-        const double *u0 = Um + (j + 1) * LS + j, *h0 = Hm + (j + 1) * LS + j;        // column j below the pivot
-        double *ut = Um + (j + 1) * (LS + 1), *ht2 = Hm + (j + 1) * (LS + 1);           // the trailing block
 #pragma unroll 2
         for (int e = lane; e < n; e += 32) {
-          const int ik = tri[e], i = ik >> 8, k = ik & 255;
-          const double l0 = u0[i * LS] * i0, l1 = h0[i * LS] * i1;
-          ut[i * LS + k] = fma(l0, u0[k * LS], ut[i * LS + k]);
-          ht2[i * LS + k] = fma(l1, h0[k * LS], ht2[i * LS + k]);
+          const int rc = tri[e], r = rc >> 8, c = rc & 255;
+          Um[e] = fma(v0[r] * i0, v0[c], Um[e]);
+          Hm[e] = fma(v1[r] * i1, v1[c], Hm[e]);
         }
         __syncwarp();
       }
@@ -277,7 +273,7 @@ void launch_expand_mask(const SceneDev& sc, const nbv_config& cfg, const ExpandB
                         const float* conf, cudaStream_t st) {
   const MaskWarpLayout lay = mask_warp_layout(sc.K, groups);
   int wpb = 8;
-  while (wpb > 1 && (size_t)wpb * lay.per_warp * 8 > 200 * 1024) wpb >>= 1;
+  while (wpb > 1 && (size_t)wpb * lay.per_warp * 8 > 108 * 1024) wpb >>= 1;        // two blocks per SM
   const int L = 11 + sc.K;
   const size_t smem = (size_t)wpb * lay.per_warp * 8 + (((size_t)L * (L - 1) / 2 * 2 + 15) & ~(size_t)15);
   // the attribute is per device and per function: set it whenever the launch needs more than the default 48 KB
