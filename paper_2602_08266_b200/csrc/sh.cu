@@ -21,7 +21,6 @@ namespace nbv {
 constexpr int SH_NB = 16;
 constexpr int SH_L = NBV_SH_L;                      // 59
 constexpr int SH_LB = SH_L * (SH_L + 1) / 2;        // 1770
-constexpr int SH_LS = SH_L + 1;                     // row stride of the shared-memory matrices (doubles)
 
 __host__ __device__ __forceinline__ constexpr int triS(int r, int c) { return r * SH_L - r * (r - 1) / 2 + (c - r); }
 
@@ -89,37 +88,16 @@ void launch_sh_colours(const SceneDev& sc, const float* sh45, const PreBatch& ba
 }
 
 // ---- S5' + S6, one warp per touched Gaussian ---------------------------------------------------------------------------
-// shared memory per warp: Hc (59 x 60 doubles, the candidate / view block), Ha (59 x 60, the matrix being factored),
-// y (4 x 11), e (4 x 59), G (11 x 11), piv0 (59)
-constexpr int SH_WARP_DOUBLES = 2 * SH_L * SH_LS + 4 * 11 + 4 * SH_L + 121 + SH_L + 1;
-constexpr int SH_WARPS = 3;
-
-// in-place right-looking L D L^T of the symmetric matrix in M (full storage, upper triangle used), pivots -> piv (or the
-// log of pivot ratios accumulated when ref != nullptr).  All 32 lanes cooperate; returns sum_j log(d_j / ref_j) or 0.
-// `tri`: entry e of a row-major lower triangle -> (a << 8) | b, b <= a (filled once per block); the trailing triangle of
-// step j is a prefix of it, and its entries are dealt to the lanes one by one (a lane per row leaves the warp waiting for
-// the longest row: 3 x the serial length).
-constexpr int SH_TRI = SH_L * (SH_L - 1) / 2;
-__device__ double warp_ldl(double* M, double* piv, const double* ref, const uint16_t* tri, int lane) {
-  double ld = 0.0;
-  for (int j = 0; j < SH_L; ++j) {
-    __syncwarp();
-    const double d = fmax(M[j * SH_LS + j], 1e-300);
-    if (ref) ld += log(d / ref[j]); else if (lane == 0) piv[j] = d;
-    const double inv = -1.0 / d;
-    // trailing update: M[i][k] -= (M[j][i] / d) M[j][k] for j < i <= k
-    const int m = SH_L - j - 1, n = m * (m + 1) / 2;
-    const double* rowj = M + j * SH_LS + j + 1;
-    double* tr = M + (j + 1) * (SH_LS + 1);
-#pragma unroll 2
-    for (int e = lane; e < n; e += 32) {
-      const int ab = tri[e], k = ab >> 8, i = ab & 255;
-      tr[i * SH_LS + k] = fma(rowj[i] * inv, rowj[k], tr[i * SH_LS + k]);
-    }
-  }
-  __syncwarp();
-  return ld;
-}
+// shared memory per warp: Hc (the candidate / view block, then c (H_T + H) + Lambda) and Ha (c H_T + Lambda), both packed
+// symmetric (1,770 doubles) in the reversed order of mask.cu -- entry (i, j >= i) at r (r + 1) / 2 + c with r = 58 - i,
+// c = 58 - j, so that the trailing block of elimination step j is the prefix [0, m (m + 1) / 2), m = 58 - j, of the array and
+// the pivot row follows it -- then y (4 x 11), e (4 x 59), G (11 x 11), the pivots (2 x 59).  32 KB per warp: 6 resident warps
+// per SM (with full 59 x 60 storage and one factorisation after the other: 60 KB, 3 warps, 2.2 x the time).
+constexpr int SH_WARP_DOUBLES = 2 * SH_LB + 4 * 11 + 4 * SH_L + 121 + 2 * SH_L + 1;
+constexpr int SH_WARPS = 6;
+constexpr int SH_TRI = SH_L * (SH_L - 1) / 2;          // `tri`: entry e of a row-major lower triangle -> (row << 8) | column
+__device__ __forceinline__ int rtri(int r) { return r * (r + 1) / 2; }
+__device__ __forceinline__ int rpk(int i, int j) { return rtri(SH_L - 1 - i) + SH_L - 1 - j; }      // i <= j
 
 __global__ void __launch_bounds__(SH_WARPS * 32) expand_sh_kernel(const __grid_constant__ SceneDev sc, const __grid_constant__ nbv_config cfg,
                                                                     const __grid_constant__ ExpandBatch batch, int mode, int view0,
@@ -134,11 +112,11 @@ __global__ void __launch_bounds__(SH_WARPS * 32) expand_sh_kernel(const __grid_c
   const ExpandView& vw = batch.v[view0 + blockIdx.y];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   double* Hc = shm + (size_t)wib * SH_WARP_DOUBLES;
-  double* Ha = Hc + SH_L * SH_LS;
-  double* ys = Ha + SH_L * SH_LS;          // [4][11]
+  double* Ha = Hc + SH_LB;
+  double* ys = Ha + SH_LB;                 // [4][11]
   double* es = ys + 44;                    // [4][59]
   double* Gs = es + 4 * SH_L;              // [11][11]
-  double* piv0 = Gs + 121;                 // [59]
+  double* piv = Gs + 121;                  // [2][59]
   const uint32_t n_touched = vw.counters->n_touched;
   float omega[4];
 #pragma unroll
@@ -230,39 +208,68 @@ __global__ void __launch_bounds__(SH_WARPS * 32) expand_sh_kernel(const __grid_c
     }
     __syncwarp();
     const double W2 = m[MOM_W2];
-    // the full symmetric block, rows dealt to lanes
-    for (int rr = lane; rr < SH_L; rr += 32)
-      for (int cc = 0; cc < SH_L; ++cc) {
-        double v = (rr < 11 && cc < 11) ? Gs[rr * 11 + cc] : 0.0;
+    // the upper triangle of the block: lane l builds columns l and 58 - l (l + 1 and 59 - l entries: 60 per lane)
+    for (int half = 0; half < 2; ++half) {
+      const int cc = half == 0 ? lane : SH_L - 1 - lane;
+      if (lane >= 30 || (half == 1 && cc <= lane)) continue;
+      double yc[4], ec[4];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) { yc[c] = cc < 11 ? ys[c * 11 + cc] : 0.0; ec[c] = es[c * SH_L + cc]; }
+      for (int rr = 0; rr <= cc; ++rr) {
+        double v = cc < 11 ? Gs[rr * 11 + cc] : 0.0;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           if (omega[c] == 0.f) continue;
-          const double yr = rr < 11 ? ys[c * 11 + rr] : 0.0, yc = cc < 11 ? ys[c * 11 + cc] : 0.0;
-          const double er = es[c * SH_L + rr], ec = es[c * SH_L + cc];
-          v += yr * ec + er * yc + (double)omega[c] * W2 * er * ec;
+          const double yr = rr < 11 ? ys[c * 11 + rr] : 0.0;
+          const double er = es[c * SH_L + rr];
+          v += yr * ec[c] + er * yc[c] + (double)omega[c] * W2 * er * ec[c];
         }
-        Hc[rr * SH_LS + cc] = v;
+        Hc[rpk(rr, cc)] = v;
       }
+    }
     __syncwarp();
     if (mode == EXPAND_TRAIN || mode == EXPAND_VIEW) {
       for (int rr = 0; rr < SH_L; ++rr)
         for (int cc = rr + lane; cc < SH_L; cc += 32) {
-          if (mode == EXPAND_TRAIN) H_T[(size_t)g * SH_LB + triS(rr, cc)] += Hc[rr * SH_LS + cc];   // one launch per view, in view order
-          else vw.out_blocks[(size_t)g * SH_LB + triS(rr, cc)] = (float)Hc[rr * SH_LS + cc];
+          if (mode == EXPAND_TRAIN) H_T[(size_t)g * SH_LB + triS(rr, cc)] += Hc[rpk(rr, cc)];   // one launch per view, in view order
+          else vw.out_blocks[(size_t)g * SH_LB + triS(rr, cc)] = (float)Hc[rpk(rr, cc)];
         }
       continue;
     }
     const double c = (double)conf[g];
     double gn = 0.0;
     if (c > 0.0) {
+      // M0 = c H_T + Lambda -> Ha,  M1 = M0 + c H -> Hc, eliminated side by side (right-looking L D L^T); the gain is the sum of
+      // log(d1_j / d0_j) over the pivots.  Step j: pivot row = entries [n, n + m], n = m (m + 1) / 2, trailing block = entries
+      // [0, n), dealt to the lanes entry by entry through `tri`.
       const double* ht = H_T + (size_t)g * SH_LB;
-      for (int rr = 0; rr < SH_L; ++rr)
-        for (int cc = rr + lane; cc < SH_L; cc += 32) Ha[rr * SH_LS + cc] = c * ht[triS(rr, cc)] + (rr == cc ? (double)prior59[rr] : 0.0);
-      warp_ldl(Ha, piv0, nullptr, tri, lane);
-      for (int rr = 0; rr < SH_L; ++rr)
-        for (int cc = rr + lane; cc < SH_L; cc += 32)
-          Ha[rr * SH_LS + cc] = c * (ht[triS(rr, cc)] + Hc[rr * SH_LS + cc]) + (rr == cc ? (double)prior59[rr] : 0.0);
-      gn = warp_ldl(Ha, nullptr, piv0, tri, lane);
+      for (int rr = 0; rr < SH_L; ++rr) {
+        const int rb = rpk(rr, 0);
+        const double pr = (double)prior59[rr];
+        for (int cc = rr + lane; cc < SH_L; cc += 32) {
+          const double m0 = fma(c, ht[triS(rr, cc)], rr == cc ? pr : 0.0);
+          Ha[rb - cc] = m0;
+          Hc[rb - cc] = fma(c, Hc[rb - cc], m0);
+        }
+      }
+      __syncwarp();
+      for (int j = 0; j < SH_L; ++j) {
+        const int m = SH_L - 1 - j, n = m * (m + 1) / 2;
+        const double *v0 = Ha + n, *v1 = Hc + n;
+        const double d0 = fmax(v0[m], 1e-300), d1 = fmax(v1[m], 1e-300);
+        if (lane == 0) { piv[j] = d0; piv[SH_L + j] = d1; }
+        const double i0 = -1.0 / d0, i1 = -1.0 / d1;
+#pragma unroll 2
+        for (int e = lane; e < n; e += 32) {
+          const int rc = tri[e], r2 = rc >> 8, c2 = rc & 255;
+          Ha[e] = fma(v0[r2] * i0, v0[c2], Ha[e]);
+          Hc[e] = fma(v1[r2] * i1, v1[c2], Hc[e]);
+        }
+        __syncwarp();
+      }
+      for (int j = lane; j < SH_L; j += 32) gn += log(piv[SH_L + j] / piv[j]);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) gn += __shfl_xor_sync(0xffffffffu, gn, o);
     }
     if (lane == 0) {
       if (vw.gains) vw.gains[g] = (float)gn;
