@@ -421,10 +421,9 @@ nbv_config mask_group_config(const nbv_ctx* ctx, int gr) {
   return g;
 }
 
-// S3 (+ S4) for a batch of views whose S1-S2 products sit in sl[0..n): ONE launch per stage (S3, S4: persistent warps over (view, tile) positions; S5+S6: grid.y = view).
-// All views share the image size (same tile grid).  Stream st must already be ordered after the slots' S1-S2.
-int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int upto, bool full_pix, cudaStream_t st) {
-  RasterBatch rb;
+// The launch descriptor of S3 / S4 over the views in sl[0..n).  again: a further S4 pass over the lists the batch's S3 left
+// (second output of a fused call): fresh work counters, S3's overflow count kept.
+int fill_raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, int n, bool full_pix, bool again, cudaStream_t st, RasterBatch& rb) {
   rb.n = n;
   rb.n_work = 0;
   rb.work = nullptr;
@@ -438,7 +437,7 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     rb.work_fb = rb.work + 1;
     rb.work_fwd = rb.work + 2;
     rb.overflow = rb.work + 3;
-    CK(cudaMemsetAsync(rb.work, 0, 16, st));
+    CK(cudaMemsetAsync(rb.work, 0, again ? 8 : 16, st));
   }
   for (int i = 0; i < n; ++i) {
     ViewSlot* s = sl[i];
@@ -455,9 +454,17 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     v.touched_flag = reinterpret_cast<uint8_t*>(s->moments.p) + sizeof(double) * NMOM * (size_t)ctx->mask_groups * (size_t)ctx->N;
     v.touched_cnt = s->touched_cnt.as<uint32_t>(); v.counters = s->d_counters;
   }
-  const TileGrid tg = sl[0]->tg;
-  CKRET(ensure_tile_order(ctx, tg, st));
+  CKRET(ensure_tile_order(ctx, sl[0]->tg, st));
   rb.tile_order = ctx->tile_order.as<uint32_t>();
+  return NBV_OK;
+}
+
+// S3 (+ S4) for a batch of views whose S1-S2 products sit in sl[0..n): ONE launch per stage (S3, S4: persistent warps over (view, tile) positions; S5+S6: grid.y = view).
+// All views share the image size (same tile grid).  Stream st must already be ordered after the slots' S1-S2.
+int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int n, int upto, bool full_pix, cudaStream_t st) {
+  RasterBatch rb;
+  CKRET(fill_raster_batch(ctx, sl, n, full_pix, false, st, rb));
+  const TileGrid tg = sl[0]->tg;
   int sp = span_begin(ctx, NBV_STAGE_FORWARD, n, st);
   launch_forward(rb, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, ctx->cfg, full_pix, st);
   CK(cudaGetLastError());
@@ -482,6 +489,20 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
     }
   }
   launch_touched(rb, ctx->N, st);            // sum w^2 of (group 0 of) every rank -> ordered touched lists
+  CK(cudaGetLastError());
+  span_end(ctx, sp, st);
+  return NBV_OK;
+}
+
+// S4 of another output over the same views (fused scoring, Eq. 10-11): S1-S3 do not depend on the output -- `T`, `last` and the
+// tile lists are the ones the batch's S3 left -- so a colour / depth context that shares the map and the compositing constants
+// of ctx sweeps them again with its own channels.  The moments and flags are clean again after ctx's own S5+S6.
+int backward_again(nbv_ctx* ctx, const nbv_ctx* other, ViewSlot* const* sl, const nbv_camera* cams, int n, cudaStream_t st) {
+  RasterBatch rb;
+  CKRET(fill_raster_batch(ctx, sl, n, false, true, st, rb));
+  const int sp = span_begin(ctx, NBV_STAGE_BACKWARD, n, st);
+  launch_backward(rb, ctx->N, sl[0]->tg, sl[0]->rank_bits, cams[0].width, cams[0].height, other->cfg, st);
+  launch_touched(rb, ctx->N, st);
   CK(cudaGetLastError());
   span_end(ctx, sp, st);
   return NBV_OK;
@@ -534,7 +555,10 @@ int expand_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int mode, flo
 // Run S1..S6 for n cameras in batches of up to `concurrency` views of equal image size.  S1-S2 of every view run on its slot's
 // stream; S3, S4 and S5+S6 of the whole batch are one launch each on the caller's stream.  Two slot sets alternate, so the
 // S1-S2 work of batch b+1 overlaps the S3-S6 launches of batch b.  Everything is ordered by events: the call never blocks.
-int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_scores, cudaStream_t st, const BlockCache* cache = nullptr) {
+// second / d_scores2 (EXPAND_GAIN only): a second colour / depth context on the same map whose scores are wanted for the same
+// views; it reuses S1-S3 of every batch (backward_again) and runs its own S4-S6 after ctx's.
+int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_scores, cudaStream_t st, const BlockCache* cache = nullptr,
+              nbv_ctx* second = nullptr, float* d_scores2 = nullptr) {
   // automatic batch size: 8 views of a 1280 x 720 image are 28,800 (view, tile) positions for the ~2,400 resident S4 warps;
   // smaller images get 16 views per batch so that every warp still draws several positions
   int V = ctx->concurrency;
@@ -575,6 +599,11 @@ int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_
     if ((mode == EXPAND_TRAIN || mode == EXPAND_CACHE) && set_used[set ^ 1])
       ck(cudaStreamWaitEvent(rs, ctx->ev_set_done[set ^ 1], 0), "cudaStreamWaitEvent(order)");
     if (rc == NBV_OK) rc = expand_batch(ctx, sl, h_cams + i0, nb, mode, nullptr, d_scores ? d_scores + i0 : nullptr, nullptr, rs, cache, i0);
+    if (second && rc == NBV_OK) rc = backward_again(ctx, second, sl, h_cams + i0, nb, rs);
+    if (second && rc == NBV_OK) {
+      rc = expand_batch(second, sl, h_cams + i0, nb, mode, nullptr, d_scores2 + i0, nullptr, rs);
+      if (rc != NBV_OK) ctx->err = second->err;
+    }
     ck(cudaEventRecord(ctx->ev_set_done[set], rs), "cudaEventRecord(set)");
     set_used[set] = true;
     i0 += nb;
@@ -864,7 +893,23 @@ int nbv_score_candidates_fused(nbv_ctx* ctx_rgb, nbv_ctx* ctx_depth, nbv_ctx* ct
   float* denom = train + (size_t)F * n_train;
   int32_t* scratch = reinterpret_cast<int32_t*>(denom + 4);
   nbv_ctx* cx[3] = {ctx_rgb, ctx_depth, ctx_mask};
-  for (int f = 0; f < F; ++f) {
+  // RGB and depth differ in S4-S6 only: when both contexts composite with the same constants, every view goes through S1-S3 once
+  const nbv_config &ca = ctx_rgb->cfg, &cb = ctx_depth->cfg;
+  const bool paired = !ctx_rgb->sh_mode && !ctx_depth->sh_mode && !ctx_rgb->mask_mode && !ctx_depth->mask_mode && ca.near_plane == cb.near_plane &&
+                      ca.blur == cb.blur && ca.alpha_min == cb.alpha_min && ca.alpha_max == cb.alpha_max && ca.t_stop == cb.t_stop;
+  if (paired) {
+    for (int i = 0; i < n + n_train; ++i)
+      if (!valid_camera(i < n ? h_cams[i] : h_train[i - n]))
+        return fail(ctx, NBV_ERR_INVALID_ARG, "invalid camera (size, focal length or non-orthonormal R_cw)");
+    CKRET(prepare_scoring(ctx_rgb, target_obj, st));
+    const int rcd = prepare_scoring(ctx_depth, target_obj, st);
+    if (rcd != NBV_OK) { ctx->err = ctx_depth->err; return rcd; }
+    CK(cudaMemsetAsync(raw, 0, 4 * (size_t)2 * n, st));
+    CK(cudaMemsetAsync(train, 0, 4 * (size_t)2 * n_train, st));
+    CKRET(run_views(ctx_rgb, h_cams, n, EXPAND_GAIN, raw, st, nullptr, ctx_depth, raw + n));
+    CKRET(run_views(ctx_rgb, h_train, n_train, EXPAND_GAIN, train, st, nullptr, ctx_depth, train + n_train));
+  }
+  for (int f = paired ? 2 : 0; f < F; ++f) {
     int rc = nbv_score_candidates(cx[f], h_cams, n, target_obj, raw + (size_t)f * n, scratch, stream);
     if (rc == NBV_OK) rc = nbv_score_candidates(cx[f], h_train, n_train, target_obj, train + (size_t)f * n_train, scratch, stream);
     if (rc != NBV_OK) {
