@@ -263,6 +263,29 @@ int nbv_exp_spec_pairs(const float* d_x, float* d_y, int64_t n, void* stream);
 /* Number of CUDA kernels this library has launched in this process so far (all contexts). */
 int64_t nbv_kernel_launches(void);
 
+/* ---- the one call that allocates nothing ------------------------------------------------------------- */
+
+/* Exclusive prefix sum of n 32-bit counts: d_out[i] = d_in[0] + ... + d_in[i-1] (mod 2^32), *d_total = the sum of all n --
+ * the scan that turns S2's count tables into list offsets (per-tile list lengths -> the offsets of nbv_tile_lists; DESIGN.md
+ * section 5, R-5), for callers that may not allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  The context calls keep their scratch in buffers the context allocates on demand; this call keeps the only
+ * scratch the scan needs (one block sum per 2,048 elements) in a static device array of 8,192 words = 32 KB inside the library,
+ * which every GPU that loads the library holds until the process exits.  It calls no cudaMalloc, cudaFree or allocating library
+ * routine: at most three kernel launches on `stream` (for n == 0 one cudaMemsetAsync of the total).  The array's device address
+ * is resolved on the first call on each device (cudaGetSymbolAddress, not an allocation); make that first call outside a
+ * graph capture.
+ *   d_in    DEVICE, n uint32 (read only);   d_out   DEVICE, n uint32, may be d_in (in place);   d_total  DEVICE, 1 uint32, or NULL
+ *   n       0 <= n <= NBV_SCAN_NOALLOC_MAX; beyond that NBV_ERR_CAPACITY and nothing is launched
+ *   stream  cudaStream_t; asynchronous, never synchronises.  The caller owns all three buffers.
+ * EVERY call on a device shares the one array, and the array keeps the previous call's contents (a call overwrites what it
+ * reads before reading it, so nothing needs clearing): calls that overlap on the GPU -- different streams without an event
+ * between them, or two host threads -- race on it and return garbage; calls in one stream, or ordered by events, are safe.
+ * Errors: NBV_ERR_INVALID_ARG (n < 0, null d_in / d_out with n > 0), NBV_ERR_CAPACITY (n too large), NBV_ERR_CUDA; the text of the
+ * calling thread's last failure: nbv_noalloc_last_error(). */
+#define NBV_SCAN_NOALLOC_MAX 16777216   /* 8,192 blocks x 2,048 elements */
+int nbv_exclusive_scan_noalloc(const uint32_t* d_in, uint32_t* d_out, int64_t n, uint32_t* d_total, void* stream);
+const char* nbv_noalloc_last_error(void);
+
 /* ---- parity / debug exports (not on the timed path) ------------------------------------------------ */
 
 /* S1 outputs of one view, indexed by Gaussian: d_visible N int32; d_rec N x 9 floats

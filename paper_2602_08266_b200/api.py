@@ -36,7 +36,7 @@ EXPORTS = [
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
     "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
     "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy", "nbv_block_size", "nbv_render_mask", "nbv_measure_ffma_peak",
-    "nbv_chain", "nbv_load_sh", "nbv_exp_spec_pairs",
+    "nbv_chain", "nbv_load_sh", "nbv_exp_spec_pairs", "nbv_exclusive_scan_noalloc", "nbv_noalloc_last_error",
 ]
 
 STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
@@ -87,6 +87,8 @@ def load_library(path: Path | None = None):
     lib.nbv_destroy.argtypes = [C.c_void_p]
     lib.nbv_default_config.restype = None
     lib.nbv_kernel_launches.restype = C.c_int64
+    lib.nbv_noalloc_last_error.restype = C.c_char_p
+    lib.nbv_noalloc_last_error.argtypes = []
     lib.nbv_block_size.restype = C.c_int64
     lib.nbv_block_size.argtypes = [C.c_void_p]
     if path is None:
@@ -355,6 +357,26 @@ def exp_spec_pairs(x):
     if rc != 0:
         raise NBVError(rc, "nbv_exp_spec_pairs failed")
     return y
+
+
+SCAN_NOALLOC_MAX = 16777216      # NBV_SCAN_NOALLOC_MAX
+
+
+def exclusive_scan_noalloc(x, out=None, total=None):
+    """nbv_exclusive_scan_noalloc: exclusive prefix sum of a CUDA int32 / uint32 tensor (the bits are taken as uint32) with the
+    scratch in the library's static device array -- the call itself allocates nothing; the tensors are the caller's: `out`
+    (same size, may be x) and `total` (1 element) are created here only when not passed in.  Returns (out, total)."""
+    import torch
+    x = x.contiguous()
+    if out is None:
+        out = torch.empty_like(x)
+    if total is None:
+        total = torch.empty(1, dtype=x.dtype, device=x.device)
+    lib = load_library()
+    rc = lib.nbv_exclusive_scan_noalloc(_ptr(x), _ptr(out), C.c_int64(x.numel()), _ptr(total), _stream())
+    if rc != 0:
+        raise NBVError(rc, (lib.nbv_noalloc_last_error() or b"").decode())
+    return out, total
 
 
 def measure_ffma_peak() -> float:

@@ -15,7 +15,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 OBJ = PKG / "build"
 LIB = PKG / "libnbv.so"
-SOURCES = ["sort.cu", "project.cu", "binning.cu", "raster.cu", "hessian.cu", "mask.cu", "sh.cu", "select.cu", "peak.cu", "nbv_api.cu"]
+SOURCES = ["sort.cu", "project.cu", "binning.cu", "raster.cu", "hessian.cu", "mask.cu", "sh.cu", "select.cu", "peak.cu", "noalloc.cu", "nbv_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
