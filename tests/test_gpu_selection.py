@@ -51,6 +51,29 @@ def test_fused_scores_match_the_oracle(target):
     assert float(unit["fused"].mean().item()) == pytest.approx(11.0, rel=1e-4)
 
 
+def test_fused_shared_and_separate_rasterisation_agree():
+    """The RGB and the depth context share S1-S3 of every batch when they composite with the same constants (the depth
+    context sweeps the tile lists S3 left again); with different constants each context rasterises for itself.  A near plane
+    moved by one part in 1e5 culls the same Gaussians, so both routes must give the same numbers -- and several batches."""
+    from paper_2602_08266_b200 import api
+    wl = _workload(3, 20)
+    nr = _ctx(wl.scene, api.CH_RGB, wl.train_cams)
+    nd = _ctx(wl.scene, api.CH_DEPTH, wl.train_cams)
+    nd2 = api.NBV(channel_mask=api.CH_DEPTH, near_plane=0.0100001)
+    nd2.load_scene(wl.scene)
+    nd2.accumulate_training(wl.train_cams)
+    for n in (nr, nd, nd2):
+        n.set_concurrency(8)                                             # 20 candidates: batches of 8, 8, 4 on both raster streams
+    shared = api.score_candidates_fused(nr, nd, wl.train_cams, wl.cand_cams, -1, 10.0)
+    separate = api.score_candidates_fused(nr, nd2, wl.train_cams, wl.cand_cams, -1, 10.0)
+    for k in ("raw", "denom", "fused"):
+        np.testing.assert_allclose(shared[k].cpu().numpy(), separate[k].cpu().numpy(), rtol=1e-6, atol=0)
+    assert int(shared["best"].item()) == int(separate["best"].item())
+    # and the contexts are left as they were: a plain scoring call on the depth context alone gives its raw row
+    sd, _ = nd.score_candidates(wl.cand_cams)
+    np.testing.assert_allclose(sd.cpu().numpy(), shared["raw"][1].cpu().numpy(), rtol=1e-6, atol=0)
+
+
 def test_fused_argument_errors():
     from paper_2602_08266_b200 import api
     wl = _workload(1, 2, n_gaussians=200)
