@@ -336,8 +336,8 @@ __device__ __forceinline__ void red_add_f64(double* dst, double v) { asm volatil
 // slot body itself (ncu r2a: 41% of the kernel's instructions).  Instead the column sums of GE = 4 entries are parked in
 // shared memory and ONE tail serves them all: lane l takes entry l / 8 and the four source lanes l % 8 + 8 k, assembles
 // their moments (the source lane's pixel column and row block follow from its index) and accumulates them in registers;
-// one shared-memory transpose then folds the eight partial sums of every entry, and the lanes issue the 16-byte reductions
-// into the L2 -- every lane assembles 4 (entry, lane) pairs instead of 4 entries x 1 lane, but the 32-row reduction per
+// one shared-memory transpose then folds the eight partial sums of every entry, and the lanes issue the binary64 reductions
+// into the L2 (red_add_f64 above) -- every lane assembles 4 (entry, lane) pairs instead of 4 entries x 1 lane, but the 32-row reduction per
 // entry becomes an 8-row reduction per FOUR entries.
 constexpr int GE = 4;
 
