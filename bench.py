@@ -46,10 +46,9 @@ FP32_LANES_PER_SM = 128
 FLOP_PER_EVAL = {"forward": 31.6, "backward": {3: 84.7, 4: 99.9}}
 FLOP_SOURCE = "profiles/r2_ncu_flops_cfg2.md"
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
-VIEWS_PER_LAUNCH = 8      # S3 / S4 / S5+S6 are one launch per batch of 8 views (16 for images of fewer than 2,000 tiles)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture named
 # in TRAFFIC_SOURCE; known for config 2 only (null elsewhere)
-NCU_TRAFFIC_BYTES = {2: {"backward": 113.8e6, "forward": 55.2e6}}
+NCU_TRAFFIC_BYTES_PER_VIEW = {2: {"backward": 235.2e6 / 16, "forward": 167.1e6 / 16}}      # the capture is of a 16-view launch
 TRAFFIC_SOURCE = "profiles/r2_ncu_raster_cfg2.md (ncu --set full of the first candidate batch; a stored figure, not measured by this run)"
 
 
@@ -377,7 +376,7 @@ def main():
     # batch b (two raster streams), so a launch's event-to-event duration there includes time the other kernel ran; with one
     # batch per call every raster launch has the GPU to itself and its duration is the kernel's own (`roofline` uses these) ----
     W_, H_ = int(wl.cand_cams[0]["width"]), int(wl.cand_cams[0]["height"])
-    vpl = args.concurrency or (16 if ((W_ + 15) // 16) * ((H_ + 15) // 16) < 2000 else VIEWS_PER_LAUNCH)
+    vpl = nbv.batch_views(W_, H_)                       # views per S3 / S4 / S5+S6 launch, as the library batches them
     vpl = min(vpl, C)
     nbv.set_stage_timing(True)                          # clears the accumulated times of the pass above
     for _ in range(args.steps):
@@ -442,8 +441,8 @@ def main():
         sec = (per_view_ms_x[k] if batched else per_view_ms[k]) * 1e-3
         ach = amount / sec if sec > 0 else 0.0
         rl[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
-                 "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(k),
-                 "traffic_source": TRAFFIC_SOURCE if NCU_TRAFFIC_BYTES.get(args.config, {}).get(k) else None,
+                 "traffic": (NCU_TRAFFIC_BYTES_PER_VIEW[args.config][k] * vpl) if k in NCU_TRAFFIC_BYTES_PER_VIEW.get(args.config, {}) else None,
+                 "traffic_source": TRAFFIC_SOURCE if k in NCU_TRAFFIC_BYTES_PER_VIEW.get(args.config, {}) else None,
                  "flops_source": ("executed fp32 flop per evaluation from " + FLOP_SOURCE) if batched else None,
                  "views_per_launch": vpl if batched else 1,
                  "ms_per_launch": (per_view_ms_x[k] * vpl) if batched else per_view_ms[k],

@@ -125,15 +125,18 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg);
 void nbv_destroy(nbv_ctx* ctx);
 const char* nbv_last_error(const nbv_ctx* ctx);
 
-/* Views per batch (1..16; default: 8, or 16 for images of fewer than 2,000 tiles; the NBV_CONCURRENCY environment variable
- * overrides the default at nbv_create).
+/* Views per batch (1..16; default, chosen per call: 16 -- for images of at least 2,000 tiles only when the two sets of 16 view
+ * slots, whose size grows with N x supertiles, fit a sixth of the device memory, else 8; the NBV_CONCURRENCY environment
+ * variable overrides the default at nbv_create).  nbv_batch_views() returns the number a call with images of the given size
+ * would use (0 on bad arguments).
  * S1-S2 of the views of a batch run concurrently on internal streams (forked from and joined back into the caller's
  * stream with events); S3, S4 and S5+S6 are ONE kernel launch each per batch (S3 and S4: persistent warps pulling
  * (view, tile) positions).  Two sets of work buffers and two internal raster streams alternate between batches.  Views are independent
- * (the arg max is over per-view gains), so this changes no result beyond the order of the binary32 reductions of S4
+ * (the arg max is over per-view gains), so this changes no result beyond the order of S4's cross-tile binary64 reductions (exact for realistic footprints)
  * (H_T is accumulated view by view in call order, and a candidate's score is summed in a fixed order).
  * Errors: INVALID_ARG outside [1, 16]. */
 int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight);
+int32_t nbv_batch_views(const nbv_ctx* ctx, int32_t width, int32_t height);
 
 /* S0 -- load the Gaussian map G with object vectors: device arrays, row-major, float32.
  *   d_mean N x 3, d_logscale N x 3, d_quat N x 4 (w,x,y,z; any non-zero norm), d_opacity N (sigma in (0,1)),

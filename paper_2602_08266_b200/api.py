@@ -36,7 +36,7 @@ EXPORTS = [
     "nbv_projected", "nbv_tile_lists", "nbv_render", "nbv_view_hessian", "nbv_training_hessian", "nbv_confidence",
     "nbv_gaussian_gains", "nbv_set_stage_timing", "nbv_stage_times", "nbv_kernel_launches", "nbv_set_concurrency",
     "nbv_tile_walk", "nbv_score_candidates_fused", "nbv_select_greedy", "nbv_block_size", "nbv_render_mask", "nbv_measure_ffma_peak",
-    "nbv_chain", "nbv_load_sh", "nbv_exp_spec_pairs", "nbv_exclusive_scan_noalloc", "nbv_noalloc_last_error",
+    "nbv_chain", "nbv_load_sh", "nbv_exp_spec_pairs", "nbv_exclusive_scan_noalloc", "nbv_noalloc_last_error", "nbv_batch_views",
 ]
 
 STAGES = ["project", "depth_sort", "bin", "coarse_sort", "forward", "backward", "expand_gain"]
@@ -230,6 +230,10 @@ class NBV:
         self._check(self.lib.nbv_select_greedy(self._h, C.c_void_p(cams.ctypes.data), n, int(rounds), int(target_obj),
                                                C.c_void_p(order.ctypes.data), _ptr(scores), _stream()))
         return order[:rounds], (scores[:rounds, :n] if want_scores else None)
+
+    def batch_views(self, width: int, height: int) -> int:
+        """nbv_batch_views: views per batch a call with images of this size would use"""
+        return int(self.lib.nbv_batch_views(self._h, int(width), int(height)))
 
     def set_concurrency(self, views_in_flight: int):
         self._check(self.lib.nbv_set_concurrency(self._h, int(views_in_flight)))

@@ -82,7 +82,8 @@ struct nbv_ctx {
   // views in flight: S1-S2 of each view run on its slot's stream, S3-S6 of a whole batch in one launch per stage on
   // the caller's stream; two sets of `concurrency` slots alternate so the next batch's S1-S2 overlap this batch's S3-S6
   std::vector<ViewSlot*> slots;
-  int concurrency = 0;                  // views per batch; 0 = automatic (8, or 16 for images of fewer than 2,000 tiles)
+  int concurrency = 0;                  // views per batch; 0 = automatic (auto_batch_views)
+  size_t dev_mem_total = 0;             // bytes of device memory (cudaMemGetInfo at nbv_create); 0 = unknown
   cudaEvent_t ev_fork = nullptr;
   cudaEvent_t ev_set_done[2] = {nullptr, nullptr};   // S3-S6 of the last batch that used slot set 0 / 1
   cudaStream_t raster_st[2] = {nullptr, nullptr};    // S3-S6 of the batches of slot set 0 / 1 (forked from / joined into the caller's stream)
@@ -552,6 +553,23 @@ int expand_view(nbv_ctx* ctx, ViewSlot* sl, const nbv_camera& cam, int mode, flo
   return expand_batch(ctx, &sl, &cam, 1, mode, out_blocks, score, gains, st);
 }
 
+// Views per batch when the caller has not fixed it.  A batch is one S3 and one S4 launch of persistent warps; between launches the
+// SMs drain, and the small launches around them (S1-S2, touched lists, S5+S6) only find room in those drains, so fewer, longer
+// batches cost less: 16 views per batch instead of 8 gave +3.6% at config 2 and +3.2% at config 4.  The
+// price is memory: two sets of V view slots (worst-case coarse lists, the binary64 moment rows), 9.7 GB at config 2 and 40.6 GB
+// at config 4 for V = 16 -- and a fused call keeps up to three contexts alive (at config 4 the mask context alone needs 86 GB
+// with V = 8).  So: 16 when the 32 slots fit a sixth of the device memory (config 2: yes, config 4: no), else 8.
+int auto_batch_views(const nbv_ctx* ctx, int W, int H) {
+  if (ctx->concurrency > 0) return ctx->concurrency;
+  const TileGrid tg = make_grid(W, H);
+  const size_t n_tiles = (size_t)tg.tiles_x * tg.tiles_y, n_super = (size_t)tg.super_x * tg.super_y, N = (size_t)ctx->N;
+  if (n_tiles < 2000) return 16;                 // small images: 16 views are needed to give every resident warp several tiles
+  const size_t per_slot = N * (2 * sizeof(Splat) + 2 * sizeof(ushort4) + 6 * 4 + 1 + (ctx->mask_mode ? sizeof(Splat) : 0)) +
+                          N * n_super * (4 + sizeof(ushort4)) + 8 * (size_t)NMOM * ctx->mask_groups * N +
+                          8 * (size_t)W * H + 4 * n_tiles * TL_CAP;
+  return ctx->dev_mem_total && 2 * MAX_BATCH * per_slot <= ctx->dev_mem_total / 6 ? 16 : 8;
+}
+
 // Run S1..S6 for n cameras in batches of up to `concurrency` views of equal image size.  S1-S2 of every view run on its slot's
 // stream; S3, S4 and S5+S6 of the whole batch are one launch each on the caller's stream.  Two slot sets alternate, so the
 // S1-S2 work of batch b+1 overlaps the S3-S6 launches of batch b.  Everything is ordered by events: the call never blocks.
@@ -561,8 +579,7 @@ int run_views(nbv_ctx* ctx, const nbv_camera* h_cams, int n, int mode, float* d_
               nbv_ctx* second = nullptr, float* d_scores2 = nullptr) {
   // automatic batch size: 8 views of a 1280 x 720 image are 28,800 (view, tile) positions for the ~2,400 resident S4 warps;
   // smaller images get 16 views per batch so that every warp still draws several positions
-  int V = ctx->concurrency;
-  if (V <= 0) V = (n > 0 && make_grid(h_cams[0].width, h_cams[0].height).tiles_x * make_grid(h_cams[0].width, h_cams[0].height).tiles_y < 2000) ? 16 : 8;
+  int V = n > 0 ? auto_batch_views(ctx, h_cams[0].width, h_cams[0].height) : 1;
   V = std::max(1, std::min(V, MAX_BATCH));
   int rc = NBV_OK;
   CK(cudaEventRecord(ctx->ev_fork, st));
@@ -710,6 +727,10 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
     return NBV_ERR_CUDA;
   }
   if (ensure(ctx, ctx->work_counters, 3 * 128) != NBV_OK) { nbv_destroy(ctx); return NBV_ERR_OOM; }
+  {
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) ctx->dev_mem_total = total_b; else cudaGetLastError();
+  }
   if (const char* e = std::getenv("NBV_PERSISTENT")) ctx->persistent = std::atoi(e) != 0;
   if (const char* e = std::getenv("NBV_GREEDY_CACHE_MB")) ctx->greedy_cache_bytes = (size_t)std::max(0, std::atoi(e)) << 20;
   if (const char* e = std::getenv("NBV_CONCURRENCY")) {
@@ -741,6 +762,11 @@ int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight) {
   if (views_in_flight < 1 || views_in_flight > MAX_BATCH) return fail(ctx, NBV_ERR_INVALID_ARG, "views_in_flight must be in [1, 16]");
   ctx->concurrency = views_in_flight;
   return NBV_OK;
+}
+
+int32_t nbv_batch_views(const nbv_ctx* ctx, int32_t width, int32_t height) {
+  if (!ctx || width <= 0 || height <= 0) return 0;
+  return (int32_t)std::max(1, std::min(auto_batch_views(ctx, width, height), MAX_BATCH));
 }
 
 const char* nbv_last_error(const nbv_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
