@@ -120,6 +120,10 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
                     cudaStream_t st);
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,
                      cudaStream_t st);
+// S3 + S4 of a batch in ONE persistent launch (a warp sweeps its tile forward, then backward from the registers S3 ends with),
+// followed by the fallback S4 launch for tiles whose list outgrew TL_CAP; needs batch.work_fwd and the tile lists.  Opt-in
+// (NBV_FUSED_RASTER=1): measured slower than the two launches
+void launch_raster_fused(const RasterBatch& batch, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg, cudaStream_t st);
 
 // ---- hessian.cu (colour / depth contexts: everything after S4's binary32 per-tile moment sums is binary64)
 // the touched lists (ranks with sum w^2 != 0, in rank order) of every view of the batch

@@ -83,6 +83,7 @@ struct nbv_ctx {
   // the caller's stream; two sets of `concurrency` slots alternate so the next batch's S1-S2 overlap this batch's S3-S6
   std::vector<ViewSlot*> slots;
   int concurrency = 0;                  // views per batch; 0 = automatic (auto_batch_views)
+  bool fused_raster = false;            // NBV_FUSED_RASTER=1: S3 + S4 of a batch in one persistent launch (raster_kernel); measured 3% slower
   size_t dev_mem_total = 0;             // bytes of device memory (cudaMemGetInfo at nbv_create); 0 = unknown
   cudaEvent_t ev_fork = nullptr;
   cudaEvent_t ev_set_done[2] = {nullptr, nullptr};   // S3-S6 of the last batch that used slot set 0 / 1
@@ -466,6 +467,15 @@ int raster_batch(nbv_ctx* ctx, ViewSlot* const* sl, const nbv_camera* cams, int 
   RasterBatch rb;
   CKRET(fill_raster_batch(ctx, sl, n, full_pix, false, st, rb));
   const TileGrid tg = sl[0]->tg;
+  if (ctx->fused_raster && upto == STAGE_BACKWARD && !full_pix && !ctx->mask_mode && rb.work_fwd && rb.v[0].tlist) {
+    // opt-in: one launch for S3 + S4 (its time is booked under the backward stage; the forward stage then shows zero)
+    const int spf = span_begin(ctx, NBV_STAGE_BACKWARD, n, st);
+    launch_raster_fused(rb, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, ctx->cfg, st);
+    launch_touched(rb, ctx->N, st);
+    CK(cudaGetLastError());
+    span_end(ctx, spf, st);
+    return NBV_OK;
+  }
   int sp = span_begin(ctx, NBV_STAGE_FORWARD, n, st);
   launch_forward(rb, tg, sl[0]->rank_bits, cams[0].width, cams[0].height, ctx->cfg, full_pix, st);
   CK(cudaGetLastError());
@@ -732,6 +742,7 @@ int nbv_create(nbv_ctx** out, const nbv_config* cfg) {
     if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) ctx->dev_mem_total = total_b; else cudaGetLastError();
   }
   if (const char* e = std::getenv("NBV_PERSISTENT")) ctx->persistent = std::atoi(e) != 0;
+  if (const char* e = std::getenv("NBV_FUSED_RASTER")) ctx->fused_raster = std::atoi(e) != 0;
   if (const char* e = std::getenv("NBV_GREEDY_CACHE_MB")) ctx->greedy_cache_bytes = (size_t)std::max(0, std::atoi(e)) << 20;
   if (const char* e = std::getenv("NBV_CONCURRENCY")) {
     const int v = std::atoi(e);

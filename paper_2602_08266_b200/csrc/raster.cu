@@ -118,24 +118,19 @@ __device__ __forceinline__ void shift_queue(uint32_t* q_rank, uint32_t* q_cpos, 
 // per lane and tile -- retires it (py = +inf: its power fails every later range test), counts it, and records in `last`
 // how many list entries precede the stop.  A pixel that never stops gets last = number of entries walked.  Every entry
 // S4 must composite at a pixel lies before `last`, and S4 re-takes the same pass decisions, so it finds the same set.
+// what S3 leaves in registers for an S4 sweep of the same tile by the same warp (raster_kernel): the final transmittance and
+// `last` of the lane's 8 pixels (pairs as in the slot bodies) and the tile's list length
+struct FwdOut {
+  f2 T2[PPL / 2];
+  int last[PPL];
+  uint32_t elast;
+};
+
+// S3 of one launch position (view, tile) by one warp.  sm: 96 float4; q_rank, q_cpos, p_rank, p_cpos: 64 words each (p_*: rect
+// hits awaiting the ellipse test, stage 2 of the tile filter).
 template <bool FULLPIX>
-__global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
-  // One launch rasterises every view of the batch (DESIGN.md section 5).  Launch position -> (view, tile): the views are
-  // interleaved, so the launch starts with the central (long-running) tiles of ALL views and its tail is made of the
-  // edge tiles of all views.
-  // Persistent warps (batch.work_fwd != nullptr): the grid is one wave of resident warps and every warp pulls launch
-  // positions from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
-  __shared__ float4 sm[32 * 3];
-  __shared__ uint32_t q_rank[64], q_cpos[64];
-  __shared__ uint32_t p_rank[64], p_cpos[64];             // rect hits awaiting the ellipse test (stage 2 of the tile filter)
-  const int lane = threadIdx.x;
-  for (uint32_t bpos = blockIdx.x;; ) {
-  if (batch.work_fwd) {
-    if (lane == 0) bpos = atomicAdd(batch.work_fwd, 1u);
-    bpos = __shfl_sync(FULL, bpos, 0);
-  }
-  if (bpos >= batch.n_work) return;
-  __syncwarp();
+__device__ __forceinline__ void forward_tile(const RasterBatch& batch, const RasterParams& prm, uint32_t bpos, int lane, float4* sm,
+                                             uint32_t* q_rank, uint32_t* q_cpos, uint32_t* p_rank, uint32_t* p_cpos, FwdOut& fo) {
   const int vidx = (int)(bpos % (uint32_t)batch.n);
   const RasterView& vw = batch.v[vidx];
   const Splat* __restrict__ splat_sorted = vw.splat_sorted;
@@ -285,10 +280,13 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   unsigned pairs = 0;
 #pragma unroll
   for (int k = 0; k < PPL; ++k) {
+    const float pyk = k < PPL / 2 ? py2[k].x : py2[PPL - 1 - k].y;
+    // never stopped: every walked entry precedes `last`; outside the image: py = inf from the start, last = 0 (and T = 1)
+    const int lk = pyk == INFINITY ? last[k] : (int)walked;
+    fo.last[k] = lk;
     if (x < prm.W && y0 + k < prm.H) {
       const size_t p = (size_t)(y0 + k) * prm.W + x;
       const float Tk = k < PPL / 2 ? T2[k].x : T2[PPL - 1 - k].y;
-      const float pyk = k < PPL / 2 ? py2[k].x : py2[PPL - 1 - k].y;
       if (FULLPIX) {
         pairs += n[k];
         out.rgb[3 * p + 0] = fmaf(prm.bg[0], Tk, C0[k]);
@@ -298,9 +296,11 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
         out.ncontrib[p] = n[k];
       }
       out.T[p] = Tk;
-      out.last[p] = pyk == INFINITY ? last[k] : (int)walked;     // never stopped: every walked entry precedes `last`
+      out.last[p] = lk;
     }
   }
+#pragma unroll
+  for (int q = 0; q < PPL / 2; ++q) fo.T2[q] = T2[q];
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     if (FULLPIX) pairs += __shfl_xor_sync(FULL, pairs, o);
@@ -317,8 +317,31 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
       atomicAdd(&counters->n_pairs, (unsigned long long)pairs);
     }
   }
-  if (!batch.work_fwd) return;
-  }  // persistent loop
+  fo.elast = elast;
+}
+
+template <bool FULLPIX>
+__global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
+  // One launch rasterises every view of the batch (DESIGN.md section 5).  Launch position -> (view, tile): the views are
+  // interleaved, so the launch starts with the central (long-running) tiles of ALL views and its tail is made of the
+  // edge tiles of all views.
+  // Persistent warps (batch.work_fwd != nullptr): the grid is one wave of resident warps and every warp pulls launch
+  // positions from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
+  __shared__ float4 sm[32 * 3];
+  __shared__ uint32_t q_rank[64], q_cpos[64];
+  __shared__ uint32_t p_rank[64], p_cpos[64];
+  const int lane = threadIdx.x;
+  for (uint32_t bpos = blockIdx.x;;) {
+    if (batch.work_fwd) {
+      if (lane == 0) bpos = atomicAdd(batch.work_fwd, 1u);
+      bpos = __shfl_sync(FULL, bpos, 0);
+    }
+    if (bpos >= batch.n_work) return;
+    __syncwarp();
+    FwdOut fo;
+    forward_tile<FULLPIX>(batch, prm, bpos, lane, sm, q_rank, q_cpos, p_rank, p_cpos, fo);
+    if (!batch.work_fwd) return;
+  }
 }
 
 
@@ -431,29 +454,30 @@ __device__ __forceinline__ void group_tail(const float4* rawA, const float2* raw
 // FROM_LIST: the tile's entries come from the list S3 wrote (RasterView::tlist), read backwards one chunk of 32 ranks ahead --
 // no rect test, no ellipse test, no gather before the staging; tiles whose list outgrew TL_CAP are left to the instantiation
 // without FROM_LIST, which filters the supertile list again as S3 did and exits at once when the batch has no such tile.
-template <int NCH, bool FROM_LIST>
-__global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
-  __shared__ float4 sm[32 * 3];
-  __shared__ float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
-  __shared__ float4 sm_ex[32];           // per staged entry: log2(sigma), P_min + P_max, P_min P_max, -
+// The shared memory of one S4 warp (12,032 bytes; raster_kernel runs S3 in the same bytes):
+struct BwdSmem {
+  float4 sm[32 * 3];
+  float4 sm_wh[32];           // per staged entry: (1/l11, l21/l11, 1/l22) of Sigma2D = L L^T, P_min
+  float4 sm_ex[32];           // per staged entry: log2(sigma), P_min + P_max, P_min P_max, -
   // folded column sums of up to GE entries awaiting their group tail: values 0..15 of lane l, entry slot g at
   // rawA[(g * 4 + m) * 32 + l] (m = 0..3), values 16, 17 at rawB[g * 32 + l]; the reduction buffer of the tail aliases rawA
-  __shared__ float4 rawA[GE * 4 * 32];
-  __shared__ float2 rawB[GE * 32];
-  __shared__ uint32_t q_rank[64];
+  float4 rawA[GE * 4 * 32];
+  float2 rawB[GE * 32];
+  uint32_t q_rank[64];
+};
+
+// S4 of one launch position (view, tile) by one warp.  FROM_REGS: the tile's `T`, `last` and list length come from the S3 sweep
+// the same warp has just finished (fo) instead of from memory.
+template <int NCH, bool FROM_LIST, bool FROM_REGS>
+__device__ __forceinline__ void backward_tile(const RasterBatch& batch, const RasterParams& prm, uint32_t bpos, int lane, BwdSmem& S,
+                                              const FwdOut* fo) {
+  float4* sm = S.sm;
+  float4* sm_wh = S.sm_wh;
+  float4* sm_ex = S.sm_ex;
+  float4* rawA = S.rawA;
+  float2* rawB = S.rawB;
+  uint32_t* q_rank = S.q_rank;
   float* red = reinterpret_cast<float*>(rawA);
-  const int lane = threadIdx.x;
-  // Persistent warps (batch.work != nullptr): the grid is one wave of resident warps and every warp pulls launch positions
-  // from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
-  uint32_t* const work = FROM_LIST ? batch.work : batch.work_fb;
-  if (!FROM_LIST && batch.overflow && *batch.overflow == 0u) return;      // no tile of the batch outgrew its list
-  for (uint32_t bpos = blockIdx.x;; ) {
-  if (work) {
-    if (lane == 0) bpos = atomicAdd(work, 1u);
-    bpos = __shfl_sync(FULL, bpos, 0);
-  }
-  if (bpos >= batch.n_work) return;
-  __syncwarp();
   const int vidx = (int)(bpos % (uint32_t)batch.n);      // views interleaved (see forward_kernel)
   const RasterView& vw = batch.v[vidx];
   const Splat* __restrict__ splat_sorted = vw.splat_sorted;
@@ -463,10 +487,10 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
   const PixelBuf pix = vw.pix;
   double* __restrict__ moments = vw.moments;
   const int tile = batch.tile_order[bpos / (uint32_t)batch.n];   // heaviest tiles first (launch order)
-  const uint32_t elast = vw.tile_elast[tile];             // list position + 1 of the last entry any pixel of the tile passed
+  const uint32_t elast = FROM_REGS ? fo->elast : vw.tile_elast[tile];      // list position + 1 of the last entry any pixel of the tile passed
   // which instantiation owns the tile: the list holds the first TL_CAP entries only
   const bool listed = vw.tlist != nullptr && elast <= (uint32_t)TL_CAP;
-  if (elast == 0u || listed != FROM_LIST) { if (work) continue; return; }
+  if (elast == 0u || listed != FROM_LIST) return;
   const int tx = tile % prm.tiles_x, ty = tile / prm.tiles_x;
   const int x = tx * TILE + (lane & 15), y0 = ty * TILE + (lane >> 4) * PPL;
   const float px = (float)x + 0.5f;
@@ -485,7 +509,10 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
       const int k = h ? PPL - 1 - q : q;
       int l = 0;
       float T = 1.0f;
-      if (x < prm.W && y0 + k < prm.H) {
+      if (FROM_REGS) {
+        l = fo->last[k];
+        T = h ? fo->T2[q].y : fo->T2[q].x;
+      } else if (x < prm.W && y0 + k < prm.H) {
         const size_t p = (size_t)(y0 + k) * prm.W + x;
         l = pix.last[p];
         T = pix.T[p];
@@ -695,8 +722,49 @@ __global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const 
     e_next -= cnt;
     if (!FROM_LIST) shift_queue(q_rank, nullptr, qn, (uint32_t)cnt);
   }
-  if (!work) return;
-  }  // persistent loop
+}
+
+template <int NCH, bool FROM_LIST>
+__global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) backward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
+  __shared__ BwdSmem S;
+  const int lane = threadIdx.x;
+  // Persistent warps (batch.work != nullptr): the grid is one wave of resident warps and every warp pulls launch positions
+  // from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
+  uint32_t* const work = FROM_LIST ? batch.work : batch.work_fb;
+  if (!FROM_LIST && batch.overflow && *batch.overflow == 0u) return;      // no tile of the batch outgrew its list
+  for (uint32_t bpos = blockIdx.x;;) {
+    if (work) {
+      if (lane == 0) bpos = atomicAdd(work, 1u);
+      bpos = __shfl_sync(FULL, bpos, 0);
+    }
+    if (bpos >= batch.n_work) return;
+    __syncwarp();
+    backward_tile<NCH, FROM_LIST, false>(batch, prm, bpos, lane, S, nullptr);
+    if (!work) return;
+  }
+}
+
+// OPT-IN (NBV_FUSED_RASTER=1; not the default: 1971 against 2036 views/s at config 2).
+// S3 and S4 of a tile back to back by the same warp: S4 of a tile needs nothing but S3 of that tile (its `T`, `last`, and the list
+// S3 wrote), so one persistent launch per batch serves both -- one drain per batch instead of two, and S4 starts from the
+// registers S3 ends with instead of re-reading 8 B per pixel.  S3 still writes `T` / `last` (the fallback launch for tiles whose
+// list outgrew TL_CAP and the parity exports read them).  Compiled for the register budget of S4 (16 warps per SM); the S3 part
+// runs in the first 2,560 bytes of the S4 part's shared memory.
+template <int NCH>
+__global__ void __launch_bounds__(32, NBV_BWD_MIN_BLOCKS) raster_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
+  __shared__ BwdSmem S;
+  const int lane = threadIdx.x;
+  uint32_t* fq = reinterpret_cast<uint32_t*>(S.rawA);        // S3's four queues of 64 words in the column-sum buffer of S4
+  for (uint32_t bpos = blockIdx.x;;) {
+    if (lane == 0) bpos = atomicAdd(batch.work_fwd, 1u);
+    bpos = __shfl_sync(FULL, bpos, 0);
+    if (bpos >= batch.n_work) return;
+    __syncwarp();
+    FwdOut fo;
+    forward_tile<false>(batch, prm, bpos, lane, S.sm, fq, fq + 64, fq + 128, fq + 192, fo);
+    __syncwarp();
+    backward_tile<NCH, true, true>(batch, prm, bpos, lane, S, &fo);
+  }
 }
 
 static RasterParams make_params(const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg) {
@@ -726,6 +794,23 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
     forward_kernel<true><<<grid, 32, 0, st>>>(b, p);
   else
     forward_kernel<false><<<grid, 32, 0, st>>>(b, p);
+}
+
+// S3 + S4 of a batch in one persistent launch (raster_kernel), then the fallback S4 launch for tiles whose list outgrew TL_CAP.
+// Needs the work counters (persistent mode) and the tile lists.
+void launch_raster_fused(const RasterBatch& batch, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg, cudaStream_t st) {
+  const RasterParams p = make_params(tg, rank_bits, W, H, cfg);
+  RasterBatch b = batch;
+  b.n_work = (uint32_t)(tg.tiles_x * tg.tiles_y * batch.n);
+  const dim3 grid(std::min(b.n_work, (unsigned)sm_count() * NBV_BWD_MIN_BLOCKS));
+  g_kernel_launches += 2;
+  if (cfg.channel_mask & NBV_CH_DEPTH) {
+    raster_kernel<4><<<grid, 32, 0, st>>>(b, p);
+    backward_kernel<4, false><<<grid, 32, 0, st>>>(b, p);
+  } else {
+    raster_kernel<3><<<grid, 32, 0, st>>>(b, p);
+    backward_kernel<3, false><<<grid, 32, 0, st>>>(b, p);
+  }
 }
 
 void launch_backward(const RasterBatch& batch, int N, const TileGrid& tg, int rank_bits, int W, int H, const nbv_config& cfg,

@@ -388,6 +388,30 @@ def test_tile_lists_longer_than_the_handover_capacity_take_the_fallback_path():
     assert int(best.item()) == ref["best"]
 
 
+def test_opt_in_fused_raster_launch_gives_the_same_numbers(wl, monkeypatch):
+    """NBV_FUSED_RASTER=1 runs S3 and S4 of a tile back to back in one persistent launch (raster_kernel: S4 starts from the
+    registers S3 ends with).  Not the default -- it measured slower -- but it is the same arithmetic in the same order per
+    (tile, Gaussian), so scores, per-Gaussian gains, blocks and H_T agree with the two-launch path to the last bits."""
+    ref = _nbv(wl.scene, channel_mask=15)
+    monkeypatch.setenv("NBV_FUSED_RASTER", "1")
+    fus = _nbv(wl.scene, channel_mask=15)
+    monkeypatch.delenv("NBV_FUSED_RASTER")
+    for n in (ref, fus):
+        n.accumulate_training(wl.train_cams)
+    np.testing.assert_array_equal(fus.training_hessian().cpu().numpy(), ref.training_hessian().cpu().numpy())
+    sr, br = ref.score_candidates(wl.cand_cams)
+    sf, bf = fus.score_candidates(wl.cand_cams)
+    np.testing.assert_allclose(sf.cpu().numpy(), sr.cpu().numpy(), rtol=1e-9)
+    assert int(bf.item()) == int(br.item())
+    cam = wl.cand_cams[1]
+    np.testing.assert_array_equal(fus.view_hessian(cam).cpu().numpy(), ref.view_hessian(cam).cpu().numpy())
+    np.testing.assert_allclose(fus.gaussian_gains(cam).cpu().numpy(), ref.gaussian_gains(cam).cpu().numpy(), rtol=1e-9, atol=0)
+    walked_f, last_f = fus.tile_walk(cam)
+    walked_r, last_r = ref.tile_walk(cam)
+    np.testing.assert_array_equal(walked_f.cpu().numpy(), walked_r.cpu().numpy())
+    np.testing.assert_array_equal(last_f.cpu().numpy(), last_r.cpu().numpy())
+
+
 def test_packed_exp_spec_is_the_specified_exp_spec_bit_for_bit():
     """The raster kernels take the last step of exp_spec (bits(p) + (k << 23)) as p * 2^k with 2^k from
     MUFU.EX2.  That is the same binary32 number only where ex2.approx is exact at integers and the product is normal: every
