@@ -126,6 +126,12 @@ struct FwdOut {
   uint32_t elast;
 };
 
+// the shared memory of one S3 warp (2,560 bytes), one struct so that every array is an offset from one base
+struct FwdSmem {
+  float4 sm[32 * 3];
+  uint32_t q_rank[64], q_cpos[64], p_rank[64], p_cpos[64];
+};
+
 // S3 of one launch position (view, tile) by one warp.  sm: 96 float4; q_rank, q_cpos, p_rank, p_cpos: 64 words each (p_*: rect
 // hits awaiting the ellipse test, stage 2 of the tile filter).
 template <bool FULLPIX>
@@ -327,9 +333,7 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
   // edge tiles of all views.
   // Persistent warps (batch.work_fwd != nullptr): the grid is one wave of resident warps and every warp pulls launch
   // positions from a counter until they run out, so a warp that drew a cheap tile immediately draws another one.
-  __shared__ float4 sm[32 * 3];
-  __shared__ uint32_t q_rank[64], q_cpos[64];
-  __shared__ uint32_t p_rank[64], p_cpos[64];
+  __shared__ FwdSmem F;
   const int lane = threadIdx.x;
   for (uint32_t bpos = blockIdx.x;;) {
     if (batch.work_fwd) {
@@ -339,7 +343,7 @@ __global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __
     if (bpos >= batch.n_work) return;
     __syncwarp();
     FwdOut fo;
-    forward_tile<FULLPIX>(batch, prm, bpos, lane, sm, q_rank, q_cpos, p_rank, p_cpos, fo);
+    forward_tile<FULLPIX>(batch, prm, bpos, lane, F.sm, F.q_rank, F.q_cpos, F.p_rank, F.p_cpos, fo);
     if (!batch.work_fwd) return;
   }
 }
