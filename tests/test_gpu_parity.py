@@ -388,6 +388,20 @@ def test_tile_lists_longer_than_the_handover_capacity_take_the_fallback_path():
     assert int(best.item()) == ref["best"]
 
 
+def test_views_per_batch_choice(wl):
+    """nbv_batch_views: 16 views per batch unless the 2 x 16 view slots (worst-case coarse lists, binary64 moment rows) would
+    take more than a sixth of the device memory; a fixed concurrency wins; bad sizes give 0."""
+    nbv = _nbv(wl.scene)
+    assert nbv.batch_views(64, 64) == 16 and nbv.batch_views(1280, 720) == 16       # 800 Gaussians: a few MB per slot
+    assert nbv.batch_views(0, 64) == 0 and nbv.batch_views(64, -1) == 0
+    nbv.set_concurrency(5)
+    assert nbv.batch_views(1280, 720) == 5
+    # a map whose slots cannot all fit: N x 60 supertiles x 12 B of coarse capacity alone is 7.2 GB per slot at 10M Gaussians
+    big = synth.make_workload(0, n_gaussians=10_000_000)
+    nb = _nbv(big.scene)
+    assert nb.batch_views(1280, 720) == 8 and nb.batch_views(64, 64) == 16
+
+
 def test_opt_in_fused_raster_launch_gives_the_same_numbers(wl, monkeypatch):
     """NBV_FUSED_RASTER=1 runs S3 and S4 of a tile back to back in one persistent launch (raster_kernel: S4 starts from the
     registers S3 ends with).  Not the default -- it measured slower -- but it is the same arithmetic in the same order per
