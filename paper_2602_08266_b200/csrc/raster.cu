@@ -327,7 +327,7 @@ __device__ __forceinline__ void forward_tile(const RasterBatch& batch, const Ras
 }
 
 template <bool FULLPIX>
-__global__ void __launch_bounds__(32, FULLPIX ? 16 : 32) forward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
+__global__ void __launch_bounds__(32, FULLPIX ? 16 : 20) forward_kernel(const __grid_constant__ RasterBatch batch, const __grid_constant__ RasterParams prm) {
   // One launch rasterises every view of the batch.  Launch position -> (view, tile): the views are
   // interleaved, so the launch starts with the central (long-running) tiles of ALL views and its tail is made of the
   // edge tiles of all views.
@@ -791,7 +791,7 @@ void launch_forward(const RasterBatch& batch, const TileGrid& tg, int rank_bits,
   RasterBatch b = batch;
   b.n_work = (uint32_t)(tg.tiles_x * tg.tiles_y * batch.n);
   unsigned blocks = b.n_work;
-  if (b.work_fwd) blocks = std::min(blocks, (unsigned)sm_count() * (full_pix ? 16u : 32u));
+  if (b.work_fwd) blocks = std::min(blocks, (unsigned)sm_count() * (full_pix ? 16u : 20u));
   const dim3 grid(blocks);
   ++g_kernel_launches;
   if (full_pix)
