@@ -48,7 +48,7 @@ FLOP_SOURCE = "profiles/r2_ncu_flops_cfg2.md"
 BYTES_PER_KEY = 8         # S2: a (supertile, depth rank) key must be written once and read once (4 + 4 B)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch (8 views) from the committed `ncu --set full` capture named
 # in TRAFFIC_SOURCE; known for config 2 only (null elsewhere)
-NCU_TRAFFIC_BYTES_PER_VIEW = {2: {"backward": 235.3e6 / 16, "forward": 168.2e6 / 16}}      # the capture is of a 16-view launch
+NCU_TRAFFIC_BYTES_PER_VIEW = {2: {"backward": 236.8e6 / 16, "forward": 158.2e6 / 16}}      # the capture is of a 16-view launch
 TRAFFIC_SOURCE = "profiles/r2_ncu_raster_cfg2.md (ncu --set full of the first candidate batch; a stored figure, not measured by this run)"
 
 
