@@ -244,7 +244,10 @@ int nbv_last_view_stats(nbv_ctx* ctx, nbv_view_stats* h_out, void* stream);
 #define NBV_N_STAGES 7
 
 /* enable != 0: bracket every stage launch (per view for S1-S2, per batch for S3-S6) with CUDA events on the stream it
- * runs on, from now on (a few microseconds per view); clears the accumulated times.  Synchronises `stream`. */
+ * runs on, from now on (a few microseconds per view); clears the accumulated times.  Synchronises `stream`. 
+ * Environment: NBV_TRACE_SPANS=<file> makes nbv_stage_times() also append every span it folds to <file>, one line
+ * `stage views start_ms end_ms` per span (times relative to the first span since the last fold), blocks ended by `-1 0 0 0`:
+ * the timeline of a call across the library's internal streams (profiles/r2_timeline_cfg2.md). */
 int nbv_set_stage_timing(nbv_ctx* ctx, int32_t enable, void* stream);
 
 /* h_ms[NBV_N_STAGES] <- milliseconds spent per stage, summed over the *h_views views processed since timing was

@@ -189,6 +189,19 @@ constexpr size_t MAX_SPANS = 1 << 20;       // beyond this, further spans are si
 
 // fold the recorded spans into ctx->stage_ms (every stream that recorded one must be idle)
 void fold_timing(nbv_ctx* ctx) {
+  if (const char* path = std::getenv("NBV_TRACE_SPANS")) {     // span timeline of the call(s) since the last fold: stage views start end (ms)
+    if (FILE* f = ctx->spans_used ? std::fopen(path, "a") : nullptr) {
+      for (size_t i = 0; i < ctx->spans_used; ++i) {
+        float t0 = 0.f, t1 = 0.f;
+        if (cudaEventElapsedTime(&t0, ctx->spans[0].a, ctx->spans[i].a) == cudaSuccess &&
+            cudaEventElapsedTime(&t1, ctx->spans[0].a, ctx->spans[i].b) == cudaSuccess)
+          std::fprintf(f, "%d %d %.4f %.4f\n", ctx->spans[i].stage, ctx->spans[i].views, t0, t1);
+      }
+      std::fprintf(f, "-1 0 0 0\n");
+      std::fclose(f);
+    }
+    cudaGetLastError();
+  }
   for (size_t i = 0; i < ctx->spans_used; ++i) {
     const Span& sp = ctx->spans[i];
     float ms = 0.f;
