@@ -134,7 +134,7 @@ const char* nbv_last_error(const nbv_ctx* ctx);
  * (view, tile) positions).  Two sets of work buffers and two internal raster streams alternate between batches.  Views are independent
  * (the arg max is over per-view gains), so this changes no result beyond the order of S4's cross-tile binary64 reductions (exact for realistic footprints)
  * (H_T is accumulated view by view in call order, and a candidate's score is summed in a fixed order).
- * Errors: INVALID_ARG outside [1, 16]. */
+ * views_in_flight = 0 restores the automatic choice.  Errors: INVALID_ARG outside [0, 16]. */
 int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight);
 int32_t nbv_batch_views(const nbv_ctx* ctx, int32_t width, int32_t height);
 

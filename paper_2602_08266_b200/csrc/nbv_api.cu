@@ -783,7 +783,7 @@ void nbv_destroy(nbv_ctx* ctx) {
 
 int nbv_set_concurrency(nbv_ctx* ctx, int32_t views_in_flight) {
   if (!ctx) return NBV_ERR_INVALID_ARG;
-  if (views_in_flight < 1 || views_in_flight > MAX_BATCH) return fail(ctx, NBV_ERR_INVALID_ARG, "views_in_flight must be in [1, 16]");
+  if (views_in_flight < 0 || views_in_flight > MAX_BATCH) return fail(ctx, NBV_ERR_INVALID_ARG, "views_in_flight must be in [1, 16], or 0 for the automatic choice");
   ctx->concurrency = views_in_flight;
   return NBV_OK;
 }

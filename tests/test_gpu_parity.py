@@ -396,6 +396,10 @@ def test_views_per_batch_choice(wl):
     assert nbv.batch_views(0, 64) == 0 and nbv.batch_views(64, -1) == 0
     nbv.set_concurrency(5)
     assert nbv.batch_views(1280, 720) == 5
+    nbv.set_concurrency(0)                                                           # back to the automatic choice
+    assert nbv.batch_views(1280, 720) == 16
+    with pytest.raises(Exception):
+        nbv.set_concurrency(17)
     # a map whose slots cannot all fit: N x 60 supertiles x 12 B of coarse capacity alone is 7.2 GB per slot at 10M Gaussians
     big = synth.make_workload(0, n_gaussians=10_000_000)
     nb = _nbv(big.scene)
