@@ -193,6 +193,9 @@ int nbv_score_candidates_host(nbv_ctx* ctx, const nbv_camera* h_cams, int32_t n,
  * NBV_CH_MASK (every output has its own Jacobian, hence its own Hessian), each with the n_train cameras of
  * h_train already accumulated.  ctx_mask may be NULL: the mask term is then left out (F = 2 outputs instead of 3).
  * h_train: HOST array of those training cameras (needed again for the denominators).
+ * When ctx_rgb and ctx_depth composite with the same constants (near plane, blur, alpha_min, alpha_max, t_stop) every view goes
+ * through S1-S3 once, in ctx_rgb's buffers, and is swept twice by S4-S6 (once per output): the maps of the two contexts must then
+ * really hold the same values, which the call cannot check beyond N and K.
  * DEVICE outputs: d_fused n floats; d_raw F*n floats (rgb row, depth row[, mask row]; may be NULL); d_denom F floats
  * (may be NULL); d_best one int32.  A zero denominator (no training view sees anything) yields non-finite
  * fused scores, not an error.  Errors: NOT_LOADED, EMPTY_CANDIDATES (n == 0), UNKNOWN_TARGET, INVALID_ARG (null
